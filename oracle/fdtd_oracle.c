@@ -1,0 +1,777 @@
+/*
+ * fdtd_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * Plain, slow, obviously-correct CPU statement of the hot path of
+ * arXiv 2412.12360 ("FDTDX"): Yee-grid FDTD time stepping with CPML, additive
+ * sources, DFT detectors, PML-interface recording, and the time-reversed
+ * gradient (inverse update + vector-Jacobian product).
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference leg may build, load or call this file.  It shares no code,
+ * header, table generator or constant with paper_2412_12360_b200/csrc.
+ *
+ * What the paper fixes:
+ *   Eq. 1-2 (L64-66)  dH/dt = -(1/mu) curl E ;  dE/dt = (1/eps) curl H
+ *   L68               Yee staggering, "curl updates ... used in every time step"
+ *   L72               convolutional PML (Roden-Gedney, ref. 7); sources
+ *   L68/L70           detectors, interpolation disabled by default
+ *   L80               "chain of function calls, each call updates either the
+ *                      electric or magnetic field"
+ *   L84               time reversibility; PML not invertible; "field values at
+ *                      the boundary between the PML and the inner simulation
+ *                      volume ... saved for every time step"
+ * Everything below that level (index convention, normalisation, CPML grading,
+ * DFT phase stamp, what the recorder stores) is silent in the paper; the
+ * readings R1..R22 are listed in DESIGN.md section 3 and followed literally here.
+ *
+ * Conventions:
+ *   grid nx*ny*nz, x fastest: lin = (k*ny + j)*nx + i
+ *   fields = [6][nz][ny][nx], components Ex,Ey,Ez,Hx,Hy,Hz
+ *   cyclic triple for component c: a = c+1, b = c+2 (mod 3);
+ *      (curl F)_c = d_a F_b - d_b F_a
+ *   dm_a F[p] = F[p] - F[p - e_a]   (in the E update, acting on H)
+ *   dp_a F[p] = F[p + e_a] - F[p]   (in the H update, acting on E)
+ *   out-of-range operand: wrapped if periodic, 0 otherwise
+ *   one step n: E update (from old H), E sources, H update (from new E),
+ *               H sources, detectors with phase omega*(n+1)
+ *   S = c dt/dx (Courant number); H is scaled by eta0.
+ *
+ * Compiled twice: -DREAL=double (parity reference) and -DREAL=float (timed
+ * CPU baseline).  No tiling, no fusion, no reordering; OpenMP (optional, only
+ * with -fopenmp) splits the outermost k loop of loops whose iterations are
+ * independent.
+ *
+ * Parity pins (tests/test_oracle_pins.py): exact discrete plane-wave
+ * eigenmode / dispersion relation, exact discrete energy invariant, discrete
+ * Gauss law, forward-N/inverse-N recovery, tape == reversible gradient,
+ * gradient vs central finite differences, adjoint dot-product identity,
+ * CPML vs big-box, late-time decay, linearity/null tests, the paper's
+ * Table 2 step counts (Courant convention).
+ * Parity unpinned: agreement with the paper's own FDTDX outputs (no numbers,
+ * code, geometry or data are available) and the specific CPML constants /
+ * DFT normalisation FDTDX uses.
+ */
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#include <stddef.h>
+#if defined(__x86_64__) || defined(__i386__)
+#include <xmmintrin.h>
+#endif
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#ifndef REAL
+#define REAL double
+#endif
+
+typedef struct {
+    int nx, ny, nz;
+    int periodic;          /* 1: periodic box (d must be 0); 0: zero outside   */
+    int d;                 /* CPML thickness in cells                          */
+    double S;              /* Courant number c dt/dx                           */
+    double m;              /* grading order of sigma and kappa                 */
+    double sigma_max;      /* sigma~_max = sigma eta0 dx at full depth         */
+    double kappa_max;
+    double alpha_max;      /* alpha~ at the PML/interior interface             */
+    double alpha_m;        /* grading order of alpha                           */
+} orc_desc;
+
+typedef struct {           /* additive patch F_c[box] += profile*waveform[n]  */
+    int comp;              /* 0..5                                             */
+    int lo[3], hi[3];      /* half-open box (i,j,k)                            */
+    const REAL *profile;   /* box-shaped [k][j][i], or NULL => 1               */
+    const REAL *waveform;  /* length >= n_steps                                */
+} orc_source;
+
+typedef struct {           /* running DFT on a box                             */
+    int mask;              /* bit c set => component c accumulated             */
+    int lo[3], hi[3];
+    int n_freq;
+    const double *omega;   /* rad per step                                     */
+    REAL *phasor;          /* [n_freq][n_comp_set][box cells][2] (re,im)       */
+} orc_detector;
+
+typedef struct {
+    orc_desc D;
+    size_t nc;                               /* cells                          */
+    REAL *bE[3], *aE[3], *ikE[3];            /* CPML tables, E positions x = p    */
+    REAL *bH[3], *aH[3], *ikH[3];            /* CPML tables, H positions x = p+1/2 */
+    REAL *psiE[3][2], *psiH[3][2];           /* primal psi, full volumes       */
+    REAL *lpsiE[3][2], *lpsiH[3][2];         /* cotangents of psi              */
+    REAL *tmp[3][2];                         /* scratch volumes for the adjoint */
+} orc_state;
+
+#define NX (D->nx)
+#define NY (D->ny)
+#define NZ (D->nz)
+#define IDX(i, j, k) (((size_t)(k) * NY + (j)) * NX + (i))
+
+/* ------------------------------------------------------------------------ */
+/* helpers                                                                  */
+/* ------------------------------------------------------------------------ */
+
+/* value of volume F at (i,j,k); out of range: wrapped if periodic, else 0 (R7) */
+static inline REAL at(const orc_desc *D, const REAL *F, int i, int j, int k)
+{
+    if (D->periodic) {
+        i = (i % NX + NX) % NX;
+        j = (j % NY + NY) % NY;
+        k = (k % NZ + NZ) % NZ;
+    } else if (i < 0 || i >= NX || j < 0 || j >= NY || k < 0 || k >= NZ) {
+        return (REAL)0;
+    }
+    return F[IDX(i, j, k)];
+}
+
+static inline int dimlen(const orc_desc *D, int axis)
+{
+    return axis == 0 ? NX : (axis == 1 ? NY : NZ);
+}
+
+/* interior box I = [d, N_a - d) on every axis (whole grid if d == 0) */
+static inline int lo_I(const orc_desc *D, int axis) { (void)axis; return D->d; }
+static inline int hi_I(const orc_desc *D, int axis) { return dimlen(D, axis) - D->d; }
+
+void orc_set_ftz(int on)
+{
+#if defined(__x86_64__) || defined(__i386__)
+#ifdef _OPENMP
+#pragma omp parallel
+#endif
+    {
+        unsigned csr = _mm_getcsr();
+        if (on) csr |= 0x8040u; else csr &= ~0x8040u;   /* FTZ | DAZ */
+        _mm_setcsr(csr);
+    }
+#else
+    (void)on;
+#endif
+}
+
+int orc_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+int orc_sizeof_real(void) { return (int)sizeof(REAL); }
+
+/* ------------------------------------------------------------------------ */
+/* CPML tables (PAPER.md L72 -> ref. 7; constants: DESIGN.md R8)            */
+/*   depth rho(x) = max(0, d - x, x - (N - d)),  r = rho/d                  */
+/*   sigma = sigma_max r^m ; kappa = 1 + (kappa_max-1) r^m ;                */
+/*   alpha = alpha_max (1-r)^alpha_m  (inside the PML, 0 outside)           */
+/*   b = exp(-(sigma/kappa + alpha) S)                                      */
+/*   a = sigma / (kappa (sigma + kappa alpha)) (b - 1)   (0 where sigma=0)  */
+/*   ik = 1/kappa                                                           */
+/* half = 0: E tables at x = p ; half = 1: H tables at x = p + 1/2          */
+/* ------------------------------------------------------------------------ */
+void orc_cpml_table(const orc_desc *D, int axis, int half,
+                    double *b, double *a, double *ik)
+{
+    int n = dimlen(D, axis);
+    for (int p = 0; p < n; ++p) {
+        double x = (double)p + (half ? 0.5 : 0.0);
+        double rho = 0.0;
+        if (D->d > 0) {
+            double r1 = (double)D->d - x;
+            double r2 = x - (double)(n - D->d);
+            if (r1 > rho) rho = r1;
+            if (r2 > rho) rho = r2;
+        }
+        if (rho <= 0.0) { b[p] = 1.0; a[p] = 0.0; ik[p] = 1.0; continue; }
+        double r = rho / (double)D->d;
+        double sig = D->sigma_max * pow(r, D->m);
+        double kap = 1.0 + (D->kappa_max - 1.0) * pow(r, D->m);
+        double alp = D->alpha_max * pow(1.0 - r, D->alpha_m);
+        double bb = exp(-(sig / kap + alp) * D->S);
+        double aa = 0.0;
+        if (sig > 0.0) aa = sig / (kap * (sig + kap * alp)) * (bb - 1.0);
+        b[p] = bb; a[p] = aa; ik[p] = 1.0 / kap;
+    }
+}
+
+/* ------------------------------------------------------------------------ */
+/* state                                                                    */
+/* ------------------------------------------------------------------------ */
+static REAL *zalloc(size_t n) { return (REAL *)calloc(n ? n : 1, sizeof(REAL)); }
+
+void orc_destroy(orc_state *st)
+{
+    if (!st) return;
+    for (int a = 0; a < 3; ++a) {
+        free(st->bE[a]); free(st->aE[a]); free(st->ikE[a]);
+        free(st->bH[a]); free(st->aH[a]); free(st->ikH[a]);
+        for (int s = 0; s < 2; ++s) {
+            free(st->psiE[a][s]); free(st->psiH[a][s]);
+            free(st->lpsiE[a][s]); free(st->lpsiH[a][s]);
+            free(st->tmp[a][s]);
+        }
+    }
+    free(st);
+}
+
+orc_state *orc_create(const orc_desc *desc)
+{
+    if (desc->nx < 1 || desc->ny < 1 || desc->nz < 1) return NULL;
+    if (desc->periodic && desc->d != 0) return NULL;
+    if (desc->d < 0) return NULL;
+    orc_state *st = (orc_state *)calloc(1, sizeof(orc_state));
+    if (!st) return NULL;
+    st->D = *desc;
+    const orc_desc *D = &st->D;
+    st->nc = (size_t)NX * NY * NZ;
+    for (int a = 0; a < 3; ++a) {
+        int n = dimlen(D, a);
+        double *b = (double *)malloc(sizeof(double) * n);
+        double *aa = (double *)malloc(sizeof(double) * n);
+        double *ik = (double *)malloc(sizeof(double) * n);
+        for (int half = 0; half < 2; ++half) {
+            orc_cpml_table(D, a, half, b, aa, ik);
+            REAL *tb = zalloc(n), *ta = zalloc(n), *tk = zalloc(n);
+            for (int p = 0; p < n; ++p) { tb[p] = (REAL)b[p]; ta[p] = (REAL)aa[p]; tk[p] = (REAL)ik[p]; }
+            if (half == 0) { st->bE[a] = tb; st->aE[a] = ta; st->ikE[a] = tk; }
+            else           { st->bH[a] = tb; st->aH[a] = ta; st->ikH[a] = tk; }
+        }
+        free(b); free(aa); free(ik);
+        for (int s = 0; s < 2; ++s) {
+            st->psiE[a][s] = zalloc(st->nc);  st->psiH[a][s] = zalloc(st->nc);
+            st->lpsiE[a][s] = zalloc(st->nc); st->lpsiH[a][s] = zalloc(st->nc);
+            st->tmp[a][s] = zalloc(st->nc);
+        }
+    }
+    return st;
+}
+
+/* accessors so tests can read / set psi and its cotangent */
+REAL *orc_psi(orc_state *st, int is_H, int c, int s)  { return is_H ? st->psiH[c][s] : st->psiE[c][s]; }
+REAL *orc_lpsi(orc_state *st, int is_H, int c, int s) { return is_H ? st->lpsiH[c][s] : st->lpsiE[c][s]; }
+
+void orc_zero_psi(orc_state *st)
+{
+    for (int c = 0; c < 3; ++c) for (int s = 0; s < 2; ++s) {
+        memset(st->psiE[c][s], 0, st->nc * sizeof(REAL));
+        memset(st->psiH[c][s], 0, st->nc * sizeof(REAL));
+    }
+}
+void orc_zero_lpsi(orc_state *st)
+{
+    for (int c = 0; c < 3; ++c) for (int s = 0; s < 2; ++s) {
+        memset(st->lpsiE[c][s], 0, st->nc * sizeof(REAL));
+        memset(st->lpsiH[c][s], 0, st->nc * sizeof(REAL));
+    }
+}
+
+/* ------------------------------------------------------------------------ */
+/* O1: E update (Eq. 2 discretised on the Yee grid; CPML psi_E recursion)   */
+/*   d1 = dm_a H_b, d2 = dm_b H_a                                           */
+/*   psiE_c0 = bE_a psiE_c0 + aE_a d1 ; psiE_c1 = bE_b psiE_c1 + aE_b d2    */
+/*   E_c += S ie (ikE_a d1 - ikE_b d2 + psiE_c0 - psiE_c1)                  */
+/* bracket (optional, [3][cells]) receives the bracketed term: dE_c/d(ie)=S*bracket */
+/* ------------------------------------------------------------------------ */
+void orc_step_E(orc_state *st, REAL *fields, const REAL *ie, REAL *bracket)
+{
+    const orc_desc *D = &st->D;
+    const REAL S = (REAL)D->S;
+    const size_t nc = st->nc;
+    REAL *E[3] = { fields, fields + nc, fields + 2 * nc };
+    const REAL *H[3] = { fields + 3 * nc, fields + 4 * nc, fields + 5 * nc };
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (int k = 0; k < NZ; ++k)
+        for (int j = 0; j < NY; ++j)
+            for (int i = 0; i < NX; ++i) {
+                const size_t p = IDX(i, j, k);
+                const int pos[3] = { i, j, k };
+                for (int c = 0; c < 3; ++c) {
+                    const int a = (c + 1) % 3, b = (c + 2) % 3;
+                    int ea[3] = { 0, 0, 0 }, eb[3] = { 0, 0, 0 };
+                    ea[a] = 1; eb[b] = 1;
+                    REAL d1 = H[b][p] - at(D, H[b], i - ea[0], j - ea[1], k - ea[2]);
+                    REAL d2 = H[a][p] - at(D, H[a], i - eb[0], j - eb[1], k - eb[2]);
+                    REAL p0 = st->bE[a][pos[a]] * st->psiE[c][0][p] + st->aE[a][pos[a]] * d1;
+                    REAL p1 = st->bE[b][pos[b]] * st->psiE[c][1][p] + st->aE[b][pos[b]] * d2;
+                    st->psiE[c][0][p] = p0;
+                    st->psiE[c][1][p] = p1;
+                    REAL br = st->ikE[a][pos[a]] * d1 - st->ikE[b][pos[b]] * d2 + p0 - p1;
+                    if (bracket) bracket[(size_t)c * nc + p] = br;
+                    E[c][p] += S * ie[p] * br;
+                }
+            }
+}
+
+/* ------------------------------------------------------------------------ */
+/* O3: H update (Eq. 1 discretised; note the minus sign)                    */
+/*   d1 = dp_a E_b, d2 = dp_b E_a  on the just-updated E                    */
+/*   H_c -= S im (ikH_a d1 - ikH_b d2 + psiH_c0 - psiH_c1)                  */
+/* im == NULL means inv_mu = 1                                              */
+/* ------------------------------------------------------------------------ */
+void orc_step_H(orc_state *st, REAL *fields, const REAL *im)
+{
+    const orc_desc *D = &st->D;
+    const REAL S = (REAL)D->S;
+    const size_t nc = st->nc;
+    const REAL *E[3] = { fields, fields + nc, fields + 2 * nc };
+    REAL *H[3] = { fields + 3 * nc, fields + 4 * nc, fields + 5 * nc };
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (int k = 0; k < NZ; ++k)
+        for (int j = 0; j < NY; ++j)
+            for (int i = 0; i < NX; ++i) {
+                const size_t p = IDX(i, j, k);
+                const int pos[3] = { i, j, k };
+                for (int c = 0; c < 3; ++c) {
+                    const int a = (c + 1) % 3, b = (c + 2) % 3;
+                    int ea[3] = { 0, 0, 0 }, eb[3] = { 0, 0, 0 };
+                    ea[a] = 1; eb[b] = 1;
+                    REAL d1 = at(D, E[b], i + ea[0], j + ea[1], k + ea[2]) - E[b][p];
+                    REAL d2 = at(D, E[a], i + eb[0], j + eb[1], k + eb[2]) - E[a][p];
+                    REAL p0 = st->bH[a][pos[a]] * st->psiH[c][0][p] + st->aH[a][pos[a]] * d1;
+                    REAL p1 = st->bH[b][pos[b]] * st->psiH[c][1][p] + st->aH[b][pos[b]] * d2;
+                    st->psiH[c][0][p] = p0;
+                    st->psiH[c][1][p] = p1;
+                    REAL br = st->ikH[a][pos[a]] * d1 - st->ikH[b][pos[b]] * d2 + p0 - p1;
+                    H[c][p] -= S * (im ? im[p] : (REAL)1) * br;
+                }
+            }
+}
+
+/* ------------------------------------------------------------------------ */
+/* O2 / O4: additive sources of one field family (E: comp 0..2, H: 3..5)    */
+/* sign = +1 in the forward step, -1 in the inverse step                    */
+/* ------------------------------------------------------------------------ */
+static void add_sources(const orc_desc *D, REAL *fields, size_t nc,
+                        const orc_source *src, int n_src, int n, int family_H, REAL sign)
+{
+    for (int s = 0; s < n_src; ++s) {
+        const orc_source *q = &src[s];
+        if ((q->comp >= 3) != (family_H != 0)) continue;
+        REAL *F = fields + (size_t)q->comp * nc;
+        const REAL w = q->waveform[n];
+        const int bx = q->hi[0] - q->lo[0], by = q->hi[1] - q->lo[1];
+        for (int k = q->lo[2]; k < q->hi[2]; ++k)
+            for (int j = q->lo[1]; j < q->hi[1]; ++j)
+                for (int i = q->lo[0]; i < q->hi[0]; ++i) {
+                    size_t c = ((size_t)(k - q->lo[2]) * by + (j - q->lo[1])) * bx + (i - q->lo[0]);
+                    REAL prof = q->profile ? q->profile[c] : (REAL)1;
+                    F[IDX(i, j, k)] += sign * prof * w;
+                }
+    }
+}
+
+static int popcount6(int m) { int n = 0; for (int c = 0; c < 6; ++c) n += (m >> c) & 1; return n; }
+
+/* O5: detectors  P_f[c][cell] += F_c[cell] (cos phi - i sin phi), phi = omega_f (n+1)  (R13) */
+static void detect(const orc_desc *D, const REAL *fields, size_t nc,
+                   const orc_detector *det, int n_det, int n)
+{
+    for (int s = 0; s < n_det; ++s) {
+        const orc_detector *q = &det[s];
+        const int bx = q->hi[0] - q->lo[0], by = q->hi[1] - q->lo[1], bz = q->hi[2] - q->lo[2];
+        const size_t bc = (size_t)bx * by * bz;
+        const int ncomp = popcount6(q->mask);
+        for (int f = 0; f < q->n_freq; ++f) {
+            const double phi = q->omega[f] * (double)(n + 1);
+            const REAL cs = (REAL)cos(phi), sn = (REAL)sin(phi);
+            int ci = 0;
+            for (int c = 0; c < 6; ++c) {
+                if (!((q->mask >> c) & 1)) continue;
+                const REAL *F = fields + (size_t)c * nc;
+                REAL *P = q->phasor + ((size_t)f * ncomp + ci) * bc * 2;
+                for (int k = q->lo[2]; k < q->hi[2]; ++k)
+                    for (int j = q->lo[1]; j < q->hi[1]; ++j)
+                        for (int i = q->lo[0]; i < q->hi[0]; ++i) {
+                            size_t cell = ((size_t)(k - q->lo[2]) * by + (j - q->lo[1])) * bx + (i - q->lo[0]);
+                            REAL v = F[IDX(i, j, k)];
+                            P[2 * cell]     += v * cs;
+                            P[2 * cell + 1] -= v * sn;
+                        }
+                ++ci;
+            }
+        }
+    }
+}
+
+/* B1: transpose of detect():  lam F_c[cell] += Gr cos phi - Gi sin phi */
+static void detect_adjoint(const orc_desc *D, REAL *lam, size_t nc,
+                           const orc_detector *det, int n_det,
+                           const REAL *const *dL_dphasor, int n)
+{
+    if (!dL_dphasor) return;
+    for (int s = 0; s < n_det; ++s) {
+        const orc_detector *q = &det[s];
+        const REAL *G = dL_dphasor[s];
+        if (!G) continue;
+        const int bx = q->hi[0] - q->lo[0], by = q->hi[1] - q->lo[1], bz = q->hi[2] - q->lo[2];
+        const size_t bc = (size_t)bx * by * bz;
+        const int ncomp = popcount6(q->mask);
+        for (int f = 0; f < q->n_freq; ++f) {
+            const double phi = q->omega[f] * (double)(n + 1);
+            const REAL cs = (REAL)cos(phi), sn = (REAL)sin(phi);
+            int ci = 0;
+            for (int c = 0; c < 6; ++c) {
+                if (!((q->mask >> c) & 1)) continue;
+                REAL *L = lam + (size_t)c * nc;
+                const REAL *Gp = G + ((size_t)f * ncomp + ci) * bc * 2;
+                for (int k = q->lo[2]; k < q->hi[2]; ++k)
+                    for (int j = q->lo[1]; j < q->hi[1]; ++j)
+                        for (int i = q->lo[0]; i < q->hi[0]; ++i) {
+                            size_t cell = ((size_t)(k - q->lo[2]) * by + (j - q->lo[1])) * bx + (i - q->lo[0]);
+                            L[IDX(i, j, k)] += Gp[2 * cell] * cs - Gp[2 * cell + 1] * sn;
+                        }
+                ++ci;
+            }
+        }
+    }
+}
+
+/* ------------------------------------------------------------------------ */
+/* Recorder (reading R15): per step, for each axis a,          */
+/*   low face : H_b, H_c (b=a+1, c=a+2) at index d-1 on axis a, BEFORE step n */
+/*   high face: E'_b, E'_c at index N_a-d on axis a, after O1/O2 of step n   */
+/* the two other indices run over I.  Layout of one step's record:          */
+/*   for a in 0..2: [low: comp b cells, comp c cells][high: comp b, comp c] */
+/* with face cells ordered (slower other axis, faster other axis).          */
+/* ------------------------------------------------------------------------ */
+static size_t face_cells(const orc_desc *D, int a)
+{
+    int u = (a + 1) % 3, v = (a + 2) % 3;
+    if (D->d == 0) return 0;
+    return (size_t)(hi_I(D, u) - lo_I(D, u)) * (size_t)(hi_I(D, v) - lo_I(D, v));
+}
+
+size_t orc_record_stride(const orc_desc *D)
+{
+    size_t n = 0;
+    for (int a = 0; a < 3; ++a) n += 4 * face_cells(D, a);
+    return n;
+}
+
+/* offset (in REALs) inside one step's record of (axis a, side 0=low/1=high, which 0/1) */
+static size_t rec_offset(const orc_desc *D, int a, int side, int which)
+{
+    size_t off = 0;
+    for (int q = 0; q < a; ++q) off += 4 * face_cells(D, q);
+    return off + (size_t)(2 * side + which) * face_cells(D, a);
+}
+
+/* index of a face cell; pos[] is the full (i,j,k); axis a is ignored.
+   face cells are ordered with the higher-numbered of the two other axes slowest */
+static size_t face_index(const orc_desc *D, int a, const int pos[3])
+{
+    int u = (a + 1) % 3, v = (a + 2) % 3;
+    if (u > v) { int t = u; u = v; v = t; }          /* u < v : v slowest */
+    return (size_t)(pos[v] - lo_I(D, v)) * (size_t)(hi_I(D, u) - lo_I(D, u)) + (size_t)(pos[u] - lo_I(D, u));
+}
+
+static void record_faces(const orc_desc *D, const REAL *fields, size_t nc, REAL *rec, int side)
+{
+    if (D->d == 0) return;
+    for (int a = 0; a < 3; ++a) {
+        const int fixed = side ? hi_I(D, a) : lo_I(D, a) - 1;
+        for (int which = 0; which < 2; ++which) {
+            const int comp = (a + 1 + which) % 3;                 /* tangential component */
+            const REAL *F = fields + (size_t)(side ? comp : 3 + comp) * nc;   /* E' high, H low */
+            REAL *out = rec + rec_offset(D, a, side, which);
+            int pos[3];
+            for (pos[2] = (a == 2 ? fixed : lo_I(D, 2)); pos[2] < (a == 2 ? fixed + 1 : hi_I(D, 2)); ++pos[2])
+                for (pos[1] = (a == 1 ? fixed : lo_I(D, 1)); pos[1] < (a == 1 ? fixed + 1 : hi_I(D, 1)); ++pos[1])
+                    for (pos[0] = (a == 0 ? fixed : lo_I(D, 0)); pos[0] < (a == 0 ? fixed + 1 : hi_I(D, 0)); ++pos[0])
+                        out[face_index(D, a, pos)] = F[IDX(pos[0], pos[1], pos[2])];
+        }
+    }
+}
+
+/* ------------------------------------------------------------------------ */
+/* forward driver: n_steps of  [O0r] O1 O2 [O2r] O3 O4 O5                   */
+/* rec   : NULL or n_steps * orc_record_stride() REALs                      */
+/* tape  : NULL or n_steps * 3 * cells REALs (bracket of every E update)    */
+/* psi is NOT reset here (callers use orc_zero_psi; R21)                    */
+/* ------------------------------------------------------------------------ */
+int orc_forward(orc_state *st, REAL *fields, const REAL *ie, const REAL *im,
+                const orc_source *src, int n_src, const orc_detector *det, int n_det,
+                int n_steps, REAL *rec, REAL *tape)
+{
+    const orc_desc *D = &st->D;
+    const size_t nc = st->nc;
+    const size_t rs = orc_record_stride(D);
+    for (int n = 0; n < n_steps; ++n) {
+        if (rec) record_faces(D, fields, nc, rec + (size_t)n * rs, 0);           /* O0r */
+        orc_step_E(st, fields, ie, tape ? tape + (size_t)n * 3 * nc : NULL);     /* O1  */
+        add_sources(D, fields, nc, src, n_src, n, 0, (REAL)1);                   /* O2  */
+        if (rec) record_faces(D, fields, nc, rec + (size_t)n * rs, 1);           /* O2r */
+        orc_step_H(st, fields, im);                                              /* O3  */
+        add_sources(D, fields, nc, src, n_src, n, 1, (REAL)1);                   /* O4  */
+        detect(D, fields, nc, det, n_det, n);                                    /* O5  */
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------ */
+/* B2: adjoint of O3 (H update incl. psi_H recursion), whole grid.          */
+/* Reverse-mode of                                                          */
+/*   p0' = bH_a p0 + aH_a d1 ; p1' = bH_b p1 + aH_b d2                       */
+/*   H_c' = H_c - S im (ikH_a d1 - ikH_b d2 + p0' - p1')                     */
+/*   d1 = dp_a E_b ; d2 = dp_b E_a                                          */
+/* with w = -S im lamH_c:  lp0 += w ; lp1 -= w ;                            */
+/*   g1 = ikH_a w + aH_a lp0 ; g2 = -ikH_b w + aH_b lp1 ;                   */
+/*   lp0 <- bH_a lp0 ; lp1 <- bH_b lp1 ;                                    */
+/*   lamE_b += (dp_a)^T g1 = -dm_a g1 ; lamE_a += (dp_b)^T g2 = -dm_b g2    */
+/* lamH passes through unchanged.  Two passes (compute g, then difference)  */
+/* so that no loop iteration writes another iteration's cells.              */
+/* ------------------------------------------------------------------------ */
+void orc_adj_H(orc_state *st, REAL *lam, const REAL *im)
+{
+    const orc_desc *D = &st->D;
+    const REAL S = (REAL)D->S;
+    const size_t nc = st->nc;
+    REAL *lE[3] = { lam, lam + nc, lam + 2 * nc };
+    const REAL *lH[3] = { lam + 3 * nc, lam + 4 * nc, lam + 5 * nc };
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (int k = 0; k < NZ; ++k)
+        for (int j = 0; j < NY; ++j)
+            for (int i = 0; i < NX; ++i) {
+                const size_t p = IDX(i, j, k);
+                const int pos[3] = { i, j, k };
+                for (int c = 0; c < 3; ++c) {
+                    const int a = (c + 1) % 3, b = (c + 2) % 3;
+                    REAL w = -S * (im ? im[p] : (REAL)1) * lH[c][p];
+                    REAL l0 = st->lpsiH[c][0][p] + w;
+                    REAL l1 = st->lpsiH[c][1][p] - w;
+                    st->tmp[c][0][p] = st->ikH[a][pos[a]] * w + st->aH[a][pos[a]] * l0;    /* g1 */
+                    st->tmp[c][1][p] = -st->ikH[b][pos[b]] * w + st->aH[b][pos[b]] * l1;   /* g2 */
+                    st->lpsiH[c][0][p] = st->bH[a][pos[a]] * l0;
+                    st->lpsiH[c][1][p] = st->bH[b][pos[b]] * l1;
+                }
+            }
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (int k = 0; k < NZ; ++k)
+        for (int j = 0; j < NY; ++j)
+            for (int i = 0; i < NX; ++i) {
+                const size_t p = IDX(i, j, k);
+                for (int c = 0; c < 3; ++c) {
+                    const int a = (c + 1) % 3, b = (c + 2) % 3;
+                    int ea[3] = { 0, 0, 0 }, eb[3] = { 0, 0, 0 };
+                    ea[a] = 1; eb[b] = 1;
+                    /* component c's g1 feeds lamE_b, its g2 feeds lamE_a */
+                    lE[b][p] -= st->tmp[c][0][p] - at(D, st->tmp[c][0], i - ea[0], j - ea[1], k - ea[2]);
+                    lE[a][p] -= st->tmp[c][1][p] - at(D, st->tmp[c][1], i - eb[0], j - eb[1], k - eb[2]);
+                }
+            }
+}
+
+/* ------------------------------------------------------------------------ */
+/* B5: adjoint of O1 (E update incl. psi_E recursion), whole grid.          */
+/*   with w = +S ie lamE_c: same pattern, E tables;                         */
+/*   lamH_b += (dm_a)^T g1 = -dp_a g1 ; lamH_a += (dm_b)^T g2 = -dp_b g2    */
+/* ------------------------------------------------------------------------ */
+void orc_adj_E(orc_state *st, REAL *lam, const REAL *ie)
+{
+    const orc_desc *D = &st->D;
+    const REAL S = (REAL)D->S;
+    const size_t nc = st->nc;
+    const REAL *lE[3] = { lam, lam + nc, lam + 2 * nc };
+    REAL *lH[3] = { lam + 3 * nc, lam + 4 * nc, lam + 5 * nc };
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (int k = 0; k < NZ; ++k)
+        for (int j = 0; j < NY; ++j)
+            for (int i = 0; i < NX; ++i) {
+                const size_t p = IDX(i, j, k);
+                const int pos[3] = { i, j, k };
+                for (int c = 0; c < 3; ++c) {
+                    const int a = (c + 1) % 3, b = (c + 2) % 3;
+                    REAL w = S * ie[p] * lE[c][p];
+                    REAL l0 = st->lpsiE[c][0][p] + w;
+                    REAL l1 = st->lpsiE[c][1][p] - w;
+                    st->tmp[c][0][p] = st->ikE[a][pos[a]] * w + st->aE[a][pos[a]] * l0;
+                    st->tmp[c][1][p] = -st->ikE[b][pos[b]] * w + st->aE[b][pos[b]] * l1;
+                    st->lpsiE[c][0][p] = st->bE[a][pos[a]] * l0;
+                    st->lpsiE[c][1][p] = st->bE[b][pos[b]] * l1;
+                }
+            }
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (int k = 0; k < NZ; ++k)
+        for (int j = 0; j < NY; ++j)
+            for (int i = 0; i < NX; ++i) {
+                const size_t p = IDX(i, j, k);
+                for (int c = 0; c < 3; ++c) {
+                    const int a = (c + 1) % 3, b = (c + 2) % 3;
+                    int ea[3] = { 0, 0, 0 }, eb[3] = { 0, 0, 0 };
+                    ea[a] = 1; eb[b] = 1;
+                    lH[b][p] -= at(D, st->tmp[c][0], i + ea[0], j + ea[1], k + ea[2]) - st->tmp[c][0][p];
+                    lH[a][p] -= at(D, st->tmp[c][1], i + eb[0], j + eb[1], k + eb[2]) - st->tmp[c][1][p];
+                }
+            }
+}
+
+/* ------------------------------------------------------------------------ */
+/* O6c: inverse H step on the interior box I ("the inverse     */
+/* function of the FDTD update"):  H = H' + S im curl+ E'                    */
+/* An E' operand one cell outside I on the high side (index N_a - d) is not  */
+/* read from the volume but from this step's record (rec_n); on a periodic   */
+/* grid I is the whole box and operands wrap.  H sources are subtracted by   */
+/* the caller before this function.                                          */
+/* ------------------------------------------------------------------------ */
+static REAL E_plus(const orc_desc *D, const REAL *const E[3], const REAL *rec_n,
+                   int comp, int axis, int i, int j, int k)
+{
+    int pos[3] = { i, j, k };
+    pos[axis] += 1;
+    if (D->d > 0 && pos[axis] == hi_I(D, axis)) {
+        int which = (comp - axis - 1 + 3) % 3;               /* 0: comp = axis+1, 1: comp = axis+2 */
+        return rec_n[rec_offset(D, axis, 1, which) + face_index(D, axis, pos)];
+    }
+    return at(D, E[comp], pos[0], pos[1], pos[2]);
+}
+
+void orc_inv_H(orc_state *st, REAL *fields, const REAL *im, const REAL *rec_n)
+{
+    const orc_desc *D = &st->D;
+    const REAL S = (REAL)D->S;
+    const size_t nc = st->nc;
+    const REAL *E[3] = { fields, fields + nc, fields + 2 * nc };
+    REAL *H[3] = { fields + 3 * nc, fields + 4 * nc, fields + 5 * nc };
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (int k = lo_I(D, 2); k < hi_I(D, 2); ++k)
+        for (int j = lo_I(D, 1); j < hi_I(D, 1); ++j)
+            for (int i = lo_I(D, 0); i < hi_I(D, 0); ++i) {
+                const size_t p = IDX(i, j, k);
+                for (int c = 0; c < 3; ++c) {
+                    const int a = (c + 1) % 3, b = (c + 2) % 3;
+                    REAL d1 = E_plus(D, E, rec_n, b, a, i, j, k) - E[b][p];
+                    REAL d2 = E_plus(D, E, rec_n, a, b, i, j, k) - E[a][p];
+                    H[c][p] += S * (im ? im[p] : (REAL)1) * (d1 - d2);
+                }
+            }
+}
+
+/* ------------------------------------------------------------------------ */
+/* O7a: q = curl- H on I (an H operand at index d-1 comes from the record),  */
+/*      g += S sum_c lamE_c q_c   (VJP wrt inv_eps; lamE is the cotangent of */
+/*      the post-update E'),  E = E' - S ie q   (inverse E step).            */
+/* E sources are subtracted by the caller before this function.             */
+/* ------------------------------------------------------------------------ */
+static REAL H_minus(const orc_desc *D, const REAL *const H[3], const REAL *rec_n,
+                    int comp, int axis, int i, int j, int k)
+{
+    int pos[3] = { i, j, k };
+    pos[axis] -= 1;
+    if (D->d > 0 && pos[axis] == lo_I(D, axis) - 1) {
+        int which = (comp - axis - 1 + 3) % 3;
+        return rec_n[rec_offset(D, axis, 0, which) + face_index(D, axis, pos)];
+    }
+    return at(D, H[comp], pos[0], pos[1], pos[2]);
+}
+
+void orc_inv_E_grad(orc_state *st, REAL *fields, const REAL *ie, const REAL *lam,
+                    REAL *g, const REAL *rec_n)
+{
+    const orc_desc *D = &st->D;
+    const REAL S = (REAL)D->S;
+    const size_t nc = st->nc;
+    REAL *E[3] = { fields, fields + nc, fields + 2 * nc };
+    const REAL *H[3] = { fields + 3 * nc, fields + 4 * nc, fields + 5 * nc };
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (int k = lo_I(D, 2); k < hi_I(D, 2); ++k)
+        for (int j = lo_I(D, 1); j < hi_I(D, 1); ++j)
+            for (int i = lo_I(D, 0); i < hi_I(D, 0); ++i) {
+                const size_t p = IDX(i, j, k);
+                REAL acc = (REAL)0;
+                for (int c = 0; c < 3; ++c) {
+                    const int a = (c + 1) % 3, b = (c + 2) % 3;
+                    REAL d1 = H[b][p] - H_minus(D, H, rec_n, b, a, i, j, k);
+                    REAL d2 = H[a][p] - H_minus(D, H, rec_n, a, b, i, j, k);
+                    REAL q = d1 - d2;
+                    if (lam) acc += lam[(size_t)c * nc + p] * q;
+                    E[c][p] -= S * ie[p] * q;
+                }
+                if (g) g[p] += S * acc;
+            }
+}
+
+/* ------------------------------------------------------------------------ */
+/* reverse driver (time-reversed gradient):                    */
+/* for n = n_steps-1 .. 0:  B1, [O4^T: nothing], B2, primal -srcH, O6c,      */
+/*                          O7a (after -srcE), B5                            */
+/* fields: in = state n_steps (valid on I), out = reconstructed state 0 on I */
+/* g (cells) and dL_dfields0 (6*cells, may be NULL) are outputs.             */
+/* ------------------------------------------------------------------------ */
+int orc_backward(orc_state *st, REAL *fields, const REAL *ie, const REAL *im,
+                 const orc_source *src, int n_src, const orc_detector *det, int n_det,
+                 const REAL *const *dL_dphasor, const REAL *dL_dfields,
+                 int n_steps, const REAL *rec, REAL *g, REAL *dL_dfields0)
+{
+    const orc_desc *D = &st->D;
+    const size_t nc = st->nc;
+    const size_t rs = orc_record_stride(D);
+    if (D->d > 0 && !rec) return -4;
+    REAL *lam = zalloc(6 * nc);
+    if (!lam) return -2;
+    if (dL_dfields) memcpy(lam, dL_dfields, 6 * nc * sizeof(REAL));      /* B0 */
+    orc_zero_lpsi(st);
+    memset(g, 0, nc * sizeof(REAL));
+    for (int n = n_steps - 1; n >= 0; --n) {
+        const REAL *rec_n = rec ? rec + (size_t)n * rs : NULL;
+        detect_adjoint(D, lam, nc, det, n_det, dL_dphasor, n);           /* B1  */
+        orc_adj_H(st, lam, im);                                          /* B2  */
+        add_sources(D, fields, nc, src, n_src, n, 1, (REAL)-1);          /* undo O4 */
+        orc_inv_H(st, fields, im, rec_n);                                /* O6c */
+        add_sources(D, fields, nc, src, n_src, n, 0, (REAL)-1);          /* undo O2 */
+        orc_inv_E_grad(st, fields, ie, lam, g, rec_n);                   /* O7a */
+        orc_adj_E(st, lam, ie);                                          /* B5  */
+    }
+    if (dL_dfields0) memcpy(dL_dfields0, lam, 6 * nc * sizeof(REAL));
+    free(lam);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------ */
+/* tape-mode gradient (the plain definition: reverse-mode derivative of the  */
+/* forward program with every E-update bracket stored):                      */
+/*   g += S sum_c lamE'_c * bracket_n,c    on ALL cells (PML included)       */
+/* ------------------------------------------------------------------------ */
+int orc_backward_tape(orc_state *st, const REAL *ie, const REAL *im,
+                      const orc_detector *det, int n_det,
+                      const REAL *const *dL_dphasor, const REAL *dL_dfields,
+                      int n_steps, const REAL *tape, REAL *g, REAL *dL_dfields0)
+{
+    const orc_desc *D = &st->D;
+    const size_t nc = st->nc;
+    const REAL S = (REAL)D->S;
+    REAL *lam = zalloc(6 * nc);
+    if (!lam) return -2;
+    if (dL_dfields) memcpy(lam, dL_dfields, 6 * nc * sizeof(REAL));
+    orc_zero_lpsi(st);
+    memset(g, 0, nc * sizeof(REAL));
+    for (int n = n_steps - 1; n >= 0; --n) {
+        const REAL *br = tape + (size_t)n * 3 * nc;
+        detect_adjoint(D, lam, nc, det, n_det, dL_dphasor, n);
+        orc_adj_H(st, lam, im);
+        for (int c = 0; c < 3; ++c)
+            for (size_t p = 0; p < nc; ++p)
+                g[p] += S * lam[(size_t)c * nc + p] * br[(size_t)c * nc + p];
+        orc_adj_E(st, lam, ie);
+    }
+    if (dL_dfields0) memcpy(dL_dfields0, lam, 6 * nc * sizeof(REAL));
+    free(lam);
+    return 0;
+}
