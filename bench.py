@@ -1,0 +1,378 @@
+#!/usr/bin/env python
+"""bench.py -- Yee cell-updates/s of the FDTD hot path on B200 (BASELINE.json metric).
+
+One "step" = one whole pass of the hot path over one synthetic problem: fdtd_forward with
+interface recording (F1..F8) + the caller's loss cotangent + fdtd_backward (B0..B5) + the
+rho chain rule (B6) on the graded config C3 (200^3, 12-cell CPML, 2000 time steps, 864k design
+voxels).  value = cells * n_time_steps * K / (time of K steps), summed over ranks.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--time-steps T]
+
+N > 1 (torchrun): every rank runs an independent problem (seed + rank), no data-path collective
+("weak" scaling over independent inverse-design problems).
+--impl reference times the CPU oracle (oracle/, fp32 build, all host cores) on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+METRIC = "Yee cell-updates/s, forward + time-reversed backward (C3 gradient)"
+UNIT = "Mcells/s"
+
+
+# ------------------------------------------------------------------------------------------------
+# algorithmic bytes: what one launch of each kernel class must move
+# ------------------------------------------------------------------------------------------------
+def algorithmic_bytes(w, grad_cells: int, recording: bool, has_mu: bool = False) -> dict:
+    nx, ny, nz, d = w.nx, w.ny, w.nz, w.pml_cells
+    cells = nx * ny * nz
+    inter = (nx - 2 * d) * (ny - 2 * d) * (nz - 2 * d)
+    slab = 2 * d * (ny * nz + nx * nz + nx * ny)            # slab cells summed over the three axes
+    face = 4 * ((ny - 2 * d) * (nz - 2 * d) + (nx - 2 * d) * (nz - 2 * d) + (nx - 2 * d) * (ny - 2 * d)) if d else 0
+    mu = 4 if has_mu else 0
+    rec = 4 * face if recording else 0                      # 2 comps x 2 sides per face cell, fp32
+    return {
+        # fused: 6 R + 6 W fields + ie (+im); psi R/W: 4 arrays (2E+2H) per slab cell per axis; recorder W
+        "fused_forward_step": cells * (52 + mu) + slab * 32 + rec,
+        # fused backward: adjoint 6R+6W+ie over the grid, inverse 6R+6W over I, g R/W on the grad box,
+        # adjoint psi R/W on slabs, recorder R
+        "fused_backward_step": cells * (52 + mu) + inter * 48 + grad_cells * 8 + slab * 32 + 4 * face,
+        "update_E": cells * 40 + slab * 16,
+        "update_H": cells * (36 + mu) + slab * 16,
+        "adjoint_H": cells * (36 + mu) + slab * 16,
+        "adjoint_E": cells * 40 + slab * 16,
+        "inverse_H": inter * (36 + mu),
+        "inverse_E_grad": inter * 52 + grad_cells * 8,
+        "record_faces": 2 * 4 * face,
+        "inject_faces": 2 * 4 * face,
+    }
+
+
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.idx = gpu_index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.idx), "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            parts = [p.strip() for p in ln.split(",")]
+            if len(parts) < 9:
+                continue
+            try:
+                sm.append(float(parts[1])); mx.append(float(parts[2]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, parts[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------
+def cpu_oracle_rate(w, sample_steps: int):
+    """Times the oracle as it stands (fp32 build, OpenMP over all host cores, FTZ on) on the first
+    `sample_steps` time steps of the workload: forward with recording + reversible backward."""
+    import numpy as np
+    from oracle.oracle import Oracle
+    o = Oracle(**w.grid_kwargs(), dtype=np.float32)
+    o.set_ftz(True)
+    f = np.zeros((6, w.nz, w.ny, w.nx), dtype=np.float32)
+    t0 = time.perf_counter()
+    out = o.forward(f, w.inv_eps, None, w.sources, w.detectors, sample_steps, record=w.pml_cells > 0)
+    t1 = time.perf_counter()
+    dLp = [2.0 * P if i in w.loss_detectors else None for i, P in enumerate(out["phasors"])]
+    o.backward(f, w.inv_eps, None, w.sources, w.detectors, dLp, None, sample_steps, out["rec"])
+    t2 = time.perf_counter()
+    cells = w.cells * sample_steps
+    return {"value": cells / (t2 - t0) / 1e6, "fwd_value": cells / (t1 - t0) / 1e6, "unit": UNIT,
+            "cores": o.num_threads(), "kind": "oracle",
+            "sample": f"{w.name} {w.nx}x{w.ny}x{w.nz} grid, first {sample_steps} of {w.n_steps} time steps, "
+                      f"forward(record)+reversible backward, fp32 build of oracle/fdtd_oracle.c, OpenMP, FTZ"}
+
+
+def workload_config(w, extra=None):
+    cfg = {"workload": f"{w.name}: {w.nx}x{w.ny}x{w.nz} fp32 Yee grid, {w.pml_cells}-cell CPML, {w.n_steps} time steps, "
+                       f"forward(record)+reversible backward, grad box = design region",
+           "time_steps": w.n_steps, "cells": w.cells,
+           "l2": "inputs larger than L2 (working set > 0.5 GB vs 126 MB L2); no flush needed"}
+    if extra:
+        cfg.update(extra)
+    return cfg
+
+
+def run_reference(args, rank):
+    """--impl reference: the CPU oracle on the host cores (bounded sample per step)."""
+    if rank != 0:
+        return
+    from paper_2412_12360_b200 import workloads as wl
+    w = wl.c3(n_steps=args.time_steps)
+    sample = args.ref_sample_steps
+    for _ in range(args.warmup):
+        cpu_oracle_rate(w, max(1, sample // 4))
+    t0 = time.perf_counter()
+    rates = [cpu_oracle_rate(w, sample) for _ in range(args.steps)]
+    dt = time.perf_counter() - t0
+    val = w.cells * sample * args.steps / sum(w.cells * sample / (r["value"] * 1e6) for r in rates) / 1e6
+    cb = dict(rates[-1]); cb["value"] = val
+    print(json.dumps({"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+                      "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+                      "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+                      "data": "synthetic", "config": workload_config(w, {"sample_time_steps": sample}),
+                      "cpu_baseline": cb,
+                      "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+# ------------------------------------------------------------------------------------------------
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--time-steps", type=int, default=2000, help="FDTD time steps per gradient (C3: 2000)")
+    ap.add_argument("--grid", type=int, default=200, help="C3 grid size per axis (200)")
+    ap.add_argument("--path", default="auto", choices=["auto", "generic", "fused"])
+    ap.add_argument("--ref-sample-steps", type=int, default=12)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2412_12360_b200 import binding as B
+    from paper_2412_12360_b200 import workloads as wl
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- workload: C3 (seed + rank: every rank an independent problem) -----------------------------
+    w = wl.c3(n=args.grid, n_steps=args.time_steps, seed=3 + rank)
+    T = w.n_steps
+    path = {"auto": B.FDTD_PATH_AUTO, "generic": B.FDTD_PATH_GENERIC, "fused": B.FDTD_PATH_FUSED}[args.path]
+    kw = w.grid_kwargs()
+    kw.update(max_steps=T, record=True, grad_lo=w.design_lo, grad_hi=w.design_hi, path=path)
+    grid = B.Grid(**kw)
+    kw_f = dict(kw); kw_f.update(record=False)
+    grid_f = B.Grid(**kw_f)                                   # forward-only grid (no recorder)
+    stream = torch.cuda.Stream()
+    dev = torch.device("cuda", local_rank)
+    ie = torch.as_tensor(w.inv_eps).to(dev)
+    fields = torch.zeros((6, w.nz, w.ny, w.nx), dtype=torch.float32, device=dev)
+    for s in w.sources:                                        # resident descriptors
+        s.waveform = torch.as_tensor(s.waveform).to(dev)
+        s.profile = None if s.profile is None else torch.as_tensor(s.profile).to(dev)
+    phasors = [torch.zeros(d.phasor_shape, dtype=torch.float32, device=dev) for d in w.detectors]
+    grad = torch.empty((w.nz, w.ny, w.nx), dtype=torch.float32, device=dev)
+    dlo, dhi = w.design_lo, w.design_hi
+    drho = torch.empty((dhi[2] - dlo[2], dhi[1] - dlo[1], dhi[0] - dlo[0]), dtype=torch.float32, device=dev)
+    grad_cells = drho.numel()
+    delta_eps = float(w.meta["delta_eps"])
+
+    def gradient_step(g):
+        """One pass of the whole hot path, inputs resident in HBM."""
+        fields.zero_()
+        for P in phasors:
+            P.zero_()
+        g.forward(fields, ie, None, w.sources, w.detectors, T, phasors=phasors)
+        dLp = [2.0 * P if i in w.loss_detectors else None for i, P in enumerate(phasors)]   # caller's loss
+        g.backward(fields, ie, None, w.sources, w.detectors, dLp, None, T, out=grad)
+        B.fdtd_grad_rho(g.h, grad, ie, delta_eps, dlo, dhi, drho, g.stream())
+
+    def forward_only(g):
+        fields.zero_()
+        for P in phasors:
+            P.zero_()
+        g.forward(fields, ie, None, w.sources, w.detectors, T, phasors=phasors)
+
+    def timed(fn, reps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record(stream)
+        for _ in range(reps):
+            fn()
+        e1.record(stream)
+        barrier()
+        ms = torch.tensor([e0.elapsed_time(e1)], device=dev)
+        if world > 1:
+            dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+        return float(ms.item())
+
+    with torch.cuda.stream(stream):
+        for _ in range(args.warmup):
+            gradient_step(grid)
+        l0 = grid.info().kernel_launches
+        sampler = ClockSampler(local_rank)
+        sampler.start()
+        ms_total = timed(lambda: gradient_step(grid), args.steps)
+        clocks = sampler.stop()
+        launches = grid.info().kernel_launches - l0
+        loss = float(sum((P.double() ** 2).sum() for i, P in enumerate(phasors) if i in w.loss_detectors))
+        gnorm = float(drho.double().abs().max())
+
+        # forward-only (record=0) rate, same workload
+        for _ in range(min(args.warmup, 2)):
+            forward_only(grid_f)
+        ms_fwd = timed(lambda: forward_only(grid_f), max(1, args.steps))
+
+        # ---- per-kernel roofline: one more pass with every step kernel bracketed by CUDA events --------
+        B.fdtd_set_profiling(grid.h, True)
+        B.fdtd_get_profile(grid.h)
+        gradient_step(grid)
+        torch.cuda.synchronize()
+        prof = B.fdtd_get_profile(grid.h)
+        B.fdtd_set_profiling(grid.h, False)
+
+    cells_steps = w.cells * T
+    value = world * cells_steps * args.steps / (ms_total * 1e-3) / 1e6
+    fwd_value = world * cells_steps * max(1, args.steps) / (ms_fwd * 1e-3) / 1e6
+
+    peaks_file = ROOT / "MEASURED_PEAKS.json"
+    if peaks_file.exists():
+        peak, peak_src = float(json.loads(peaks_file.read_text())["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    else:
+        peak, peak_src = 6650.0, "fallback (B200_PROFILING.md)"
+    alg = algorithmic_bytes(w, grad_cells, recording=True)
+    kernels = {}
+    for name, (n, ms) in prof.items():
+        if name in alg and n:
+            gbs = alg[name] * n / (ms * 1e-3) / 1e9
+            kernels[name] = {"launches": n, "avg_us": ms / n * 1e3, "alg_bytes_per_launch": alg[name],
+                             "achieved_gbs": gbs, "frac": gbs / peak, "share_of_step": None}
+        else:
+            kernels[name] = {"launches": n, "avg_us": ms / n * 1e3 if n else None}
+    tot_ms = sum(ms for _, ms in prof.values()) or 1.0
+    for name, (n, ms) in prof.items():
+        kernels[name]["share_of_step"] = ms / tot_ms
+    dom = max((k for k in kernels if "achieved_gbs" in kernels[k]), key=lambda k: prof[k][1], default=None)
+    roofline = None
+    if dom:
+        traffic = None
+        tf = ROOT / "profiles" / "traffic.json"      # dram bytes per launch from the committed ncu --set full capture
+        if tf.exists():
+            traffic = json.loads(tf.read_text()).get(dom)
+        roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["achieved_gbs"], "peak": peak,
+                    "peak_source": peak_src, "unit": "GB/s", "frac": kernels[dom]["frac"], "traffic": traffic,
+                    "alg_bytes_per_launch": alg[dom], "avg_launch_us": kernels[dom]["avg_us"],
+                    "frac_of_8000": kernels[dom]["achieved_gbs"] / 8000.0}
+
+    # ---- end to end through the host-buffer C ABI (pinned host memory, H2D/D2H inside the timed region) ----
+    e2e = None
+    if not args.no_e2e:
+        h_ie = torch.as_tensor(w.inv_eps).pin_memory()
+        h_grad = torch.empty((w.nz, w.ny, w.nx), dtype=torch.float32).pin_memory()
+        h_ph = [torch.zeros(d.phasor_shape, dtype=torch.float32).pin_memory() for d in w.detectors]
+        h_cot = [torch.zeros(d.phasor_shape, dtype=torch.float32).pin_memory() for d in w.detectors]
+        host_src = [wl.Source(s.component, s.lo, s.hi, s.waveform.cpu().numpy(),
+                              None if s.profile is None else s.profile.cpu().numpy()) for s in w.sources]
+        sarr, ns, k1 = grid.marshal_sources(host_src, host=True)
+        darr, nd, k2 = grid.marshal_detectors(w.detectors, h_ph)
+        import ctypes as C
+        cot = (C.c_void_p * max(nd, 1))()
+        for i in range(nd):
+            cot[i] = h_cot[i].data_ptr() if i in w.loss_detectors else None
+        sp = C.c_void_p(stream.cuda_stream)
+        h2d = h_ie.numel() * 4 * 2 + sum(p.numel() * 4 for p in h_ph) + sum(h_cot[i].numel() * 4 for i in w.loss_detectors)
+        h2d += sum(s.waveform.size * 4 + (0 if s.profile is None else s.profile.size * 4) for s in host_src) * 2
+        d2h = h_grad.numel() * 4 + sum(p.numel() * 4 for p in h_ph)
+
+        def e2e_step():
+            for P in h_ph:
+                P.zero_()
+            B.fdtd_forward_host(grid.h, None, h_ie, None, sarr, ns, darr, nd, T, sp)
+            for i in w.loss_detectors:
+                torch.mul(h_ph[i], 2.0, out=h_cot[i])                      # caller's loss cotangent on the host
+            B.fdtd_backward_host(grid.h, None, h_ie, None, sarr, ns, darr, nd, cot, None, T, h_grad, None, sp)
+
+        e2e_step()
+        t0 = time.perf_counter()
+        ms_e2e = timed(e2e_step, max(1, min(args.steps, 3)))
+        reps = max(1, min(args.steps, 3))
+        e2e = {"value": world * cells_steps * reps / (ms_e2e * 1e-3) / 1e6, "unit": UNIT,
+               "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "ms_per_step": ms_e2e / reps,
+               "api": "fdtd_forward_host + fdtd_backward_host (pinned host buffers)"}
+
+    info = grid.info()
+    if rank == 0:
+        cpu = None
+        if not args.no_cpu_baseline and world == 1:
+            cpu = cpu_oracle_rate(wl.c3(n=args.grid, n_steps=args.time_steps), args.ref_sample_steps)
+        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+               "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+               "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+               "config": workload_config(w, {"path": {1: "generic", 2: "fused"}[info.path],
+                                             "tile": [info.tile_x, info.tile_y, info.tile_z],
+                                             "parallelism": f"independent problems x{world}"}),
+               "fwd": {"value": fwd_value, "unit": UNIT, "ms_per_pass": ms_fwd / max(1, args.steps),
+                       "what": "forward only, record=0, same workload"},
+               "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+               "roofline": roofline, "kernels": kernels, "cpu_baseline": cpu,
+               "check": {"loss": loss, "max_abs_dL_drho": gnorm}}
+        print(json.dumps(out))
+    grid.close()
+    grid_f.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,221 @@
+/*
+ * fdtd.h -- C ABI of the B200-native FDTD hot path (arXiv 2412.12360, "FDTDX").
+ *
+ * What the library computes (citations: /root/reference/PAPER.md line numbers; the
+ * discretisation choices the paper leaves open are the readings R1..R22 of DESIGN.md):
+ *
+ *   forward  : n_steps of the Yee-grid leapfrog (Eq. 1-2; Yee staggering L68):
+ *              E update with per-voxel inverse permittivity and CPML psi_E recursion (L72),
+ *              additive E sources (L72), [record interface values, L84], H update with per-voxel
+ *              inverse permeability and CPML psi_H, additive H sources, running-DFT detectors
+ *              (L68 "detector object"; interpolation off, L70).
+ *   backward : the memory-efficient gradient of L84: for n = n_steps-1 .. 0 an inverse update
+ *              reconstructs the interior fields of step n from those of step n+1 (the PML is not
+ *              invertible, so the recorded PML/interior interface values are re-imposed), fused
+ *              with the vector-Jacobian product (L78-84) that propagates the cotangents through
+ *              the whole grid (adjoint CPML included) and accumulates dL/d(inv_eps) per voxel.
+ *
+ * Conventions
+ *   grid nx*ny*nz cells, cell (i,j,k), x fastest: lin = (k*ny + j)*nx + i.  All volumes are fp32
+ *   [nz][ny][nx].  `fields` is [6][nz][ny][nx], components Ex,Ey,Ez,Hx,Hy,Hz.  H is scaled by
+ *   eta0, lengths by dx, times by dt: the only constant is the Courant number S = c dt/dx.
+ *   For component c let a = c+1, b = c+2 (mod 3):
+ *     E_c += S*ie*( ikE_a*dm_a H_b - ikE_b*dm_b H_a + psiE_c0 - psiE_c1 ),  dm_a F[p] = F[p]-F[p-e_a]
+ *     H_c -= S*im*( ikH_a*dp_a E_b - ikH_b*dp_b E_a + psiH_c0 - psiH_c1 ),  dp_a F[p] = F[p+e_a]-F[p]
+ *   (H from the just-updated E).  A neighbour outside the grid is the wrapped cell on a periodic
+ *   grid and 0 otherwise.  One step n maps (E^n, H^{n+1/2}) to (E^{n+1}, H^{n+3/2}).
+ *   Interior box I = [d, N-d) on every axis (d = pml_cells); whole grid when d == 0.
+ *
+ * Memory / ownership
+ *   Every pointer marked DEVICE is caller-owned CUDA device memory (e.g. a PyTorch allocation),
+ *   contiguous and 16-byte aligned; the library never frees or retains it beyond the call.
+ *   Pointers marked HOST are ordinary host memory read during the call.  The grid object owns
+ *   only scratch: CPML tables, psi slabs, cotangent fields, ping-pong copies, the recorder.
+ *
+ * Execution
+ *   All work is enqueued on `cuda_stream` (a cudaStream_t passed as void*, NULL = legacy default
+ *   stream).  The device entry points do not synchronise the host with the device and copy
+ *   nothing device->host.  The *_host entry points (below) copy host<->device and synchronise.
+ *
+ * Errors
+ *   Every function returns FDTD_OK (0) or a negative code; fdtd_last_error() returns a
+ *   thread-local, never-NULL description of the last failure.  No exceptions, aborts or prints.
+ */
+#ifndef FDTD_B200_H
+#define FDTD_B200_H
+
+#include <stdint.h>
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define FDTD_API __attribute__((visibility("default")))
+#else
+#define FDTD_API
+#endif
+
+#define FDTD_OK        0
+#define FDTD_EINVAL   -1   /* bad dims / Courant / boxes / NULL required pointer / n_steps > max_steps */
+#define FDTD_ENOMEM   -2   /* device allocation failed (recorder, scratch)                           */
+#define FDTD_ECUDA    -3   /* CUDA runtime / driver error; message holds cudaGetErrorString           */
+#define FDTD_ESTATE   -4   /* backward on a CPML grid without a matching recorded forward              */
+
+/* kernel path selection (fdtd_grid_desc.path) */
+#define FDTD_PATH_AUTO     0   /* fused TMA kernels when the grid qualifies, else generic            */
+#define FDTD_PATH_GENERIC  1   /* one-thread-per-cell kernels (periodic grids, odd sizes, debugging)  */
+#define FDTD_PATH_FUSED    2   /* fused kernels; create_grid fails with EINVAL if not applicable      */
+
+typedef struct fdtd_grid fdtd_grid;      /* opaque */
+
+/* Grid descriptor.  A zero in any CPML constant selects its default (reading R8). */
+typedef struct {
+    int32_t nx, ny, nz;        /* cells per axis, each >= 1                                          */
+    float   courant;           /* S = c*dt/dx, 0 < S < 1/sqrt(3) (stability for ie*im <= 1 everywhere;
+                                  keeping S*sqrt(max ie*im) < 1/sqrt(3) is the caller's job)         */
+    int32_t periodic;          /* 1: periodic box (pml_cells must be 0); 0: zero outside the grid    */
+    int32_t pml_cells;         /* d >= 0; if d > 0 then 2*d + 2 <= min(nx,ny,nz)                     */
+    float   pml_m;             /* polynomial grading order of sigma and kappa      (default 3)      */
+    float   pml_sigma_scale;   /* sigma~_max = scale/sqrt(pml_eps_bg)              (default 0.8*(m+1)) */
+    float   pml_kappa_max;     /* kappa at full depth                              (default 1)      */
+    float   pml_alpha_max;     /* alpha~ at the interface, graded to 0 at full depth (default 0)    */
+    float   pml_alpha_m;       /* grading order of alpha                           (default 1)      */
+    float   pml_eps_bg;        /* background relative permittivity used in sigma~_max (default 1)   */
+    int32_t max_steps;         /* upper bound of n_steps; sizes the recorder when record != 0       */
+    int32_t record;            /* 0: forward only; 1: record the PML/interior interface every step  */
+    int32_t grad_lo[3];        /* half-open (i,j,k) box on which dL_dinv_eps is wanted;             */
+    int32_t grad_hi[3];        /*   all zero => the whole interior I.  Always clipped to I.         */
+    int32_t path;              /* FDTD_PATH_*                                                       */
+    int32_t reserved[7];       /* must be zero                                                      */
+} fdtd_grid_desc;
+
+/* Additive source patch (reading R10/R11): during step n,
+ * F_c[box] += profile[cell] * waveform[n], after the update of F's family (E or H).
+ * A one-directional TFSF plane is one E patch plus one H patch. */
+typedef struct {
+    int32_t component;         /* 0..5 = Ex,Ey,Ez,Hx,Hy,Hz                                          */
+    int32_t lo[3], hi[3];      /* half-open box in (i,j,k), inside the grid, non-empty              */
+    const float *profile;      /* DEVICE, box-shaped [k][j][i]; NULL => 1.0                         */
+    const float *waveform;     /* DEVICE, length >= n_steps                                         */
+} fdtd_source;
+
+/* Running-DFT detector (reading R13): after step n,
+ * P_f[c][cell] += F_c[cell] * exp(-i*omega_f*(n+1)) for every component c in component_mask. */
+typedef struct {
+    int32_t component_mask;    /* bit c set => component c is accumulated                            */
+    int32_t lo[3], hi[3];      /* half-open box in (i,j,k), inside the grid, non-empty              */
+    int32_t n_freq;            /* >= 1                                                              */
+    const float *omega;        /* HOST, n_freq angular frequencies in rad per step                  */
+    float *phasor;             /* DEVICE, [n_freq][n_comp_set][box cells][2] (re,im), box cells
+                                  ordered [k][j][i]; accumulated INTO (caller zeroes).  Ignored by
+                                  fdtd_backward.                                                    */
+} fdtd_detector;
+
+/* Creates a grid: validates the descriptor, builds the CPML tables (fp64 on the host, stored
+ * fp32), allocates psi slabs and, when record != 0, the recorder for max_steps steps.
+ * Errors: EINVAL (see above), ENOMEM, ECUDA.  *out is NULL on failure. */
+FDTD_API int fdtd_create_grid(const fdtd_grid_desc *desc, fdtd_grid **out);
+
+/* Runs n_steps forward steps (0 <= n_steps <= max_steps) from the state in `fields`
+ * (DEVICE, [6][nz][ny][nx]; in: state 0, out: state n_steps), with psi = 0 at entry (R21).
+ * inv_eps: DEVICE [nz][ny][nx]; inv_mu: DEVICE [nz][ny][nx] or NULL (= 1).
+ * src/det: HOST arrays of n_src / n_det descriptors (may be NULL when the count is 0).
+ * With record != 0 the interface values of steps 0..n_steps-1 are stored in the grid. */
+FDTD_API int fdtd_forward(fdtd_grid *grid, float *fields, const float *inv_eps, const float *inv_mu,
+                 const fdtd_source *src, int32_t n_src,
+                 const fdtd_detector *det, int32_t n_det,
+                 int32_t n_steps, void *cuda_stream);
+
+/* Time-reversed gradient of a scalar loss L(fields_n, phasors).
+ * fields      : DEVICE, in: state n_steps as left by fdtd_forward; out: reconstructed state 0
+ *               on I (cells outside I are unspecified).
+ * src, det    : the descriptors of the forward call (sources are subtracted in the inverse step;
+ *               detectors give geometry and omega).
+ * dL_dphasor  : HOST array of n_det DEVICE pointers, each laid out like the detector's phasor
+ *               (dL/dRe, dL/dIm); the array or any entry may be NULL (= zero cotangent).
+ * dL_dfields  : DEVICE [6][nz][ny][nx] cotangent of state n_steps, or NULL (= 0).
+ * dL_dinv_eps : DEVICE [nz][ny][nx], OUT; zero-filled by the library, non-zero only on
+ *               I intersected with the grad box (R17).  inv_mu and source gradients are not computed.
+ * dL_dfields0 : DEVICE [6][nz][ny][nx] OUT cotangent of state 0, or NULL.
+ * Errors: ESTATE if pml_cells > 0 and the last fdtd_forward on this grid did not record exactly
+ *         n_steps steps. */
+FDTD_API int fdtd_backward(fdtd_grid *grid, float *fields, const float *inv_eps, const float *inv_mu,
+                  const fdtd_source *src, int32_t n_src,
+                  const fdtd_detector *det, int32_t n_det,
+                  const float *const *dL_dphasor, const float *dL_dfields,
+                  int32_t n_steps, float *dL_dinv_eps, float *dL_dfields0,
+                  void *cuda_stream);
+
+/* B6, chain rule to design parameters (once per gradient, not per step): for a design box whose
+ * permittivity is eps = eps_bg + delta_eps*rho (reading R20),
+ *   dL_drho[cell] = dL_dinv_eps[cell] * d(1/eps)/drho = -dL_dinv_eps[cell] * delta_eps * inv_eps[cell]^2.
+ * dL_dinv_eps, inv_eps: DEVICE volumes; dL_drho: DEVICE, box-shaped [k][j][i], OUT. */
+FDTD_API int fdtd_grad_rho(fdtd_grid *grid, const float *dL_dinv_eps, const float *inv_eps, float delta_eps,
+                           const int32_t lo[3], const int32_t hi[3], float *dL_drho, void *cuda_stream);
+
+/* Frees the grid and everything it owns (synchronises the device first).  NULL is a no-op. */
+FDTD_API int fdtd_destroy(fdtd_grid *grid);
+
+/* Thread-local description of the last error on this thread ("" if none).  Never NULL. */
+FDTD_API const char *fdtd_last_error(void);
+
+/* Introspection for benchmarks and tests (no device work). */
+typedef struct {
+    int32_t path;                    /* FDTD_PATH_GENERIC or FDTD_PATH_FUSED actually in use          */
+    int32_t tile_x, tile_y, tile_z;  /* fused path: cells per tile and z-chunk length (0 otherwise)  */
+    int64_t kernel_launches;         /* kernels launched by this grid so far (graph nodes * replays) */
+    int64_t recorder_bytes;          /* bytes of the interface recorder                              */
+    int64_t scratch_bytes;           /* all other device bytes owned by the grid                     */
+    int64_t record_floats_per_step;  /* recorder stride in floats                                    */
+    int64_t reserved[4];
+} fdtd_grid_info;
+FDTD_API int fdtd_get_info(const fdtd_grid *grid, fdtd_grid_info *info);
+
+/* Per-kernel timing for roofline reports.  While profiling is enabled the per-step kernels are
+ * launched directly (no CUDA graph) and every launch of a step kernel is bracketed by CUDA events
+ * recorded on the launch stream.  fdtd_get_profile synchronises those events and returns, per kernel
+ * class, the number of launches and their summed device time since profiling was enabled (or since
+ * the last fdtd_get_profile, which resets the counters). */
+#define FDTD_PROF_CLASSES 12
+typedef struct {
+    int32_t n_classes;                          /* number of valid entries below                       */
+    int32_t reserved;
+    char    name[FDTD_PROF_CLASSES][32];        /* kernel class names, e.g. "fused_forward_step"       */
+    int64_t launches[FDTD_PROF_CLASSES];
+    double  total_ms[FDTD_PROF_CLASSES];
+} fdtd_profile;
+FDTD_API int fdtd_set_profiling(fdtd_grid *grid, int32_t enable);
+FDTD_API int fdtd_get_profile(fdtd_grid *grid, fdtd_profile *out);
+
+/* Library version string, e.g. "fdtd-b200 0.1 sm_100a". */
+FDTD_API const char *fdtd_version(void);
+
+/* ------------------------------------------------------------------------------------------
+ * Host-buffer entry points: same computation, every array argument (and every pointer inside
+ * the descriptors) is HOST memory; the library stages them through device buffers it owns,
+ * runs the device path on `cuda_stream`, copies the results back and synchronises the stream
+ * before returning.  Used for the end-to-end measurement.
+ *   fdtd_forward_host : h_fields in/out (NULL => start from all-zero fields and leave the final
+ *                       state on the device inside the grid); phasors are copied in before and
+ *                       out after the run.
+ *   fdtd_backward_host: h_fields NULL => use the state the last fdtd_forward_host left in the grid;
+ *                       otherwise in: state n, out: reconstructed state 0.  h_dL_dphasor is a HOST
+ *                       array of HOST pointers.  h_dL_dinv_eps is written; h_dL_dfields0 may be NULL.
+ * ------------------------------------------------------------------------------------------ */
+FDTD_API int fdtd_forward_host(fdtd_grid *grid, float *h_fields, const float *h_inv_eps, const float *h_inv_mu,
+                      const fdtd_source *h_src, int32_t n_src,
+                      const fdtd_detector *h_det, int32_t n_det,
+                      int32_t n_steps, void *cuda_stream);
+FDTD_API int fdtd_backward_host(fdtd_grid *grid, float *h_fields, const float *h_inv_eps, const float *h_inv_mu,
+                       const fdtd_source *h_src, int32_t n_src,
+                       const fdtd_detector *h_det, int32_t n_det,
+                       const float *const *h_dL_dphasor, const float *h_dL_dfields,
+                       int32_t n_steps, float *h_dL_dinv_eps, float *h_dL_dfields0,
+                       void *cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FDTD_B200_H */

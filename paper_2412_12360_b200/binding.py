@@ -1,0 +1,302 @@
+"""Thin ctypes binding of include/fdtd.h -- argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI; this module converts Python /
+PyTorch objects to the plain pointers and structs the ABI takes.  PyTorch is used only for
+device allocation and the current stream.  There is NO CPU fallback: if the shared library is
+missing or cannot be loaded, importing this module raises.
+
+The functions fdtd_create_grid / fdtd_forward / fdtd_backward / fdtd_destroy / fdtd_last_error /
+fdtd_get_info / fdtd_version / fdtd_forward_host / fdtd_backward_host mirror the C entry points
+one to one; `Grid` is a small convenience wrapper used by the tests and bench.py.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+from typing import Optional, Sequence
+
+_HERE = Path(__file__).resolve().parent
+LIB_PATH = _HERE / "libfdtd_b200.so"
+
+FDTD_OK, FDTD_EINVAL, FDTD_ENOMEM, FDTD_ECUDA, FDTD_ESTATE = 0, -1, -2, -3, -4
+FDTD_PATH_AUTO, FDTD_PATH_GENERIC, FDTD_PATH_FUSED = 0, 1, 2
+
+
+class fdtd_grid_desc(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32), ("courant", C.c_float),
+                ("periodic", C.c_int32), ("pml_cells", C.c_int32),
+                ("pml_m", C.c_float), ("pml_sigma_scale", C.c_float), ("pml_kappa_max", C.c_float),
+                ("pml_alpha_max", C.c_float), ("pml_alpha_m", C.c_float), ("pml_eps_bg", C.c_float),
+                ("max_steps", C.c_int32), ("record", C.c_int32),
+                ("grad_lo", C.c_int32 * 3), ("grad_hi", C.c_int32 * 3),
+                ("path", C.c_int32), ("reserved", C.c_int32 * 7)]
+
+
+class fdtd_source(C.Structure):
+    _fields_ = [("component", C.c_int32), ("lo", C.c_int32 * 3), ("hi", C.c_int32 * 3),
+                ("profile", C.c_void_p), ("waveform", C.c_void_p)]
+
+
+class fdtd_detector(C.Structure):
+    _fields_ = [("component_mask", C.c_int32), ("lo", C.c_int32 * 3), ("hi", C.c_int32 * 3),
+                ("n_freq", C.c_int32), ("omega", C.POINTER(C.c_float)), ("phasor", C.c_void_p)]
+
+
+class fdtd_grid_info(C.Structure):
+    _fields_ = [("path", C.c_int32), ("tile_x", C.c_int32), ("tile_y", C.c_int32), ("tile_z", C.c_int32),
+                ("kernel_launches", C.c_int64), ("recorder_bytes", C.c_int64), ("scratch_bytes", C.c_int64),
+                ("record_floats_per_step", C.c_int64), ("reserved", C.c_int64 * 4)]
+
+
+FDTD_PROF_CLASSES = 12
+
+
+class fdtd_profile(C.Structure):
+    _fields_ = [("n_classes", C.c_int32), ("reserved", C.c_int32),
+                ("name", (C.c_char * 32) * FDTD_PROF_CLASSES),
+                ("launches", C.c_int64 * FDTD_PROF_CLASSES), ("total_ms", C.c_double * FDTD_PROF_CLASSES)]
+
+
+EXPORTS = ("fdtd_grad_rho", "fdtd_set_profiling", "fdtd_get_profile", "fdtd_create_grid", "fdtd_forward", "fdtd_backward", "fdtd_destroy", "fdtd_last_error",
+           "fdtd_get_info", "fdtd_version", "fdtd_forward_host", "fdtd_backward_host")
+
+
+def _load():
+    if not LIB_PATH.exists():
+        raise ImportError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_2412_12360_b200.build` "
+            "(there is no CPU fallback)")
+    L = C.CDLL(str(LIB_PATH))
+    vp, i32 = C.c_void_p, C.c_int32
+    L.fdtd_create_grid.restype = C.c_int
+    L.fdtd_create_grid.argtypes = [C.POINTER(fdtd_grid_desc), C.POINTER(vp)]
+    L.fdtd_forward.restype = C.c_int
+    L.fdtd_forward.argtypes = [vp, vp, vp, vp, C.POINTER(fdtd_source), i32, C.POINTER(fdtd_detector), i32, i32, vp]
+    L.fdtd_backward.restype = C.c_int
+    L.fdtd_backward.argtypes = [vp, vp, vp, vp, C.POINTER(fdtd_source), i32, C.POINTER(fdtd_detector), i32,
+                                C.POINTER(vp), vp, i32, vp, vp, vp]
+    L.fdtd_destroy.restype = C.c_int
+    L.fdtd_destroy.argtypes = [vp]
+    L.fdtd_last_error.restype = C.c_char_p
+    L.fdtd_last_error.argtypes = []
+    L.fdtd_get_info.restype = C.c_int
+    L.fdtd_get_info.argtypes = [vp, C.POINTER(fdtd_grid_info)]
+    L.fdtd_version.restype = C.c_char_p
+    L.fdtd_grad_rho.restype = C.c_int
+    L.fdtd_grad_rho.argtypes = [vp, vp, vp, C.c_float, C.POINTER(i32), C.POINTER(i32), vp, vp]
+    L.fdtd_set_profiling.restype = C.c_int
+    L.fdtd_set_profiling.argtypes = [vp, i32]
+    L.fdtd_get_profile.restype = C.c_int
+    L.fdtd_get_profile.argtypes = [vp, C.POINTER(fdtd_profile)]
+    L.fdtd_forward_host.restype = C.c_int
+    L.fdtd_forward_host.argtypes = L.fdtd_forward.argtypes
+    L.fdtd_backward_host.restype = C.c_int
+    L.fdtd_backward_host.argtypes = L.fdtd_backward.argtypes
+    return L
+
+
+_L = _load()
+
+
+class FdtdError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"fdtd error {code}: {msg}")
+        self.code = code
+
+
+def fdtd_last_error() -> str:
+    return _L.fdtd_last_error().decode()
+
+
+def fdtd_version() -> str:
+    return _L.fdtd_version().decode()
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise FdtdError(rc, fdtd_last_error())
+
+
+def fdtd_create_grid(desc: fdtd_grid_desc) -> C.c_void_p:
+    h = C.c_void_p()
+    _check(_L.fdtd_create_grid(C.byref(desc), C.byref(h)))
+    return h
+
+
+def fdtd_destroy(grid) -> None:
+    _check(_L.fdtd_destroy(grid))
+
+
+def fdtd_get_info(grid) -> fdtd_grid_info:
+    info = fdtd_grid_info()
+    _check(_L.fdtd_get_info(grid, C.byref(info)))
+    return info
+
+
+def fdtd_grad_rho(grid, dL_dinv_eps, inv_eps, delta_eps, lo, hi, dL_drho, stream) -> None:
+    lo_a, hi_a = (C.c_int32 * 3)(*lo), (C.c_int32 * 3)(*hi)
+    _check(_L.fdtd_grad_rho(grid, _ptr(dL_dinv_eps), _ptr(inv_eps), float(delta_eps), lo_a, hi_a, _ptr(dL_drho), stream))
+
+
+def fdtd_set_profiling(grid, enable: bool) -> None:
+    _check(_L.fdtd_set_profiling(grid, int(bool(enable))))
+
+
+def fdtd_get_profile(grid) -> dict:
+    """{kernel class: (launches, total_ms)} since profiling was enabled / last read."""
+    p = fdtd_profile()
+    _check(_L.fdtd_get_profile(grid, C.byref(p)))
+    return {bytes(p.name[c]).split(b"\0")[0].decode(): (int(p.launches[c]), float(p.total_ms[c]))
+            for c in range(p.n_classes) if p.launches[c]}
+
+
+def _ptr(t) -> Optional[int]:
+    """Device/host pointer of a torch tensor or numpy array (None passes through)."""
+    if t is None:
+        return None
+    if hasattr(t, "data_ptr"):
+        assert t.is_contiguous()
+        return t.data_ptr()
+    assert t.flags.c_contiguous
+    return t.ctypes.data
+
+
+def fdtd_forward(grid, fields, inv_eps, inv_mu, src, n_src, det, n_det, n_steps, stream) -> None:
+    _check(_L.fdtd_forward(grid, _ptr(fields), _ptr(inv_eps), _ptr(inv_mu), src, n_src, det, n_det, n_steps, stream))
+
+
+def fdtd_backward(grid, fields, inv_eps, inv_mu, src, n_src, det, n_det, dL_dphasor, dL_dfields, n_steps,
+                  dL_dinv_eps, dL_dfields0, stream) -> None:
+    _check(_L.fdtd_backward(grid, _ptr(fields), _ptr(inv_eps), _ptr(inv_mu), src, n_src, det, n_det,
+                            dL_dphasor, _ptr(dL_dfields), n_steps, _ptr(dL_dinv_eps), _ptr(dL_dfields0), stream))
+
+
+def fdtd_forward_host(grid, h_fields, h_inv_eps, h_inv_mu, src, n_src, det, n_det, n_steps, stream) -> None:
+    _check(_L.fdtd_forward_host(grid, _ptr(h_fields), _ptr(h_inv_eps), _ptr(h_inv_mu), src, n_src, det, n_det,
+                                n_steps, stream))
+
+
+def fdtd_backward_host(grid, h_fields, h_inv_eps, h_inv_mu, src, n_src, det, n_det, h_dL_dphasor, h_dL_dfields,
+                       n_steps, h_dL_dinv_eps, h_dL_dfields0, stream) -> None:
+    _check(_L.fdtd_backward_host(grid, _ptr(h_fields), _ptr(h_inv_eps), _ptr(h_inv_mu), src, n_src, det, n_det,
+                                 h_dL_dphasor, _ptr(h_dL_dfields), n_steps, _ptr(h_dL_dinv_eps),
+                                 _ptr(h_dL_dfields0), stream))
+
+
+# --------------------------------------------------------------------------------------------
+# convenience wrapper (marshalling only)
+# --------------------------------------------------------------------------------------------
+def make_desc(nx, ny, nz, courant, periodic=False, pml_cells=0, pml_m=0.0, pml_sigma_scale=0.0,
+              pml_kappa_max=0.0, pml_alpha_max=0.0, pml_alpha_m=0.0, pml_eps_bg=0.0, max_steps=0,
+              record=False, grad_lo=None, grad_hi=None, path=FDTD_PATH_AUTO) -> fdtd_grid_desc:
+    d = fdtd_grid_desc()
+    d.nx, d.ny, d.nz, d.courant = nx, ny, nz, courant
+    d.periodic, d.pml_cells = int(bool(periodic)), pml_cells
+    d.pml_m, d.pml_sigma_scale, d.pml_kappa_max = pml_m, pml_sigma_scale, pml_kappa_max
+    d.pml_alpha_max, d.pml_alpha_m, d.pml_eps_bg = pml_alpha_max, pml_alpha_m, pml_eps_bg
+    d.max_steps, d.record, d.path = max_steps, int(bool(record)), path
+    if grad_lo is not None:
+        d.grad_lo[:] = list(grad_lo)
+        d.grad_hi[:] = list(grad_hi)
+    return d
+
+
+class Grid:
+    """Owns one fdtd_grid handle; marshals workloads.Source / workloads.Detector style objects."""
+
+    def __init__(self, **kw):
+        import torch  # device memory + streams only
+        self.torch = torch
+        self.desc = make_desc(**kw)
+        self.shape = (self.desc.nz, self.desc.ny, self.desc.nx)
+        self.h = fdtd_create_grid(self.desc)
+        self._keep = []
+
+    def close(self):
+        if getattr(self, "h", None):
+            fdtd_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def info(self) -> fdtd_grid_info:
+        return fdtd_get_info(self.h)
+
+    # -- marshalling -----------------------------------------------------------------------------
+    def _dev(self, a):
+        torch = self.torch
+        if a is None:
+            return None
+        if isinstance(a, torch.Tensor):
+            return a.to(device="cuda", dtype=torch.float32).contiguous()
+        return torch.as_tensor(a, dtype=torch.float32).contiguous().cuda()
+
+    def marshal_sources(self, sources, host=False):
+        n = len(sources)
+        arr = (fdtd_source * max(n, 1))()
+        keep = []
+        for s, q in zip(arr, sources):
+            s.component = int(q.component)
+            s.lo[:] = list(q.lo)
+            s.hi[:] = list(q.hi)
+            if host:
+                import numpy as np
+                prof = None if q.profile is None else np.ascontiguousarray(q.profile, dtype=np.float32)
+                wav = np.ascontiguousarray(q.waveform, dtype=np.float32)
+            else:
+                prof, wav = self._dev(q.profile), self._dev(q.waveform)
+            keep += [prof, wav]
+            s.profile = _ptr(prof)
+            s.waveform = _ptr(wav)
+        return arr, n, keep
+
+    def marshal_detectors(self, detectors, phasors):
+        n = len(detectors)
+        arr = (fdtd_detector * max(n, 1))()
+        keep = []
+        for idx, (s, q) in enumerate(zip(arr, detectors)):
+            s.component_mask = int(q.component_mask)
+            s.lo[:] = list(q.lo)
+            s.hi[:] = list(q.hi)
+            om = (C.c_float * len(q.omega))(*[float(o) for o in q.omega])
+            keep.append(om)
+            s.n_freq = len(q.omega)
+            s.omega = C.cast(om, C.POINTER(C.c_float))
+            s.phasor = None if phasors is None else _ptr(phasors[idx])
+        return arr, n, keep
+
+    def stream(self):
+        return C.c_void_p(self.torch.cuda.current_stream().cuda_stream)
+
+    # -- device entry points ---------------------------------------------------------------------
+    def forward(self, fields, inv_eps, inv_mu=None, sources=(), detectors=(), n_steps=0, phasors=None):
+        """fields: cuda float32 [6,nz,ny,nx], updated in place.  Returns the phasor tensors."""
+        torch = self.torch
+        if phasors is None:
+            phasors = [torch.zeros(d.phasor_shape, dtype=torch.float32, device="cuda") for d in detectors]
+        sarr, ns, k1 = self.marshal_sources(sources)
+        darr, nd, k2 = self.marshal_detectors(detectors, phasors)
+        fdtd_forward(self.h, fields, inv_eps, inv_mu, sarr, ns, darr, nd, int(n_steps), self.stream())
+        self._keep = [k1, k2, sarr, darr]
+        return phasors
+
+    def backward(self, fields, inv_eps, inv_mu=None, sources=(), detectors=(), dL_dphasor=None,
+                 dL_dfields=None, n_steps=0, want_dL_dfields0=False, out=None):
+        torch = self.torch
+        sarr, ns, k1 = self.marshal_sources(sources)
+        darr, nd, k2 = self.marshal_detectors(detectors, None)
+        cot = None
+        if dL_dphasor is not None:
+            cot = (C.c_void_p * max(nd, 1))()
+            for i, G in enumerate(dL_dphasor):
+                cot[i] = _ptr(G)
+        g = out if out is not None else torch.empty(self.shape, dtype=torch.float32, device="cuda")
+        lam0 = torch.empty((6,) + self.shape, dtype=torch.float32, device="cuda") if want_dL_dfields0 else None
+        fdtd_backward(self.h, fields, inv_eps, inv_mu, sarr, ns, darr, nd, cot, dL_dfields, int(n_steps),
+                      g, lam0, self.stream())
+        self._keep = [k1, k2, sarr, darr, cot, dL_dphasor]
+        return g, lam0

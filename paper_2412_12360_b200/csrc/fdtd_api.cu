@@ -1,0 +1,750 @@
+// fdtd_api.cu -- the C ABI of include/fdtd.h: validation, the grid object, host orchestration.
+// Every step of the path runs in the kernels of kernels_generic.cu / kernels_fused_*.cu; this
+// file only owns memory, builds tables and enqueues launches (through CUDA graphs).
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+#include <new>
+
+#include "fdtd_internal.h"
+#include "fdtd_grid.h"
+
+using namespace fdtd;
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const std::string &msg)
+{
+    g_err = msg;
+    return code;
+}
+
+}  // namespace
+int fdtd_fail(int code, const std::string &msg) { return fail(code, msg); }
+namespace {
+
+int cuda_fail(cudaError_t e, const char *what)
+{
+    // clear the sticky-less error state so later calls report their own errors
+    (void)cudaGetLastError();
+    return fail(e == cudaErrorMemoryAllocation ? FDTD_ENOMEM : FDTD_ECUDA,
+                std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+#define CK(call)                                                       \
+    do {                                                               \
+        cudaError_t e__ = (call);                                      \
+        if (e__ != cudaSuccess) return cuda_fail(e__, #call);          \
+    } while (0)
+
+int dim_of(const Dims &G, int a) { return a == 0 ? G.nx : (a == 1 ? G.ny : G.nz); }
+
+// CPML tables (PAPER.md L72 -> ref. 7; constants: reading R8), fp64 on the host.
+//   depth rho(x) = max(0, d - x, x - (N - d)), r = rho/d
+//   sigma = sigma_max r^m, kappa = 1 + (kappa_max - 1) r^m, alpha = alpha_max (1 - r)^m_alpha
+//   b = exp(-(sigma/kappa + alpha) S), a = sigma (b - 1) / (kappa (sigma + kappa alpha)), ik = 1/kappa
+void make_table(int n, int d, int half, double S, double m, double smax, double kmax, double amax,
+                double am, float *b, float *a, float *ik)
+{
+    for (int p = 0; p < n; ++p) {
+        const double x = p + (half ? 0.5 : 0.0);
+        double rho = 0.0;
+        if (d > 0) rho = std::max(0.0, std::max((double)d - x, x - (double)(n - d)));
+        if (rho <= 0.0) { b[p] = 1.f; a[p] = 0.f; ik[p] = 1.f; continue; }
+        const double r = rho / d;
+        const double rm = std::pow(r, m);
+        const double sig = smax * rm, kap = 1.0 + (kmax - 1.0) * rm, alp = amax * std::pow(1.0 - r, am);
+        const double bb = std::exp(-(sig / kap + alp) * S);
+        const double aa = sig > 0.0 ? sig * (bb - 1.0) / (kap * (sig + kap * alp)) : 0.0;
+        b[p] = (float)bb; a[p] = (float)aa; ik[p] = (float)(1.0 / kap);
+    }
+}
+
+void make_rec_layout(const Dims &G, RecLayout &R)
+{
+    std::memset(&R, 0, sizeof(R));
+    if (G.d == 0) return;
+    long long off = 0;
+    for (int a = 0; a < 3; ++a) {
+        int u = (a + 1) % 3, v = (a + 2) % 3;
+        if (u > v) std::swap(u, v);
+        R.fast[a] = u; R.slow[a] = v;
+        R.cells[a] = (long long)(G.hi[u] - G.lo[u]) * (G.hi[v] - G.lo[v]);
+        const long long seg = (R.cells[a] + 3) / 4 * 4;
+        for (int side = 0; side < 2; ++side)
+            for (int which = 0; which < 2; ++which) { R.off[a][side][which] = off; off += seg; }
+    }
+    R.stride = (off + 31) / 32 * 32;
+}
+
+bool box_ok(const Dims &G, const int32_t lo[3], const int32_t hi[3])
+{
+    for (int a = 0; a < 3; ++a)
+        if (lo[a] < 0 || hi[a] > dim_of(G, a) || lo[a] >= hi[a]) return false;
+    return true;
+}
+
+int popcount6(int m) { int n = 0; for (int c = 0; c < 6; ++c) n += (m >> c) & 1; return n; }
+
+}  // namespace
+
+// ================================================================================================
+// grid lifetime
+// ================================================================================================
+int fdtd_grid::alloc(void **p, size_t bytes, bool recorder)
+{
+    *p = nullptr;
+    if (bytes == 0) return FDTD_OK;
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e != cudaSuccess) {
+        (void)cudaGetLastError();
+        char buf[160];
+        std::snprintf(buf, sizeof buf, "cudaMalloc(%zu bytes) failed: %s", bytes, cudaGetErrorString(e));
+        return fail(FDTD_ENOMEM, buf);
+    }
+    owned.push_back(*p);
+    if (recorder) recorder_bytes += (long long)bytes; else scratch_bytes += (long long)bytes;
+    return FDTD_OK;
+}
+
+int fdtd_grid::alloc_psi(PsiSet &s)
+{
+    for (int c = 0; c < 3; ++c)
+        for (int q = 0; q < 2; ++q) {
+            const size_t bytes = (size_t)psi_elems(G, psi_axis(c, q)) * sizeof(float);
+            int rc = alloc((void **)&s.p[c][q], bytes);
+            if (rc) return rc;
+        }
+    return FDTD_OK;
+}
+
+int fdtd_grid::zero_psi(const PsiSet &s, cudaStream_t st)
+{
+    for (int c = 0; c < 3; ++c)
+        for (int q = 0; q < 2; ++q) {
+            const size_t bytes = (size_t)psi_elems(G, psi_axis(c, q)) * sizeof(float);
+            if (bytes) CK(cudaMemsetAsync(s.p[c][q], 0, bytes, st));
+        }
+    return FDTD_OK;
+}
+
+void fdtd_grid::drop_graphs()
+{
+    for (GraphCache *gc : { &fwd_graph, &bwd_graph }) {
+        if (gc->done) { cudaEventSynchronize(gc->done); }
+        if (gc->exec_main) cudaGraphExecDestroy(gc->exec_main);
+        if (gc->exec_tail) cudaGraphExecDestroy(gc->exec_tail);
+        gc->exec_main = gc->exec_tail = nullptr;
+        gc->key.clear();
+    }
+}
+
+extern "C" int fdtd_create_grid(const fdtd_grid_desc *desc, fdtd_grid **out)
+{
+    if (out) *out = nullptr;
+    if (!desc || !out) return fail(FDTD_EINVAL, "fdtd_create_grid: NULL argument");
+    if (desc->nx < 1 || desc->ny < 1 || desc->nz < 1) return fail(FDTD_EINVAL, "grid dims must be >= 1");
+    if ((long long)desc->nx * desc->ny * desc->nz > (1LL << 40)) return fail(FDTD_EINVAL, "grid too large");
+    if (!(desc->courant > 0.f) || !(desc->courant < 0.57735027f))
+        return fail(FDTD_EINVAL, "courant must satisfy 0 < S < 1/sqrt(3)");
+    if (desc->pml_cells < 0) return fail(FDTD_EINVAL, "pml_cells must be >= 0");
+    if (desc->periodic && desc->pml_cells != 0) return fail(FDTD_EINVAL, "a periodic grid cannot have a PML");
+    const int mn = std::min(desc->nx, std::min(desc->ny, desc->nz));
+    if (desc->pml_cells > 0 && 2 * desc->pml_cells + 2 > mn)
+        return fail(FDTD_EINVAL, "need 2*pml_cells + 2 <= min(nx,ny,nz)");
+    if (desc->max_steps < 0) return fail(FDTD_EINVAL, "max_steps must be >= 0");
+    if (desc->record != 0 && desc->record != 1) return fail(FDTD_EINVAL, "record must be 0 or 1");
+    if (desc->path < 0 || desc->path > 2) return fail(FDTD_EINVAL, "unknown path");
+    for (int q = 0; q < 7; ++q) if (desc->reserved[q]) return fail(FDTD_EINVAL, "reserved fields must be zero");
+    if (desc->pml_m < 0 || desc->pml_sigma_scale < 0 || desc->pml_kappa_max < 0 || desc->pml_alpha_max < 0 ||
+        desc->pml_alpha_m < 0 || desc->pml_eps_bg < 0)
+        return fail(FDTD_EINVAL, "CPML constants must be >= 0");
+    if (desc->pml_kappa_max != 0.f && desc->pml_kappa_max < 1.f) return fail(FDTD_EINVAL, "pml_kappa_max must be >= 1");
+
+    fdtd_grid *g = new (std::nothrow) fdtd_grid();
+    if (!g) return fail(FDTD_ENOMEM, "host allocation failed");
+    g->desc = *desc;
+    Dims &G = g->G;
+    G.nx = desc->nx; G.ny = desc->ny; G.nz = desc->nz;
+    G.d = desc->pml_cells;
+    G.periodic = desc->periodic ? 1 : 0;
+    G.S = desc->courant;
+    G.nc = (long long)G.nx * G.ny * G.nz;
+    const int dp4 = (G.d + 3) / 4 * 4;
+    G.dpx = (G.nx % 4 == 0 && G.nx >= 2 * dp4) ? dp4 : G.d;
+    for (int a = 0; a < 3; ++a) { G.lo[a] = G.d; G.hi[a] = dim_of(G, a) - G.d; }
+    bool all_zero = true;
+    for (int a = 0; a < 3; ++a) if (desc->grad_lo[a] || desc->grad_hi[a]) all_zero = false;
+    for (int a = 0; a < 3; ++a) {
+        if (all_zero) { G.glo[a] = G.lo[a]; G.ghi[a] = G.hi[a]; }
+        else {
+            if (desc->grad_lo[a] < 0 || desc->grad_hi[a] > dim_of(G, a) || desc->grad_lo[a] >= desc->grad_hi[a]) {
+                delete g;
+                return fail(FDTD_EINVAL, "grad box outside the grid or empty");
+            }
+            G.glo[a] = std::max(desc->grad_lo[a], G.lo[a]);
+            G.ghi[a] = std::max(G.glo[a], std::min(desc->grad_hi[a], G.hi[a]));
+        }
+    }
+    make_rec_layout(G, g->R);
+
+    int rc = FDTD_OK;
+    auto bail = [&](int code) { std::string keep = g_err; fdtd_destroy(g); g_err = keep; return code; };
+
+    // CPML tables
+    {
+        const double m = desc->pml_m > 0 ? desc->pml_m : 3.0;
+        const double ss = desc->pml_sigma_scale > 0 ? desc->pml_sigma_scale : 0.8 * (m + 1.0);
+        const double km = desc->pml_kappa_max > 0 ? desc->pml_kappa_max : 1.0;
+        const double am = desc->pml_alpha_m > 0 ? desc->pml_alpha_m : 1.0;
+        const double eb = desc->pml_eps_bg > 0 ? desc->pml_eps_bg : 1.0;
+        const double smax = ss / std::sqrt(eb);
+        const int tot = 6 * (G.nx + G.ny + G.nz);
+        std::vector<float> h(tot);
+        float *dev = nullptr;
+        if ((rc = g->alloc((void **)&dev, tot * sizeof(float)))) return bail(rc);
+        int off = 0;
+        for (int fam = 0; fam < 2; ++fam)
+            for (int a = 0; a < 3; ++a) {
+                const int n = dim_of(G, a);
+                make_table(n, G.d, fam, (double)G.S, m, smax, km, (double)desc->pml_alpha_max, am,
+                           &h[off], &h[off + n], &h[off + 2 * n]);
+                g->T.b[fam][a] = dev + off; g->T.a[fam][a] = dev + off + n; g->T.ik[fam][a] = dev + off + 2 * n;
+                off += 3 * n;
+            }
+        cudaError_t e = cudaMemcpy(dev, h.data(), tot * sizeof(float), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) return bail(cuda_fail(e, "upload CPML tables"));
+        g->h_tables = h;
+    }
+    if ((rc = g->alloc((void **)&g->d_step, 64))) return bail(rc);
+    if ((rc = g->alloc_psi(g->psiE[0])) || (rc = g->alloc_psi(g->psiH[0]))) return bail(rc);
+    if (desc->record && G.d > 0 && desc->max_steps > 0) {
+        const size_t bytes = (size_t)g->R.stride * sizeof(float) * (size_t)desc->max_steps;
+        if ((rc = g->alloc((void **)&g->rec, bytes, true))) return bail(rc);
+    }
+    {
+        cudaError_t e = cudaStreamCreateWithFlags(&g->cap_stream, cudaStreamNonBlocking);
+        if (e != cudaSuccess) return bail(cuda_fail(e, "cudaStreamCreate"));
+        e = cudaEventCreateWithFlags(&g->fwd_graph.done, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&g->bwd_graph.done, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&g->table_done, cudaEventDisableTiming);
+        if (e != cudaSuccess) return bail(cuda_fail(e, "cudaEventCreate"));
+    }
+    g->path = FDTD_PATH_GENERIC;
+    rc = fused_setup(g);          // may switch g->path to FDTD_PATH_FUSED (kernels_fused_*.cu)
+    if (rc) return bail(rc);
+    if (desc->path == FDTD_PATH_FUSED && g->path != FDTD_PATH_FUSED)
+        return bail(fail(FDTD_EINVAL, "FDTD_PATH_FUSED requested but the grid does not qualify: " + g->fused_why_not));
+    *out = g;
+    return FDTD_OK;
+}
+
+extern "C" int fdtd_destroy(fdtd_grid *g)
+{
+    if (!g) return FDTD_OK;
+    cudaDeviceSynchronize();
+    g->drop_graphs();
+    fused_teardown(g);
+    for (void *p : g->owned) cudaFree(p);
+    if (g->h_cs) cudaFreeHost(g->h_cs);
+    if (g->cap_stream) cudaStreamDestroy(g->cap_stream);
+    if (g->fwd_graph.done) cudaEventDestroy(g->fwd_graph.done);
+    if (g->bwd_graph.done) cudaEventDestroy(g->bwd_graph.done);
+    if (g->table_done) cudaEventDestroy(g->table_done);
+    for (auto &sp : g->prof_spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
+    for (cudaEvent_t e : g->prof_pool) cudaEventDestroy(e);
+    (void)cudaGetLastError();
+    delete g;
+    return FDTD_OK;
+}
+
+extern "C" const char *fdtd_last_error(void) { return g_err.c_str(); }
+extern "C" const char *fdtd_version(void) { return "fdtd-b200 0.1 sm_100a"; }
+
+cudaEvent_t fdtd_grid::prof_begin(cudaStream_t st)
+{
+    if (!profiling || prof_capturing) return nullptr;
+    cudaEvent_t a = nullptr;
+    if (!prof_pool.empty()) { a = prof_pool.back(); prof_pool.pop_back(); }
+    else if (cudaEventCreate(&a) != cudaSuccess) return nullptr;
+    cudaEventRecord(a, st);
+    return a;
+}
+
+void fdtd_grid::prof_end(int cls, cudaEvent_t a, cudaStream_t st)
+{
+    cudaEvent_t b = nullptr;
+    if (!prof_pool.empty()) { b = prof_pool.back(); prof_pool.pop_back(); }
+    else if (cudaEventCreate(&b) != cudaSuccess) { prof_pool.push_back(a); return; }
+    cudaEventRecord(b, st);
+    prof_spans.push_back({ cls, a, b });
+}
+
+extern "C" int fdtd_set_profiling(fdtd_grid *g, int32_t enable)
+{
+    if (!g) return fail(FDTD_EINVAL, "fdtd_set_profiling: NULL grid");
+    g->profiling = enable != 0;
+    return FDTD_OK;
+}
+
+extern "C" int fdtd_get_profile(fdtd_grid *g, fdtd_profile *out)
+{
+    if (!g || !out) return fail(FDTD_EINVAL, "fdtd_get_profile: NULL argument");
+    static const char *names[fdtd_grid::PC_COUNT] = { "update_E", "update_H", "adjoint_H", "inverse_H", "inverse_E_grad",
+        "adjoint_E", "fused_forward_step", "fused_backward_step", "record_faces", "inject_faces", "source_detector", "other" };
+    for (auto &sp : g->prof_spans) {
+        cudaError_t e = cudaEventSynchronize(sp.b);
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, sp.a, sp.b);
+        if (e != cudaSuccess) return cuda_fail(e, "fdtd_get_profile");
+        g->prof_ms[sp.cls] += ms;
+        g->prof_launches[sp.cls] += 1;
+        g->prof_pool.push_back(sp.a);
+        g->prof_pool.push_back(sp.b);
+    }
+    g->prof_spans.clear();
+    std::memset(out, 0, sizeof(*out));
+    out->n_classes = fdtd_grid::PC_COUNT;
+    for (int c = 0; c < fdtd_grid::PC_COUNT; ++c) {
+        std::snprintf(out->name[c], sizeof out->name[c], "%s", names[c]);
+        out->launches[c] = g->prof_launches[c];
+        out->total_ms[c] = g->prof_ms[c];
+        g->prof_launches[c] = 0;
+        g->prof_ms[c] = 0.0;
+    }
+    return FDTD_OK;
+}
+
+extern "C" int fdtd_get_info(const fdtd_grid *g, fdtd_grid_info *info)
+{
+    if (!g || !info) return fail(FDTD_EINVAL, "fdtd_get_info: NULL argument");
+    std::memset(info, 0, sizeof(*info));
+    info->path = g->path;
+    info->tile_x = g->tile_x; info->tile_y = g->tile_y; info->tile_z = g->tile_z;
+    info->kernel_launches = g->kernel_launches;
+    info->recorder_bytes = g->recorder_bytes;
+    info->scratch_bytes = g->scratch_bytes;
+    info->record_floats_per_step = g->R.stride;
+    return FDTD_OK;
+}
+
+// ================================================================================================
+// argument checking and descriptor translation
+// ================================================================================================
+namespace {
+
+int check_common(fdtd_grid *g, const float *fields, const float *inv_eps, const fdtd_source *src, int n_src,
+                 const fdtd_detector *det, int n_det, int n_steps, const char *who)
+{
+    if (!g) return fail(FDTD_EINVAL, std::string(who) + ": NULL grid");
+    if (!fields || !inv_eps) return fail(FDTD_EINVAL, std::string(who) + ": fields and inv_eps are required");
+    if (n_steps < 0 || n_steps > g->desc.max_steps) return fail(FDTD_EINVAL, std::string(who) + ": need 0 <= n_steps <= max_steps");
+    if (n_src < 0 || n_det < 0 || (n_src && !src) || (n_det && !det))
+        return fail(FDTD_EINVAL, std::string(who) + ": bad source/detector array");
+    for (int s = 0; s < n_src; ++s) {
+        if (src[s].component < 0 || src[s].component > 5) return fail(FDTD_EINVAL, "source component must be 0..5");
+        if (!box_ok(g->G, src[s].lo, src[s].hi)) return fail(FDTD_EINVAL, "source box outside the grid or empty");
+        if (!src[s].waveform) return fail(FDTD_EINVAL, "source waveform is NULL");
+    }
+    for (int s = 0; s < n_det; ++s) {
+        if (det[s].component_mask <= 0 || det[s].component_mask > 63) return fail(FDTD_EINVAL, "detector component_mask must be 1..63");
+        if (!box_ok(g->G, det[s].lo, det[s].hi)) return fail(FDTD_EINVAL, "detector box outside the grid or empty");
+        if (det[s].n_freq < 1 || !det[s].omega) return fail(FDTD_EINVAL, "detector needs n_freq >= 1 and omega");
+    }
+    return FDTD_OK;
+}
+
+void translate(const fdtd_source *src, int n_src, std::vector<SourceDev> &out)
+{
+    out.resize(n_src);
+    for (int s = 0; s < n_src; ++s) {
+        out[s].comp = src[s].component;
+        for (int a = 0; a < 3; ++a) { out[s].lo[a] = src[s].lo[a]; out[s].hi[a] = src[s].hi[a]; }
+        out[s].profile = src[s].profile;
+        out[s].waveform = src[s].waveform;
+    }
+}
+
+int translate(const fdtd_detector *det, int n_det, std::vector<DetectorDev> &out)
+{
+    out.resize(n_det);
+    int tot = 0;
+    for (int s = 0; s < n_det; ++s) {
+        out[s].mask = det[s].component_mask;
+        out[s].ncomp = popcount6(det[s].component_mask);
+        for (int a = 0; a < 3; ++a) { out[s].lo[a] = det[s].lo[a]; out[s].hi[a] = det[s].hi[a]; }
+        out[s].n_freq = det[s].n_freq;
+        out[s].cs_off = tot;
+        out[s].phasor = det[s].phasor;
+        tot += det[s].n_freq;
+    }
+    return tot;
+}
+
+// (cos, sin) of omega_f*(n+1) for n < n_steps, fp64 on the host, stored fp32 (reading R13)
+int upload_cs_table(fdtd_grid *g, const fdtd_detector *det, int n_det, int total_freq, int n_steps, cudaStream_t st)
+{
+    if (total_freq == 0 || n_steps == 0) return FDTD_OK;
+    const size_t need = (size_t)n_steps * total_freq * 2;
+    if (need > g->cs_cap) {
+        // grow (device + pinned host); previous copies have to be finished first
+        CK(cudaEventSynchronize(g->table_done));
+        if (g->h_cs) { cudaFreeHost(g->h_cs); g->h_cs = nullptr; }
+        const size_t cap = (size_t)std::max(n_steps, g->desc.max_steps) * total_freq * 2;
+        CK(cudaMallocHost((void **)&g->h_cs, cap * sizeof(float)));
+        int rc = g->alloc((void **)&g->d_cs, cap * sizeof(float));
+        if (rc) return rc;
+        g->cs_cap = cap;
+    }
+    CK(cudaEventSynchronize(g->table_done));
+    int f0 = 0;
+    for (int s = 0; s < n_det; ++s) {
+        for (int q = 0; q < det[s].n_freq; ++q) {
+            const double om = (double)det[s].omega[q];
+            for (int n = 0; n < n_steps; ++n) {
+                const double phi = om * (double)(n + 1);
+                g->h_cs[((size_t)n * total_freq + f0 + q) * 2] = (float)std::cos(phi);
+                g->h_cs[((size_t)n * total_freq + f0 + q) * 2 + 1] = (float)std::sin(phi);
+            }
+        }
+        f0 += det[s].n_freq;
+    }
+    CK(cudaMemcpyAsync(g->d_cs, g->h_cs, need * sizeof(float), cudaMemcpyHostToDevice, st));
+    CK(cudaEventRecord(g->table_done, st));
+    return FDTD_OK;
+}
+
+// Replays a captured per-step sequence: `unroll` steps per graph launch plus single-step launches for
+// the remainder.  `enqueue(stream)` must enqueue exactly one step (reading n from *d_step).
+template <class F>
+int run_steps(fdtd_grid *g, fdtd_grid::GraphCache &gc, const std::string &key, int n_steps, int launches_per_step,
+              cudaStream_t st, F enqueue)
+{
+    if (n_steps == 0) return FDTD_OK;
+    if (g->profiling) {
+        for (int n = 0; n < n_steps; ++n) enqueue(st);
+        g->kernel_launches += (long long)n_steps * launches_per_step;
+        return FDTD_OK;
+    }
+    const int unroll = g->graph_unroll;
+    if (gc.key != key || !gc.exec_tail) {
+        if (gc.key.size()) CK(cudaEventSynchronize(gc.done));
+        if (gc.exec_main) { cudaGraphExecDestroy(gc.exec_main); gc.exec_main = nullptr; }
+        if (gc.exec_tail) { cudaGraphExecDestroy(gc.exec_tail); gc.exec_tail = nullptr; }
+        gc.key.clear();
+        for (int which = 0; which < 2; ++which) {
+            const int reps = which ? 1 : unroll;
+            cudaGraph_t graph = nullptr;
+            CK(cudaStreamBeginCapture(g->cap_stream, cudaStreamCaptureModeThreadLocal));
+            g->prof_capturing = true;
+            for (int r = 0; r < reps; ++r) enqueue(g->cap_stream);
+            g->prof_capturing = false;
+            cudaError_t e = cudaStreamEndCapture(g->cap_stream, &graph);
+            if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture");
+            cudaGraphExec_t exec = nullptr;
+            e = cudaGraphInstantiate(&exec, graph, 0);
+            cudaGraphDestroy(graph);
+            if (e != cudaSuccess) return cuda_fail(e, "cudaGraphInstantiate");
+            (which ? gc.exec_tail : gc.exec_main) = exec;
+        }
+        gc.key = key;
+    }
+    int left = n_steps;
+    while (left >= unroll) { CK(cudaGraphLaunch(gc.exec_main, st)); left -= unroll; }
+    while (left > 0) { CK(cudaGraphLaunch(gc.exec_tail, st)); --left; }
+    CK(cudaEventRecord(gc.done, st));
+    g->kernel_launches += (long long)n_steps * launches_per_step;
+    return FDTD_OK;
+}
+
+std::string make_key(const char *tag, const void *a, const void *b, const void *c, const void *d, const void *e,
+                     const std::vector<SourceDev> &S, const std::vector<DetectorDev> &D, int extra)
+{
+    std::string k(tag);
+    auto add = [&](const void *p, size_t n) { k.append((const char *)p, n); };
+    add(&a, sizeof a); add(&b, sizeof b); add(&c, sizeof c); add(&d, sizeof d); add(&e, sizeof e);
+    add(&extra, sizeof extra);
+    if (!S.empty()) add(S.data(), S.size() * sizeof(SourceDev));
+    if (!D.empty()) add(D.data(), D.size() * sizeof(DetectorDev));
+    return k;
+}
+
+}  // namespace
+
+// ================================================================================================
+// forward
+// ================================================================================================
+extern "C" int fdtd_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
+                            const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
+                            int32_t n_steps, void *cuda_stream)
+{
+    int rc = check_common(g, fields, inv_eps, src, n_src, det, n_det, n_steps, "fdtd_forward");
+    if (rc) return rc;
+    for (int s = 0; s < n_det; ++s)
+        if (!det[s].phasor) return fail(FDTD_EINVAL, "fdtd_forward: detector phasor is NULL");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const Dims &G = g->G;
+    std::vector<SourceDev> S;
+    std::vector<DetectorDev> D;
+    translate(src, n_src, S);
+    const int total_freq = translate(det, n_det, D);
+    const bool recording = g->desc.record && G.d > 0;
+    g->recorded_steps = -1;
+    if ((rc = upload_cs_table(g, det, n_det, total_freq, n_steps, st))) return rc;
+    CK(cudaMemsetAsync(g->d_step, 0, sizeof(int), st));
+
+    if (g->path == FDTD_PATH_FUSED) {
+        rc = fused_forward(g, fields, inv_eps, inv_mu, S, D, total_freq, n_steps, recording, st);
+        if (rc) return rc;
+    } else {
+        if ((rc = g->zero_psi(g->psiE[0], st)) || (rc = g->zero_psi(g->psiH[0], st))) return rc;
+        const int launches = 3 + n_src + n_det + (recording ? 1 : 0);
+        const std::string key = make_key("gf", fields, inv_eps, inv_mu, g->rec, nullptr, S, D, recording);
+        rc = run_steps(g, g->fwd_graph, key, n_steps, launches, st, [&](cudaStream_t cs) {
+            { ProfScope p(g, fdtd_grid::PC_UPDATE_E, cs); launch_update_E(G, g->T, fields, inv_eps, g->psiE[0], cs); }
+            { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
+              for (const SourceDev &s : S) if (s.comp < 3) launch_add_source(G, fields, s, g->d_step, 1.f, cs); }
+            if (recording) { ProfScope p(g, fdtd_grid::PC_RECORD, cs); launch_record(G, g->R, fields, fields, g->rec, g->d_step, cs); }
+            { ProfScope p(g, fdtd_grid::PC_UPDATE_H, cs); launch_update_H(G, g->T, fields, inv_mu, g->psiH[0], cs); }
+            { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
+              for (const SourceDev &s : S) if (s.comp >= 3) launch_add_source(G, fields, s, g->d_step, 1.f, cs);
+              for (const DetectorDev &dt : D) launch_detector(G, fields, dt, g->d_cs, total_freq, g->d_step, cs); }
+            { ProfScope p(g, fdtd_grid::PC_OTHER, cs); launch_advance(g->d_step, 1, cs); }
+        });
+        if (rc) return rc;
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "fdtd_forward launch");
+    if (recording) g->recorded_steps = n_steps;
+    return FDTD_OK;
+}
+
+// ================================================================================================
+// backward
+// ================================================================================================
+int fdtd_grid::ensure_backward_buffers()
+{
+    if (lam) return FDTD_OK;
+    int rc;
+    if ((rc = alloc((void **)&lam, (size_t)G.nc * 6 * sizeof(float)))) return rc;
+    for (int q = 0; q < 2; ++q)
+        if ((rc = alloc_psi(lpsiE[q])) || (rc = alloc_psi(lpsiH[q]))) return rc;
+    return FDTD_OK;
+}
+
+extern "C" int fdtd_backward(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
+                             const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
+                             const float *const *dL_dphasor, const float *dL_dfields,
+                             int32_t n_steps, float *dL_dinv_eps, float *dL_dfields0, void *cuda_stream)
+{
+    int rc = check_common(g, fields, inv_eps, src, n_src, det, n_det, n_steps, "fdtd_backward");
+    if (rc) return rc;
+    if (!dL_dinv_eps) return fail(FDTD_EINVAL, "fdtd_backward: dL_dinv_eps is required");
+    const Dims &G = g->G;
+    if (G.d > 0 && (!g->desc.record || g->recorded_steps != n_steps))
+        return fail(FDTD_ESTATE, "fdtd_backward: no matching recorded forward (need record=1 and the same n_steps)");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    std::vector<SourceDev> S;
+    std::vector<DetectorDev> D;
+    translate(src, n_src, S);
+    const int total_freq = translate(det, n_det, D);
+    for (int s = 0; s < n_det; ++s)
+        D[s].phasor = const_cast<float *>(dL_dphasor ? dL_dphasor[s] : nullptr);
+    if ((rc = g->ensure_backward_buffers())) return rc;
+    if ((rc = upload_cs_table(g, det, n_det, total_freq, n_steps, st))) return rc;
+
+    // B0: seed cotangents
+    const size_t vol = (size_t)G.nc * sizeof(float);
+    if (dL_dfields) CK(cudaMemcpyAsync(g->lam, dL_dfields, 6 * vol, cudaMemcpyDeviceToDevice, st));
+    else            CK(cudaMemsetAsync(g->lam, 0, 6 * vol, st));
+    for (int q = 0; q < 2; ++q)
+        if ((rc = g->zero_psi(g->lpsiE[q], st)) || (rc = g->zero_psi(g->lpsiH[q], st))) return rc;
+    CK(cudaMemsetAsync(dL_dinv_eps, 0, vol, st));
+    CK(cudaMemsetAsync(g->d_step, 0, sizeof(int), st));
+    if (n_steps > 0) launch_advance(g->d_step, n_steps - 1, st);
+
+    if (g->path == FDTD_PATH_FUSED) {
+        rc = fused_backward(g, fields, inv_eps, inv_mu, S, D, total_freq, n_steps, dL_dinv_eps, st);
+        if (rc) return rc;
+    } else {
+        int n_adj = 0;
+        for (const DetectorDev &dt : D) if (dt.phasor) ++n_adj;
+        const int launches = 5 + n_adj + n_src + (G.d > 0 ? 1 : 0);
+        const std::string key = make_key("gb", fields, inv_eps, inv_mu, g->rec, dL_dinv_eps, S, D, 0);
+        rc = run_steps(g, g->bwd_graph, key, n_steps, launches, st, [&](cudaStream_t cs) {
+            { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
+              for (const DetectorDev &dt : D) if (dt.phasor) launch_detector_adjoint(G, g->lam, dt, g->d_cs, total_freq, g->d_step, cs); }
+            { ProfScope p(g, fdtd_grid::PC_ADJ_H, cs); launch_adj_H(G, g->T, g->lam, inv_mu, g->lpsiH[0], g->lpsiH[1], g->d_step, cs); }
+            { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
+              for (const SourceDev &s : S) if (s.comp >= 3) launch_add_source(G, fields, s, g->d_step, -1.f, cs); }
+            if (G.d > 0) { ProfScope p(g, fdtd_grid::PC_INJECT, cs); launch_inject(G, g->R, fields, g->rec, g->d_step, cs); }
+            { ProfScope p(g, fdtd_grid::PC_INV_H, cs); launch_inv_H(G, fields, inv_mu, cs); }
+            { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
+              for (const SourceDev &s : S) if (s.comp < 3) launch_add_source(G, fields, s, g->d_step, -1.f, cs); }
+            { ProfScope p(g, fdtd_grid::PC_INV_E_GRAD, cs); launch_inv_E_grad(G, fields, inv_eps, g->lam, dL_dinv_eps, cs); }
+            { ProfScope p(g, fdtd_grid::PC_ADJ_E, cs); launch_adj_E(G, g->T, g->lam, inv_eps, g->lpsiE[0], g->lpsiE[1], g->d_step, cs); }
+            { ProfScope p(g, fdtd_grid::PC_OTHER, cs); launch_advance(g->d_step, -1, cs); }
+        });
+        if (rc) return rc;
+    }
+    if (dL_dfields0) CK(cudaMemcpyAsync(dL_dfields0, g->lam_result ? g->lam_result : g->lam, 6 * vol, cudaMemcpyDeviceToDevice, st));
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "fdtd_backward launch");
+    return FDTD_OK;
+}
+
+extern "C" int fdtd_grad_rho(fdtd_grid *g, const float *dL_dinv_eps, const float *inv_eps, float delta_eps,
+                             const int32_t lo[3], const int32_t hi[3], float *dL_drho, void *cuda_stream)
+{
+    if (!g || !dL_dinv_eps || !inv_eps || !lo || !hi || !dL_drho) return fail(FDTD_EINVAL, "fdtd_grad_rho: NULL argument");
+    if (!box_ok(g->G, lo, hi)) return fail(FDTD_EINVAL, "fdtd_grad_rho: box outside the grid or empty");
+    launch_grad_rho(g->G, dL_dinv_eps, inv_eps, delta_eps, lo, hi, dL_drho, (cudaStream_t)cuda_stream);
+    g->kernel_launches += 1;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "fdtd_grad_rho launch");
+    return FDTD_OK;
+}
+
+// ================================================================================================
+// host-buffer entry points (end-to-end measurement): stage through grid-owned device buffers
+// ================================================================================================
+namespace {
+
+struct HostStage {
+    std::vector<fdtd_source> src;
+    std::vector<fdtd_detector> det;
+    std::vector<size_t> phasor_bytes;
+};
+
+size_t box_cells(const int32_t lo[3], const int32_t hi[3])
+{
+    return (size_t)(hi[0] - lo[0]) * (hi[1] - lo[1]) * (hi[2] - lo[2]);
+}
+
+}  // namespace
+
+int fdtd_grid::ensure_host_buffers(bool need_mu)
+{
+    int rc;
+    const size_t vol = (size_t)G.nc * sizeof(float);
+    if (!hb_fields && (rc = alloc((void **)&hb_fields, 6 * vol))) return rc;
+    if (!hb_ie && (rc = alloc((void **)&hb_ie, vol))) return rc;
+    if (need_mu && !hb_im && (rc = alloc((void **)&hb_im, vol))) return rc;
+    return FDTD_OK;
+}
+
+// copies the descriptor payloads (profiles, waveforms, phasors) to device scratch; grows on demand
+static int stage_descriptors(fdtd_grid *g, const fdtd_source *h_src, int n_src, const fdtd_detector *h_det, int n_det,
+                             int n_steps, bool copy_phasors_in, const float *const *h_cot, HostStage &hs, cudaStream_t st)
+{
+    size_t need = 0;
+    auto pad = [](size_t b) { return (b + 255) / 256 * 256; };
+    for (int s = 0; s < n_src; ++s) {
+        if (h_src[s].profile) need += pad(box_cells(h_src[s].lo, h_src[s].hi) * sizeof(float));
+        need += pad((size_t)n_steps * sizeof(float));
+    }
+    hs.phasor_bytes.resize(n_det);
+    for (int s = 0; s < n_det; ++s) {
+        hs.phasor_bytes[s] = (size_t)h_det[s].n_freq * popcount6(h_det[s].component_mask) * box_cells(h_det[s].lo, h_det[s].hi) * 2 * sizeof(float);
+        need += 2 * pad(hs.phasor_bytes[s]);
+    }
+    if (need > g->hb_desc_cap) {
+        int rc = g->alloc((void **)&g->hb_desc, need);
+        if (rc) return rc;
+        g->hb_desc_cap = need;
+    }
+    char *cur = (char *)g->hb_desc;
+    hs.src.assign(h_src, h_src + n_src);
+    hs.det.assign(h_det, h_det + n_det);
+    for (int s = 0; s < n_src; ++s) {
+        if (h_src[s].profile) {
+            const size_t b = box_cells(h_src[s].lo, h_src[s].hi) * sizeof(float);
+            CK(cudaMemcpyAsync(cur, h_src[s].profile, b, cudaMemcpyHostToDevice, st));
+            hs.src[s].profile = (const float *)cur; cur += pad(b);
+        }
+        const size_t b = (size_t)n_steps * sizeof(float);
+        if (b) CK(cudaMemcpyAsync(cur, h_src[s].waveform, b, cudaMemcpyHostToDevice, st));
+        hs.src[s].waveform = (const float *)cur; cur += pad(b);
+    }
+    g->hb_cot.assign(n_det, nullptr);
+    for (int s = 0; s < n_det; ++s) {
+        const size_t b = hs.phasor_bytes[s];
+        hs.det[s].phasor = (float *)cur;
+        if (copy_phasors_in && h_det[s].phasor) CK(cudaMemcpyAsync(cur, h_det[s].phasor, b, cudaMemcpyHostToDevice, st));
+        cur += pad(b);
+        if (h_cot && h_cot[s]) {
+            CK(cudaMemcpyAsync(cur, h_cot[s], b, cudaMemcpyHostToDevice, st));
+            g->hb_cot[s] = (const float *)cur;
+        }
+        cur += pad(b);
+    }
+    return FDTD_OK;
+}
+
+extern "C" int fdtd_forward_host(fdtd_grid *g, float *h_fields, const float *h_inv_eps, const float *h_inv_mu,
+                                 const fdtd_source *h_src, int32_t n_src, const fdtd_detector *h_det, int32_t n_det,
+                                 int32_t n_steps, void *cuda_stream)
+{
+    if (!g) return fail(FDTD_EINVAL, "fdtd_forward_host: NULL grid");
+    if (!h_inv_eps) return fail(FDTD_EINVAL, "fdtd_forward_host: inv_eps is required");
+    if (n_steps < 0 || n_steps > g->desc.max_steps) return fail(FDTD_EINVAL, "fdtd_forward_host: need 0 <= n_steps <= max_steps");
+    if (n_src < 0 || n_det < 0 || (n_src && !h_src) || (n_det && !h_det)) return fail(FDTD_EINVAL, "fdtd_forward_host: bad descriptor arrays");
+    for (int s = 0; s < n_src; ++s) if (!box_ok(g->G, h_src[s].lo, h_src[s].hi) || !h_src[s].waveform) return fail(FDTD_EINVAL, "fdtd_forward_host: bad source");
+    for (int s = 0; s < n_det; ++s) if (!box_ok(g->G, h_det[s].lo, h_det[s].hi) || !h_det[s].phasor || h_det[s].n_freq < 1) return fail(FDTD_EINVAL, "fdtd_forward_host: bad detector");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = g->ensure_host_buffers(h_inv_mu != nullptr);
+    if (rc) return rc;
+    const size_t vol = (size_t)g->G.nc * sizeof(float);
+    if (h_fields) CK(cudaMemcpyAsync(g->hb_fields, h_fields, 6 * vol, cudaMemcpyHostToDevice, st));
+    else          CK(cudaMemsetAsync(g->hb_fields, 0, 6 * vol, st));
+    CK(cudaMemcpyAsync(g->hb_ie, h_inv_eps, vol, cudaMemcpyHostToDevice, st));
+    if (h_inv_mu) CK(cudaMemcpyAsync(g->hb_im, h_inv_mu, vol, cudaMemcpyHostToDevice, st));
+    HostStage hs;
+    if ((rc = stage_descriptors(g, h_src, n_src, h_det, n_det, n_steps, true, nullptr, hs, st))) return rc;
+    rc = fdtd_forward(g, g->hb_fields, g->hb_ie, h_inv_mu ? g->hb_im : nullptr, hs.src.data(), n_src, hs.det.data(), n_det, n_steps, st);
+    if (rc) return rc;
+    for (int s = 0; s < n_det; ++s)
+        CK(cudaMemcpyAsync(h_det[s].phasor, hs.det[s].phasor, hs.phasor_bytes[s], cudaMemcpyDeviceToHost, st));
+    if (h_fields) CK(cudaMemcpyAsync(h_fields, g->hb_fields, 6 * vol, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return FDTD_OK;
+}
+
+extern "C" int fdtd_backward_host(fdtd_grid *g, float *h_fields, const float *h_inv_eps, const float *h_inv_mu,
+                                  const fdtd_source *h_src, int32_t n_src, const fdtd_detector *h_det, int32_t n_det,
+                                  const float *const *h_dL_dphasor, const float *h_dL_dfields,
+                                  int32_t n_steps, float *h_dL_dinv_eps, float *h_dL_dfields0, void *cuda_stream)
+{
+    if (!g) return fail(FDTD_EINVAL, "fdtd_backward_host: NULL grid");
+    if (!h_inv_eps || !h_dL_dinv_eps) return fail(FDTD_EINVAL, "fdtd_backward_host: inv_eps and dL_dinv_eps are required");
+    if (n_steps < 0 || n_steps > g->desc.max_steps) return fail(FDTD_EINVAL, "fdtd_backward_host: need 0 <= n_steps <= max_steps");
+    if (n_src < 0 || n_det < 0 || (n_src && !h_src) || (n_det && !h_det)) return fail(FDTD_EINVAL, "fdtd_backward_host: bad descriptor arrays");
+    for (int s = 0; s < n_src; ++s) if (!box_ok(g->G, h_src[s].lo, h_src[s].hi) || !h_src[s].waveform) return fail(FDTD_EINVAL, "fdtd_backward_host: bad source");
+    for (int s = 0; s < n_det; ++s) if (!box_ok(g->G, h_det[s].lo, h_det[s].hi) || h_det[s].n_freq < 1) return fail(FDTD_EINVAL, "fdtd_backward_host: bad detector");
+    if (!h_fields && !g->hb_fields) return fail(FDTD_ESTATE, "fdtd_backward_host: no state left by fdtd_forward_host");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = g->ensure_host_buffers(h_inv_mu != nullptr);
+    if (rc) return rc;
+    const size_t vol = (size_t)g->G.nc * sizeof(float);
+    if (!g->hb_grad && (rc = g->alloc((void **)&g->hb_grad, vol))) return rc;
+    if ((h_dL_dfields || h_dL_dfields0) && !g->hb_cotf && (rc = g->alloc((void **)&g->hb_cotf, 6 * vol))) return rc;
+    if (h_fields) CK(cudaMemcpyAsync(g->hb_fields, h_fields, 6 * vol, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(g->hb_ie, h_inv_eps, vol, cudaMemcpyHostToDevice, st));
+    if (h_inv_mu) CK(cudaMemcpyAsync(g->hb_im, h_inv_mu, vol, cudaMemcpyHostToDevice, st));
+    if (h_dL_dfields) CK(cudaMemcpyAsync(g->hb_cotf, h_dL_dfields, 6 * vol, cudaMemcpyHostToDevice, st));
+    HostStage hs;
+    if ((rc = stage_descriptors(g, h_src, n_src, h_det, n_det, n_steps, false, h_dL_dphasor, hs, st))) return rc;
+    rc = fdtd_backward(g, g->hb_fields, g->hb_ie, h_inv_mu ? g->hb_im : nullptr, hs.src.data(), n_src, hs.det.data(), n_det,
+                       h_dL_dphasor ? g->hb_cot.data() : nullptr, h_dL_dfields ? g->hb_cotf : nullptr, n_steps,
+                       g->hb_grad, h_dL_dfields0 ? g->hb_cotf : nullptr, st);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(h_dL_dinv_eps, g->hb_grad, vol, cudaMemcpyDeviceToHost, st));
+    if (h_dL_dfields0) CK(cudaMemcpyAsync(h_dL_dfields0, g->hb_cotf, 6 * vol, cudaMemcpyDeviceToHost, st));
+    if (h_fields) CK(cudaMemcpyAsync(h_fields, g->hb_fields, 6 * vol, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return FDTD_OK;
+}

@@ -1,0 +1,93 @@
+// fdtd_grid.h -- the grid object behind the opaque fdtd_grid handle (host side, private).
+#pragma once
+#include <string>
+#include <vector>
+#include "fdtd_internal.h"
+
+struct FusedState;   // kernels_fused.cu
+
+struct fdtd_grid {
+    fdtd_grid_desc desc{};
+    fdtd::Dims G{};
+    fdtd::Tables T{};
+    fdtd::RecLayout R{};
+    std::vector<float> h_tables;          // host copy of the CPML tables (layout as uploaded)
+
+    int path = FDTD_PATH_GENERIC;
+    int tile_x = 0, tile_y = 0, tile_z = 0;
+    std::string fused_why_not;
+    int graph_unroll = 8;
+
+    // device memory owned by the grid
+    std::vector<void *> owned;
+    long long recorder_bytes = 0, scratch_bytes = 0;
+    int *d_step = nullptr;
+    fdtd::PsiSet psiE[2]{}, psiH[2]{};     // primal psi ([1] only used by the fused path's ping-pong)
+    fdtd::PsiSet lpsiE[2]{}, lpsiH[2]{};   // psi cotangents, ping-ponged by step parity
+    float *lam = nullptr;                  // cotangent fields [6][nz][ny][nx]
+    float *lam_result = nullptr;           // where the final cotangent lives if not in `lam` (fused path)
+    float *rec = nullptr;                  // interface recorder
+    int recorded_steps = -1;               // n_steps of the last recorded forward, or -1
+    float *d_cs = nullptr;                 // per-step (cos, sin) table
+    float *h_cs = nullptr;                 // pinned staging of the same
+    size_t cs_cap = 0;
+    cudaEvent_t table_done = nullptr;
+
+    // host-buffer entry points
+    float *hb_fields = nullptr, *hb_ie = nullptr, *hb_im = nullptr, *hb_grad = nullptr, *hb_cotf = nullptr;
+    void *hb_desc = nullptr;
+    size_t hb_desc_cap = 0;
+    std::vector<const float *> hb_cot;
+
+    // graphs
+    struct GraphCache {
+        std::string key;
+        cudaGraphExec_t exec_main = nullptr, exec_tail = nullptr;
+        cudaEvent_t done = nullptr;
+    } fwd_graph, bwd_graph;
+    cudaStream_t cap_stream = nullptr;
+    long long kernel_launches = 0;
+
+    FusedState *fused = nullptr;
+
+    // per-kernel profiling (fdtd_set_profiling)
+    enum ProfClass { PC_UPDATE_E, PC_UPDATE_H, PC_ADJ_H, PC_INV_H, PC_INV_E_GRAD, PC_ADJ_E,
+                     PC_FUSED_FWD, PC_FUSED_BWD, PC_RECORD, PC_INJECT, PC_SRC_DET, PC_OTHER, PC_COUNT };
+    bool profiling = false;
+    struct ProfSpan { int cls; cudaEvent_t a, b; };
+    std::vector<ProfSpan> prof_spans;
+    std::vector<cudaEvent_t> prof_pool;
+    long long prof_launches[PC_COUNT] = {};
+    double prof_ms[PC_COUNT] = {};
+    bool prof_capturing = false;           // true while a graph is being captured (no events then)
+    cudaEvent_t prof_begin(cudaStream_t st);
+    void prof_end(int cls, cudaEvent_t a, cudaStream_t st);
+
+    int alloc(void **p, size_t bytes, bool recorder = false);
+    int alloc_psi(fdtd::PsiSet &s);
+    int zero_psi(const fdtd::PsiSet &s, cudaStream_t st);
+    int ensure_backward_buffers();
+    int ensure_host_buffers(bool need_mu);
+    void drop_graphs();
+};
+
+// fused TMA path (kernels_fused.cu).  fused_setup decides whether the grid qualifies and, if so,
+// sets g->path = FDTD_PATH_FUSED; otherwise it records the reason in g->fused_why_not.
+int fused_setup(fdtd_grid *g);
+void fused_teardown(fdtd_grid *g);
+int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
+                  const std::vector<fdtd::SourceDev> &S, const std::vector<fdtd::DetectorDev> &D,
+                  int total_freq, int n_steps, bool recording, cudaStream_t st);
+int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
+                   const std::vector<fdtd::SourceDev> &S, const std::vector<fdtd::DetectorDev> &D,
+                   int total_freq, int n_steps, float *dL_dinv_eps, cudaStream_t st);
+
+// RAII span: brackets the launches made in its lifetime with two events when profiling is on
+struct ProfScope {
+    fdtd_grid *g; int cls; cudaStream_t st; cudaEvent_t a;
+    ProfScope(fdtd_grid *g_, int cls_, cudaStream_t st_) : g(g_), cls(cls_), st(st_), a(g_->prof_begin(st_)) {}
+    ~ProfScope() { if (a) g->prof_end(cls, a, st); }
+};
+
+// shared by the API and the fused path
+int fdtd_fail(int code, const std::string &msg);

@@ -1,0 +1,123 @@
+// fdtd_internal.h -- private structures shared by the host API and the kernels.
+// Product code: shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "../../include/fdtd.h"
+
+namespace fdtd {
+
+// ----------------------------------------------------------------------------------------------
+// Geometry shared by every kernel (passed by value).
+// ----------------------------------------------------------------------------------------------
+struct Dims {
+    int nx, ny, nz;
+    int d;            // CPML thickness
+    int dpx;          // half-width of the x-slab psi storage (d rounded up to 4 when it fits)
+    int periodic;
+    float S;
+    long long nc;     // cells
+    int lo[3], hi[3]; // interior box I
+    int glo[3], ghi[3]; // gradient box (already clipped to I)
+};
+
+// CPML tables on the device: [family 0=E 1=H][axis] -> pointer to N_axis floats
+struct Tables {
+    const float *b[2][3];
+    const float *a[2][3];
+    const float *ik[2][3];
+};
+
+// psi arrays: [component c][s]; array (c,s) belongs to derivative axis (c+1+s)%3 and is stored
+// slab-compact on the two slabs normal to that axis:
+//   axis x: [nz][ny][2*dpx]   axis y: [nz][2*d][nx]   axis z: [2*d][ny][nx]
+struct PsiSet {
+    float *p[3][2];
+};
+
+__host__ __device__ inline int psi_axis(int c, int s) { return (c + 1 + s) % 3; }
+
+__host__ __device__ inline long long psi_elems(const Dims &G, int axis)
+{
+    if (G.d == 0) return 0;
+    if (axis == 0) return (long long)G.nz * G.ny * (2 * G.dpx);
+    if (axis == 1) return (long long)G.nz * (2 * G.d) * G.nx;
+    return (long long)(2 * G.d) * G.ny * G.nx;
+}
+
+// slab-compact index of cell (i,j,k) in a psi array of `axis`, or -1 if the cell is not in the PML
+// slab of that axis.
+__host__ __device__ inline long long psi_index(const Dims &G, int axis, int i, int j, int k)
+{
+    if (axis == 0) {
+        int s;
+        if (i < G.d) s = i; else if (i >= G.nx - G.d) s = i - (G.nx - 2 * G.dpx); else return -1;
+        return ((long long)k * G.ny + j) * (2 * G.dpx) + s;
+    } else if (axis == 1) {
+        int s;
+        if (j < G.d) s = j; else if (j >= G.ny - G.d) s = j - (G.ny - 2 * G.d); else return -1;
+        return ((long long)k * (2 * G.d) + s) * G.nx + i;
+    } else {
+        int s;
+        if (k < G.d) s = k; else if (k >= G.nz - G.d) s = k - (G.nz - 2 * G.d); else return -1;
+        return ((long long)s * G.ny + j) * G.nx + i;
+    }
+}
+
+// ----------------------------------------------------------------------------------------------
+// Interface recorder (reading R15).  One step's record = 12 segments:
+// for axis a: [low H_{a+1}] [low H_{a+2}] [high E'_{a+1}] [high E'_{a+2}], each holding the face
+// cells (other two indices over I; the lower-numbered of the two other axes is fastest), padded to
+// a multiple of 4 floats.
+// ----------------------------------------------------------------------------------------------
+struct RecLayout {
+    long long off[3][2][2];   // [axis][side 0=low,1=high][which]
+    long long cells[3];       // face cells per axis
+    int fast[3], slow[3];     // the two in-face axes
+    long long stride;         // floats per step (multiple of 32)
+};
+
+struct SourceDev {
+    int comp;
+    int lo[3], hi[3];
+    const float *profile;
+    const float *waveform;
+};
+
+struct DetectorDev {
+    int mask, ncomp;
+    int lo[3], hi[3];
+    int n_freq;
+    int cs_off;               // offset (in frequencies) into the per-step cos/sin table
+    float *phasor;            // forward: accumulate into;  backward: cotangent (may be NULL)
+};
+
+// ----------------------------------------------------------------------------------------------
+// Generic (one thread per cell) kernel launchers -- kernels_generic.cu
+// All kernels read the current step index n from *step (device memory) so that the per-step
+// launch sequence is identical for every n and can be replayed from a CUDA graph.
+// ----------------------------------------------------------------------------------------------
+void launch_update_E(const Dims &G, const Tables &T, float *fields, const float *ie, PsiSet psiE, cudaStream_t st);
+void launch_update_H(const Dims &G, const Tables &T, float *fields, const float *im, PsiSet psiH, cudaStream_t st);
+void launch_add_source(const Dims &G, float *fields, const SourceDev &s, const int *step, float sign, cudaStream_t st);
+void launch_detector(const Dims &G, const float *fields, const DetectorDev &dt, const float *cs_table,
+                     int total_freq, const int *step, cudaStream_t st);
+void launch_detector_adjoint(const Dims &G, float *lam, const DetectorDev &dt, const float *cs_table,
+                             int total_freq, const int *step, cudaStream_t st);
+// H source: fields that hold the pre-step H (low faces); E source: fields that hold the post-E-update E'
+void launch_record(const Dims &G, const RecLayout &R, const float *fields_H, const float *fields_E,
+                   float *rec, const int *step, cudaStream_t st);
+void launch_inject(const Dims &G, const RecLayout &R, float *fields, const float *rec, const int *step, cudaStream_t st);
+void launch_advance(int *step, int delta, cudaStream_t st);
+// psi cotangents are ping-ponged by step parity: read set[n&1], write set[(n&1)^1]
+void launch_adj_H(const Dims &G, const Tables &T, float *lam, const float *im, PsiSet set0, PsiSet set1,
+                  const int *step, cudaStream_t st);
+void launch_adj_E(const Dims &G, const Tables &T, float *lam, const float *ie, PsiSet set0, PsiSet set1,
+                  const int *step, cudaStream_t st);
+void launch_grad_rho(const Dims &G, const float *g, const float *ie, float delta_eps, const int lo[3], const int hi[3],
+                     float *out, cudaStream_t st);
+void launch_inv_H(const Dims &G, float *fields, const float *im, cudaStream_t st);
+void launch_inv_E_grad(const Dims &G, float *fields, const float *ie, const float *lam, float *g, cudaStream_t st);
+
+}  // namespace fdtd

@@ -1,0 +1,451 @@
+// kernels_generic.cu -- one-thread-per-cell kernels for every row of the hot path.
+//
+// These are the general path: any grid size, periodic or zero-padded walls, in-place updates.
+// They serve periodic grids and sizes the fused TMA kernels do not take, and they are the
+// simple statement the fused kernels are cross-checked against on the GPU.
+// Formulas: include/fdtd.h (conventions) and DESIGN.md section 2; Eq. 1-2, L72, L84.
+#include "fdtd_internal.h"
+
+namespace fdtd {
+
+namespace {
+
+constexpr int BX = 64, BY = 4;
+
+__device__ __forceinline__ long long lin(const Dims &G, int i, int j, int k)
+{
+    return ((long long)k * G.ny + j) * G.nx + i;
+}
+
+// neighbour fetch with wrap (periodic) or zero (walls); offsets are at most +-1
+template <bool PER>
+__device__ __forceinline__ float fetch(const Dims &G, const float *__restrict__ F, int i, int j, int k)
+{
+    if (PER) {
+        i = i < 0 ? i + G.nx : (i >= G.nx ? i - G.nx : i);
+        j = j < 0 ? j + G.ny : (j >= G.ny ? j - G.ny : j);
+        k = k < 0 ? k + G.nz : (k >= G.nz ? k - G.nz : k);
+    } else if (i < 0 || i >= G.nx || j < 0 || j >= G.ny || k < 0 || k >= G.nz) {
+        return 0.f;
+    }
+    return __ldg(F + lin(G, i, j, k));
+}
+
+#define CELL_IJK()                                                   \
+    const int i = blockIdx.x * BX + threadIdx.x;                     \
+    const int j = blockIdx.y * BY + threadIdx.y;                     \
+    const int k = blockIdx.z;                                        \
+    if (i >= G.nx || j >= G.ny) return;                              \
+    const long long p = lin(G, i, j, k);                             \
+    const int pos[3] = { i, j, k };                                  \
+    (void)pos;
+
+// ------------------------------------------------------------------------------------------ F1+F2
+template <bool PER>
+__global__ void __launch_bounds__(BX *BY) k_update_E(Dims G, Tables T, float *__restrict__ f,
+                                                     const float *__restrict__ ie, PsiSet psi)
+{
+    CELL_IJK();
+    const float sie = G.S * __ldg(ie + p);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const int a = (c + 1) % 3, b = (c + 2) % 3;
+        const float *Hb = f + (3 + b) * G.nc, *Ha = f + (3 + a) * G.nc;
+        const float d1 = Hb[p] - fetch<PER>(G, Hb, i - (a == 0), j - (a == 1), k - (a == 2));
+        const float d2 = Ha[p] - fetch<PER>(G, Ha, i - (b == 0), j - (b == 1), k - (b == 2));
+        float t = __ldg(T.ik[0][a] + pos[a]) * d1 - __ldg(T.ik[0][b] + pos[b]) * d2;
+        if (G.d > 0) {
+            const long long s0 = psi_index(G, a, i, j, k);
+            if (s0 >= 0) {
+                const float ps = __ldg(T.b[0][a] + pos[a]) * psi.p[c][0][s0] + __ldg(T.a[0][a] + pos[a]) * d1;
+                psi.p[c][0][s0] = ps;
+                t += ps;
+            }
+            const long long s1 = psi_index(G, b, i, j, k);
+            if (s1 >= 0) {
+                const float ps = __ldg(T.b[0][b] + pos[b]) * psi.p[c][1][s1] + __ldg(T.a[0][b] + pos[b]) * d2;
+                psi.p[c][1][s1] = ps;
+                t -= ps;
+            }
+        }
+        f[c * G.nc + p] += sie * t;
+    }
+}
+
+// ------------------------------------------------------------------------------------------ F4+F5
+template <bool PER>
+__global__ void __launch_bounds__(BX *BY) k_update_H(Dims G, Tables T, float *__restrict__ f,
+                                                     const float *__restrict__ im, PsiSet psi)
+{
+    CELL_IJK();
+    const float sim = G.S * (im ? __ldg(im + p) : 1.f);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const int a = (c + 1) % 3, b = (c + 2) % 3;
+        const float *Eb = f + b * G.nc, *Ea = f + a * G.nc;
+        const float d1 = fetch<PER>(G, Eb, i + (a == 0), j + (a == 1), k + (a == 2)) - Eb[p];
+        const float d2 = fetch<PER>(G, Ea, i + (b == 0), j + (b == 1), k + (b == 2)) - Ea[p];
+        float t = __ldg(T.ik[1][a] + pos[a]) * d1 - __ldg(T.ik[1][b] + pos[b]) * d2;
+        if (G.d > 0) {
+            const long long s0 = psi_index(G, a, i, j, k);
+            if (s0 >= 0) {
+                const float ps = __ldg(T.b[1][a] + pos[a]) * psi.p[c][0][s0] + __ldg(T.a[1][a] + pos[a]) * d1;
+                psi.p[c][0][s0] = ps;
+                t += ps;
+            }
+            const long long s1 = psi_index(G, b, i, j, k);
+            if (s1 >= 0) {
+                const float ps = __ldg(T.b[1][b] + pos[b]) * psi.p[c][1][s1] + __ldg(T.a[1][b] + pos[b]) * d2;
+                psi.p[c][1][s1] = ps;
+                t -= ps;
+            }
+        }
+        f[(3 + c) * G.nc + p] -= sim * t;
+    }
+}
+
+// ------------------------------------------------------------------------------------------ F3/F6
+__global__ void k_add_source(Dims G, float *__restrict__ f, SourceDev s, const int *__restrict__ step, float sign)
+{
+    const int bx = s.hi[0] - s.lo[0], by = s.hi[1] - s.lo[1], bz = s.hi[2] - s.lo[2];
+    const long long n_cells = (long long)bx * by * bz;
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n_cells) return;
+    const int i = (int)(t % bx), j = (int)((t / bx) % by), k = (int)(t / ((long long)bx * by));
+    const float w = sign * __ldg(s.waveform + *step);
+    const float pr = s.profile ? __ldg(s.profile + t) : 1.f;
+    f[s.comp * G.nc + lin(G, s.lo[0] + i, s.lo[1] + j, s.lo[2] + k)] += pr * w;
+}
+
+// ------------------------------------------------------------------------------------------ F7 / B1
+// cs_table: [max_steps][total_freq][2] = (cos, sin) of omega_f*(n+1), built on the host in fp64 (R13)
+template <bool ADJ>
+__global__ void k_detector(Dims G, float *__restrict__ f, DetectorDev dt, const float *__restrict__ cs,
+                           int total_freq, const int *__restrict__ step)
+{
+    const int bx = dt.hi[0] - dt.lo[0], by = dt.hi[1] - dt.lo[1], bz = dt.hi[2] - dt.lo[2];
+    const long long bc = (long long)bx * by * bz;
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= bc) return;
+    const int i = (int)(t % bx), j = (int)((t / bx) % by), k = (int)(t / ((long long)bx * by));
+    const long long p = lin(G, dt.lo[0] + i, dt.lo[1] + j, dt.lo[2] + k);
+    const float *csn = cs + ((long long)(*step) * total_freq + dt.cs_off) * 2;
+    int ci = 0;
+    for (int c = 0; c < 6; ++c) {
+        if (!((dt.mask >> c) & 1)) continue;
+        if (!ADJ) {
+            const float v = f[c * G.nc + p];
+            for (int q = 0; q < dt.n_freq; ++q) {
+                float2 *P = reinterpret_cast<float2 *>(dt.phasor) + ((long long)q * dt.ncomp + ci) * bc + t;
+                float2 acc = *P;
+                acc.x += v * __ldg(csn + 2 * q);
+                acc.y -= v * __ldg(csn + 2 * q + 1);
+                *P = acc;
+            }
+        } else {
+            float acc = 0.f;
+            for (int q = 0; q < dt.n_freq; ++q) {
+                const float2 Gq = __ldg(reinterpret_cast<const float2 *>(dt.phasor) + ((long long)q * dt.ncomp + ci) * bc + t);
+                acc += Gq.x * __ldg(csn + 2 * q) - Gq.y * __ldg(csn + 2 * q + 1);
+            }
+            f[c * G.nc + p] += acc;
+        }
+        ++ci;
+    }
+}
+
+// ------------------------------------------------------------------------------------------ F8
+// One thread per float of a step's record.  INJECT=false: fields -> rec[n]; true: rec[n] -> fields.
+template <bool INJECT>
+__global__ void k_record(Dims G, RecLayout R, const float *__restrict__ fH, const float *__restrict__ fE,
+                         float *__restrict__ fout, float *__restrict__ rec, const int *__restrict__ step)
+{
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= R.stride) return;
+    // locate the segment
+    int a = 0, side = 0, which = 0;
+    long long local = -1;
+#pragma unroll
+    for (int aa = 0; aa < 3; ++aa)
+#pragma unroll
+        for (int ss = 0; ss < 2; ++ss)
+#pragma unroll
+            for (int ww = 0; ww < 2; ++ww) {
+                const long long o = R.off[aa][ss][ww];
+                if (t >= o && t < o + R.cells[aa]) { a = aa; side = ss; which = ww; local = t - o; }
+            }
+    if (local < 0) return;   // padding
+    const int fa = R.fast[a], sl = R.slow[a];
+    const int nf = G.hi[fa] - G.lo[fa];
+    int pos[3];
+    pos[a] = side ? G.hi[a] : G.lo[a] - 1;
+    pos[fa] = G.lo[fa] + (int)(local % nf);
+    pos[sl] = G.lo[sl] + (int)(local / nf);
+    const int comp = (a + 1 + which) % 3;
+    const long long p = lin(G, pos[0], pos[1], pos[2]);
+    float *r = rec + (long long)(*step) * R.stride + t;
+    if (!INJECT) {
+        *r = side ? __ldg(fE + comp * G.nc + p) : __ldg(fH + (3 + comp) * G.nc + p);
+    } else {
+        fout[(side ? comp : 3 + comp) * G.nc + p] = *r;
+    }
+}
+
+__global__ void k_advance(int *step, int delta) { *step += delta; }
+
+// ------------------------------------------------------------------------------------------ B2 / B5
+// Adjoint of the H update (FAMILY=1: reads lamH, updates lamE, psi_H cotangents) or of the E update
+// (FAMILY=0: reads lamE, updates lamH, psi_E cotangents), in gather form:
+//   w_c(q)  = sgn*S*med(q)*lam_c(q)          sgn = -1 (H update), +1 (E update)
+//   g1_c(q) =  ik_a w + a_a (lpsi_c0 + w)    a = c+1 (tables of FAMILY at q_a)
+//   g2_c(q) = -ik_b w + a_b (lpsi_c1 - w)    b = c+2
+//   lpsi_c0 <- b_a (lpsi_c0 + w) ; lpsi_c1 <- b_b (lpsi_c1 - w)          (owner cell only)
+//   FAMILY=1: lamE_t(p) -= [g1_{t+1}(p) - g1_{t+1}(p-e_{t+2})] + [g2_{t+2}(p) - g2_{t+2}(p-e_{t+1})]
+//   FAMILY=0: lamH_t(p) -= [g1_{t+1}(p+e_{t+2}) - g1_{t+1}(p)] + [g2_{t+2}(p+e_{t+1}) - g2_{t+2}(p)]
+// psi cotangents are ping-ponged (read set[n&1], write set[(n&1)^1]) because the neighbour's g is
+// recomputed from its OLD psi cotangent.
+template <int FAMILY>
+struct AdjCtx {
+    const Dims &G;
+    const Tables &T;
+    const float *lam_src;    // 3 volumes (lamH for FAMILY 1, lamE for FAMILY 0)
+    const float *med;        // inv_mu (may be NULL) or inv_eps
+    const PsiSet &lin_;      // old psi cotangents
+    __device__ __forceinline__ float w(int c, long long q) const
+    {
+        const float m = med ? __ldg(med + q) : 1.f;
+        return (FAMILY ? -G.S : G.S) * m * __ldg(lam_src + c * G.nc + q);
+    }
+    // g1 of component c at cell (i,j,k) (in range)
+    __device__ __forceinline__ float g(int c, int s, int i, int j, int k, float *new_psi) const
+    {
+        const int ax = psi_axis(c, s);
+        const int pa = ax == 0 ? i : (ax == 1 ? j : k);
+        const long long q = lin(G, i, j, k);
+        const float ww = w(c, q);
+        const float sg = s ? -1.f : 1.f;
+        float r = sg * __ldg(T.ik[FAMILY][ax] + pa) * ww;
+        if (G.d > 0) {
+            const long long si = psi_index(G, ax, i, j, k);
+            if (si >= 0) {
+                const float l = __ldg(lin_.p[c][s] + si) + sg * ww;
+                r += __ldg(T.a[FAMILY][ax] + pa) * l;
+                if (new_psi) *new_psi = __ldg(T.b[FAMILY][ax] + pa) * l;
+            }
+        }
+        return r;
+    }
+};
+
+template <int FAMILY, bool PER>
+__global__ void __launch_bounds__(BX *BY) k_adjoint(Dims G, Tables T, float *__restrict__ lam,
+                                                    const float *__restrict__ med, PsiSet set0, PsiSet set1,
+                                                    const int *__restrict__ step)
+{
+    CELL_IJK();
+    const int par = (*step) & 1;
+    const PsiSet &pin = par ? set1 : set0;
+    const PsiSet &pout = par ? set0 : set1;
+    const float *src = lam + (FAMILY ? 3 : 0) * G.nc;
+    float *dst = lam + (FAMILY ? 0 : 3) * G.nc;
+    AdjCtx<FAMILY> C{ G, T, src, med, pin };
+    const int sgn = FAMILY ? -1 : +1;     // neighbour offset: p - e (H-update adjoint), p + e (E-update adjoint)
+    // own-cell g values and psi-cotangent updates
+    float g_own[3][2];
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+            float np_ = 0.f;
+            bool has = false;
+            if (G.d > 0) {
+                const long long si = psi_index(G, psi_axis(c, s), i, j, k);
+                has = si >= 0;
+                g_own[c][s] = C.g(c, s, i, j, k, has ? &np_ : nullptr);
+                if (has) pout.p[c][s][si] = np_;
+            } else {
+                g_own[c][s] = C.g(c, s, i, j, k, nullptr);
+            }
+        }
+#pragma unroll
+    for (int t = 0; t < 3; ++t) {
+        const int c1 = (t + 1) % 3, ax1 = (t + 2) % 3;   // g1 of component t+1, derivative axis t+2
+        const int c2 = (t + 2) % 3, ax2 = (t + 1) % 3;   // g2 of component t+2, derivative axis t+1
+        int q1[3] = { i, j, k }, q2[3] = { i, j, k };
+        q1[ax1] += sgn;
+        q2[ax2] += sgn;
+        float n1 = 0.f, n2 = 0.f;
+        {
+            int qi = q1[0], qj = q1[1], qk = q1[2];
+            bool ok = true;
+            if (PER) {
+                qi = qi < 0 ? qi + G.nx : (qi >= G.nx ? qi - G.nx : qi);
+                qj = qj < 0 ? qj + G.ny : (qj >= G.ny ? qj - G.ny : qj);
+                qk = qk < 0 ? qk + G.nz : (qk >= G.nz ? qk - G.nz : qk);
+            } else {
+                ok = qi >= 0 && qi < G.nx && qj >= 0 && qj < G.ny && qk >= 0 && qk < G.nz;
+            }
+            if (ok) n1 = C.g(c1, 0, qi, qj, qk, nullptr);
+        }
+        {
+            int qi = q2[0], qj = q2[1], qk = q2[2];
+            bool ok = true;
+            if (PER) {
+                qi = qi < 0 ? qi + G.nx : (qi >= G.nx ? qi - G.nx : qi);
+                qj = qj < 0 ? qj + G.ny : (qj >= G.ny ? qj - G.ny : qj);
+                qk = qk < 0 ? qk + G.nz : (qk >= G.nz ? qk - G.nz : qk);
+            } else {
+                ok = qi >= 0 && qi < G.nx && qj >= 0 && qj < G.ny && qk >= 0 && qk < G.nz;
+            }
+            if (ok) n2 = C.g(c2, 1, qi, qj, qk, nullptr);
+        }
+        // FAMILY=1: -(own - nbr) ; FAMILY=0: -(nbr - own)
+        const float diff1 = FAMILY ? (g_own[c1][0] - n1) : (n1 - g_own[c1][0]);
+        const float diff2 = FAMILY ? (g_own[c2][1] - n2) : (n2 - g_own[c2][1]);
+        dst[t * G.nc + p] -= diff1 + diff2;
+    }
+}
+
+// ------------------------------------------------------------------------------------------ B3
+// inverse H step on I:  H = H' + S im curl+ E'   (sources already subtracted; the E' operand at
+// index N_a-d was injected from the record)
+template <bool PER>
+__global__ void __launch_bounds__(BX *BY) k_inv_H(Dims G, float *__restrict__ f, const float *__restrict__ im)
+{
+    CELL_IJK();
+    if (i < G.lo[0] || i >= G.hi[0] || j < G.lo[1] || j >= G.hi[1] || k < G.lo[2] || k >= G.hi[2]) return;
+    const float sim = G.S * (im ? __ldg(im + p) : 1.f);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const int a = (c + 1) % 3, b = (c + 2) % 3;
+        const float *Eb = f + b * G.nc, *Ea = f + a * G.nc;
+        const float d1 = fetch<PER>(G, Eb, i + (a == 0), j + (a == 1), k + (a == 2)) - Eb[p];
+        const float d2 = fetch<PER>(G, Ea, i + (b == 0), j + (b == 1), k + (b == 2)) - Ea[p];
+        f[(3 + c) * G.nc + p] += sim * (d1 - d2);
+    }
+}
+
+// ------------------------------------------------------------------------------------------ B4
+// q = curl- H on I (operand at d-1 injected from the record); g += S sum_c lamE_c q_c on the
+// gradient box; E = E' - S ie q.
+template <bool PER>
+__global__ void __launch_bounds__(BX *BY) k_inv_E_grad(Dims G, float *__restrict__ f, const float *__restrict__ ie,
+                                                       const float *__restrict__ lam, float *__restrict__ g)
+{
+    CELL_IJK();
+    if (i < G.lo[0] || i >= G.hi[0] || j < G.lo[1] || j >= G.hi[1] || k < G.lo[2] || k >= G.hi[2]) return;
+    const float sie = G.S * __ldg(ie + p);
+    float acc = 0.f;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const int a = (c + 1) % 3, b = (c + 2) % 3;
+        const float *Hb = f + (3 + b) * G.nc, *Ha = f + (3 + a) * G.nc;
+        const float d1 = Hb[p] - fetch<PER>(G, Hb, i - (a == 0), j - (a == 1), k - (a == 2));
+        const float d2 = Ha[p] - fetch<PER>(G, Ha, i - (b == 0), j - (b == 1), k - (b == 2));
+        const float q = d1 - d2;
+        acc += __ldg(lam + c * G.nc + p) * q;
+        f[c * G.nc + p] -= sie * q;
+    }
+    if (i >= G.glo[0] && i < G.ghi[0] && j >= G.glo[1] && j < G.ghi[1] && k >= G.glo[2] && k < G.ghi[2])
+        g[p] += G.S * acc;
+}
+
+// ------------------------------------------------------------------------------------------ B6
+__global__ void k_grad_rho(Dims G, const float *__restrict__ g, const float *__restrict__ ie, float delta_eps,
+                           int lx, int ly, int lz, int bx, int by, int bz, float *__restrict__ out)
+{
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (long long)bx * by * bz) return;
+    const int i = (int)(t % bx), j = (int)((t / bx) % by), k = (int)(t / ((long long)bx * by));
+    const long long p = lin(G, lx + i, ly + j, lz + k);
+    const float v = __ldg(ie + p);
+    out[t] = -__ldg(g + p) * delta_eps * v * v;
+}
+
+inline dim3 vol_grid(const Dims &G) { return dim3((G.nx + BX - 1) / BX, (G.ny + BY - 1) / BY, G.nz); }
+inline dim3 vol_block() { return dim3(BX, BY, 1); }
+
+}  // namespace
+
+void launch_update_E(const Dims &G, const Tables &T, float *fields, const float *ie, PsiSet psiE, cudaStream_t st)
+{
+    if (G.periodic) k_update_E<true><<<vol_grid(G), vol_block(), 0, st>>>(G, T, fields, ie, psiE);
+    else            k_update_E<false><<<vol_grid(G), vol_block(), 0, st>>>(G, T, fields, ie, psiE);
+}
+
+void launch_update_H(const Dims &G, const Tables &T, float *fields, const float *im, PsiSet psiH, cudaStream_t st)
+{
+    if (G.periodic) k_update_H<true><<<vol_grid(G), vol_block(), 0, st>>>(G, T, fields, im, psiH);
+    else            k_update_H<false><<<vol_grid(G), vol_block(), 0, st>>>(G, T, fields, im, psiH);
+}
+
+void launch_add_source(const Dims &G, float *fields, const SourceDev &s, const int *step, float sign, cudaStream_t st)
+{
+    const long long n = (long long)(s.hi[0] - s.lo[0]) * (s.hi[1] - s.lo[1]) * (s.hi[2] - s.lo[2]);
+    k_add_source<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(G, fields, s, step, sign);
+}
+
+void launch_detector(const Dims &G, const float *fields, const DetectorDev &dt, const float *cs_table,
+                     int total_freq, const int *step, cudaStream_t st)
+{
+    const long long n = (long long)(dt.hi[0] - dt.lo[0]) * (dt.hi[1] - dt.lo[1]) * (dt.hi[2] - dt.lo[2]);
+    k_detector<false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(G, const_cast<float *>(fields), dt, cs_table, total_freq, step);
+}
+
+void launch_detector_adjoint(const Dims &G, float *lam, const DetectorDev &dt, const float *cs_table,
+                             int total_freq, const int *step, cudaStream_t st)
+{
+    const long long n = (long long)(dt.hi[0] - dt.lo[0]) * (dt.hi[1] - dt.lo[1]) * (dt.hi[2] - dt.lo[2]);
+    k_detector<true><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(G, lam, dt, cs_table, total_freq, step);
+}
+
+void launch_record(const Dims &G, const RecLayout &R, const float *fields_H, const float *fields_E,
+                   float *rec, const int *step, cudaStream_t st)
+{
+    if (R.stride == 0) return;
+    k_record<false><<<(unsigned)((R.stride + 255) / 256), 256, 0, st>>>(G, R, fields_H, fields_E, nullptr, rec, step);
+}
+
+void launch_inject(const Dims &G, const RecLayout &R, float *fields, const float *rec, const int *step, cudaStream_t st)
+{
+    if (R.stride == 0) return;
+    k_record<true><<<(unsigned)((R.stride + 255) / 256), 256, 0, st>>>(G, R, nullptr, nullptr, fields, const_cast<float *>(rec), step);
+}
+
+void launch_advance(int *step, int delta, cudaStream_t st) { k_advance<<<1, 1, 0, st>>>(step, delta); }
+
+void launch_adj_H(const Dims &G, const Tables &T, float *lam, const float *im, PsiSet s0, PsiSet s1,
+                  const int *step, cudaStream_t st)
+{
+    if (G.periodic) k_adjoint<1, true><<<vol_grid(G), vol_block(), 0, st>>>(G, T, lam, im, s0, s1, step);
+    else            k_adjoint<1, false><<<vol_grid(G), vol_block(), 0, st>>>(G, T, lam, im, s0, s1, step);
+}
+
+void launch_adj_E(const Dims &G, const Tables &T, float *lam, const float *ie, PsiSet s0, PsiSet s1,
+                  const int *step, cudaStream_t st)
+{
+    if (G.periodic) k_adjoint<0, true><<<vol_grid(G), vol_block(), 0, st>>>(G, T, lam, ie, s0, s1, step);
+    else            k_adjoint<0, false><<<vol_grid(G), vol_block(), 0, st>>>(G, T, lam, ie, s0, s1, step);
+}
+
+void launch_grad_rho(const Dims &G, const float *g, const float *ie, float delta_eps, const int lo[3], const int hi[3],
+                     float *out, cudaStream_t st)
+{
+    const int bx = hi[0] - lo[0], by = hi[1] - lo[1], bz = hi[2] - lo[2];
+    const long long n = (long long)bx * by * bz;
+    k_grad_rho<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(G, g, ie, delta_eps, lo[0], lo[1], lo[2], bx, by, bz, out);
+}
+
+void launch_inv_H(const Dims &G, float *fields, const float *im, cudaStream_t st)
+{
+    if (G.periodic) k_inv_H<true><<<vol_grid(G), vol_block(), 0, st>>>(G, fields, im);
+    else            k_inv_H<false><<<vol_grid(G), vol_block(), 0, st>>>(G, fields, im);
+}
+
+void launch_inv_E_grad(const Dims &G, float *fields, const float *ie, const float *lam, float *g, cudaStream_t st)
+{
+    if (G.periodic) k_inv_E_grad<true><<<vol_grid(G), vol_block(), 0, st>>>(G, fields, ie, lam, g);
+    else            k_inv_E_grad<false><<<vol_grid(G), vol_block(), 0, st>>>(G, fields, ie, lam, g);
+}
+
+}  // namespace fdtd

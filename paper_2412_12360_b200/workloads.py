@@ -40,7 +40,10 @@ class Detector:
     component_mask: int
     lo: Tuple[int, int, int]
     hi: Tuple[int, int, int]
-    omega: Sequence[float]               # rad / step
+    omega: Sequence[float]               # rad / step (rounded to fp32 so both sides see the same value)
+
+    def __post_init__(self):
+        self.omega = [float(np.float32(o)) for o in self.omega]
 
     @property
     def n_comp(self) -> int:
@@ -173,6 +176,30 @@ def c3(n: int = 200, d: int = 12, n_steps: int = 2000, seed: int = 3) -> Workloa
                     meta={"rho": rho, "delta_eps": 12.25 - 2.085})
 
 
+def c3_mini(nx: int = 88, ny: int = 52, nz: int = 44, d: int = 8, n_steps: int = 120, seed: int = 33,
+            kappa_max: float = 0.0, alpha_max: float = 0.0) -> Workload:
+    """Non-cubic miniature of C3 (ragged tile tails on every axis) that the oracle finishes in seconds:
+    cladding eps=2.085, random design block, Gaussian-profile Ey source plane, Ey+Hx DFT plane."""
+    eps_bg = np.float32(2.085)
+    eps = np.full((nz, ny, nx), eps_bg, dtype=np.float32)
+    x0, x1 = d + (nx - 2 * d) // 4, nx - d - (nx - 2 * d) // 4
+    y0, y1 = d + (ny - 2 * d) // 4, ny - d - (ny - 2 * d) // 4
+    z0, z1 = d + (nz - 2 * d) // 3, nz - d - (nz - 2 * d) // 3
+    rho = np.random.default_rng(seed).random((z1 - z0, y1 - y0, x1 - x0), dtype=np.float32)
+    eps[z0:z1, y0:y1, x0:x1] = eps_bg + np.float32(12.25 - 2.085) * rho
+    ks, kd = d + 2, nz - d - 3
+    lo, hi = (d, d, ks), (nx - d, ny - d, ks + 1)
+    prof = gaussian_profile(lo, hi, ((nx - 1) / 2.0, (ny - 1) / 2.0), 0.15 * nx)
+    wav = gaussian_sine(n_steps, 30, 10, 12)
+    src = Source(1, lo, hi, wav, prof)
+    det = Detector((1 << 1) | (1 << 3), (d, d, kd), (nx - d, ny - d, kd + 1), [omega_ppw(12), omega_ppw(14)])
+    return Workload("C3-mini", nx, ny, nz, n_steps, _inv(eps), [src], [det], pml_cells=d,
+                    pml_eps_bg=2.085, pml_kappa_max=kappa_max, pml_alpha_max=alpha_max,
+                    loss="phasor_power", loss_detectors=(0,),
+                    design_lo=(x0, y0, z0), design_hi=(x1, y1, z1), eps=eps,
+                    meta={"rho": rho, "delta_eps": 12.25 - 2.085})
+
+
 def c4(nx: int = 800, ny: int = 800, nz: int = 600, d: int = 16, n_steps: int = 5000,
        seed: int = 4) -> Workload:
     """configs[3]: memory-scale run; binary 4x4x4 blocks in the design region, 2 detector planes,
@@ -222,11 +249,14 @@ def tiny_pml(nx=14, ny=13, nz=12, d=3, n_steps=30, seed=7, kappa_max=3.0, alpha_
     mu = (np.float32(1.0) + np.float32(0.5) * rng.random((nz, ny, nx), dtype=np.float32)).astype(np.float32)
     wavE = gaussian_sine(n_steps, 8, 3, 7)
     wavH = (0.5 * gaussian_sine(n_steps, 10, 4, 9)).astype(np.float32)
-    lo, hi = (d + 1, d, d + 2), (nx - d - 1, ny - d, d + 3)
+    wide = nx - 2 * d >= 3
+    ks = min(d + 2, nz - d - 1)
+    lo, hi = (d + 1 if wide else d, d, ks), (nx - d - 1 if wide else nx - d, ny - d, ks + 1)
     prof = (0.5 + rng.random((1, hi[1] - lo[1], hi[0] - lo[0]), dtype=np.float32)).astype(np.float32)
     srcs = [Source(1, lo, hi, wavE, prof),
             Source(3, (nx // 2, ny // 2, nz // 2), (nx // 2 + 1, ny // 2 + 1, nz // 2 + 1), wavH)]
-    det = Detector((1 << 1) | (1 << 3), (d, d, nz - d - 2), (nx - d, ny - d, nz - d - 1),
+    kd = max(d, nz - d - 2)
+    det = Detector((1 << 1) | (1 << 3), (d, d, kd), (nx - d, ny - d, kd + 1),
                    [omega_ppw(7), omega_ppw(9)])
     w = Workload("tiny", nx, ny, nz, n_steps, _inv(eps), srcs, [det], pml_cells=d,
                  pml_kappa_max=kappa_max, pml_alpha_max=alpha_max, loss="phasor_power",

@@ -1,0 +1,297 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 CPU oracle, element by element on
+the same seeded fp32 inputs.  Error metric (reading R19): max-norm relative per group,
+max|x_gpu - x_ref| / max|x_ref|.  Tolerances (BASELINE.json north_star / SURVEY 8(c)):
+fields <= 1e-5 after 100 fp32 steps, phasors <= 1e-4, gradient <= 1e-3.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2412_12360_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL_FIELD, TOL_PHASOR, TOL_GRAD = 1e-5, 1e-4, 1e-3
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device")
+    from paper_2412_12360_b200 import binding
+    return binding
+
+
+def relerr(x, ref):
+    ref = np.asarray(ref, dtype=np.float64)
+    x = np.asarray(x, dtype=np.float64)
+    den = np.max(np.abs(ref))
+    return float(np.max(np.abs(x - ref)) / den) if den > 0 else float(np.max(np.abs(x)))
+
+
+def paths(B, w):
+    """Kernel paths to test on this workload."""
+    out = [B.FDTD_PATH_GENERIC]
+    if not w.periodic and w.nx % 4 == 0 and os.environ.get("FDTD_TEST_PATHS", "all") != "generic":
+        out.append(B.FDTD_PATH_FUSED)
+    return out
+
+
+def loss_cotangents(w, fields, phasors, interior_only=False):
+    """Returns (dL_dphasor list | None, dL_dfields | None) for the workload's loss; works on numpy
+    (oracle, fp64) and on torch tensors (GPU) alike."""
+    if w.loss == "phasor_power":
+        return [2.0 * P if i in w.loss_detectors else None for i, P in enumerate(phasors)], None
+    if w.loss in ("final_E2", "final_E2_interior"):
+        dLf = fields * 0
+        if w.loss == "final_E2":
+            dLf[:3] = 2.0 * fields[:3]
+        else:
+            d = w.pml_cells
+            sl = (slice(0, 3), slice(d, w.nz - d), slice(d, w.ny - d), slice(d, w.nx - d))
+            dLf[sl] = 2.0 * fields[sl]
+        return None, dLf
+    return None, None
+
+
+def run_oracle(w, n_steps=None, backward=True, f0=None):
+    from oracle.oracle import Oracle
+    n = w.n_steps if n_steps is None else n_steps
+    o = Oracle(**w.grid_kwargs())
+    f = np.zeros((6, w.nz, w.ny, w.nx)) if f0 is None else f0.astype(np.float64).copy()
+    out = o.forward(f, w.inv_eps, w.meta.get("inv_mu"), w.sources, w.detectors, n, record=backward and w.pml_cells > 0)
+    res = {"fields": f.copy(), "phasors": out["phasors"]}
+    if backward:
+        dLp, dLf = loss_cotangents(w, f, out["phasors"])
+        g, lam0 = o.backward(f, w.inv_eps, w.meta.get("inv_mu"), w.sources, w.detectors, dLp, dLf, n, out["rec"])
+        res.update(grad=g, lam0=lam0, state0=f)
+    return res
+
+
+def run_gpu(B, w, path, n_steps=None, backward=True, f0=None, grad_box=None):
+    import torch
+    n = w.n_steps if n_steps is None else n_steps
+    kw = w.grid_kwargs()
+    kw.update(max_steps=n, record=backward and w.pml_cells > 0, path=path)
+    if grad_box:
+        kw.update(grad_lo=grad_box[0], grad_hi=grad_box[1])
+    g = B.Grid(**kw)
+    f = torch.zeros((6, w.nz, w.ny, w.nx), dtype=torch.float32, device="cuda")
+    if f0 is not None:
+        f.copy_(torch.as_tensor(f0, dtype=torch.float32))
+    ie = torch.as_tensor(w.inv_eps).cuda()
+    im = None if w.meta.get("inv_mu") is None else torch.as_tensor(w.meta["inv_mu"]).cuda()
+    ph = g.forward(f, ie, im, w.sources, w.detectors, n)
+    torch.cuda.synchronize()
+    res = {"fields": f.cpu().numpy(), "phasors": [p.cpu().numpy() for p in ph], "info": g.info()}
+    if backward:
+        dLp, dLf = loss_cotangents(w, f, ph)
+        grad, lam0 = g.backward(f, ie, im, w.sources, w.detectors, dLp, dLf, n, want_dL_dfields0=True)
+        torch.cuda.synchronize()
+        res.update(grad=grad.cpu().numpy(), lam0=lam0.cpu().numpy(), state0=f.cpu().numpy())
+    g.close()
+    return res
+
+
+def interior(w, a):
+    d = w.pml_cells
+    return a[..., d:w.nz - d, d:w.ny - d, d:w.nx - d]
+
+
+def compare(w, gpu, ref, backward=True, tol_field=TOL_FIELD):
+    errs = {"E": relerr(gpu["fields"][:3], ref["fields"][:3]), "H": relerr(gpu["fields"][3:], ref["fields"][3:])}
+    assert errs["E"] <= tol_field and errs["H"] <= tol_field, errs
+    for i, (P, Pr) in enumerate(zip(gpu["phasors"], ref["phasors"])):
+        errs[f"P{i}"] = relerr(P, Pr)
+        assert errs[f"P{i}"] <= TOL_PHASOR, errs
+    if backward:
+        errs["grad"] = relerr(gpu["grad"], ref["grad"])
+        errs["lam0"] = relerr(gpu["lam0"], ref["lam0"])
+        assert errs["grad"] <= TOL_GRAD and errs["lam0"] <= TOL_GRAD, errs
+        # reconstructed state 0 on I: absolute residue against the largest field seen at state n
+        scale = max(np.max(np.abs(ref["fields"])), 1e-30)
+        errs["state0"] = float(np.max(np.abs(interior(w, gpu["state0"]) - interior(w, ref["state0"]))) / scale)
+        assert errs["state0"] <= 1e-4, errs
+    return errs
+
+
+# ------------------------------------------------------------------------------------------------
+def test_c1_periodic_forward_and_gradient(B):
+    """configs[0]: 16^3 periodic, 100 steps, loss = sum E^2, gradient wrt inv_eps (all 4096 voxels)."""
+    w = wl.c1()
+    ref = run_oracle(w)
+    gpu = run_gpu(B, w, B.FDTD_PATH_GENERIC)
+    errs = compare(w, gpu, ref)
+    assert gpu["info"].path == B.FDTD_PATH_GENERIC
+    assert np.max(np.abs(gpu["state0"])) < 1e-4 * np.max(np.abs(ref["fields"]))   # state 0 was all zero
+    print("C1", errs)
+
+
+@pytest.mark.parametrize("kappa,alpha,with_mu", [(3.0, 0.05, True), (0.0, 0.0, False)])
+def test_tiny_pml_every_term(B, kappa, alpha, with_mu):
+    """14x13x12, d=3: kappa/alpha CPML, E and H sources, inv_mu, 2 components x 2 frequencies.
+    nx is not a multiple of 4, so this is the generic path only."""
+    w = wl.tiny_pml(n_steps=60, kappa_max=kappa, alpha_max=alpha, with_inv_mu=with_mu)
+    ref = run_oracle(w)
+    gpu = run_gpu(B, w, B.FDTD_PATH_GENERIC)
+    print("tiny", compare(w, gpu, ref))
+
+
+@pytest.mark.parametrize("kappa,alpha", [(0.0, 0.0), (3.0, 0.05)])
+def test_c3_mini_all_paths(B, kappa, alpha):
+    """88x52x44 miniature of the graded config: several tiles and ragged tails on every axis;
+    forward fields + phasors + reversible gradient + cotangent of state 0, every kernel path."""
+    w = wl.c3_mini(kappa_max=kappa, alpha_max=alpha)
+    ref = run_oracle(w)
+    for path in paths(B, w):
+        gpu = run_gpu(B, w, path)
+        assert gpu["info"].path == path
+        print("c3-mini path", path, compare(w, gpu, ref))
+
+
+def test_c3_mini_with_inv_mu_and_h_source(B):
+    w = wl.c3_mini(nx=64, ny=40, nz=36, d=6, n_steps=80)
+    rng = np.random.default_rng(5)
+    w.meta["inv_mu"] = (np.float32(1) / (np.float32(1) + np.float32(0.5) * rng.random((w.nz, w.ny, w.nx), dtype=np.float32))).astype(np.float32)
+    w.sources.append(wl.Source(3, (20, 12, 14), (30, 20, 16), (0.3 * wl.gaussian_sine(80, 20, 8, 10)).astype(np.float32)))
+    ref = run_oracle(w)
+    for path in paths(B, w):
+        print("c3-mini mu", path, compare(w, run_gpu(B, w, path), ref))
+
+
+def test_c2_fields_at_100_200_and_phasor_at_1000(B):
+    """configs[1]: 64^3, d=10, eps block, Ey plane source, Ey DFT plane; forward only."""
+    w = wl.c2()
+    for n in (100, 200):
+        ref = run_oracle(w, n_steps=n, backward=False)
+        for path in paths(B, w):
+            print("C2", n, path, compare(w, run_gpu(B, w, path, n_steps=n, backward=False), ref, backward=False))
+    ref = run_oracle(w, n_steps=1000, backward=False)
+    for path in paths(B, w):
+        gpu = run_gpu(B, w, path, n_steps=1000, backward=False)
+        e = relerr(gpu["phasors"][0], ref["phasors"][0])
+        assert e <= TOL_PHASOR, e
+        print("C2 phasor", path, e)
+
+
+def test_c5_small_sweep_point(B):
+    """configs[4] at N=64 (d=10, random eps extruded into the PML, dipole, loss = sum E^2 over I)."""
+    w = wl.c5(64, n_steps=150)
+    ref = run_oracle(w)
+    for path in paths(B, w):
+        print("C5-64", path, compare(w, run_gpu(B, w, path), ref))
+
+
+# ------------------------------------------------------------------------------------------------ edge cases
+def test_zero_steps_and_walls_without_pml(B):
+    import torch
+    w = wl.c3_mini(nx=24, ny=20, nz=16, d=0, n_steps=40)
+    w.loss, w.loss_detectors = "final_E2", ()
+    ref = run_oracle(w)
+    for path in paths(B, w):
+        print("walls", path, compare(w, run_gpu(B, w, path), ref))
+    # n_steps = 0: fields untouched, gradient zero
+    f0 = np.random.default_rng(1).standard_normal((6, w.nz, w.ny, w.nx)).astype(np.float32)
+    gpu = run_gpu(B, w, B.FDTD_PATH_GENERIC, n_steps=0, f0=f0)
+    assert np.array_equal(gpu["fields"], f0) and np.all(gpu["grad"] == 0)
+    assert np.array_equal(gpu["lam0"][:3], 2 * f0[:3])
+
+
+def test_minimum_grid_2d_plus_2(B):
+    d = 3
+    w = wl.tiny_pml(nx=2 * d + 2, ny=2 * d + 2, nz=2 * d + 2, d=d, n_steps=25, with_inv_mu=False)
+    ref = run_oracle(w)
+    for path in paths(B, w):
+        print("min grid", path, compare(w, run_gpu(B, w, path), ref))
+
+
+def test_nonzero_initial_state(B):
+    w = wl.c3_mini(nx=40, ny=36, nz=32, d=6, n_steps=50)
+    f0 = (0.1 * np.random.default_rng(2).standard_normal((6, w.nz, w.ny, w.nx))).astype(np.float32)
+    ref = run_oracle(w, f0=f0)
+    for path in paths(B, w):
+        print("f0", path, compare(w, run_gpu(B, w, path, f0=f0), ref))
+
+
+def test_grad_box_restricts_the_gradient(B):
+    w = wl.c3_mini(nx=40, ny=36, nz=32, d=6, n_steps=50)
+    ref = run_oracle(w)
+    lo, hi = w.design_lo, w.design_hi
+    for path in paths(B, w):
+        gpu = run_gpu(B, w, path, grad_box=(lo, hi))
+        box = (slice(lo[2], hi[2]), slice(lo[1], hi[1]), slice(lo[0], hi[0]))
+        assert relerr(gpu["grad"][box], ref["grad"][box]) <= TOL_GRAD
+        mask = np.ones_like(gpu["grad"], bool)
+        mask[box] = False
+        assert np.all(gpu["grad"][mask] == 0)
+
+
+def test_error_codes_on_device(B):
+    import torch
+    w = wl.c3_mini(nx=24, ny=20, nz=20, d=4, n_steps=5)
+    kw = w.grid_kwargs()
+    kw.update(max_steps=5, record=False)
+    g = B.Grid(**kw)
+    f = torch.zeros((6, w.nz, w.ny, w.nx), device="cuda")
+    ie = torch.as_tensor(w.inv_eps).cuda()
+    with pytest.raises(B.FdtdError) as ei:
+        g.forward(f, ie, None, w.sources, w.detectors, 6)            # n_steps > max_steps
+    assert ei.value.code == B.FDTD_EINVAL
+    bad = wl.Source(1, (0, 0, 0), (w.nx + 1, 1, 1), w.sources[0].waveform)
+    with pytest.raises(B.FdtdError) as ei:
+        g.forward(f, ie, None, [bad], [], 5)
+    assert ei.value.code == B.FDTD_EINVAL
+    g.forward(f, ie, None, w.sources, w.detectors, 5)
+    with pytest.raises(B.FdtdError) as ei:
+        g.backward(f, ie, None, w.sources, w.detectors, None, None, 5)   # CPML grid, nothing recorded
+    assert ei.value.code == B.FDTD_ESTATE
+    g.close()
+    kw.update(record=True)
+    g = B.Grid(**kw)
+    g.forward(f, ie, None, w.sources, w.detectors, 4)
+    with pytest.raises(B.FdtdError) as ei:
+        g.backward(f, ie, None, w.sources, w.detectors, None, None, 5)   # different n_steps
+    assert ei.value.code == B.FDTD_ESTATE
+    g.close()
+
+
+def test_translation_invariance_bitwise_periodic(B):
+    """P12: on a periodic grid, shifting eps and the source shifts the fields bit for bit."""
+    import torch
+    w = wl.c1(n=16, n_steps=60)
+    sx, sy, sz = 5, 3, 7
+    a = run_gpu(B, w, B.FDTD_PATH_GENERIC, backward=False)["fields"]
+    w2 = wl.c1(n=16, n_steps=60)
+    w2.inv_eps = np.roll(w.inv_eps, (sz, sy, sx), axis=(0, 1, 2)).copy()
+    s = w.sources[0]
+    lo = ((s.lo[0] + sx) % 16, (s.lo[1] + sy) % 16, (s.lo[2] + sz) % 16)
+    w2.sources = [wl.Source(s.component, lo, (lo[0] + 1, lo[1] + 1, lo[2] + 1), s.waveform)]
+    b = run_gpu(B, w2, B.FDTD_PATH_GENERIC, backward=False)["fields"]
+    assert np.array_equal(np.roll(a, (sz, sy, sx), axis=(1, 2, 3)), b)
+
+
+def test_translation_invariance_bitwise_before_the_walls(B):
+    """Tile-edge check for every path: in a zero-padded box, before anything reaches a wall, shifting
+    the medium and the source by a vector that is not a multiple of any tile size shifts the result
+    bit for bit (per-cell arithmetic does not depend on the position inside a tile)."""
+    nx, ny, nz, n = 96, 80, 72, 16
+    rng = np.random.default_rng(8)
+    blob = (np.float32(1) / (np.float32(1) + np.float32(3) * rng.random((24, 24, 24), dtype=np.float32))).astype(np.float32)
+    wav = wl.gaussian_sine(n, 6, 3, 8)
+
+    def make(off):
+        ie = np.ones((nz, ny, nx), dtype=np.float32)
+        ie[off[2]:off[2] + 24, off[1]:off[1] + 24, off[0]:off[0] + 24] = blob
+        c = (off[0] + 12, off[1] + 12, off[2] + 12)
+        w = wl.Workload("shift", nx, ny, nz, n, ie, [wl.Source(2, c, (c[0] + 1, c[1] + 1, c[2] + 1), wav)], [])
+        return w
+
+    o1, o2 = (20, 22, 21), (20 + 29, 22 + 11, 21 + 6)
+    for path in paths(B, make(o1)):
+        a = run_gpu(B, make(o1), path, backward=False)["fields"]
+        b = run_gpu(B, make(o2), path, backward=False)["fields"]
+        assert np.max(np.abs(a)) > 0
+        sh = np.roll(a, (o2[2] - o1[2], o2[1] - o1[1], o2[0] - o1[0]), axis=(1, 2, 3))
+        assert np.array_equal(sh, b), path
