@@ -203,18 +203,22 @@ extern "C" int fdtd_create_grid(const fdtd_grid_desc *desc, fdtd_grid **out)
         const double am = desc->pml_alpha_m > 0 ? desc->pml_alpha_m : 1.0;
         const double eb = desc->pml_eps_bg > 0 ? desc->pml_eps_bg : 1.0;
         const double smax = ss / std::sqrt(eb);
-        const int tot = 6 * (G.nx + G.ny + G.nz);
+        // every table is padded to a multiple of 4 floats plus 4 tail entries (b=1, a=0, ik=1) so that the
+        // fused kernels can read float4s and index N (the first cell outside the grid)
+        auto padded = [](int n) { return (n + 4 + 3) / 4 * 4; };
+        const int tot = 6 * (padded(G.nx) + padded(G.ny) + padded(G.nz));
         std::vector<float> h(tot);
         float *dev = nullptr;
         if ((rc = g->alloc((void **)&dev, tot * sizeof(float)))) return bail(rc);
         int off = 0;
         for (int fam = 0; fam < 2; ++fam)
             for (int a = 0; a < 3; ++a) {
-                const int n = dim_of(G, a);
+                const int n = dim_of(G, a), np = padded(n);
+                for (int q = 0; q < np; ++q) { h[off + q] = 1.f; h[off + np + q] = 0.f; h[off + 2 * np + q] = 1.f; }
                 make_table(n, G.d, fam, (double)G.S, m, smax, km, (double)desc->pml_alpha_max, am,
-                           &h[off], &h[off + n], &h[off + 2 * n]);
-                g->T.b[fam][a] = dev + off; g->T.a[fam][a] = dev + off + n; g->T.ik[fam][a] = dev + off + 2 * n;
-                off += 3 * n;
+                           &h[off], &h[off + np], &h[off + 2 * np]);
+                g->T.b[fam][a] = dev + off; g->T.a[fam][a] = dev + off + np; g->T.ik[fam][a] = dev + off + 2 * np;
+                off += 3 * np;
             }
         cudaError_t e = cudaMemcpy(dev, h.data(), tot * sizeof(float), cudaMemcpyHostToDevice);
         if (e != cudaSuccess) return bail(cuda_fail(e, "upload CPML tables"));
@@ -461,6 +465,19 @@ int run_steps(fdtd_grid *g, fdtd_grid::GraphCache &gc, const std::string &key, i
     return FDTD_OK;
 }
 
+}  // namespace
+int fdtd_run_steps_fwd(fdtd_grid *g, const std::string &key, int n_steps, int launches_per_step, cudaStream_t st,
+                       void (*enqueue)(void *, cudaStream_t), void *ctx)
+{
+    return run_steps(g, g->fwd_graph, key, n_steps, launches_per_step, st, [&](cudaStream_t cs) { enqueue(ctx, cs); });
+}
+int fdtd_run_steps_bwd(fdtd_grid *g, const std::string &key, int n_steps, int launches_per_step, cudaStream_t st,
+                       void (*enqueue)(void *, cudaStream_t), void *ctx)
+{
+    return run_steps(g, g->bwd_graph, key, n_steps, launches_per_step, st, [&](cudaStream_t cs) { enqueue(ctx, cs); });
+}
+namespace {
+
 std::string make_key(const char *tag, const void *a, const void *b, const void *c, const void *d, const void *e,
                      const std::vector<SourceDev> &S, const std::vector<DetectorDev> &D, int extra)
 {
@@ -567,7 +584,7 @@ extern "C" int fdtd_backward(fdtd_grid *g, float *fields, const float *inv_eps, 
     CK(cudaMemsetAsync(g->d_step, 0, sizeof(int), st));
     if (n_steps > 0) launch_advance(g->d_step, n_steps - 1, st);
 
-    if (g->path == FDTD_PATH_FUSED) {
+    if (g->path == FDTD_PATH_FUSED && g->fused_backward_ready) {
         rc = fused_backward(g, fields, inv_eps, inv_mu, S, D, total_freq, n_steps, dL_dinv_eps, st);
         if (rc) return rc;
     } else {

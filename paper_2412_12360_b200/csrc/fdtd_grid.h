@@ -16,6 +16,7 @@ struct fdtd_grid {
     int path = FDTD_PATH_GENERIC;
     int tile_x = 0, tile_y = 0, tile_z = 0;
     std::string fused_why_not;
+    bool fused_backward_ready = false;    // false: fdtd_backward uses the generic reverse kernels
     int graph_unroll = 8;
 
     // device memory owned by the grid

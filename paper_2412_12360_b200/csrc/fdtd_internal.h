@@ -108,6 +108,11 @@ void launch_detector_adjoint(const Dims &G, float *lam, const DetectorDev &dt, c
 // H source: fields that hold the pre-step H (low faces); E source: fields that hold the post-E-update E'
 void launch_record(const Dims &G, const RecLayout &R, const float *fields_H, const float *fields_E,
                    float *rec, const int *step, cudaStream_t st);
+// ping-pong variants for the fused path (buffers picked by step parity inside the kernel)
+void launch_record_pp(const Dims &G, const RecLayout &R, const float *bufA, const float *bufB, float *rec,
+                      const int *step, cudaStream_t st);
+void launch_inject_pp(const Dims &G, const RecLayout &R, float *bufA, float *bufB, const float *rec,
+                      const int *step, cudaStream_t st);
 void launch_inject(const Dims &G, const RecLayout &R, float *fields, const float *rec, const int *step, cudaStream_t st);
 void launch_advance(int *step, int delta, cudaStream_t st);
 // psi cotangents are ping-ponged by step parity: read set[n&1], write set[(n&1)^1]

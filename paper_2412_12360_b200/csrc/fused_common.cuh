@@ -1,0 +1,108 @@
+// fused_common.cuh -- PTX wrappers (TMA, mbarrier, named barriers) and shared structures of the
+// fused z-marching kernels.  sm_100a only.
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "fdtd_internal.h"
+
+namespace fdtd {
+
+// ------------------------------------------------------------------------------------------------
+// Work decomposition: the xy plane is cut into TX x TY tiles; each tile's z column is cut into
+// segments; a persistent CTA marches its list of segments plane by plane.
+// ------------------------------------------------------------------------------------------------
+struct Segment {
+    int i0, j0;       // tile origin
+    int k0, k1;       // planes [k0, k1) owned by this segment
+    int flags;        // SEG_X_LO | SEG_X_HI | SEG_Y_LO | SEG_Y_HI : which CPML slabs the tile touches
+    int xbase;        // first x of the x-slab psi box (see kernels_fused.cu)
+    int pad[2];
+};
+enum { SEG_X_LO = 1, SEG_X_HI = 2, SEG_Y_LO = 4, SEG_Y_HI = 8 };
+
+// logical arrays of one pipeline stage
+enum StageArray {
+    SA_EX = 0, SA_EY, SA_EZ, SA_HX, SA_HY, SA_HZ, SA_IE, SA_IM,
+    SA_PE_Y0, SA_PE_Y1,     // psi_E of the y axis: psiE_x0, psiE_z1
+    SA_PE_Z0, SA_PE_Z1,     // psi_E of the z axis: psiE_y0, psiE_x1
+    SA_PH_Y0, SA_PH_Y1,     // psi_H of the y axis: psiH_x0, psiH_z1      (lagging plane)
+    SA_PH_Z0, SA_PH_Z1,     // psi_H of the z axis: psiH_y0, psiH_x1      (lagging plane)
+    SA_PE_X0, SA_PE_X1,     // psi_E of the x axis: psiE_z0, psiE_y1      (narrow boxes)
+    SA_PH_X0, SA_PH_X1,     // psi_H of the x axis: psiH_z0, psiH_y1      (narrow boxes, lagging plane)
+    SA_COUNT
+};
+
+// tensor-map table (device memory, 64 B aligned entries); index helpers
+enum {
+    TM_FIELD = 0,                 // + set*6 + comp                     (12)
+    TM_IE = 12, TM_IM = 13,
+    TM_PSI = 14,                  // + set*20 + family*10 + local       (40)
+    TM_COUNT = 54
+};
+// local index inside a (set, family) block of 10 maps:
+//   0,1: x axis arrays (c=z,s=0),(c=y,s=1) low view ; 2,3: same, high view
+//   4,5: y axis arrays (c=x,s=0),(c=z,s=1) low view ; 6,7: same, high view
+//   8,9: z axis arrays (c=y,s=0),(c=x,s=1)
+__host__ __device__ inline int tm_psi(int set, int family, int local) { return TM_PSI + set * 20 + family * 10 + local; }
+
+// ------------------------------------------------------------------------------------------------
+// PTX wrappers
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init()
+{
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void fence_proxy_async()
+{
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    uint32_t ok;
+    do {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n" : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!ok);
+}
+// 3-D tiled TMA load: box at (x, y, z) of the tensor described by *tm into smem, completing on bar
+__device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *tm, int x, int y, int z, uint64_t *bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+        ::"r"(smem_u32(dst)), "l"(tm), "r"(x), "r"(y), "r"(z), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+__device__ __forceinline__ float4 operator+(float4 a, float4 b) { return make_float4(a.x + b.x, a.y + b.y, a.z + b.z, a.w + b.w); }
+__device__ __forceinline__ float4 operator-(float4 a, float4 b) { return make_float4(a.x - b.x, a.y - b.y, a.z - b.z, a.w - b.w); }
+__device__ __forceinline__ float4 operator*(float4 a, float4 b) { return make_float4(a.x * b.x, a.y * b.y, a.z * b.z, a.w * b.w); }
+__device__ __forceinline__ float4 operator*(float s, float4 b) { return make_float4(s * b.x, s * b.y, s * b.z, s * b.w); }
+__device__ __forceinline__ float4 splat(float s) { return make_float4(s, s, s, s); }
+// backward difference along x inside a float4: (v.x - left, v.y - v.x, v.z - v.y, v.w - v.z)
+__device__ __forceinline__ float4 dminus_x(float4 v, float left) { return make_float4(v.x - left, v.y - v.x, v.z - v.y, v.w - v.z); }
+// forward difference along x inside a float4: (v.y - v.x, v.z - v.y, v.w - v.z, right - v.w)
+__device__ __forceinline__ float4 dplus_x(float4 v, float right) { return make_float4(v.y - v.x, v.z - v.y, v.w - v.z, right - v.w); }
+
+}  // namespace fdtd

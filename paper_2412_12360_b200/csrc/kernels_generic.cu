@@ -156,12 +156,21 @@ __global__ void k_detector(Dims G, float *__restrict__ f, DetectorDev dt, const 
 
 // ------------------------------------------------------------------------------------------ F8
 // One thread per float of a step's record.  INJECT=false: fields -> rec[n]; true: rec[n] -> fields.
-template <bool INJECT>
+// PP=true (fused ping-pong path): fH/fE are the two field buffers A/B; step n read buffer n&1 (pre-step H)
+// and wrote buffer (n+1)&1 (E'); for INJECT the target is buffer (n+1)&1 (the state the reverse step reads).
+template <bool INJECT, bool PP>
 __global__ void k_record(Dims G, RecLayout R, const float *__restrict__ fH, const float *__restrict__ fE,
                          float *__restrict__ fout, float *__restrict__ rec, const int *__restrict__ step)
 {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= R.stride) return;
+    if (PP) {
+        const float *A = fH, *B = fE;
+        const int par = (*step) & 1;
+        fH = par ? B : A;
+        fE = par ? A : B;
+        fout = const_cast<float *>(fE);
+    }
     // locate the segment
     int a = 0, side = 0, which = 0;
     long long local = -1;
@@ -403,13 +412,27 @@ void launch_record(const Dims &G, const RecLayout &R, const float *fields_H, con
                    float *rec, const int *step, cudaStream_t st)
 {
     if (R.stride == 0) return;
-    k_record<false><<<(unsigned)((R.stride + 255) / 256), 256, 0, st>>>(G, R, fields_H, fields_E, nullptr, rec, step);
+    k_record<false, false><<<(unsigned)((R.stride + 255) / 256), 256, 0, st>>>(G, R, fields_H, fields_E, nullptr, rec, step);
+}
+
+void launch_record_pp(const Dims &G, const RecLayout &R, const float *bufA, const float *bufB, float *rec,
+                      const int *step, cudaStream_t st)
+{
+    if (R.stride == 0) return;
+    k_record<false, true><<<(unsigned)((R.stride + 255) / 256), 256, 0, st>>>(G, R, bufA, bufB, nullptr, rec, step);
+}
+
+void launch_inject_pp(const Dims &G, const RecLayout &R, float *bufA, float *bufB, const float *rec,
+                      const int *step, cudaStream_t st)
+{
+    if (R.stride == 0) return;
+    k_record<true, true><<<(unsigned)((R.stride + 255) / 256), 256, 0, st>>>(G, R, bufA, bufB, nullptr, const_cast<float *>(rec), step);
 }
 
 void launch_inject(const Dims &G, const RecLayout &R, float *fields, const float *rec, const int *step, cudaStream_t st)
 {
     if (R.stride == 0) return;
-    k_record<true><<<(unsigned)((R.stride + 255) / 256), 256, 0, st>>>(G, R, nullptr, nullptr, fields, const_cast<float *>(rec), step);
+    k_record<true, false><<<(unsigned)((R.stride + 255) / 256), 256, 0, st>>>(G, R, nullptr, nullptr, fields, const_cast<float *>(rec), step);
 }
 
 void launch_advance(int *step, int delta, cudaStream_t st) { k_advance<<<1, 1, 0, st>>>(step, delta); }
