@@ -5,11 +5,15 @@
 //   * ping-pong: step n reads buffer n&1 and writes buffer (n+1)&1, so tiles are independent;
 //   * the xy plane is cut into TX x TY tiles, a tile's z column into segments; a persistent CTA
 //     (one per SM) marches its segments plane by plane (2.5-D blocking);
-//   * one producer warp streams each plane's boxes (6 fields, inv_eps, psi slabs) global->shared with
-//     TMA (cp.async.bulk.tensor, zero fill outside the grid = the zero-pad wall convention) through an
-//     mbarrier full/empty ring; consumer warps hold a float4 of cells per thread;
-//   * plane kk: phase A computes E'(kk) on the tile plus a +x halo column and +y halo row (recomputed,
-//     not exchanged), phase B computes H'(kk-1) from E'(kk-1) (registers + shared ring) and E'(kk);
+//   * one producer thread streams each plane's boxes (6 fields, inv_eps, psi slabs) global->shared with
+//     TMA (cp.async.bulk.tensor; zero fill outside the grid IS the zero-pad wall convention) into a ring
+//     of equally sized slots; a plane takes as many slots as it has arrays (7 in the interior, up to 18 in
+//     a CPML corner), so interior planes are prefetched ~5 deep; mbarrier full/empty per plane;
+//   * consumer threads own a float4 of cells; plane kk: phase A computes E'(kk) on the tile plus a +y halo
+//     row and a +x halo column (recomputed, not exchanged), phase B computes H'(kk-1) from E'(kk-1)
+//     (registers + a shared E' ring) and E'(kk);
+//   * the update is written as  base curl  +  per-axis CPML corrections  (ik-1)*d + psi  that only run
+//     on planes / warps that touch a slab;
 //   * algorithmic traffic: 6 reads + 6 writes + inv_eps per cell, psi read+write on slab cells only.
 #include <algorithm>
 #include <cstdio>
@@ -26,23 +30,21 @@ using namespace fdtd;
 namespace {
 
 constexpr int MAX_SRC = 4, MAX_DET = 4;
-constexpr int MAX_THREADS = 512;      // 128 registers per thread at one CTA per SM
+constexpr int NBAR = 16;                // plane-loads in flight (mbarrier ring)
 
 struct FwdParams {
     Dims G;
     Tables T;
     const CUtensorMap *maps;
-    const Segment *segs;
-    const int *seg_begin;          // [n_cta + 1]
+    const Segment *segs;           // [n_rot][...]
+    const int *seg_begin;          // [n_rot][n_cta + 1]
+    int n_rot, seg_stride, n_cta;
     float *buf[2];                 // ping-pong field buffers, [6][nc] each
     PsiSet psiE[2], psiH[2];
     const int *step;
-    int TX, TY, TX4, NT, NCW;      // tile, float4s per row, active consumer threads, consumer warps
-    int PW, ROWS, XW;              // box width / rows, narrow x-psi box width
-    int big_bytes, small_bytes, stage_bytes, nstages;
-    int slot_off[SA_COUNT];        // byte offset of each logical array inside a stage
-    int ring_off, bar_off;         // byte offsets in dynamic smem
-    int RP;                        // ring row pitch (floats)
+    int nslots;                    // slots in the shared-memory ring
+    int XW, small_bytes;           // narrow x-psi box: width (floats) and exact byte size (TMA transaction bytes)
+    int small_off, xslots;         // a pair of narrow boxes sits at offsets 0 / small_off of `xslots` consecutive slots
     int has_mu;
     int n_src, n_det, total_freq;
     SourceDev src[MAX_SRC];
@@ -50,13 +52,39 @@ struct FwdParams {
     const float *cs;
 };
 
-__device__ __forceinline__ float4 lds4(const uint8_t *base, int off_bytes)
+template <int TX4_, int TY_>
+struct Cfg {
+    static constexpr int TX4 = TX4_, TY = TY_, TX = 4 * TX4_;
+    static constexpr int PW = TX + 8, ROWS = TY + 2;
+    static constexpr int BOX_BYTES = PW * ROWS * 4;                    // TMA transaction bytes of a big box
+    static constexpr int SLOT = (BOX_BYTES + 127) / 128 * 128;          // slot pitch
+    static constexpr int RP = TX + 4;                                   // E' ring row pitch (floats)
+    static constexpr int RING_COMP = (TY + 1) * RP, RING_SLOT = 3 * RING_COMP;
+    static constexpr int RING_BYTES = (2 * RING_SLOT * 4 + 127) / 128 * 128;
+    static constexpr int NT = TX4 * (TY + 1);                           // float4 threads (incl. the +y halo row)
+    static constexpr int NCW = (NT + TY + 31) / 32;                     // consumer warps (halo-column threads appended)
+    static constexpr int THREADS = NCW * 32 + 32;
+};
+
+__device__ __forceinline__ float4 lds4(uint32_t addr)
 {
-    return *reinterpret_cast<const float4 *>(base + off_bytes);
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
 }
-__device__ __forceinline__ float lds1(const uint8_t *base, int off_bytes)
+__device__ __forceinline__ float lds1(uint32_t addr)
 {
-    return *reinterpret_cast<const float *>(base + off_bytes);
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void sts4(uint32_t addr, float4 v)
+{
+    asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+__device__ __forceinline__ void sts1(uint32_t addr, float v)
+{
+    asm volatile("st.shared.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
 }
 __device__ __forceinline__ float4 ldg4(const float *p) { return __ldg(reinterpret_cast<const float4 *>(p)); }
 __device__ __forceinline__ void stg4(float *p, float4 v) { *reinterpret_cast<float4 *>(p) = v; }
@@ -64,8 +92,34 @@ __device__ __forceinline__ void stg4(float *p, float4 v) { *reinterpret_cast<flo
 __device__ __forceinline__ bool in_zslab(const Dims &G, int k) { return G.d > 0 && k >= 0 && k < G.nz && (k < G.d || k >= G.nz - G.d); }
 __device__ __forceinline__ int zslab_index(const Dims &G, int k) { return k < G.d ? k : k - (G.nz - 2 * G.d); }
 
+// Which arrays a plane-load carries and where they sit (slot ordinals).  Shared by producer and consumers.
+struct PlaneLayout {
+    int n;                 // slots taken
+    int im, pez, pey, pex, phz, phy, phx;     // ordinals (valid only when present)
+};
+__device__ __forceinline__ PlaneLayout plane_layout(bool prolog, bool doB, bool has_mu, bool zE, bool zH, bool ys, bool xs, int xslots)
+{
+    PlaneLayout L;
+    int o = 3;                                  // HX, HY, HZ always
+    L.im = L.pez = L.pey = L.pex = L.phz = L.phy = L.phx = 0;
+    if (!prolog) {
+        o = 7;                                  // + EX, EY, EZ, IE
+        if (zE) { L.pez = o; o += 2; }
+        if (ys) { L.pey = o; o += 2; }
+        if (xs) { L.pex = o; o += xslots; }
+    }
+    if (doB) {
+        if (has_mu) { L.im = o; o += 1; }
+        if (zH) { L.phz = o; o += 2; }
+        if (ys) { L.phy = o; o += 2; }
+        if (xs) { L.phx = o; o += xslots; }
+    }
+    L.n = o;
+    return L;
+}
+
 // additive source contribution to component `comp` at cell (i,j,k) during this step
-__device__ __forceinline__ float source_at(const FwdParams &P, int n, int comp, int i, int j, int k)
+__device__ __noinline__ float source_at(const FwdParams &P, int n, int comp, int i, int j, int k)
 {
     float acc = 0.f;
     for (int s = 0; s < P.n_src; ++s) {
@@ -87,7 +141,7 @@ __device__ __forceinline__ bool any_source_plane(const FwdParams &P, int family,
 }
 
 // running DFT of component `comp` (value v) at cell (i,j,k): P_f += v (cos - i sin)
-__device__ __forceinline__ void detect_cell(const FwdParams &P, int n, int comp, float v, int i, int j, int k)
+__device__ __noinline__ void detect_cell(const FwdParams &P, int n, int comp, float v, int i, int j, int k)
 {
     for (int s = 0; s < P.n_det; ++s) {
         const DetectorDev &q = P.det[s];
@@ -118,92 +172,130 @@ __device__ __forceinline__ bool any_detector_plane(const FwdParams &P, int famil
     return false;
 }
 
-__device__ __forceinline__ float &f4at(float4 &v, int q) { return q == 0 ? v.x : (q == 1 ? v.y : (q == 2 ? v.z : v.w)); }
+__device__ __forceinline__ float f4get(const float4 &v, int q) { return q == 0 ? v.x : (q == 1 ? v.y : (q == 2 ? v.z : v.w)); }
+__device__ __forceinline__ void f4add(float4 &v, int q, float a) { if (q == 0) v.x += a; else if (q == 1) v.y += a; else if (q == 2) v.z += a; else v.w += a; }
+
+// psi recursion + bracket correction for one psi array:   p = b*psi + a*d ;  t += sgn*((ik-1)*d + p)
+__device__ __forceinline__ float4 psi_fix(float4 &t, float sgn, float4 b, float4 a, float4 ikm1, float4 psi, float4 d)
+{
+    float4 p;
+    p.x = fmaf(b.x, psi.x, a.x * d.x); p.y = fmaf(b.y, psi.y, a.y * d.y);
+    p.z = fmaf(b.z, psi.z, a.z * d.z); p.w = fmaf(b.w, psi.w, a.w * d.w);
+    t.x += sgn * fmaf(ikm1.x, d.x, p.x); t.y += sgn * fmaf(ikm1.y, d.y, p.y);
+    t.z += sgn * fmaf(ikm1.z, d.z, p.z); t.w += sgn * fmaf(ikm1.w, d.w, p.w);
+    return p;
+}
+__device__ __forceinline__ float psi_fix1(float &t, float sgn, float b, float a, float ikm1, float psi, float d)
+{
+    const float p = fmaf(b, psi, a * d);
+    t += sgn * fmaf(ikm1, d, p);
+    return p;
+}
 
 // ================================================================================================
-__global__ void __launch_bounds__(MAX_THREADS, 1) k_fused_forward(const __grid_constant__ FwdParams P)
+template <class C>
+__global__ void __launch_bounds__(C::THREADS, 1) k_fused_forward(const __grid_constant__ FwdParams P)
 {
     extern __shared__ __align__(1024) uint8_t smem[];
     const Dims &G = P.G;
-    uint64_t *full = reinterpret_cast<uint64_t *>(smem + P.bar_off);
-    uint64_t *empty = full + P.nstages;
+    const uint32_t slots_base = smem_u32(smem);
+    const uint32_t ring_base = slots_base + (uint32_t)P.nslots * C::SLOT;
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + (size_t)P.nslots * C::SLOT + C::RING_BYTES);
+    uint64_t *empty = full + NBAR;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n = *P.step;
     const int par = n & 1;
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < P.nstages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], P.NCW); }
+        for (int s = 0; s < NBAR; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], C::NCW); }
         fence_mbar_init();
     }
     __syncthreads();
 
-    const int seg_lo = P.seg_begin[blockIdx.x], seg_hi = P.seg_begin[blockIdx.x + 1];
+    const int rot = n % P.n_rot;
+    const int *sb = P.seg_begin + rot * (P.n_cta + 1);
+    const Segment *segs = P.segs + (size_t)rot * P.seg_stride;
+    const int seg_lo = sb[blockIdx.x], seg_hi = sb[blockIdx.x + 1];
+    const bool has_mu = P.has_mu != 0;
 
-    // ============================================================================== producer warp
-    if (warp == P.NCW) {
+    // ============================================================================== producer
+    if (warp == C::NCW) {
         if (lane != 0) return;
         const CUtensorMap *M = P.maps;
-        int ld = 0;
+        int ld = 0;                 // plane-loads issued
+        int head = 0;               // next free slot
+        int tail_ld = 0;            // oldest plane-load not yet known to be released
+        int start[NBAR];            // first slot of each in-flight plane-load
+        int tail_pos = 0;
         for (int sg = seg_lo; sg < seg_hi; ++sg) {
-            const Segment S = P.segs[sg];
+            const Segment S = segs[sg];
             const int x = S.i0 - 4, y = S.j0 - 1;
             const bool xs = (S.flags & (SEG_X_LO | SEG_X_HI)) != 0, ys = (S.flags & (SEG_Y_LO | SEG_Y_HI)) != 0;
             const int xhi = (S.flags & SEG_X_HI) ? 1 : 0, yhi = (S.flags & SEG_Y_HI) ? 1 : 0;
             const int xv = (xhi ? S.xbase - (G.nx - G.dpx) : S.xbase) - 4;     // x-psi box start in view coordinates
             const int yv = yhi ? y - (G.ny - G.d) : y;                          // y-psi box start in view coordinates
             for (int kk = S.k0 - 1; kk <= S.k1; ++kk, ++ld) {
-                const int s = ld % P.nstages;
-                mbar_wait(&empty[s], ((ld / P.nstages) & 1) ^ 1);
-                uint8_t *st = smem + (size_t)s * P.stage_bytes;
                 const bool prolog = kk == S.k0 - 1;
                 const bool doB = kk >= S.k0 + 1;
                 const bool zE = !prolog && in_zslab(G, kk), zH = doB && in_zslab(G, kk - 1);
-                uint32_t bytes = 3 * P.big_bytes;
-                if (!prolog) {
-                    bytes += 4 * P.big_bytes;
-                    if (zE) bytes += 2 * P.big_bytes;
-                    if (ys) bytes += 2 * P.big_bytes;
-                    if (xs) bytes += 2 * P.small_bytes;
+                const PlaneLayout L = plane_layout(prolog, doB, has_mu, zE, zH, ys, xs, P.xslots);
+                // ---- allocate L.n contiguous slots (never wrapping inside a plane-load)
+                int base = head + L.n > P.nslots ? 0 : head;
+                for (;;) {
+                    const int inflight = ld - tail_ld;
+                    bool fits;
+                    if (inflight == 0) fits = true;
+                    else if (inflight >= NBAR) fits = false;
+                    else if (head > tail_pos) fits = (base == head) ? true : (L.n <= tail_pos);      // free: [head,N) U [0,tail)
+                    else if (head < tail_pos) fits = (base == head) && (head + L.n <= tail_pos);     // free: [head,tail)
+                    else fits = false;                                                                // ring full
+                    if (fits) break;
+                    mbar_wait(&empty[tail_ld % NBAR], (tail_ld / NBAR) & 1);
+                    ++tail_ld;
+                    tail_pos = (tail_ld < ld) ? start[tail_ld % NBAR] : base;
                 }
-                if (doB) {
-                    if (P.has_mu) bytes += P.big_bytes;
-                    if (zH) bytes += 2 * P.big_bytes;
-                    if (ys) bytes += 2 * P.big_bytes;
-                    if (xs) bytes += 2 * P.small_bytes;
-                }
-                mbar_expect_tx(&full[s], bytes);
-                for (int c = 3; c < 6; ++c) tma_load_3d(st + P.slot_off[c], M + TM_FIELD + par * 6 + c, x, y, kk, &full[s]);
+                if (ld - tail_ld == 0) tail_pos = base;
+                start[ld % NBAR] = base;
+                head = base + L.n;
+                const int bi = ld % NBAR;
+                uint64_t *fb = &full[bi];
+                uint8_t *st = smem + (size_t)base * C::SLOT;
+                uint32_t bytes = 3 * C::BOX_BYTES;
+                if (!prolog) bytes += 4 * C::BOX_BYTES + (zE ? 2 * C::BOX_BYTES : 0) + (ys ? 2 * C::BOX_BYTES : 0) + (xs ? 2 * P.small_bytes : 0);
+                if (doB) bytes += (has_mu ? C::BOX_BYTES : 0) + (zH ? 2 * C::BOX_BYTES : 0) + (ys ? 2 * C::BOX_BYTES : 0) + (xs ? 2 * P.small_bytes : 0);
+                mbar_expect_tx(fb, bytes);
+                for (int c = 0; c < 3; ++c) tma_load_3d(st + c * C::SLOT, M + TM_FIELD + par * 6 + 3 + c, x, y, kk, fb);
                 if (!prolog) {
-                    for (int c = 0; c < 3; ++c) tma_load_3d(st + P.slot_off[c], M + TM_FIELD + par * 6 + c, x, y, kk, &full[s]);
-                    tma_load_3d(st + P.slot_off[SA_IE], M + TM_IE, x, y, kk, &full[s]);
+                    for (int c = 0; c < 3; ++c) tma_load_3d(st + (3 + c) * C::SLOT, M + TM_FIELD + par * 6 + c, x, y, kk, fb);
+                    tma_load_3d(st + 6 * C::SLOT, M + TM_IE, x, y, kk, fb);
                     if (zE) {
                         const int kz = zslab_index(G, kk);
-                        tma_load_3d(st + P.slot_off[SA_PE_Z0], M + tm_psi(par, 0, 8), x, y, kz, &full[s]);
-                        tma_load_3d(st + P.slot_off[SA_PE_Z1], M + tm_psi(par, 0, 9), x, y, kz, &full[s]);
+                        tma_load_3d(st + L.pez * C::SLOT, M + tm_psi(par, 0, 8), x, y, kz, fb);
+                        tma_load_3d(st + (L.pez + 1) * C::SLOT, M + tm_psi(par, 0, 9), x, y, kz, fb);
                     }
                     if (ys) {
-                        tma_load_3d(st + P.slot_off[SA_PE_Y0], M + tm_psi(par, 0, 4 + 2 * yhi), x, yv, kk, &full[s]);
-                        tma_load_3d(st + P.slot_off[SA_PE_Y1], M + tm_psi(par, 0, 5 + 2 * yhi), x, yv, kk, &full[s]);
+                        tma_load_3d(st + L.pey * C::SLOT, M + tm_psi(par, 0, 4 + 2 * yhi), x, yv, kk, fb);
+                        tma_load_3d(st + (L.pey + 1) * C::SLOT, M + tm_psi(par, 0, 5 + 2 * yhi), x, yv, kk, fb);
                     }
                     if (xs) {
-                        tma_load_3d(st + P.slot_off[SA_PE_X0], M + tm_psi(par, 0, 0 + 2 * xhi), xv, y, kk, &full[s]);
-                        tma_load_3d(st + P.slot_off[SA_PE_X1], M + tm_psi(par, 0, 1 + 2 * xhi), xv, y, kk, &full[s]);
+                        tma_load_3d(st + L.pex * C::SLOT, M + tm_psi(par, 0, 0 + 2 * xhi), xv, y, kk, fb);
+                        tma_load_3d(st + L.pex * C::SLOT + P.small_off, M + tm_psi(par, 0, 1 + 2 * xhi), xv, y, kk, fb);
                     }
                 }
                 if (doB) {
-                    if (P.has_mu) tma_load_3d(st + P.slot_off[SA_IM], M + TM_IM, x, y, kk - 1, &full[s]);
+                    if (has_mu) tma_load_3d(st + L.im * C::SLOT, M + TM_IM, x, y, kk - 1, fb);
                     if (zH) {
                         const int kz = zslab_index(G, kk - 1);
-                        tma_load_3d(st + P.slot_off[SA_PH_Z0], M + tm_psi(par, 1, 8), x, y, kz, &full[s]);
-                        tma_load_3d(st + P.slot_off[SA_PH_Z1], M + tm_psi(par, 1, 9), x, y, kz, &full[s]);
+                        tma_load_3d(st + L.phz * C::SLOT, M + tm_psi(par, 1, 8), x, y, kz, fb);
+                        tma_load_3d(st + (L.phz + 1) * C::SLOT, M + tm_psi(par, 1, 9), x, y, kz, fb);
                     }
                     if (ys) {
-                        tma_load_3d(st + P.slot_off[SA_PH_Y0], M + tm_psi(par, 1, 4 + 2 * yhi), x, yv, kk - 1, &full[s]);
-                        tma_load_3d(st + P.slot_off[SA_PH_Y1], M + tm_psi(par, 1, 5 + 2 * yhi), x, yv, kk - 1, &full[s]);
+                        tma_load_3d(st + L.phy * C::SLOT, M + tm_psi(par, 1, 4 + 2 * yhi), x, yv, kk - 1, fb);
+                        tma_load_3d(st + (L.phy + 1) * C::SLOT, M + tm_psi(par, 1, 5 + 2 * yhi), x, yv, kk - 1, fb);
                     }
                     if (xs) {
-                        tma_load_3d(st + P.slot_off[SA_PH_X0], M + tm_psi(par, 1, 0 + 2 * xhi), xv, y, kk - 1, &full[s]);
-                        tma_load_3d(st + P.slot_off[SA_PH_X1], M + tm_psi(par, 1, 1 + 2 * xhi), xv, y, kk - 1, &full[s]);
+                        tma_load_3d(st + L.phx * C::SLOT, M + tm_psi(par, 1, 0 + 2 * xhi), xv, y, kk - 1, fb);
+                        tma_load_3d(st + L.phx * C::SLOT + P.small_off, M + tm_psi(par, 1, 1 + 2 * xhi), xv, y, kk - 1, fb);
                     }
                 }
             }
@@ -211,219 +303,201 @@ __global__ void __launch_bounds__(MAX_THREADS, 1) k_fused_forward(const __grid_c
         return;
     }
 
-    // ============================================================================== consumer warps
+    // ============================================================================== consumers
     const int t = threadIdx.x;
-    const bool active = t < P.NT;
-    const int ty = active ? t / P.TX4 : 0;
-    const int tx = active ? t - ty * P.TX4 : 0;
-    const bool halo_row = ty == P.TY;
-    const bool last_col = tx == P.TX4 - 1;
-    const int o_own = ((1 + ty) * P.PW + 4 + 4 * tx) * 4;        // byte offset of my float4 inside a big box
-    const int o_my = o_own - P.PW * 4;                           // row below (-y)
-    const int o_mx = o_own - 4;                                  // cell to the left (-x)
-    const int o_hc = o_own + 16;                                 // +x halo column cell (for last_col threads)
-    float *ring = reinterpret_cast<float *>(smem + P.ring_off);
-    const int ring_comp = (P.TY + 1) * P.RP, ring_slot = 3 * ring_comp;
-    const int r_own = ty * P.RP + 4 * tx;
+    const bool vec = t < C::NT;                                   // float4 thread
+    const bool hcol = t >= C::NT && t < C::NT + C::TY;            // +x halo column thread (one scalar cell per row)
+    const int ty = vec ? t / C::TX4 : (hcol ? t - C::NT : 0);
+    const int tx = vec ? t - ty * C::TX4 : C::TX4;                // halo column sits at float4 index TX4
+    const bool halo_row = vec && ty == C::TY;
+    // byte offset of my first cell inside a big box / a narrow box / the E' ring
+    const uint32_t o_own = ((1 + ty) * C::PW + 4 + 4 * tx) * 4;
+    const uint32_t r_own = (ty * C::RP + 4 * tx) * 4;
     float *dst = P.buf[par ^ 1];
     const PsiSet &pE = P.psiE[par ^ 1], &pH = P.psiH[par ^ 1];
     const float S = G.S;
     const long long nc = G.nc;
-    const int consumer_threads = P.NCW * 32;
+    const long long plane = (long long)G.ny * G.nx;
 
-    int ld = 0;
+    int ld = 0, head = 0;
     for (int sg = seg_lo; sg < seg_hi; ++sg) {
-        const Segment Sg = P.segs[sg];
+        const Segment Sg = segs[sg];
         const int i = Sg.i0 + 4 * tx, j = Sg.j0 + ty;
         const bool in_x = i < G.nx, in_y = j < G.ny;
-        const bool own_ok = active && !halo_row && in_x && in_y;
+        const bool own_ok = vec && !halo_row && in_x && in_y;
+        const bool xs = (Sg.flags & (SEG_X_LO | SEG_X_HI)) != 0, ys = (Sg.flags & (SEG_Y_LO | SEG_Y_HI)) != 0;
         const bool ypml = G.d > 0 && in_y && (j < G.d || j >= G.ny - G.d);
         const bool xpml = G.d > 0 && in_x && (i < G.dpx || i >= G.nx - G.dpx);
-        const int ih = i + 4;                                     // +x halo column
-        const bool xpml_h = G.d > 0 && ih < G.nx && (ih < G.dpx || ih >= G.nx - G.dpx);
-        const int o_x = ((1 + ty) * P.XW + (i - Sg.xbase + 4)) * 4;   // my float4 inside a narrow x-psi box
-        // per-thread coefficients (constant along z)
-        const float4 ikEx = in_x ? ldg4(P.T.ik[0][0] + i) : splat(1.f);
-        const float4 ikHx = in_x ? ldg4(P.T.ik[1][0] + i) : splat(1.f);
-        const float ikEx_h = ih < G.nx ? __ldg(P.T.ik[0][0] + ih) : 1.f;
-        const float ikEy = in_y ? __ldg(P.T.ik[0][1] + j) : 1.f, ikHy = in_y ? __ldg(P.T.ik[1][1] + j) : 1.f;
-        float bEy = 1.f, aEy = 0.f, bHy = 1.f, aHy = 0.f;
-        if (ypml) { bEy = __ldg(P.T.b[0][1] + j); aEy = __ldg(P.T.a[0][1] + j); bHy = __ldg(P.T.b[1][1] + j); aHy = __ldg(P.T.a[1][1] + j); }
+        const bool warp_x = xs && __any_sync(0xffffffffu, xpml), warp_y = ys && __any_sync(0xffffffffu, ypml);
+        const uint32_t o_x = xpml ? ((1 + ty) * P.XW + (i - Sg.xbase + 4)) * 4 : 0;   // my cells inside a narrow x-psi box
         const int sy = j < G.d ? j : j - (G.ny - 2 * G.d);
         const int sx = i < G.dpx ? i : i - (G.nx - 2 * G.dpx);
         const long long own_xy = (long long)j * G.nx + i;
 
-        float4 hxk = splat(0.f), hyk = splat(0.f), hzk = splat(0.f);      // H(kk-1) at my cells
-        float4 e1x = splat(0.f), e1y = splat(0.f), e1z = splat(0.f);      // E'(kk-1) at my cells
-        float hxk_h = 0.f;                                                // H_x(kk-1) at the +x halo column
+        float4 hxk = splat(0.f), hyk = hxk, hzk = hxk;      // H(kk-1) at my cells   (halo column thread: .x only)
+        float4 e1x = hxk, e1y = hxk, e1z = hxk;             // E'(kk-1) at my cells
 
         for (int kk = Sg.k0 - 1; kk <= Sg.k1; ++kk, ++ld) {
-            const int s = ld % P.nstages;
-            mbar_wait(&full[s], (ld / P.nstages) & 1);
-            const uint8_t *st = smem + (size_t)s * P.stage_bytes;
             const bool prolog = kk == Sg.k0 - 1;
+            const bool doB = kk >= Sg.k0 + 1;
+            const bool zE = !prolog && in_zslab(G, kk), zH = doB && in_zslab(G, kk - 1);
+            const PlaneLayout L = plane_layout(prolog, doB, has_mu, zE, zH, ys, xs, P.xslots);
+            const int base = head + L.n > P.nslots ? 0 : head;
+            head = base + L.n;
+            const int bi = ld % NBAR;
+            mbar_wait(&full[bi], (ld / NBAR) & 1);
+            const uint32_t sb0 = slots_base + (uint32_t)base * C::SLOT;     // first slot of this plane-load
+            const uint32_t so = sb0 + o_own;
             if (prolog) {
-                if (active) {
-                    hxk = lds4(st + P.slot_off[SA_HX], o_own);
-                    hyk = lds4(st + P.slot_off[SA_HY], o_own);
-                    hzk = lds4(st + P.slot_off[SA_HZ], o_own);
-                    hxk_h = lds1(st + P.slot_off[SA_HX], o_hc);
-                }
+                if (vec) { hxk = lds4(so); hyk = lds4(so + C::SLOT); hzk = lds4(so + 2 * C::SLOT); }
+                else if (hcol) hxk.x = lds1(so);
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&empty[s]);
+                if (lane == 0) mbar_arrive(&empty[bi]);
                 continue;
             }
             const bool storeE = kk < Sg.k1;
-            const bool doB = kk >= Sg.k0 + 1;
+            const uint32_t rgA = ring_base + (kk & 1) * (C::RING_SLOT * 4) + r_own;
+            const bool src_plane = P.n_src && any_source_plane(P, 0, kk);
             float4 hx = splat(0.f), hy = hx, hz = hx, e2x = hx, e2y = hx, e2z = hx;
-            if (active) {
-                // ---------------------------------------------------------------- phase A: E'(kk)
-                const bool zE = in_zslab(G, kk);
-                const int kc = kk < G.nz ? kk : G.nz;                 // tables are padded past N
-                const float ikEz = __ldg(P.T.ik[0][2] + kc);
-                float bEz = 1.f, aEz = 0.f;
-                if (zE) { bEz = __ldg(P.T.b[0][2] + kk); aEz = __ldg(P.T.a[0][2] + kk); }
-                const float4 ex = lds4(st + P.slot_off[SA_EX], o_own), ey = lds4(st + P.slot_off[SA_EY], o_own),
-                             ez = lds4(st + P.slot_off[SA_EZ], o_own);
-                const float4 sie = S * lds4(st + P.slot_off[SA_IE], o_own);
-                hx = lds4(st + P.slot_off[SA_HX], o_own);
-                hy = lds4(st + P.slot_off[SA_HY], o_own);
-                hz = lds4(st + P.slot_off[SA_HZ], o_own);
-                const float4 hx_my = lds4(st + P.slot_off[SA_HX], o_my), hz_my = lds4(st + P.slot_off[SA_HZ], o_my);
-                const float hy_mx = lds1(st + P.slot_off[SA_HY], o_mx), hz_mx = lds1(st + P.slot_off[SA_HZ], o_mx);
+            if (vec) {
+                // ------------------------------------------------------------ phase A: E'(kk), 4 cells
+                hx = lds4(so); hy = lds4(so + C::SLOT); hz = lds4(so + 2 * C::SLOT);
+                const float4 hx_my = lds4(so - C::PW * 4), hz_my = lds4(so + 2 * C::SLOT - C::PW * 4);
+                const float hy_mx = lds1(so + C::SLOT - 4), hz_mx = lds1(so + 2 * C::SLOT - 4);
                 const float4 dHz_dy = hz - hz_my, dHx_dy = hx - hx_my;
                 const float4 dHy_dz = hy - hyk, dHx_dz = hx - hxk;
                 const float4 dHy_dx = dminus_x(hy, hy_mx), dHz_dx = dminus_x(hz, hz_mx);
-                const bool wr = own_ok && storeE;                      // I own these cells: write E' and psi_E
-                const long long zoff = (long long)kk * G.ny * G.nx;
-                float4 bEx = splat(1.f), aEx = splat(0.f);
-                if (xpml) { bEx = ldg4(P.T.b[0][0] + i); aEx = ldg4(P.T.a[0][0] + i); }
-                const long long ix = ((long long)kk * G.ny + j) * (2 * G.dpx) + sx;      // x-slab psi index
-                const long long iy = ((long long)kk * (2 * G.d) + sy) * G.nx + i;        // y-slab psi index
-                const long long iz = zE ? ((long long)zslab_index(G, kk) * G.ny + j) * G.nx + i : 0;
-
-                // E'_x: a = y (psiE_x0), b = z (psiE_x1)
-                float4 tE = ikEy * dHz_dy - ikEz * dHy_dz;
-                if (ypml) { const float4 p = bEy * lds4(st + P.slot_off[SA_PE_Y0], o_own) + aEy * dHz_dy; tE = tE + p; if (wr) stg4(pE.p[0][0] + iy, p); }
-                if (zE)   { const float4 p = bEz * lds4(st + P.slot_off[SA_PE_Z1], o_own) + aEz * dHy_dz; tE = tE - p; if (wr) stg4(pE.p[0][1] + iz, p); }
-                e2x = ex + sie * tE;
-                // E'_y: a = z (psiE_y0), b = x (psiE_y1)
-                tE = ikEz * dHx_dz - ikEx * dHz_dx;
-                if (zE)   { const float4 p = bEz * lds4(st + P.slot_off[SA_PE_Z0], o_own) + aEz * dHx_dz; tE = tE + p; if (wr) stg4(pE.p[1][0] + iz, p); }
-                if (xpml) { const float4 p = bEx * lds4(st + P.slot_off[SA_PE_X1], o_x) + aEx * dHz_dx; tE = tE - p; if (wr) stg4(pE.p[1][1] + ix, p); }
-                e2y = ey + sie * tE;
-                // E'_z: a = x (psiE_z0), b = y (psiE_z1)
-                tE = ikEx * dHy_dx - ikEy * dHx_dy;
-                if (xpml) { const float4 p = bEx * lds4(st + P.slot_off[SA_PE_X0], o_x) + aEx * dHy_dx; tE = tE + p; if (wr) stg4(pE.p[2][0] + ix, p); }
-                if (ypml) { const float4 p = bEy * lds4(st + P.slot_off[SA_PE_Y1], o_own) + aEy * dHx_dy; tE = tE - p; if (wr) stg4(pE.p[2][1] + iy, p); }
-                e2z = ez + sie * tE;
-
-                const bool src_plane = P.n_src && any_source_plane(P, 0, kk);
+                float4 tEx = dHz_dy - dHy_dz, tEy = dHx_dz - dHz_dx, tEz = dHy_dx - dHx_dy;
+                const bool wr = own_ok && storeE;                  // I own these cells: write E' and psi_E
+                if (zE) {       // z axis: psiE_y0 (d = dHx_dz, +), psiE_x1 (d = dHy_dz, -)
+                    const float4 b = splat(__ldg(P.T.b[0][2] + kk)), a = splat(__ldg(P.T.a[0][2] + kk)), km = splat(__ldg(P.T.ik[0][2] + kk) - 1.f);
+                    const long long iz = ((long long)zslab_index(G, kk) * G.ny + j) * G.nx + i;
+                    const float4 p0 = psi_fix(tEy, 1.f, b, a, km, lds4(so + L.pez * C::SLOT), dHx_dz);
+                    const float4 p1 = psi_fix(tEx, -1.f, b, a, km, lds4(so + (L.pez + 1) * C::SLOT), dHy_dz);
+                    if (wr) { stg4(pE.p[1][0] + iz, p0); stg4(pE.p[0][1] + iz, p1); }
+                }
+                if (warp_y) {   // y axis: psiE_x0 (d = dHz_dy, +), psiE_z1 (d = dHx_dy, -)
+                    float b = 1.f, a = 0.f, km = 0.f;
+                    if (ypml) { b = __ldg(P.T.b[0][1] + j); a = __ldg(P.T.a[0][1] + j); km = __ldg(P.T.ik[0][1] + j) - 1.f; }
+                    const long long iy = ((long long)kk * (2 * G.d) + sy) * G.nx + i;
+                    const float4 p0 = psi_fix(tEx, 1.f, splat(b), splat(a), splat(km), lds4(so + L.pey * C::SLOT), dHz_dy);
+                    const float4 p1 = psi_fix(tEz, -1.f, splat(b), splat(a), splat(km), lds4(so + (L.pey + 1) * C::SLOT), dHx_dy);
+                    if (wr && ypml) { stg4(pE.p[0][0] + iy, p0); stg4(pE.p[2][1] + iy, p1); }
+                }
+                if (warp_x) {   // x axis: psiE_z0 (d = dHy_dx, +), psiE_y1 (d = dHz_dx, -)
+                    float4 b = splat(1.f), a = splat(0.f), km = splat(0.f), q0 = a, q1 = a;
+                    if (xpml) {
+                        b = ldg4(P.T.b[0][0] + i); a = ldg4(P.T.a[0][0] + i); km = ldg4(P.T.ik[0][0] + i) - splat(1.f);
+                        q0 = lds4(sb0 + L.pex * C::SLOT + o_x); q1 = lds4(sb0 + L.pex * C::SLOT + P.small_off + o_x);
+                    }
+                    const long long ix = ((long long)kk * G.ny + j) * (2 * G.dpx) + sx;
+                    const float4 p0 = psi_fix(tEz, 1.f, b, a, km, q0, dHy_dx);
+                    const float4 p1 = psi_fix(tEy, -1.f, b, a, km, q1, dHz_dx);
+                    if (wr && xpml) { stg4(pE.p[2][0] + ix, p0); stg4(pE.p[1][1] + ix, p1); }
+                }
+                const float4 sie = S * lds4(so + 6 * C::SLOT);
+                e2x = lds4(so + 3 * C::SLOT) + sie * tEx;
+                e2y = lds4(so + 4 * C::SLOT) + sie * tEy;
+                e2z = lds4(so + 5 * C::SLOT) + sie * tEz;
                 if (src_plane) {
 #pragma unroll
                     for (int q = 0; q < 4; ++q) {
-                        f4at(e2x, q) += source_at(P, n, 0, i + q, j, kk);
-                        f4at(e2y, q) += source_at(P, n, 1, i + q, j, kk);
-                        f4at(e2z, q) += source_at(P, n, 2, i + q, j, kk);
+                        f4add(e2x, q, source_at(P, n, 0, i + q, j, kk));
+                        f4add(e2y, q, source_at(P, n, 1, i + q, j, kk));
+                        f4add(e2z, q, source_at(P, n, 2, i + q, j, kk));
                     }
                 }
-                float *rg = ring + (kk & 1) * ring_slot + r_own;
-                *reinterpret_cast<float4 *>(rg) = e2x;
-                *reinterpret_cast<float4 *>(rg + ring_comp) = e2y;
-                *reinterpret_cast<float4 *>(rg + 2 * ring_comp) = e2z;
+                sts4(rgA, e2x); sts4(rgA + C::RING_COMP * 4, e2y); sts4(rgA + 2 * C::RING_COMP * 4, e2z);
                 if (wr) {
-                    stg4(dst + 0 * nc + zoff + own_xy, e2x);
-                    stg4(dst + 1 * nc + zoff + own_xy, e2y);
-                    stg4(dst + 2 * nc + zoff + own_xy, e2z);
+                    float *o = dst + (long long)kk * plane + own_xy;
+                    stg4(o, e2x); stg4(o + nc, e2y); stg4(o + 2 * nc, e2z);
                     if (P.n_det && any_detector_plane(P, 0, kk)) {
 #pragma unroll
                         for (int q = 0; q < 4; ++q) {
-                            detect_cell(P, n, 0, f4at(e2x, q), i + q, j, kk);
-                            detect_cell(P, n, 1, f4at(e2y, q), i + q, j, kk);
-                            detect_cell(P, n, 2, f4at(e2z, q), i + q, j, kk);
+                            detect_cell(P, n, 0, f4get(e2x, q), i + q, j, kk);
+                            detect_cell(P, n, 1, f4get(e2y, q), i + q, j, kk);
+                            detect_cell(P, n, 2, f4get(e2z, q), i + q, j, kk);
                         }
                     }
                 }
-                // +x halo column: E'_y and E'_z at (i+4, j, kk), recomputed for my row (not stored)
-                if (last_col) {
-                    const float hx_h = lds1(st + P.slot_off[SA_HX], o_hc);
-                    if (!halo_row) {
-                        const float hy_h = lds1(st + P.slot_off[SA_HY], o_hc), hz_h = lds1(st + P.slot_off[SA_HZ], o_hc);
-                        const float hx_h_my = lds1(st + P.slot_off[SA_HX], o_hc - P.PW * 4);
-                        const float sie_h = S * lds1(st + P.slot_off[SA_IE], o_hc);
-                        const float dHx_dz_h = hx_h - hxk_h, dHz_dx_h = hz_h - hz.w, dHy_dx_h = hy_h - hy.w, dHx_dy_h = hx_h - hx_h_my;
-                        float bx_h = 1.f, ax_h = 0.f;
-                        if (xpml_h) { bx_h = __ldg(P.T.b[0][0] + ih); ax_h = __ldg(P.T.a[0][0] + ih); }
-                        float tH = ikEz * dHx_dz_h - ikEx_h * dHz_dx_h;
-                        if (zE)     tH += bEz * lds1(st + P.slot_off[SA_PE_Z0], o_hc) + aEz * dHx_dz_h;
-                        if (xpml_h) tH -= bx_h * lds1(st + P.slot_off[SA_PE_X1], o_x + 16) + ax_h * dHz_dx_h;
-                        float ey_h = lds1(st + P.slot_off[SA_EY], o_hc) + sie_h * tH;
-                        tH = ikEx_h * dHy_dx_h - ikEy * dHx_dy_h;
-                        if (xpml_h) tH += bx_h * lds1(st + P.slot_off[SA_PE_X0], o_x + 16) + ax_h * dHy_dx_h;
-                        if (ypml)   tH -= bEy * lds1(st + P.slot_off[SA_PE_Y1], o_hc) + aEy * dHx_dy_h;
-                        float ez_h = lds1(st + P.slot_off[SA_EZ], o_hc) + sie_h * tH;
-                        if (src_plane) { ey_h += source_at(P, n, 1, ih, j, kk); ez_h += source_at(P, n, 2, ih, j, kk); }
-                        rg[ring_comp + 4] = ey_h;
-                        rg[2 * ring_comp + 4] = ez_h;
-                    }
-                    hxk_h = hx_h;
+            } else if (hcol) {
+                // ------------------------------------------------------------ phase A, +x halo column: E'_y, E'_z of one cell
+                const float hx_h = lds1(so), hy_h = lds1(so + C::SLOT), hz_h = lds1(so + 2 * C::SLOT);
+                const float dHx_dz = hx_h - hxk.x, dHz_dx = hz_h - lds1(so + 2 * C::SLOT - 4), dHy_dx = hy_h - lds1(so + C::SLOT - 4);
+                const float dHx_dy = hx_h - lds1(so - C::PW * 4);
+                float tEy = dHx_dz - dHz_dx, tEz = dHy_dx - dHx_dy;
+                if (zE) psi_fix1(tEy, 1.f, __ldg(P.T.b[0][2] + kk), __ldg(P.T.a[0][2] + kk), __ldg(P.T.ik[0][2] + kk) - 1.f,
+                                 lds1(so + L.pez * C::SLOT), dHx_dz);
+                if (ypml) psi_fix1(tEz, -1.f, __ldg(P.T.b[0][1] + j), __ldg(P.T.a[0][1] + j), __ldg(P.T.ik[0][1] + j) - 1.f,
+                                   lds1(so + (L.pey + 1) * C::SLOT), dHx_dy);
+                if (xpml) {
+                    const float b = __ldg(P.T.b[0][0] + i), a = __ldg(P.T.a[0][0] + i), km = __ldg(P.T.ik[0][0] + i) - 1.f;
+                    psi_fix1(tEz, 1.f, b, a, km, lds1(sb0 + L.pex * C::SLOT + o_x), dHy_dx);
+                    psi_fix1(tEy, -1.f, b, a, km, lds1(sb0 + L.pex * C::SLOT + P.small_off + o_x), dHz_dx);
                 }
+                const float sie = S * lds1(so + 6 * C::SLOT);
+                float ey_h = lds1(so + 4 * C::SLOT) + sie * tEy, ez_h = lds1(so + 5 * C::SLOT) + sie * tEz;
+                if (src_plane) { ey_h += source_at(P, n, 1, i, j, kk); ez_h += source_at(P, n, 2, i, j, kk); }
+                sts1(rgA + C::RING_COMP * 4, ey_h);
+                sts1(rgA + 2 * C::RING_COMP * 4, ez_h);
+                hx.x = hx_h;
             }
-            // ---------------------------------------------------------------- phase B: H'(kk-1)
-            if (active && doB && !halo_row) {
-                const int km = kk - 1;
-                const bool zH = in_zslab(G, km);
-                const float ikHz = __ldg(P.T.ik[1][2] + km);
-                float bHz = 1.f, aHz = 0.f;
-                if (zH) { bHz = __ldg(P.T.b[1][2] + km); aHz = __ldg(P.T.a[1][2] + km); }
-                const float4 sim = P.has_mu ? S * lds4(st + P.slot_off[SA_IM], o_own) : splat(S);
-                const float *rg = ring + (km & 1) * ring_slot + r_own;
-                const float4 ex_py = *reinterpret_cast<const float4 *>(rg + P.RP);
-                const float4 ez_py = *reinterpret_cast<const float4 *>(rg + 2 * ring_comp + P.RP);
-                const float ey_px = rg[ring_comp + 4], ez_px = rg[2 * ring_comp + 4];
+            // ---------------------------------------------------------------- phase B: H'(kk-1), 4 cells
+            if (vec && doB && !halo_row) {
+                const int km1 = kk - 1;
+                const uint32_t rgB = ring_base + (km1 & 1) * (C::RING_SLOT * 4) + r_own;
+                const float4 ex_py = lds4(rgB + C::RP * 4), ez_py = lds4(rgB + (2 * C::RING_COMP + C::RP) * 4);
+                const float ey_px = lds1(rgB + (C::RING_COMP + 4) * 4), ez_px = lds1(rgB + (2 * C::RING_COMP + 4) * 4);
                 const float4 dEz_dy = ez_py - e1z, dEx_dy = ex_py - e1x;
                 const float4 dEy_dz = e2y - e1y, dEx_dz = e2x - e1x;
                 const float4 dEz_dx = dplus_x(e1z, ez_px), dEy_dx = dplus_x(e1y, ey_px);
-                float4 bHx = splat(1.f), aHx = splat(0.f);
-                if (xpml) { bHx = ldg4(P.T.b[1][0] + i); aHx = ldg4(P.T.a[1][0] + i); }
-                const long long zoff = (long long)km * G.ny * G.nx;
-                const long long ix = ((long long)km * G.ny + j) * (2 * G.dpx) + sx;
-                const long long iy = ((long long)km * (2 * G.d) + sy) * G.nx + i;
-                const long long iz = zH ? ((long long)zslab_index(G, km) * G.ny + j) * G.nx + i : 0;
+                float4 tHx = dEz_dy - dEy_dz, tHy = dEx_dz - dEz_dx, tHz = dEy_dx - dEx_dy;
                 const bool wr = own_ok;
-                // H'_x: a = y (psiH_x0), b = z (psiH_x1)
-                float4 tH = ikHy * dEz_dy - ikHz * dEy_dz;
-                if (ypml) { const float4 p = bHy * lds4(st + P.slot_off[SA_PH_Y0], o_own) + aHy * dEz_dy; tH = tH + p; if (wr) stg4(pH.p[0][0] + iy, p); }
-                if (zH)   { const float4 p = bHz * lds4(st + P.slot_off[SA_PH_Z1], o_own) + aHz * dEy_dz; tH = tH - p; if (wr) stg4(pH.p[0][1] + iz, p); }
-                float4 h2x = hxk - sim * tH;
-                // H'_y: a = z (psiH_y0), b = x (psiH_y1)
-                tH = ikHz * dEx_dz - ikHx * dEz_dx;
-                if (zH)   { const float4 p = bHz * lds4(st + P.slot_off[SA_PH_Z0], o_own) + aHz * dEx_dz; tH = tH + p; if (wr) stg4(pH.p[1][0] + iz, p); }
-                if (xpml) { const float4 p = bHx * lds4(st + P.slot_off[SA_PH_X1], o_x) + aHx * dEz_dx; tH = tH - p; if (wr) stg4(pH.p[1][1] + ix, p); }
-                float4 h2y = hyk - sim * tH;
-                // H'_z: a = x (psiH_z0), b = y (psiH_z1)
-                tH = ikHx * dEy_dx - ikHy * dEx_dy;
-                if (xpml) { const float4 p = bHx * lds4(st + P.slot_off[SA_PH_X0], o_x) + aHx * dEy_dx; tH = tH + p; if (wr) stg4(pH.p[2][0] + ix, p); }
-                if (ypml) { const float4 p = bHy * lds4(st + P.slot_off[SA_PH_Y1], o_own) + aHy * dEx_dy; tH = tH - p; if (wr) stg4(pH.p[2][1] + iy, p); }
-                float4 h2z = hzk - sim * tH;
+                if (zH) {       // z axis: psiH_y0 (d = dEx_dz, +), psiH_x1 (d = dEy_dz, -)
+                    const float4 b = splat(__ldg(P.T.b[1][2] + km1)), a = splat(__ldg(P.T.a[1][2] + km1)), km = splat(__ldg(P.T.ik[1][2] + km1) - 1.f);
+                    const long long iz = ((long long)zslab_index(G, km1) * G.ny + j) * G.nx + i;
+                    const float4 p0 = psi_fix(tHy, 1.f, b, a, km, lds4(so + L.phz * C::SLOT), dEx_dz);
+                    const float4 p1 = psi_fix(tHx, -1.f, b, a, km, lds4(so + (L.phz + 1) * C::SLOT), dEy_dz);
+                    if (wr) { stg4(pH.p[1][0] + iz, p0); stg4(pH.p[0][1] + iz, p1); }
+                }
+                if (warp_y) {   // y axis: psiH_x0 (d = dEz_dy, +), psiH_z1 (d = dEx_dy, -)
+                    float b = 1.f, a = 0.f, km = 0.f;
+                    if (ypml) { b = __ldg(P.T.b[1][1] + j); a = __ldg(P.T.a[1][1] + j); km = __ldg(P.T.ik[1][1] + j) - 1.f; }
+                    const long long iy = ((long long)km1 * (2 * G.d) + sy) * G.nx + i;
+                    const float4 p0 = psi_fix(tHx, 1.f, splat(b), splat(a), splat(km), lds4(so + L.phy * C::SLOT), dEz_dy);
+                    const float4 p1 = psi_fix(tHz, -1.f, splat(b), splat(a), splat(km), lds4(so + (L.phy + 1) * C::SLOT), dEx_dy);
+                    if (wr && ypml) { stg4(pH.p[0][0] + iy, p0); stg4(pH.p[2][1] + iy, p1); }
+                }
+                if (warp_x) {   // x axis: psiH_z0 (d = dEy_dx, +), psiH_y1 (d = dEz_dx, -)
+                    float4 b = splat(1.f), a = splat(0.f), km = splat(0.f), q0 = a, q1 = a;
+                    if (xpml) {
+                        b = ldg4(P.T.b[1][0] + i); a = ldg4(P.T.a[1][0] + i); km = ldg4(P.T.ik[1][0] + i) - splat(1.f);
+                        q0 = lds4(sb0 + L.phx * C::SLOT + o_x); q1 = lds4(sb0 + L.phx * C::SLOT + P.small_off + o_x);
+                    }
+                    const long long ix = ((long long)km1 * G.ny + j) * (2 * G.dpx) + sx;
+                    const float4 p0 = psi_fix(tHz, 1.f, b, a, km, q0, dEy_dx);
+                    const float4 p1 = psi_fix(tHy, -1.f, b, a, km, q1, dEz_dx);
+                    if (wr && xpml) { stg4(pH.p[2][0] + ix, p0); stg4(pH.p[1][1] + ix, p1); }
+                }
+                const float4 sim = has_mu ? S * lds4(so + L.im * C::SLOT) : splat(S);
+                float4 h2x = hxk - sim * tHx, h2y = hyk - sim * tHy, h2z = hzk - sim * tHz;
                 if (wr) {
-                    if (P.n_src && any_source_plane(P, 1, km)) {
+                    if (P.n_src && any_source_plane(P, 1, km1)) {
 #pragma unroll
                         for (int q = 0; q < 4; ++q) {
-                            f4at(h2x, q) += source_at(P, n, 3, i + q, j, km);
-                            f4at(h2y, q) += source_at(P, n, 4, i + q, j, km);
-                            f4at(h2z, q) += source_at(P, n, 5, i + q, j, km);
+                            f4add(h2x, q, source_at(P, n, 3, i + q, j, km1));
+                            f4add(h2y, q, source_at(P, n, 4, i + q, j, km1));
+                            f4add(h2z, q, source_at(P, n, 5, i + q, j, km1));
                         }
                     }
-                    stg4(dst + 3 * nc + zoff + own_xy, h2x);
-                    stg4(dst + 4 * nc + zoff + own_xy, h2y);
-                    stg4(dst + 5 * nc + zoff + own_xy, h2z);
-                    if (P.n_det && any_detector_plane(P, 1, km)) {
+                    float *o = dst + 3 * nc + (long long)km1 * plane + own_xy;
+                    stg4(o, h2x); stg4(o + nc, h2y); stg4(o + 2 * nc, h2z);
+                    if (P.n_det && any_detector_plane(P, 1, km1)) {
 #pragma unroll
                         for (int q = 0; q < 4; ++q) {
-                            detect_cell(P, n, 3, f4at(h2x, q), i + q, j, km);
-                            detect_cell(P, n, 4, f4at(h2y, q), i + q, j, km);
-                            detect_cell(P, n, 5, f4at(h2z, q), i + q, j, km);
+                            detect_cell(P, n, 3, f4get(h2x, q), i + q, j, km1);
+                            detect_cell(P, n, 4, f4get(h2y, q), i + q, j, km1);
+                            detect_cell(P, n, 5, f4get(h2z, q), i + q, j, km1);
                         }
                     }
                 }
@@ -431,8 +505,8 @@ __global__ void __launch_bounds__(MAX_THREADS, 1) k_fused_forward(const __grid_c
             e1x = e2x; e1y = e2y; e1z = e2z;
             hxk = hx; hyk = hy; hzk = hz;
             __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[s]);
-            named_bar_sync(1, consumer_threads);      // ring slot (kk-1)&1 may be overwritten next iteration
+            if (lane == 0) mbar_arrive(&empty[bi]);
+            named_bar_sync(1, C::NCW * 32);      // E' ring slot (kk-1)&1 may be overwritten in the next iteration
         }
     }
 }
@@ -474,10 +548,31 @@ bool encode3d(CUtensorMap *out, const float *base, long long dx, long long dy, l
 
 int align_up(int v, int a) { return (v + a - 1) / a * a; }
 
+// ---- the compiled tile shapes ----------------------------------------------------------------------
+struct TileImpl {
+    int TX, TY, threads, slot, ring_bytes;
+    void (*launch)(const FwdParams &, int n_cta, size_t smem, cudaStream_t);
+    cudaError_t (*set_smem)(size_t);
+};
+template <class C> void launch_impl(const FwdParams &P, int n_cta, size_t smem, cudaStream_t st)
+{
+    k_fused_forward<C><<<n_cta, C::THREADS, smem, st>>>(P);
+}
+template <class C> cudaError_t set_smem_impl(size_t smem)
+{
+    return cudaFuncSetAttribute(k_fused_forward<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+}
+#define TILE(TX4, TY) { 4 * TX4, TY, Cfg<TX4, TY>::THREADS, Cfg<TX4, TY>::SLOT, Cfg<TX4, TY>::RING_BYTES, launch_impl<Cfg<TX4, TY>>, set_smem_impl<Cfg<TX4, TY>> }
+const TileImpl kTiles[] = {
+    TILE(2, 2), TILE(4, 4), TILE(8, 8), TILE(16, 8), TILE(16, 16), TILE(25, 10), TILE(25, 16), TILE(32, 8), TILE(32, 12),
+};
+constexpr int kNumTiles = sizeof(kTiles) / sizeof(kTiles[0]);
+
 }  // namespace
 
 struct FusedState {
-    int TX = 0, TY = 0, nst = 0, n_cta = 0, threads = 0;
+    const TileImpl *tile = nullptr;
+    int TX = 0, TY = 0, nslots = 0, n_cta = 0, n_rot = 1;
     size_t smem = 0;
     FwdParams fp{};
     float *bufB = nullptr;                 // second field buffer
@@ -491,23 +586,37 @@ struct FusedState {
 
 namespace {
 
-struct TileChoice { int TX, TY, nst; size_t smem; int stage_bytes, big, small, XW; double score; };
-
-// smem layout for a candidate tile; returns false if it does not fit
-bool layout(const Dims &G, bool has_mu, int TX, int TY, int nst, int smem_cap, TileChoice &c)
+// cuts the flattened (tile, plane) sequence, rotated by `rot` planes, into n_cta equal runs
+void make_segments(const Dims &G, int TX, int TY, int n_cta, long long rot, std::vector<Segment> &segs, std::vector<int> &seg_begin)
 {
-    const int PW = TX + 8, ROWS = TY + 2;
-    c.TX = TX; c.TY = TY; c.nst = nst;
-    c.big = align_up(PW * ROWS * 4, 128);
-    c.XW = G.dpx + 8;
-    c.small = align_up(c.XW * ROWS * 4, 128);
-    int n_big = 7 + (has_mu ? 1 : 0) + (G.d > 0 ? 8 : 0);
-    int n_small = G.d > 0 ? 4 : 0;
-    c.stage_bytes = align_up(n_big * c.big + n_small * c.small, 1024);
-    const int RP = TX + 4;
-    const size_t ring = (size_t)2 * 3 * (TY + 1) * RP * 4;
-    c.smem = (size_t)nst * c.stage_bytes + align_up((int)ring, 128) + 128;
-    return c.smem <= (size_t)smem_cap;
+    const int ntx = (G.nx + TX - 1) / TX, nty = (G.ny + TY - 1) / TY;
+    const long long total = (long long)ntx * nty * G.nz;
+    segs.clear();
+    seg_begin.assign(n_cta + 1, 0);
+    rot = ((rot % total) + total) % total;
+    for (int cta = 0; cta < n_cta; ++cta) {
+        seg_begin[cta] = (int)segs.size();
+        long long a = total * cta / n_cta, b = total * (cta + 1) / n_cta;      // positions in the rotated sequence
+        while (a < b) {
+            const long long pos = (a + rot) % total;                            // position in the canonical sequence
+            const long long tile = pos / G.nz;
+            const int k = (int)(pos % G.nz);
+            const int len = (int)std::min<long long>(b - a, G.nz - k);
+            const int txi = (int)(tile / nty), tyi = (int)(tile % nty);
+            Segment s{};
+            s.i0 = txi * TX; s.j0 = tyi * TY; s.k0 = k; s.k1 = k + len;
+            if (G.d > 0) {
+                if (s.i0 < G.dpx) s.flags |= SEG_X_LO;
+                if (s.i0 + TX >= G.nx - G.dpx) s.flags |= SEG_X_HI;
+                if (s.j0 < G.d) s.flags |= SEG_Y_LO;
+                if (s.j0 + TY >= G.ny - G.d) s.flags |= SEG_Y_HI;
+            }
+            s.xbase = (s.flags & SEG_X_HI) ? std::max(s.i0, G.nx - G.dpx) : s.i0;
+            segs.push_back(s);
+            a += len;
+        }
+    }
+    seg_begin[n_cta] = (int)segs.size();
 }
 
 }  // namespace
@@ -527,38 +636,42 @@ int fused_setup(fdtd_grid *g)
         g->fused_why_not = "cannot query the device";
         return FDTD_OK;
     }
-    const bool has_mu = true;   // the stage layout always reserves the inv_mu slot (8 big arrays); cheap and keeps one kernel
 
-    // ---- tile choice: maximise useful work per byte staged, subject to shared memory and slab rules -------------
-    const int tx_max = G.d > 0 ? std::min(248, G.nx - 2 * G.dpx - 4) / 4 * 4 : std::min(248, G.nx);
-    const int ty_max = G.d > 0 ? std::min(64, G.ny - 2 * G.d - 2) : std::min(64, G.ny);
-    TileChoice best{}; best.score = -1;
-    int fTX = 0, fTY = 0, fNST = 0;
-    if (const char *e = getenv("FDTD_TILE")) sscanf(e, "%d,%d,%d", &fTX, &fTY, &fNST);
-    for (int TX = 4; TX <= tx_max; TX += 4)
-        for (int TY = 1; TY <= ty_max; ++TY) {
-            if (fTX && (TX != fTX || TY != fTY)) continue;
-            const int NT = (TX / 4) * (TY + 1);
-            if (align_up(NT, 32) + 32 > MAX_THREADS) continue;
-            for (int nst = 4; nst >= 2; --nst) {
-                if (fNST && nst != fNST) continue;
-                TileChoice c{};
-                if (!layout(G, has_mu, TX, TY, nst, smem_cap, c)) continue;
-                const double eff_x = (double)G.nx / (((G.nx + TX - 1) / TX) * TX);
-                const double eff_y = (double)G.ny / (((G.ny + TY - 1) / TY) * TY);
-                const double halo = (double)(TX + 8) * (TY + 2) / ((double)TX * TY);
-                const double thr = (double)NT / (align_up(NT, 32));
-                // bytes through L2 per useful cell (7 loads * halo + 6 stores), wasted thread slots, sync depth bonus
-                c.score = eff_x * eff_y * thr / (28.0 * halo + 24.0) * (nst >= 3 ? 1.0 : 0.93) * (NT >= 192 ? 1.0 : 0.85);
-                if (c.score > best.score) best = c;
-                break;
-            }
+    // ---- tile choice among the compiled shapes --------------------------------------------------------------------
+    // A tile (with its +x halo column / +y halo row) may touch at most one CPML slab per axis, and the two narrow
+    // x-psi boxes must fit into one slot.
+    const int base_slots_per_plane = 7 + 1 + (G.d > 0 ? 8 : 0);
+    int fTX = 0, fTY = 0;
+    if (const char *e = getenv("FDTD_TILE")) sscanf(e, "%d,%d", &fTX, &fTY);
+    const TileImpl *best = nullptr;
+    double best_score = -1;
+    int best_slots = 0;
+    for (int q = 0; q < kNumTiles; ++q) {
+        const TileImpl &t = kTiles[q];
+        if (fTX && (t.TX != fTX || t.TY != fTY)) continue;
+        if (G.d > 0) {
+            if (t.TX >= G.nx - 2 * G.dpx || t.TY + 1 >= G.ny - 2 * G.d) continue;
         }
-    if (best.score < 0) { g->fused_why_not = "no tile fits (grid too small for its PML)"; return FDTD_OK; }
+        const int xsl = G.d > 0 ? (2 * align_up((G.dpx + 8) * (t.TY + 2) * 4, 128) + t.slot - 1) / t.slot : 0;
+        const int max_slots_per_plane = base_slots_per_plane + 2 * xsl;
+        const int nslots = std::min(4096, (smem_cap - t.ring_bytes - 2 * NBAR * 8 - 1024) / t.slot);
+        if (nslots < max_slots_per_plane + 3) continue;              // at least one plane of lookahead even in a corner
+        const double eff_x = (double)G.nx / (((G.nx + t.TX - 1) / t.TX) * t.TX);
+        const double eff_y = (double)G.ny / (((G.ny + t.TY - 1) / t.TY) * t.TY);
+        const double halo = (double)(t.TX + 8) * (t.TY + 2) / ((double)t.TX * t.TY);
+        const int NT = (t.TX / 4) * (t.TY + 1);
+        const double thr = (double)NT / (t.threads - 32);
+        const long long n_tiles = (long long)((G.nx + t.TX - 1) / t.TX) * ((G.ny + t.TY - 1) / t.TY);
+        const double fill = std::min(1.0, (double)n_tiles * G.nz / (8.0 * n_sm));   // enough planes per CTA to amortise prologues
+        const double score = eff_x * eff_y * thr * fill / (28.0 * halo + 24.0);
+        if (score > best_score) { best_score = score; best = &t; best_slots = nslots; }
+    }
+    if (!best) { g->fused_why_not = "no compiled tile shape fits this grid (too small for its PML)"; return FDTD_OK; }
 
     FusedState *F = new FusedState();
     g->fused = F;
-    F->TX = best.TX; F->TY = best.TY; F->nst = best.nst; F->smem = best.smem;
+    F->tile = best; F->TX = best->TX; F->TY = best->TY; F->nslots = best_slots;
+    F->smem = (size_t)best_slots * best->slot + best->ring_bytes + 2 * NBAR * 8;
     int rc;
     if ((rc = g->alloc((void **)&F->bufB, (size_t)G.nc * 6 * sizeof(float)))) return rc;
     if ((rc = g->alloc_psi(g->psiE[1])) || (rc = g->alloc_psi(g->psiH[1]))) return rc;
@@ -569,50 +682,35 @@ int fused_setup(fdtd_grid *g)
         return fdtd_fail(FDTD_ENOMEM, "pinned tensor-map staging allocation failed");
     }
 
-    // ---- segments: flatten (tile, plane) and cut into n_cta equal-cost runs ------------------------------------
+    // ---- segments ---------------------------------------------------------------------------------------------------
     const int ntx = (G.nx + F->TX - 1) / F->TX, nty = (G.ny + F->TY - 1) / F->TY;
     const long long total = (long long)ntx * nty * G.nz;
     int n_cta = (int)std::min<long long>(n_sm, std::max<long long>(1, total / 6));
     if (const char *e = getenv("FDTD_NCTA")) n_cta = std::max(1, atoi(e));
-    std::vector<Segment> segs;
-    std::vector<int> seg_begin(n_cta + 1, 0);
-    {
-        long long done = 0;
-        int cta = 0;
-        for (int txi = 0; txi < ntx; ++txi)
-            for (int tyi = 0; tyi < nty; ++tyi) {
-                int k = 0;
-                while (k < G.nz) {
-                    // planes left for the current CTA
-                    long long quota_end = (total * (cta + 1)) / n_cta;
-                    long long room = quota_end - done;
-                    if (room <= 0) { ++cta; seg_begin[cta] = (int)segs.size(); continue; }
-                    int len = (int)std::min<long long>(room, G.nz - k);
-                    Segment s{};
-                    s.i0 = txi * F->TX; s.j0 = tyi * F->TY; s.k0 = k; s.k1 = k + len;
-                    if (G.d > 0) {
-                        if (s.i0 < G.dpx) s.flags |= SEG_X_LO;
-                        if (s.i0 + F->TX >= G.nx - G.dpx) s.flags |= SEG_X_HI;
-                        if (s.j0 < G.d) s.flags |= SEG_Y_LO;
-                        if (s.j0 + F->TY >= G.ny - G.d) s.flags |= SEG_Y_HI;
-                    }
-                    s.xbase = (s.flags & SEG_X_HI) ? std::max(s.i0, G.nx - G.dpx) : s.i0;
-                    segs.push_back(s);
-                    k += len; done += len;
-                }
-            }
-        for (int c = cta + 1; c <= n_cta; ++c) seg_begin[c] = (int)segs.size();
+    // rotation of the work sequence between steps (L2 reuse: a CTA starts where the data written last step is
+    // still cached); n_rot tables, step n uses table n % n_rot
+    int n_rot = 1;
+    if (const char *e = getenv("FDTD_NROT")) n_rot = std::max(1, std::min(16, atoi(e)));
+    F->n_cta = n_cta; F->n_rot = n_rot;
+    std::vector<Segment> all;
+    std::vector<int> begins;
+    std::vector<std::vector<Segment>> per(n_rot);
+    std::vector<std::vector<int>> per_b(n_rot);
+    size_t stride = 0;
+    for (int r = 0; r < n_rot; ++r) {
+        const long long per_cta = total / n_cta;
+        make_segments(G, F->TX, F->TY, n_cta, -(long long)r * (per_cta / n_rot), per[r], per_b[r]);
+        stride = std::max(stride, per[r].size());
     }
-    for (const Segment &s : segs)
-        if (((s.flags & SEG_X_LO) && (s.flags & SEG_X_HI)) || ((s.flags & SEG_Y_LO) && (s.flags & SEG_Y_HI))) {
-            g->fused_why_not = "a tile touches both slabs of an axis";
-            return FDTD_OK;
-        }
-    F->n_cta = n_cta;
-    if ((rc = g->alloc((void **)&F->d_segs, segs.size() * sizeof(Segment)))) return rc;
-    if ((rc = g->alloc((void **)&F->d_seg_begin, seg_begin.size() * sizeof(int)))) return rc;
-    if (cudaMemcpy(F->d_segs, segs.data(), segs.size() * sizeof(Segment), cudaMemcpyHostToDevice) != cudaSuccess ||
-        cudaMemcpy(F->d_seg_begin, seg_begin.data(), seg_begin.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess) {
+    all.resize(stride * n_rot);
+    for (int r = 0; r < n_rot; ++r) {
+        std::copy(per[r].begin(), per[r].end(), all.begin() + r * stride);
+        begins.insert(begins.end(), per_b[r].begin(), per_b[r].end());
+    }
+    if ((rc = g->alloc((void **)&F->d_segs, all.size() * sizeof(Segment)))) return rc;
+    if ((rc = g->alloc((void **)&F->d_seg_begin, begins.size() * sizeof(int)))) return rc;
+    if (cudaMemcpy(F->d_segs, all.data(), all.size() * sizeof(Segment), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(F->d_seg_begin, begins.data(), begins.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess) {
         (void)cudaGetLastError();
         return fdtd_fail(FDTD_ECUDA, "upload of the segment table failed");
     }
@@ -620,32 +718,20 @@ int fused_setup(fdtd_grid *g)
     // ---- kernel parameters that do not depend on the call -----------------------------------------------------------
     FwdParams &P = F->fp;
     P.G = G; P.T = g->T; P.maps = F->d_maps; P.segs = F->d_segs; P.seg_begin = F->d_seg_begin;
+    P.n_rot = n_rot; P.seg_stride = (int)stride; P.n_cta = n_cta;
     P.step = g->d_step;
-    P.TX = F->TX; P.TY = F->TY; P.TX4 = F->TX / 4; P.NT = P.TX4 * (F->TY + 1); P.NCW = (P.NT + 31) / 32;
-    P.PW = F->TX + 8; P.ROWS = F->TY + 2; P.XW = best.XW;
-    P.big_bytes = P.PW * P.ROWS * 4; P.small_bytes = P.XW * P.ROWS * 4;
-    P.stage_bytes = best.stage_bytes; P.nstages = F->nst;
-    {
-        int off = 0;
-        const int bigs[] = { SA_EX, SA_EY, SA_EZ, SA_HX, SA_HY, SA_HZ, SA_IE, SA_IM, SA_PE_Y0, SA_PE_Y1, SA_PE_Z0, SA_PE_Z1,
-                             SA_PH_Y0, SA_PH_Y1, SA_PH_Z0, SA_PH_Z1 };
-        const int n_big = G.d > 0 ? 16 : 8;
-        for (int q = 0; q < SA_COUNT; ++q) P.slot_off[q] = 0;
-        for (int q = 0; q < n_big; ++q) { P.slot_off[bigs[q]] = off; off += best.big; }
-        if (G.d > 0)
-            for (int q = SA_PE_X0; q <= SA_PH_X1; ++q) { P.slot_off[q] = off; off += best.small; }
-    }
-    P.RP = F->TX + 4;
-    P.ring_off = F->nst * best.stage_bytes;
-    P.bar_off = P.ring_off + align_up(2 * 3 * (F->TY + 1) * P.RP * 4, 128);
-    F->threads = (P.NCW + 1) * 32;
-    if (cudaFuncSetAttribute(k_fused_forward, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F->smem) != cudaSuccess) {
+    P.nslots = F->nslots;
+    P.XW = G.dpx + 8;
+    P.small_bytes = P.XW * (F->TY + 2) * 4;
+    P.small_off = align_up(P.small_bytes, 128);       // the second narrow box stays 128-byte aligned
+    P.xslots = G.d > 0 ? (2 * P.small_off + best->slot - 1) / best->slot : 0;
+    if (best->set_smem(F->smem) != cudaSuccess) {
         (void)cudaGetLastError();
         g->fused_why_not = "cannot reserve shared memory";
         return FDTD_OK;
     }
     g->path = FDTD_PATH_FUSED;
-    g->tile_x = F->TX; g->tile_y = F->TY; g->tile_z = (int)(total / n_cta / std::max(1, ntx * nty / std::max(1, ntx * nty)));
+    g->tile_x = F->TX; g->tile_y = F->TY;
     g->tile_z = (int)std::min<long long>(G.nz, total / n_cta);
     return FDTD_OK;
 }
@@ -701,8 +787,6 @@ int build_maps(fdtd_grid *g, float *fields, const float *ie, const float *im, cu
             }
     }
     if (!ok) return fdtd_fail(FDTD_ECUDA, "cuTensorMapEncodeTiled failed");
-    // the previous maps may still be in use by kernels of an earlier call on another stream: the copy is stream ordered
-    // on `st`, and callers that switch streams between calls must synchronise them (documented in DESIGN.md)
     cudaError_t e = cudaMemcpyAsync(F->d_maps, F->h_maps, sizeof(CUtensorMap) * TM_COUNT, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaEventRecord(F->maps_done, st);
     if (e != cudaSuccess) { (void)cudaGetLastError(); return fdtd_fail(FDTD_ECUDA, std::string("tensor map upload: ") + cudaGetErrorString(e)); }
@@ -712,7 +796,7 @@ int build_maps(fdtd_grid *g, float *fields, const float *ie, const float *im, cu
 
 }  // namespace
 
-// run_steps lives in fdtd_api.cu; re-declared here through a small trampoline
+// run_steps lives in fdtd_api.cu; reached through a small trampoline
 int fdtd_run_steps_fwd(fdtd_grid *g, const std::string &key, int n_steps, int launches_per_step, cudaStream_t st,
                        void (*enqueue)(void *, cudaStream_t), void *ctx);
 
@@ -726,7 +810,7 @@ void enqueue_fwd(void *vctx, cudaStream_t cs)
     fdtd_grid *g = c->g;
     FusedState *F = g->fused;
     { ProfScope p(g, fdtd_grid::PC_FUSED_FWD, cs);
-      k_fused_forward<<<F->n_cta, F->threads, F->smem, cs>>>(c->P); }
+      F->tile->launch(c->P, F->n_cta, F->smem, cs); }
     if (c->recording) {
         // step n read buffer n&1 (pre-step H) and wrote buffer (n+1)&1 (E'); the record kernel picks them by parity
         ProfScope p(g, fdtd_grid::PC_RECORD, cs);
