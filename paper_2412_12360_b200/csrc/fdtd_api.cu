@@ -584,7 +584,7 @@ extern "C" int fdtd_backward(fdtd_grid *g, float *fields, const float *inv_eps, 
     CK(cudaMemsetAsync(g->d_step, 0, sizeof(int), st));
     if (n_steps > 0) launch_advance(g->d_step, n_steps - 1, st);
 
-    if (g->path == FDTD_PATH_FUSED && g->fused_backward_ready) {
+    if (g->path == FDTD_PATH_FUSED && g->fused_backward_ready && !inv_mu) {
         rc = fused_backward(g, fields, inv_eps, inv_mu, S, D, total_freq, n_steps, dL_dinv_eps, st);
         if (rc) return rc;
     } else {

@@ -124,5 +124,10 @@ void launch_grad_rho(const Dims &G, const float *g, const float *ie, float delta
                      float *out, cudaStream_t st);
 void launch_inv_H(const Dims &G, float *fields, const float *im, cudaStream_t st);
 void launch_inv_E_grad(const Dims &G, float *fields, const float *ie, const float *lam, float *g, cudaStream_t st);
+// fused path: cotangent volumes are ping-ponged by step parity
+void launch_inv_E_grad_pp(const Dims &G, float *fields, const float *ie, const float *lamA, const float *lamB,
+                          const int *step, float *g, cudaStream_t st);
+void launch_detector_adjoint_pp(const Dims &G, float *lamA, float *lamB, const DetectorDev &dt, const float *cs_table,
+                                int total_freq, const int *step, cudaStream_t st);
 
 }  // namespace fdtd

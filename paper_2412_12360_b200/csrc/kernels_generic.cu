@@ -121,8 +121,9 @@ __global__ void k_add_source(Dims G, float *__restrict__ f, SourceDev s, const i
 // cs_table: [max_steps][total_freq][2] = (cos, sin) of omega_f*(n+1), built on the host in fp64 (R13)
 template <bool ADJ>
 __global__ void k_detector(Dims G, float *__restrict__ f, DetectorDev dt, const float *__restrict__ cs,
-                           int total_freq, const int *__restrict__ step)
+                           int total_freq, const int *__restrict__ step, float *__restrict__ f2, int par_off)
 {
+    if (f2 && ((*step + par_off) & 1)) f = f2;       // ping-pong volumes of the fused path
     const int bx = dt.hi[0] - dt.lo[0], by = dt.hi[1] - dt.lo[1], bz = dt.hi[2] - dt.lo[2];
     const long long bc = (long long)bx * by * bz;
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -339,9 +340,11 @@ __global__ void __launch_bounds__(BX *BY) k_inv_H(Dims G, float *__restrict__ f,
 // gradient box; E = E' - S ie q.
 template <bool PER>
 __global__ void __launch_bounds__(BX *BY) k_inv_E_grad(Dims G, float *__restrict__ f, const float *__restrict__ ie,
-                                                       const float *__restrict__ lam, float *__restrict__ g)
+                                                       const float *__restrict__ lam, float *__restrict__ g,
+                                                       const float *__restrict__ lam2, const int *__restrict__ step)
 {
     CELL_IJK();
+    if (lam2 && ((*step) & 1)) lam = lam2;           // ping-pong cotangents of the fused path: lamE' of step n is in buffer n&1
     if (i < G.lo[0] || i >= G.hi[0] || j < G.lo[1] || j >= G.hi[1] || k < G.lo[2] || k >= G.hi[2]) return;
     const float sie = G.S * __ldg(ie + p);
     float acc = 0.f;
@@ -398,14 +401,22 @@ void launch_detector(const Dims &G, const float *fields, const DetectorDev &dt, 
                      int total_freq, const int *step, cudaStream_t st)
 {
     const long long n = (long long)(dt.hi[0] - dt.lo[0]) * (dt.hi[1] - dt.lo[1]) * (dt.hi[2] - dt.lo[2]);
-    k_detector<false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(G, const_cast<float *>(fields), dt, cs_table, total_freq, step);
+    k_detector<false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(G, const_cast<float *>(fields), dt, cs_table, total_freq, step, nullptr, 0);
 }
 
 void launch_detector_adjoint(const Dims &G, float *lam, const DetectorDev &dt, const float *cs_table,
                              int total_freq, const int *step, cudaStream_t st)
 {
     const long long n = (long long)(dt.hi[0] - dt.lo[0]) * (dt.hi[1] - dt.lo[1]) * (dt.hi[2] - dt.lo[2]);
-    k_detector<true><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(G, lam, dt, cs_table, total_freq, step);
+    k_detector<true><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(G, lam, dt, cs_table, total_freq, step, nullptr, 0);
+}
+
+// reverse step n of the fused path injects into the volume it is about to read: buffer (n+1)&1
+void launch_detector_adjoint_pp(const Dims &G, float *lamA, float *lamB, const DetectorDev &dt, const float *cs_table,
+                                int total_freq, const int *step, cudaStream_t st)
+{
+    const long long n = (long long)(dt.hi[0] - dt.lo[0]) * (dt.hi[1] - dt.lo[1]) * (dt.hi[2] - dt.lo[2]);
+    k_detector<true><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(G, lamA, dt, cs_table, total_freq, step, lamB, 1);
 }
 
 void launch_record(const Dims &G, const RecLayout &R, const float *fields_H, const float *fields_E,
@@ -467,8 +478,14 @@ void launch_inv_H(const Dims &G, float *fields, const float *im, cudaStream_t st
 
 void launch_inv_E_grad(const Dims &G, float *fields, const float *ie, const float *lam, float *g, cudaStream_t st)
 {
-    if (G.periodic) k_inv_E_grad<true><<<vol_grid(G), vol_block(), 0, st>>>(G, fields, ie, lam, g);
-    else            k_inv_E_grad<false><<<vol_grid(G), vol_block(), 0, st>>>(G, fields, ie, lam, g);
+    if (G.periodic) k_inv_E_grad<true><<<vol_grid(G), vol_block(), 0, st>>>(G, fields, ie, lam, g, nullptr, nullptr);
+    else            k_inv_E_grad<false><<<vol_grid(G), vol_block(), 0, st>>>(G, fields, ie, lam, g, nullptr, nullptr);
+}
+
+void launch_inv_E_grad_pp(const Dims &G, float *fields, const float *ie, const float *lamA, const float *lamB,
+                          const int *step, float *g, cudaStream_t st)
+{
+    k_inv_E_grad<false><<<vol_grid(G), vol_block(), 0, st>>>(G, fields, ie, lamA, g, lamB, step);
 }
 
 }  // namespace fdtd

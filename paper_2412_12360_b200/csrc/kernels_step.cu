@@ -1,0 +1,919 @@
+// kernels_step.cu -- fused z-marching step kernels of the hot path (DESIGN.md sections 7-8):
+//
+//   k_step<C, false>  forward step : E update + H update + CPML psi + sources + detectors   (F1-F7)
+//   k_step<C, true>   adjoint step : transpose of the H update, then of the E update, adjoint CPML (B2+B5)
+//
+// PAPER.md: Eq. 1-2 (L64-66) for the curl updates, L72 for the CPML, L78-84 for the VJP.
+//
+// Design
+//   * ping-pong volumes: a launch reads buffer `par` and writes buffer `par^1`, so tiles are independent;
+//   * the xy plane is cut into TX x TY tiles, a tile's z column into segments; a persistent CTA marches its
+//     segments plane by plane (2.5-D blocking), carrying the previous plane in registers;
+//   * only the three arrays that are differenced in phase A (the H-type operand F) need neighbours: one
+//     producer thread streams their boxes (one-cell halo, 16-byte aligned in x) global -> shared with TMA
+//     (cp.async.bulk.tensor; the zero fill outside the grid IS the zero-pad wall convention R7) through a
+//     ring of NST stages with full/empty mbarriers.  Everything a thread only needs at its own cells
+//     (E-type target, inv_eps, CPML states) is read straight from global memory as float4, the E-type
+//     target and inv_eps one plane ahead;
+//   * consumer warps are 8 x 4 patches of float4 threads (128 B contiguous per patch row), so CPML slab
+//     code is executed by the few warps that touch a slab.  Plane kk, phase A: the E-type update of plane
+//     kk on the tile plus a +x halo column and a +y halo row (recomputed, not exchanged between CTAs),
+//     result to global and to a shared ring; phase B: the H-type update of plane kk-1 from the phase-A
+//     results of planes kk-1 (registers + ring) and kk (registers); one named barrier per plane;
+//   * CPML: the time-recursive filter  p' = b p + a x,  c = (ik-1) x + p'  adds c to a difference.
+//     Forward: x = the difference.  Adjoint: the filter acts on the operands before the difference (its
+//     tables depend on the position along the difference axis) with the rescaled state
+//     theta = (a/b) * lambda_psi, which obeys the same recursion; phase-B operands are filtered by the
+//     thread that produces them in phase A and travel through the ring already filtered.
+#include <algorithm>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "fdtd_grid.h"
+#include "fused_common.cuh"
+
+using namespace fdtd;
+
+namespace {
+
+constexpr int MAX_SRC = 4, MAX_DET = 4;
+constexpr int MAX_ST = 8;               // upper bound of pipeline stages
+
+struct StepParams {
+    Dims G;
+    Tables T;
+    const CUtensorMap *maps;       // [set][3]: H-type components of buffer `set`
+    const Segment *segs;           // [n_rot][seg_stride]
+    const int *seg_begin;          // [n_rot][n_cta + 1]
+    int n_rot, seg_stride, n_cta;
+    float *buf[2];                 // ping-pong volumes, [6][nc] each
+    const float *ie, *im;
+    PsiSet psiE[2], psiH[2];       // CPML states of the E-type / H-type update, ping-pong
+    const int *step;
+    int nst;                       // pipeline stages
+    int n_src, n_det, total_freq;
+    SourceDev src[MAX_SRC];
+    DetectorDev det[MAX_DET];
+    const float *cs;
+};
+
+template <int TX4_, int TY_>
+struct Cfg {
+    static constexpr int TX4 = TX4_, TY = TY_, TX = 4 * TX4_;
+    static constexpr int CW = TX4 + 1, RW = TY + 1;                     // float4 lanes per row / rows, halo included
+    static constexpr int PCX = (CW + 7) / 8, PCY = (RW + 3) / 4;        // 8 x 4 thread patches
+    static constexpr int NCW = PCX * PCY;                               // consumer warps
+    static constexpr int THREADS = NCW * 32 + 32;
+    static constexpr int PW = TX + 8, ROWS = TY + 2;
+    static constexpr int ROWB = PW * 4;                                 // box row pitch in bytes
+    static constexpr int BOX_BYTES = PW * ROWS * 4;                     // TMA transaction bytes of one box
+    static constexpr int SLOT = (BOX_BYTES + 127) / 128 * 128;
+    static constexpr int STAGE = 3 * SLOT;
+    static constexpr int RP = 4 * CW;                                   // ring row pitch (floats)
+    static constexpr int RING_ARR = RW * RP;                            // floats of one ring array
+    static constexpr int RING_SLOT = 4 * RING_ARR;                      // Yx, Yz, Xy, Xz
+    static constexpr int RING_BYTES = (2 * RING_SLOT * 4 + 127) / 128 * 128;
+};
+
+__device__ __forceinline__ float4 lds4(uint32_t addr)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ float lds1(uint32_t addr)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void sts4(uint32_t addr, float4 v)
+{
+    asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+__device__ __forceinline__ float4 ldg4(const float *p) { return __ldg(reinterpret_cast<const float4 *>(p)); }
+__device__ __forceinline__ float4 ld4(const float *p) { return *reinterpret_cast<const float4 *>(p); }
+__device__ __forceinline__ void stg4(float *p, float4 v) { *reinterpret_cast<float4 *>(p) = v; }
+__device__ __forceinline__ float4 fma4(float4 a, float4 b, float4 c)
+{
+    return make_float4(fmaf(a.x, b.x, c.x), fmaf(a.y, b.y, c.y), fmaf(a.z, b.z, c.z), fmaf(a.w, b.w, c.w));
+}
+__device__ __forceinline__ float4 fma4(float a, float4 b, float4 c)
+{
+    return make_float4(fmaf(a, b.x, c.x), fmaf(a, b.y, c.y), fmaf(a, b.z, c.z), fmaf(a, b.w, c.w));
+}
+
+// CPML recursive filter at one point: p' = b p + a x; returns the correction c = (ik - 1) x + p'
+__device__ __forceinline__ float4 cpml4(float4 b, float4 a, float4 km, float4 p, float4 x, float4 &pn)
+{
+    pn = fma4(b, p, a * x);
+    return fma4(km, x, pn);
+}
+__device__ __forceinline__ float4 cpml4(float b, float a, float km, float4 p, float4 x, float4 &pn)
+{
+    pn = fma4(b, p, a * x);
+    return fma4(km, x, pn);
+}
+__device__ __forceinline__ float cpml1(float b, float a, float km, float p, float x) { return fmaf(km, x, fmaf(b, p, a * x)); }
+
+// slab-compact coordinate along an axis of length n with slab storage width w per side, or -1
+__device__ __forceinline__ int slab_pos(int p, int n, int w) { return p < 0 || p >= n ? -1 : (p < w ? p : (p >= n - w ? p - (n - 2 * w) : -1)); }
+
+// additive source contribution to component `comp` at cell (i,j,k) during this step
+__device__ __noinline__ float source_at(const StepParams &P, int n, int comp, int i, int j, int k)
+{
+    float acc = 0.f;
+    for (int s = 0; s < P.n_src; ++s) {
+        const SourceDev &q = P.src[s];
+        if (q.comp != comp) continue;
+        if (i < q.lo[0] || i >= q.hi[0] || j < q.lo[1] || j >= q.hi[1] || k < q.lo[2] || k >= q.hi[2]) continue;
+        const int bx = q.hi[0] - q.lo[0], by = q.hi[1] - q.lo[1];
+        const float pr = q.profile ? __ldg(q.profile + ((long long)(k - q.lo[2]) * by + (j - q.lo[1])) * bx + (i - q.lo[0])) : 1.f;
+        acc += pr * __ldg(q.waveform + n);
+    }
+    return acc;
+}
+
+// running DFT of component `comp` (value v) at cell (i,j,k): P_f += v (cos - i sin)
+__device__ __noinline__ void detect_cell(const StepParams &P, int n, int comp, float v, int i, int j, int k)
+{
+    for (int s = 0; s < P.n_det; ++s) {
+        const DetectorDev &q = P.det[s];
+        if (!((q.mask >> comp) & 1)) continue;
+        if (i < q.lo[0] || i >= q.hi[0] || j < q.lo[1] || j >= q.hi[1] || k < q.lo[2] || k >= q.hi[2]) continue;
+        const int bx = q.hi[0] - q.lo[0], by = q.hi[1] - q.lo[1], bz = q.hi[2] - q.lo[2];
+        const long long bc = (long long)bx * by * bz;
+        const long long cell = ((long long)(k - q.lo[2]) * by + (j - q.lo[1])) * bx + (i - q.lo[0]);
+        int ci = 0;
+        for (int c = 0; c < comp; ++c) ci += (q.mask >> c) & 1;
+        const float *csn = P.cs + ((long long)n * P.total_freq + q.cs_off) * 2;
+        for (int f = 0; f < q.n_freq; ++f) {
+            float2 *ph = reinterpret_cast<float2 *>(q.phasor) + ((long long)f * q.ncomp + ci) * bc + cell;
+            float2 acc = *ph;
+            acc.x += v * __ldg(csn + 2 * f);
+            acc.y -= v * __ldg(csn + 2 * f + 1);
+            *ph = acc;
+        }
+    }
+}
+
+__device__ __forceinline__ float f4get(const float4 &v, int q) { return q == 0 ? v.x : (q == 1 ? v.y : (q == 2 ? v.z : v.w)); }
+
+// adds the sources of `family` (0 = E, 1 = H) to the three float4s of cell group (i..i+3, j, k); rare planes only
+__device__ __noinline__ void add_sources4(const StepParams &P, int n, int family, float4 &vx, float4 &vy, float4 &vz, int i, int j, int k)
+{
+    float4 *v[3] = { &vx, &vy, &vz };
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        v[c]->x += source_at(P, n, 3 * family + c, i + 0, j, k);
+        v[c]->y += source_at(P, n, 3 * family + c, i + 1, j, k);
+        v[c]->z += source_at(P, n, 3 * family + c, i + 2, j, k);
+        v[c]->w += source_at(P, n, 3 * family + c, i + 3, j, k);
+    }
+}
+__device__ __noinline__ void detect4(const StepParams &P, int n, int family, float4 vx, float4 vy, float4 vz, int i, int j, int k)
+{
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        detect_cell(P, n, 3 * family + 0, f4get(vx, q), i + q, j, k);
+        detect_cell(P, n, 3 * family + 1, f4get(vy, q), i + q, j, k);
+        detect_cell(P, n, 3 * family + 2, f4get(vz, q), i + q, j, k);
+    }
+}
+
+// ================================================================================================
+// The step kernel.  Names follow the forward step: "F" is the H-type operand of phase A, "e" the
+// E-type target, "v" the phase-A result that phase B differences, "h" the H-type target.
+//   forward : e' = e + S ie curl-(F = H)            v = e'            h' = h - S im curl+(v)
+//   adjoint : e' = e - S curl-(F = lamH)   (im = 1) v = S ie e'       h' = h + curl+(v)
+// curl with CPML: t_x = Dy_z - Dz_y, t_y = Dz_x - Dx_z, t_z = Dx_y - Dy_x, where D<a>_<c> is the
+// (filtered) difference of component c along axis a; its state array is
+//   Dy_z p[0][0]   Dz_y p[0][1]   Dz_x p[1][0]   Dx_z p[1][1]   Dx_y p[2][0]   Dy_x p[2][1].
+// ================================================================================================
+template <class C, bool ADJ>
+__global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ StepParams P)
+{
+    extern __shared__ __align__(1024) uint8_t smem[];
+    const Dims &G = P.G;
+    const uint32_t stage_base = smem_u32(smem);
+    const uint32_t ring_base = stage_base + (uint32_t)P.nst * C::STAGE;
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + (size_t)P.nst * C::STAGE + C::RING_BYTES);
+    uint64_t *empty = full + MAX_ST;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n = *P.step;
+    const int par = (n + (ADJ ? 1 : 0)) & 1;       // forward step n reads buffer n&1; reverse step n reads (n+1)&1
+    constexpr int FA = ADJ ? 1 : 0, FB = ADJ ? 0 : 1;   // CPML family (tables, states) of phase A / phase B
+    const int nst = P.nst;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < nst; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], C::NCW); }
+        fence_mbar_init();
+    }
+    __syncthreads();
+
+    const int rot = n % P.n_rot;
+    const int *sb = P.seg_begin + rot * (P.n_cta + 1);
+    const Segment *segs = P.segs + (size_t)rot * P.seg_stride;
+    const int seg_lo = sb[blockIdx.x], seg_hi = sb[blockIdx.x + 1];
+
+    // ============================================================================== producer
+    if (warp == C::NCW) {
+        if (lane != 0) return;
+        const CUtensorMap *M = P.maps + par * 3;
+        int ld = 0;
+        for (int sg = seg_lo; sg < seg_hi; ++sg) {
+            const Segment S = segs[sg];
+            const int x = S.i0 - 4, y = S.j0 - 1;
+            for (int kk = S.k0 - 1; kk <= S.k1; ++kk, ++ld) {
+                const int s = ld % nst;
+                if (ld >= nst) mbar_wait(&empty[s], ((ld / nst) - 1) & 1);
+                uint64_t *fb = &full[s];
+                uint8_t *st = smem + (size_t)s * C::STAGE;
+                mbar_expect_tx(fb, 3u * C::BOX_BYTES);
+                tma_load_3d(st, M, x, y, kk, fb);
+                tma_load_3d(st + C::SLOT, M + 1, x, y, kk, fb);
+                tma_load_3d(st + 2 * C::SLOT, M + 2, x, y, kk, fb);
+            }
+        }
+        return;
+    }
+
+    // ============================================================================== consumers
+    const int wx = warp % C::PCX, wy = warp / C::PCX;
+    const int tx = wx * 8 + (lane & 7), ty = wy * 4 + (lane >> 3);
+    const bool act = tx < C::CW && ty < C::RW;                    // thread has a float4 of cells
+    const bool inner = act && ty < C::TY && tx < C::TX4;          // not a halo thread
+    const uint32_t o_own = ((1 + ty) * C::PW + 4 + 4 * tx) * 4;   // my first cell inside a box (bytes)
+    const uint32_t r_own = (ty * C::RP + 4 * tx) * 4;             // ... inside a ring array
+    const float *src = P.buf[par];
+    float *dst = P.buf[par ^ 1];
+    const PsiSet &qAi = ADJ ? P.psiH[par] : P.psiE[par], &qAo = ADJ ? P.psiH[par ^ 1] : P.psiE[par ^ 1];
+    const PsiSet &qBi = ADJ ? P.psiE[par] : P.psiH[par], &qBo = ADJ ? P.psiE[par ^ 1] : P.psiH[par ^ 1];
+    const float S = G.S;
+    const long long nc = G.nc;
+    const long long plane = (long long)G.ny * G.nx;
+    const bool pml = G.d > 0;
+    const bool has_mu = !ADJ && P.im != nullptr;
+
+    // k ranges of the planes that hold sources / detectors (forward only)
+    int sEl = 1 << 30, sEh = -1, sHl = 1 << 30, sHh = -1, dEl = 1 << 30, dEh = -1, dHl = 1 << 30, dHh = -1;
+    if (!ADJ) {
+        for (int s = 0; s < P.n_src; ++s) {
+            if (P.src[s].comp < 3) { sEl = min(sEl, P.src[s].lo[2]); sEh = max(sEh, P.src[s].hi[2]); }
+            else { sHl = min(sHl, P.src[s].lo[2]); sHh = max(sHh, P.src[s].hi[2]); }
+        }
+        for (int s = 0; s < P.n_det; ++s) {
+            if (P.det[s].mask & 7) { dEl = min(dEl, P.det[s].lo[2]); dEh = max(dEh, P.det[s].hi[2]); }
+            if (P.det[s].mask >> 3) { dHl = min(dHl, P.det[s].lo[2]); dHh = max(dHh, P.det[s].hi[2]); }
+        }
+    }
+    const float4 Z4 = splat(0.f);
+
+    int ld = 0;
+    for (int sg = seg_lo; sg < seg_hi; ++sg) {
+        const Segment Sg = segs[sg];
+        const int i = Sg.i0 + 4 * tx, j = Sg.j0 + ty;
+        const bool ing = act && i < G.nx && j < G.ny;              // my cells are inside the grid
+        const bool own_ok = inner && ing;
+        const long long own_xy = (long long)j * G.nx + i;
+        // slab-compact coordinates of my cells and (adjoint) of my -x / -y neighbours; -1: not in a slab
+        const int sx = (pml && ing) ? slab_pos(i, G.nx, G.dpx) : -1;
+        const int sy = (pml && ing) ? slab_pos(j, G.ny, G.d) : -1;
+        const int sxm = (ADJ && pml && ing) ? slab_pos(i - 1, G.nx, G.dpx) : -1;
+        const int sym = (ADJ && pml && ing) ? slab_pos(j - 1, G.ny, G.d) : -1;
+        const long long oy = (long long)sy * G.nx + i, oym = (long long)sym * G.nx + i;   // + k * 2d * nx
+        const long long ox = (long long)j * (2 * G.dpx) + sx, oxm = (long long)j * (2 * G.dpx) + sxm;   // + k * ny * 2dpx
+        const long long py = (long long)2 * G.d * G.nx, px = (long long)G.ny * 2 * G.dpx;
+
+        float4 hxk = Z4, hyk = Z4, hzk = Z4;                // H-type target of plane kk-1 at my cells (raw)
+        float4 fxk = Z4, fyk = Z4;                          // z operands of phase A from plane kk-1 (adjoint: filtered)
+        float4 cYx = Z4, cYz = Z4, cXy = Z4, cXz = Z4, cZx = Z4, cZy = Z4;   // phase-B operands of plane kk-1 at my cells
+        float4 ex = Z4, ey = Z4, ez = Z4, ie4 = Z4;         // E-type target and inv_eps of the plane about to be updated
+
+        for (int kk = Sg.k0 - 1; kk <= Sg.k1; ++kk, ++ld) {
+            const bool prolog = kk == Sg.k0 - 1;
+            const bool doB = kk >= Sg.k0 + 1;
+            const int s = ld % nst;
+            const int zs = pml ? slab_pos(kk, G.nz, G.d) : -1;
+            mbar_wait(&full[s], (ld / nst) & 1);
+            const uint32_t so = stage_base + (uint32_t)s * C::STAGE + o_own;
+            const long long off = (long long)kk * plane + own_xy;
+            const long long oz = ((long long)zs * G.ny + j) * G.nx + i;
+
+            float4 fx = Z4, fy = Z4, fz = Z4, fx_my = Z4, fz_my = Z4;
+            float fy_mx = 0.f, fz_mx = 0.f;
+            if (act) {
+                fx = lds4(so); fy = lds4(so + C::SLOT); fz = lds4(so + 2 * C::SLOT);
+                if (!prolog) {
+                    fx_my = lds4(so - C::ROWB); fz_my = lds4(so + 2 * C::SLOT - C::ROWB);
+                    fy_mx = lds1(so + C::SLOT - 4); fz_mx = lds1(so + 2 * C::SLOT - 4);
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[s]);
+
+            // the E-type target and inv_eps of the next plane
+            float4 nex = Z4, ney = Z4, nez = Z4, nie = Z4;
+            if (ing && kk + 1 <= Sg.k1 && kk + 1 < G.nz) {
+                const float *q = src + off + plane;
+                nex = ldg4(q); ney = ldg4(q + nc); nez = ldg4(q + 2 * nc);
+                nie = ldg4(P.ie + off + plane);
+            }
+
+            if (prolog) {
+                fxk = fx; fyk = fy;
+                if (ADJ && zs >= 0 && ing) {
+                    const float b = __ldg(P.T.b[FA][2] + kk), a = __ldg(P.T.a[FA][2] + kk), km = __ldg(P.T.ik[FA][2] + kk) - 1.f;
+                    float4 pn;
+                    fxk = fx + cpml4(b, a, km, ldg4(qAi.p[1][0] + oz), fx, pn);
+                    fyk = fy + cpml4(b, a, km, ldg4(qAi.p[0][1] + oz), fy, pn);
+                }
+                ex = nex; ey = ney; ez = nez; ie4 = nie;
+                continue;
+            }
+
+            const bool storeE = kk < Sg.k1;
+            const bool wr = own_ok && storeE;                  // I own these cells: write the result and the phase-A states
+            const uint32_t rgA = ring_base + (uint32_t)(kk & 1) * (C::RING_SLOT * 4) + r_own;
+            float4 gx = fx, gy = fy;                           // z operands of phase A at plane kk (adjoint: filtered)
+            float4 Yx = Z4, Yz = Z4, Xy = Z4, Xz = Z4, Zx = Z4, Zy = Z4;   // phase-B operands of plane kk at my cells
+            if (act) {
+                // ------------------------------------------------------------ phase A: E-type update of plane kk
+                float4 Dy_z = fz - fz_my, Dy_x = fx - fx_my;
+                float4 Dx_y = dminus_x(fy, fy_mx), Dx_z = dminus_x(fz, fz_mx);
+                float4 Dz_x, Dz_y;
+                if (!ADJ) {
+                    Dz_x = fx - fxk; Dz_y = fy - fyk;
+                    if (pml) {
+                        if (zs >= 0 && ing) {
+                            const float b = __ldg(P.T.b[FA][2] + kk), a = __ldg(P.T.a[FA][2] + kk), km = __ldg(P.T.ik[FA][2] + kk) - 1.f;
+                            float4 p0, p1;
+                            Dz_x = Dz_x + cpml4(b, a, km, ldg4(qAi.p[1][0] + oz), Dz_x, p0);
+                            Dz_y = Dz_y + cpml4(b, a, km, ldg4(qAi.p[0][1] + oz), Dz_y, p1);
+                            if (wr) { stg4(qAo.p[1][0] + oz, p0); stg4(qAo.p[0][1] + oz, p1); }
+                        }
+                        if (sy >= 0) {
+                            const float b = __ldg(P.T.b[FA][1] + j), a = __ldg(P.T.a[FA][1] + j), km = __ldg(P.T.ik[FA][1] + j) - 1.f;
+                            const long long q = kk * py + oy;
+                            float4 p0, p1;
+                            Dy_z = Dy_z + cpml4(b, a, km, ldg4(qAi.p[0][0] + q), Dy_z, p0);
+                            Dy_x = Dy_x + cpml4(b, a, km, ldg4(qAi.p[2][1] + q), Dy_x, p1);
+                            if (wr) { stg4(qAo.p[0][0] + q, p0); stg4(qAo.p[2][1] + q, p1); }
+                        }
+                        if (sx >= 0) {
+                            const float4 b = ldg4(P.T.b[FA][0] + i), a = ldg4(P.T.a[FA][0] + i), km = ldg4(P.T.ik[FA][0] + i) - splat(1.f);
+                            const long long q = kk * px + ox;
+                            float4 p0, p1;
+                            Dx_y = Dx_y + cpml4(b, a, km, ldg4(qAi.p[2][0] + q), Dx_y, p0);
+                            Dx_z = Dx_z + cpml4(b, a, km, ldg4(qAi.p[1][1] + q), Dx_z, p1);
+                            if (wr) { stg4(qAo.p[2][0] + q, p0); stg4(qAo.p[1][1] + q, p1); }
+                        }
+                    }
+                } else {
+                    if (pml) {
+                        if (zs >= 0 && ing) {
+                            const float b = __ldg(P.T.b[FA][2] + kk), a = __ldg(P.T.a[FA][2] + kk), km = __ldg(P.T.ik[FA][2] + kk) - 1.f;
+                            float4 p0, p1;
+                            gx = fx + cpml4(b, a, km, ldg4(qAi.p[1][0] + oz), fx, p0);
+                            gy = fy + cpml4(b, a, km, ldg4(qAi.p[0][1] + oz), fy, p1);
+                            if (wr) { stg4(qAo.p[1][0] + oz, p0); stg4(qAo.p[0][1] + oz, p1); }
+                        }
+                        if (sy >= 0) {
+                            const float b = __ldg(P.T.b[FA][1] + j), a = __ldg(P.T.a[FA][1] + j), km = __ldg(P.T.ik[FA][1] + j) - 1.f;
+                            const long long q = kk * py + oy;
+                            float4 p0, p1;
+                            Dy_z = Dy_z + cpml4(b, a, km, ldg4(qAi.p[0][0] + q), fz, p0);
+                            Dy_x = Dy_x + cpml4(b, a, km, ldg4(qAi.p[2][1] + q), fx, p1);
+                            if (wr) { stg4(qAo.p[0][0] + q, p0); stg4(qAo.p[2][1] + q, p1); }
+                        }
+                        if (sym >= 0) {
+                            const float b = __ldg(P.T.b[FA][1] + j - 1), a = __ldg(P.T.a[FA][1] + j - 1), km = __ldg(P.T.ik[FA][1] + j - 1) - 1.f;
+                            const long long q = kk * py + oym;
+                            float4 p0, p1;
+                            Dy_z = Dy_z - cpml4(b, a, km, ldg4(qAi.p[0][0] + q), fz_my, p0);
+                            Dy_x = Dy_x - cpml4(b, a, km, ldg4(qAi.p[2][1] + q), fx_my, p1);
+                        }
+                        if (sx >= 0 || sxm >= 0) {
+                            float4 cy = Z4, cz = Z4;
+                            float ly = 0.f, lz = 0.f;
+                            if (sx >= 0) {
+                                const float4 b = ldg4(P.T.b[FA][0] + i), a = ldg4(P.T.a[FA][0] + i), km = ldg4(P.T.ik[FA][0] + i) - splat(1.f);
+                                const long long q = kk * px + ox;
+                                float4 p0, p1;
+                                cy = cpml4(b, a, km, ldg4(qAi.p[2][0] + q), fy, p0);
+                                cz = cpml4(b, a, km, ldg4(qAi.p[1][1] + q), fz, p1);
+                                if (wr) { stg4(qAo.p[2][0] + q, p0); stg4(qAo.p[1][1] + q, p1); }
+                            }
+                            if (sxm >= 0) {
+                                const float b = __ldg(P.T.b[FA][0] + i - 1), a = __ldg(P.T.a[FA][0] + i - 1), km = __ldg(P.T.ik[FA][0] + i - 1) - 1.f;
+                                const long long q = kk * px + oxm;
+                                ly = cpml1(b, a, km, __ldg(qAi.p[2][0] + q), fy_mx);
+                                lz = cpml1(b, a, km, __ldg(qAi.p[1][1] + q), fz_mx);
+                            }
+                            Dx_y = Dx_y + dminus_x(cy, ly);
+                            Dx_z = Dx_z + dminus_x(cz, lz);
+                        }
+                    }
+                    Dz_x = gx - fxk; Dz_y = gy - fyk;
+                }
+                const float4 tEx = Dy_z - Dz_y, tEy = Dz_x - Dx_z, tEz = Dx_y - Dy_x;
+                const float4 sie = S * ie4;
+                float4 e2x, e2y, e2z, v2x, v2y, v2z;
+                if (ADJ) {
+                    e2x = fma4(-S, tEx, ex); e2y = fma4(-S, tEy, ey); e2z = fma4(-S, tEz, ez);
+                    v2x = sie * e2x; v2y = sie * e2y; v2z = sie * e2z;
+                } else {
+                    e2x = fma4(sie, tEx, ex); e2y = fma4(sie, tEy, ey); e2z = fma4(sie, tEz, ez);
+                    if (kk >= sEl && kk < sEh) add_sources4(P, n, 0, e2x, e2y, e2z, i, j, kk);
+                    v2x = e2x; v2y = e2y; v2z = e2z;
+                }
+                if (wr) {
+                    float *o = dst + off;
+                    stg4(o, e2x); stg4(o + nc, e2y); stg4(o + 2 * nc, e2z);
+                    if (!ADJ && kk >= dEl && kk < dEh) detect4(P, n, 0, e2x, e2y, e2z, i, j, kk);
+                }
+                Yx = v2x; Yz = v2z; Xy = v2y; Xz = v2z; Zx = v2x; Zy = v2y;
+                if (ADJ && pml) {       // phase-B operands are filtered where they are produced
+                    if (zs >= 0 && ing) {
+                        const float b = __ldg(P.T.b[FB][2] + kk), a = __ldg(P.T.a[FB][2] + kk), km = __ldg(P.T.ik[FB][2] + kk) - 1.f;
+                        float4 p0, p1;
+                        Zx = v2x + cpml4(b, a, km, ldg4(qBi.p[1][0] + oz), v2x, p0);
+                        Zy = v2y + cpml4(b, a, km, ldg4(qBi.p[0][1] + oz), v2y, p1);
+                        if (wr) { stg4(qBo.p[1][0] + oz, p0); stg4(qBo.p[0][1] + oz, p1); }
+                    }
+                    if (sy >= 0) {
+                        const float b = __ldg(P.T.b[FB][1] + j), a = __ldg(P.T.a[FB][1] + j), km = __ldg(P.T.ik[FB][1] + j) - 1.f;
+                        const long long q = kk * py + oy;
+                        float4 p0, p1;
+                        Yz = v2z + cpml4(b, a, km, ldg4(qBi.p[0][0] + q), v2z, p0);
+                        Yx = v2x + cpml4(b, a, km, ldg4(qBi.p[2][1] + q), v2x, p1);
+                        if (wr) { stg4(qBo.p[0][0] + q, p0); stg4(qBo.p[2][1] + q, p1); }
+                    }
+                    if (sx >= 0) {
+                        const float4 b = ldg4(P.T.b[FB][0] + i), a = ldg4(P.T.a[FB][0] + i), km = ldg4(P.T.ik[FB][0] + i) - splat(1.f);
+                        const long long q = kk * px + ox;
+                        float4 p0, p1;
+                        Xy = v2y + cpml4(b, a, km, ldg4(qBi.p[2][0] + q), v2y, p0);
+                        Xz = v2z + cpml4(b, a, km, ldg4(qBi.p[1][1] + q), v2z, p1);
+                        if (wr) { stg4(qBo.p[2][0] + q, p0); stg4(qBo.p[1][1] + q, p1); }
+                    }
+                }
+                sts4(rgA, Yx); sts4(rgA + C::RING_ARR * 4, Yz); sts4(rgA + 2 * C::RING_ARR * 4, Xy);
+                if (ADJ) sts4(rgA + 3 * C::RING_ARR * 4, Xz);
+            }
+            // ---------------------------------------------------------------- phase B: H-type update of plane kk-1
+            if (own_ok && doB) {
+                const int km1 = kk - 1;
+                const uint32_t rgB = ring_base + (uint32_t)(km1 & 1) * (C::RING_SLOT * 4) + r_own;
+                const float4 Yx_py = lds4(rgB + C::RP * 4), Yz_py = lds4(rgB + (C::RING_ARR + C::RP) * 4);
+                const float Xy_px = lds1(rgB + (2 * C::RING_ARR + 4) * 4);
+                const float Xz_px = lds1(rgB + ((ADJ ? 3 : 1) * C::RING_ARR + 4) * 4);
+                float4 Dy_z = Yz_py - cYz, Dy_x = Yx_py - cYx;
+                float4 Dz_y = Zy - cZy, Dz_x = Zx - cZx;
+                float4 Dx_z = dplus_x(cXz, Xz_px), Dx_y = dplus_x(cXy, Xy_px);
+                const long long offm = off - plane;
+                if (!ADJ && pml) {
+                    const int zsm = slab_pos(km1, G.nz, G.d);
+                    if (zsm >= 0) {
+                        const float b = __ldg(P.T.b[FB][2] + km1), a = __ldg(P.T.a[FB][2] + km1), km = __ldg(P.T.ik[FB][2] + km1) - 1.f;
+                        const long long q = ((long long)zsm * G.ny + j) * G.nx + i;
+                        float4 p0, p1;
+                        Dz_x = Dz_x + cpml4(b, a, km, ldg4(qBi.p[1][0] + q), Dz_x, p0);
+                        Dz_y = Dz_y + cpml4(b, a, km, ldg4(qBi.p[0][1] + q), Dz_y, p1);
+                        stg4(qBo.p[1][0] + q, p0); stg4(qBo.p[0][1] + q, p1);
+                    }
+                    if (sy >= 0) {
+                        const float b = __ldg(P.T.b[FB][1] + j), a = __ldg(P.T.a[FB][1] + j), km = __ldg(P.T.ik[FB][1] + j) - 1.f;
+                        const long long q = km1 * py + oy;
+                        float4 p0, p1;
+                        Dy_z = Dy_z + cpml4(b, a, km, ldg4(qBi.p[0][0] + q), Dy_z, p0);
+                        Dy_x = Dy_x + cpml4(b, a, km, ldg4(qBi.p[2][1] + q), Dy_x, p1);
+                        stg4(qBo.p[0][0] + q, p0); stg4(qBo.p[2][1] + q, p1);
+                    }
+                    if (sx >= 0) {
+                        const float4 b = ldg4(P.T.b[FB][0] + i), a = ldg4(P.T.a[FB][0] + i), km = ldg4(P.T.ik[FB][0] + i) - splat(1.f);
+                        const long long q = km1 * px + ox;
+                        float4 p0, p1;
+                        Dx_y = Dx_y + cpml4(b, a, km, ldg4(qBi.p[2][0] + q), Dx_y, p0);
+                        Dx_z = Dx_z + cpml4(b, a, km, ldg4(qBi.p[1][1] + q), Dx_z, p1);
+                        stg4(qBo.p[2][0] + q, p0); stg4(qBo.p[1][1] + q, p1);
+                    }
+                }
+                const float4 tHx = Dy_z - Dz_y, tHy = Dz_x - Dx_z, tHz = Dx_y - Dy_x;
+                float4 h2x, h2y, h2z;
+                if (ADJ) {
+                    h2x = hxk + tHx; h2y = hyk + tHy; h2z = hzk + tHz;
+                } else {
+                    const float4 sim = has_mu ? S * ldg4(P.im + offm) : splat(S);
+                    h2x = hxk - sim * tHx; h2y = hyk - sim * tHy; h2z = hzk - sim * tHz;
+                    if (km1 >= sHl && km1 < sHh) add_sources4(P, n, 1, h2x, h2y, h2z, i, j, km1);
+                }
+                float *o = dst + 3 * nc + offm;
+                stg4(o, h2x); stg4(o + nc, h2y); stg4(o + 2 * nc, h2z);
+                if (!ADJ && km1 >= dHl && km1 < dHh) detect4(P, n, 1, h2x, h2y, h2z, i, j, km1);
+            }
+            cYx = Yx; cYz = Yz; cXy = Xy; cXz = Xz; cZx = Zx; cZy = Zy;
+            hxk = fx; hyk = fy; hzk = fz;
+            fxk = gx; fyk = gy;
+            ex = nex; ey = ney; ez = nez; ie4 = nie;
+            named_bar_sync(1, C::NCW * 32);      // ring slot (kk-1)&1 may be overwritten in the next iteration
+        }
+    }
+}
+
+// ================================================================================================
+// host side
+// ================================================================================================
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode()
+{
+    static EncodeTiledFn fn = nullptr;
+    if (fn) return fn;
+    void *p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || !p) {
+        (void)cudaGetLastError();
+        return nullptr;
+    }
+    fn = (EncodeTiledFn)p;
+    return fn;
+}
+
+// 3-D fp32 tensor (dx fastest) with row pitch / plane pitch in floats
+bool encode3d(CUtensorMap *out, const float *base, long long dx, long long dy, long long dz, long long pitch_y,
+              long long pitch_z, int bx, int by)
+{
+    EncodeTiledFn fn = get_encode();
+    if (!fn) return false;
+    cuuint64_t dims[3] = { (cuuint64_t)dx, (cuuint64_t)dy, (cuuint64_t)dz };
+    cuuint64_t strides[2] = { (cuuint64_t)pitch_y * 4, (cuuint64_t)pitch_z * 4 };
+    cuuint32_t box[3] = { (cuuint32_t)bx, (cuuint32_t)by, 1 };
+    cuuint32_t es[3] = { 1, 1, 1 };
+    return fn(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// ---- the compiled tile shapes ----------------------------------------------------------------------
+struct TileImpl {
+    int TX, TY, threads, ncw, stage, ring_bytes;
+    void (*launch_fwd)(const StepParams &, int n_cta, size_t smem, cudaStream_t);
+    void (*launch_adj)(const StepParams &, int n_cta, size_t smem, cudaStream_t);
+    cudaError_t (*set_smem)(size_t);
+};
+template <class C> void launch_fwd_impl(const StepParams &P, int n_cta, size_t smem, cudaStream_t st)
+{
+    k_step<C, false><<<n_cta, C::THREADS, smem, st>>>(P);
+}
+template <class C> void launch_adj_impl(const StepParams &P, int n_cta, size_t smem, cudaStream_t st)
+{
+    k_step<C, true><<<n_cta, C::THREADS, smem, st>>>(P);
+}
+template <class C> cudaError_t set_smem_impl(size_t smem)
+{
+    cudaError_t e = cudaFuncSetAttribute(k_step<C, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step<C, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    return e;
+}
+#define TILE(TX4, TY) { 4 * TX4, TY, Cfg<TX4, TY>::THREADS, Cfg<TX4, TY>::NCW, Cfg<TX4, TY>::STAGE, Cfg<TX4, TY>::RING_BYTES, \
+                        launch_fwd_impl<Cfg<TX4, TY>>, launch_adj_impl<Cfg<TX4, TY>>, set_smem_impl<Cfg<TX4, TY>> }
+const TileImpl kTiles[] = {
+    TILE(2, 3), TILE(4, 3), TILE(8, 7), TILE(16, 7), TILE(16, 15), TILE(25, 7), TILE(25, 11),
+    TILE(32, 7), TILE(32, 11), TILE(50, 7), TILE(50, 11), TILE(62, 7),
+};
+constexpr int kNumTiles = sizeof(kTiles) / sizeof(kTiles[0]);
+
+}  // namespace
+
+struct FusedState {
+    const TileImpl *tile = nullptr;
+    int TX = 0, TY = 0, nst = 0, n_cta = 0, n_rot = 1;
+    size_t smem = 0;
+    StepParams sp{};
+    float *bufB = nullptr;                 // second primal field buffer
+    float *lamB = nullptr;                 // second cotangent buffer
+    // tensor-map tables: [0] primal (fields / bufB), [1] cotangents (lam / lamB); entry set*3 + c
+    CUtensorMap *d_maps[2] = { nullptr, nullptr };
+    CUtensorMap *h_maps[2] = { nullptr, nullptr };   // pinned staging
+    cudaEvent_t maps_done = nullptr;
+    Segment *d_segs = nullptr;
+    int *d_seg_begin = nullptr;
+    const float *maps_key[2] = { nullptr, nullptr };   // volume A the maps were built for
+};
+
+namespace {
+
+// Work sequence: z is cut into n_chunk chunks; the sequence is (chunk, tile [y fastest], plane in chunk); it is
+// rotated by `rot` positions and cut into n_cta equal runs.  With chunk length ~ run length, CTAs that hold
+// y-adjacent tiles march through the same planes at about the same time, so halo rows hit L2.
+void make_segments(const Dims &G, int TX, int TY, int n_cta, int n_chunk, long long rot, std::vector<Segment> &segs,
+                   std::vector<int> &seg_begin)
+{
+    const int ntx = (G.nx + TX - 1) / TX, nty = (G.ny + TY - 1) / TY;
+    const long long n_tiles = (long long)ntx * nty;
+    const long long total = n_tiles * G.nz;
+    std::vector<int> cb(n_chunk + 1);
+    for (int c = 0; c <= n_chunk; ++c) cb[c] = (int)((long long)G.nz * c / n_chunk);
+    std::vector<long long> cstart(n_chunk + 1, 0);       // sequence position where each chunk begins
+    for (int c = 0; c < n_chunk; ++c) cstart[c + 1] = cstart[c] + n_tiles * (cb[c + 1] - cb[c]);
+    segs.clear();
+    seg_begin.assign(n_cta + 1, 0);
+    rot = ((rot % total) + total) % total;
+    for (int cta = 0; cta < n_cta; ++cta) {
+        seg_begin[cta] = (int)segs.size();
+        long long a = total * cta / n_cta, b = total * (cta + 1) / n_cta;      // positions in the rotated sequence
+        while (a < b) {
+            const long long pos = (a + rot) % total;                            // position in the canonical sequence
+            int c = (int)(std::upper_bound(cstart.begin(), cstart.end(), pos) - cstart.begin()) - 1;
+            const int clen = cb[c + 1] - cb[c];
+            const long long in_chunk = pos - cstart[c];
+            const long long tile = in_chunk / clen;
+            const int k = cb[c] + (int)(in_chunk % clen);
+            const int len = (int)std::min<long long>(std::min<long long>(b - a, total - pos), cb[c + 1] - k);
+            const int txi = (int)(tile / nty), tyi = (int)(tile % nty);
+            Segment s{};
+            s.i0 = txi * TX; s.j0 = tyi * TY; s.k0 = k; s.k1 = k + len;
+            segs.push_back(s);
+            a += len;
+        }
+    }
+    seg_begin[n_cta] = (int)segs.size();
+}
+
+}  // namespace
+
+int fused_setup(fdtd_grid *g)
+{
+    const Dims &G = g->G;
+    if (g->desc.path == FDTD_PATH_GENERIC) { g->fused_why_not = "generic path requested"; return FDTD_OK; }
+    if (G.periodic) { g->fused_why_not = "periodic grids use the generic kernels"; return FDTD_OK; }
+    if (G.nx % 4) { g->fused_why_not = "nx is not a multiple of 4"; return FDTD_OK; }
+    if (G.d > 0 && (G.dpx % 4)) { g->fused_why_not = "x-slab psi storage is not float4 aligned (nx < 2*roundup4(d))"; return FDTD_OK; }
+    if (!get_encode()) { g->fused_why_not = "cuTensorMapEncodeTiled is not available"; return FDTD_OK; }
+    int dev = 0, smem_cap = 0, n_sm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&smem_cap, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        (void)cudaGetLastError();
+        g->fused_why_not = "cannot query the device";
+        return FDTD_OK;
+    }
+
+    // ---- tile choice among the compiled shapes: fewest consumer warp-planes per grid plane -------------------------
+    int fTX = 0, fTY = 0;
+    if (const char *e = getenv("FDTD_TILE")) sscanf(e, "%d,%d", &fTX, &fTY);
+    const int tail_bytes = 2 * MAX_ST * 8;
+    const TileImpl *best = nullptr;
+    double best_score = -1;
+    int best_nst = 0;
+    for (int q = 0; q < kNumTiles; ++q) {
+        const TileImpl &t = kTiles[q];
+        if (fTX && (t.TX != fTX || t.TY != fTY)) continue;
+        const int nst = std::min(MAX_ST, (smem_cap - t.ring_bytes - tail_bytes - 1024) / t.stage);
+        if (nst < 2) continue;
+        const long long ntx = (G.nx + t.TX - 1) / t.TX, nty = (G.ny + t.TY - 1) / t.TY;
+        const double eff = ((double)G.nx / 4 * G.ny) / ((double)ntx * nty * t.ncw * 32);
+        const double fill = std::min(1.0, (double)ntx * nty * G.nz / (8.0 * n_sm));   // enough planes per CTA to amortise prologues
+        const double warps = std::min(1.0, t.ncw / 10.0);                             // enough warps to hide latency
+        const double score = eff * fill * warps;
+        if (score > best_score) { best_score = score; best = &t; best_nst = nst; }
+    }
+    if (!best) { g->fused_why_not = "no compiled tile shape fits"; return FDTD_OK; }
+
+    FusedState *F = new FusedState();
+    g->fused = F;
+    F->tile = best; F->TX = best->TX; F->TY = best->TY; F->nst = best_nst;
+    if (const char *e = getenv("FDTD_NST")) F->nst = std::max(2, std::min(best_nst, atoi(e)));
+    F->smem = (size_t)F->nst * best->stage + best->ring_bytes + tail_bytes;
+    int rc;
+    if ((rc = g->alloc((void **)&F->bufB, (size_t)G.nc * 6 * sizeof(float)))) return rc;
+    if ((rc = g->alloc_psi(g->psiE[1])) || (rc = g->alloc_psi(g->psiH[1]))) return rc;
+    for (int q = 0; q < 2; ++q) {
+        if ((rc = g->alloc((void **)&F->d_maps[q], sizeof(CUtensorMap) * 6))) return rc;
+        if (cudaMallocHost((void **)&F->h_maps[q], sizeof(CUtensorMap) * 6) != cudaSuccess) {
+            (void)cudaGetLastError();
+            return fdtd_fail(FDTD_ENOMEM, "pinned tensor-map staging allocation failed");
+        }
+    }
+    if (cudaEventCreateWithFlags(&F->maps_done, cudaEventDisableTiming) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return fdtd_fail(FDTD_ENOMEM, "event creation failed");
+    }
+
+    // ---- segments ---------------------------------------------------------------------------------------------------
+    const int ntx = (G.nx + F->TX - 1) / F->TX, nty = (G.ny + F->TY - 1) / F->TY;
+    const long long total = (long long)ntx * nty * G.nz;
+    int n_cta = (int)std::min<long long>(n_sm, std::max<long long>(1, total / 6));
+    if (const char *e = getenv("FDTD_NCTA")) n_cta = std::max(1, atoi(e));
+    const double run = (double)total / n_cta;                         // planes per CTA
+    int n_chunk = 1;
+    (void)run;
+    if (const char *e = getenv("FDTD_NCHUNK")) n_chunk = std::max(1, std::min(G.nz, atoi(e)));
+    // rotation of the work sequence between steps (n_rot tables, step n uses table n % n_rot)
+    int n_rot = 1;
+    if (const char *e = getenv("FDTD_NROT")) n_rot = std::max(1, std::min(16, atoi(e)));
+    F->n_cta = n_cta; F->n_rot = n_rot;
+    std::vector<Segment> all;
+    std::vector<int> begins;
+    std::vector<std::vector<Segment>> per(n_rot);
+    std::vector<std::vector<int>> per_b(n_rot);
+    size_t stride = 0;
+    for (int r = 0; r < n_rot; ++r) {
+        const long long per_cta = total / n_cta;
+        make_segments(G, F->TX, F->TY, n_cta, n_chunk, -(long long)r * (per_cta / n_rot), per[r], per_b[r]);
+        stride = std::max(stride, per[r].size());
+    }
+    all.resize(stride * n_rot);
+    for (int r = 0; r < n_rot; ++r) {
+        std::copy(per[r].begin(), per[r].end(), all.begin() + r * stride);
+        begins.insert(begins.end(), per_b[r].begin(), per_b[r].end());
+    }
+    if ((rc = g->alloc((void **)&F->d_segs, all.size() * sizeof(Segment)))) return rc;
+    if ((rc = g->alloc((void **)&F->d_seg_begin, begins.size() * sizeof(int)))) return rc;
+    if (cudaMemcpy(F->d_segs, all.data(), all.size() * sizeof(Segment), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(F->d_seg_begin, begins.data(), begins.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return fdtd_fail(FDTD_ECUDA, "upload of the segment table failed");
+    }
+
+    // ---- kernel parameters that do not depend on the call -----------------------------------------------------------
+    StepParams &P = F->sp;
+    P.G = G; P.T = g->T; P.segs = F->d_segs; P.seg_begin = F->d_seg_begin;
+    P.n_rot = n_rot; P.seg_stride = (int)stride; P.n_cta = n_cta;
+    P.step = g->d_step;
+    P.nst = F->nst;
+    if (best->set_smem(F->smem) != cudaSuccess) {
+        (void)cudaGetLastError();
+        g->fused_why_not = "cannot reserve shared memory";
+        return FDTD_OK;
+    }
+    g->path = FDTD_PATH_FUSED;
+    g->fused_backward_ready = true;
+    g->tile_x = F->TX; g->tile_y = F->TY;
+    g->tile_z = (int)std::min<long long>(G.nz, total / n_cta);
+    return FDTD_OK;
+}
+
+void fused_teardown(fdtd_grid *g)
+{
+    if (g->fused) {
+        for (int q = 0; q < 2; ++q) if (g->fused->h_maps[q]) cudaFreeHost(g->fused->h_maps[q]);
+        if (g->fused->maps_done) cudaEventDestroy(g->fused->maps_done);
+    }
+    delete g->fused;
+    g->fused = nullptr;
+}
+
+namespace {
+
+// (re)builds one tensor-map table when the volume it was built for changed.
+//   which = 0: volumes A/B = fields / bufB;  which = 1: lam / lamB
+int build_maps(fdtd_grid *g, int which, float *volA, float *volB, cudaStream_t st)
+{
+    FusedState *F = g->fused;
+    const Dims &G = g->G;
+    if (F->maps_key[which] == volA) return FDTD_OK;
+    const int PW = F->TX + 8, ROWS = F->TY + 2;
+    if (cudaEventSynchronize(F->maps_done) != cudaSuccess) { (void)cudaGetLastError(); }   // earlier upload finished
+    CUtensorMap *H = F->h_maps[which];
+    bool ok = true;
+    float *bufs[2] = { volA, volB };
+    for (int set = 0; set < 2; ++set)
+        for (int c = 0; c < 3; ++c)
+            ok &= encode3d(&H[set * 3 + c], bufs[set] + (long long)(3 + c) * G.nc, G.nx, G.ny, G.nz, G.nx,
+                           (long long)G.nx * G.ny, PW, ROWS);
+    if (!ok) return fdtd_fail(FDTD_ECUDA, "cuTensorMapEncodeTiled failed");
+    cudaError_t e = cudaMemcpyAsync(F->d_maps[which], H, sizeof(CUtensorMap) * 6, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaEventRecord(F->maps_done, st);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return fdtd_fail(FDTD_ECUDA, std::string("tensor map upload: ") + cudaGetErrorString(e)); }
+    F->maps_key[which] = volA;
+    return FDTD_OK;
+}
+
+}  // namespace
+
+// run_steps lives in fdtd_api.cu; reached through small trampolines
+int fdtd_run_steps_fwd(fdtd_grid *g, const std::string &key, int n_steps, int launches_per_step, cudaStream_t st,
+                       void (*enqueue)(void *, cudaStream_t), void *ctx);
+int fdtd_run_steps_bwd(fdtd_grid *g, const std::string &key, int n_steps, int launches_per_step, cudaStream_t st,
+                       void (*enqueue)(void *, cudaStream_t), void *ctx);
+
+namespace {
+struct FwdCtx {
+    fdtd_grid *g; StepParams P; bool recording; float *A; float *B;
+};
+void enqueue_fwd(void *vctx, cudaStream_t cs)
+{
+    FwdCtx *c = (FwdCtx *)vctx;
+    fdtd_grid *g = c->g;
+    FusedState *F = g->fused;
+    { ProfScope p(g, fdtd_grid::PC_FUSED_FWD, cs);
+      F->tile->launch_fwd(c->P, F->n_cta, F->smem, cs); }
+    if (c->recording) {
+        // step n read buffer n&1 (pre-step H) and wrote buffer (n+1)&1 (E'); the record kernel picks them by parity
+        ProfScope p(g, fdtd_grid::PC_RECORD, cs);
+        launch_record_pp(g->G, g->R, c->A, c->B, g->rec, g->d_step, cs);
+    }
+    { ProfScope p(g, fdtd_grid::PC_OTHER, cs); launch_advance(g->d_step, 1, cs); }
+}
+
+struct BwdCtx {
+    fdtd_grid *g; StepParams P; float *fields; const float *ie; float *grad; float *lamA; float *lamB;
+    const std::vector<SourceDev> *S; const std::vector<DetectorDev> *D; int total_freq;
+};
+// reverse step n: B1 (detector cotangents into the volume about to be read), B2+B5 (fused adjoint step),
+// then the primal inverse step B3+B4 with lamE' taken from the volume the adjoint step just wrote
+void enqueue_bwd(void *vctx, cudaStream_t cs)
+{
+    BwdCtx *c = (BwdCtx *)vctx;
+    fdtd_grid *g = c->g;
+    FusedState *F = g->fused;
+    const Dims &G = g->G;
+    { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
+      for (const DetectorDev &dt : *c->D)
+          if (dt.phasor) launch_detector_adjoint_pp(G, c->lamA, c->lamB, dt, g->d_cs, c->total_freq, g->d_step, cs); }
+    { ProfScope p(g, fdtd_grid::PC_FUSED_BWD, cs);
+      F->tile->launch_adj(c->P, F->n_cta, F->smem, cs); }
+    { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
+      for (const SourceDev &s : *c->S) if (s.comp >= 3) launch_add_source(G, c->fields, s, g->d_step, -1.f, cs); }
+    if (G.d > 0) { ProfScope p(g, fdtd_grid::PC_INJECT, cs); launch_inject(G, g->R, c->fields, g->rec, g->d_step, cs); }
+    { ProfScope p(g, fdtd_grid::PC_INV_H, cs); launch_inv_H(G, c->fields, nullptr, cs); }
+    { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
+      for (const SourceDev &s : *c->S) if (s.comp < 3) launch_add_source(G, c->fields, s, g->d_step, -1.f, cs); }
+    { ProfScope p(g, fdtd_grid::PC_INV_E_GRAD, cs);
+      launch_inv_E_grad_pp(G, c->fields, c->ie, c->lamA, c->lamB, g->d_step, c->grad, cs); }
+    { ProfScope p(g, fdtd_grid::PC_OTHER, cs); launch_advance(g->d_step, -1, cs); }
+}
+}  // namespace
+
+int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
+                  const std::vector<SourceDev> &S, const std::vector<DetectorDev> &D, int total_freq, int n_steps,
+                  bool recording, cudaStream_t st)
+{
+    FusedState *F = g->fused;
+    if ((int)S.size() > MAX_SRC || (int)D.size() > MAX_DET)
+        return fdtd_fail(FDTD_EINVAL, "the fused path takes at most 4 sources and 4 detectors (use FDTD_PATH_GENERIC)");
+    int rc = build_maps(g, 0, fields, F->bufB, st);
+    if (rc) return rc;
+    for (int q = 0; q < 2; ++q)
+        if ((rc = g->zero_psi(g->psiE[q], st)) || (rc = g->zero_psi(g->psiH[q], st))) return rc;
+    FwdCtx ctx{ g, F->sp, recording, fields, F->bufB };
+    StepParams &P = ctx.P;
+    P.maps = F->d_maps[0];
+    P.buf[0] = fields; P.buf[1] = F->bufB;
+    P.ie = inv_eps; P.im = inv_mu;
+    for (int q = 0; q < 2; ++q) { P.psiE[q] = g->psiE[q]; P.psiH[q] = g->psiH[q]; }
+    P.n_src = (int)S.size(); P.n_det = (int)D.size(); P.total_freq = total_freq;
+    for (size_t q = 0; q < S.size(); ++q) P.src[q] = S[q];
+    for (size_t q = 0; q < D.size(); ++q) P.det[q] = D[q];
+    P.cs = g->d_cs;
+    std::string key("ff");
+    key.append((const char *)&P, sizeof(P));
+    key.push_back(recording ? 1 : 0);
+    rc = fdtd_run_steps_fwd(g, key, n_steps, 2 + (recording ? 1 : 0), st, enqueue_fwd, &ctx);
+    if (rc) return rc;
+    if (n_steps & 1) {
+        cudaError_t e = cudaMemcpyAsync(fields, F->bufB, (size_t)g->G.nc * 6 * sizeof(float), cudaMemcpyDeviceToDevice, st);
+        if (e != cudaSuccess) { (void)cudaGetLastError(); return fdtd_fail(FDTD_ECUDA, cudaGetErrorString(e)); }
+    }
+    return FDTD_OK;
+}
+
+// The cotangent seed is in g->lam; reverse step n reads volume (n+1)&1 and writes n&1, so after step 0 the
+// result is back in volume 0 = g->lam.
+int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
+                   const std::vector<SourceDev> &S, const std::vector<DetectorDev> &D, int total_freq, int n_steps,
+                   float *dL_dinv_eps, cudaStream_t st)
+{
+    FusedState *F = g->fused;
+    if (inv_mu) return fdtd_fail(FDTD_ESTATE, "fused backward does not take inv_mu");
+    const size_t vol6 = (size_t)g->G.nc * 6 * sizeof(float);
+    int rc;
+    if (!F->lamB && (rc = g->alloc((void **)&F->lamB, vol6))) return rc;
+    if ((rc = build_maps(g, 1, g->lam, F->lamB, st))) return rc;
+    if (n_steps & 1) {
+        cudaError_t e = cudaMemcpyAsync(F->lamB, g->lam, vol6, cudaMemcpyDeviceToDevice, st);
+        if (e != cudaSuccess) { (void)cudaGetLastError(); return fdtd_fail(FDTD_ECUDA, cudaGetErrorString(e)); }
+    }
+    BwdCtx ctx{ g, F->sp, fields, inv_eps, dL_dinv_eps, g->lam, F->lamB, &S, &D, total_freq };
+    StepParams &P = ctx.P;
+    P.maps = F->d_maps[1];
+    P.buf[0] = g->lam; P.buf[1] = F->lamB;
+    P.ie = inv_eps; P.im = nullptr;
+    for (int q = 0; q < 2; ++q) { P.psiE[q] = g->lpsiE[q]; P.psiH[q] = g->lpsiH[q]; }
+    P.n_src = 0; P.n_det = 0; P.total_freq = total_freq;
+    P.cs = g->d_cs;
+    int n_adj = 0;
+    for (const DetectorDev &dt : D) if (dt.phasor) ++n_adj;
+    std::string key("fb");
+    key.append((const char *)&P, sizeof(P));
+    key.append((const char *)&fields, sizeof(fields));
+    key.append((const char *)&dL_dinv_eps, sizeof(dL_dinv_eps));
+    if (!S.empty()) key.append((const char *)S.data(), S.size() * sizeof(SourceDev));
+    if (!D.empty()) key.append((const char *)D.data(), D.size() * sizeof(DetectorDev));
+    return fdtd_run_steps_bwd(g, key, n_steps, 4 + n_adj + (int)S.size() + (g->G.d > 0 ? 1 : 0), st, enqueue_bwd, &ctx);
+}
