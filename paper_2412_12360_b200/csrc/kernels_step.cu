@@ -45,7 +45,7 @@ constexpr int MAX_ST = 8;               // upper bound of pipeline stages
 struct StepParams {
     Dims G;
     Tables T;
-    const CUtensorMap *maps;       // [set][3]: H-type components of buffer `set`
+    const CUtensorMap *maps;       // [set][6]: components of buffer `set`; [12]: inv_eps
     const Segment *segs;           // [n_rot][seg_stride]
     const int *seg_begin;          // [n_rot][n_cta + 1]
     int n_rot, seg_stride, n_cta;
@@ -55,6 +55,7 @@ struct StepParams {
     const int *step;
     int nst;                       // pipeline stages
     int n_src, n_det, total_freq;
+    int sEl, sEh, sHl, sHh, dEl, dEh, dHl, dHh;   // k ranges of the planes that hold E/H sources and E/H detectors
     SourceDev src[MAX_SRC];
     DetectorDev det[MAX_DET];
     const float *cs;
@@ -71,7 +72,7 @@ struct Cfg {
     static constexpr int ROWB = PW * 4;                                 // box row pitch in bytes
     static constexpr int BOX_BYTES = PW * ROWS * 4;                     // TMA transaction bytes of one box
     static constexpr int SLOT = (BOX_BYTES + 127) / 128 * 128;
-    static constexpr int STAGE = 3 * SLOT;
+    static constexpr int STAGE = 7 * SLOT;                               // F x3, e x3, inv_eps
     static constexpr int RP = 4 * CW;                                   // ring row pitch (floats)
     static constexpr int RING_ARR = RW * RP;                            // floats of one ring array
     static constexpr int RING_SLOT = 4 * RING_ARR;                      // Yx, Yz, Xy, Xz
@@ -162,17 +163,14 @@ __device__ __noinline__ void detect_cell(const StepParams &P, int n, int comp, f
 
 __device__ __forceinline__ float f4get(const float4 &v, int q) { return q == 0 ? v.x : (q == 1 ? v.y : (q == 2 ? v.z : v.w)); }
 
-// adds the sources of `family` (0 = E, 1 = H) to the three float4s of cell group (i..i+3, j, k); rare planes only
-__device__ __noinline__ void add_sources4(const StepParams &P, int n, int family, float4 &vx, float4 &vy, float4 &vz, int i, int j, int k)
+// adds the sources of component `comp` to the float4 of cells (i..i+3, j, k); rare planes only
+__device__ __noinline__ float4 add_sources4(const StepParams &P, int n, int comp, float4 v, int i, int j, int k)
 {
-    float4 *v[3] = { &vx, &vy, &vz };
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        v[c]->x += source_at(P, n, 3 * family + c, i + 0, j, k);
-        v[c]->y += source_at(P, n, 3 * family + c, i + 1, j, k);
-        v[c]->z += source_at(P, n, 3 * family + c, i + 2, j, k);
-        v[c]->w += source_at(P, n, 3 * family + c, i + 3, j, k);
-    }
+    v.x += source_at(P, n, comp, i + 0, j, k);
+    v.y += source_at(P, n, comp, i + 1, j, k);
+    v.z += source_at(P, n, comp, i + 2, j, k);
+    v.w += source_at(P, n, comp, i + 3, j, k);
+    return v;
 }
 __device__ __noinline__ void detect4(const StepParams &P, int n, int family, float4 vx, float4 vy, float4 vz, int i, int j, int k)
 {
@@ -193,6 +191,16 @@ __device__ __noinline__ void detect4(const StepParams &P, int n, int family, flo
 // (filtered) difference of component c along axis a; its state array is
 //   Dy_z p[0][0]   Dz_y p[0][1]   Dz_x p[1][0]   Dx_z p[1][1]   Dx_y p[2][0]   Dy_x p[2][1].
 // ================================================================================================
+// what a thread carries from plane kk-1 to plane kk (two copies alternate, so nothing is moved)
+struct Carry {
+    float4 hx, hy, hz;          // H-type target (= raw F) at my cells
+    float4 gx, gy;              // adjoint: z-filtered F_x, F_y (forward: hx, hy)
+    float4 Yx, Yz, Xy;          // phase-B operands at my cells: forward v_x, v_z, v_y
+    float4 Xz, Zx, Zy;          // adjoint only (forward: Yz, Yx, Xy)
+};
+
+__device__ __forceinline__ void pf_l1(const float *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
 template <class C, bool ADJ>
 __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ StepParams P)
 {
@@ -222,248 +230,227 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
     // ============================================================================== producer
     if (warp == C::NCW) {
         if (lane != 0) return;
-        const CUtensorMap *M = P.maps + par * 3;
-        int ld = 0;
+        const CUtensorMap *M = P.maps + par * 6;
+        const CUtensorMap *Mie = P.maps + 12;
+        int s = 0, use = 0;
         for (int sg = seg_lo; sg < seg_hi; ++sg) {
             const Segment S = segs[sg];
             const int x = S.i0 - 4, y = S.j0 - 1;
-            for (int kk = S.k0 - 1; kk <= S.k1; ++kk, ++ld) {
-                const int s = ld % nst;
-                if (ld >= nst) mbar_wait(&empty[s], ((ld / nst) - 1) & 1);
+            for (int kk = S.k0 - 1; kk <= S.k1; ++kk) {
+                if (use > 0) mbar_wait(&empty[s], (use - 1) & 1);
                 uint64_t *fb = &full[s];
                 uint8_t *st = smem + (size_t)s * C::STAGE;
-                mbar_expect_tx(fb, 3u * C::BOX_BYTES);
-                tma_load_3d(st, M, x, y, kk, fb);
-                tma_load_3d(st + C::SLOT, M + 1, x, y, kk, fb);
-                tma_load_3d(st + 2 * C::SLOT, M + 2, x, y, kk, fb);
+                const bool prolog = kk == S.k0 - 1;
+                mbar_expect_tx(fb, (prolog ? 3u : 7u) * C::BOX_BYTES);
+                tma_load_3d(st, M + 3, x, y, kk, fb);
+                tma_load_3d(st + C::SLOT, M + 4, x, y, kk, fb);
+                tma_load_3d(st + 2 * C::SLOT, M + 5, x, y, kk, fb);
+                if (!prolog) {
+                    tma_load_3d(st + 3 * C::SLOT, M + 0, x, y, kk, fb);
+                    tma_load_3d(st + 4 * C::SLOT, M + 1, x, y, kk, fb);
+                    tma_load_3d(st + 5 * C::SLOT, M + 2, x, y, kk, fb);
+                    tma_load_3d(st + 6 * C::SLOT, Mie, x, y, kk, fb);
+                }
+                if (++s == nst) { s = 0; ++use; }
             }
         }
         return;
     }
 
     // ============================================================================== consumers
-    const int wx = warp % C::PCX, wy = warp / C::PCX;
-    const int tx = wx * 8 + (lane & 7), ty = wy * 4 + (lane >> 3);
-    const bool act = tx < C::CW && ty < C::RW;                    // thread has a float4 of cells
-    const bool inner = act && ty < C::TY && tx < C::TX4;          // not a halo thread
+    // 8 x 4 patches of float4 threads; threads beyond the tile duplicate the last column / row (they never store)
+    const int tx0 = (warp % C::PCX) * 8 + (lane & 7), ty0 = (warp / C::PCX) * 4 + (lane >> 3);
+    const bool dup = tx0 >= C::CW || ty0 >= C::RW;
+    const int tx = min(tx0, C::CW - 1), ty = min(ty0, C::RW - 1);
+    const bool inner = !dup && ty < C::TY && tx < C::TX4;         // not a halo thread
     const uint32_t o_own = ((1 + ty) * C::PW + 4 + 4 * tx) * 4;   // my first cell inside a box (bytes)
     const uint32_t r_own = (ty * C::RP + 4 * tx) * 4;             // ... inside a ring array
-    const float *src = P.buf[par];
     float *dst = P.buf[par ^ 1];
     const PsiSet &qAi = ADJ ? P.psiH[par] : P.psiE[par], &qAo = ADJ ? P.psiH[par ^ 1] : P.psiE[par ^ 1];
     const PsiSet &qBi = ADJ ? P.psiE[par] : P.psiH[par], &qBo = ADJ ? P.psiE[par ^ 1] : P.psiH[par ^ 1];
     const float S = G.S;
     const long long nc = G.nc;
-    const long long plane = (long long)G.ny * G.nx;
+    const int plane = G.ny * G.nx;
     const bool pml = G.d > 0;
     const bool has_mu = !ADJ && P.im != nullptr;
+    const int pz = plane, py = 2 * G.d * G.nx, px = G.ny * 2 * G.dpx;      // plane pitch of the z / y / x state arrays
 
-    // k ranges of the planes that hold sources / detectors (forward only)
-    int sEl = 1 << 30, sEh = -1, sHl = 1 << 30, sHh = -1, dEl = 1 << 30, dEh = -1, dHl = 1 << 30, dHh = -1;
-    if (!ADJ) {
-        for (int s = 0; s < P.n_src; ++s) {
-            if (P.src[s].comp < 3) { sEl = min(sEl, P.src[s].lo[2]); sEh = max(sEh, P.src[s].hi[2]); }
-            else { sHl = min(sHl, P.src[s].lo[2]); sHh = max(sHh, P.src[s].hi[2]); }
-        }
-        for (int s = 0; s < P.n_det; ++s) {
-            if (P.det[s].mask & 7) { dEl = min(dEl, P.det[s].lo[2]); dEh = max(dEh, P.det[s].hi[2]); }
-            if (P.det[s].mask >> 3) { dHl = min(dHl, P.det[s].lo[2]); dHh = max(dHh, P.det[s].hi[2]); }
-        }
-    }
     const float4 Z4 = splat(0.f);
 
-    int ld = 0;
+    int st_i = 0;                 // pipeline stage of the next plane
+    uint32_t st_ph = 0;           // its full-barrier parity
+    uint32_t st_off = 0;          // st_i * STAGE
     for (int sg = seg_lo; sg < seg_hi; ++sg) {
         const Segment Sg = segs[sg];
         const int i = Sg.i0 + 4 * tx, j = Sg.j0 + ty;
-        const bool ing = act && i < G.nx && j < G.ny;              // my cells are inside the grid
+        const bool ing = i < G.nx && j < G.ny;                      // my cells are inside the grid
         const bool own_ok = inner && ing;
-        const long long own_xy = (long long)j * G.nx + i;
+        const int own_xy = j * G.nx + i;
         // slab-compact coordinates of my cells and (adjoint) of my -x / -y neighbours; -1: not in a slab
         const int sx = (pml && ing) ? slab_pos(i, G.nx, G.dpx) : -1;
         const int sy = (pml && ing) ? slab_pos(j, G.ny, G.d) : -1;
         const int sxm = (ADJ && pml && ing) ? slab_pos(i - 1, G.nx, G.dpx) : -1;
         const int sym = (ADJ && pml && ing) ? slab_pos(j - 1, G.ny, G.d) : -1;
-        const long long oy = (long long)sy * G.nx + i, oym = (long long)sym * G.nx + i;   // + k * 2d * nx
-        const long long ox = (long long)j * (2 * G.dpx) + sx, oxm = (long long)j * (2 * G.dpx) + sxm;   // + k * ny * 2dpx
-        const long long py = (long long)2 * G.d * G.nx, px = (long long)G.ny * 2 * G.dpx;
+        const bool slab_xy = __any_sync(0xffffffffu, (sx & sy & sxm & sym) >= 0);   // this warp runs x / y slab code
+        const int oy = sy * G.nx + i, oym = sym * G.nx + i;                          // + k * py
+        const int ox = j * (2 * G.dpx) + sx, oxm = j * (2 * G.dpx) + sxm;           // + k * px
+        const int k1 = Sg.k1;
 
-        float4 hxk = Z4, hyk = Z4, hzk = Z4;                // H-type target of plane kk-1 at my cells (raw)
-        float4 fxk = Z4, fyk = Z4;                          // z operands of phase A from plane kk-1 (adjoint: filtered)
-        float4 cYx = Z4, cYz = Z4, cXy = Z4, cXz = Z4, cZx = Z4, cZy = Z4;   // phase-B operands of plane kk-1 at my cells
-        float4 ex = Z4, ey = Z4, ez = Z4, ie4 = Z4;         // E-type target and inv_eps of the plane about to be updated
-
-        for (int kk = Sg.k0 - 1; kk <= Sg.k1; ++kk, ++ld) {
-            const bool prolog = kk == Sg.k0 - 1;
-            const bool doB = kk >= Sg.k0 + 1;
-            const int s = ld % nst;
+        // ---------------------------------------------------------------- one plane (phase A of kk, phase B of kk-1)
+        auto plane_step = [&](const int kk, const Carry &in, Carry &out, const bool doB) {
             const int zs = pml ? slab_pos(kk, G.nz, G.d) : -1;
-            mbar_wait(&full[s], (ld / nst) & 1);
-            const uint32_t so = stage_base + (uint32_t)s * C::STAGE + o_own;
-            const long long off = (long long)kk * plane + own_xy;
-            const long long oz = ((long long)zs * G.ny + j) * G.nx + i;
+            mbar_wait(&full[st_i], st_ph);
+            const uint32_t so = stage_base + st_off + o_own;
+            const float4 fx = lds4(so), fy = lds4(so + C::SLOT), fz = lds4(so + 2 * C::SLOT);
+            const float4 fx_my = lds4(so - C::ROWB), fz_my = lds4(so + 2 * C::SLOT - C::ROWB);
+            const float fy_mx = lds1(so + C::SLOT - 4), fz_mx = lds1(so + 2 * C::SLOT - 4);
 
-            float4 fx = Z4, fy = Z4, fz = Z4, fx_my = Z4, fz_my = Z4;
-            float fy_mx = 0.f, fz_mx = 0.f;
-            if (act) {
-                fx = lds4(so); fy = lds4(so + C::SLOT); fz = lds4(so + 2 * C::SLOT);
-                if (!prolog) {
-                    fx_my = lds4(so - C::ROWB); fz_my = lds4(so + 2 * C::SLOT - C::ROWB);
-                    fy_mx = lds1(so + C::SLOT - 4); fz_mx = lds1(so + 2 * C::SLOT - 4);
-                }
-            }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[s]);
-
-            // the E-type target and inv_eps of the next plane
-            float4 nex = Z4, ney = Z4, nez = Z4, nie = Z4;
-            if (ing && kk + 1 <= Sg.k1 && kk + 1 < G.nz) {
-                const float *q = src + off + plane;
-                nex = ldg4(q); ney = ldg4(q + nc); nez = ldg4(q + 2 * nc);
-                nie = ldg4(P.ie + off + plane);
-            }
-
-            if (prolog) {
-                fxk = fx; fyk = fy;
-                if (ADJ && zs >= 0 && ing) {
-                    const float b = __ldg(P.T.b[FA][2] + kk), a = __ldg(P.T.a[FA][2] + kk), km = __ldg(P.T.ik[FA][2] + kk) - 1.f;
-                    float4 pn;
-                    fxk = fx + cpml4(b, a, km, ldg4(qAi.p[1][0] + oz), fx, pn);
-                    fyk = fy + cpml4(b, a, km, ldg4(qAi.p[0][1] + oz), fy, pn);
-                }
-                ex = nex; ey = ney; ez = nez; ie4 = nie;
-                continue;
-            }
-
-            const bool storeE = kk < Sg.k1;
-            const bool wr = own_ok && storeE;                  // I own these cells: write the result and the phase-A states
+            const bool wr = own_ok && kk < k1;                 // I own these cells: write the result and the phase-A states
+            const int off = kk * plane + own_xy;
+            const int oz = zs * pz + own_xy;
             const uint32_t rgA = ring_base + (uint32_t)(kk & 1) * (C::RING_SLOT * 4) + r_own;
-            float4 gx = fx, gy = fy;                           // z operands of phase A at plane kk (adjoint: filtered)
-            float4 Yx = Z4, Yz = Z4, Xy = Z4, Xz = Z4, Zx = Z4, Zy = Z4;   // phase-B operands of plane kk at my cells
-            if (act) {
-                // ------------------------------------------------------------ phase A: E-type update of plane kk
-                float4 Dy_z = fz - fz_my, Dy_x = fx - fx_my;
-                float4 Dx_y = dminus_x(fy, fy_mx), Dx_z = dminus_x(fz, fz_mx);
-                float4 Dz_x, Dz_y;
-                if (!ADJ) {
-                    Dz_x = fx - fxk; Dz_y = fy - fyk;
-                    if (pml) {
-                        if (zs >= 0 && ing) {
-                            const float b = __ldg(P.T.b[FA][2] + kk), a = __ldg(P.T.a[FA][2] + kk), km = __ldg(P.T.ik[FA][2] + kk) - 1.f;
-                            float4 p0, p1;
-                            Dz_x = Dz_x + cpml4(b, a, km, ldg4(qAi.p[1][0] + oz), Dz_x, p0);
-                            Dz_y = Dz_y + cpml4(b, a, km, ldg4(qAi.p[0][1] + oz), Dz_y, p1);
-                            if (wr) { stg4(qAo.p[1][0] + oz, p0); stg4(qAo.p[0][1] + oz, p1); }
-                        }
-                        if (sy >= 0) {
-                            const float b = __ldg(P.T.b[FA][1] + j), a = __ldg(P.T.a[FA][1] + j), km = __ldg(P.T.ik[FA][1] + j) - 1.f;
-                            const long long q = kk * py + oy;
-                            float4 p0, p1;
-                            Dy_z = Dy_z + cpml4(b, a, km, ldg4(qAi.p[0][0] + q), Dy_z, p0);
-                            Dy_x = Dy_x + cpml4(b, a, km, ldg4(qAi.p[2][1] + q), Dy_x, p1);
-                            if (wr) { stg4(qAo.p[0][0] + q, p0); stg4(qAo.p[2][1] + q, p1); }
-                        }
-                        if (sx >= 0) {
-                            const float4 b = ldg4(P.T.b[FA][0] + i), a = ldg4(P.T.a[FA][0] + i), km = ldg4(P.T.ik[FA][0] + i) - splat(1.f);
-                            const long long q = kk * px + ox;
-                            float4 p0, p1;
-                            Dx_y = Dx_y + cpml4(b, a, km, ldg4(qAi.p[2][0] + q), Dx_y, p0);
-                            Dx_z = Dx_z + cpml4(b, a, km, ldg4(qAi.p[1][1] + q), Dx_z, p1);
-                            if (wr) { stg4(qAo.p[2][0] + q, p0); stg4(qAo.p[1][1] + q, p1); }
-                        }
-                    }
-                } else {
-                    if (pml) {
-                        if (zs >= 0 && ing) {
-                            const float b = __ldg(P.T.b[FA][2] + kk), a = __ldg(P.T.a[FA][2] + kk), km = __ldg(P.T.ik[FA][2] + kk) - 1.f;
-                            float4 p0, p1;
-                            gx = fx + cpml4(b, a, km, ldg4(qAi.p[1][0] + oz), fx, p0);
-                            gy = fy + cpml4(b, a, km, ldg4(qAi.p[0][1] + oz), fy, p1);
-                            if (wr) { stg4(qAo.p[1][0] + oz, p0); stg4(qAo.p[0][1] + oz, p1); }
-                        }
-                        if (sy >= 0) {
-                            const float b = __ldg(P.T.b[FA][1] + j), a = __ldg(P.T.a[FA][1] + j), km = __ldg(P.T.ik[FA][1] + j) - 1.f;
-                            const long long q = kk * py + oy;
-                            float4 p0, p1;
-                            Dy_z = Dy_z + cpml4(b, a, km, ldg4(qAi.p[0][0] + q), fz, p0);
-                            Dy_x = Dy_x + cpml4(b, a, km, ldg4(qAi.p[2][1] + q), fx, p1);
-                            if (wr) { stg4(qAo.p[0][0] + q, p0); stg4(qAo.p[2][1] + q, p1); }
-                        }
-                        if (sym >= 0) {
-                            const float b = __ldg(P.T.b[FA][1] + j - 1), a = __ldg(P.T.a[FA][1] + j - 1), km = __ldg(P.T.ik[FA][1] + j - 1) - 1.f;
-                            const long long q = kk * py + oym;
-                            float4 p0, p1;
-                            Dy_z = Dy_z - cpml4(b, a, km, ldg4(qAi.p[0][0] + q), fz_my, p0);
-                            Dy_x = Dy_x - cpml4(b, a, km, ldg4(qAi.p[2][1] + q), fx_my, p1);
-                        }
-                        if (sx >= 0 || sxm >= 0) {
-                            float4 cy = Z4, cz = Z4;
-                            float ly = 0.f, lz = 0.f;
-                            if (sx >= 0) {
-                                const float4 b = ldg4(P.T.b[FA][0] + i), a = ldg4(P.T.a[FA][0] + i), km = ldg4(P.T.ik[FA][0] + i) - splat(1.f);
-                                const long long q = kk * px + ox;
-                                float4 p0, p1;
-                                cy = cpml4(b, a, km, ldg4(qAi.p[2][0] + q), fy, p0);
-                                cz = cpml4(b, a, km, ldg4(qAi.p[1][1] + q), fz, p1);
-                                if (wr) { stg4(qAo.p[2][0] + q, p0); stg4(qAo.p[1][1] + q, p1); }
-                            }
-                            if (sxm >= 0) {
-                                const float b = __ldg(P.T.b[FA][0] + i - 1), a = __ldg(P.T.a[FA][0] + i - 1), km = __ldg(P.T.ik[FA][0] + i - 1) - 1.f;
-                                const long long q = kk * px + oxm;
-                                ly = cpml1(b, a, km, __ldg(qAi.p[2][0] + q), fy_mx);
-                                lz = cpml1(b, a, km, __ldg(qAi.p[1][1] + q), fz_mx);
-                            }
-                            Dx_y = Dx_y + dminus_x(cy, ly);
-                            Dx_z = Dx_z + dminus_x(cz, lz);
-                        }
-                    }
-                    Dz_x = gx - fxk; Dz_y = gy - fyk;
-                }
-                const float4 tEx = Dy_z - Dz_y, tEy = Dz_x - Dx_z, tEz = Dx_y - Dy_x;
-                const float4 sie = S * ie4;
-                float4 e2x, e2y, e2z, v2x, v2y, v2z;
-                if (ADJ) {
-                    e2x = fma4(-S, tEx, ex); e2y = fma4(-S, tEy, ey); e2z = fma4(-S, tEz, ez);
-                    v2x = sie * e2x; v2y = sie * e2y; v2z = sie * e2z;
-                } else {
-                    e2x = fma4(sie, tEx, ex); e2y = fma4(sie, tEy, ey); e2z = fma4(sie, tEz, ez);
-                    if (kk >= sEl && kk < sEh) add_sources4(P, n, 0, e2x, e2y, e2z, i, j, kk);
-                    v2x = e2x; v2y = e2y; v2z = e2z;
-                }
-                if (wr) {
-                    float *o = dst + off;
-                    stg4(o, e2x); stg4(o + nc, e2y); stg4(o + 2 * nc, e2z);
-                    if (!ADJ && kk >= dEl && kk < dEh) detect4(P, n, 0, e2x, e2y, e2z, i, j, kk);
-                }
-                Yx = v2x; Yz = v2z; Xy = v2y; Xz = v2z; Zx = v2x; Zy = v2y;
-                if (ADJ && pml) {       // phase-B operands are filtered where they are produced
+            // ------------------------------------------------------------ phase A: E-type update of plane kk
+            float4 Dy_z = fz - fz_my, Dy_x = fx - fx_my;
+            float4 Dx_y = dminus_x(fy, fy_mx), Dx_z = dminus_x(fz, fz_mx);
+            float4 Dz_x, Dz_y;
+            out.hx = fx; out.hy = fy; out.hz = fz;
+            if (!ADJ) {
+                Dz_x = fx - in.hx; Dz_y = fy - in.hy;
+                if (slab_xy || zs >= 0) {
                     if (zs >= 0 && ing) {
-                        const float b = __ldg(P.T.b[FB][2] + kk), a = __ldg(P.T.a[FB][2] + kk), km = __ldg(P.T.ik[FB][2] + kk) - 1.f;
+                        const float b = __ldg(P.T.b[FA][2] + kk), a = __ldg(P.T.a[FA][2] + kk), km = __ldg(P.T.ik[FA][2] + kk) - 1.f;
                         float4 p0, p1;
-                        Zx = v2x + cpml4(b, a, km, ldg4(qBi.p[1][0] + oz), v2x, p0);
-                        Zy = v2y + cpml4(b, a, km, ldg4(qBi.p[0][1] + oz), v2y, p1);
-                        if (wr) { stg4(qBo.p[1][0] + oz, p0); stg4(qBo.p[0][1] + oz, p1); }
+                        Dz_x = Dz_x + cpml4(b, a, km, ldg4(qAi.p[1][0] + oz), Dz_x, p0);
+                        Dz_y = Dz_y + cpml4(b, a, km, ldg4(qAi.p[0][1] + oz), Dz_y, p1);
+                        if (wr) { stg4(qAo.p[1][0] + oz, p0); stg4(qAo.p[0][1] + oz, p1); }
                     }
                     if (sy >= 0) {
-                        const float b = __ldg(P.T.b[FB][1] + j), a = __ldg(P.T.a[FB][1] + j), km = __ldg(P.T.ik[FB][1] + j) - 1.f;
-                        const long long q = kk * py + oy;
+                        const float b = __ldg(P.T.b[FA][1] + j), a = __ldg(P.T.a[FA][1] + j), km = __ldg(P.T.ik[FA][1] + j) - 1.f;
+                        const int q = kk * py + oy;
                         float4 p0, p1;
-                        Yz = v2z + cpml4(b, a, km, ldg4(qBi.p[0][0] + q), v2z, p0);
-                        Yx = v2x + cpml4(b, a, km, ldg4(qBi.p[2][1] + q), v2x, p1);
-                        if (wr) { stg4(qBo.p[0][0] + q, p0); stg4(qBo.p[2][1] + q, p1); }
+                        Dy_z = Dy_z + cpml4(b, a, km, ldg4(qAi.p[0][0] + q), Dy_z, p0);
+                        Dy_x = Dy_x + cpml4(b, a, km, ldg4(qAi.p[2][1] + q), Dy_x, p1);
+                        pf_l1(qAi.p[0][0] + q + py); pf_l1(qAi.p[2][1] + q + py);
+                        if (wr) { stg4(qAo.p[0][0] + q, p0); stg4(qAo.p[2][1] + q, p1); }
                     }
                     if (sx >= 0) {
-                        const float4 b = ldg4(P.T.b[FB][0] + i), a = ldg4(P.T.a[FB][0] + i), km = ldg4(P.T.ik[FB][0] + i) - splat(1.f);
-                        const long long q = kk * px + ox;
+                        const float4 b = ldg4(P.T.b[FA][0] + i), a = ldg4(P.T.a[FA][0] + i), km = ldg4(P.T.ik[FA][0] + i) - splat(1.f);
+                        const int q = kk * px + ox;
                         float4 p0, p1;
-                        Xy = v2y + cpml4(b, a, km, ldg4(qBi.p[2][0] + q), v2y, p0);
-                        Xz = v2z + cpml4(b, a, km, ldg4(qBi.p[1][1] + q), v2z, p1);
-                        if (wr) { stg4(qBo.p[2][0] + q, p0); stg4(qBo.p[1][1] + q, p1); }
+                        Dx_y = Dx_y + cpml4(b, a, km, ldg4(qAi.p[2][0] + q), Dx_y, p0);
+                        Dx_z = Dx_z + cpml4(b, a, km, ldg4(qAi.p[1][1] + q), Dx_z, p1);
+                        pf_l1(qAi.p[2][0] + q + px); pf_l1(qAi.p[1][1] + q + px);
+                        if (wr) { stg4(qAo.p[2][0] + q, p0); stg4(qAo.p[1][1] + q, p1); }
                     }
                 }
-                sts4(rgA, Yx); sts4(rgA + C::RING_ARR * 4, Yz); sts4(rgA + 2 * C::RING_ARR * 4, Xy);
-                if (ADJ) sts4(rgA + 3 * C::RING_ARR * 4, Xz);
+            } else {
+                float4 gx = fx, gy = fy;                       // z operands at plane kk, filtered
+                if (slab_xy || zs >= 0) {
+                    if (zs >= 0 && ing) {
+                        const float b = __ldg(P.T.b[FA][2] + kk), a = __ldg(P.T.a[FA][2] + kk), km = __ldg(P.T.ik[FA][2] + kk) - 1.f;
+                        float4 p0, p1;
+                        gx = fx + cpml4(b, a, km, ldg4(qAi.p[1][0] + oz), fx, p0);
+                        gy = fy + cpml4(b, a, km, ldg4(qAi.p[0][1] + oz), fy, p1);
+                        if (wr) { stg4(qAo.p[1][0] + oz, p0); stg4(qAo.p[0][1] + oz, p1); }
+                    }
+                    if (sy >= 0) {
+                        const float b = __ldg(P.T.b[FA][1] + j), a = __ldg(P.T.a[FA][1] + j), km = __ldg(P.T.ik[FA][1] + j) - 1.f;
+                        const int q = kk * py + oy;
+                        float4 p0, p1;
+                        Dy_z = Dy_z + cpml4(b, a, km, ldg4(qAi.p[0][0] + q), fz, p0);
+                        Dy_x = Dy_x + cpml4(b, a, km, ldg4(qAi.p[2][1] + q), fx, p1);
+                        pf_l1(qAi.p[0][0] + q + py); pf_l1(qAi.p[2][1] + q + py);
+                        if (wr) { stg4(qAo.p[0][0] + q, p0); stg4(qAo.p[2][1] + q, p1); }
+                    }
+                    if (sym >= 0) {
+                        const float b = __ldg(P.T.b[FA][1] + j - 1), a = __ldg(P.T.a[FA][1] + j - 1), km = __ldg(P.T.ik[FA][1] + j - 1) - 1.f;
+                        const int q = kk * py + oym;
+                        float4 p0, p1;
+                        Dy_z = Dy_z - cpml4(b, a, km, ldg4(qAi.p[0][0] + q), fz_my, p0);
+                        Dy_x = Dy_x - cpml4(b, a, km, ldg4(qAi.p[2][1] + q), fx_my, p1);
+                        if (sy < 0) { pf_l1(qAi.p[0][0] + q + py); pf_l1(qAi.p[2][1] + q + py); }
+                    }
+                    if (sx >= 0 || sxm >= 0) {
+                        float4 cy = Z4, cz = Z4;
+                        float ly = 0.f, lz = 0.f;
+                        if (sx >= 0) {
+                            const float4 b = ldg4(P.T.b[FA][0] + i), a = ldg4(P.T.a[FA][0] + i), km = ldg4(P.T.ik[FA][0] + i) - splat(1.f);
+                            const int q = kk * px + ox;
+                            float4 p0, p1;
+                            cy = cpml4(b, a, km, ldg4(qAi.p[2][0] + q), fy, p0);
+                            cz = cpml4(b, a, km, ldg4(qAi.p[1][1] + q), fz, p1);
+                            pf_l1(qAi.p[2][0] + q + px); pf_l1(qAi.p[1][1] + q + px);
+                            if (wr) { stg4(qAo.p[2][0] + q, p0); stg4(qAo.p[1][1] + q, p1); }
+                        }
+                        if (sxm >= 0) {
+                            const float b = __ldg(P.T.b[FA][0] + i - 1), a = __ldg(P.T.a[FA][0] + i - 1), km = __ldg(P.T.ik[FA][0] + i - 1) - 1.f;
+                            const int q = kk * px + oxm;
+                            ly = cpml1(b, a, km, __ldg(qAi.p[2][0] + q), fy_mx);
+                            lz = cpml1(b, a, km, __ldg(qAi.p[1][1] + q), fz_mx);
+                            if (sx < 0) { pf_l1(qAi.p[2][0] + q + px); pf_l1(qAi.p[1][1] + q + px); }
+                        }
+                        Dx_y = Dx_y + dminus_x(cy, ly);
+                        Dx_z = Dx_z + dminus_x(cz, lz);
+                    }
+                }
+                Dz_x = gx - in.gx; Dz_y = gy - in.gy;
+                out.gx = gx; out.gy = gy;
             }
+            const float4 tEx = Dy_z - Dz_y, tEy = Dz_x - Dx_z, tEz = Dx_y - Dy_x;
+            const float4 ex = lds4(so + 3 * C::SLOT), ey = lds4(so + 4 * C::SLOT), ez = lds4(so + 5 * C::SLOT);
+            const float4 sie = S * lds4(so + 6 * C::SLOT);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[st_i]);
+            st_off += C::STAGE;
+            if (++st_i == nst) { st_i = 0; st_off = 0; st_ph ^= 1; }
+            float4 e2x, e2y, e2z, v2x, v2y, v2z;
+            if (ADJ) {
+                e2x = fma4(-S, tEx, ex); e2y = fma4(-S, tEy, ey); e2z = fma4(-S, tEz, ez);
+                v2x = sie * e2x; v2y = sie * e2y; v2z = sie * e2z;
+            } else {
+                e2x = fma4(sie, tEx, ex); e2y = fma4(sie, tEy, ey); e2z = fma4(sie, tEz, ez);
+                if (kk >= P.sEl && kk < P.sEh) {
+                    e2x = add_sources4(P, n, 0, e2x, i, j, kk); e2y = add_sources4(P, n, 1, e2y, i, j, kk); e2z = add_sources4(P, n, 2, e2z, i, j, kk);
+                }
+                v2x = e2x; v2y = e2y; v2z = e2z;
+            }
+            if (wr) {
+                float *o = dst + off;
+                stg4(o, e2x); stg4(o + nc, e2y); stg4(o + 2 * nc, e2z);
+                if (!ADJ && kk >= P.dEl && kk < P.dEh) detect4(P, n, 0, e2x, e2y, e2z, i, j, kk);
+            }
+            float4 Yx = v2x, Yz = v2z, Xy = v2y, Xz = v2z, Zx = v2x, Zy = v2y;
+            if (ADJ && (slab_xy || zs >= 0)) {       // phase-B operands are filtered where they are produced
+                if (zs >= 0 && ing) {
+                    const float b = __ldg(P.T.b[FB][2] + kk), a = __ldg(P.T.a[FB][2] + kk), km = __ldg(P.T.ik[FB][2] + kk) - 1.f;
+                    float4 p0, p1;
+                    Zx = v2x + cpml4(b, a, km, ldg4(qBi.p[1][0] + oz), v2x, p0);
+                    Zy = v2y + cpml4(b, a, km, ldg4(qBi.p[0][1] + oz), v2y, p1);
+                    if (wr) { stg4(qBo.p[1][0] + oz, p0); stg4(qBo.p[0][1] + oz, p1); }
+                }
+                if (sy >= 0) {
+                    const float b = __ldg(P.T.b[FB][1] + j), a = __ldg(P.T.a[FB][1] + j), km = __ldg(P.T.ik[FB][1] + j) - 1.f;
+                    const int q = kk * py + oy;
+                    float4 p0, p1;
+                    Yz = v2z + cpml4(b, a, km, ldg4(qBi.p[0][0] + q), v2z, p0);
+                    Yx = v2x + cpml4(b, a, km, ldg4(qBi.p[2][1] + q), v2x, p1);
+                    pf_l1(qBi.p[0][0] + q + py); pf_l1(qBi.p[2][1] + q + py);
+                    if (wr) { stg4(qBo.p[0][0] + q, p0); stg4(qBo.p[2][1] + q, p1); }
+                }
+                if (sx >= 0) {
+                    const float4 b = ldg4(P.T.b[FB][0] + i), a = ldg4(P.T.a[FB][0] + i), km = ldg4(P.T.ik[FB][0] + i) - splat(1.f);
+                    const int q = kk * px + ox;
+                    float4 p0, p1;
+                    Xy = v2y + cpml4(b, a, km, ldg4(qBi.p[2][0] + q), v2y, p0);
+                    Xz = v2z + cpml4(b, a, km, ldg4(qBi.p[1][1] + q), v2z, p1);
+                    pf_l1(qBi.p[2][0] + q + px); pf_l1(qBi.p[1][1] + q + px);
+                    if (wr) { stg4(qBo.p[2][0] + q, p0); stg4(qBo.p[1][1] + q, p1); }
+                }
+            }
+            sts4(rgA, Yx); sts4(rgA + C::RING_ARR * 4, Yz); sts4(rgA + 2 * C::RING_ARR * 4, Xy);
+            if (ADJ) sts4(rgA + 3 * C::RING_ARR * 4, Xz);
+            out.Yx = Yx; out.Yz = Yz; out.Xy = Xy;
+            if (ADJ) { out.Xz = Xz; out.Zx = Zx; out.Zy = Zy; }
             // ---------------------------------------------------------------- phase B: H-type update of plane kk-1
             if (own_ok && doB) {
                 const int km1 = kk - 1;
@@ -471,15 +458,15 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                 const float4 Yx_py = lds4(rgB + C::RP * 4), Yz_py = lds4(rgB + (C::RING_ARR + C::RP) * 4);
                 const float Xy_px = lds1(rgB + (2 * C::RING_ARR + 4) * 4);
                 const float Xz_px = lds1(rgB + ((ADJ ? 3 : 1) * C::RING_ARR + 4) * 4);
-                float4 Dy_z = Yz_py - cYz, Dy_x = Yx_py - cYx;
-                float4 Dz_y = Zy - cZy, Dz_x = Zx - cZx;
-                float4 Dx_z = dplus_x(cXz, Xz_px), Dx_y = dplus_x(cXy, Xy_px);
-                const long long offm = off - plane;
-                if (!ADJ && pml) {
-                    const int zsm = slab_pos(km1, G.nz, G.d);
+                float4 Dy_z = Yz_py - in.Yz, Dy_x = Yx_py - in.Yx;
+                float4 Dz_y = Zy - (ADJ ? in.Zy : in.Xy), Dz_x = Zx - (ADJ ? in.Zx : in.Yx);
+                float4 Dx_z = dplus_x(ADJ ? in.Xz : in.Yz, Xz_px), Dx_y = dplus_x(in.Xy, Xy_px);
+                const int offm = off - plane;
+                const int zsm = (!ADJ && pml) ? slab_pos(km1, G.nz, G.d) : -1;
+                if (!ADJ && (slab_xy || zsm >= 0)) {
                     if (zsm >= 0) {
                         const float b = __ldg(P.T.b[FB][2] + km1), a = __ldg(P.T.a[FB][2] + km1), km = __ldg(P.T.ik[FB][2] + km1) - 1.f;
-                        const long long q = ((long long)zsm * G.ny + j) * G.nx + i;
+                        const int q = zsm * pz + own_xy;
                         float4 p0, p1;
                         Dz_x = Dz_x + cpml4(b, a, km, ldg4(qBi.p[1][0] + q), Dz_x, p0);
                         Dz_y = Dz_y + cpml4(b, a, km, ldg4(qBi.p[0][1] + q), Dz_y, p1);
@@ -487,40 +474,72 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                     }
                     if (sy >= 0) {
                         const float b = __ldg(P.T.b[FB][1] + j), a = __ldg(P.T.a[FB][1] + j), km = __ldg(P.T.ik[FB][1] + j) - 1.f;
-                        const long long q = km1 * py + oy;
+                        const int q = km1 * py + oy;
                         float4 p0, p1;
                         Dy_z = Dy_z + cpml4(b, a, km, ldg4(qBi.p[0][0] + q), Dy_z, p0);
                         Dy_x = Dy_x + cpml4(b, a, km, ldg4(qBi.p[2][1] + q), Dy_x, p1);
+                        pf_l1(qBi.p[0][0] + q + py); pf_l1(qBi.p[2][1] + q + py);
                         stg4(qBo.p[0][0] + q, p0); stg4(qBo.p[2][1] + q, p1);
                     }
                     if (sx >= 0) {
                         const float4 b = ldg4(P.T.b[FB][0] + i), a = ldg4(P.T.a[FB][0] + i), km = ldg4(P.T.ik[FB][0] + i) - splat(1.f);
-                        const long long q = km1 * px + ox;
+                        const int q = km1 * px + ox;
                         float4 p0, p1;
                         Dx_y = Dx_y + cpml4(b, a, km, ldg4(qBi.p[2][0] + q), Dx_y, p0);
                         Dx_z = Dx_z + cpml4(b, a, km, ldg4(qBi.p[1][1] + q), Dx_z, p1);
+                        pf_l1(qBi.p[2][0] + q + px); pf_l1(qBi.p[1][1] + q + px);
                         stg4(qBo.p[2][0] + q, p0); stg4(qBo.p[1][1] + q, p1);
                     }
                 }
                 const float4 tHx = Dy_z - Dz_y, tHy = Dz_x - Dx_z, tHz = Dx_y - Dy_x;
                 float4 h2x, h2y, h2z;
                 if (ADJ) {
-                    h2x = hxk + tHx; h2y = hyk + tHy; h2z = hzk + tHz;
+                    h2x = in.hx + tHx; h2y = in.hy + tHy; h2z = in.hz + tHz;
                 } else {
                     const float4 sim = has_mu ? S * ldg4(P.im + offm) : splat(S);
-                    h2x = hxk - sim * tHx; h2y = hyk - sim * tHy; h2z = hzk - sim * tHz;
-                    if (km1 >= sHl && km1 < sHh) add_sources4(P, n, 1, h2x, h2y, h2z, i, j, km1);
+                    h2x = in.hx - sim * tHx; h2y = in.hy - sim * tHy; h2z = in.hz - sim * tHz;
+                    if (km1 >= P.sHl && km1 < P.sHh) {
+                        h2x = add_sources4(P, n, 3, h2x, i, j, km1); h2y = add_sources4(P, n, 4, h2y, i, j, km1); h2z = add_sources4(P, n, 5, h2z, i, j, km1);
+                    }
                 }
                 float *o = dst + 3 * nc + offm;
                 stg4(o, h2x); stg4(o + nc, h2y); stg4(o + 2 * nc, h2z);
-                if (!ADJ && km1 >= dHl && km1 < dHh) detect4(P, n, 1, h2x, h2y, h2z, i, j, km1);
+                if (!ADJ && km1 >= P.dHl && km1 < P.dHh) detect4(P, n, 1, h2x, h2y, h2z, i, j, km1);
             }
-            cYx = Yx; cYz = Yz; cXy = Xy; cXz = Xz; cZx = Zx; cZy = Zy;
-            hxk = fx; hyk = fy; hzk = fz;
-            fxk = gx; fyk = gy;
-            ex = nex; ey = ney; ez = nez; ie4 = nie;
             named_bar_sync(1, C::NCW * 32);      // ring slot (kk-1)&1 may be overwritten in the next iteration
+        };
+
+        // ---------------------------------------------------------------- prologue: the z operands of plane k0-1
+        Carry A, B;
+        {
+            const int kk = Sg.k0 - 1;
+            mbar_wait(&full[st_i], st_ph);
+            const uint32_t so = stage_base + st_off + o_own;
+            A.hx = lds4(so); A.hy = lds4(so + C::SLOT); A.hz = Z4;
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[st_i]);
+            st_off += C::STAGE;
+            if (++st_i == nst) { st_i = 0; st_off = 0; st_ph ^= 1; }
+            A.gx = A.hx; A.gy = A.hy;
+            if (ADJ && pml) {
+                const int zs = slab_pos(kk, G.nz, G.d);
+                if (zs >= 0 && ing) {
+                    const float b = __ldg(P.T.b[FA][2] + kk), a = __ldg(P.T.a[FA][2] + kk), km = __ldg(P.T.ik[FA][2] + kk) - 1.f;
+                    const int oz = zs * pz + own_xy;
+                    float4 pn;
+                    A.gx = A.hx + cpml4(b, a, km, ldg4(qAi.p[1][0] + oz), A.hx, pn);
+                    A.gy = A.hy + cpml4(b, a, km, ldg4(qAi.p[0][1] + oz), A.hy, pn);
+                }
+            }
+            A.Yx = A.Yz = A.Xy = A.Xz = A.Zx = A.Zy = Z4;
         }
+        plane_step(Sg.k0, A, B, false);
+        int kk = Sg.k0 + 1;
+        for (; kk + 1 <= k1; kk += 2) {
+            plane_step(kk, B, A, true);
+            plane_step(kk + 1, A, B, true);
+        }
+        if (kk <= k1) plane_step(kk, B, A, true);
     }
 }
 
@@ -597,13 +616,13 @@ struct FusedState {
     StepParams sp{};
     float *bufB = nullptr;                 // second primal field buffer
     float *lamB = nullptr;                 // second cotangent buffer
-    // tensor-map tables: [0] primal (fields / bufB), [1] cotangents (lam / lamB); entry set*3 + c
+    // tensor-map tables: [0] primal (fields / bufB), [1] cotangents (lam / lamB); entry set*6 + c, [12] = inv_eps
     CUtensorMap *d_maps[2] = { nullptr, nullptr };
     CUtensorMap *h_maps[2] = { nullptr, nullptr };   // pinned staging
     cudaEvent_t maps_done = nullptr;
     Segment *d_segs = nullptr;
     int *d_seg_begin = nullptr;
-    const float *maps_key[2] = { nullptr, nullptr };   // volume A the maps were built for
+    const float *maps_key[2][2] = { { nullptr, nullptr }, { nullptr, nullptr } };   // volume A / inv_eps the maps were built for
 };
 
 namespace {
@@ -654,6 +673,7 @@ int fused_setup(fdtd_grid *g)
     if (G.periodic) { g->fused_why_not = "periodic grids use the generic kernels"; return FDTD_OK; }
     if (G.nx % 4) { g->fused_why_not = "nx is not a multiple of 4"; return FDTD_OK; }
     if (G.d > 0 && (G.dpx % 4)) { g->fused_why_not = "x-slab psi storage is not float4 aligned (nx < 2*roundup4(d))"; return FDTD_OK; }
+    if (G.nc >= (1LL << 31) - 4LL * G.nx * G.ny) { g->fused_why_not = "more than 2^31 cells (32-bit plane offsets)"; return FDTD_OK; }
     if (!get_encode()) { g->fused_why_not = "cuTensorMapEncodeTiled is not available"; return FDTD_OK; }
     int dev = 0, smem_cap = 0, n_sm = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&smem_cap, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess ||
@@ -693,8 +713,8 @@ int fused_setup(fdtd_grid *g)
     if ((rc = g->alloc((void **)&F->bufB, (size_t)G.nc * 6 * sizeof(float)))) return rc;
     if ((rc = g->alloc_psi(g->psiE[1])) || (rc = g->alloc_psi(g->psiH[1]))) return rc;
     for (int q = 0; q < 2; ++q) {
-        if ((rc = g->alloc((void **)&F->d_maps[q], sizeof(CUtensorMap) * 6))) return rc;
-        if (cudaMallocHost((void **)&F->h_maps[q], sizeof(CUtensorMap) * 6) != cudaSuccess) {
+        if ((rc = g->alloc((void **)&F->d_maps[q], sizeof(CUtensorMap) * 13))) return rc;
+        if (cudaMallocHost((void **)&F->h_maps[q], sizeof(CUtensorMap) * 13) != cudaSuccess) {
             (void)cudaGetLastError();
             return fdtd_fail(FDTD_ENOMEM, "pinned tensor-map staging allocation failed");
         }
@@ -772,25 +792,26 @@ namespace {
 
 // (re)builds one tensor-map table when the volume it was built for changed.
 //   which = 0: volumes A/B = fields / bufB;  which = 1: lam / lamB
-int build_maps(fdtd_grid *g, int which, float *volA, float *volB, cudaStream_t st)
+int build_maps(fdtd_grid *g, int which, float *volA, float *volB, const float *ie, cudaStream_t st)
 {
     FusedState *F = g->fused;
     const Dims &G = g->G;
-    if (F->maps_key[which] == volA) return FDTD_OK;
+    if (F->maps_key[which][0] == volA && F->maps_key[which][1] == ie) return FDTD_OK;
     const int PW = F->TX + 8, ROWS = F->TY + 2;
     if (cudaEventSynchronize(F->maps_done) != cudaSuccess) { (void)cudaGetLastError(); }   // earlier upload finished
     CUtensorMap *H = F->h_maps[which];
     bool ok = true;
     float *bufs[2] = { volA, volB };
     for (int set = 0; set < 2; ++set)
-        for (int c = 0; c < 3; ++c)
-            ok &= encode3d(&H[set * 3 + c], bufs[set] + (long long)(3 + c) * G.nc, G.nx, G.ny, G.nz, G.nx,
+        for (int c = 0; c < 6; ++c)
+            ok &= encode3d(&H[set * 6 + c], bufs[set] + (long long)c * G.nc, G.nx, G.ny, G.nz, G.nx,
                            (long long)G.nx * G.ny, PW, ROWS);
+    ok &= encode3d(&H[12], ie, G.nx, G.ny, G.nz, G.nx, (long long)G.nx * G.ny, PW, ROWS);
     if (!ok) return fdtd_fail(FDTD_ECUDA, "cuTensorMapEncodeTiled failed");
-    cudaError_t e = cudaMemcpyAsync(F->d_maps[which], H, sizeof(CUtensorMap) * 6, cudaMemcpyHostToDevice, st);
+    cudaError_t e = cudaMemcpyAsync(F->d_maps[which], H, sizeof(CUtensorMap) * 13, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaEventRecord(F->maps_done, st);
     if (e != cudaSuccess) { (void)cudaGetLastError(); return fdtd_fail(FDTD_ECUDA, std::string("tensor map upload: ") + cudaGetErrorString(e)); }
-    F->maps_key[which] = volA;
+    F->maps_key[which][0] = volA; F->maps_key[which][1] = ie;
     return FDTD_OK;
 }
 
@@ -857,7 +878,7 @@ int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float
     FusedState *F = g->fused;
     if ((int)S.size() > MAX_SRC || (int)D.size() > MAX_DET)
         return fdtd_fail(FDTD_EINVAL, "the fused path takes at most 4 sources and 4 detectors (use FDTD_PATH_GENERIC)");
-    int rc = build_maps(g, 0, fields, F->bufB, st);
+    int rc = build_maps(g, 0, fields, F->bufB, inv_eps, st);
     if (rc) return rc;
     for (int q = 0; q < 2; ++q)
         if ((rc = g->zero_psi(g->psiE[q], st)) || (rc = g->zero_psi(g->psiH[q], st))) return rc;
@@ -871,6 +892,15 @@ int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float
     for (size_t q = 0; q < S.size(); ++q) P.src[q] = S[q];
     for (size_t q = 0; q < D.size(); ++q) P.det[q] = D[q];
     P.cs = g->d_cs;
+    P.sEl = P.sHl = P.dEl = P.dHl = 1 << 30; P.sEh = P.sHh = P.dEh = P.dHh = -1;
+    for (const SourceDev &q : S) {
+        if (q.comp < 3) { P.sEl = std::min(P.sEl, q.lo[2]); P.sEh = std::max(P.sEh, q.hi[2]); }
+        else { P.sHl = std::min(P.sHl, q.lo[2]); P.sHh = std::max(P.sHh, q.hi[2]); }
+    }
+    for (const DetectorDev &q : D) {
+        if (q.mask & 7) { P.dEl = std::min(P.dEl, q.lo[2]); P.dEh = std::max(P.dEh, q.hi[2]); }
+        if (q.mask >> 3) { P.dHl = std::min(P.dHl, q.lo[2]); P.dHh = std::max(P.dHh, q.hi[2]); }
+    }
     std::string key("ff");
     key.append((const char *)&P, sizeof(P));
     key.push_back(recording ? 1 : 0);
@@ -894,7 +924,7 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     const size_t vol6 = (size_t)g->G.nc * 6 * sizeof(float);
     int rc;
     if (!F->lamB && (rc = g->alloc((void **)&F->lamB, vol6))) return rc;
-    if ((rc = build_maps(g, 1, g->lam, F->lamB, st))) return rc;
+    if ((rc = build_maps(g, 1, g->lam, F->lamB, inv_eps, st))) return rc;
     if (n_steps & 1) {
         cudaError_t e = cudaMemcpyAsync(F->lamB, g->lam, vol6, cudaMemcpyDeviceToDevice, st);
         if (e != cudaSuccess) { (void)cudaGetLastError(); return fdtd_fail(FDTD_ECUDA, cudaGetErrorString(e)); }
@@ -906,6 +936,7 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     P.ie = inv_eps; P.im = nullptr;
     for (int q = 0; q < 2; ++q) { P.psiE[q] = g->lpsiE[q]; P.psiH[q] = g->lpsiH[q]; }
     P.n_src = 0; P.n_det = 0; P.total_freq = total_freq;
+    P.sEl = P.sHl = P.dEl = P.dHl = 1 << 30; P.sEh = P.sHh = P.dEh = P.dHh = -1;
     P.cs = g->d_cs;
     int n_adj = 0;
     for (const DetectorDev &dt : D) if (dt.phasor) ++n_adj;
