@@ -8,7 +8,7 @@
 // Design
 //   * ping-pong volumes: a launch reads buffer `par` and writes buffer `par^1`, so tiles are independent;
 //   * the xy plane is cut into TX x TY tiles, a tile's z column into segments; a persistent CTA marches its
-//     segments plane by plane (2.5-D blocking), carrying the previous plane in registers;
+//     segments plane by plane (2.5-D blocking); the previous plane stays in its stage / in the ring;
 //   * only the three arrays that are differenced in phase A (the H-type operand F) need neighbours: one
 //     producer thread streams their boxes (one-cell halo, 16-byte aligned in x) global -> shared with TMA
 //     (cp.async.bulk.tensor; the zero fill outside the grid IS the zero-pad wall convention R7) through a
@@ -191,14 +191,6 @@ __device__ __noinline__ void detect4(const StepParams &P, int n, int family, flo
 // (filtered) difference of component c along axis a; its state array is
 //   Dy_z p[0][0]   Dz_y p[0][1]   Dz_x p[1][0]   Dx_z p[1][1]   Dx_y p[2][0]   Dy_x p[2][1].
 // ================================================================================================
-// what a thread carries from plane kk-1 to plane kk (two copies alternate, so nothing is moved)
-struct Carry {
-    float4 hx, hy, hz;          // H-type target (= raw F) at my cells
-    float4 gx, gy;              // adjoint: z-filtered F_x, F_y (forward: hx, hy)
-    float4 Yx, Yz, Xy;          // phase-B operands at my cells: forward v_x, v_z, v_y
-    float4 Xz, Zx, Zy;          // adjoint only (forward: Yz, Yx, Xy)
-};
-
 __device__ __forceinline__ void pf_l1(const float *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
 template <class C, bool ADJ>
@@ -280,6 +272,9 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
     int st_i = 0;                 // pipeline stage of the next plane
     uint32_t st_ph = 0;           // its full-barrier parity
     uint32_t st_off = 0;          // st_i * STAGE
+    int pv_i = 0;                 // the stage that holds the previous plane
+    uint32_t pv_off = 0;
+    float4 cgx = Z4, cgy = Z4, cZx = Z4, cZy = Z4;   // adjoint: z-filtered operands of the previous plane at my cells
     for (int sg = seg_lo; sg < seg_hi; ++sg) {
         const Segment Sg = segs[sg];
         const int i = Sg.i0 + 4 * tx, j = Sg.j0 + ty;
@@ -297,10 +292,11 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
         const int k1 = Sg.k1;
 
         // ---------------------------------------------------------------- one plane (phase A of kk, phase B of kk-1)
-        auto plane_step = [&](const int kk, const Carry &in, Carry &out, const bool doB) {
+        auto plane_step = [&](const int kk, const bool doB) {
             const int zs = pml ? slab_pos(kk, G.nz, G.d) : -1;
             mbar_wait(&full[st_i], st_ph);
             const uint32_t so = stage_base + st_off + o_own;
+            const uint32_t sp = stage_base + pv_off + o_own;       // the stage of plane kk-1 is still held
             const float4 fx = lds4(so), fy = lds4(so + C::SLOT), fz = lds4(so + 2 * C::SLOT);
             const float4 fx_my = lds4(so - C::ROWB), fz_my = lds4(so + 2 * C::SLOT - C::ROWB);
             const float fy_mx = lds1(so + C::SLOT - 4), fz_mx = lds1(so + 2 * C::SLOT - 4);
@@ -313,9 +309,8 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
             float4 Dy_z = fz - fz_my, Dy_x = fx - fx_my;
             float4 Dx_y = dminus_x(fy, fy_mx), Dx_z = dminus_x(fz, fz_mx);
             float4 Dz_x, Dz_y;
-            out.hx = fx; out.hy = fy; out.hz = fz;
             if (!ADJ) {
-                Dz_x = fx - in.hx; Dz_y = fy - in.hy;
+                Dz_x = fx - lds4(sp); Dz_y = fy - lds4(sp + C::SLOT);
                 if (slab_xy || zs >= 0) {
                     if (zs >= 0 && ing) {
                         const float b = __ldg(P.T.b[FA][2] + kk), a = __ldg(P.T.a[FA][2] + kk), km = __ldg(P.T.ik[FA][2] + kk) - 1.f;
@@ -393,16 +388,12 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                         Dx_z = Dx_z + dminus_x(cz, lz);
                     }
                 }
-                Dz_x = gx - in.gx; Dz_y = gy - in.gy;
-                out.gx = gx; out.gy = gy;
+                Dz_x = gx - cgx; Dz_y = gy - cgy;
+                cgx = gx; cgy = gy;
             }
             const float4 tEx = Dy_z - Dz_y, tEy = Dz_x - Dx_z, tEz = Dx_y - Dy_x;
             const float4 ex = lds4(so + 3 * C::SLOT), ey = lds4(so + 4 * C::SLOT), ez = lds4(so + 5 * C::SLOT);
             const float4 sie = S * lds4(so + 6 * C::SLOT);
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[st_i]);
-            st_off += C::STAGE;
-            if (++st_i == nst) { st_i = 0; st_off = 0; st_ph ^= 1; }
             float4 e2x, e2y, e2z, v2x, v2y, v2z;
             if (ADJ) {
                 e2x = fma4(-S, tEx, ex); e2y = fma4(-S, tEy, ey); e2z = fma4(-S, tEz, ez);
@@ -449,8 +440,6 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
             }
             sts4(rgA, Yx); sts4(rgA + C::RING_ARR * 4, Yz); sts4(rgA + 2 * C::RING_ARR * 4, Xy);
             if (ADJ) sts4(rgA + 3 * C::RING_ARR * 4, Xz);
-            out.Yx = Yx; out.Yz = Yz; out.Xy = Xy;
-            if (ADJ) { out.Xz = Xz; out.Zx = Zx; out.Zy = Zy; }
             // ---------------------------------------------------------------- phase B: H-type update of plane kk-1
             if (own_ok && doB) {
                 const int km1 = kk - 1;
@@ -458,9 +447,11 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                 const float4 Yx_py = lds4(rgB + C::RP * 4), Yz_py = lds4(rgB + (C::RING_ARR + C::RP) * 4);
                 const float Xy_px = lds1(rgB + (2 * C::RING_ARR + 4) * 4);
                 const float Xz_px = lds1(rgB + ((ADJ ? 3 : 1) * C::RING_ARR + 4) * 4);
-                float4 Dy_z = Yz_py - in.Yz, Dy_x = Yx_py - in.Yx;
-                float4 Dz_y = Zy - (ADJ ? in.Zy : in.Xy), Dz_x = Zx - (ADJ ? in.Zx : in.Yx);
-                float4 Dx_z = dplus_x(ADJ ? in.Xz : in.Yz, Xz_px), Dx_y = dplus_x(in.Xy, Xy_px);
+                const float4 oYx = lds4(rgB), oYz = lds4(rgB + C::RING_ARR * 4), oXy = lds4(rgB + 2 * C::RING_ARR * 4);
+                const float4 oXz = ADJ ? lds4(rgB + 3 * C::RING_ARR * 4) : oYz;
+                float4 Dy_z = Yz_py - oYz, Dy_x = Yx_py - oYx;
+                float4 Dz_y = Zy - (ADJ ? cZy : oXy), Dz_x = Zx - (ADJ ? cZx : oYx);
+                float4 Dx_z = dplus_x(oXz, Xz_px), Dx_y = dplus_x(oXy, Xy_px);
                 const int offm = off - plane;
                 const int zsm = (!ADJ && pml) ? slab_pos(km1, G.nz, G.d) : -1;
                 if (!ADJ && (slab_xy || zsm >= 0)) {
@@ -492,12 +483,13 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                     }
                 }
                 const float4 tHx = Dy_z - Dz_y, tHy = Dz_x - Dx_z, tHz = Dx_y - Dy_x;
+                const float4 hx = lds4(sp), hy = lds4(sp + C::SLOT), hz = lds4(sp + 2 * C::SLOT);
                 float4 h2x, h2y, h2z;
                 if (ADJ) {
-                    h2x = in.hx + tHx; h2y = in.hy + tHy; h2z = in.hz + tHz;
+                    h2x = hx + tHx; h2y = hy + tHy; h2z = hz + tHz;
                 } else {
                     const float4 sim = has_mu ? S * ldg4(P.im + offm) : splat(S);
-                    h2x = in.hx - sim * tHx; h2y = in.hy - sim * tHy; h2z = in.hz - sim * tHz;
+                    h2x = hx - sim * tHx; h2y = hy - sim * tHy; h2z = hz - sim * tHz;
                     if (km1 >= P.sHl && km1 < P.sHh) {
                         h2x = add_sources4(P, n, 3, h2x, i, j, km1); h2y = add_sources4(P, n, 4, h2y, i, j, km1); h2z = add_sources4(P, n, 5, h2z, i, j, km1);
                     }
@@ -506,40 +498,42 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                 stg4(o, h2x); stg4(o + nc, h2y); stg4(o + 2 * nc, h2z);
                 if (!ADJ && km1 >= P.dHl && km1 < P.dHh) detect4(P, n, 1, h2x, h2y, h2z, i, j, km1);
             }
+            if (ADJ) { cZx = Zx; cZy = Zy; }
+            // the stage of plane kk-1 is no longer needed; the stage of plane kk stays for the next iteration
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[pv_i]);
+            pv_i = st_i; pv_off = st_off;
+            st_off += C::STAGE;
+            if (++st_i == nst) { st_i = 0; st_off = 0; st_ph ^= 1; }
             named_bar_sync(1, C::NCW * 32);      // ring slot (kk-1)&1 may be overwritten in the next iteration
         };
 
-        // ---------------------------------------------------------------- prologue: the z operands of plane k0-1
-        Carry A, B;
+        // ---------------------------------------------------------------- prologue: plane k0-1 (F only) becomes the held stage
         {
             const int kk = Sg.k0 - 1;
             mbar_wait(&full[st_i], st_ph);
-            const uint32_t so = stage_base + st_off + o_own;
-            A.hx = lds4(so); A.hy = lds4(so + C::SLOT); A.hz = Z4;
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[st_i]);
-            st_off += C::STAGE;
-            if (++st_i == nst) { st_i = 0; st_off = 0; st_ph ^= 1; }
-            A.gx = A.hx; A.gy = A.hy;
-            if (ADJ && pml) {
-                const int zs = slab_pos(kk, G.nz, G.d);
-                if (zs >= 0 && ing) {
-                    const float b = __ldg(P.T.b[FA][2] + kk), a = __ldg(P.T.a[FA][2] + kk), km = __ldg(P.T.ik[FA][2] + kk) - 1.f;
-                    const int oz = zs * pz + own_xy;
-                    float4 pn;
-                    A.gx = A.hx + cpml4(b, a, km, ldg4(qAi.p[1][0] + oz), A.hx, pn);
-                    A.gy = A.hy + cpml4(b, a, km, ldg4(qAi.p[0][1] + oz), A.hy, pn);
+            if (ADJ) {
+                const uint32_t so = stage_base + st_off + o_own;
+                cgx = lds4(so); cgy = lds4(so + C::SLOT);
+                if (pml) {
+                    const int zs = slab_pos(kk, G.nz, G.d);
+                    if (zs >= 0 && ing) {
+                        const float b = __ldg(P.T.b[FA][2] + kk), a = __ldg(P.T.a[FA][2] + kk), km = __ldg(P.T.ik[FA][2] + kk) - 1.f;
+                        const int oz = zs * pz + own_xy;
+                        float4 pn;
+                        cgx = cgx + cpml4(b, a, km, ldg4(qAi.p[1][0] + oz), cgx, pn);
+                        cgy = cgy + cpml4(b, a, km, ldg4(qAi.p[0][1] + oz), cgy, pn);
+                    }
                 }
             }
-            A.Yx = A.Yz = A.Xy = A.Xz = A.Zx = A.Zy = Z4;
+            pv_i = st_i; pv_off = st_off;
+            st_off += C::STAGE;
+            if (++st_i == nst) { st_i = 0; st_off = 0; st_ph ^= 1; }
         }
-        plane_step(Sg.k0, A, B, false);
-        int kk = Sg.k0 + 1;
-        for (; kk + 1 <= k1; kk += 2) {
-            plane_step(kk, B, A, true);
-            plane_step(kk + 1, A, B, true);
-        }
-        if (kk <= k1) plane_step(kk, B, A, true);
+        plane_step(Sg.k0, false);
+        for (int kk = Sg.k0 + 1; kk <= k1; ++kk) plane_step(kk, true);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[pv_i]);      // the stage of plane k1
     }
 }
 
@@ -694,7 +688,7 @@ int fused_setup(fdtd_grid *g)
         const TileImpl &t = kTiles[q];
         if (fTX && (t.TX != fTX || t.TY != fTY)) continue;
         const int nst = std::min(MAX_ST, (smem_cap - t.ring_bytes - tail_bytes - 1024) / t.stage);
-        if (nst < 2) continue;
+        if (nst < 3) continue;                                   // previous plane held + current + one in flight
         const long long ntx = (G.nx + t.TX - 1) / t.TX, nty = (G.ny + t.TY - 1) / t.TY;
         const double eff = ((double)G.nx / 4 * G.ny) / ((double)ntx * nty * t.ncw * 32);
         const double fill = std::min(1.0, (double)ntx * nty * G.nz / (8.0 * n_sm));   // enough planes per CTA to amortise prologues
@@ -707,7 +701,7 @@ int fused_setup(fdtd_grid *g)
     FusedState *F = new FusedState();
     g->fused = F;
     F->tile = best; F->TX = best->TX; F->TY = best->TY; F->nst = best_nst;
-    if (const char *e = getenv("FDTD_NST")) F->nst = std::max(2, std::min(best_nst, atoi(e)));
+    if (const char *e = getenv("FDTD_NST")) F->nst = std::max(3, std::min(best_nst, atoi(e)));
     F->smem = (size_t)F->nst * best->stage + best->ring_bytes + tail_bytes;
     int rc;
     if ((rc = g->alloc((void **)&F->bufB, (size_t)G.nc * 6 * sizeof(float)))) return rc;
