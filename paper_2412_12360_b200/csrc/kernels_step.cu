@@ -45,7 +45,7 @@ constexpr int MAX_ST = 8;               // upper bound of pipeline stages
 struct StepParams {
     Dims G;
     Tables T;
-    const CUtensorMap *maps;       // [set][6]: components of buffer `set`; [12]: inv_eps
+    const CUtensorMap *maps;       // [set][6]: components of buffer `set`; [12]: inv_eps; [13 + set*4 + family*2 + a]: x-slab states
     const Segment *segs;           // [n_rot][seg_stride]
     const int *seg_begin;          // [n_rot][n_cta + 1]
     int n_rot, seg_stride, n_cta;
@@ -54,6 +54,9 @@ struct StepParams {
     PsiSet psiE[2], psiH[2];       // CPML states of the E-type / H-type update, ping-pong
     const int *step;
     int nst;                       // pipeline stages
+    int stage;                     // bytes of one stage: 7 boxes + 4 x-slab state boxes
+    int xs_bytes, xs_pitch;        // x-slab state box [ROWS][2*dpx]: exact bytes (TMA transaction) and 128-byte aligned pitch
+    int dbg;                       // timing experiments only (FDTD_DBG): 1 no global stores, 2 no phase B, 4 no barrier
     int n_src, n_det, total_freq;
     int sEl, sEh, sHl, sHh, dEl, dEh, dHl, dHh;   // k ranges of the planes that hold E/H sources and E/H detectors
     SourceDev src[MAX_SRC];
@@ -191,7 +194,7 @@ __device__ __noinline__ void detect4(const StepParams &P, int n, int family, flo
 // (filtered) difference of component c along axis a; its state array is
 //   Dy_z p[0][0]   Dz_y p[0][1]   Dz_x p[1][0]   Dx_z p[1][1]   Dx_y p[2][0]   Dy_x p[2][1].
 // ================================================================================================
-__device__ __forceinline__ void pf_l1(const float *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+__device__ __forceinline__ void pf_l2(const float *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 template <class C, bool ADJ>
 __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ StepParams P)
@@ -199,8 +202,8 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
     extern __shared__ __align__(1024) uint8_t smem[];
     const Dims &G = P.G;
     const uint32_t stage_base = smem_u32(smem);
-    const uint32_t ring_base = stage_base + (uint32_t)P.nst * C::STAGE;
-    uint64_t *full = reinterpret_cast<uint64_t *>(smem + (size_t)P.nst * C::STAGE + C::RING_BYTES);
+    const uint32_t ring_base = stage_base + (uint32_t)P.nst * P.stage;
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + (size_t)P.nst * P.stage + C::RING_BYTES);
     uint64_t *empty = full + MAX_ST;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n = *P.step;
@@ -231,9 +234,10 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
             for (int kk = S.k0 - 1; kk <= S.k1; ++kk) {
                 if (use > 0) mbar_wait(&empty[s], (use - 1) & 1);
                 uint64_t *fb = &full[s];
-                uint8_t *st = smem + (size_t)s * C::STAGE;
+                uint8_t *st = smem + (size_t)s * P.stage;
                 const bool prolog = kk == S.k0 - 1;
-                mbar_expect_tx(fb, (prolog ? 3u : 7u) * C::BOX_BYTES);
+                const bool xs = G.d > 0 && !prolog;
+                mbar_expect_tx(fb, (prolog ? 3u : 7u) * C::BOX_BYTES + (xs ? 4u * P.xs_bytes : 0u));
                 tma_load_3d(st, M + 3, x, y, kk, fb);
                 tma_load_3d(st + C::SLOT, M + 4, x, y, kk, fb);
                 tma_load_3d(st + 2 * C::SLOT, M + 5, x, y, kk, fb);
@@ -242,6 +246,15 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                     tma_load_3d(st + 4 * C::SLOT, M + 1, x, y, kk, fb);
                     tma_load_3d(st + 5 * C::SLOT, M + 2, x, y, kk, fb);
                     tma_load_3d(st + 6 * C::SLOT, Mie, x, y, kk, fb);
+                }
+                if (xs) {      // phase A states of plane kk; phase B states of plane kk-1 (forward) / kk (adjoint)
+                    const CUtensorMap *MA = P.maps + 13 + par * 4 + FA * 2, *MB = P.maps + 13 + par * 4 + FB * 2;
+                    uint8_t *sx0 = st + 7 * C::SLOT;
+                    const int kb = ADJ ? kk : kk - 1;
+                    tma_load_3d(sx0, MA, 0, y, kk, fb);
+                    tma_load_3d(sx0 + P.xs_pitch, MA + 1, 0, y, kk, fb);
+                    tma_load_3d(sx0 + 2 * P.xs_pitch, MB, 0, y, kb, fb);
+                    tma_load_3d(sx0 + 3 * P.xs_pitch, MB + 1, 0, y, kb, fb);
                 }
                 if (++s == nst) { s = 0; ++use; }
             }
@@ -263,7 +276,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
     const float S = G.S;
     const long long nc = G.nc;
     const int plane = G.ny * G.nx;
-    const bool pml = G.d > 0;
+    const bool pml = G.d > 0 && !(P.dbg & 16);
     const bool has_mu = !ADJ && P.im != nullptr;
     const int pz = plane, py = 2 * G.d * G.nx, px = G.ny * 2 * G.dpx;      // plane pitch of the z / y / x state arrays
 
@@ -282,33 +295,46 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
         const bool own_ok = inner && ing;
         const int own_xy = j * G.nx + i;
         // slab-compact coordinates of my cells and (adjoint) of my -x / -y neighbours; -1: not in a slab
-        const int sx = (pml && ing) ? slab_pos(i, G.nx, G.dpx) : -1;
-        const int sy = (pml && ing) ? slab_pos(j, G.ny, G.d) : -1;
-        const int sxm = (ADJ && pml && ing) ? slab_pos(i - 1, G.nx, G.dpx) : -1;
-        const int sym = (ADJ && pml && ing) ? slab_pos(j - 1, G.ny, G.d) : -1;
+        const int sx = (pml && ing && !(P.dbg & 32)) ? slab_pos(i, G.nx, G.dpx) : -1;
+        const int sy = (pml && ing && !(P.dbg & 64)) ? slab_pos(j, G.ny, G.d) : -1;
+        const int sxm = (ADJ && pml && ing && !(P.dbg & 32)) ? slab_pos(i - 1, G.nx, G.dpx) : -1;
+        const int sym = (ADJ && pml && ing && !(P.dbg & 64)) ? slab_pos(j - 1, G.ny, G.d) : -1;
         const bool slab_xy = __any_sync(0xffffffffu, (sx & sy & sxm & sym) >= 0);   // this warp runs x / y slab code
         const int oy = sy * G.nx + i, oym = sym * G.nx + i;                          // + k * py
         const int ox = j * (2 * G.dpx) + sx, oxm = j * (2 * G.dpx) + sxm;           // + k * px
+        const uint32_t xo = ((1 + ty) * 2 * G.dpx + sx) * 4, xom = ((1 + ty) * 2 * G.dpx + sxm) * 4;   // inside an x-slab state box
         const int k1 = Sg.k1;
 
         // ---------------------------------------------------------------- one plane (phase A of kk, phase B of kk-1)
         auto plane_step = [&](const int kk, const bool doB) {
-            const int zs = pml ? slab_pos(kk, G.nz, G.d) : -1;
+            const int zs = (pml && !(P.dbg & 128)) ? slab_pos(kk, G.nz, G.d) : -1;
             mbar_wait(&full[st_i], st_ph);
             const uint32_t so = stage_base + st_off + o_own;
             const uint32_t sp = stage_base + pv_off + o_own;       // the stage of plane kk-1 is still held
+            const uint32_t xs0 = stage_base + st_off + 7 * C::SLOT; // x-slab state boxes of this stage
             const float4 fx = lds4(so), fy = lds4(so + C::SLOT), fz = lds4(so + 2 * C::SLOT);
             const float4 fx_my = lds4(so - C::ROWB), fz_my = lds4(so + 2 * C::SLOT - C::ROWB);
             const float fy_mx = lds1(so + C::SLOT - 4), fz_mx = lds1(so + 2 * C::SLOT - 4);
 
-            const bool wr = own_ok && kk < k1;                 // I own these cells: write the result and the phase-A states
+            const bool wr = own_ok && kk < k1 && !(P.dbg & 1);                 // I own these cells: write the result and the phase-A states
             const int off = kk * plane + own_xy;
             const int oz = zs * pz + own_xy;
             const uint32_t rgA = ring_base + (uint32_t)(kk & 1) * (C::RING_SLOT * 4) + r_own;
+            // plane nz (the zero wall behind the last plane) has no CPML states: all its inputs are zero
+            const bool kin = kk < G.nz;
+            const bool pf = kk + 2 < G.nz;                     // L2 prefetch of the states two planes ahead stays inside the arrays
+            const int sxk = kin ? sx : -1, syk = kin ? sy : -1, sxmk = kin ? sxm : -1, symk = kin ? sym : -1;
             // ------------------------------------------------------------ phase A: E-type update of plane kk
             float4 Dy_z = fz - fz_my, Dy_x = fx - fx_my;
             float4 Dx_y = dminus_x(fy, fy_mx), Dx_z = dminus_x(fz, fz_mx);
             float4 Dz_x, Dz_y;
+            if (pml && ing) {
+                const int zs2 = slab_pos(kk + 2, G.nz, G.d);
+                if (zs2 >= 0) {
+                    const int q = zs2 * pz + own_xy;
+                    pf_l2(qAi.p[1][0] + q); pf_l2(qAi.p[0][1] + q); pf_l2(qBi.p[1][0] + q); pf_l2(qBi.p[0][1] + q);
+                }
+            }
             if (!ADJ) {
                 Dz_x = fx - lds4(sp); Dz_y = fy - lds4(sp + C::SLOT);
                 if (slab_xy || zs >= 0) {
@@ -319,22 +345,21 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                         Dz_y = Dz_y + cpml4(b, a, km, ldg4(qAi.p[0][1] + oz), Dz_y, p1);
                         if (wr) { stg4(qAo.p[1][0] + oz, p0); stg4(qAo.p[0][1] + oz, p1); }
                     }
-                    if (sy >= 0) {
+                    if (syk >= 0) {
                         const float b = __ldg(P.T.b[FA][1] + j), a = __ldg(P.T.a[FA][1] + j), km = __ldg(P.T.ik[FA][1] + j) - 1.f;
                         const int q = kk * py + oy;
                         float4 p0, p1;
                         Dy_z = Dy_z + cpml4(b, a, km, ldg4(qAi.p[0][0] + q), Dy_z, p0);
                         Dy_x = Dy_x + cpml4(b, a, km, ldg4(qAi.p[2][1] + q), Dy_x, p1);
-                        pf_l1(qAi.p[0][0] + q + py); pf_l1(qAi.p[2][1] + q + py);
+                        if (pf) { pf_l2(qAi.p[0][0] + q + 2 * py); pf_l2(qAi.p[2][1] + q + 2 * py); }
                         if (wr) { stg4(qAo.p[0][0] + q, p0); stg4(qAo.p[2][1] + q, p1); }
                     }
-                    if (sx >= 0) {
+                    if (sxk >= 0) {
                         const float4 b = ldg4(P.T.b[FA][0] + i), a = ldg4(P.T.a[FA][0] + i), km = ldg4(P.T.ik[FA][0] + i) - splat(1.f);
                         const int q = kk * px + ox;
                         float4 p0, p1;
-                        Dx_y = Dx_y + cpml4(b, a, km, ldg4(qAi.p[2][0] + q), Dx_y, p0);
-                        Dx_z = Dx_z + cpml4(b, a, km, ldg4(qAi.p[1][1] + q), Dx_z, p1);
-                        pf_l1(qAi.p[2][0] + q + px); pf_l1(qAi.p[1][1] + q + px);
+                        Dx_y = Dx_y + cpml4(b, a, km, lds4(xs0 + xo), Dx_y, p0);
+                        Dx_z = Dx_z + cpml4(b, a, km, lds4(xs0 + P.xs_pitch + xo), Dx_z, p1);
                         if (wr) { stg4(qAo.p[2][0] + q, p0); stg4(qAo.p[1][1] + q, p1); }
                     }
                 }
@@ -348,41 +373,39 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                         gy = fy + cpml4(b, a, km, ldg4(qAi.p[0][1] + oz), fy, p1);
                         if (wr) { stg4(qAo.p[1][0] + oz, p0); stg4(qAo.p[0][1] + oz, p1); }
                     }
-                    if (sy >= 0) {
+                    if (syk >= 0) {
                         const float b = __ldg(P.T.b[FA][1] + j), a = __ldg(P.T.a[FA][1] + j), km = __ldg(P.T.ik[FA][1] + j) - 1.f;
                         const int q = kk * py + oy;
                         float4 p0, p1;
                         Dy_z = Dy_z + cpml4(b, a, km, ldg4(qAi.p[0][0] + q), fz, p0);
                         Dy_x = Dy_x + cpml4(b, a, km, ldg4(qAi.p[2][1] + q), fx, p1);
-                        pf_l1(qAi.p[0][0] + q + py); pf_l1(qAi.p[2][1] + q + py);
+                        if (pf) { pf_l2(qAi.p[0][0] + q + 2 * py); pf_l2(qAi.p[2][1] + q + 2 * py); }
                         if (wr) { stg4(qAo.p[0][0] + q, p0); stg4(qAo.p[2][1] + q, p1); }
                     }
-                    if (sym >= 0) {
+                    if (symk >= 0) {
                         const float b = __ldg(P.T.b[FA][1] + j - 1), a = __ldg(P.T.a[FA][1] + j - 1), km = __ldg(P.T.ik[FA][1] + j - 1) - 1.f;
                         const int q = kk * py + oym;
                         float4 p0, p1;
                         Dy_z = Dy_z - cpml4(b, a, km, ldg4(qAi.p[0][0] + q), fz_my, p0);
                         Dy_x = Dy_x - cpml4(b, a, km, ldg4(qAi.p[2][1] + q), fx_my, p1);
-                        if (sy < 0) { pf_l1(qAi.p[0][0] + q + py); pf_l1(qAi.p[2][1] + q + py); }
+                        if (pf && syk < 0) { pf_l2(qAi.p[0][0] + q + 2 * py); pf_l2(qAi.p[2][1] + q + 2 * py); }
                     }
-                    if (sx >= 0 || sxm >= 0) {
+                    if (sxk >= 0 || sxmk >= 0) {
                         float4 cy = Z4, cz = Z4;
                         float ly = 0.f, lz = 0.f;
-                        if (sx >= 0) {
+                        if (sxk >= 0) {
                             const float4 b = ldg4(P.T.b[FA][0] + i), a = ldg4(P.T.a[FA][0] + i), km = ldg4(P.T.ik[FA][0] + i) - splat(1.f);
                             const int q = kk * px + ox;
                             float4 p0, p1;
-                            cy = cpml4(b, a, km, ldg4(qAi.p[2][0] + q), fy, p0);
-                            cz = cpml4(b, a, km, ldg4(qAi.p[1][1] + q), fz, p1);
-                            pf_l1(qAi.p[2][0] + q + px); pf_l1(qAi.p[1][1] + q + px);
+                            cy = cpml4(b, a, km, lds4(xs0 + xo), fy, p0);
+                            cz = cpml4(b, a, km, lds4(xs0 + P.xs_pitch + xo), fz, p1);
                             if (wr) { stg4(qAo.p[2][0] + q, p0); stg4(qAo.p[1][1] + q, p1); }
                         }
-                        if (sxm >= 0) {
+                        if (sxmk >= 0) {
                             const float b = __ldg(P.T.b[FA][0] + i - 1), a = __ldg(P.T.a[FA][0] + i - 1), km = __ldg(P.T.ik[FA][0] + i - 1) - 1.f;
                             const int q = kk * px + oxm;
-                            ly = cpml1(b, a, km, __ldg(qAi.p[2][0] + q), fy_mx);
-                            lz = cpml1(b, a, km, __ldg(qAi.p[1][1] + q), fz_mx);
-                            if (sx < 0) { pf_l1(qAi.p[2][0] + q + px); pf_l1(qAi.p[1][1] + q + px); }
+                            ly = cpml1(b, a, km, lds1(xs0 + xom), fy_mx);
+                            lz = cpml1(b, a, km, lds1(xs0 + P.xs_pitch + xom), fz_mx);
                         }
                         Dx_y = Dx_y + dminus_x(cy, ly);
                         Dx_z = Dx_z + dminus_x(cz, lz);
@@ -419,29 +442,28 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                     Zy = v2y + cpml4(b, a, km, ldg4(qBi.p[0][1] + oz), v2y, p1);
                     if (wr) { stg4(qBo.p[1][0] + oz, p0); stg4(qBo.p[0][1] + oz, p1); }
                 }
-                if (sy >= 0) {
+                if (syk >= 0) {
                     const float b = __ldg(P.T.b[FB][1] + j), a = __ldg(P.T.a[FB][1] + j), km = __ldg(P.T.ik[FB][1] + j) - 1.f;
                     const int q = kk * py + oy;
                     float4 p0, p1;
                     Yz = v2z + cpml4(b, a, km, ldg4(qBi.p[0][0] + q), v2z, p0);
                     Yx = v2x + cpml4(b, a, km, ldg4(qBi.p[2][1] + q), v2x, p1);
-                    pf_l1(qBi.p[0][0] + q + py); pf_l1(qBi.p[2][1] + q + py);
+                    if (pf) { pf_l2(qBi.p[0][0] + q + 2 * py); pf_l2(qBi.p[2][1] + q + 2 * py); }
                     if (wr) { stg4(qBo.p[0][0] + q, p0); stg4(qBo.p[2][1] + q, p1); }
                 }
-                if (sx >= 0) {
+                if (sxk >= 0) {
                     const float4 b = ldg4(P.T.b[FB][0] + i), a = ldg4(P.T.a[FB][0] + i), km = ldg4(P.T.ik[FB][0] + i) - splat(1.f);
                     const int q = kk * px + ox;
                     float4 p0, p1;
-                    Xy = v2y + cpml4(b, a, km, ldg4(qBi.p[2][0] + q), v2y, p0);
-                    Xz = v2z + cpml4(b, a, km, ldg4(qBi.p[1][1] + q), v2z, p1);
-                    pf_l1(qBi.p[2][0] + q + px); pf_l1(qBi.p[1][1] + q + px);
+                    Xy = v2y + cpml4(b, a, km, lds4(xs0 + 2 * P.xs_pitch + xo), v2y, p0);
+                    Xz = v2z + cpml4(b, a, km, lds4(xs0 + 3 * P.xs_pitch + xo), v2z, p1);
                     if (wr) { stg4(qBo.p[2][0] + q, p0); stg4(qBo.p[1][1] + q, p1); }
                 }
             }
             sts4(rgA, Yx); sts4(rgA + C::RING_ARR * 4, Yz); sts4(rgA + 2 * C::RING_ARR * 4, Xy);
             if (ADJ) sts4(rgA + 3 * C::RING_ARR * 4, Xz);
             // ---------------------------------------------------------------- phase B: H-type update of plane kk-1
-            if (own_ok && doB) {
+            if (own_ok && doB && !(P.dbg & 2)) {
                 const int km1 = kk - 1;
                 const uint32_t rgB = ring_base + (uint32_t)(km1 & 1) * (C::RING_SLOT * 4) + r_own;
                 const float4 Yx_py = lds4(rgB + C::RP * 4), Yz_py = lds4(rgB + (C::RING_ARR + C::RP) * 4);
@@ -453,7 +475,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                 float4 Dz_y = Zy - (ADJ ? cZy : oXy), Dz_x = Zx - (ADJ ? cZx : oYx);
                 float4 Dx_z = dplus_x(oXz, Xz_px), Dx_y = dplus_x(oXy, Xy_px);
                 const int offm = off - plane;
-                const int zsm = (!ADJ && pml) ? slab_pos(km1, G.nz, G.d) : -1;
+                const int zsm = (!ADJ && pml && !(P.dbg & 128)) ? slab_pos(km1, G.nz, G.d) : -1;
                 if (!ADJ && (slab_xy || zsm >= 0)) {
                     if (zsm >= 0) {
                         const float b = __ldg(P.T.b[FB][2] + km1), a = __ldg(P.T.a[FB][2] + km1), km = __ldg(P.T.ik[FB][2] + km1) - 1.f;
@@ -469,16 +491,15 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                         float4 p0, p1;
                         Dy_z = Dy_z + cpml4(b, a, km, ldg4(qBi.p[0][0] + q), Dy_z, p0);
                         Dy_x = Dy_x + cpml4(b, a, km, ldg4(qBi.p[2][1] + q), Dy_x, p1);
-                        pf_l1(qBi.p[0][0] + q + py); pf_l1(qBi.p[2][1] + q + py);
+                        if (pf) { pf_l2(qBi.p[0][0] + q + 2 * py); pf_l2(qBi.p[2][1] + q + 2 * py); }
                         stg4(qBo.p[0][0] + q, p0); stg4(qBo.p[2][1] + q, p1);
                     }
                     if (sx >= 0) {
                         const float4 b = ldg4(P.T.b[FB][0] + i), a = ldg4(P.T.a[FB][0] + i), km = ldg4(P.T.ik[FB][0] + i) - splat(1.f);
                         const int q = km1 * px + ox;
                         float4 p0, p1;
-                        Dx_y = Dx_y + cpml4(b, a, km, ldg4(qBi.p[2][0] + q), Dx_y, p0);
-                        Dx_z = Dx_z + cpml4(b, a, km, ldg4(qBi.p[1][1] + q), Dx_z, p1);
-                        pf_l1(qBi.p[2][0] + q + px); pf_l1(qBi.p[1][1] + q + px);
+                        Dx_y = Dx_y + cpml4(b, a, km, lds4(xs0 + 2 * P.xs_pitch + xo), Dx_y, p0);
+                        Dx_z = Dx_z + cpml4(b, a, km, lds4(xs0 + 3 * P.xs_pitch + xo), Dx_z, p1);
                         stg4(qBo.p[2][0] + q, p0); stg4(qBo.p[1][1] + q, p1);
                     }
                 }
@@ -503,9 +524,9 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[pv_i]);
             pv_i = st_i; pv_off = st_off;
-            st_off += C::STAGE;
+            st_off += P.stage;
             if (++st_i == nst) { st_i = 0; st_off = 0; st_ph ^= 1; }
-            named_bar_sync(1, C::NCW * 32);      // ring slot (kk-1)&1 may be overwritten in the next iteration
+            if (!(P.dbg & 4)) named_bar_sync(1, C::NCW * 32);      // ring slot (kk-1)&1 may be overwritten in the next iteration
         };
 
         // ---------------------------------------------------------------- prologue: plane k0-1 (F only) becomes the held stage
@@ -527,7 +548,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                 }
             }
             pv_i = st_i; pv_off = st_off;
-            st_off += C::STAGE;
+            st_off += P.stage;
             if (++st_i == nst) { st_i = 0; st_off = 0; st_ph ^= 1; }
         }
         plane_step(Sg.k0, false);
@@ -621,36 +642,43 @@ struct FusedState {
 
 namespace {
 
-// Work sequence: z is cut into n_chunk chunks; the sequence is (chunk, tile [y fastest], plane in chunk); it is
-// rotated by `rot` positions and cut into n_cta equal runs.  With chunk length ~ run length, CTAs that hold
-// y-adjacent tiles march through the same planes at about the same time, so halo rows hit L2.
-void make_segments(const Dims &G, int TX, int TY, int n_cta, int n_chunk, long long rot, std::vector<Segment> &segs,
+// Work sequence: (tile [y fastest], plane); it is cut into n_cta runs of equal estimated cost.  A plane of a tile
+// costs 1, plus wy if the tile has rows in a y slab, plus wz if the plane is in a z slab (their CPML states are
+// read by every thread of the tile).  With y fastest, CTAs that hold y-adjacent tiles march through the same
+// planes at about the same time, so halo rows hit L2.
+void make_segments(const Dims &G, int TX, int TY, int n_cta, double wy, double wz, std::vector<Segment> &segs,
                    std::vector<int> &seg_begin)
 {
     const int ntx = (G.nx + TX - 1) / TX, nty = (G.ny + TY - 1) / TY;
     const long long n_tiles = (long long)ntx * nty;
     const long long total = n_tiles * G.nz;
-    std::vector<int> cb(n_chunk + 1);
-    for (int c = 0; c <= n_chunk; ++c) cb[c] = (int)((long long)G.nz * c / n_chunk);
-    std::vector<long long> cstart(n_chunk + 1, 0);       // sequence position where each chunk begins
-    for (int c = 0; c < n_chunk; ++c) cstart[c + 1] = cstart[c] + n_tiles * (cb[c + 1] - cb[c]);
+    std::vector<double> pre(total + 1, 0.0);
+    for (long long t = 0; t < n_tiles; ++t) {
+        const int j0 = (int)(t % nty) * TY;
+        const bool ys = G.d > 0 && (j0 <= G.d || j0 + TY >= G.ny - G.d);
+        for (int k = 0; k < G.nz; ++k) {
+            const bool zs = G.d > 0 && (k <= G.d || k >= G.nz - G.d - 1);
+            pre[t * G.nz + k + 1] = pre[t * G.nz + k] + 1.0 + (ys ? wy : 0.0) + (zs ? wz : 0.0);
+        }
+    }
     segs.clear();
     seg_begin.assign(n_cta + 1, 0);
-    rot = ((rot % total) + total) % total;
+    std::vector<long long> cut(n_cta + 1, 0);
+    for (int c = 1; c < n_cta; ++c) {
+        const double target = pre[total] * c / n_cta;
+        cut[c] = std::max<long long>(cut[c - 1], std::lower_bound(pre.begin(), pre.end(), target) - pre.begin());
+    }
+    cut[n_cta] = total;
     for (int cta = 0; cta < n_cta; ++cta) {
         seg_begin[cta] = (int)segs.size();
-        long long a = total * cta / n_cta, b = total * (cta + 1) / n_cta;      // positions in the rotated sequence
+        long long a = cut[cta];
+        const long long b = cut[cta + 1];
         while (a < b) {
-            const long long pos = (a + rot) % total;                            // position in the canonical sequence
-            int c = (int)(std::upper_bound(cstart.begin(), cstart.end(), pos) - cstart.begin()) - 1;
-            const int clen = cb[c + 1] - cb[c];
-            const long long in_chunk = pos - cstart[c];
-            const long long tile = in_chunk / clen;
-            const int k = cb[c] + (int)(in_chunk % clen);
-            const int len = (int)std::min<long long>(std::min<long long>(b - a, total - pos), cb[c + 1] - k);
-            const int txi = (int)(tile / nty), tyi = (int)(tile % nty);
+            const long long tile = a / G.nz;
+            const int k = (int)(a % G.nz);
+            const int len = (int)std::min<long long>(b - a, G.nz - k);
             Segment s{};
-            s.i0 = txi * TX; s.j0 = tyi * TY; s.k0 = k; s.k1 = k + len;
+            s.i0 = (int)(tile / nty) * TX; s.j0 = (int)(tile % nty) * TY; s.k0 = k; s.k1 = k + len;
             segs.push_back(s);
             a += len;
         }
@@ -687,7 +715,9 @@ int fused_setup(fdtd_grid *g)
     for (int q = 0; q < kNumTiles; ++q) {
         const TileImpl &t = kTiles[q];
         if (fTX && (t.TX != fTX || t.TY != fTY)) continue;
-        const int nst = std::min(MAX_ST, (smem_cap - t.ring_bytes - tail_bytes - 1024) / t.stage);
+        const int xs_pitch = G.d > 0 ? (2 * G.dpx * (t.TY + 2) * 4 + 127) / 128 * 128 : 0;
+        const int stage = t.stage + 4 * xs_pitch;
+        const int nst = std::min(MAX_ST, (smem_cap - t.ring_bytes - tail_bytes - 1024) / stage);
         if (nst < 3) continue;                                   // previous plane held + current + one in flight
         const long long ntx = (G.nx + t.TX - 1) / t.TX, nty = (G.ny + t.TY - 1) / t.TY;
         const double eff = ((double)G.nx / 4 * G.ny) / ((double)ntx * nty * t.ncw * 32);
@@ -702,13 +732,15 @@ int fused_setup(fdtd_grid *g)
     g->fused = F;
     F->tile = best; F->TX = best->TX; F->TY = best->TY; F->nst = best_nst;
     if (const char *e = getenv("FDTD_NST")) F->nst = std::max(3, std::min(best_nst, atoi(e)));
-    F->smem = (size_t)F->nst * best->stage + best->ring_bytes + tail_bytes;
+    const int xs_bytes = G.d > 0 ? 2 * G.dpx * (best->TY + 2) * 4 : 0, xs_pitch = (xs_bytes + 127) / 128 * 128;
+    const int stage_bytes = best->stage + 4 * xs_pitch;
+    F->smem = (size_t)F->nst * stage_bytes + best->ring_bytes + tail_bytes;
     int rc;
     if ((rc = g->alloc((void **)&F->bufB, (size_t)G.nc * 6 * sizeof(float)))) return rc;
     if ((rc = g->alloc_psi(g->psiE[1])) || (rc = g->alloc_psi(g->psiH[1]))) return rc;
     for (int q = 0; q < 2; ++q) {
-        if ((rc = g->alloc((void **)&F->d_maps[q], sizeof(CUtensorMap) * 13))) return rc;
-        if (cudaMallocHost((void **)&F->h_maps[q], sizeof(CUtensorMap) * 13) != cudaSuccess) {
+        if ((rc = g->alloc((void **)&F->d_maps[q], sizeof(CUtensorMap) * 21))) return rc;
+        if (cudaMallocHost((void **)&F->h_maps[q], sizeof(CUtensorMap) * 21) != cudaSuccess) {
             (void)cudaGetLastError();
             return fdtd_fail(FDTD_ENOMEM, "pinned tensor-map staging allocation failed");
         }
@@ -723,29 +755,15 @@ int fused_setup(fdtd_grid *g)
     const long long total = (long long)ntx * nty * G.nz;
     int n_cta = (int)std::min<long long>(n_sm, std::max<long long>(1, total / 6));
     if (const char *e = getenv("FDTD_NCTA")) n_cta = std::max(1, atoi(e));
-    const double run = (double)total / n_cta;                         // planes per CTA
-    int n_chunk = 1;
-    (void)run;
-    if (const char *e = getenv("FDTD_NCHUNK")) n_chunk = std::max(1, std::min(G.nz, atoi(e)));
-    // rotation of the work sequence between steps (n_rot tables, step n uses table n % n_rot)
-    int n_rot = 1;
-    if (const char *e = getenv("FDTD_NROT")) n_rot = std::max(1, std::min(16, atoi(e)));
+    double wy = 1.5, wz = 1.0;                   // relative extra cost of y-slab tiles / z-slab planes (measured on C3)
+    if (const char *e = getenv("FDTD_WY")) wy = atof(e);
+    if (const char *e = getenv("FDTD_WZ")) wz = atof(e);
+    const int n_rot = 1;
     F->n_cta = n_cta; F->n_rot = n_rot;
     std::vector<Segment> all;
     std::vector<int> begins;
-    std::vector<std::vector<Segment>> per(n_rot);
-    std::vector<std::vector<int>> per_b(n_rot);
-    size_t stride = 0;
-    for (int r = 0; r < n_rot; ++r) {
-        const long long per_cta = total / n_cta;
-        make_segments(G, F->TX, F->TY, n_cta, n_chunk, -(long long)r * (per_cta / n_rot), per[r], per_b[r]);
-        stride = std::max(stride, per[r].size());
-    }
-    all.resize(stride * n_rot);
-    for (int r = 0; r < n_rot; ++r) {
-        std::copy(per[r].begin(), per[r].end(), all.begin() + r * stride);
-        begins.insert(begins.end(), per_b[r].begin(), per_b[r].end());
-    }
+    make_segments(G, F->TX, F->TY, n_cta, wy, wz, all, begins);
+    const size_t stride = all.size();
     if ((rc = g->alloc((void **)&F->d_segs, all.size() * sizeof(Segment)))) return rc;
     if ((rc = g->alloc((void **)&F->d_seg_begin, begins.size() * sizeof(int)))) return rc;
     if (cudaMemcpy(F->d_segs, all.data(), all.size() * sizeof(Segment), cudaMemcpyHostToDevice) != cudaSuccess ||
@@ -760,6 +778,8 @@ int fused_setup(fdtd_grid *g)
     P.n_rot = n_rot; P.seg_stride = (int)stride; P.n_cta = n_cta;
     P.step = g->d_step;
     P.nst = F->nst;
+    P.stage = stage_bytes; P.xs_bytes = xs_bytes; P.xs_pitch = xs_pitch;
+    P.dbg = getenv("FDTD_DBG") ? atoi(getenv("FDTD_DBG")) : 0;
     if (best->set_smem(F->smem) != cudaSuccess) {
         (void)cudaGetLastError();
         g->fused_why_not = "cannot reserve shared memory";
@@ -801,8 +821,19 @@ int build_maps(fdtd_grid *g, int which, float *volA, float *volB, const float *i
             ok &= encode3d(&H[set * 6 + c], bufs[set] + (long long)c * G.nc, G.nx, G.ny, G.nz, G.nx,
                            (long long)G.nx * G.ny, PW, ROWS);
     ok &= encode3d(&H[12], ie, G.nx, G.ny, G.nz, G.nx, (long long)G.nx * G.ny, PW, ROWS);
+    if (G.d > 0) {
+        // x-slab states (c=z,s=0) and (c=y,s=1): layout [nz][ny][2*dpx], box = whole storage rows of the tile's rows
+        for (int set = 0; set < 2; ++set)
+            for (int fam = 0; fam < 2; ++fam) {
+                const PsiSet &ps = which ? (fam ? g->lpsiH[set] : g->lpsiE[set]) : (fam ? g->psiH[set] : g->psiE[set]);
+                const float *xa[2] = { ps.p[2][0], ps.p[1][1] };
+                for (int a = 0; a < 2; ++a)
+                    ok &= encode3d(&H[13 + set * 4 + fam * 2 + a], xa[a], 2 * G.dpx, G.ny, G.nz, 2 * G.dpx,
+                                   (long long)2 * G.dpx * G.ny, 2 * G.dpx, ROWS);
+            }
+    }
     if (!ok) return fdtd_fail(FDTD_ECUDA, "cuTensorMapEncodeTiled failed");
-    cudaError_t e = cudaMemcpyAsync(F->d_maps[which], H, sizeof(CUtensorMap) * 13, cudaMemcpyHostToDevice, st);
+    cudaError_t e = cudaMemcpyAsync(F->d_maps[which], H, sizeof(CUtensorMap) * 21, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaEventRecord(F->maps_done, st);
     if (e != cudaSuccess) { (void)cudaGetLastError(); return fdtd_fail(FDTD_ECUDA, std::string("tensor map upload: ") + cudaGetErrorString(e)); }
     F->maps_key[which][0] = volA; F->maps_key[which][1] = ie;
