@@ -127,7 +127,8 @@ __device__ __forceinline__ float cpml1(float b, float a, float km, float p, floa
 __device__ __forceinline__ int slab_pos(int p, int n, int w) { return p < 0 || p >= n ? -1 : (p < w ? p : (p >= n - w ? p - (n - 2 * w) : -1)); }
 
 // additive source contribution to component `comp` at cell (i,j,k) during this step
-__device__ __noinline__ float source_at(const StepParams &P, int n, int comp, int i, int j, int k)
+template <class PT>
+__device__ __noinline__ float source_at(const PT &P, int n, int comp, int i, int j, int k)
 {
     float acc = 0.f;
     for (int s = 0; s < P.n_src; ++s) {
@@ -167,7 +168,8 @@ __device__ __noinline__ void detect_cell(const StepParams &P, int n, int comp, f
 __device__ __forceinline__ float f4get(const float4 &v, int q) { return q == 0 ? v.x : (q == 1 ? v.y : (q == 2 ? v.z : v.w)); }
 
 // adds the sources of component `comp` to the float4 of cells (i..i+3, j, k); rare planes only
-__device__ __noinline__ float4 add_sources4(const StepParams &P, int n, int comp, float4 v, int i, int j, int k)
+template <class PT>
+__device__ __noinline__ float4 add_sources4(const PT &P, int n, int comp, float4 v, int i, int j, int k)
 {
     v.x += source_at(P, n, comp, i + 0, j, k);
     v.y += source_at(P, n, comp, i + 1, j, k);
@@ -559,6 +561,218 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
 }
 
 // ================================================================================================
+// The inverse step kernel (B3 + B4): on the interior box I
+//   H  = H' - srcH + S curl+(E')                 (E' at index hi comes from the record, injected before the launch)
+//   q  = curl-(H)                                (H at index lo-1 is the recorded pre-step H, injected likewise)
+//   g += S sum_c lamE'_c q_c   on the gradient box;      E = E' - srcE - S ie q
+// Reads primal volume (n+1)&1 and cotangent volume n&1 (lamE' as the adjoint step left it), writes primal
+// volume n&1.  Same tiling as k_step with the halo on the minus side: thread column 0 / row 0 recompute H on
+// the cells left of / below the tile; cells outside I keep their (recorded or stale) values.
+// Stage slots: 0-2 E', 3-5 H', 6 inv_eps, 7-9 lamE'.
+// ================================================================================================
+struct InvParams {
+    Dims G;
+    const CUtensorMap *maps;       // primal table: [set][6], [12] inv_eps
+    const CUtensorMap *lmaps;      // lamE' components of cotangent volume `set`: [set][3]
+    const Segment *segs;
+    const int *seg_begin;          // [n_cta + 1]
+    float *buf[2];                 // primal ping-pong volumes
+    float *grad;                   // dL/d inv_eps, accumulated
+    const int *step;
+    int nst, stage;
+    int n_src;
+    int sEl, sEh, sHl, sHh;
+    SourceDev src[MAX_SRC];
+};
+
+__device__ __forceinline__ float4 sel4(bool m0, bool m1, bool m2, bool m3, float4 a, float4 b)
+{
+    return make_float4(m0 ? a.x : b.x, m1 ? a.y : b.y, m2 ? a.z : b.z, m3 ? a.w : b.w);
+}
+__device__ __forceinline__ void st_masked(float *p, float4 v, bool all, bool m0, bool m1, bool m2, bool m3)
+{
+    if (all) { stg4(p, v); return; }
+    if (m0) p[0] = v.x;
+    if (m1) p[1] = v.y;
+    if (m2) p[2] = v.z;
+    if (m3) p[3] = v.w;
+}
+
+template <class C>
+__global__ void __launch_bounds__(C::THREADS, 1) k_inverse(const __grid_constant__ InvParams P)
+{
+    extern __shared__ __align__(1024) uint8_t smem[];
+    const Dims &G = P.G;
+    const uint32_t stage_base = smem_u32(smem);
+    const uint32_t ring_base = stage_base + (uint32_t)P.nst * P.stage;
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + (size_t)P.nst * P.stage + C::RING_BYTES);
+    uint64_t *empty = full + MAX_ST;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n = *P.step;
+    const int rd = (n + 1) & 1, wv = n & 1;
+    const int nst = P.nst;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < nst; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], C::NCW); }
+        fence_mbar_init();
+    }
+    __syncthreads();
+    const int seg_lo = P.seg_begin[blockIdx.x], seg_hi = P.seg_begin[blockIdx.x + 1];
+
+    // ============================================================================== producer
+    if (warp == C::NCW) {
+        if (lane != 0) return;
+        const CUtensorMap *M = P.maps + rd * 6, *Mie = P.maps + 12, *ML = P.lmaps + wv * 3;
+        int s = 0, use = 0;
+        for (int sg = seg_lo; sg < seg_hi; ++sg) {
+            const Segment S = P.segs[sg];
+            const int x = S.i0 - 4, y = S.j0 - 1;
+            for (int kk = S.k0 - 1; kk <= S.k1; ++kk) {
+                if (use > 0) mbar_wait(&empty[s], (use - 1) & 1);
+                uint64_t *fb = &full[s];
+                uint8_t *st = smem + (size_t)s * P.stage;
+                const bool first = kk == S.k0 - 1, last = kk == S.k1;
+                mbar_expect_tx(fb, (last ? 2u : (first ? 6u : 10u)) * C::BOX_BYTES);
+                tma_load_3d(st, M, x, y, kk, fb);
+                tma_load_3d(st + C::SLOT, M + 1, x, y, kk, fb);
+                if (!last) {
+                    tma_load_3d(st + 2 * C::SLOT, M + 2, x, y, kk, fb);
+                    for (int c = 0; c < 3; ++c) tma_load_3d(st + (3 + c) * C::SLOT, M + 3 + c, x, y, kk, fb);
+                    if (!first) {
+                        tma_load_3d(st + 6 * C::SLOT, Mie, x, y, kk, fb);
+                        for (int c = 0; c < 3; ++c) tma_load_3d(st + (7 + c) * C::SLOT, ML + c, x, y, kk, fb);
+                    }
+                }
+                if (++s == nst) { s = 0; ++use; }
+            }
+        }
+        return;
+    }
+
+    // ============================================================================== consumers
+    const int tx0 = (warp % C::PCX) * 8 + (lane & 7), ty0 = (warp / C::PCX) * 4 + (lane >> 3);
+    const bool dup = tx0 >= C::CW || ty0 >= C::RW;
+    const int tx = min(tx0, C::CW - 1), ty = min(ty0, C::RW - 1);
+    const bool inner = !dup && tx >= 1 && ty >= 1;                 // column 0 / row 0 are the halo threads
+    const uint32_t o_own = (ty * C::PW + 4 * tx) * 4;
+    const uint32_t r_own = (ty * C::RP + 4 * tx) * 4;
+    float *dst = P.buf[wv];
+    const float S = G.S;
+    const long long nc = G.nc;
+    const int plane = G.ny * G.nx;
+
+    int st_i = 0, pv_i = 0;
+    uint32_t st_ph = 0, st_off = 0, pv_off = 0;
+    for (int sg = seg_lo; sg < seg_hi; ++sg) {
+        const Segment Sg = P.segs[sg];
+        const int i = Sg.i0 - 4 + 4 * tx, j = Sg.j0 - 1 + ty;
+        const bool iny = j >= G.lo[1] && j < G.hi[1];
+        const bool m0 = iny && i + 0 >= G.lo[0] && i + 0 < G.hi[0], m1 = iny && i + 1 >= G.lo[0] && i + 1 < G.hi[0];
+        const bool m2 = iny && i + 2 >= G.lo[0] && i + 2 < G.hi[0], m3 = iny && i + 3 >= G.lo[0] && i + 3 < G.hi[0];
+        const bool mall = m0 && m1 && m2 && m3, many = m0 || m1 || m2 || m3;
+        const bool gy = j >= G.glo[1] && j < G.ghi[1];
+        const bool g0 = gy && i + 0 >= G.glo[0] && i + 0 < G.ghi[0], g1 = gy && i + 1 >= G.glo[0] && i + 1 < G.ghi[0];
+        const bool g2 = gy && i + 2 >= G.glo[0] && i + 2 < G.ghi[0], g3 = gy && i + 3 >= G.glo[0] && i + 3 < G.ghi[0];
+        const bool gall = g0 && g1 && g2 && g3, gany = g0 || g1 || g2 || g3;
+        const bool own_ok = inner && many;
+        const int own_xy = j * G.nx + i;
+        float4 cHx = splat(0.f), cHy = cHx;      // H_x, H_y of plane kk-1 at my cells
+
+        // the first plane's stage becomes the held one
+        mbar_wait(&full[st_i], st_ph);
+        pv_i = st_i; pv_off = st_off;
+        st_off += P.stage;
+        if (++st_i == nst) { st_i = 0; st_off = 0; st_ph ^= 1; }
+
+        for (int kk = Sg.k0 - 1; kk < Sg.k1; ++kk) {
+            const bool prolog = kk == Sg.k0 - 1;
+            const bool inz = kk >= G.lo[2] && kk < G.hi[2];
+            mbar_wait(&full[st_i], st_ph);                          // plane kk+1 (E'_x, E'_y at my cells)
+            const uint32_t sp = stage_base + pv_off + o_own;        // plane kk
+            const uint32_t so = stage_base + st_off + o_own;
+            // ------------------------------------------------------------ H of plane kk
+            const float4 Ex = lds4(sp), Ey = lds4(sp + C::SLOT), Ez = lds4(sp + 2 * C::SLOT);
+            const float4 Ex_py = lds4(sp + C::ROWB), Ez_py = lds4(sp + 2 * C::SLOT + C::ROWB);
+            const float Ey_px = lds1(sp + C::SLOT + 16), Ez_px = lds1(sp + 2 * C::SLOT + 16);
+            const float4 Ex_pz = lds4(so), Ey_pz = lds4(so + C::SLOT);
+            const float4 Hpx = lds4(sp + 3 * C::SLOT), Hpy = lds4(sp + 4 * C::SLOT), Hpz = lds4(sp + 5 * C::SLOT);
+            const float4 Dy_z = Ez_py - Ez, Dy_x = Ex_py - Ex;
+            const float4 Dx_y = dplus_x(Ey, Ey_px), Dx_z = dplus_x(Ez, Ez_px);
+            const float4 Dz_x = Ex_pz - Ex, Dz_y = Ey_pz - Ey;
+            float4 Hx = fma4(S, Dy_z - Dz_y, Hpx), Hy = fma4(S, Dz_x - Dx_z, Hpy), Hz = fma4(S, Dx_y - Dy_x, Hpz);
+            if (kk >= P.sHl && kk < P.sHh) {
+                Hx = Hx - add_sources4(P, n, 3, splat(0.f), i, j, kk);
+                Hy = Hy - add_sources4(P, n, 4, splat(0.f), i, j, kk);
+                Hz = Hz - add_sources4(P, n, 5, splat(0.f), i, j, kk);
+            }
+            // outside I the volume's own value stands (the recorded pre-step H at index lo-1)
+            Hx = sel4(m0 && inz, m1 && inz, m2 && inz, m3 && inz, Hx, Hpx);
+            Hy = sel4(m0 && inz, m1 && inz, m2 && inz, m3 && inz, Hy, Hpy);
+            Hz = sel4(m0 && inz, m1 && inz, m2 && inz, m3 && inz, Hz, Hpz);
+            if (prolog) {
+                cHx = Hx; cHy = Hy;
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty[pv_i]);
+                pv_i = st_i; pv_off = st_off;
+                st_off += P.stage;
+                if (++st_i == nst) { st_i = 0; st_off = 0; st_ph ^= 1; }
+                continue;
+            }
+            const uint32_t rg = ring_base + (uint32_t)(kk & 1) * (C::RING_SLOT * 4) + r_own;
+            sts4(rg, Hx); sts4(rg + C::RING_ARR * 4, Hy); sts4(rg + 2 * C::RING_ARR * 4, Hz);
+            const int off = kk * plane + own_xy;
+            float4 gv = splat(0.f);
+            const bool gz = kk >= G.glo[2] && kk < G.ghi[2];
+            if (own_ok && gz && gall) gv = ld4(P.grad + off);
+            named_bar_sync(1, C::NCW * 32);
+            // ------------------------------------------------------------ q, gradient, E of plane kk
+            if (own_ok) {
+                const float4 Hx_my = lds4(rg - C::RP * 4), Hz_my = lds4(rg + 2 * C::RING_ARR * 4 - C::RP * 4);
+                const float Hy_mx = lds1(rg + C::RING_ARR * 4 - 4), Hz_mx = lds1(rg + 2 * C::RING_ARR * 4 - 4);
+                const float4 By_z = Hz - Hz_my, By_x = Hx - Hx_my;
+                const float4 Bx_y = dminus_x(Hy, Hy_mx), Bx_z = dminus_x(Hz, Hz_mx);
+                const float4 Bz_x = Hx - cHx, Bz_y = Hy - cHy;
+                const float4 qx = By_z - Bz_y, qy = Bz_x - Bx_z, qz = Bx_y - By_x;
+                const float4 sie = S * lds4(sp + 6 * C::SLOT);
+                const float4 lx = lds4(sp + 7 * C::SLOT), ly = lds4(sp + 8 * C::SLOT), lz = lds4(sp + 9 * C::SLOT);
+                float4 E2x = Ex - sie * qx, E2y = Ey - sie * qy, E2z = Ez - sie * qz;
+                if (kk >= P.sEl && kk < P.sEh) {
+                    E2x = E2x - add_sources4(P, n, 0, splat(0.f), i, j, kk);
+                    E2y = E2y - add_sources4(P, n, 1, splat(0.f), i, j, kk);
+                    E2z = E2z - add_sources4(P, n, 2, splat(0.f), i, j, kk);
+                }
+                float *o = dst + off;
+                st_masked(o, E2x, mall, m0, m1, m2, m3);
+                st_masked(o + nc, E2y, mall, m0, m1, m2, m3);
+                st_masked(o + 2 * nc, E2z, mall, m0, m1, m2, m3);
+                st_masked(o + 3 * nc, Hx, mall, m0, m1, m2, m3);
+                st_masked(o + 4 * nc, Hy, mall, m0, m1, m2, m3);
+                st_masked(o + 5 * nc, Hz, mall, m0, m1, m2, m3);
+                if (gz && gany) {
+                    const float4 ga = S * fma4(lx, qx, fma4(ly, qy, lz * qz));
+                    if (gall) stg4(P.grad + off, gv + ga);
+                    else {
+                        float *gp = P.grad + off;
+                        if (g0) gp[0] += ga.x;
+                        if (g1) gp[1] += ga.y;
+                        if (g2) gp[2] += ga.z;
+                        if (g3) gp[3] += ga.w;
+                    }
+                }
+            }
+            cHx = Hx; cHy = Hy;
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[pv_i]);
+            pv_i = st_i; pv_off = st_off;
+            st_off += P.stage;
+            if (++st_i == nst) { st_i = 0; st_off = 0; st_ph ^= 1; }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[pv_i]);      // the stage of plane k1
+    }
+}
+
+// ================================================================================================
 // host side
 // ================================================================================================
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
@@ -599,7 +813,17 @@ struct TileImpl {
     void (*launch_fwd)(const StepParams &, int n_cta, size_t smem, cudaStream_t);
     void (*launch_adj)(const StepParams &, int n_cta, size_t smem, cudaStream_t);
     cudaError_t (*set_smem)(size_t);
+    void (*launch_inv)(const InvParams &, int n_cta, size_t smem, cudaStream_t);
+    cudaError_t (*set_smem_inv)(size_t);
 };
+template <class C> void launch_inv_impl(const InvParams &P, int n_cta, size_t smem, cudaStream_t st)
+{
+    k_inverse<C><<<n_cta, C::THREADS, smem, st>>>(P);
+}
+template <class C> cudaError_t set_smem_inv_impl(size_t smem)
+{
+    return cudaFuncSetAttribute(k_inverse<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+}
 template <class C> void launch_fwd_impl(const StepParams &P, int n_cta, size_t smem, cudaStream_t st)
 {
     k_step<C, false><<<n_cta, C::THREADS, smem, st>>>(P);
@@ -615,7 +839,8 @@ template <class C> cudaError_t set_smem_impl(size_t smem)
     return e;
 }
 #define TILE(TX4, TY) { 4 * TX4, TY, Cfg<TX4, TY>::THREADS, Cfg<TX4, TY>::NCW, Cfg<TX4, TY>::STAGE, Cfg<TX4, TY>::RING_BYTES, \
-                        launch_fwd_impl<Cfg<TX4, TY>>, launch_adj_impl<Cfg<TX4, TY>>, set_smem_impl<Cfg<TX4, TY>> }
+                        launch_fwd_impl<Cfg<TX4, TY>>, launch_adj_impl<Cfg<TX4, TY>>, set_smem_impl<Cfg<TX4, TY>>, \
+                        launch_inv_impl<Cfg<TX4, TY>>, set_smem_inv_impl<Cfg<TX4, TY>> }
 const TileImpl kTiles[] = {
     TILE(2, 3), TILE(4, 3), TILE(8, 7), TILE(16, 7), TILE(16, 15), TILE(25, 7), TILE(25, 11),
     TILE(32, 7), TILE(32, 11), TILE(50, 7), TILE(50, 11), TILE(62, 7),
@@ -629,15 +854,23 @@ struct FusedState {
     int TX = 0, TY = 0, nst = 0, n_cta = 0, n_rot = 1;
     size_t smem = 0;
     StepParams sp{};
+    // inverse step kernel: its own tile shape and segment table (interior box only)
+    const TileImpl *itile = nullptr;
+    int inst = 0, in_cta = 0;
+    size_t ismem = 0;
+    InvParams ip{};
+    Segment *d_isegs = nullptr;
+    int *d_iseg_begin = nullptr;
     float *bufB = nullptr;                 // second primal field buffer
     float *lamB = nullptr;                 // second cotangent buffer
     // tensor-map tables: [0] primal (fields / bufB), [1] cotangents (lam / lamB); entry set*6 + c, [12] = inv_eps
-    CUtensorMap *d_maps[2] = { nullptr, nullptr };
-    CUtensorMap *h_maps[2] = { nullptr, nullptr };   // pinned staging
+    // [2]: the inverse kernel's table (its own box shape): [set][6] primal, [12] inv_eps, [13 + set*3 + c] lamE'
+    CUtensorMap *d_maps[3] = { nullptr, nullptr, nullptr };
+    CUtensorMap *h_maps[3] = { nullptr, nullptr, nullptr };   // pinned staging
     cudaEvent_t maps_done = nullptr;
     Segment *d_segs = nullptr;
     int *d_seg_begin = nullptr;
-    const float *maps_key[2][2] = { { nullptr, nullptr }, { nullptr, nullptr } };   // volume A / inv_eps the maps were built for
+    const float *maps_key[3][2] = { { nullptr, nullptr }, { nullptr, nullptr }, { nullptr, nullptr } };   // volume A / inv_eps the maps were built for
 };
 
 namespace {
@@ -738,7 +971,7 @@ int fused_setup(fdtd_grid *g)
     int rc;
     if ((rc = g->alloc((void **)&F->bufB, (size_t)G.nc * 6 * sizeof(float)))) return rc;
     if ((rc = g->alloc_psi(g->psiE[1])) || (rc = g->alloc_psi(g->psiH[1]))) return rc;
-    for (int q = 0; q < 2; ++q) {
+    for (int q = 0; q < 3; ++q) {
         if ((rc = g->alloc((void **)&F->d_maps[q], sizeof(CUtensorMap) * 21))) return rc;
         if (cudaMallocHost((void **)&F->h_maps[q], sizeof(CUtensorMap) * 21) != cudaSuccess) {
             (void)cudaGetLastError();
@@ -772,6 +1005,66 @@ int fused_setup(fdtd_grid *g)
         return fdtd_fail(FDTD_ECUDA, "upload of the segment table failed");
     }
 
+    // ---- inverse step kernel: tile shape (10 boxes per stage), segments over the interior box ----------------------
+    {
+        const TileImpl *ib = nullptr;
+        double ib_score = -1;
+        int ib_nst = 0;
+        int iTX = 0, iTY = 0;
+        if (const char *e = getenv("FDTD_ITILE")) sscanf(e, "%d,%d", &iTX, &iTY);
+        const int ny_i = G.hi[1] - G.lo[1], nz_i = G.hi[2] - G.lo[2];
+        for (int q = 0; q < kNumTiles; ++q) {
+            const TileImpl &t = kTiles[q];
+            if (iTX && (t.TX != iTX || t.TY != iTY)) continue;
+            const int nst = std::min(MAX_ST, (smem_cap - t.ring_bytes - tail_bytes - 1024) / (t.stage / 7 * 10));
+            if (nst < 3) continue;
+            const long long ntx = (G.nx + t.TX - 1) / t.TX, nty = (ny_i + t.TY - 1) / t.TY;
+            const double eff = ((double)(G.hi[0] - G.lo[0]) / 4 * ny_i) / ((double)ntx * nty * t.ncw * 32);
+            const double fill = std::min(1.0, (double)ntx * nty * nz_i / (8.0 * n_sm));
+            const double warps = std::min(1.0, t.ncw / 10.0);
+            const double score = eff * fill * warps;
+            if (score > ib_score) { ib_score = score; ib = &t; ib_nst = nst; }
+        }
+        if (ib && ny_i > 0 && nz_i > 0) {
+            // tiles start at row lo_y (their first halo row is lo_y - 1); x starts at 0 (float4 alignment)
+            const int ntx = (G.nx + ib->TX - 1) / ib->TX, nty = (ny_i + ib->TY - 1) / ib->TY;
+            const long long itotal = (long long)ntx * nty * nz_i;
+            const int in_cta = (int)std::min<long long>(n_sm, std::max<long long>(1, itotal / 6));
+            std::vector<Segment> isegs;
+            std::vector<int> ibeg(in_cta + 1, 0);
+            for (int cta = 0; cta < in_cta; ++cta) {
+                ibeg[cta] = (int)isegs.size();
+                long long a = itotal * cta / in_cta;
+                const long long b = itotal * (cta + 1) / in_cta;
+                while (a < b) {
+                    const long long tile = a / nz_i;
+                    const int k = (int)(a % nz_i);
+                    const int len = (int)std::min<long long>(b - a, nz_i - k);
+                    Segment sgm{};
+                    sgm.i0 = (int)(tile / nty) * ib->TX; sgm.j0 = G.lo[1] + (int)(tile % nty) * ib->TY;
+                    sgm.k0 = G.lo[2] + k; sgm.k1 = sgm.k0 + len;
+                    isegs.push_back(sgm);
+                    a += len;
+                }
+            }
+            ibeg[in_cta] = (int)isegs.size();
+            if ((rc = g->alloc((void **)&F->d_isegs, isegs.size() * sizeof(Segment)))) return rc;
+            if ((rc = g->alloc((void **)&F->d_iseg_begin, ibeg.size() * sizeof(int)))) return rc;
+            if (cudaMemcpy(F->d_isegs, isegs.data(), isegs.size() * sizeof(Segment), cudaMemcpyHostToDevice) != cudaSuccess ||
+                cudaMemcpy(F->d_iseg_begin, ibeg.data(), ibeg.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess) {
+                (void)cudaGetLastError();
+                return fdtd_fail(FDTD_ECUDA, "upload of the inverse segment table failed");
+            }
+            F->itile = ib; F->inst = ib_nst; F->in_cta = in_cta;
+            const int istage = ib->stage / 7 * 10;
+            F->ismem = (size_t)ib_nst * istage + ib->ring_bytes + tail_bytes;
+            InvParams &I = F->ip;
+            I.G = G; I.segs = F->d_isegs; I.seg_begin = F->d_iseg_begin; I.step = g->d_step;
+            I.nst = ib_nst; I.stage = istage;
+            if (ib->set_smem_inv(F->ismem) != cudaSuccess) { (void)cudaGetLastError(); F->itile = nullptr; }
+        }
+    }
+
     // ---- kernel parameters that do not depend on the call -----------------------------------------------------------
     StepParams &P = F->sp;
     P.G = G; P.T = g->T; P.segs = F->d_segs; P.seg_begin = F->d_seg_begin;
@@ -795,7 +1088,7 @@ int fused_setup(fdtd_grid *g)
 void fused_teardown(fdtd_grid *g)
 {
     if (g->fused) {
-        for (int q = 0; q < 2; ++q) if (g->fused->h_maps[q]) cudaFreeHost(g->fused->h_maps[q]);
+        for (int q = 0; q < 3; ++q) if (g->fused->h_maps[q]) cudaFreeHost(g->fused->h_maps[q]);
         if (g->fused->maps_done) cudaEventDestroy(g->fused->maps_done);
     }
     delete g->fused;
@@ -840,6 +1133,33 @@ int build_maps(fdtd_grid *g, int which, float *volA, float *volB, const float *i
     return FDTD_OK;
 }
 
+// the inverse kernel's table: primal volumes, inv_eps and the lamE' components of both cotangent volumes
+int build_inv_maps(fdtd_grid *g, float *volA, float *volB, const float *ie, float *lamA, float *lamB, cudaStream_t st)
+{
+    FusedState *F = g->fused;
+    const Dims &G = g->G;
+    if (F->maps_key[2][0] == volA && F->maps_key[2][1] == ie) return FDTD_OK;
+    const int PW = F->itile->TX + 8, ROWS = F->itile->TY + 2;
+    if (cudaEventSynchronize(F->maps_done) != cudaSuccess) { (void)cudaGetLastError(); }
+    CUtensorMap *H = F->h_maps[2];
+    bool ok = true;
+    float *bufs[2] = { volA, volB }, *lams[2] = { lamA, lamB };
+    const long long pl = (long long)G.nx * G.ny;
+    for (int set = 0; set < 2; ++set) {
+        for (int c = 0; c < 6; ++c)
+            ok &= encode3d(&H[set * 6 + c], bufs[set] + (long long)c * G.nc, G.nx, G.ny, G.nz, G.nx, pl, PW, ROWS);
+        for (int c = 0; c < 3; ++c)
+            ok &= encode3d(&H[13 + set * 3 + c], lams[set] + (long long)c * G.nc, G.nx, G.ny, G.nz, G.nx, pl, PW, ROWS);
+    }
+    ok &= encode3d(&H[12], ie, G.nx, G.ny, G.nz, G.nx, pl, PW, ROWS);
+    if (!ok) return fdtd_fail(FDTD_ECUDA, "cuTensorMapEncodeTiled failed");
+    cudaError_t e = cudaMemcpyAsync(F->d_maps[2], H, sizeof(CUtensorMap) * 19, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaEventRecord(F->maps_done, st);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return fdtd_fail(FDTD_ECUDA, std::string("tensor map upload: ") + cudaGetErrorString(e)); }
+    F->maps_key[2][0] = volA; F->maps_key[2][1] = ie;
+    return FDTD_OK;
+}
+
 }  // namespace
 
 // run_steps lives in fdtd_api.cu; reached through small trampolines
@@ -868,7 +1188,7 @@ void enqueue_fwd(void *vctx, cudaStream_t cs)
 }
 
 struct BwdCtx {
-    fdtd_grid *g; StepParams P; float *fields; const float *ie; float *grad; float *lamA; float *lamB;
+    fdtd_grid *g; StepParams P; InvParams I; bool fused_inv; float *bufB; float *fields; const float *ie; float *grad; float *lamA; float *lamB;
     const std::vector<SourceDev> *S; const std::vector<DetectorDev> *D; int total_freq;
 };
 // reverse step n: B1 (detector cotangents into the volume about to be read), B2+B5 (fused adjoint step),
@@ -884,6 +1204,12 @@ void enqueue_bwd(void *vctx, cudaStream_t cs)
           if (dt.phasor) launch_detector_adjoint_pp(G, c->lamA, c->lamB, dt, g->d_cs, c->total_freq, g->d_step, cs); }
     { ProfScope p(g, fdtd_grid::PC_FUSED_BWD, cs);
       F->tile->launch_adj(c->P, F->n_cta, F->smem, cs); }
+    if (c->fused_inv) {
+        if (G.d > 0) { ProfScope p(g, fdtd_grid::PC_INJECT, cs); launch_inject_pp(G, g->R, c->fields, c->bufB, g->rec, g->d_step, cs); }
+        { ProfScope p(g, fdtd_grid::PC_INV_E_GRAD, cs); F->itile->launch_inv(c->I, F->in_cta, F->ismem, cs); }
+        { ProfScope p(g, fdtd_grid::PC_OTHER, cs); launch_advance(g->d_step, -1, cs); }
+        return;
+    }
     { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
       for (const SourceDev &s : *c->S) if (s.comp >= 3) launch_add_source(G, c->fields, s, g->d_step, -1.f, cs); }
     if (G.d > 0) { ProfScope p(g, fdtd_grid::PC_INJECT, cs); launch_inject(G, g->R, c->fields, g->rec, g->d_step, cs); }
@@ -954,7 +1280,26 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
         cudaError_t e = cudaMemcpyAsync(F->lamB, g->lam, vol6, cudaMemcpyDeviceToDevice, st);
         if (e != cudaSuccess) { (void)cudaGetLastError(); return fdtd_fail(FDTD_ECUDA, cudaGetErrorString(e)); }
     }
-    BwdCtx ctx{ g, F->sp, fields, inv_eps, dL_dinv_eps, g->lam, F->lamB, &S, &D, total_freq };
+    const bool fused_inv = F->itile != nullptr && (int)S.size() <= MAX_SRC && !getenv("FDTD_GENERIC_INVERSE");
+    BwdCtx ctx{ g, F->sp, F->ip, fused_inv, F->bufB, fields, inv_eps, dL_dinv_eps, g->lam, F->lamB, &S, &D, total_freq };
+    if (fused_inv) {
+        // reverse step n reads primal volume (n+1)&1 and writes n&1: state n_steps must sit in volume n_steps&1
+        if ((rc = build_inv_maps(g, fields, F->bufB, inv_eps, g->lam, F->lamB, st))) return rc;
+        if (n_steps & 1) {
+            cudaError_t e = cudaMemcpyAsync(F->bufB, fields, vol6, cudaMemcpyDeviceToDevice, st);
+            if (e != cudaSuccess) { (void)cudaGetLastError(); return fdtd_fail(FDTD_ECUDA, cudaGetErrorString(e)); }
+        }
+        InvParams &I = ctx.I;
+        I.maps = F->d_maps[2]; I.lmaps = F->d_maps[2] + 13;
+        I.buf[0] = fields; I.buf[1] = F->bufB; I.grad = dL_dinv_eps;
+        I.n_src = (int)S.size();
+        I.sEl = I.sHl = 1 << 30; I.sEh = I.sHh = -1;
+        for (size_t q = 0; q < S.size(); ++q) {
+            I.src[q] = S[q];
+            if (S[q].comp < 3) { I.sEl = std::min(I.sEl, S[q].lo[2]); I.sEh = std::max(I.sEh, S[q].hi[2]); }
+            else { I.sHl = std::min(I.sHl, S[q].lo[2]); I.sHh = std::max(I.sHh, S[q].hi[2]); }
+        }
+    }
     StepParams &P = ctx.P;
     P.maps = F->d_maps[1];
     P.buf[0] = g->lam; P.buf[1] = F->lamB;
@@ -965,8 +1310,9 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     P.cs = g->d_cs;
     int n_adj = 0;
     for (const DetectorDev &dt : D) if (dt.phasor) ++n_adj;
-    std::string key("fb");
+    std::string key(fused_inv ? "fB" : "fb");
     key.append((const char *)&P, sizeof(P));
+    if (fused_inv) key.append((const char *)&ctx.I, sizeof(ctx.I));
     key.append((const char *)&fields, sizeof(fields));
     key.append((const char *)&dL_dinv_eps, sizeof(dL_dinv_eps));
     if (!S.empty()) key.append((const char *)S.data(), S.size() * sizeof(SourceDev));
