@@ -43,11 +43,12 @@ def algorithmic_bytes(w, grad_cells: int, recording: bool, has_mu: bool = False)
     mu = 4 if has_mu else 0
     rec = 4 * face if recording else 0                      # 2 comps x 2 sides per face cell, fp32
     return {
-        # fused: 6 R + 6 W fields + ie (+im); psi R/W: 4 arrays (2E+2H) per slab cell per axis; recorder W
-        "fused_forward_step": cells * (52 + mu) + slab * 32 + rec,
-        # fused backward: adjoint 6R+6W+ie over the grid, inverse 6R+6W over I, g R/W on the grad box,
-        # adjoint psi R/W on slabs, recorder R
-        "fused_backward_step": cells * (52 + mu) + inter * 48 + grad_cells * 8 + slab * 32 + 4 * face,
+        # fused step: 6 R + 6 W fields + ie (+im); psi R/W: 4 arrays (2E+2H) per slab cell per axis
+        "fused_forward_step": cells * (52 + mu) + slab * 32,
+        # fused adjoint step (B2+B5): 6 R + 6 W cotangents + ie over the grid, adjoint psi R/W on slabs
+        "fused_adjoint_step": cells * 52 + slab * 32,
+        # fused inverse step (B3+B4) over I: R E',H' (6), ie, lamE' (3), W E,H (6); g R/W on the grad box
+        "fused_inverse_step": inter * 64 + grad_cells * 8,
         "update_E": cells * 40 + slab * 16,
         "update_H": cells * (36 + mu) + slab * 16,
         "adjoint_H": cells * (36 + mu) + slab * 16,

@@ -178,7 +178,7 @@ FDTD_API int fdtd_get_info(const fdtd_grid *grid, fdtd_grid_info *info);
  * recorded on the launch stream.  fdtd_get_profile synchronises those events and returns, per kernel
  * class, the number of launches and their summed device time since profiling was enabled (or since
  * the last fdtd_get_profile, which resets the counters). */
-#define FDTD_PROF_CLASSES 12
+#define FDTD_PROF_CLASSES 16
 typedef struct {
     int32_t n_classes;                          /* number of valid entries below                       */
     int32_t reserved;

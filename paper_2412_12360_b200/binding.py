@@ -48,7 +48,7 @@ class fdtd_grid_info(C.Structure):
                 ("record_floats_per_step", C.c_int64), ("reserved", C.c_int64 * 4)]
 
 
-FDTD_PROF_CLASSES = 12
+FDTD_PROF_CLASSES = 16
 
 
 class fdtd_profile(C.Structure):

@@ -299,7 +299,7 @@ extern "C" int fdtd_get_profile(fdtd_grid *g, fdtd_profile *out)
 {
     if (!g || !out) return fail(FDTD_EINVAL, "fdtd_get_profile: NULL argument");
     static const char *names[fdtd_grid::PC_COUNT] = { "update_E", "update_H", "adjoint_H", "inverse_H", "inverse_E_grad",
-        "adjoint_E", "fused_forward_step", "fused_backward_step", "record_faces", "inject_faces", "source_detector", "other" };
+        "adjoint_E", "fused_forward_step", "fused_adjoint_step", "fused_inverse_step", "record_faces", "inject_faces", "source_detector", "other" };
     for (auto &sp : g->prof_spans) {
         cudaError_t e = cudaEventSynchronize(sp.b);
         float ms = 0.f;

@@ -53,7 +53,7 @@ struct fdtd_grid {
 
     // per-kernel profiling (fdtd_set_profiling)
     enum ProfClass { PC_UPDATE_E, PC_UPDATE_H, PC_ADJ_H, PC_INV_H, PC_INV_E_GRAD, PC_ADJ_E,
-                     PC_FUSED_FWD, PC_FUSED_BWD, PC_RECORD, PC_INJECT, PC_SRC_DET, PC_OTHER, PC_COUNT };
+                     PC_FUSED_FWD, PC_FUSED_BWD, PC_FUSED_INV, PC_RECORD, PC_INJECT, PC_SRC_DET, PC_OTHER, PC_COUNT };
     bool profiling = false;
     struct ProfSpan { int cls; cudaEvent_t a, b; };
     std::vector<ProfSpan> prof_spans;

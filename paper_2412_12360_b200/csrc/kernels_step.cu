@@ -1206,7 +1206,7 @@ void enqueue_bwd(void *vctx, cudaStream_t cs)
       F->tile->launch_adj(c->P, F->n_cta, F->smem, cs); }
     if (c->fused_inv) {
         if (G.d > 0) { ProfScope p(g, fdtd_grid::PC_INJECT, cs); launch_inject_pp(G, g->R, c->fields, c->bufB, g->rec, g->d_step, cs); }
-        { ProfScope p(g, fdtd_grid::PC_INV_E_GRAD, cs); F->itile->launch_inv(c->I, F->in_cta, F->ismem, cs); }
+        { ProfScope p(g, fdtd_grid::PC_FUSED_INV, cs); F->itile->launch_inv(c->I, F->in_cta, F->ismem, cs); }
         { ProfScope p(g, fdtd_grid::PC_OTHER, cs); launch_advance(g->d_step, -1, cs); }
         return;
     }
