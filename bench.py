@@ -34,12 +34,14 @@ UNIT = "Mcells/s"
 # ------------------------------------------------------------------------------------------------
 # algorithmic bytes: what one launch of each kernel class must move
 # ------------------------------------------------------------------------------------------------
-def algorithmic_bytes(w, grad_cells: int, recording: bool, has_mu: bool = False) -> dict:
+def algorithmic_bytes(w, grad_cells: int, recording: bool, has_mu: bool = False, rbox=None) -> dict:
+    """rbox = (bx, by, bz): the reconstruction box (record=2: the design box; default: the interior I)."""
     nx, ny, nz, d = w.nx, w.ny, w.nz, w.pml_cells
     cells = nx * ny * nz
-    inter = (nx - 2 * d) * (ny - 2 * d) * (nz - 2 * d)
+    bx, by, bz = rbox if rbox else (nx - 2 * d, ny - 2 * d, nz - 2 * d)
+    inter = bx * by * bz
     slab = 2 * d * (ny * nz + nx * nz + nx * ny)            # slab cells summed over the three axes
-    face = 4 * ((ny - 2 * d) * (nz - 2 * d) + (nx - 2 * d) * (nz - 2 * d) + (nx - 2 * d) * (ny - 2 * d)) if d else 0
+    face = 4 * (by * bz + bx * bz + bx * by) if d else 0
     mu = 4 if has_mu else 0
     rec = 4 * face if recording else 0                      # 2 comps x 2 sides per face cell, fp32
     return {
@@ -136,6 +138,7 @@ def cpu_oracle_rate(w, sample_steps: int):
 def workload_config(w, extra=None):
     cfg = {"workload": f"{w.name}: {w.nx}x{w.ny}x{w.nz} fp32 Yee grid, {w.pml_cells}-cell CPML, {w.n_steps} time steps, "
                        f"forward(record)+reversible backward, grad box = design region",
+           "recorder": "faces of the design box (record=2)",
            "time_steps": w.n_steps, "cells": w.cells,
            "l2": "inputs larger than L2 (working set > 0.5 GB vs 126 MB L2); no flush needed"}
     if extra:
@@ -178,6 +181,8 @@ def main():
     ap.add_argument("--ref-sample-steps", type=int, default=12)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--record", type=int, default=2, choices=[1, 2],
+                    help="1: record the PML/interior interface, reconstruct the interior; 2: record the faces of the design box, reconstruct that box only")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -211,7 +216,7 @@ def main():
     T = w.n_steps
     path = {"auto": B.FDTD_PATH_AUTO, "generic": B.FDTD_PATH_GENERIC, "fused": B.FDTD_PATH_FUSED}[args.path]
     kw = w.grid_kwargs()
-    kw.update(max_steps=T, record=True, grad_lo=w.design_lo, grad_hi=w.design_hi, path=path)
+    kw.update(max_steps=T, record=args.record, grad_lo=w.design_lo, grad_hi=w.design_hi, path=path)
     grid = B.Grid(**kw)
     kw_f = dict(kw); kw_f.update(record=False)
     grid_f = B.Grid(**kw_f)                                   # forward-only grid (no recorder)
@@ -292,7 +297,8 @@ def main():
         peak, peak_src = float(json.loads(peaks_file.read_text())["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     else:
         peak, peak_src = 6650.0, "fallback (B200_PROFILING.md)"
-    alg = algorithmic_bytes(w, grad_cells, recording=True)
+    rbox = tuple(dhi[a] - dlo[a] for a in range(3)) if args.record == 2 else None
+    alg = algorithmic_bytes(w, grad_cells, recording=True, rbox=rbox)
     kernels = {}
     for name, (n, ms) in prof.items():
         if name in alg and n:

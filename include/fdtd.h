@@ -84,7 +84,9 @@ typedef struct {
     float   pml_alpha_m;       /* grading order of alpha                           (default 1)      */
     float   pml_eps_bg;        /* background relative permittivity used in sigma~_max (default 1)   */
     int32_t max_steps;         /* upper bound of n_steps; sizes the recorder when record != 0       */
-    int32_t record;            /* 0: forward only; 1: record the PML/interior interface every step  */
+    int32_t record;            /* 0: forward only; 1: record the PML/interior interface every step; */
+                               /* 2: record the faces of the gradient box instead (pml_cells > 0):  */
+                               /*    fdtd_backward then reconstructs the fields on that box only    */
     int32_t grad_lo[3];        /* half-open (i,j,k) box on which dL_dinv_eps is wanted;             */
     int32_t grad_hi[3];        /*   all zero => the whole interior I.  Always clipped to I.         */
     int32_t path;              /* FDTD_PATH_*                                                       */

@@ -194,7 +194,7 @@ def make_desc(nx, ny, nz, courant, periodic=False, pml_cells=0, pml_m=0.0, pml_s
     d.periodic, d.pml_cells = int(bool(periodic)), pml_cells
     d.pml_m, d.pml_sigma_scale, d.pml_kappa_max = pml_m, pml_sigma_scale, pml_kappa_max
     d.pml_alpha_max, d.pml_alpha_m, d.pml_eps_bg = pml_alpha_max, pml_alpha_m, pml_eps_bg
-    d.max_steps, d.record, d.path = max_steps, int(bool(record)), path
+    d.max_steps, d.record, d.path = max_steps, int(record), path
     if grad_lo is not None:
         d.grad_lo[:] = list(grad_lo)
         d.grad_hi[:] = list(grad_hi)

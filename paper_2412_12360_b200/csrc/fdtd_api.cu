@@ -157,7 +157,7 @@ extern "C" int fdtd_create_grid(const fdtd_grid_desc *desc, fdtd_grid **out)
     if (desc->pml_cells > 0 && 2 * desc->pml_cells + 2 > mn)
         return fail(FDTD_EINVAL, "need 2*pml_cells + 2 <= min(nx,ny,nz)");
     if (desc->max_steps < 0) return fail(FDTD_EINVAL, "max_steps must be >= 0");
-    if (desc->record != 0 && desc->record != 1) return fail(FDTD_EINVAL, "record must be 0 or 1");
+    if (desc->record < 0 || desc->record > 2) return fail(FDTD_EINVAL, "record must be 0, 1 or 2");
     if (desc->path < 0 || desc->path > 2) return fail(FDTD_EINVAL, "unknown path");
     for (int q = 0; q < 7; ++q) if (desc->reserved[q]) return fail(FDTD_EINVAL, "reserved fields must be zero");
     if (desc->pml_m < 0 || desc->pml_sigma_scale < 0 || desc->pml_kappa_max < 0 || desc->pml_alpha_max < 0 ||
@@ -188,6 +188,14 @@ extern "C" int fdtd_create_grid(const fdtd_grid_desc *desc, fdtd_grid **out)
             }
             G.glo[a] = std::max(desc->grad_lo[a], G.lo[a]);
             G.ghi[a] = std::max(G.glo[a], std::min(desc->grad_hi[a], G.hi[a]));
+        }
+    }
+    // record == 2 (NEXT N1, design-box recorder): the reconstruction box shrinks from the interior I to the
+    // gradient box -- the faces recorded, the inverse step and the reconstructed fields all follow G.lo / G.hi
+    if (desc->record == 2 && G.d > 0) {
+        for (int a = 0; a < 3; ++a) {
+            if (G.ghi[a] <= G.glo[a]) { delete g; return fail(FDTD_EINVAL, "record=2 needs a non-empty gradient box inside the interior"); }
+            G.lo[a] = G.glo[a]; G.hi[a] = G.ghi[a];
         }
     }
     make_rec_layout(G, g->R);

@@ -1012,22 +1012,23 @@ int fused_setup(fdtd_grid *g)
         int ib_nst = 0;
         int iTX = 0, iTY = 0;
         if (const char *e = getenv("FDTD_ITILE")) sscanf(e, "%d,%d", &iTX, &iTY);
-        const int ny_i = G.hi[1] - G.lo[1], nz_i = G.hi[2] - G.lo[2];
+        const int x0 = G.lo[0] / 4 * 4;                       // first tile column (float4 aligned)
+        const int nx_i = G.hi[0] - x0, ny_i = G.hi[1] - G.lo[1], nz_i = G.hi[2] - G.lo[2];
         for (int q = 0; q < kNumTiles; ++q) {
             const TileImpl &t = kTiles[q];
             if (iTX && (t.TX != iTX || t.TY != iTY)) continue;
             const int nst = std::min(MAX_ST, (smem_cap - t.ring_bytes - tail_bytes - 1024) / (t.stage / 7 * 10));
             if (nst < 3) continue;
-            const long long ntx = (G.nx + t.TX - 1) / t.TX, nty = (ny_i + t.TY - 1) / t.TY;
+            const long long ntx = (nx_i + t.TX - 1) / t.TX, nty = (ny_i + t.TY - 1) / t.TY;
             const double eff = ((double)(G.hi[0] - G.lo[0]) / 4 * ny_i) / ((double)ntx * nty * t.ncw * 32);
             const double fill = std::min(1.0, (double)ntx * nty * nz_i / (8.0 * n_sm));
             const double warps = std::min(1.0, t.ncw / 10.0);
             const double score = eff * fill * warps;
             if (score > ib_score) { ib_score = score; ib = &t; ib_nst = nst; }
         }
-        if (ib && ny_i > 0 && nz_i > 0) {
-            // tiles start at row lo_y (their first halo row is lo_y - 1); x starts at 0 (float4 alignment)
-            const int ntx = (G.nx + ib->TX - 1) / ib->TX, nty = (ny_i + ib->TY - 1) / ib->TY;
+        if (ib && nx_i > 0 && ny_i > 0 && nz_i > 0) {
+            // tiles start at row lo_y (their first halo row is lo_y - 1) and at column x0
+            const int ntx = (nx_i + ib->TX - 1) / ib->TX, nty = (ny_i + ib->TY - 1) / ib->TY;
             const long long itotal = (long long)ntx * nty * nz_i;
             const int in_cta = (int)std::min<long long>(n_sm, std::max<long long>(1, itotal / 6));
             std::vector<Segment> isegs;
@@ -1041,7 +1042,7 @@ int fused_setup(fdtd_grid *g)
                     const int k = (int)(a % nz_i);
                     const int len = (int)std::min<long long>(b - a, nz_i - k);
                     Segment sgm{};
-                    sgm.i0 = (int)(tile / nty) * ib->TX; sgm.j0 = G.lo[1] + (int)(tile % nty) * ib->TY;
+                    sgm.i0 = x0 + (int)(tile / nty) * ib->TX; sgm.j0 = G.lo[1] + (int)(tile % nty) * ib->TY;
                     sgm.k0 = G.lo[2] + k; sgm.k1 = sgm.k0 + len;
                     isegs.push_back(sgm);
                     a += len;
