@@ -138,7 +138,6 @@ def cpu_oracle_rate(w, sample_steps: int):
 def workload_config(w, extra=None):
     cfg = {"workload": f"{w.name}: {w.nx}x{w.ny}x{w.nz} fp32 Yee grid, {w.pml_cells}-cell CPML, {w.n_steps} time steps, "
                        f"forward(record)+reversible backward, grad box = design region",
-           "recorder": "faces of the design box (record=2)",
            "time_steps": w.n_steps, "cells": w.cells,
            "l2": "inputs larger than L2 (working set > 0.5 GB vs 126 MB L2); no flush needed"}
     if extra:
@@ -368,7 +367,9 @@ def main():
                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                "config": workload_config(w, {"path": {1: "generic", 2: "fused"}[info.path],
                                              "tile": [info.tile_x, info.tile_y, info.tile_z],
-                                             "parallelism": f"independent problems x{world}"}),
+                                             "parallelism": f"independent problems x{world}",
+                                             "recorder": "faces of the design box, record=2 (SURVEY 8(f) N1)" if args.record == 2
+                                             else "PML/interior interface, record=1"}),
                "fwd": {"value": fwd_value, "unit": UNIT, "ms_per_pass": ms_fwd / max(1, args.steps),
                        "what": "forward only, record=0, same workload"},
                "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
