@@ -197,6 +197,7 @@ def main():
     import torch.distributed as dist
     from paper_2412_12360_b200 import binding as B
     from paper_2412_12360_b200 import workloads as wl
+    from paper_2412_12360_b200 import sharding
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
@@ -211,7 +212,7 @@ def main():
         torch.cuda.synchronize()
 
     # ---- workload: C3 (seed + rank: every rank an independent problem) -----------------------------
-    w = wl.c3(n=args.grid, n_steps=args.time_steps, seed=3 + rank)
+    w = wl.c3(n=args.grid, n_steps=args.time_steps, seed=sharding.problem_seed(3, rank))
     T = w.n_steps
     path = {"auto": B.FDTD_PATH_AUTO, "generic": B.FDTD_PATH_GENERIC, "fused": B.FDTD_PATH_FUSED}[args.path]
     kw = w.grid_kwargs()
@@ -257,10 +258,7 @@ def main():
             fn()
         e1.record(stream)
         barrier()
-        ms = torch.tensor([e0.elapsed_time(e1)], device=dev)
-        if world > 1:
-            dist.all_reduce(ms, op=dist.ReduceOp.MAX)
-        return float(ms.item())
+        return sharding.max_over_ranks(e0.elapsed_time(e1), device=dev)
 
     with torch.cuda.stream(stream):
         for _ in range(args.warmup):
@@ -288,8 +286,8 @@ def main():
         B.fdtd_set_profiling(grid.h, False)
 
     cells_steps = w.cells * T
-    value = world * cells_steps * args.steps / (ms_total * 1e-3) / 1e6
-    fwd_value = world * cells_steps * max(1, args.steps) / (ms_fwd * 1e-3) / 1e6
+    value = sharding.whole_job_rate(cells_steps, args.steps, ms_total, world)
+    fwd_value = sharding.whole_job_rate(cells_steps, max(1, args.steps), ms_fwd, world)
 
     peaks_file = ROOT / "MEASURED_PEAKS.json"
     if peaks_file.exists():

@@ -152,7 +152,7 @@ def c2(n: int = 64, d: int = 10, n_steps: int = 1000) -> Workload:
     return Workload("C2", n, n, n, n_steps, _inv(eps), [src], [det], pml_cells=d, eps=eps)
 
 
-def c3(n: int = 200, d: int = 12, n_steps: int = 2000, seed: int = 3) -> Workload:
+def c3(n: int = 200, d: int = 12, n_steps: int = 2000, seed: int = 3, source_k: int | None = None) -> Workload:
     """configs[2] (the graded config): silica-like cladding, random design block, Gaussian-profile
     Ey source plane, Ey DFT plane; loss = phasor power; gradient wrt rho via inv_eps."""
     s = n / 200.0
@@ -163,6 +163,8 @@ def c3(n: int = 200, d: int = 12, n_steps: int = 2000, seed: int = 3) -> Workloa
     rho = np.random.default_rng(seed).random((z1 - z0, x1 - x0, x1 - x0), dtype=np.float32)
     eps[z0:z1, x0:x1, x0:x1] = eps_bg + np.float32(12.25 - 2.085) * rho
     ks, kd = max(d + 1, int(round(20 * s))), min(n - d - 2, int(round(170 * s)))
+    if source_k is not None:          # truncated full-size parity runs: the source plane next to the design box
+        ks = source_k
     lo, hi = (d, d, ks), (n - d, n - d, ks + 1)
     ctr = (n - 1) / 2.0
     prof = gaussian_profile(lo, hi, (ctr, ctr), 20.0 * s)

@@ -255,6 +255,28 @@ def test_gradient_box_recorder(B):
             assert np.all(gpu["grad"][mask] == 0)
 
 
+def test_c3_full_size_truncated_in_the_bench_configuration(B):
+    """configs[2] at its full 200^3 size in the launch configuration bench.py times (fused kernels, tile and
+    grid chosen by the library, grad box = design region, record=2 and record=1), truncated to 40 time steps
+    so that the fp64 oracle finishes in seconds.  The source plane sits just below the design box (k = 66)
+    and the loss is sum E^2 at the final state, so fields, gradient and cotangents are non-trivial."""
+    w = wl.c3(n_steps=40, source_k=66)
+    w.loss = "final_E2"
+    ref = run_oracle(w)
+    lo, hi = w.design_lo, w.design_hi
+    box = (slice(lo[2], hi[2]), slice(lo[1], hi[1]), slice(lo[0], hi[0]))
+    assert np.max(np.abs(ref["grad"][box])) > 0
+    scale = np.max(np.abs(ref["fields"]))
+    for mode in (2, 1):
+        gpu = run_gpu(B, w, B.FDTD_PATH_FUSED, grad_box=(lo, hi), record_mode=mode)
+        assert gpu["info"].path == B.FDTD_PATH_FUSED
+        eE, eH = relerr(gpu["fields"][:3], ref["fields"][:3]), relerr(gpu["fields"][3:], ref["fields"][3:])
+        eG, eL = relerr(gpu["grad"][box], ref["grad"][box]), relerr(gpu["lam0"], ref["lam0"])
+        e0 = max(float(np.max(np.abs(gpu["state0"][c][box] - ref["state0"][c][box]))) for c in range(6)) / scale
+        print("C3 full size, record", mode, "tile", gpu["info"].tile_x, gpu["info"].tile_y, eE, eH, eG, eL, e0)
+        assert eE <= TOL_FIELD and eH <= TOL_FIELD and eG <= TOL_GRAD and eL <= TOL_GRAD and e0 <= 1e-4
+
+
 def test_error_codes_on_device(B):
     import torch
     w = wl.c3_mini(nx=24, ny=20, nz=20, d=4, n_steps=5)
