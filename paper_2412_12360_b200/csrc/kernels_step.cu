@@ -40,6 +40,13 @@ using namespace fdtd;
 namespace {
 
 constexpr int MAX_SRC = 4, MAX_DET = 4;
+// timing experiments (wrong results): build with -DFDTD_TIMING_EXPERIMENTS and set FDTD_DBG to a bit mask:
+// 1 no global stores, 2 no phase B, 4 no barrier, 8 load pipeline only, 16 no CPML, 32/64/128 no x/y/z slab code
+#ifdef FDTD_TIMING_EXPERIMENTS
+#define DBG(bit) (P.dbg & (bit))
+#else
+#define DBG(bit) 0
+#endif
 constexpr int MAX_ST = 8;               // upper bound of pipeline stages
 
 struct StepParams {
@@ -56,6 +63,7 @@ struct StepParams {
     int nst;                       // pipeline stages
     int stage;                     // bytes of one stage: 7 boxes + 4 x-slab state boxes
     int xs_bytes, xs_pitch;        // x-slab state box [ROWS][2*dpx]: exact bytes (TMA transaction) and 128-byte aligned pitch
+    unsigned long long *dbg_t;     // timing experiments only (FDTD_DBG_TIMES): per-CTA start / end globaltimer
     int dbg;                       // timing experiments only (FDTD_DBG): 1 no global stores, 2 no phase B, 4 no barrier
     int n_src, n_det, total_freq;
     int sEl, sEh, sHl, sHh, dEl, dEh, dHl, dHh;   // k ranges of the planes that hold E/H sources and E/H detectors
@@ -216,6 +224,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
     if (threadIdx.x == 0) {
         for (int s = 0; s < nst; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], C::NCW); }
         fence_mbar_init();
+        if (P.dbg_t) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); P.dbg_t[2 * blockIdx.x] = t; }
     }
     __syncthreads();
 
@@ -278,7 +287,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
     const float S = G.S;
     const long long nc = G.nc;
     const int plane = G.ny * G.nx;
-    const bool pml = G.d > 0 && !(P.dbg & 16);
+    const bool pml = G.d > 0 && !DBG(16);
     const bool has_mu = !ADJ && P.im != nullptr;
     const int pz = plane, py = 2 * G.d * G.nx, px = G.ny * 2 * G.dpx;      // plane pitch of the z / y / x state arrays
 
@@ -297,10 +306,10 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
         const bool own_ok = inner && ing;
         const int own_xy = j * G.nx + i;
         // slab-compact coordinates of my cells and (adjoint) of my -x / -y neighbours; -1: not in a slab
-        const int sx = (pml && ing && !(P.dbg & 32)) ? slab_pos(i, G.nx, G.dpx) : -1;
-        const int sy = (pml && ing && !(P.dbg & 64)) ? slab_pos(j, G.ny, G.d) : -1;
-        const int sxm = (ADJ && pml && ing && !(P.dbg & 32)) ? slab_pos(i - 1, G.nx, G.dpx) : -1;
-        const int sym = (ADJ && pml && ing && !(P.dbg & 64)) ? slab_pos(j - 1, G.ny, G.d) : -1;
+        const int sx = (pml && ing && !DBG(32)) ? slab_pos(i, G.nx, G.dpx) : -1;
+        const int sy = (pml && ing && !DBG(64)) ? slab_pos(j, G.ny, G.d) : -1;
+        const int sxm = (ADJ && pml && ing && !DBG(32)) ? slab_pos(i - 1, G.nx, G.dpx) : -1;
+        const int sym = (ADJ && pml && ing && !DBG(64)) ? slab_pos(j - 1, G.ny, G.d) : -1;
         const bool slab_xy = __any_sync(0xffffffffu, (sx & sy & sxm & sym) >= 0);   // this warp runs x / y slab code
         const int oy = sy * G.nx + i, oym = sym * G.nx + i;                          // + k * py
         const int ox = j * (2 * G.dpx) + sx, oxm = j * (2 * G.dpx) + sxm;           // + k * px
@@ -309,7 +318,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
 
         // ---------------------------------------------------------------- one plane (phase A of kk, phase B of kk-1)
         auto plane_step = [&](const int kk, const bool doB) {
-            const int zs = (pml && !(P.dbg & 128)) ? slab_pos(kk, G.nz, G.d) : -1;
+            const int zs = (pml && !DBG(128)) ? slab_pos(kk, G.nz, G.d) : -1;
             mbar_wait(&full[st_i], st_ph);
             const uint32_t so = stage_base + st_off + o_own;
             const uint32_t sp = stage_base + pv_off + o_own;       // the stage of plane kk-1 is still held
@@ -318,7 +327,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
             const float4 fx_my = lds4(so - C::ROWB), fz_my = lds4(so + 2 * C::SLOT - C::ROWB);
             const float fy_mx = lds1(so + C::SLOT - 4), fz_mx = lds1(so + 2 * C::SLOT - 4);
 
-            const bool wr = own_ok && kk < k1 && !(P.dbg & 1);                 // I own these cells: write the result and the phase-A states
+            const bool wr = own_ok && kk < k1 && !DBG(1);                 // I own these cells: write the result and the phase-A states
             const int off = kk * plane + own_xy;
             const int oz = zs * pz + own_xy;
             const uint32_t rgA = ring_base + (uint32_t)(kk & 1) * (C::RING_SLOT * 4) + r_own;
@@ -465,7 +474,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
             sts4(rgA, Yx); sts4(rgA + C::RING_ARR * 4, Yz); sts4(rgA + 2 * C::RING_ARR * 4, Xy);
             if (ADJ) sts4(rgA + 3 * C::RING_ARR * 4, Xz);
             // ---------------------------------------------------------------- phase B: H-type update of plane kk-1
-            if (own_ok && doB && !(P.dbg & 2)) {
+            if (own_ok && doB && !DBG(2)) {
                 const int km1 = kk - 1;
                 const uint32_t rgB = ring_base + (uint32_t)(km1 & 1) * (C::RING_SLOT * 4) + r_own;
                 const float4 Yx_py = lds4(rgB + C::RP * 4), Yz_py = lds4(rgB + (C::RING_ARR + C::RP) * 4);
@@ -477,7 +486,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                 float4 Dz_y = Zy - (ADJ ? cZy : oXy), Dz_x = Zx - (ADJ ? cZx : oYx);
                 float4 Dx_z = dplus_x(oXz, Xz_px), Dx_y = dplus_x(oXy, Xy_px);
                 const int offm = off - plane;
-                const int zsm = (!ADJ && pml && !(P.dbg & 128)) ? slab_pos(km1, G.nz, G.d) : -1;
+                const int zsm = (!ADJ && pml && !DBG(128)) ? slab_pos(km1, G.nz, G.d) : -1;
                 if (!ADJ && (slab_xy || zsm >= 0)) {
                     if (zsm >= 0) {
                         const float b = __ldg(P.T.b[FB][2] + km1), a = __ldg(P.T.a[FB][2] + km1), km = __ldg(P.T.ik[FB][2] + km1) - 1.f;
@@ -528,7 +537,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
             pv_i = st_i; pv_off = st_off;
             st_off += P.stage;
             if (++st_i == nst) { st_i = 0; st_off = 0; st_ph ^= 1; }
-            if (!(P.dbg & 4)) named_bar_sync(1, C::NCW * 32);      // ring slot (kk-1)&1 may be overwritten in the next iteration
+            if (!DBG(4)) named_bar_sync(1, C::NCW * 32);      // ring slot (kk-1)&1 may be overwritten in the next iteration
         };
 
         // ---------------------------------------------------------------- prologue: plane k0-1 (F only) becomes the held stage
@@ -558,6 +567,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[pv_i]);      // the stage of plane k1
     }
+    if (P.dbg_t && threadIdx.x == 0) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); P.dbg_t[2 * blockIdx.x + 1] = t; }
 }
 
 // ================================================================================================
@@ -868,40 +878,61 @@ struct FusedState {
     CUtensorMap *d_maps[3] = { nullptr, nullptr, nullptr };
     CUtensorMap *h_maps[3] = { nullptr, nullptr, nullptr };   // pinned staging
     cudaEvent_t maps_done = nullptr;
-    Segment *d_segs = nullptr;
-    int *d_seg_begin = nullptr;
+    Segment *d_segs[2] = { nullptr, nullptr };      // work tables of the forward / adjoint step kernel
+    int *d_seg_begin[2] = { nullptr, nullptr };
+    size_t seg_cap = 0;
+    unsigned long long *d_cta_t = nullptr;          // per-CTA start / end timestamps (calibration)
+    double calibrated_us[2] = { 0.0, 0.0 };
     const float *maps_key[3][2] = { { nullptr, nullptr }, { nullptr, nullptr }, { nullptr, nullptr } };   // volume A / inv_eps the maps were built for
 };
 
 namespace {
 
-// Work sequence: (tile [y fastest], plane); it is cut into n_cta runs of equal estimated cost.  A plane of a tile
-// costs 1, plus wy if the tile has rows in a y slab, plus wz if the plane is in a z slab (their CPML states are
-// read by every thread of the tile).  With y fastest, CTAs that hold y-adjacent tiles march through the same
-// planes at about the same time, so halo rows hit L2.
-void make_segments(const Dims &G, int TX, int TY, int n_cta, double wy, double wz, std::vector<Segment> &segs,
-                   std::vector<int> &seg_begin)
+// Work sequence: (tile [y fastest], plane); it is cut into n_cta runs of equal estimated cost.  The cost model
+// (a plane of a tile costs 1, plus wy if the tile has rows in a y slab, plus wz if the plane is in a z slab:
+// their CPML states are read by every thread of the tile) is only the starting point: calibrate() measures
+// the CTAs and moves the cuts.  With y fastest, CTAs that hold y-adjacent tiles march through the same planes
+// at about the same time, so halo rows hit L2.
+std::vector<double> model_cost(const Dims &G, int TX, int TY, double wy, double wz)
 {
     const int ntx = (G.nx + TX - 1) / TX, nty = (G.ny + TY - 1) / TY;
     const long long n_tiles = (long long)ntx * nty;
-    const long long total = n_tiles * G.nz;
-    std::vector<double> pre(total + 1, 0.0);
+    std::vector<double> w((size_t)n_tiles * G.nz);
     for (long long t = 0; t < n_tiles; ++t) {
         const int j0 = (int)(t % nty) * TY;
         const bool ys = G.d > 0 && (j0 <= G.d || j0 + TY >= G.ny - G.d);
         for (int k = 0; k < G.nz; ++k) {
             const bool zs = G.d > 0 && (k <= G.d || k >= G.nz - G.d - 1);
-            pre[t * G.nz + k + 1] = pre[t * G.nz + k] + 1.0 + (ys ? wy : 0.0) + (zs ? wz : 0.0);
+            w[t * G.nz + k] = 1.0 + (ys ? wy : 0.0) + (zs ? wz : 0.0);
         }
     }
-    segs.clear();
-    seg_begin.assign(n_cta + 1, 0);
+    return w;
+}
+
+// n_cta + 1 cut positions that split the sequence into runs of equal summed cost (every run non-empty)
+std::vector<long long> equal_cost_cuts(const std::vector<double> &w, int n_cta)
+{
+    const long long total = (long long)w.size();
+    std::vector<double> pre(total + 1, 0.0);
+    for (long long q = 0; q < total; ++q) pre[q + 1] = pre[q] + w[q];
     std::vector<long long> cut(n_cta + 1, 0);
     for (int c = 1; c < n_cta; ++c) {
         const double target = pre[total] * c / n_cta;
-        cut[c] = std::max<long long>(cut[c - 1], std::lower_bound(pre.begin(), pre.end(), target) - pre.begin());
+        long long q = std::lower_bound(pre.begin(), pre.end(), target) - pre.begin();
+        q = std::max(q, cut[c - 1] + 1);
+        cut[c] = std::min(q, total - (n_cta - c));
     }
     cut[n_cta] = total;
+    return cut;
+}
+
+void segments_from_cuts(const Dims &G, int TX, int TY, const std::vector<long long> &cut, std::vector<Segment> &segs,
+                        std::vector<int> &seg_begin)
+{
+    const int nty = (G.ny + TY - 1) / TY;
+    const int n_cta = (int)cut.size() - 1;
+    segs.clear();
+    seg_begin.assign(n_cta + 1, 0);
     for (int cta = 0; cta < n_cta; ++cta) {
         seg_begin[cta] = (int)segs.size();
         long long a = cut[cta];
@@ -920,6 +951,8 @@ void make_segments(const Dims &G, int TX, int TY, int n_cta, double wy, double w
 }
 
 }  // namespace
+
+static int calibrate(fdtd_grid *g);
 
 int fused_setup(fdtd_grid *g)
 {
@@ -988,22 +1021,26 @@ int fused_setup(fdtd_grid *g)
     const long long total = (long long)ntx * nty * G.nz;
     int n_cta = (int)std::min<long long>(n_sm, std::max<long long>(1, total / 6));
     if (const char *e = getenv("FDTD_NCTA")) n_cta = std::max(1, atoi(e));
-    double wy = 1.5, wz = 1.0;                   // relative extra cost of y-slab tiles / z-slab planes (measured on C3)
+    double wy = 1.0, wz = 0.8;                   // starting point of the cost model (measured on C3); see calibrate()
     if (const char *e = getenv("FDTD_WY")) wy = atof(e);
     if (const char *e = getenv("FDTD_WZ")) wz = atof(e);
     const int n_rot = 1;
     F->n_cta = n_cta; F->n_rot = n_rot;
     std::vector<Segment> all;
     std::vector<int> begins;
-    make_segments(G, F->TX, F->TY, n_cta, wy, wz, all, begins);
-    const size_t stride = all.size();
-    if ((rc = g->alloc((void **)&F->d_segs, all.size() * sizeof(Segment)))) return rc;
-    if ((rc = g->alloc((void **)&F->d_seg_begin, begins.size() * sizeof(int)))) return rc;
-    if (cudaMemcpy(F->d_segs, all.data(), all.size() * sizeof(Segment), cudaMemcpyHostToDevice) != cudaSuccess ||
-        cudaMemcpy(F->d_seg_begin, begins.data(), begins.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess) {
-        (void)cudaGetLastError();
-        return fdtd_fail(FDTD_ECUDA, "upload of the segment table failed");
+    segments_from_cuts(G, F->TX, F->TY, equal_cost_cuts(model_cost(G, F->TX, F->TY, wy, wz), n_cta), all, begins);
+    F->seg_cap = (size_t)n_cta + (size_t)ntx * nty + 8;        // a run adds at most one segment per tile boundary
+    const size_t stride = F->seg_cap;
+    for (int q = 0; q < 2; ++q) {
+        if ((rc = g->alloc((void **)&F->d_segs[q], F->seg_cap * sizeof(Segment)))) return rc;
+        if ((rc = g->alloc((void **)&F->d_seg_begin[q], begins.size() * sizeof(int)))) return rc;
+        if (cudaMemcpy(F->d_segs[q], all.data(), all.size() * sizeof(Segment), cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(F->d_seg_begin[q], begins.data(), begins.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess) {
+            (void)cudaGetLastError();
+            return fdtd_fail(FDTD_ECUDA, "upload of the segment table failed");
+        }
     }
+    if ((rc = g->alloc((void **)&F->d_cta_t, 2 * (size_t)n_cta * sizeof(unsigned long long)))) return rc;
 
     // ---- inverse step kernel: tile shape (10 boxes per stage), segments over the interior box ----------------------
     {
@@ -1068,12 +1105,13 @@ int fused_setup(fdtd_grid *g)
 
     // ---- kernel parameters that do not depend on the call -----------------------------------------------------------
     StepParams &P = F->sp;
-    P.G = G; P.T = g->T; P.segs = F->d_segs; P.seg_begin = F->d_seg_begin;
+    P.G = G; P.T = g->T; P.segs = F->d_segs[0]; P.seg_begin = F->d_seg_begin[0];
     P.n_rot = n_rot; P.seg_stride = (int)stride; P.n_cta = n_cta;
     P.step = g->d_step;
     P.nst = F->nst;
     P.stage = stage_bytes; P.xs_bytes = xs_bytes; P.xs_pitch = xs_pitch;
     P.dbg = getenv("FDTD_DBG") ? atoi(getenv("FDTD_DBG")) : 0;
+    P.dbg_t = nullptr;
     if (best->set_smem(F->smem) != cudaSuccess) {
         (void)cudaGetLastError();
         g->fused_why_not = "cannot reserve shared memory";
@@ -1083,6 +1121,7 @@ int fused_setup(fdtd_grid *g)
     g->fused_backward_ready = true;
     g->tile_x = F->TX; g->tile_y = F->TY;
     g->tile_z = (int)std::min<long long>(G.nz, total / n_cta);
+    if (!getenv("FDTD_NO_CALIBRATE") && total >= 8LL * n_cta) return calibrate(g);
     return FDTD_OK;
 }
 
@@ -1162,6 +1201,84 @@ int build_inv_maps(fdtd_grid *g, float *volA, float *volB, const float *ie, floa
 }
 
 }  // namespace
+
+// Measures the CTAs of both step kernels on scratch volumes and moves the cuts of the work sequence until the
+// CTAs finish together: a CTA's measured time is spread over its positions in proportion to the current cost
+// estimate, the new cuts equalise that.  Static cost weights cannot capture how the per-plane cost of a slab
+// tile depends on what the neighbouring SMs are doing; five rounds of two launches per kernel do (~3 ms at C3).
+static int calibrate(fdtd_grid *g)
+{
+    FusedState *F = g->fused;
+    const Dims &G = g->G;
+    const size_t vol = (size_t)G.nc * sizeof(float);
+    float *T = nullptr, *tie = nullptr;
+    if (cudaMalloc((void **)&T, 6 * vol) != cudaSuccess || cudaMalloc((void **)&tie, vol) != cudaSuccess) {
+        (void)cudaGetLastError();
+        if (T) cudaFree(T);
+        return FDTD_OK;                                   // no room for the scratch volumes: keep the model's cuts
+    }
+    auto done = [&](int rc) { cudaFree(T); cudaFree(tie); F->maps_key[0][0] = nullptr; return rc; };
+    cudaMemset(T, 0, 6 * vol); cudaMemset(F->bufB, 0, 6 * vol); cudaMemset(tie, 0, vol);
+    cudaMemset(g->d_step, 0, sizeof(int));
+    int rc;
+    for (int q = 0; q < 2; ++q)
+        if ((rc = g->zero_psi(g->psiE[q], 0)) || (rc = g->zero_psi(g->psiH[q], 0))) return done(rc);
+    if ((rc = build_maps(g, 0, T, F->bufB, tie, 0))) return done(rc);
+    StepParams P = F->sp;
+    P.maps = F->d_maps[0];
+    P.buf[0] = T; P.buf[1] = F->bufB;
+    P.ie = tie; P.im = nullptr;
+    for (int q = 0; q < 2; ++q) { P.psiE[q] = g->psiE[q]; P.psiH[q] = g->psiH[q]; }
+    P.n_src = P.n_det = P.total_freq = 0;
+    P.sEl = P.sHl = P.dEl = P.dHl = 1 << 30; P.sEh = P.sHh = P.dEh = P.dHh = -1;
+    P.cs = nullptr;
+    P.dbg_t = F->d_cta_t;
+    const int n_cta = F->n_cta;
+    std::vector<unsigned long long> t(2 * (size_t)n_cta);
+    std::vector<Segment> segs;
+    std::vector<int> begins;
+    for (int mode = 0; mode < 2; ++mode) {
+        std::vector<double> w = model_cost(G, F->TX, F->TY, 1.0, 0.8);
+        std::vector<long long> cut = equal_cost_cuts(w, n_cta), best_cut = cut;
+        double best = 1e30;
+        P.segs = F->d_segs[mode]; P.seg_begin = F->d_seg_begin[mode];
+        for (int it = 0; it < 6; ++it) {
+            segments_from_cuts(G, F->TX, F->TY, cut, segs, begins);
+            if (segs.size() > F->seg_cap) break;
+            if (cudaMemcpy(F->d_segs[mode], segs.data(), segs.size() * sizeof(Segment), cudaMemcpyHostToDevice) != cudaSuccess ||
+                cudaMemcpy(F->d_seg_begin[mode], begins.data(), begins.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess)
+                return done(fdtd_fail(FDTD_ECUDA, "calibration: upload of the segment table failed"));
+            for (int rep = 0; rep < 2; ++rep) {
+                if (mode) F->tile->launch_adj(P, n_cta, F->smem, 0); else F->tile->launch_fwd(P, n_cta, F->smem, 0);
+            }
+            if (cudaDeviceSynchronize() != cudaSuccess ||
+                cudaMemcpy(t.data(), F->d_cta_t, t.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost) != cudaSuccess) {
+                cudaError_t e = cudaGetLastError();
+                return done(fdtd_fail(FDTD_ECUDA, std::string("calibration launch: ") + cudaGetErrorString(e)));
+            }
+            unsigned long long t0 = ~0ull, t1 = 0;
+            for (int c = 0; c < n_cta; ++c) { t0 = std::min(t0, t[2 * c]); t1 = std::max(t1, t[2 * c + 1]); }
+            const double span = (double)(t1 - t0) * 1e-3;
+            if (span < best) { best = span; best_cut = cut; }
+            // spread each CTA's time over its positions in proportion to the current estimate
+            for (int c = 0; c < n_cta; ++c) {
+                double sum = 0.0;
+                for (long long q = cut[c]; q < cut[c + 1]; ++q) sum += w[q];
+                const double scale = (double)(t[2 * c + 1] - t0) / sum;
+                for (long long q = cut[c]; q < cut[c + 1]; ++q) w[q] *= scale;
+            }
+            cut = equal_cost_cuts(w, n_cta);
+        }
+        segments_from_cuts(G, F->TX, F->TY, best_cut, segs, begins);
+        if (cudaMemcpy(F->d_segs[mode], segs.data(), segs.size() * sizeof(Segment), cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(F->d_seg_begin[mode], begins.data(), begins.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess)
+            return done(fdtd_fail(FDTD_ECUDA, "calibration: upload of the segment table failed"));
+        F->calibrated_us[mode] = best;
+        if (getenv("FDTD_VERBOSE")) fprintf(stderr, "fdtd: calibrated %s step kernel: %.1f us per launch\n", mode ? "adjoint" : "forward", best);
+    }
+    cudaMemset(F->bufB, 0, 6 * vol);
+    return done(FDTD_OK);
+}
 
 // run_steps lives in fdtd_api.cu; reached through small trampolines
 int fdtd_run_steps_fwd(fdtd_grid *g, const std::string &key, int n_steps, int launches_per_step, cudaStream_t st,
@@ -1303,6 +1420,7 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     }
     StepParams &P = ctx.P;
     P.maps = F->d_maps[1];
+    P.segs = F->d_segs[1]; P.seg_begin = F->d_seg_begin[1];
     P.buf[0] = g->lam; P.buf[1] = F->lamB;
     P.ie = inv_eps; P.im = nullptr;
     for (int q = 0; q < 2; ++q) { P.psiE[q] = g->lpsiE[q]; P.psiH[q] = g->lpsiH[q]; }
