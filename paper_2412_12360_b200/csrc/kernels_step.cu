@@ -832,7 +832,9 @@ template <class C> void launch_inv_impl(const InvParams &P, int n_cta, size_t sm
 }
 template <class C> cudaError_t set_smem_inv_impl(size_t smem)
 {
-    return cudaFuncSetAttribute(k_inverse<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(k_inverse<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_inverse<C>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    return e;
 }
 template <class C> void launch_fwd_impl(const StepParams &P, int n_cta, size_t smem, cudaStream_t st)
 {
@@ -846,6 +848,9 @@ template <class C> cudaError_t set_smem_impl(size_t smem)
 {
     cudaError_t e = cudaFuncSetAttribute(k_step<C, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step<C, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    // the same shared-memory carve-out for every kernel of the time loop: no L1 / shared reconfiguration between launches
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step<C, false>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step<C, true>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     return e;
 }
 #define TILE(TX4, TY) { 4 * TX4, TY, Cfg<TX4, TY>::THREADS, Cfg<TX4, TY>::NCW, Cfg<TX4, TY>::STAGE, Cfg<TX4, TY>::RING_BYTES, \

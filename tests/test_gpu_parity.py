@@ -277,6 +277,57 @@ def test_c3_full_size_truncated_in_the_bench_configuration(B):
         assert eE <= TOL_FIELD and eH <= TOL_FIELD and eG <= TOL_GRAD and eL <= TOL_GRAD and e0 <= 1e-4
 
 
+def test_c4_full_size_self_consistency(B):
+    """configs[3] at its full 800 x 800 x 600 size (384 M cells; maximum size, 6 nc > 2^31 elements) in the
+    bench launch configuration (fused kernels, record=2), truncated to 24 steps with the source plane moved next
+    to the design box.  The oracle cannot run this size in seconds, so the checks are properties that hold at
+    any size: a directional central finite difference of the loss against <dL/d inv_eps, delta>, and the
+    reconstructed state 0 (true value 0) on the design box."""
+    import torch
+    free, _ = torch.cuda.mem_get_info()
+    if free < 100e9:
+        pytest.skip("needs ~100 GB of device memory")
+    n = 24
+    w = wl.c4(n_steps=n)
+    d, lo, hi = w.pml_cells, w.design_lo, w.design_hi
+    s0 = w.sources[0]
+    w.sources[0] = wl.Source(s0.component, (d, d, lo[2] - 4), (w.nx - d, w.ny - d, lo[2] - 3), s0.waveform, s0.profile)
+    kw = w.grid_kwargs()
+    kw.update(max_steps=n, record=2, grad_lo=lo, grad_hi=hi, path=B.FDTD_PATH_FUSED)
+    g = B.Grid(**kw)
+    assert g.info().path == B.FDTD_PATH_FUSED
+    ie = torch.as_tensor(w.inv_eps).cuda()
+    box = (slice(lo[2], hi[2]), slice(lo[1], hi[1]), slice(lo[0], hi[0]))
+    f = torch.zeros((6, w.nz, w.ny, w.nx), dtype=torch.float32, device="cuda")
+
+    def loss_of(ie_t):
+        f.zero_()
+        g.forward(f, ie_t, None, w.sources, w.detectors, n)
+        return float((f[:3].double() ** 2).sum())
+
+    L0 = loss_of(ie)
+    assert np.isfinite(L0) and L0 > 0
+    fmax = float(f.abs().max())
+    dLf = torch.zeros_like(f)
+    dLf[:3] = 2.0 * f[:3]
+    grad, _ = g.backward(f, ie, None, w.sources, w.detectors, None, dLf, n)
+    torch.cuda.synchronize()
+    del dLf
+    resid = max(float(f[c][box].abs().max()) for c in range(6)) / fmax
+    gen = torch.Generator(device="cuda").manual_seed(4)
+    delta = torch.zeros_like(ie)
+    delta[box] = torch.randint(0, 2, delta[box].shape, generator=gen, device="cuda").float() * 2 - 1
+    an = float((grad.double() * delta.double()).sum())
+    h = 2e-3
+    fd = (loss_of(ie + h * delta) - loss_of(ie - h * delta)) / (2 * h)
+    g.close()
+    print("C4 full size: L", L0, "directional derivative analytic", an, "finite difference", fd, "state-0 residue", resid)
+    assert abs(fd - an) <= 2e-2 * abs(an)
+    assert resid <= 1e-4
+    grad[box] = 0
+    assert float(grad.abs().max()) == 0.0
+
+
 def test_error_codes_on_device(B):
     import torch
     w = wl.c3_mini(nx=24, ny=20, nz=20, d=4, n_steps=5)
