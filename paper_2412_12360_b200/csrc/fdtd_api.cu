@@ -3,6 +3,7 @@
 // file only owns memory, builds tables and enqueues launches (through CUDA graphs).
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -137,8 +138,8 @@ void fdtd_grid::drop_graphs()
     for (GraphCache *gc : { &fwd_graph, &bwd_graph }) {
         if (gc->done) { cudaEventSynchronize(gc->done); }
         if (gc->exec_main) cudaGraphExecDestroy(gc->exec_main);
-        if (gc->exec_tail) cudaGraphExecDestroy(gc->exec_tail);
-        gc->exec_main = gc->exec_tail = nullptr;
+        for (int q = 0; q < 2; ++q) if (gc->exec_tail[q]) { cudaGraphExecDestroy(gc->exec_tail[q]); gc->exec_tail[q] = nullptr; }
+        gc->exec_main = nullptr;
         gc->key.clear();
     }
 }
@@ -438,22 +439,24 @@ int run_steps(fdtd_grid *g, fdtd_grid::GraphCache &gc, const std::string &key, i
 {
     if (n_steps == 0) return FDTD_OK;
     if (g->profiling) {
-        for (int n = 0; n < n_steps; ++n) enqueue(st);
+        g->step_par = 0;
+        for (int n = 0; n < n_steps; ++n) { enqueue(st); g->step_par ^= 1; }
         g->kernel_launches += (long long)n_steps * launches_per_step;
         return FDTD_OK;
     }
-    const int unroll = g->graph_unroll;
-    if (gc.key != key || !gc.exec_tail) {
+    const int unroll = g->graph_unroll;                  // even: a replay of the main graph ends in the slot it began in
+    if (gc.key != key || !gc.exec_tail[1]) {
         if (gc.key.size()) CK(cudaEventSynchronize(gc.done));
         if (gc.exec_main) { cudaGraphExecDestroy(gc.exec_main); gc.exec_main = nullptr; }
-        if (gc.exec_tail) { cudaGraphExecDestroy(gc.exec_tail); gc.exec_tail = nullptr; }
+        for (int q = 0; q < 2; ++q) if (gc.exec_tail[q]) { cudaGraphExecDestroy(gc.exec_tail[q]); gc.exec_tail[q] = nullptr; }
         gc.key.clear();
-        for (int which = 0; which < 2; ++which) {
+        for (int which = 0; which < 3; ++which) {            // 0: main graph (slot 0 first), 1 / 2: one step from slot 0 / 1
             const int reps = which ? 1 : unroll;
             cudaGraph_t graph = nullptr;
             CK(cudaStreamBeginCapture(g->cap_stream, cudaStreamCaptureModeThreadLocal));
             g->prof_capturing = true;
-            for (int r = 0; r < reps; ++r) enqueue(g->cap_stream);
+            g->step_par = which == 2 ? 1 : 0;
+            for (int r = 0; r < reps; ++r) { enqueue(g->cap_stream); g->step_par ^= 1; }
             g->prof_capturing = false;
             cudaError_t e = cudaStreamEndCapture(g->cap_stream, &graph);
             if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture");
@@ -461,13 +464,13 @@ int run_steps(fdtd_grid *g, fdtd_grid::GraphCache &gc, const std::string &key, i
             e = cudaGraphInstantiate(&exec, graph, 0);
             cudaGraphDestroy(graph);
             if (e != cudaSuccess) return cuda_fail(e, "cudaGraphInstantiate");
-            (which ? gc.exec_tail : gc.exec_main) = exec;
+            (which ? gc.exec_tail[which - 1] : gc.exec_main) = exec;
         }
         gc.key = key;
     }
-    int left = n_steps;
+    int left = n_steps, par = 0;
     while (left >= unroll) { CK(cudaGraphLaunch(gc.exec_main, st)); left -= unroll; }
-    while (left > 0) { CK(cudaGraphLaunch(gc.exec_tail, st)); --left; }
+    while (left > 0) { CK(cudaGraphLaunch(gc.exec_tail[par], st)); par ^= 1; --left; }
     CK(cudaEventRecord(gc.done, st));
     g->kernel_launches += (long long)n_steps * launches_per_step;
     return FDTD_OK;
@@ -520,7 +523,7 @@ extern "C" int fdtd_forward(fdtd_grid *g, float *fields, const float *inv_eps, c
     const bool recording = g->desc.record && G.d > 0;
     g->recorded_steps = -1;
     if ((rc = upload_cs_table(g, det, n_det, total_freq, n_steps, st))) return rc;
-    CK(cudaMemsetAsync(g->d_step, 0, sizeof(int), st));
+    launch_set_step(g->d_step, 0, st);                   // step 0 reads slot 0
 
     if (g->path == FDTD_PATH_FUSED) {
         rc = fused_forward(g, fields, inv_eps, inv_mu, S, D, total_freq, n_steps, recording, st);
@@ -532,13 +535,13 @@ extern "C" int fdtd_forward(fdtd_grid *g, float *fields, const float *inv_eps, c
         rc = run_steps(g, g->fwd_graph, key, n_steps, launches, st, [&](cudaStream_t cs) {
             { ProfScope p(g, fdtd_grid::PC_UPDATE_E, cs); launch_update_E(G, g->T, fields, inv_eps, g->psiE[0], cs); }
             { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
-              for (const SourceDev &s : S) if (s.comp < 3) launch_add_source(G, fields, s, g->d_step, 1.f, cs); }
-            if (recording) { ProfScope p(g, fdtd_grid::PC_RECORD, cs); launch_record(G, g->R, fields, fields, g->rec, g->d_step, cs); }
+              for (const SourceDev &s : S) if (s.comp < 3) launch_add_source(G, fields, s, g->step_in(), 1.f, cs); }
+            if (recording) { ProfScope p(g, fdtd_grid::PC_RECORD, cs); launch_record(G, g->R, fields, fields, g->rec, g->step_in(), cs); }
             { ProfScope p(g, fdtd_grid::PC_UPDATE_H, cs); launch_update_H(G, g->T, fields, inv_mu, g->psiH[0], cs); }
             { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
-              for (const SourceDev &s : S) if (s.comp >= 3) launch_add_source(G, fields, s, g->d_step, 1.f, cs);
-              for (const DetectorDev &dt : D) launch_detector(G, fields, dt, g->d_cs, total_freq, g->d_step, cs); }
-            { ProfScope p(g, fdtd_grid::PC_OTHER, cs); launch_advance(g->d_step, 1, cs); }
+              for (const SourceDev &s : S) if (s.comp >= 3) launch_add_source(G, fields, s, g->step_in(), 1.f, cs);
+              for (const DetectorDev &dt : D) launch_detector(G, fields, dt, g->d_cs, total_freq, g->step_in(), cs); }
+            { ProfScope p(g, fdtd_grid::PC_OTHER, cs); launch_next_step(g->step_in(), g->step_out(), 1, cs); }
         });
         if (rc) return rc;
     }
@@ -589,8 +592,7 @@ extern "C" int fdtd_backward(fdtd_grid *g, float *fields, const float *inv_eps, 
     for (int q = 0; q < 2; ++q)
         if ((rc = g->zero_psi(g->lpsiE[q], st)) || (rc = g->zero_psi(g->lpsiH[q], st))) return rc;
     CK(cudaMemsetAsync(dL_dinv_eps, 0, vol, st));
-    CK(cudaMemsetAsync(g->d_step, 0, sizeof(int), st));
-    if (n_steps > 0) launch_advance(g->d_step, n_steps - 1, st);
+    launch_set_step(g->d_step, std::max(n_steps - 1, 0), st);   // the first reverse step reads slot 0
 
     if (g->path == FDTD_PATH_FUSED && g->fused_backward_ready && !inv_mu) {
         rc = fused_backward(g, fields, inv_eps, inv_mu, S, D, total_freq, n_steps, dL_dinv_eps, st);
@@ -602,17 +604,17 @@ extern "C" int fdtd_backward(fdtd_grid *g, float *fields, const float *inv_eps, 
         const std::string key = make_key("gb", fields, inv_eps, inv_mu, g->rec, dL_dinv_eps, S, D, 0);
         rc = run_steps(g, g->bwd_graph, key, n_steps, launches, st, [&](cudaStream_t cs) {
             { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
-              for (const DetectorDev &dt : D) if (dt.phasor) launch_detector_adjoint(G, g->lam, dt, g->d_cs, total_freq, g->d_step, cs); }
-            { ProfScope p(g, fdtd_grid::PC_ADJ_H, cs); launch_adj_H(G, g->T, g->lam, inv_mu, g->lpsiH[0], g->lpsiH[1], g->d_step, cs); }
+              for (const DetectorDev &dt : D) if (dt.phasor) launch_detector_adjoint(G, g->lam, dt, g->d_cs, total_freq, g->step_in(), cs); }
+            { ProfScope p(g, fdtd_grid::PC_ADJ_H, cs); launch_adj_H(G, g->T, g->lam, inv_mu, g->lpsiH[0], g->lpsiH[1], g->step_in(), cs); }
             { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
-              for (const SourceDev &s : S) if (s.comp >= 3) launch_add_source(G, fields, s, g->d_step, -1.f, cs); }
-            if (G.d > 0) { ProfScope p(g, fdtd_grid::PC_INJECT, cs); launch_inject(G, g->R, fields, g->rec, g->d_step, cs); }
+              for (const SourceDev &s : S) if (s.comp >= 3) launch_add_source(G, fields, s, g->step_in(), -1.f, cs); }
+            if (G.d > 0) { ProfScope p(g, fdtd_grid::PC_INJECT, cs); launch_inject(G, g->R, fields, g->rec, g->step_in(), cs); }
             { ProfScope p(g, fdtd_grid::PC_INV_H, cs); launch_inv_H(G, fields, inv_mu, cs); }
             { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
-              for (const SourceDev &s : S) if (s.comp < 3) launch_add_source(G, fields, s, g->d_step, -1.f, cs); }
+              for (const SourceDev &s : S) if (s.comp < 3) launch_add_source(G, fields, s, g->step_in(), -1.f, cs); }
             { ProfScope p(g, fdtd_grid::PC_INV_E_GRAD, cs); launch_inv_E_grad(G, fields, inv_eps, g->lam, dL_dinv_eps, cs); }
-            { ProfScope p(g, fdtd_grid::PC_ADJ_E, cs); launch_adj_E(G, g->T, g->lam, inv_eps, g->lpsiE[0], g->lpsiE[1], g->d_step, cs); }
-            { ProfScope p(g, fdtd_grid::PC_OTHER, cs); launch_advance(g->d_step, -1, cs); }
+            { ProfScope p(g, fdtd_grid::PC_ADJ_E, cs); launch_adj_E(G, g->T, g->lam, inv_eps, g->lpsiE[0], g->lpsiE[1], g->step_in(), cs); }
+            { ProfScope p(g, fdtd_grid::PC_OTHER, cs); launch_next_step(g->step_in(), g->step_out(), -1, cs); }
         });
         if (rc) return rc;
     }

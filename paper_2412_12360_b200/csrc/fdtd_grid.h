@@ -22,7 +22,10 @@ struct fdtd_grid {
     // device memory owned by the grid
     std::vector<void *> owned;
     long long recorder_bytes = 0, scratch_bytes = 0;
-    int *d_step = nullptr;
+    int *d_step = nullptr;                 // two slots; the step being enqueued reads slot step_par, the next one the other
+    int step_par = 0;
+    int *step_in() const { return d_step + step_par; }
+    int *step_out() const { return d_step + (step_par ^ 1); }
     fdtd::PsiSet psiE[2]{}, psiH[2]{};     // primal psi ([1] only used by the fused path's ping-pong)
     fdtd::PsiSet lpsiE[2]{}, lpsiH[2]{};   // psi cotangents, ping-ponged by step parity
     float *lam = nullptr;                  // cotangent fields [6][nz][ny][nx]
@@ -43,7 +46,7 @@ struct fdtd_grid {
     // graphs
     struct GraphCache {
         std::string key;
-        cudaGraphExec_t exec_main = nullptr, exec_tail = nullptr;
+        cudaGraphExec_t exec_main = nullptr, exec_tail[2] = { nullptr, nullptr };   // tail: one step, per counter slot
         cudaEvent_t done = nullptr;
     } fwd_graph, bwd_graph;
     cudaStream_t cap_stream = nullptr;

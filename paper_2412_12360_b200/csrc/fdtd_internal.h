@@ -115,6 +115,9 @@ void launch_inject_pp(const Dims &G, const RecLayout &R, float *bufA, float *buf
                       const int *step, cudaStream_t st);
 void launch_inject(const Dims &G, const RecLayout &R, float *fields, const float *rec, const int *step, cudaStream_t st);
 void launch_advance(int *step, int delta, cudaStream_t st);
+// two-slot step counter: step p reads slot p&1; one kernel of that step writes the other slot for the next step
+void launch_next_step(const int *in, int *out, int delta, cudaStream_t st);
+void launch_set_step(int *p, int v, cudaStream_t st);
 // psi cotangents are ping-ponged by step parity: read set[n&1], write set[(n&1)^1]
 void launch_adj_H(const Dims &G, const Tables &T, float *lam, const float *im, PsiSet set0, PsiSet set1,
                   const int *step, cudaStream_t st);

@@ -202,6 +202,9 @@ __global__ void k_record(Dims G, RecLayout R, const float *__restrict__ fH, cons
 }
 
 __global__ void k_advance(int *step, int delta) { *step += delta; }
+// the step counter lives in two slots that alternate between steps: nobody reads `out` during the step that writes it
+__global__ void k_next_step(const int *in, int *out, int delta) { *out = *in + delta; }
+__global__ void k_set_step(int *p, int v) { *p = v; }
 
 // ------------------------------------------------------------------------------------------ B2 / B5
 // Adjoint of the H update (FAMILY=1: reads lamH, updates lamE, psi_H cotangents) or of the E update
@@ -447,6 +450,8 @@ void launch_inject(const Dims &G, const RecLayout &R, float *fields, const float
 }
 
 void launch_advance(int *step, int delta, cudaStream_t st) { k_advance<<<1, 1, 0, st>>>(step, delta); }
+void launch_next_step(const int *in, int *out, int delta, cudaStream_t st) { k_next_step<<<1, 1, 0, st>>>(in, out, delta); }
+void launch_set_step(int *p, int v, cudaStream_t st) { k_set_step<<<1, 1, 0, st>>>(p, v); }
 
 void launch_adj_H(const Dims &G, const Tables &T, float *lam, const float *im, PsiSet s0, PsiSet s1,
                   const int *step, cudaStream_t st)

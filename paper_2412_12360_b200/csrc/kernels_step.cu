@@ -59,7 +59,9 @@ struct StepParams {
     float *buf[2];                 // ping-pong volumes, [6][nc] each
     const float *ie, *im;
     PsiSet psiE[2], psiH[2];       // CPML states of the E-type / H-type update, ping-pong
-    const int *step;
+    const int *step;               // the slot of the two-slot step counter this step reads
+    int *step_next;                // the other slot: block 0 writes n + step_delta for the next step (or NULL)
+    int step_delta;
     int nst;                       // pipeline stages
     int stage;                     // bytes of one stage: 7 boxes + 4 x-slab state boxes
     int xs_bytes, xs_pitch;        // x-slab state box [ROWS][2*dpx]: exact bytes (TMA transaction) and 128-byte aligned pitch
@@ -224,6 +226,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
     if (threadIdx.x == 0) {
         for (int s = 0; s < nst; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], C::NCW); }
         fence_mbar_init();
+        if (blockIdx.x == 0 && P.step_next) *P.step_next = n + P.step_delta;
         if (P.dbg_t) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); P.dbg_t[2 * blockIdx.x] = t; }
     }
     __syncthreads();
@@ -1112,7 +1115,7 @@ int fused_setup(fdtd_grid *g)
     StepParams &P = F->sp;
     P.G = G; P.T = g->T; P.segs = F->d_segs[0]; P.seg_begin = F->d_seg_begin[0];
     P.n_rot = n_rot; P.seg_stride = (int)stride; P.n_cta = n_cta;
-    P.step = g->d_step;
+    P.step = g->d_step; P.step_next = nullptr; P.step_delta = 0;
     P.nst = F->nst;
     P.stage = stage_bytes; P.xs_bytes = xs_bytes; P.xs_pitch = xs_pitch;
     P.dbg = getenv("FDTD_DBG") ? atoi(getenv("FDTD_DBG")) : 0;
@@ -1300,14 +1303,15 @@ void enqueue_fwd(void *vctx, cudaStream_t cs)
     FwdCtx *c = (FwdCtx *)vctx;
     fdtd_grid *g = c->g;
     FusedState *F = g->fused;
+    StepParams Q = c->P;
+    Q.step = g->step_in(); Q.step_next = g->step_out(); Q.step_delta = 1;
     { ProfScope p(g, fdtd_grid::PC_FUSED_FWD, cs);
-      F->tile->launch_fwd(c->P, F->n_cta, F->smem, cs); }
+      F->tile->launch_fwd(Q, F->n_cta, F->smem, cs); }
     if (c->recording) {
         // step n read buffer n&1 (pre-step H) and wrote buffer (n+1)&1 (E'); the record kernel picks them by parity
         ProfScope p(g, fdtd_grid::PC_RECORD, cs);
-        launch_record_pp(g->G, g->R, c->A, c->B, g->rec, g->d_step, cs);
+        launch_record_pp(g->G, g->R, c->A, c->B, g->rec, g->step_in(), cs);
     }
-    { ProfScope p(g, fdtd_grid::PC_OTHER, cs); launch_advance(g->d_step, 1, cs); }
 }
 
 struct BwdCtx {
@@ -1324,24 +1328,26 @@ void enqueue_bwd(void *vctx, cudaStream_t cs)
     const Dims &G = g->G;
     { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
       for (const DetectorDev &dt : *c->D)
-          if (dt.phasor) launch_detector_adjoint_pp(G, c->lamA, c->lamB, dt, g->d_cs, c->total_freq, g->d_step, cs); }
+          if (dt.phasor) launch_detector_adjoint_pp(G, c->lamA, c->lamB, dt, g->d_cs, c->total_freq, g->step_in(), cs); }
+    StepParams Q = c->P;
+    Q.step = g->step_in(); Q.step_next = g->step_out(); Q.step_delta = -1;
     { ProfScope p(g, fdtd_grid::PC_FUSED_BWD, cs);
-      F->tile->launch_adj(c->P, F->n_cta, F->smem, cs); }
+      F->tile->launch_adj(Q, F->n_cta, F->smem, cs); }
     if (c->fused_inv) {
-        if (G.d > 0) { ProfScope p(g, fdtd_grid::PC_INJECT, cs); launch_inject_pp(G, g->R, c->fields, c->bufB, g->rec, g->d_step, cs); }
-        { ProfScope p(g, fdtd_grid::PC_FUSED_INV, cs); F->itile->launch_inv(c->I, F->in_cta, F->ismem, cs); }
-        { ProfScope p(g, fdtd_grid::PC_OTHER, cs); launch_advance(g->d_step, -1, cs); }
+        if (G.d > 0) { ProfScope p(g, fdtd_grid::PC_INJECT, cs); launch_inject_pp(G, g->R, c->fields, c->bufB, g->rec, g->step_in(), cs); }
+        InvParams J = c->I;
+        J.step = g->step_in();
+        { ProfScope p(g, fdtd_grid::PC_FUSED_INV, cs); F->itile->launch_inv(J, F->in_cta, F->ismem, cs); }
         return;
     }
     { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
-      for (const SourceDev &s : *c->S) if (s.comp >= 3) launch_add_source(G, c->fields, s, g->d_step, -1.f, cs); }
-    if (G.d > 0) { ProfScope p(g, fdtd_grid::PC_INJECT, cs); launch_inject(G, g->R, c->fields, g->rec, g->d_step, cs); }
+      for (const SourceDev &s : *c->S) if (s.comp >= 3) launch_add_source(G, c->fields, s, g->step_in(), -1.f, cs); }
+    if (G.d > 0) { ProfScope p(g, fdtd_grid::PC_INJECT, cs); launch_inject(G, g->R, c->fields, g->rec, g->step_in(), cs); }
     { ProfScope p(g, fdtd_grid::PC_INV_H, cs); launch_inv_H(G, c->fields, nullptr, cs); }
     { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
-      for (const SourceDev &s : *c->S) if (s.comp < 3) launch_add_source(G, c->fields, s, g->d_step, -1.f, cs); }
+      for (const SourceDev &s : *c->S) if (s.comp < 3) launch_add_source(G, c->fields, s, g->step_in(), -1.f, cs); }
     { ProfScope p(g, fdtd_grid::PC_INV_E_GRAD, cs);
-      launch_inv_E_grad_pp(G, c->fields, c->ie, c->lamA, c->lamB, g->d_step, c->grad, cs); }
-    { ProfScope p(g, fdtd_grid::PC_OTHER, cs); launch_advance(g->d_step, -1, cs); }
+      launch_inv_E_grad_pp(G, c->fields, c->ie, c->lamA, c->lamB, g->step_in(), c->grad, cs); }
 }
 }  // namespace
 
@@ -1378,7 +1384,7 @@ int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float
     std::string key("ff");
     key.append((const char *)&P, sizeof(P));
     key.push_back(recording ? 1 : 0);
-    rc = fdtd_run_steps_fwd(g, key, n_steps, 2 + (recording ? 1 : 0), st, enqueue_fwd, &ctx);
+    rc = fdtd_run_steps_fwd(g, key, n_steps, 1 + (recording ? 1 : 0), st, enqueue_fwd, &ctx);
     if (rc) return rc;
     if (n_steps & 1) {
         cudaError_t e = cudaMemcpyAsync(fields, F->bufB, (size_t)g->G.nc * 6 * sizeof(float), cudaMemcpyDeviceToDevice, st);
@@ -1441,5 +1447,5 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     key.append((const char *)&dL_dinv_eps, sizeof(dL_dinv_eps));
     if (!S.empty()) key.append((const char *)S.data(), S.size() * sizeof(SourceDev));
     if (!D.empty()) key.append((const char *)D.data(), D.size() * sizeof(DetectorDev));
-    return fdtd_run_steps_bwd(g, key, n_steps, 4 + n_adj + (int)S.size() + (g->G.d > 0 ? 1 : 0), st, enqueue_bwd, &ctx);
+    return fdtd_run_steps_bwd(g, key, n_steps, fused_inv ? 2 + n_adj + (g->G.d > 0 ? 1 : 0) : 3 + n_adj + (int)S.size() + (g->G.d > 0 ? 1 : 0), st, enqueue_bwd, &ctx);
 }
