@@ -175,6 +175,37 @@ __device__ __noinline__ void detect_cell(const StepParams &P, int n, int comp, f
     }
 }
 
+// adjoint of the running DFT (B1) at cell (i,j,k) of component `comp`: sum_f Gr cos - Gi sin, with the caller's
+// phasor cotangents in det[].phasor (NULL: no cotangent for that detector)
+__device__ __noinline__ float det_adjoint_at(const StepParams &P, int n, int comp, int i, int j, int k)
+{
+    float acc = 0.f;
+    for (int s = 0; s < P.n_det; ++s) {
+        const DetectorDev &q = P.det[s];
+        if (!q.phasor || !((q.mask >> comp) & 1)) continue;
+        if (i < q.lo[0] || i >= q.hi[0] || j < q.lo[1] || j >= q.hi[1] || k < q.lo[2] || k >= q.hi[2]) continue;
+        const int bx = q.hi[0] - q.lo[0], by = q.hi[1] - q.lo[1], bz = q.hi[2] - q.lo[2];
+        const long long bc = (long long)bx * by * bz;
+        const long long cell = ((long long)(k - q.lo[2]) * by + (j - q.lo[1])) * bx + (i - q.lo[0]);
+        int ci = 0;
+        for (int c = 0; c < comp; ++c) ci += (q.mask >> c) & 1;
+        const float *csn = P.cs + ((long long)n * P.total_freq + q.cs_off) * 2;
+        for (int f = 0; f < q.n_freq; ++f) {
+            const float2 Gq = __ldg(reinterpret_cast<const float2 *>(q.phasor) + ((long long)f * q.ncomp + ci) * bc + cell);
+            acc += Gq.x * __ldg(csn + 2 * f) - Gq.y * __ldg(csn + 2 * f + 1);
+        }
+    }
+    return acc;
+}
+__device__ __noinline__ float4 det_adjoint4(const StepParams &P, int n, int comp, float4 v, int i, int j, int k)
+{
+    v.x += det_adjoint_at(P, n, comp, i + 0, j, k);
+    v.y += det_adjoint_at(P, n, comp, i + 1, j, k);
+    v.z += det_adjoint_at(P, n, comp, i + 2, j, k);
+    v.w += det_adjoint_at(P, n, comp, i + 3, j, k);
+    return v;
+}
+
 __device__ __forceinline__ float f4get(const float4 &v, int q) { return q == 0 ? v.x : (q == 1 ? v.y : (q == 2 ? v.z : v.w)); }
 
 // adds the sources of component `comp` to the float4 of cells (i..i+3, j, k); rare planes only
@@ -325,6 +356,15 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
             mbar_wait(&full[st_i], st_ph);
             const uint32_t so = stage_base + st_off + o_own;
             const uint32_t sp = stage_base + pv_off + o_own;       // the stage of plane kk-1 is still held
+            if (ADJ && kk >= P.dEl && kk < P.dEh && !dup) {
+                // B1 for E-component detectors: the cotangents are added to lamE in the stage, at my cells, before
+                // anything is live in registers (lamE is only ever read at a thread's own cells)
+                for (int c = 0; c < 3; ++c) {
+                    const uint32_t se = so + (3 + c) * C::SLOT;
+                    sts4(se, det_adjoint4(P, n, c, lds4(se), i, j, kk));
+                }
+                fence_proxy_async();
+            }
             const uint32_t xs0 = stage_base + st_off + 7 * C::SLOT; // x-slab state boxes of this stage
             const float4 fx = lds4(so), fy = lds4(so + C::SLOT), fz = lds4(so + 2 * C::SLOT);
             const float4 fx_my = lds4(so - C::ROWB), fz_my = lds4(so + 2 * C::SLOT - C::ROWB);
@@ -1315,7 +1355,7 @@ void enqueue_fwd(void *vctx, cudaStream_t cs)
 }
 
 struct BwdCtx {
-    fdtd_grid *g; StepParams P; InvParams I; bool fused_inv; float *bufB; float *fields; const float *ie; float *grad; float *lamA; float *lamB;
+    fdtd_grid *g; StepParams P; InvParams I; bool fused_inv; bool fused_det; float *bufB; float *fields; const float *ie; float *grad; float *lamA; float *lamB;
     const std::vector<SourceDev> *S; const std::vector<DetectorDev> *D; int total_freq;
 };
 // reverse step n: B1 (detector cotangents into the volume about to be read), B2+B5 (fused adjoint step),
@@ -1326,7 +1366,7 @@ void enqueue_bwd(void *vctx, cudaStream_t cs)
     fdtd_grid *g = c->g;
     FusedState *F = g->fused;
     const Dims &G = g->G;
-    { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
+    if (!c->fused_det) { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
       for (const DetectorDev &dt : *c->D)
           if (dt.phasor) launch_detector_adjoint_pp(G, c->lamA, c->lamB, dt, g->d_cs, c->total_freq, g->step_in(), cs); }
     StepParams Q = c->P;
@@ -1410,7 +1450,10 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
         if (e != cudaSuccess) { (void)cudaGetLastError(); return fdtd_fail(FDTD_ECUDA, cudaGetErrorString(e)); }
     }
     const bool fused_inv = F->itile != nullptr && (int)S.size() <= MAX_SRC && !getenv("FDTD_GENERIC_INVERSE");
-    BwdCtx ctx{ g, F->sp, F->ip, fused_inv, F->bufB, fields, inv_eps, dL_dinv_eps, g->lam, F->lamB, &S, &D, total_freq };
+    // B1 inside the adjoint kernel when every detector with a cotangent is on E components (else a kernel per detector)
+    bool fused_det = (int)D.size() <= MAX_DET;
+    for (const DetectorDev &dt : D) if (dt.phasor && (dt.mask >> 3)) fused_det = false;
+    BwdCtx ctx{ g, F->sp, F->ip, fused_inv, fused_det, F->bufB, fields, inv_eps, dL_dinv_eps, g->lam, F->lamB, &S, &D, total_freq };
     if (fused_inv) {
         // reverse step n reads primal volume (n+1)&1 and writes n&1: state n_steps must sit in volume n_steps&1
         if ((rc = build_inv_maps(g, fields, F->bufB, inv_eps, g->lam, F->lamB, st))) return rc;
@@ -1437,6 +1480,13 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     for (int q = 0; q < 2; ++q) { P.psiE[q] = g->lpsiE[q]; P.psiH[q] = g->lpsiH[q]; }
     P.n_src = 0; P.n_det = 0; P.total_freq = total_freq;
     P.sEl = P.sHl = P.dEl = P.dHl = 1 << 30; P.sEh = P.sHh = P.dEh = P.dHh = -1;
+    if (fused_det) {
+        P.n_det = (int)D.size();
+        for (size_t q = 0; q < D.size(); ++q) {
+            P.det[q] = D[q];
+            if (D[q].phasor) { P.dEl = std::min(P.dEl, D[q].lo[2]); P.dEh = std::max(P.dEh, D[q].hi[2]); }
+        }
+    }
     P.cs = g->d_cs;
     int n_adj = 0;
     for (const DetectorDev &dt : D) if (dt.phasor) ++n_adj;
@@ -1447,5 +1497,5 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     key.append((const char *)&dL_dinv_eps, sizeof(dL_dinv_eps));
     if (!S.empty()) key.append((const char *)S.data(), S.size() * sizeof(SourceDev));
     if (!D.empty()) key.append((const char *)D.data(), D.size() * sizeof(DetectorDev));
-    return fdtd_run_steps_bwd(g, key, n_steps, fused_inv ? 2 + n_adj + (g->G.d > 0 ? 1 : 0) : 3 + n_adj + (int)S.size() + (g->G.d > 0 ? 1 : 0), st, enqueue_bwd, &ctx);
+    return fdtd_run_steps_bwd(g, key, n_steps, fused_inv ? 2 + (fused_det ? 0 : n_adj) + (g->G.d > 0 ? 1 : 0) : 3 + (fused_det ? 0 : n_adj) + (int)S.size() + (g->G.d > 0 ? 1 : 0), st, enqueue_bwd, &ctx);
 }
