@@ -254,6 +254,22 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
     constexpr int FA = ADJ ? 1 : 0, FB = ADJ ? 0 : 1;   // CPML family (tables, states) of phase A / phase B
     const int nst = P.nst;
 
+    // CPML tables of the slab cells in shared memory, indexed by slab-compact coordinate:
+    // [family][b, a, 1/kappa - 1][x: 2 dpx | y: 2 d | z: 2 d]
+    float *tabs = reinterpret_cast<float *>(empty + MAX_ST);
+    const uint32_t tab_base = smem_u32(tabs);
+    const int YO = 2 * G.dpx, ZO = 2 * G.dpx + 2 * G.d, TL = 2 * G.dpx + 4 * G.d;
+#define TB1(F, kind, off) lds1(tab_base + (uint32_t)((((F) * 3 + (kind)) * TL + (off)) * 4))
+#define TB4(F, kind, off) lds4(tab_base + (uint32_t)((((F) * 3 + (kind)) * TL + (off)) * 4))
+    for (int e = threadIdx.x; e < 6 * TL; e += blockDim.x) {
+        const int fk = e / TL, q = e - fk * TL, fam = fk / 3, kind = fk - 3 * fam;
+        const int ax = q < YO ? 0 : (q < ZO ? 1 : 2);
+        const int sc = q - (ax == 0 ? 0 : (ax == 1 ? YO : ZO));
+        const int w = ax == 0 ? G.dpx : G.d, N = ax == 0 ? G.nx : (ax == 1 ? G.ny : G.nz);
+        const int pos = sc < w ? sc : N - 2 * w + sc;
+        const float *src = kind == 0 ? P.T.b[fam][ax] : (kind == 1 ? P.T.a[fam][ax] : P.T.ik[fam][ax]);
+        tabs[e] = __ldg(src + pos) - (kind == 2 ? 1.f : 0.f);
+    }
     if (threadIdx.x == 0) {
         for (int s = 0; s < nst; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], C::NCW); }
         fence_mbar_init();
@@ -393,14 +409,14 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                 Dz_x = fx - lds4(sp); Dz_y = fy - lds4(sp + C::SLOT);
                 if (slab_xy || zs >= 0) {
                     if (zs >= 0 && ing) {
-                        const float b = __ldg(P.T.b[FA][2] + kk), a = __ldg(P.T.a[FA][2] + kk), km = __ldg(P.T.ik[FA][2] + kk) - 1.f;
+                        const float b = TB1(FA, 0, ZO + zs), a = TB1(FA, 1, ZO + zs), km = TB1(FA, 2, ZO + zs);
                         float4 p0, p1;
                         Dz_x = Dz_x + cpml4(b, a, km, ldg4(qAi.p[1][0] + oz), Dz_x, p0);
                         Dz_y = Dz_y + cpml4(b, a, km, ldg4(qAi.p[0][1] + oz), Dz_y, p1);
                         if (wr) { stg4(qAo.p[1][0] + oz, p0); stg4(qAo.p[0][1] + oz, p1); }
                     }
                     if (syk >= 0) {
-                        const float b = __ldg(P.T.b[FA][1] + j), a = __ldg(P.T.a[FA][1] + j), km = __ldg(P.T.ik[FA][1] + j) - 1.f;
+                        const float b = TB1(FA, 0, YO + sy), a = TB1(FA, 1, YO + sy), km = TB1(FA, 2, YO + sy);
                         const int q = kk * py + oy;
                         float4 p0, p1;
                         Dy_z = Dy_z + cpml4(b, a, km, ldg4(qAi.p[0][0] + q), Dy_z, p0);
@@ -409,7 +425,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                         if (wr) { stg4(qAo.p[0][0] + q, p0); stg4(qAo.p[2][1] + q, p1); }
                     }
                     if (sxk >= 0) {
-                        const float4 b = ldg4(P.T.b[FA][0] + i), a = ldg4(P.T.a[FA][0] + i), km = ldg4(P.T.ik[FA][0] + i) - splat(1.f);
+                        const float4 b = TB4(FA, 0, sx), a = TB4(FA, 1, sx), km = TB4(FA, 2, sx);
                         const int q = kk * px + ox;
                         float4 p0, p1;
                         Dx_y = Dx_y + cpml4(b, a, km, lds4(xs0 + xo), Dx_y, p0);
@@ -421,14 +437,14 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                 float4 gx = fx, gy = fy;                       // z operands at plane kk, filtered
                 if (slab_xy || zs >= 0) {
                     if (zs >= 0 && ing) {
-                        const float b = __ldg(P.T.b[FA][2] + kk), a = __ldg(P.T.a[FA][2] + kk), km = __ldg(P.T.ik[FA][2] + kk) - 1.f;
+                        const float b = TB1(FA, 0, ZO + zs), a = TB1(FA, 1, ZO + zs), km = TB1(FA, 2, ZO + zs);
                         float4 p0, p1;
                         gx = fx + cpml4(b, a, km, ldg4(qAi.p[1][0] + oz), fx, p0);
                         gy = fy + cpml4(b, a, km, ldg4(qAi.p[0][1] + oz), fy, p1);
                         if (wr) { stg4(qAo.p[1][0] + oz, p0); stg4(qAo.p[0][1] + oz, p1); }
                     }
                     if (syk >= 0) {
-                        const float b = __ldg(P.T.b[FA][1] + j), a = __ldg(P.T.a[FA][1] + j), km = __ldg(P.T.ik[FA][1] + j) - 1.f;
+                        const float b = TB1(FA, 0, YO + sy), a = TB1(FA, 1, YO + sy), km = TB1(FA, 2, YO + sy);
                         const int q = kk * py + oy;
                         float4 p0, p1;
                         Dy_z = Dy_z + cpml4(b, a, km, ldg4(qAi.p[0][0] + q), fz, p0);
@@ -437,7 +453,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                         if (wr) { stg4(qAo.p[0][0] + q, p0); stg4(qAo.p[2][1] + q, p1); }
                     }
                     if (symk >= 0) {
-                        const float b = __ldg(P.T.b[FA][1] + j - 1), a = __ldg(P.T.a[FA][1] + j - 1), km = __ldg(P.T.ik[FA][1] + j - 1) - 1.f;
+                        const float b = TB1(FA, 0, YO + sym), a = TB1(FA, 1, YO + sym), km = TB1(FA, 2, YO + sym);
                         const int q = kk * py + oym;
                         float4 p0, p1;
                         Dy_z = Dy_z - cpml4(b, a, km, ldg4(qAi.p[0][0] + q), fz_my, p0);
@@ -448,7 +464,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                         float4 cy = Z4, cz = Z4;
                         float ly = 0.f, lz = 0.f;
                         if (sxk >= 0) {
-                            const float4 b = ldg4(P.T.b[FA][0] + i), a = ldg4(P.T.a[FA][0] + i), km = ldg4(P.T.ik[FA][0] + i) - splat(1.f);
+                            const float4 b = TB4(FA, 0, sx), a = TB4(FA, 1, sx), km = TB4(FA, 2, sx);
                             const int q = kk * px + ox;
                             float4 p0, p1;
                             cy = cpml4(b, a, km, lds4(xs0 + xo), fy, p0);
@@ -456,7 +472,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                             if (wr) { stg4(qAo.p[2][0] + q, p0); stg4(qAo.p[1][1] + q, p1); }
                         }
                         if (sxmk >= 0) {
-                            const float b = __ldg(P.T.b[FA][0] + i - 1), a = __ldg(P.T.a[FA][0] + i - 1), km = __ldg(P.T.ik[FA][0] + i - 1) - 1.f;
+                            const float b = TB1(FA, 0, sxm), a = TB1(FA, 1, sxm), km = TB1(FA, 2, sxm);
                             const int q = kk * px + oxm;
                             ly = cpml1(b, a, km, lds1(xs0 + xom), fy_mx);
                             lz = cpml1(b, a, km, lds1(xs0 + P.xs_pitch + xom), fz_mx);
@@ -490,14 +506,14 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
             float4 Yx = v2x, Yz = v2z, Xy = v2y, Xz = v2z, Zx = v2x, Zy = v2y;
             if (ADJ && (slab_xy || zs >= 0)) {       // phase-B operands are filtered where they are produced
                 if (zs >= 0 && ing) {
-                    const float b = __ldg(P.T.b[FB][2] + kk), a = __ldg(P.T.a[FB][2] + kk), km = __ldg(P.T.ik[FB][2] + kk) - 1.f;
+                    const float b = TB1(FB, 0, ZO + zs), a = TB1(FB, 1, ZO + zs), km = TB1(FB, 2, ZO + zs);
                     float4 p0, p1;
                     Zx = v2x + cpml4(b, a, km, ldg4(qBi.p[1][0] + oz), v2x, p0);
                     Zy = v2y + cpml4(b, a, km, ldg4(qBi.p[0][1] + oz), v2y, p1);
                     if (wr) { stg4(qBo.p[1][0] + oz, p0); stg4(qBo.p[0][1] + oz, p1); }
                 }
                 if (syk >= 0) {
-                    const float b = __ldg(P.T.b[FB][1] + j), a = __ldg(P.T.a[FB][1] + j), km = __ldg(P.T.ik[FB][1] + j) - 1.f;
+                    const float b = TB1(FB, 0, YO + sy), a = TB1(FB, 1, YO + sy), km = TB1(FB, 2, YO + sy);
                     const int q = kk * py + oy;
                     float4 p0, p1;
                     Yz = v2z + cpml4(b, a, km, ldg4(qBi.p[0][0] + q), v2z, p0);
@@ -506,7 +522,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                     if (wr) { stg4(qBo.p[0][0] + q, p0); stg4(qBo.p[2][1] + q, p1); }
                 }
                 if (sxk >= 0) {
-                    const float4 b = ldg4(P.T.b[FB][0] + i), a = ldg4(P.T.a[FB][0] + i), km = ldg4(P.T.ik[FB][0] + i) - splat(1.f);
+                    const float4 b = TB4(FB, 0, sx), a = TB4(FB, 1, sx), km = TB4(FB, 2, sx);
                     const int q = kk * px + ox;
                     float4 p0, p1;
                     Xy = v2y + cpml4(b, a, km, lds4(xs0 + 2 * P.xs_pitch + xo), v2y, p0);
@@ -532,7 +548,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                 const int zsm = (!ADJ && pml && !DBG(128)) ? slab_pos(km1, G.nz, G.d) : -1;
                 if (!ADJ && (slab_xy || zsm >= 0)) {
                     if (zsm >= 0) {
-                        const float b = __ldg(P.T.b[FB][2] + km1), a = __ldg(P.T.a[FB][2] + km1), km = __ldg(P.T.ik[FB][2] + km1) - 1.f;
+                        const float b = TB1(FB, 0, ZO + zsm), a = TB1(FB, 1, ZO + zsm), km = TB1(FB, 2, ZO + zsm);
                         const int q = zsm * pz + own_xy;
                         float4 p0, p1;
                         Dz_x = Dz_x + cpml4(b, a, km, ldg4(qBi.p[1][0] + q), Dz_x, p0);
@@ -540,7 +556,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                         stg4(qBo.p[1][0] + q, p0); stg4(qBo.p[0][1] + q, p1);
                     }
                     if (sy >= 0) {
-                        const float b = __ldg(P.T.b[FB][1] + j), a = __ldg(P.T.a[FB][1] + j), km = __ldg(P.T.ik[FB][1] + j) - 1.f;
+                        const float b = TB1(FB, 0, YO + sy), a = TB1(FB, 1, YO + sy), km = TB1(FB, 2, YO + sy);
                         const int q = km1 * py + oy;
                         float4 p0, p1;
                         Dy_z = Dy_z + cpml4(b, a, km, ldg4(qBi.p[0][0] + q), Dy_z, p0);
@@ -549,7 +565,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                         stg4(qBo.p[0][0] + q, p0); stg4(qBo.p[2][1] + q, p1);
                     }
                     if (sx >= 0) {
-                        const float4 b = ldg4(P.T.b[FB][0] + i), a = ldg4(P.T.a[FB][0] + i), km = ldg4(P.T.ik[FB][0] + i) - splat(1.f);
+                        const float4 b = TB4(FB, 0, sx), a = TB4(FB, 1, sx), km = TB4(FB, 2, sx);
                         const int q = km1 * px + ox;
                         float4 p0, p1;
                         Dx_y = Dx_y + cpml4(b, a, km, lds4(xs0 + 2 * P.xs_pitch + xo), Dx_y, p0);
@@ -593,7 +609,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                 if (pml) {
                     const int zs = slab_pos(kk, G.nz, G.d);
                     if (zs >= 0 && ing) {
-                        const float b = __ldg(P.T.b[FA][2] + kk), a = __ldg(P.T.a[FA][2] + kk), km = __ldg(P.T.ik[FA][2] + kk) - 1.f;
+                        const float b = TB1(FA, 0, ZO + zs), a = TB1(FA, 1, ZO + zs), km = TB1(FA, 2, ZO + zs);
                         const int oz = zs * pz + own_xy;
                         float4 pn;
                         cgx = cgx + cpml4(b, a, km, ldg4(qAi.p[1][0] + oz), cgx, pn);
@@ -1022,7 +1038,7 @@ int fused_setup(fdtd_grid *g)
     // ---- tile choice among the compiled shapes: fewest consumer warp-planes per grid plane -------------------------
     int fTX = 0, fTY = 0;
     if (const char *e = getenv("FDTD_TILE")) sscanf(e, "%d,%d", &fTX, &fTY);
-    const int tail_bytes = 2 * MAX_ST * 8;
+    const int tail_bytes = 2 * MAX_ST * 8 + 6 * (2 * G.dpx + 4 * G.d) * 4;     // mbarriers + CPML tables
     const TileImpl *best = nullptr;
     double best_score = -1;
     int best_nst = 0;
