@@ -237,7 +237,20 @@ __device__ __noinline__ void detect4(const StepParams &P, int n, int family, flo
 // (filtered) difference of component c along axis a; its state array is
 //   Dy_z p[0][0]   Dz_y p[0][1]   Dz_x p[1][0]   Dx_z p[1][1]   Dx_y p[2][0]   Dy_x p[2][1].
 // ================================================================================================
-__device__ __forceinline__ void pf_l2(const float *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+#ifndef FDTD_PF_MODE
+#define FDTD_PF_MODE 2
+#endif
+__device__ __forceinline__ void pf_l2(const float *p)
+{
+#if FDTD_PF_MODE == 2
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+#elif FDTD_PF_MODE == 1
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
+#endif
+}
+#ifndef FDTD_PF_DIST
+#define FDTD_PF_DIST 1
+#endif
 
 template <class C, bool ADJ>
 __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ StepParams P)
@@ -392,14 +405,14 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
             const uint32_t rgA = ring_base + (uint32_t)(kk & 1) * (C::RING_SLOT * 4) + r_own;
             // plane nz (the zero wall behind the last plane) has no CPML states: all its inputs are zero
             const bool kin = kk < G.nz;
-            const bool pf = kk + 2 < G.nz;                     // L2 prefetch of the states two planes ahead stays inside the arrays
+            const bool pf = kk + FDTD_PF_DIST < G.nz;                     // L2 prefetch of the states two planes ahead stays inside the arrays
             const int sxk = kin ? sx : -1, syk = kin ? sy : -1, sxmk = kin ? sxm : -1, symk = kin ? sym : -1;
             // ------------------------------------------------------------ phase A: E-type update of plane kk
             float4 Dy_z = fz - fz_my, Dy_x = fx - fx_my;
             float4 Dx_y = dminus_x(fy, fy_mx), Dx_z = dminus_x(fz, fz_mx);
             float4 Dz_x, Dz_y;
             if (pml && ing) {
-                const int zs2 = slab_pos(kk + 2, G.nz, G.d);
+                const int zs2 = slab_pos(kk + FDTD_PF_DIST, G.nz, G.d);
                 if (zs2 >= 0) {
                     const int q = zs2 * pz + own_xy;
                     pf_l2(qAi.p[1][0] + q); pf_l2(qAi.p[0][1] + q); pf_l2(qBi.p[1][0] + q); pf_l2(qBi.p[0][1] + q);
@@ -421,7 +434,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                         float4 p0, p1;
                         Dy_z = Dy_z + cpml4(b, a, km, ldg4(qAi.p[0][0] + q), Dy_z, p0);
                         Dy_x = Dy_x + cpml4(b, a, km, ldg4(qAi.p[2][1] + q), Dy_x, p1);
-                        if (pf) { pf_l2(qAi.p[0][0] + q + 2 * py); pf_l2(qAi.p[2][1] + q + 2 * py); }
+                        if (pf) { pf_l2(qAi.p[0][0] + q + FDTD_PF_DIST * py); pf_l2(qAi.p[2][1] + q + FDTD_PF_DIST * py); }
                         if (wr) { stg4(qAo.p[0][0] + q, p0); stg4(qAo.p[2][1] + q, p1); }
                     }
                     if (sxk >= 0) {
@@ -449,7 +462,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                         float4 p0, p1;
                         Dy_z = Dy_z + cpml4(b, a, km, ldg4(qAi.p[0][0] + q), fz, p0);
                         Dy_x = Dy_x + cpml4(b, a, km, ldg4(qAi.p[2][1] + q), fx, p1);
-                        if (pf) { pf_l2(qAi.p[0][0] + q + 2 * py); pf_l2(qAi.p[2][1] + q + 2 * py); }
+                        if (pf) { pf_l2(qAi.p[0][0] + q + FDTD_PF_DIST * py); pf_l2(qAi.p[2][1] + q + FDTD_PF_DIST * py); }
                         if (wr) { stg4(qAo.p[0][0] + q, p0); stg4(qAo.p[2][1] + q, p1); }
                     }
                     if (symk >= 0) {
@@ -458,7 +471,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                         float4 p0, p1;
                         Dy_z = Dy_z - cpml4(b, a, km, ldg4(qAi.p[0][0] + q), fz_my, p0);
                         Dy_x = Dy_x - cpml4(b, a, km, ldg4(qAi.p[2][1] + q), fx_my, p1);
-                        if (pf && syk < 0) { pf_l2(qAi.p[0][0] + q + 2 * py); pf_l2(qAi.p[2][1] + q + 2 * py); }
+                        if (pf && syk < 0) { pf_l2(qAi.p[0][0] + q + FDTD_PF_DIST * py); pf_l2(qAi.p[2][1] + q + FDTD_PF_DIST * py); }
                     }
                     if (sxk >= 0 || sxmk >= 0) {
                         float4 cy = Z4, cz = Z4;
@@ -518,7 +531,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                     float4 p0, p1;
                     Yz = v2z + cpml4(b, a, km, ldg4(qBi.p[0][0] + q), v2z, p0);
                     Yx = v2x + cpml4(b, a, km, ldg4(qBi.p[2][1] + q), v2x, p1);
-                    if (pf) { pf_l2(qBi.p[0][0] + q + 2 * py); pf_l2(qBi.p[2][1] + q + 2 * py); }
+                    if (pf) { pf_l2(qBi.p[0][0] + q + FDTD_PF_DIST * py); pf_l2(qBi.p[2][1] + q + FDTD_PF_DIST * py); }
                     if (wr) { stg4(qBo.p[0][0] + q, p0); stg4(qBo.p[2][1] + q, p1); }
                 }
                 if (sxk >= 0) {
@@ -561,7 +574,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                         float4 p0, p1;
                         Dy_z = Dy_z + cpml4(b, a, km, ldg4(qBi.p[0][0] + q), Dy_z, p0);
                         Dy_x = Dy_x + cpml4(b, a, km, ldg4(qBi.p[2][1] + q), Dy_x, p1);
-                        if (pf) { pf_l2(qBi.p[0][0] + q + 2 * py); pf_l2(qBi.p[2][1] + q + 2 * py); }
+                        if (pf) { pf_l2(qBi.p[0][0] + q + FDTD_PF_DIST * py); pf_l2(qBi.p[2][1] + q + FDTD_PF_DIST * py); }
                         stg4(qBo.p[0][0] + q, p0); stg4(qBo.p[2][1] + q, p1);
                     }
                     if (sx >= 0) {
