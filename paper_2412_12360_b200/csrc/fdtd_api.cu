@@ -245,6 +245,11 @@ extern "C" int fdtd_create_grid(const fdtd_grid_desc *desc, fdtd_grid **out)
         e = cudaEventCreateWithFlags(&g->fwd_graph.done, cudaEventDisableTiming);
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&g->bwd_graph.done, cudaEventDisableTiming);
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&g->table_done, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&g->fork_ev, cudaEventDisableTiming);
+        for (int q = 0; q < 2 && e == cudaSuccess; ++q) {
+            e = cudaStreamCreateWithFlags(&g->side_stream[q], cudaStreamNonBlocking);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&g->join_ev[q], cudaEventDisableTiming);
+        }
         if (e != cudaSuccess) return bail(cuda_fail(e, "cudaEventCreate"));
     }
     g->path = FDTD_PATH_GENERIC;
@@ -268,6 +273,11 @@ extern "C" int fdtd_destroy(fdtd_grid *g)
     if (g->fwd_graph.done) cudaEventDestroy(g->fwd_graph.done);
     if (g->bwd_graph.done) cudaEventDestroy(g->bwd_graph.done);
     if (g->table_done) cudaEventDestroy(g->table_done);
+    if (g->fork_ev) cudaEventDestroy(g->fork_ev);
+    for (int q = 0; q < 2; ++q) {
+        if (g->side_stream[q]) cudaStreamDestroy(g->side_stream[q]);
+        if (g->join_ev[q]) cudaEventDestroy(g->join_ev[q]);
+    }
     for (auto &sp : g->prof_spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
     for (cudaEvent_t e : g->prof_pool) cudaEventDestroy(e);
     (void)cudaGetLastError();

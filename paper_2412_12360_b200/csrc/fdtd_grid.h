@@ -50,6 +50,10 @@ struct fdtd_grid {
         cudaEvent_t done = nullptr;
     } fwd_graph, bwd_graph;
     cudaStream_t cap_stream = nullptr;
+    // fork / join of the launches that run beside a step kernel (recorder, inverse step, face injection): the side
+    // streams wait for fork_ev recorded on the main stream, the main stream waits for their join events
+    cudaStream_t side_stream[2] = { nullptr, nullptr };
+    cudaEvent_t fork_ev = nullptr, join_ev[2] = { nullptr, nullptr };
     long long kernel_launches = 0;
 
     FusedState *fused = nullptr;

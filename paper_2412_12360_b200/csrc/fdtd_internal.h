@@ -111,6 +111,10 @@ void launch_record(const Dims &G, const RecLayout &R, const float *fields_H, con
 // ping-pong variants for the fused path (buffers picked by step parity inside the kernel)
 void launch_record_pp(const Dims &G, const RecLayout &R, const float *bufA, const float *bufB, float *rec,
                       const int *step, cudaStream_t st);
+void launch_record_pipe(const Dims &G, const RecLayout &R, const float *bufA, const float *bufB, float *rec,
+                        const int *step, int n_steps, cudaStream_t st);
+void launch_inject_pipe(const Dims &G, const RecLayout &R, float *bufA, float *bufB, const float *rec,
+                        const int *step, cudaStream_t st);
 void launch_inject_pp(const Dims &G, const RecLayout &R, float *bufA, float *bufB, const float *rec,
                       const int *step, cudaStream_t st);
 void launch_inject(const Dims &G, const RecLayout &R, float *fields, const float *rec, const int *step, cudaStream_t st);

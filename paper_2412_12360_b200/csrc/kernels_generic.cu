@@ -201,6 +201,72 @@ __global__ void k_record(Dims G, RecLayout R, const float *__restrict__ fH, cons
     }
 }
 
+// Pipelined recorder of the fused path: runs beside forward step n and reads the buffer that step reads
+// (n&1): pre-step H at lo-1 -> rec[n] (n < n_steps), E' at hi, written by step n-1, -> rec[n-1] (n >= 1).
+// 128 threads x <= 32 registers and no shared memory, so a block fits beside a resident k_step CTA.
+__global__ void __launch_bounds__(128, 16) k_record_pipe(Dims G, RecLayout R, const float *__restrict__ A,
+                                                         const float *__restrict__ B, float *__restrict__ rec,
+                                                         const int *__restrict__ step, int n_steps)
+{
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= R.stride) return;
+    const int n = *step;
+    const float *f = (n & 1) ? B : A;
+    int a = 0, side = 0, which = 0;
+    long long local = -1;
+#pragma unroll
+    for (int aa = 0; aa < 3; ++aa)
+#pragma unroll
+        for (int ss = 0; ss < 2; ++ss)
+#pragma unroll
+            for (int ww = 0; ww < 2; ++ww) {
+                const long long o = R.off[aa][ss][ww];
+                if (t >= o && t < o + R.cells[aa]) { a = aa; side = ss; which = ww; local = t - o; }
+            }
+    if (local < 0) return;   // padding
+    if (side ? n < 1 : n >= n_steps) return;
+    const int fa = R.fast[a], sl = R.slow[a];
+    const int nf = G.hi[fa] - G.lo[fa];
+    int pos[3];
+    pos[a] = side ? G.hi[a] : G.lo[a] - 1;
+    pos[fa] = G.lo[fa] + (int)(local % nf);
+    pos[sl] = G.lo[sl] + (int)(local / nf);
+    const int comp = (a + 1 + which) % 3;
+    const long long p = lin(G, pos[0], pos[1], pos[2]);
+    rec[(long long)(side ? n - 1 : n) * R.stride + t] = __ldg(f + (side ? comp : 3 + comp) * G.nc + p);
+}
+
+// Face injection of the fused reverse sweep, run beside adjoint step n: rec[n] -> buffer (n+1)&1, the volume
+// the inverse step n reads (pre-step H at lo-1, E' at hi).  Sized like k_record_pipe to fit beside a k_step CTA.
+__global__ void __launch_bounds__(128, 16) k_inject_pipe(Dims G, RecLayout R, float *__restrict__ A, float *__restrict__ B,
+                                                         const float *__restrict__ rec, const int *__restrict__ step)
+{
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= R.stride) return;
+    const int n = *step;
+    float *f = (n & 1) ? A : B;
+    int a = 0, side = 0, which = 0;
+    long long local = -1;
+#pragma unroll
+    for (int aa = 0; aa < 3; ++aa)
+#pragma unroll
+        for (int ss = 0; ss < 2; ++ss)
+#pragma unroll
+            for (int ww = 0; ww < 2; ++ww) {
+                const long long o = R.off[aa][ss][ww];
+                if (t >= o && t < o + R.cells[aa]) { a = aa; side = ss; which = ww; local = t - o; }
+            }
+    if (local < 0) return;   // padding
+    const int fa = R.fast[a], sl = R.slow[a];
+    const int nf = G.hi[fa] - G.lo[fa];
+    int pos[3];
+    pos[a] = side ? G.hi[a] : G.lo[a] - 1;
+    pos[fa] = G.lo[fa] + (int)(local % nf);
+    pos[sl] = G.lo[sl] + (int)(local / nf);
+    const int comp = (a + 1 + which) % 3;
+    f[(side ? comp : 3 + comp) * G.nc + lin(G, pos[0], pos[1], pos[2])] = __ldg(rec + (long long)n * R.stride + t);
+}
+
 __global__ void k_advance(int *step, int delta) { *step += delta; }
 // the step counter lives in two slots that alternate between steps: nobody reads `out` during the step that writes it
 __global__ void k_next_step(const int *in, int *out, int delta) { *out = *in + delta; }
@@ -434,6 +500,20 @@ void launch_record_pp(const Dims &G, const RecLayout &R, const float *bufA, cons
 {
     if (R.stride == 0) return;
     k_record<false, true><<<(unsigned)((R.stride + 255) / 256), 256, 0, st>>>(G, R, bufA, bufB, nullptr, rec, step);
+}
+
+void launch_record_pipe(const Dims &G, const RecLayout &R, const float *bufA, const float *bufB, float *rec,
+                        const int *step, int n_steps, cudaStream_t st)
+{
+    if (R.stride == 0) return;
+    k_record_pipe<<<(unsigned)((R.stride + 127) / 128), 128, 0, st>>>(G, R, bufA, bufB, rec, step, n_steps);
+}
+
+void launch_inject_pipe(const Dims &G, const RecLayout &R, float *bufA, float *bufB, const float *rec,
+                        const int *step, cudaStream_t st)
+{
+    if (R.stride == 0) return;
+    k_inject_pipe<<<(unsigned)((R.stride + 127) / 128), 128, 0, st>>>(G, R, bufA, bufB, rec, step);
 }
 
 void launch_inject_pp(const Dims &G, const RecLayout &R, float *bufA, float *bufB, const float *rec,

@@ -264,10 +264,11 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
     uint64_t *full = reinterpret_cast<uint64_t *>(smem + (size_t)P.nst * P.stage + C::RING_BYTES);
     uint64_t *empty = full + MAX_ST;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int n = *P.step;
-    const int par = (n + (ADJ ? 1 : 0)) & 1;       // forward step n reads buffer n&1; reverse step n reads (n+1)&1
     constexpr int FA = ADJ ? 1 : 0, FB = ADJ ? 0 : 1;   // CPML family (tables, states) of phase A / phase B
     const int nst = P.nst;
+    // programmatic dependent launch: the next step kernel may be placed on an SM as soon as this CTA has left it;
+    // its prologue (tables, barriers) touches nothing a step writes and it waits below before it reads the counter
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
     // CPML tables of the slab cells in shared memory, indexed by slab-compact coordinate:
     // [family][b, a, 1/kappa - 1][x: 2 dpx | y: 2 d | z: 2 d]
@@ -288,6 +289,11 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
     if (threadIdx.x == 0) {
         for (int s = 0; s < nst; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], C::NCW); }
         fence_mbar_init();
+    }
+    asm volatile("griddepcontrol.wait;" ::: "memory");   // everything the previous launches wrote is visible from here on
+    const int n = *P.step;
+    const int par = (n + (ADJ ? 1 : 0)) & 1;       // forward step n reads buffer n&1; reverse step n reads (n+1)&1
+    if (threadIdx.x == 0) {
         if (blockIdx.x == 0 && P.step_next) *P.step_next = n + P.step_delta;
         if (P.dbg_t) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); P.dbg_t[2 * blockIdx.x] = t; }
     }
@@ -663,6 +669,7 @@ struct InvParams {
     float *buf[2];                 // primal ping-pong volumes
     float *grad;                   // dL/d inv_eps, accumulated
     const int *step;
+    int bias, n_steps;             // this launch inverts step n = *step + bias; nothing to do if n >= n_steps (see enqueue_bwd)
     int nst, stage;
     int n_src;
     int sEl, sEh, sHl, sHh;
@@ -692,7 +699,8 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_inverse(const __grid_constant
     uint64_t *full = reinterpret_cast<uint64_t *>(smem + (size_t)P.nst * P.stage + C::RING_BYTES);
     uint64_t *empty = full + MAX_ST;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int n = *P.step;
+    const int n = *P.step + P.bias;
+    if (n >= P.n_steps) return;
     const int rd = (n + 1) & 1, wv = n & 1;
     const int nst = P.nst;
 
@@ -910,14 +918,20 @@ template <class C> cudaError_t set_smem_inv_impl(size_t smem)
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_inverse<C>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     return e;
 }
-template <class C> void launch_fwd_impl(const StepParams &P, int n_cta, size_t smem, cudaStream_t st)
+// step kernels are launched with programmatic stream serialisation (see the top of k_step)
+template <class C, bool ADJ> void launch_step_impl(const StepParams &P, int n_cta, size_t smem, cudaStream_t st)
 {
-    k_step<C, false><<<n_cta, C::THREADS, smem, st>>>(P);
+    static const bool pdl = !getenv("FDTD_NO_PDL");
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(n_cta); cfg.blockDim = dim3(C::THREADS); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+    cudaLaunchKernelEx(&cfg, k_step<C, ADJ>, P);
 }
-template <class C> void launch_adj_impl(const StepParams &P, int n_cta, size_t smem, cudaStream_t st)
-{
-    k_step<C, true><<<n_cta, C::THREADS, smem, st>>>(P);
-}
+template <class C> void launch_fwd_impl(const StepParams &P, int n_cta, size_t smem, cudaStream_t st) { launch_step_impl<C, false>(P, n_cta, smem, st); }
+template <class C> void launch_adj_impl(const StepParams &P, int n_cta, size_t smem, cudaStream_t st) { launch_step_impl<C, true>(P, n_cta, smem, st); }
 template <class C> cudaError_t set_smem_impl(size_t smem)
 {
     cudaError_t e = cudaFuncSetAttribute(k_step<C, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -941,6 +955,11 @@ constexpr int kNumTiles = sizeof(kTiles) / sizeof(kTiles[0]);
 struct FusedState {
     const TileImpl *tile = nullptr;
     int TX = 0, TY = 0, nst = 0, n_cta = 0, n_rot = 1;
+    // pipelined reverse sweep (enqueue_bwd): the adjoint step runs on n_adj CTAs beside the inverse step of the
+    // step before it on n_inv_p CTAs (n_adj + n_inv_p = number of SMs); n_inv_p = 0: one kernel after the other
+    int n_adj = 0, n_inv_p = 0;
+    Segment *d_isegs_p = nullptr;
+    int *d_iseg_begin_p = nullptr;
     size_t smem = 0;
     StepParams sp{};
     // inverse step kernel: its own tile shape and segment table (interior box only)
@@ -1264,9 +1283,46 @@ int fused_setup(fdtd_grid *g)
             InvParams &I = F->ip;
             I.G = G; I.segs = F->d_isegs; I.seg_begin = F->d_iseg_begin; I.step = g->d_step;
             I.nst = ib_nst; I.stage = istage;
+            I.bias = 0; I.n_steps = 1 << 30;
             if (ib->set_smem_inv(F->ismem) != cudaSuccess) { (void)cudaGetLastError(); F->itile = nullptr; }
+
+            // ---- pipelined reverse sweep (opt-in, FDTD_PIPELINE_REVERSE=1; measured on C3: no gain, 134.6 vs 133.8 us per
+            // reverse step, because both kernels are bound by per-SM latency, not by DRAM): SMs split between the adjoint
+            // step and the inverse step by their bytes, the inverse step's weighted 1.3
+            F->n_adj = n_cta;
+            if (F->itile && n_cta == n_sm && getenv("FDTD_PIPELINE_REVERSE")) {
+                const double slab = 2.0 * G.d * ((double)G.ny * G.nz + (double)G.nx * G.nz + (double)G.nx * G.ny);
+                const double b_adj = 52.0 * G.nc + 32.0 * slab;
+                const double gcells = (double)(G.ghi[0] - G.glo[0]) * (G.ghi[1] - G.glo[1]) * (G.ghi[2] - G.glo[2]);
+                const double b_inv = 1.3 * (64.0 * (double)(G.hi[0] - G.lo[0]) * ny_i * nz_i + 8.0 * gcells);
+                int k = (int)std::lround(n_sm * b_inv / (b_adj + b_inv));
+                if (const char *e = getenv("FDTD_INV_CTAS")) k = atoi(e);
+                k = std::max(1, std::min(k, n_sm / 2));
+                if (itotal >= 4LL * k && total >= 8LL * (n_sm - k)) {
+                    std::vector<Segment> psegs;
+                    std::vector<int> pbeg;
+                    segments_from_runs(nty, nz_i, ib->TX, ib->TY, x0, G.lo[1], G.lo[2],
+                                       make_runs(std::vector<double>((size_t)itotal, 1.0), nz_i, k), psegs, pbeg);
+                    if ((rc = g->alloc((void **)&F->d_isegs_p, psegs.size() * sizeof(Segment)))) return rc;
+                    if ((rc = g->alloc((void **)&F->d_iseg_begin_p, pbeg.size() * sizeof(int)))) return rc;
+                    if (cudaMemcpy(F->d_isegs_p, psegs.data(), psegs.size() * sizeof(Segment), cudaMemcpyHostToDevice) != cudaSuccess ||
+                        cudaMemcpy(F->d_iseg_begin_p, pbeg.data(), pbeg.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess) {
+                        (void)cudaGetLastError();
+                        return fdtd_fail(FDTD_ECUDA, "upload of the inverse segment table failed");
+                    }
+                    F->n_inv_p = k; F->n_adj = n_sm - k;
+                    const int nty_s = (G.ny + F->TY - 1) / F->TY;
+                    segments_from_runs(nty_s, G.nz, F->TX, F->TY, 0, 0, 0, make_runs(model_cost(G, F->TX, F->TY, wy, wz), G.nz, F->n_adj), all, begins);
+                    if (cudaMemcpy(F->d_segs[1], all.data(), all.size() * sizeof(Segment), cudaMemcpyHostToDevice) != cudaSuccess ||
+                        cudaMemcpy(F->d_seg_begin[1], begins.data(), begins.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess) {
+                        (void)cudaGetLastError();
+                        return fdtd_fail(FDTD_ECUDA, "upload of the segment table failed");
+                    }
+                }
+            }
         }
     }
+    if (F->n_adj == 0) F->n_adj = n_cta;
 
     // ---- kernel parameters that do not depend on the call -----------------------------------------------------------
     StepParams &P = F->sp;
@@ -1398,13 +1454,14 @@ static int calibrate(fdtd_grid *g)
     P.sEl = P.sHl = P.dEl = P.dHl = 1 << 30; P.sEh = P.sHh = P.dEh = P.dHh = -1;
     P.cs = nullptr;
     P.dbg_t = F->d_cta_t;
-    const int n_cta = F->n_cta;
-    std::vector<unsigned long long> t(2 * (size_t)n_cta);
+    std::vector<unsigned long long> t(2 * (size_t)F->n_cta);
     std::vector<Segment> segs;
     std::vector<int> begins;
     const int nty = (G.ny + F->TY - 1) / F->TY;
     const std::vector<int> cls = column_classes(G, F->TX, F->TY);
     for (int mode = 0; mode < 2; ++mode) {
+        const int n_cta = mode ? F->n_adj : F->n_cta;
+        P.n_cta = n_cta;
         std::vector<double> w = model_cost(G, F->TX, F->TY, 1.0, 0.8);
         Runs runs = make_runs(w, G.nz, n_cta), best_runs = runs;
         double best = 1e30;
@@ -1419,7 +1476,7 @@ static int calibrate(fdtd_grid *g)
                 if (mode) F->tile->launch_adj(P, n_cta, F->smem, 0); else F->tile->launch_fwd(P, n_cta, F->smem, 0);
             }
             if (cudaDeviceSynchronize() != cudaSuccess ||
-                cudaMemcpy(t.data(), F->d_cta_t, t.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost) != cudaSuccess) {
+                cudaMemcpy(t.data(), F->d_cta_t, 2 * (size_t)n_cta * sizeof(unsigned long long), cudaMemcpyDeviceToHost) != cudaSuccess) {
                 cudaError_t e = cudaGetLastError();
                 return done(fdtd_fail(FDTD_ECUDA, std::string("calibration launch: ") + cudaGetErrorString(e)));
             }
@@ -1456,9 +1513,28 @@ int fdtd_run_steps_bwd(fdtd_grid *g, const std::string &key, int n_steps, int la
                        void (*enqueue)(void *, cudaStream_t), void *ctx);
 
 namespace {
+// fork: the side streams wait for what the main stream has enqueued so far; join: the main stream waits for them.
+// While profiling everything stays on the main stream's timeline between the two events of the caller's ProfScope
+// (the side streams still run concurrently: the span measures the group).
+void fork_side(fdtd_grid *g, cudaStream_t cs, int n_side)
+{
+    cudaEventRecord(g->fork_ev, cs);
+    for (int q = 0; q < n_side; ++q) cudaStreamWaitEvent(g->side_stream[q], g->fork_ev, 0);
+}
+void join_side(fdtd_grid *g, cudaStream_t cs, int n_side)
+{
+    for (int q = 0; q < n_side; ++q) {
+        cudaEventRecord(g->join_ev[q], g->side_stream[q]);
+        cudaStreamWaitEvent(cs, g->join_ev[q], 0);
+    }
+}
+
 struct FwdCtx {
-    fdtd_grid *g; StepParams P; bool recording; float *A; float *B;
+    fdtd_grid *g; StepParams P; bool recording; float *A; float *B; int n_steps;
 };
+// forward step n; with the recorder on, k_record_pipe runs beside it on a side stream: both only read buffer n&1
+// (pre-step H of step n -> rec[n], E' of step n-1 -> rec[n-1]); the step after next overwrites that buffer, so the
+// join comes before the next step.  fused_forward() adds the last E' record after the loop.
 void enqueue_fwd(void *vctx, cudaStream_t cs)
 {
     FwdCtx *c = (FwdCtx *)vctx;
@@ -1466,36 +1542,60 @@ void enqueue_fwd(void *vctx, cudaStream_t cs)
     FusedState *F = g->fused;
     StepParams Q = c->P;
     Q.step = g->step_in(); Q.step_next = g->step_out(); Q.step_delta = 1;
-    { ProfScope p(g, fdtd_grid::PC_FUSED_FWD, cs);
-      F->tile->launch_fwd(Q, F->n_cta, F->smem, cs); }
+    ProfScope p(g, fdtd_grid::PC_FUSED_FWD, cs);
     if (c->recording) {
-        // step n read buffer n&1 (pre-step H) and wrote buffer (n+1)&1 (E'); the record kernel picks them by parity
-        ProfScope p(g, fdtd_grid::PC_RECORD, cs);
-        launch_record_pp(g->G, g->R, c->A, c->B, g->rec, g->step_in(), cs);
+        fork_side(g, cs, 1);
+        launch_record_pipe(g->G, g->R, c->A, c->B, g->rec, g->step_in(), c->n_steps, g->side_stream[0]);
     }
+    F->tile->launch_fwd(Q, F->n_cta, F->smem, cs);
+    if (c->recording) join_side(g, cs, 1);
 }
 
 struct BwdCtx {
-    fdtd_grid *g; StepParams P; InvParams I; bool fused_inv; bool fused_det; float *bufB; float *fields; const float *ie; float *grad; float *lamA; float *lamB;
+    fdtd_grid *g; StepParams P; InvParams I; bool fused_inv; bool fused_det; bool pipelined; float *bufB; float *fields; const float *ie; float *grad; float *lamA; float *lamB;
     const std::vector<SourceDev> *S; const std::vector<DetectorDev> *D; int total_freq;
 };
-// reverse step n: B1 (detector cotangents into the volume about to be read), B2+B5 (fused adjoint step),
-// then the primal inverse step B3+B4 with lamE' taken from the volume the adjoint step just wrote
+// Reverse step n.  One kernel after the other: B1 (detector cotangents into the volume about to be read), B2+B5
+// (fused adjoint step), face injection, then the primal inverse step B3+B4 with lamE' taken from the volume the
+// adjoint step just wrote.
+// Pipelined (c->pipelined): launch n runs, side by side on disjoint SMs, the adjoint step n (n_adj CTAs), the
+// inverse step n+1 (n_inv_p CTAs; nothing at the first launch) and the face injection for step n.  All three
+// depend only on launch n+1: inverse step n+1 reads primal volume n&1 and the lamE' that adjoint step n+1 wrote
+// into cotangent volume (n+1)&1 (adjoint step n only reads it) and writes the box of primal volume (n+1)&1; the
+// injection for step n writes cells outside the box of that same volume.  fused_backward() adds inverse step 0.
 void enqueue_bwd(void *vctx, cudaStream_t cs)
 {
     BwdCtx *c = (BwdCtx *)vctx;
     fdtd_grid *g = c->g;
     FusedState *F = g->fused;
     const Dims &G = g->G;
+    StepParams Q = c->P;
+    Q.step = g->step_in(); Q.step_next = g->step_out(); Q.step_delta = -1;
+    if (c->pipelined) {
+        ProfScope p(g, fdtd_grid::PC_FUSED_BWD, cs);
+        const int n_side = G.d > 0 ? 2 : 1;
+        fork_side(g, cs, n_side);
+        InvParams J = c->I;
+        J.step = g->step_in();
+        F->itile->launch_inv(J, F->n_inv_p, F->ismem, g->side_stream[0]);
+        if (G.d > 0) launch_inject_pipe(G, g->R, c->fields, c->bufB, g->rec, g->step_in(), g->side_stream[1]);
+        F->tile->launch_adj(Q, F->n_adj, F->smem, cs);
+        join_side(g, cs, n_side);
+        return;
+    }
     if (!c->fused_det) { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
       for (const DetectorDev &dt : *c->D)
           if (dt.phasor) launch_detector_adjoint_pp(G, c->lamA, c->lamB, dt, g->d_cs, c->total_freq, g->step_in(), cs); }
-    StepParams Q = c->P;
-    Q.step = g->step_in(); Q.step_next = g->step_out(); Q.step_delta = -1;
+    // the face injection (it writes cells of the primal volume, which the adjoint step never touches) runs beside it
+    const bool side_inject = c->fused_inv && G.d > 0;
     { ProfScope p(g, fdtd_grid::PC_FUSED_BWD, cs);
-      F->tile->launch_adj(Q, F->n_cta, F->smem, cs); }
+      if (side_inject) {
+          fork_side(g, cs, 1);
+          launch_inject_pipe(G, g->R, c->fields, c->bufB, g->rec, g->step_in(), g->side_stream[0]);
+      }
+      F->tile->launch_adj(Q, F->n_adj, F->smem, cs);
+      if (side_inject) join_side(g, cs, 1); }
     if (c->fused_inv) {
-        if (G.d > 0) { ProfScope p(g, fdtd_grid::PC_INJECT, cs); launch_inject_pp(G, g->R, c->fields, c->bufB, g->rec, g->step_in(), cs); }
         InvParams J = c->I;
         J.step = g->step_in();
         { ProfScope p(g, fdtd_grid::PC_FUSED_INV, cs); F->itile->launch_inv(J, F->in_cta, F->ismem, cs); }
@@ -1523,7 +1623,7 @@ int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float
     if (rc) return rc;
     for (int q = 0; q < 2; ++q)
         if ((rc = g->zero_psi(g->psiE[q], st)) || (rc = g->zero_psi(g->psiH[q], st))) return rc;
-    FwdCtx ctx{ g, F->sp, recording, fields, F->bufB };
+    FwdCtx ctx{ g, F->sp, recording, fields, F->bufB, n_steps };
     StepParams &P = ctx.P;
     P.maps = F->d_maps[0];
     P.buf[0] = fields; P.buf[1] = F->bufB;
@@ -1545,8 +1645,14 @@ int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float
     std::string key("ff");
     key.append((const char *)&P, sizeof(P));
     key.push_back(recording ? 1 : 0);
+    key.append((const char *)&n_steps, recording ? sizeof(n_steps) : 0);
     rc = fdtd_run_steps_fwd(g, key, n_steps, 1 + (recording ? 1 : 0), st, enqueue_fwd, &ctx);
     if (rc) return rc;
+    if (recording) {      // E' of the last step; step p read counter slot p&1, so the count n_steps sits in slot n_steps&1
+        ProfScope p(g, fdtd_grid::PC_RECORD, st);
+        launch_record_pipe(g->G, g->R, fields, F->bufB, g->rec, g->d_step + (n_steps & 1), n_steps, st);
+        g->kernel_launches += 1;
+    }
     if (n_steps & 1) {
         cudaError_t e = cudaMemcpyAsync(fields, F->bufB, (size_t)g->G.nc * 6 * sizeof(float), cudaMemcpyDeviceToDevice, st);
         if (e != cudaSuccess) { (void)cudaGetLastError(); return fdtd_fail(FDTD_ECUDA, cudaGetErrorString(e)); }
@@ -1574,7 +1680,8 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     // B1 inside the adjoint kernel when every detector with a cotangent is on E components (else a kernel per detector)
     bool fused_det = (int)D.size() <= MAX_DET;
     for (const DetectorDev &dt : D) if (dt.phasor && (dt.mask >> 3)) fused_det = false;
-    BwdCtx ctx{ g, F->sp, F->ip, fused_inv, fused_det, F->bufB, fields, inv_eps, dL_dinv_eps, g->lam, F->lamB, &S, &D, total_freq };
+    const bool pipelined = fused_inv && fused_det && F->n_inv_p > 0;
+    BwdCtx ctx{ g, F->sp, F->ip, fused_inv, fused_det, pipelined, F->bufB, fields, inv_eps, dL_dinv_eps, g->lam, F->lamB, &S, &D, total_freq };
     if (fused_inv) {
         // reverse step n reads primal volume (n+1)&1 and writes n&1: state n_steps must sit in volume n_steps&1
         if ((rc = build_inv_maps(g, fields, F->bufB, inv_eps, g->lam, F->lamB, st))) return rc;
@@ -1592,6 +1699,7 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
             if (S[q].comp < 3) { I.sEl = std::min(I.sEl, S[q].lo[2]); I.sEh = std::max(I.sEh, S[q].hi[2]); }
             else { I.sHl = std::min(I.sHl, S[q].lo[2]); I.sHh = std::max(I.sHh, S[q].hi[2]); }
         }
+        if (pipelined) { I.segs = F->d_isegs_p; I.seg_begin = F->d_iseg_begin_p; I.bias = 1; I.n_steps = n_steps; }
     }
     StepParams &P = ctx.P;
     P.maps = F->d_maps[1];
@@ -1618,5 +1726,15 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     key.append((const char *)&dL_dinv_eps, sizeof(dL_dinv_eps));
     if (!S.empty()) key.append((const char *)S.data(), S.size() * sizeof(SourceDev));
     if (!D.empty()) key.append((const char *)D.data(), D.size() * sizeof(DetectorDev));
-    return fdtd_run_steps_bwd(g, key, n_steps, fused_inv ? 2 + (fused_det ? 0 : n_adj) + (g->G.d > 0 ? 1 : 0) : 3 + (fused_det ? 0 : n_adj) + (int)S.size() + (g->G.d > 0 ? 1 : 0), st, enqueue_bwd, &ctx);
+    const int n_inj = g->G.d > 0 ? 1 : 0;
+    const int launches = fused_inv ? 2 + (fused_det ? 0 : n_adj) + n_inj : 3 + (fused_det ? 0 : n_adj) + (int)S.size() + n_inj;
+    rc = fdtd_run_steps_bwd(g, key, n_steps, launches, st, enqueue_bwd, &ctx);
+    if (rc || !pipelined) return rc;
+    // inverse step 0 on every SM; reverse step p read counter slot p&1 (p counted from the end), so -1 sits in slot n_steps&1
+    InvParams J = ctx.I;
+    J.segs = F->d_isegs; J.seg_begin = F->d_iseg_begin;
+    J.step = g->d_step + (n_steps & 1);
+    { ProfScope p(g, fdtd_grid::PC_FUSED_INV, st); F->itile->launch_inv(J, F->in_cta, F->ismem, st); }
+    g->kernel_launches += 1;
+    return FDTD_OK;
 }
