@@ -191,6 +191,17 @@ typedef struct {
 FDTD_API int fdtd_set_profiling(fdtd_grid *grid, int32_t enable);
 FDTD_API int fdtd_get_profile(fdtd_grid *grid, fdtd_profile *out);
 
+/* Host-only introspection of the fused step kernels' work partition (no device work, no
+ * grid needed): the (tile column, plane) sequence of an nx x ny x nz grid with d CPML cells, tiles of
+ * tile_x x tile_y cells, split into n_cta runs of equal model cost (a plane of a tile costs 1, + wy if the tile
+ * has rows in a y slab, + wz if the plane is in a z slab).  lockstep != 0: the lock-step split (columns of one
+ * cost class get identical cuts); 0: the plain contiguous split.  Writes up to `cap` segments as
+ * {cta, i0, j0, k0, k1} (cells [i0, i0+tile_x) x [j0, j0+tile_y) clipped to the grid, planes [k0, k1)) into
+ * `segments` (HOST, caller-owned, 5 int32 each), in marching order per CTA, and returns the number of segments
+ * of the partition (which may exceed cap), or a negative FDTD_E* code for bad arguments. */
+FDTD_API int fdtd_debug_partition(int32_t nx, int32_t ny, int32_t nz, int32_t d, int32_t tile_x, int32_t tile_y,
+                         int32_t n_cta, double wy, double wz, int32_t lockstep, int32_t *segments, int32_t cap);
+
 /* Library version string, e.g. "fdtd-b200 0.1 sm_100a". */
 FDTD_API const char *fdtd_version(void);
 

@@ -58,7 +58,7 @@ class fdtd_profile(C.Structure):
 
 
 EXPORTS = ("fdtd_grad_rho", "fdtd_set_profiling", "fdtd_get_profile", "fdtd_create_grid", "fdtd_forward", "fdtd_backward", "fdtd_destroy", "fdtd_last_error",
-           "fdtd_get_info", "fdtd_version", "fdtd_forward_host", "fdtd_backward_host")
+           "fdtd_get_info", "fdtd_version", "fdtd_forward_host", "fdtd_backward_host", "fdtd_debug_partition")
 
 
 def _load():
@@ -110,6 +110,18 @@ def fdtd_last_error() -> str:
 
 def fdtd_version() -> str:
     return _L.fdtd_version().decode()
+
+
+def fdtd_debug_partition(nx, ny, nz, d, tile_x, tile_y, n_cta, wy=1.0, wz=0.8, lockstep=True):
+    """Host-only: the step kernels' work partition as a list of (cta, i0, j0, k0, k1) (include/fdtd.h)."""
+    _L.fdtd_debug_partition.restype = C.c_int
+    _L.fdtd_debug_partition.argtypes = [C.c_int32] * 7 + [C.c_double, C.c_double, C.c_int32, C.POINTER(C.c_int32), C.c_int32]
+    n = _L.fdtd_debug_partition(nx, ny, nz, d, tile_x, tile_y, n_cta, wy, wz, int(bool(lockstep)), None, 0)
+    if n < 0:
+        raise FdtdError(n, fdtd_last_error())
+    buf = (C.c_int32 * (5 * n))()
+    _L.fdtd_debug_partition(nx, ny, nz, d, tile_x, tile_y, n_cta, wy, wz, int(bool(lockstep)), buf, n)
+    return [tuple(buf[5 * q:5 * q + 5]) for q in range(n)]
 
 
 def _check(rc: int):

@@ -1123,10 +1123,67 @@ Runs lockstep_runs(const std::vector<double> &w, int nz, int n_cta)
     return runs;
 }
 
+// Large grids: more columns than CTAs.  Whole columns are dealt out in waves (CTA c takes columns c, c + n_cta,
+// ...): every CTA starts a column at plane 0 at time 0, so the n_cta y-consecutive columns of a wave are marched in
+// lock step.  The columns that do not fill a wave form a pool that is cut, in sequence order, into one chunk per
+// CTA sized so that every CTA ends up with the same total cost (a CTA whose whole columns already cost more gets
+// nothing from the pool).
+Runs wave_runs(const std::vector<double> &w, int nz, int n_cta)
+{
+    const long long n_col = (long long)w.size() / nz;
+    std::vector<double> colw(n_col, 0.0);
+    double total = 0.0;
+    for (long long t = 0; t < n_col; ++t) { for (int k = 0; k < nz; ++k) colw[t] += w[t * nz + k]; total += colw[t]; }
+    // as many full waves as the pool can still level out (columns in CPML slabs cost about twice the others)
+    long long waves = n_col / n_cta;
+    std::vector<double> used(n_cta, 0.0);
+    for (; waves >= 1; --waves) {
+        std::fill(used.begin(), used.end(), 0.0);
+        for (long long t = 0; t < waves * n_cta; ++t) used[t % n_cta] += colw[t];
+        if (*std::max_element(used.begin(), used.end()) <= total / n_cta * (1.0 + 1e-9)) break;
+    }
+    if (waves < 1) return lockstep_runs(w, nz, n_cta);
+    Runs runs(n_cta);
+    for (long long t = 0; t < waves * n_cta; ++t) runs[t % n_cta].push_back({ t * nz, (t + 1) * nz });
+    const long long q0 = waves * n_cta * nz, q1 = n_col * nz;
+    if (q0 == q1) return runs;
+    double pool = 0.0;
+    for (long long q = q0; q < q1; ++q) pool += w[q];
+    // level: sum_c max(0, level - used[c]) = pool
+    std::vector<double> u(used);
+    std::sort(u.begin(), u.end());
+    double level = u[0] + pool, below = 0.0;
+    for (int m = 1; m <= n_cta; ++m) {           // the m cheapest CTAs share the pool
+        below += u[m - 1];
+        level = (pool + below) / m;
+        if (m == n_cta || level <= u[m]) break;
+    }
+    long long q = q0;
+    double acc = 0.0, target = 0.0;
+    for (int c = 0; c < n_cta && q < q1; ++c) {
+        const double budget = std::max(0.0, level - used[c]);
+        if (budget <= 0.0) continue;
+        target += budget;
+        long long e = q;
+        while (e < q1 && (acc + w[e] <= target + 1e-9 * target || e == q)) acc += w[e++];
+        bool later = false;                      // the last CTA with a budget takes what is left
+        for (int c2 = c + 1; c2 < n_cta; ++c2) later |= level - used[c2] > 0.0;
+        if (!later) { while (e < q1) acc += w[e++]; }
+        for (long long a = q; a < e;) {
+            const long long b = std::min(e, (a / nz + 1) * nz);
+            runs[c].push_back({ a, b });
+            a = b;
+        }
+        q = e;
+    }
+    return runs;
+}
+
 Runs make_runs(const std::vector<double> &w, int nz, int n_cta)
 {
     static const bool contiguous = getenv("FDTD_PARTITION") && !strcmp(getenv("FDTD_PARTITION"), "contiguous");
-    return contiguous ? contiguous_runs(w, nz, n_cta) : lockstep_runs(w, nz, n_cta);
+    if (contiguous) return contiguous_runs(w, nz, n_cta);
+    return (long long)w.size() / nz >= n_cta ? wave_runs(w, nz, n_cta) : lockstep_runs(w, nz, n_cta);
 }
 
 // origin (i_org, j_org, k_org) of the tiled box; nz planes per column
@@ -1149,6 +1206,29 @@ void segments_from_runs(int nty, int nz, int TX, int TY, int i_org, int j_org, i
 }
 
 }  // namespace
+
+extern "C" int fdtd_debug_partition(int32_t nx, int32_t ny, int32_t nz, int32_t d, int32_t tile_x, int32_t tile_y,
+                                    int32_t n_cta, double wy, double wz, int32_t lockstep, int32_t *segments, int32_t cap)
+{
+    if (nx < 1 || ny < 1 || nz < 1 || d < 0 || tile_x < 1 || tile_y < 1 || n_cta < 1 || cap < 0 || (cap > 0 && !segments))
+        return fdtd_fail(FDTD_EINVAL, "fdtd_debug_partition: bad argument");
+    Dims G{};
+    G.nx = nx; G.ny = ny; G.nz = nz; G.d = d;
+    const int nty = (ny + tile_y - 1) / tile_y, ntx = (nx + tile_x - 1) / tile_x;
+    if ((long long)ntx * nty * nz < n_cta) return fdtd_fail(FDTD_EINVAL, "fdtd_debug_partition: more CTAs than (tile, plane) positions");
+    const std::vector<double> w = model_cost(G, tile_x, tile_y, wy, wz);
+    const Runs runs = !lockstep ? contiguous_runs(w, nz, n_cta)
+                      : ((long long)ntx * nty >= n_cta ? wave_runs(w, nz, n_cta) : lockstep_runs(w, nz, n_cta));
+    std::vector<Segment> segs;
+    std::vector<int> begins;
+    segments_from_runs(nty, nz, tile_x, tile_y, 0, 0, 0, runs, segs, begins);
+    for (size_t c = 0; c + 1 < begins.size(); ++c)
+        for (int q = begins[c]; q < begins[c + 1] && q < cap; ++q) {
+            int32_t *o = segments + 5 * (size_t)q;
+            o[0] = (int32_t)c; o[1] = segs[q].i0; o[2] = segs[q].j0; o[3] = segs[q].k0; o[4] = segs[q].k1;
+        }
+    return (int)segs.size();
+}
 
 static int calibrate(fdtd_grid *g);
 
@@ -1265,7 +1345,8 @@ int fused_setup(fdtd_grid *g)
             // tiles start at row lo_y (their first halo row is lo_y - 1) and at column x0
             const int ntx = (nx_i + ib->TX - 1) / ib->TX, nty = (ny_i + ib->TY - 1) / ib->TY;
             const long long itotal = (long long)ntx * nty * nz_i;
-            const int in_cta = (int)std::min<long long>(n_sm, std::max<long long>(1, itotal / 6));
+            int in_cta = (int)std::min<long long>(n_sm, std::max<long long>(1, itotal / 6));
+            if (const char *e = getenv("FDTD_INV_NCTA")) in_cta = std::max(1, atoi(e));
             std::vector<Segment> isegs;
             std::vector<int> ibeg;
             segments_from_runs(nty, nz_i, ib->TX, ib->TY, x0, G.lo[1], G.lo[2],
