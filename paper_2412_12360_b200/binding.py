@@ -45,7 +45,8 @@ class fdtd_detector(C.Structure):
 class fdtd_grid_info(C.Structure):
     _fields_ = [("path", C.c_int32), ("tile_x", C.c_int32), ("tile_y", C.c_int32), ("tile_z", C.c_int32),
                 ("kernel_launches", C.c_int64), ("recorder_bytes", C.c_int64), ("scratch_bytes", C.c_int64),
-                ("record_floats_per_step", C.c_int64), ("reserved", C.c_int64 * 4)]
+                ("record_floats_per_step", C.c_int64), ("pipelined_inverse_ctas", C.c_int64),
+                ("reserved", C.c_int64 * 3)]
 
 
 FDTD_PROF_CLASSES = 16

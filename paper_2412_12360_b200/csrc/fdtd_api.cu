@@ -352,6 +352,7 @@ extern "C" int fdtd_get_info(const fdtd_grid *g, fdtd_grid_info *info)
     info->recorder_bytes = g->recorder_bytes;
     info->scratch_bytes = g->scratch_bytes;
     info->record_floats_per_step = g->R.stride;
+    info->pipelined_inverse_ctas = g->pipelined_inverse_ctas;
     return FDTD_OK;
 }
 

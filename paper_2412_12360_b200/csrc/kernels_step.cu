@@ -1392,6 +1392,7 @@ int fused_setup(fdtd_grid *g)
                         return fdtd_fail(FDTD_ECUDA, "upload of the inverse segment table failed");
                     }
                     F->n_inv_p = k; F->n_adj = n_sm - k;
+                    g->pipelined_inverse_ctas = k;
                     const int nty_s = (G.ny + F->TY - 1) / F->TY;
                     segments_from_runs(nty_s, G.nz, F->TX, F->TY, 0, 0, 0, make_runs(model_cost(G, F->TX, F->TY, wy, wz), G.nz, F->n_adj), all, begins);
                     if (cudaMemcpy(F->d_segs[1], all.data(), all.size() * sizeof(Segment), cudaMemcpyHostToDevice) != cudaSuccess ||
