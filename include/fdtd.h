@@ -171,7 +171,7 @@ typedef struct {
     int64_t recorder_bytes;          /* bytes of the interface recorder                              */
     int64_t scratch_bytes;           /* all other device bytes owned by the grid                     */
     int64_t record_floats_per_step;  /* recorder stride in floats                                    */
-    int64_t pipelined_inverse_ctas;  /* CTAs of the inverse step in the opt-in pipelined reverse sweep; 0: off */
+    int64_t pipelined_inverse_ctas;  /* CTAs of the inverse step in the pipelined reverse sweep; 0: sequential */
     int64_t reserved[3];
 } fdtd_grid_info;
 FDTD_API int fdtd_get_info(const fdtd_grid *grid, fdtd_grid_info *info);

@@ -18,7 +18,7 @@ struct fdtd_grid {
     std::string fused_why_not;
     bool fused_backward_ready = false;    // false: fdtd_backward uses the generic reverse kernels
     int graph_unroll = 8;
-    int pipelined_inverse_ctas = 0;       // fused path, FDTD_PIPELINE_REVERSE: CTAs given to the inverse step (0: off)
+    int pipelined_inverse_ctas = 0;       // fused path: CTAs of the inverse step in the pipelined reverse sweep (0: sequential)
 
     // device memory owned by the grid
     std::vector<void *> owned;

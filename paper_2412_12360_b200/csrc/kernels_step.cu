@@ -955,8 +955,8 @@ constexpr int kNumTiles = sizeof(kTiles) / sizeof(kTiles[0]);
 struct FusedState {
     const TileImpl *tile = nullptr;
     int TX = 0, TY = 0, nst = 0, n_cta = 0, n_rot = 1;
-    // pipelined reverse sweep (enqueue_bwd): the adjoint step runs on n_adj CTAs beside the inverse step of the
-    // step before it on n_inv_p CTAs (n_adj + n_inv_p = number of SMs); n_inv_p = 0: one kernel after the other
+    // pipelined reverse sweep (enqueue_bwd): the adjoint step (n_adj CTAs) is launched together with the inverse step
+    // of the step before it (n_inv_p CTAs); n_inv_p = 0: one kernel after the other (see fused_setup)
     int n_adj = 0, n_inv_p = 0;
     Segment *d_isegs_p = nullptr;
     int *d_iseg_begin_p = nullptr;
@@ -1367,11 +1367,20 @@ int fused_setup(fdtd_grid *g)
             I.bias = 0; I.n_steps = 1 << 30;
             if (ib->set_smem_inv(F->ismem) != cudaSuccess) { (void)cudaGetLastError(); F->itile = nullptr; }
 
-            // ---- pipelined reverse sweep (opt-in, FDTD_PIPELINE_REVERSE=1; measured on C3: no gain, 134.6 vs 133.8 us per
-            // reverse step, because both kernels are bound by per-SM latency, not by DRAM): SMs split between the adjoint
-            // step and the inverse step by their bytes, the inverse step's weighted 1.3
+            // ---- pipelined reverse sweep (enqueue_bwd): launch n = {adjoint step n, inverse step n+1, injection n} ------
+            // FDTD_REVERSE_SWEEP = grouped (default): both kernels keep their full grids; they cannot share an SM (shared
+            //   memory), so the CTAs of one follow the CTAs of the other SM by SM without a kernel boundary in between
+            //   (C3: 125.1 vs 134.1 us per reverse step);
+            // = split: disjoint SMs, divided by the kernels' bytes (the inverse step's weighted 1.3; C3: 129.1 us: each
+            //   CTA keeps one ~50 KB stage in flight per plane, so neither kernel gets faster per SM when it owns fewer);
+            // = sequential: one kernel after the other (round-1 checkpoints A-D).
             F->n_adj = n_cta;
-            if (F->itile && n_cta == n_sm && getenv("FDTD_PIPELINE_REVERSE")) {
+            const char *sweep = getenv("FDTD_REVERSE_SWEEP");
+            const bool full = !sweep || !strcmp(sweep, "grouped");
+            if (F->itile && full) {
+                F->n_inv_p = in_cta; F->d_isegs_p = F->d_isegs; F->d_iseg_begin_p = F->d_iseg_begin;
+                g->pipelined_inverse_ctas = in_cta;
+            } else if (F->itile && n_cta == n_sm && !strcmp(sweep, "split")) {
                 const double slab = 2.0 * G.d * ((double)G.ny * G.nz + (double)G.nx * G.nz + (double)G.nx * G.ny);
                 const double b_adj = 52.0 * G.nc + 32.0 * slab;
                 const double gcells = (double)(G.ghi[0] - G.glo[0]) * (G.ghi[1] - G.glo[1]) * (G.ghi[2] - G.glo[2]);
@@ -1379,7 +1388,8 @@ int fused_setup(fdtd_grid *g)
                 int k = (int)std::lround(n_sm * b_inv / (b_adj + b_inv));
                 if (const char *e = getenv("FDTD_INV_CTAS")) k = atoi(e);
                 k = std::max(1, std::min(k, n_sm / 2));
-                if (itotal >= 4LL * k && total >= 8LL * (n_sm - k)) {
+                const int n_adj_p = n_sm - k;
+                if (itotal >= 4LL * k && total >= 8LL * n_adj_p) {
                     std::vector<Segment> psegs;
                     std::vector<int> pbeg;
                     segments_from_runs(nty, nz_i, ib->TX, ib->TY, x0, G.lo[1], G.lo[2],
@@ -1391,7 +1401,7 @@ int fused_setup(fdtd_grid *g)
                         (void)cudaGetLastError();
                         return fdtd_fail(FDTD_ECUDA, "upload of the inverse segment table failed");
                     }
-                    F->n_inv_p = k; F->n_adj = n_sm - k;
+                    F->n_inv_p = k; F->n_adj = n_adj_p;
                     g->pipelined_inverse_ctas = k;
                     const int nty_s = (G.ny + F->TY - 1) / F->TY;
                     segments_from_runs(nty_s, G.nz, F->TX, F->TY, 0, 0, 0, make_runs(model_cost(G, F->TX, F->TY, wy, wz), G.nz, F->n_adj), all, begins);
@@ -1640,8 +1650,9 @@ struct BwdCtx {
 // Reverse step n.  One kernel after the other: B1 (detector cotangents into the volume about to be read), B2+B5
 // (fused adjoint step), face injection, then the primal inverse step B3+B4 with lamE' taken from the volume the
 // adjoint step just wrote.
-// Pipelined (c->pipelined): launch n runs, side by side on disjoint SMs, the adjoint step n (n_adj CTAs), the
-// inverse step n+1 (n_inv_p CTAs; nothing at the first launch) and the face injection for step n.  All three
+// Pipelined (c->pipelined; see fused_setup for the variants): launch n is a group of three kernels without an
+// order among them, the adjoint step n (n_adj CTAs), the inverse step n+1 (n_inv_p CTAs; nothing at the first
+// launch) and the face injection for step n.  All three
 // depend only on launch n+1: inverse step n+1 reads primal volume n&1 and the lamE' that adjoint step n+1 wrote
 // into cotangent volume (n+1)&1 (adjoint step n only reads it) and writes the box of primal volume (n+1)&1; the
 // injection for step n writes cells outside the box of that same volume.  fused_backward() adds inverse step 0.
@@ -1762,7 +1773,8 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     // B1 inside the adjoint kernel when every detector with a cotangent is on E components (else a kernel per detector)
     bool fused_det = (int)D.size() <= MAX_DET;
     for (const DetectorDev &dt : D) if (dt.phasor && (dt.mask >> 3)) fused_det = false;
-    const bool pipelined = fused_inv && fused_det && F->n_inv_p > 0;
+    // while profiling (events around every launch) the kernels run one after the other, so each is timed alone
+    const bool pipelined = fused_inv && fused_det && F->n_inv_p > 0 && !g->profiling;
     BwdCtx ctx{ g, F->sp, F->ip, fused_inv, fused_det, pipelined, F->bufB, fields, inv_eps, dL_dinv_eps, g->lam, F->lamB, &S, &D, total_freq };
     if (fused_inv) {
         // reverse step n reads primal volume (n+1)&1 and writes n&1: state n_steps must sit in volume n_steps&1

@@ -256,27 +256,35 @@ def test_gradient_box_recorder(B):
 
 
 def test_pipelined_reverse_sweep_is_the_same_computation(B, monkeypatch):
-    """FDTD_PIPELINE_REVERSE=1 (opt-in): adjoint step n, inverse step n+1 and the injection
-    for step n in one launch group on disjoint SMs.  Same arithmetic in the same order per cell, so gradient,
-    cotangent and reconstructed state are bit-identical to the default sweep; both match the oracle."""
+    """The reverse sweep is pipelined by default: adjoint step n, inverse step n+1 and the
+    injection for step n form one launch group (FDTD_REVERSE_SWEEP=grouped; =split puts them on disjoint SMs;
+    =sequential is one kernel after the other).  Same arithmetic in the same order per cell, so gradient,
+    cotangent and reconstructed state are bit-identical across the three; all match the oracle."""
     for n_steps, rmode in [(41, 2), (40, 1)]:
         w = wl.c3(n=120, n_steps=n_steps, source_k=38)        # source plane just below the design box (k = 42..78)
         w.loss = "final_E2"
         lo, hi = w.design_lo, w.design_hi
         box = (slice(lo[2], hi[2]), slice(lo[1], hi[1]), slice(lo[0], hi[0]))
         ref = run_oracle(w)
-        monkeypatch.delenv("FDTD_PIPELINE_REVERSE", raising=False)
-        base = run_gpu(B, w, B.FDTD_PATH_FUSED, grad_box=(lo, hi), record_mode=rmode)
-        monkeypatch.setenv("FDTD_PIPELINE_REVERSE", "1")
-        pipe = run_gpu(B, w, B.FDTD_PATH_FUSED, grad_box=(lo, hi), record_mode=rmode)
-        monkeypatch.delenv("FDTD_PIPELINE_REVERSE", raising=False)
-        assert base["info"].pipelined_inverse_ctas == 0 and pipe["info"].pipelined_inverse_ctas > 0
-        assert np.array_equal(pipe["grad"], base["grad"]) and np.array_equal(pipe["lam0"], base["lam0"])
-        for c in range(6):
-            assert np.array_equal(pipe["state0"][c][box], base["state0"][c][box])
         assert np.max(np.abs(ref["grad"][box])) > 0
-        assert relerr(pipe["grad"][box], ref["grad"][box]) <= TOL_GRAD
-        assert relerr(pipe["lam0"], ref["lam0"]) <= TOL_GRAD
+        monkeypatch.setenv("FDTD_REVERSE_SWEEP", "sequential")
+        base = run_gpu(B, w, B.FDTD_PATH_FUSED, grad_box=(lo, hi), record_mode=rmode)
+        assert base["info"].pipelined_inverse_ctas == 0
+        assert relerr(base["grad"][box], ref["grad"][box]) <= TOL_GRAD and relerr(base["lam0"], ref["lam0"]) <= TOL_GRAD
+        seen = []
+        for mode in (None, "split"):
+            if mode:
+                monkeypatch.setenv("FDTD_REVERSE_SWEEP", mode)
+            else:
+                monkeypatch.delenv("FDTD_REVERSE_SWEEP")
+            pipe = run_gpu(B, w, B.FDTD_PATH_FUSED, grad_box=(lo, hi), record_mode=rmode)
+            assert pipe["info"].pipelined_inverse_ctas > 0
+            seen.append(pipe["info"].pipelined_inverse_ctas)
+            assert np.array_equal(pipe["grad"], base["grad"]) and np.array_equal(pipe["lam0"], base["lam0"])
+            for c in range(6):
+                assert np.array_equal(pipe["state0"][c][box], base["state0"][c][box])
+        assert seen[0] != seen[1]                               # two different launch configurations did run
+        monkeypatch.delenv("FDTD_REVERSE_SWEEP", raising=False)
 
 
 def test_c3_full_size_truncated_in_the_bench_configuration(B):
