@@ -309,6 +309,51 @@ def test_c3_full_size_truncated_in_the_bench_configuration(B):
         assert eE <= TOL_FIELD and eH <= TOL_FIELD and eG <= TOL_GRAD and eL <= TOL_GRAD and e0 <= 1e-4
 
 
+def test_c3_full_length_self_consistency(B):
+    """configs[2] exactly as bench.py runs it: 200^3, all 2000 time steps, loss = DFT phasor power on the output
+    plane, record=2, fused kernels with the library's own launch configuration.  The oracle needs minutes for this,
+    so the checks are properties: the directional derivative of the loss along delta = sign(dL/d inv_eps) on the
+    design box by central finite differences against <dL/d inv_eps, delta>, the state reconstructed by 2000
+    inverse steps on the box against its true value 0, and a gradient that vanishes outside the box."""
+    import torch
+    n = 2000
+    w = wl.c3(n_steps=n)
+    lo, hi = w.design_lo, w.design_hi
+    kw = w.grid_kwargs()
+    kw.update(max_steps=n, record=2, grad_lo=lo, grad_hi=hi, path=B.FDTD_PATH_FUSED)
+    g = B.Grid(**kw)
+    assert g.info().path == B.FDTD_PATH_FUSED and g.info().pipelined_inverse_ctas > 0
+    ie = torch.as_tensor(w.inv_eps).cuda()
+    box = (slice(lo[2], hi[2]), slice(lo[1], hi[1]), slice(lo[0], hi[0]))
+    f = torch.zeros((6, w.nz, w.ny, w.nx), dtype=torch.float32, device="cuda")
+    g.forward(f, ie, None, w.sources, w.detectors, 400)
+    fmax = float(f.abs().max())                              # field scale while the pulse is inside the grid
+    assert fmax > 0
+
+    def run(ie_t):
+        f.zero_()
+        ph = g.forward(f, ie_t, None, w.sources, w.detectors, n)
+        return ph, float(sum((P.double() ** 2).sum() for i, P in enumerate(ph) if i in w.loss_detectors))
+
+    ph, L0 = run(ie)
+    assert np.isfinite(L0) and L0 > 0
+    dLp = [2.0 * P if i in w.loss_detectors else None for i, P in enumerate(ph)]
+    grad, _ = g.backward(f, ie, None, w.sources, w.detectors, dLp, None, n)
+    torch.cuda.synchronize()
+    resid = max(float(f[c][box].abs().max()) for c in range(6)) / fmax
+    delta = torch.zeros_like(ie)
+    delta[box] = torch.sign(grad[box])
+    an = float((grad.double() * delta.double()).sum())
+    h = 2e-4
+    fd = (run(ie + h * delta)[1] - run(ie - h * delta)[1]) / (2 * h)
+    g.close()
+    print("C3 full length: L", L0, "directional derivative analytic", an, "finite difference", fd, "state-0 residue", resid)
+    assert an > 0 and abs(fd - an) <= 5e-3 * abs(an)         # measured 2.4e-4
+    assert resid <= 1e-5                                     # measured 6.7e-7
+    grad[box] = 0
+    assert float(grad.abs().max()) == 0.0
+
+
 def test_c4_full_size_self_consistency(B):
     """configs[3] at its full 800 x 800 x 600 size (384 M cells; maximum size, 6 nc > 2^31 elements) in the
     bench launch configuration (fused kernels, record=2), truncated to 24 steps with the source plane moved next
