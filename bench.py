@@ -279,6 +279,16 @@ def main():
             forward_only(grid_f)
         ms_fwd = timed(lambda: forward_only(grid_f), max(1, args.steps))
 
+        # adjoint sweep only (dL_dinv_eps = NULL: one k_step<adjoint> launch per time step), same cotangent seed
+        dLp_t = [2.0 * P if i in w.loss_detectors else None for i, P in enumerate(phasors)]
+
+        def adjoint_only(g):
+            g.backward(fields, ie, None, w.sources, w.detectors, dLp_t, None, T, want_grad=False)
+
+        adjoint_only(grid_f)
+        ms_adj = timed(lambda: adjoint_only(grid_f), max(1, min(args.steps, 3)))
+        reps_adj = max(1, min(args.steps, 3))
+
         # ---- per-kernel roofline: one more pass with every step kernel bracketed by CUDA events --------
         B.fdtd_set_profiling(grid.h, True)
         B.fdtd_get_profile(grid.h)
@@ -328,6 +338,22 @@ def main():
             us = ms_fwd / max(1, args.steps) / T * 1e3
             roofline["forward_step_in_graph"] = {"avg_launch_us": us, "alg_bytes_per_launch": fb,
                                                  "achieved": fb / us / 1e3, "frac": fb / us / 1e3 / peak}
+            # likewise the adjoint-sweep-only pass: one k_step<adjoint> launch per time step (its time also holds the
+            # cotangent seed and the copy of the result: 6 volumes each, once per 2000 launches)
+            ab = algorithmic_bytes(w, grad_cells, recording=False)["fused_adjoint_step"]
+            us = ms_adj / reps_adj / T * 1e3
+            roofline["adjoint_step_in_graph"] = {"avg_launch_us": us, "alg_bytes_per_launch": ab,
+                                                 "achieved": ab / us / 1e3, "frac": ab / us / 1e3 / peak}
+            # headline = the dominant kernel as it runs in the job (replayed graph, back-to-back launches, CUDA events
+            # around the timed region / launches); the figure with events around every single launch stays beside it
+            ing = {"fused_adjoint_step": "adjoint_step_in_graph", "fused_forward_step": "forward_step_in_graph"}.get(dom)
+            if ing:
+                roofline["events_around_every_launch"] = {k: roofline[k] for k in ("achieved", "frac", "avg_launch_us", "frac_of_8000")}
+                g_ = roofline[ing]
+                roofline.update(achieved=g_["achieved"], frac=g_["frac"], avg_launch_us=g_["avg_launch_us"],
+                                alg_bytes_per_launch=g_["alg_bytes_per_launch"], frac_of_8000=g_["achieved"] / 8000.0,
+                                method=f"{ing}: CUDA events around a pass of {T} back-to-back launches of this kernel "
+                                       "in the replayed graph, time / launches")
 
     # ---- end to end through the host-buffer C ABI (pinned host memory, H2D/D2H inside the timed region) ----
     e2e = None

@@ -140,9 +140,12 @@ FDTD_API int fdtd_forward(fdtd_grid *grid, float *fields, const float *inv_eps, 
  * dL_dfields  : DEVICE [6][nz][ny][nx] cotangent of state n_steps, or NULL (= 0).
  * dL_dinv_eps : DEVICE [nz][ny][nx], OUT; zero-filled by the library, non-zero only on
  *               I intersected with the grad box (R17).  inv_mu and source gradients are not computed.
+ *               NULL (then dL_dfields0 is required) = adjoint sweep only: the cotangent of state 0 does not
+ *               depend on the primal fields (the steps are linear in the fields), so nothing is reconstructed,
+ *               `fields` is not touched and no recorded forward is needed.
  * dL_dfields0 : DEVICE [6][nz][ny][nx] OUT cotangent of state 0, or NULL.
- * Errors: ESTATE if pml_cells > 0 and the last fdtd_forward on this grid did not record exactly
- *         n_steps steps. */
+ * Errors: ESTATE if dL_dinv_eps is wanted, pml_cells > 0 and the last fdtd_forward on this grid did not record
+ *         exactly n_steps steps. */
 FDTD_API int fdtd_backward(fdtd_grid *grid, float *fields, const float *inv_eps, const float *inv_mu,
                   const fdtd_source *src, int32_t n_src,
                   const fdtd_detector *det, int32_t n_det,

@@ -298,7 +298,8 @@ class Grid:
         return phasors
 
     def backward(self, fields, inv_eps, inv_mu=None, sources=(), detectors=(), dL_dphasor=None,
-                 dL_dfields=None, n_steps=0, want_dL_dfields0=False, out=None):
+                 dL_dfields=None, n_steps=0, want_dL_dfields0=False, out=None, want_grad=True):
+        """want_grad=False: adjoint sweep only (dL_dinv_eps = NULL): returns (None, cotangent of state 0)."""
         torch = self.torch
         sarr, ns, k1 = self.marshal_sources(sources)
         darr, nd, k2 = self.marshal_detectors(detectors, None)
@@ -307,8 +308,8 @@ class Grid:
             cot = (C.c_void_p * max(nd, 1))()
             for i, G in enumerate(dL_dphasor):
                 cot[i] = _ptr(G)
-        g = out if out is not None else torch.empty(self.shape, dtype=torch.float32, device="cuda")
-        lam0 = torch.empty((6,) + self.shape, dtype=torch.float32, device="cuda") if want_dL_dfields0 else None
+        g = None if not want_grad else (out if out is not None else torch.empty(self.shape, dtype=torch.float32, device="cuda"))
+        lam0 = torch.empty((6,) + self.shape, dtype=torch.float32, device="cuda") if (want_dL_dfields0 or not want_grad) else None
         fdtd_backward(self.h, fields, inv_eps, inv_mu, sarr, ns, darr, nd, cot, dL_dfields, int(n_steps),
                       g, lam0, self.stream())
         self._keep = [k1, k2, sarr, darr, cot, dL_dphasor]

@@ -582,9 +582,9 @@ extern "C" int fdtd_backward(fdtd_grid *g, float *fields, const float *inv_eps, 
 {
     int rc = check_common(g, fields, inv_eps, src, n_src, det, n_det, n_steps, "fdtd_backward");
     if (rc) return rc;
-    if (!dL_dinv_eps) return fail(FDTD_EINVAL, "fdtd_backward: dL_dinv_eps is required");
+    if (!dL_dinv_eps && !dL_dfields0) return fail(FDTD_EINVAL, "fdtd_backward: dL_dinv_eps or dL_dfields0 is required");
     const Dims &G = g->G;
-    if (G.d > 0 && (!g->desc.record || g->recorded_steps != n_steps))
+    if (dL_dinv_eps && G.d > 0 && (!g->desc.record || g->recorded_steps != n_steps))
         return fail(FDTD_ESTATE, "fdtd_backward: no matching recorded forward (need record=1 and the same n_steps)");
     cudaStream_t st = (cudaStream_t)cuda_stream;
     std::vector<SourceDev> S;
@@ -602,8 +602,9 @@ extern "C" int fdtd_backward(fdtd_grid *g, float *fields, const float *inv_eps, 
     else            CK(cudaMemsetAsync(g->lam, 0, 6 * vol, st));
     for (int q = 0; q < 2; ++q)
         if ((rc = g->zero_psi(g->lpsiE[q], st)) || (rc = g->zero_psi(g->lpsiH[q], st))) return rc;
-    CK(cudaMemsetAsync(dL_dinv_eps, 0, vol, st));
+    if (dL_dinv_eps) CK(cudaMemsetAsync(dL_dinv_eps, 0, vol, st));
     launch_set_step(g->d_step, std::max(n_steps - 1, 0), st);   // the first reverse step reads slot 0
+    const bool want_grad = dL_dinv_eps != nullptr;              // false: adjoint sweep only (B1, B2, B5)
 
     if (g->path == FDTD_PATH_FUSED && g->fused_backward_ready && !inv_mu) {
         rc = fused_backward(g, fields, inv_eps, inv_mu, S, D, total_freq, n_steps, dL_dinv_eps, st);
@@ -611,12 +612,13 @@ extern "C" int fdtd_backward(fdtd_grid *g, float *fields, const float *inv_eps, 
     } else {
         int n_adj = 0;
         for (const DetectorDev &dt : D) if (dt.phasor) ++n_adj;
-        const int launches = 5 + n_adj + n_src + (G.d > 0 ? 1 : 0);
+        const int launches = want_grad ? 5 + n_adj + n_src + (G.d > 0 ? 1 : 0) : 3 + n_adj;
         const std::string key = make_key("gb", fields, inv_eps, inv_mu, g->rec, dL_dinv_eps, S, D, 0);
         rc = run_steps(g, g->bwd_graph, key, n_steps, launches, st, [&](cudaStream_t cs) {
             { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
               for (const DetectorDev &dt : D) if (dt.phasor) launch_detector_adjoint(G, g->lam, dt, g->d_cs, total_freq, g->step_in(), cs); }
             { ProfScope p(g, fdtd_grid::PC_ADJ_H, cs); launch_adj_H(G, g->T, g->lam, inv_mu, g->lpsiH[0], g->lpsiH[1], g->step_in(), cs); }
+            if (want_grad) {
             { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
               for (const SourceDev &s : S) if (s.comp >= 3) launch_add_source(G, fields, s, g->step_in(), -1.f, cs); }
             if (G.d > 0) { ProfScope p(g, fdtd_grid::PC_INJECT, cs); launch_inject(G, g->R, fields, g->rec, g->step_in(), cs); }
@@ -624,6 +626,7 @@ extern "C" int fdtd_backward(fdtd_grid *g, float *fields, const float *inv_eps, 
             { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
               for (const SourceDev &s : S) if (s.comp < 3) launch_add_source(G, fields, s, g->step_in(), -1.f, cs); }
             { ProfScope p(g, fdtd_grid::PC_INV_E_GRAD, cs); launch_inv_E_grad(G, fields, inv_eps, g->lam, dL_dinv_eps, cs); }
+            }
             { ProfScope p(g, fdtd_grid::PC_ADJ_E, cs); launch_adj_E(G, g->T, g->lam, inv_eps, g->lpsiE[0], g->lpsiE[1], g->step_in(), cs); }
             { ProfScope p(g, fdtd_grid::PC_OTHER, cs); launch_next_step(g->step_in(), g->step_out(), -1, cs); }
         });

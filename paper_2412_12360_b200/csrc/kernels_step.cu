@@ -1655,7 +1655,7 @@ void enqueue_fwd(void *vctx, cudaStream_t cs)
 }
 
 struct BwdCtx {
-    fdtd_grid *g; StepParams P; InvParams I; bool fused_inv; bool fused_det; bool pipelined; float *bufB; float *fields; const float *ie; float *grad; float *lamA; float *lamB;
+    fdtd_grid *g; StepParams P; InvParams I; bool fused_inv; bool fused_det; bool pipelined; bool want_grad; float *bufB; float *fields; const float *ie; float *grad; float *lamA; float *lamB;
     const std::vector<SourceDev> *S; const std::vector<DetectorDev> *D; int total_freq;
 };
 // Reverse step n.  One kernel after the other: B1 (detector cotangents into the volume about to be read), B2+B5
@@ -1691,7 +1691,7 @@ void enqueue_bwd(void *vctx, cudaStream_t cs)
       for (const DetectorDev &dt : *c->D)
           if (dt.phasor) launch_detector_adjoint_pp(G, c->lamA, c->lamB, dt, g->d_cs, c->total_freq, g->step_in(), cs); }
     // the face injection (it writes cells of the primal volume, which the adjoint step never touches) runs beside it
-    const bool side_inject = c->fused_inv && G.d > 0;
+    const bool side_inject = c->fused_inv && G.d > 0;       // fused_inv implies want_grad
     { ProfScope p(g, fdtd_grid::PC_FUSED_BWD, cs);
       if (side_inject) {
           fork_side(g, cs, 1);
@@ -1705,6 +1705,7 @@ void enqueue_bwd(void *vctx, cudaStream_t cs)
         { ProfScope p(g, fdtd_grid::PC_FUSED_INV, cs); F->itile->launch_inv(J, F->in_cta, F->ismem, cs); }
         return;
     }
+    if (!c->want_grad) return;
     { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
       for (const SourceDev &s : *c->S) if (s.comp >= 3) launch_add_source(G, c->fields, s, g->step_in(), -1.f, cs); }
     if (G.d > 0) { ProfScope p(g, fdtd_grid::PC_INJECT, cs); launch_inject(G, g->R, c->fields, g->rec, g->step_in(), cs); }
@@ -1780,13 +1781,14 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
         cudaError_t e = cudaMemcpyAsync(F->lamB, g->lam, vol6, cudaMemcpyDeviceToDevice, st);
         if (e != cudaSuccess) { (void)cudaGetLastError(); return fdtd_fail(FDTD_ECUDA, cudaGetErrorString(e)); }
     }
-    const bool fused_inv = F->itile != nullptr && (int)S.size() <= MAX_SRC && !getenv("FDTD_GENERIC_INVERSE");
+    const bool want_grad = dL_dinv_eps != nullptr;      // false: adjoint sweep only, the primal volumes are not touched
+    const bool fused_inv = want_grad && F->itile != nullptr && (int)S.size() <= MAX_SRC && !getenv("FDTD_GENERIC_INVERSE");
     // B1 inside the adjoint kernel when every detector with a cotangent is on E components (else a kernel per detector)
     bool fused_det = (int)D.size() <= MAX_DET;
     for (const DetectorDev &dt : D) if (dt.phasor && (dt.mask >> 3)) fused_det = false;
     // while profiling (events around every launch) the kernels run one after the other, so each is timed alone
     const bool pipelined = fused_inv && fused_det && F->n_inv_p > 0 && !g->profiling;
-    BwdCtx ctx{ g, F->sp, F->ip, fused_inv, fused_det, pipelined, F->bufB, fields, inv_eps, dL_dinv_eps, g->lam, F->lamB, &S, &D, total_freq };
+    BwdCtx ctx{ g, F->sp, F->ip, fused_inv, fused_det, pipelined, want_grad, F->bufB, fields, inv_eps, dL_dinv_eps, g->lam, F->lamB, &S, &D, total_freq };
     if (fused_inv) {
         // reverse step n reads primal volume (n+1)&1 and writes n&1: state n_steps must sit in volume n_steps&1
         if ((rc = build_inv_maps(g, fields, F->bufB, inv_eps, g->lam, F->lamB, st))) return rc;
@@ -1832,7 +1834,8 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     if (!S.empty()) key.append((const char *)S.data(), S.size() * sizeof(SourceDev));
     if (!D.empty()) key.append((const char *)D.data(), D.size() * sizeof(DetectorDev));
     const int n_inj = g->G.d > 0 ? 1 : 0;
-    const int launches = fused_inv ? 2 + (fused_det ? 0 : n_adj) + n_inj : 3 + (fused_det ? 0 : n_adj) + (int)S.size() + n_inj;
+    const int launches = !want_grad ? 1 + (fused_det ? 0 : n_adj)
+                         : (fused_inv ? 2 + (fused_det ? 0 : n_adj) + n_inj : 3 + (fused_det ? 0 : n_adj) + (int)S.size() + n_inj);
     rc = fdtd_run_steps_bwd(g, key, n_steps, launches, st, enqueue_bwd, &ctx);
     if (rc || !pipelined) return rc;
     // inverse step 0 on every SM; reverse step p read counter slot p&1 (p counted from the end), so -1 sits in slot n_steps&1

@@ -287,6 +287,33 @@ def test_pipelined_reverse_sweep_is_the_same_computation(B, monkeypatch):
         monkeypatch.delenv("FDTD_REVERSE_SWEEP", raising=False)
 
 
+def test_adjoint_sweep_only(B):
+    """dL_dinv_eps = NULL (include/fdtd.h): the cotangent of state 0 alone.  It does not depend on the primal
+    fields, so it needs no recorded forward, leaves `fields` untouched and is bit-identical to the cotangent the
+    full backward pass returns; checked against the oracle on both kernel paths."""
+    import torch
+    w = wl.c3_mini(n_steps=61, kappa_max=3.0, alpha_max=0.05)
+    ref = run_oracle(w)
+    for path in paths(B, w):
+        full = run_gpu(B, w, path)
+        kw = w.grid_kwargs()
+        kw.update(max_steps=w.n_steps, record=0, path=path)              # no recorder at all
+        g = B.Grid(**kw)
+        f = torch.zeros((6, w.nz, w.ny, w.nx), dtype=torch.float32, device="cuda")
+        ie = torch.as_tensor(w.inv_eps).cuda()
+        ph = g.forward(f, ie, None, w.sources, w.detectors, w.n_steps)
+        keep = f.clone()
+        dLp, dLf = loss_cotangents(w, f, ph)
+        none, lam0 = g.backward(f, ie, None, w.sources, w.detectors, dLp, dLf, w.n_steps, want_grad=False)
+        torch.cuda.synchronize()
+        assert none is None and torch.equal(f, keep)
+        assert np.array_equal(lam0.cpu().numpy(), full["lam0"])
+        assert relerr(lam0.cpu().numpy(), ref["lam0"]) <= TOL_GRAD
+        with pytest.raises(B.FdtdError):                                  # a gradient still needs the recorded forward
+            g.backward(f, ie, None, w.sources, w.detectors, dLp, dLf, w.n_steps)
+        g.close()
+
+
 def test_c3_full_size_truncated_in_the_bench_configuration(B):
     """configs[2] at its full 200^3 size in the launch configuration bench.py times (fused kernels, tile and
     grid chosen by the library, grad box = design region, record=2 and record=1), truncated to 40 time steps
