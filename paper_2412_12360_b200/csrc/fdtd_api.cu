@@ -455,7 +455,8 @@ int run_steps(fdtd_grid *g, fdtd_grid::GraphCache &gc, const std::string &key, i
         g->kernel_launches += (long long)n_steps * launches_per_step;
         return FDTD_OK;
     }
-    const int unroll = g->graph_unroll;                  // even: a replay of the main graph ends in the slot it began in
+    static const int env_unroll = getenv("FDTD_GRAPH_UNROLL") ? std::max(2, atoi(getenv("FDTD_GRAPH_UNROLL")) / 2 * 2) : 0;
+    const int unroll = env_unroll ? env_unroll : g->graph_unroll;   // even: a replay of the main graph ends in the slot it began in
     if (gc.key != key || !gc.exec_tail[1]) {
         if (gc.key.size()) CK(cudaEventSynchronize(gc.done));
         if (gc.exec_main) { cudaGraphExecDestroy(gc.exec_main); gc.exec_main = nullptr; }
