@@ -402,6 +402,8 @@ def main():
                "config": workload_config(w, {"path": {1: "generic", 2: "fused"}[info.path],
                                              "tile": [info.tile_x, info.tile_y, info.tile_z],
                                              "parallelism": f"independent problems x{world}",
+                                             "partition": "lock-step runs (DESIGN.md section 8)",
+                                             "reverse_sweep": "grouped launches" if info.pipelined_inverse_ctas else "sequential",
                                              "recorder": "faces of the design box, record=2 (SURVEY 8(f) N1)" if args.record == 2
                                              else "PML/interior interface, record=1"}),
                "fwd": {"value": fwd_value, "unit": UNIT, "ms_per_pass": ms_fwd / max(1, args.steps),
