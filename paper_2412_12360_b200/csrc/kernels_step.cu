@@ -1123,32 +1123,42 @@ Runs lockstep_runs(const std::vector<double> &w, int nz, int n_cta)
     return runs;
 }
 
-// Large grids: more columns than CTAs.  Whole columns are dealt out in waves (CTA c takes columns c, c + n_cta,
-// ...): every CTA starts a column at plane 0 at time 0, so the n_cta y-consecutive columns of a wave are marched in
-// lock step.  The columns that do not fill a wave form a pool that is cut, in sequence order, into one chunk per
-// CTA sized so that every CTA ends up with the same total cost (a CTA whose whole columns already cost more gets
-// nothing from the pool).
+// Large grids: more columns than CTAs.  Whole columns are dealt out in waves (CTA c takes the c-th, (c + n_cta)-th,
+// ... of them): every CTA starts a column at plane 0 at time 0, so the n_cta y-consecutive columns of a wave are
+// marched in lock step.  Only the cheap columns (no y slab: they all cost the same, so the CTAs stay together) are
+// dealt, for as long as a CTA's total stays below the mean; the last wave may be partial.  The other columns form
+// a pool that is cut, in sequence order, into one chunk per CTA sized so that every CTA ends up with the same
+// total cost (a CTA whose whole columns already cost the mean gets nothing from the pool).
 Runs wave_runs(const std::vector<double> &w, int nz, int n_cta)
 {
     const long long n_col = (long long)w.size() / nz;
     std::vector<double> colw(n_col, 0.0);
-    double total = 0.0;
-    for (long long t = 0; t < n_col; ++t) { for (int k = 0; k < nz; ++k) colw[t] += w[t * nz + k]; total += colw[t]; }
-    // as many full waves as the pool can still level out (columns in CPML slabs cost about twice the others)
-    long long waves = n_col / n_cta;
-    std::vector<double> used(n_cta, 0.0);
-    for (; waves >= 1; --waves) {
-        std::fill(used.begin(), used.end(), 0.0);
-        for (long long t = 0; t < waves * n_cta; ++t) used[t % n_cta] += colw[t];
-        if (*std::max_element(used.begin(), used.end()) <= total / n_cta * (1.0 + 1e-9)) break;
+    double total = 0.0, cheapest = 1e300;
+    for (long long t = 0; t < n_col; ++t) {
+        for (int k = 0; k < nz; ++k) colw[t] += w[t * nz + k];
+        total += colw[t];
+        cheapest = std::min(cheapest, colw[t]);
     }
-    if (waves < 1) return lockstep_runs(w, nz, n_cta);
+    std::vector<long long> order;                       // cheap columns first, each group in sequence order
+    for (long long t = 0; t < n_col; ++t) if (colw[t] <= 1.2 * cheapest) order.push_back(t);
+    const size_t n_cheap = order.size();
+    for (long long t = 0; t < n_col; ++t) if (colw[t] > 1.2 * cheapest) order.push_back(t);
+    const double mean = total / n_cta;
     Runs runs(n_cta);
-    for (long long t = 0; t < waves * n_cta; ++t) runs[t % n_cta].push_back({ t * nz, (t + 1) * nz });
-    const long long q0 = waves * n_cta * nz, q1 = n_col * nz;
-    if (q0 == q1) return runs;
+    std::vector<double> used(n_cta, 0.0);
+    size_t dealt = 0;
+    for (; dealt < n_cheap; ++dealt) {
+        const int c = (int)(dealt % n_cta);
+        const long long t = order[dealt];
+        if (used[c] + colw[t] > mean * (1.0 + 1e-9)) break;
+        runs[c].push_back({ t * nz, (t + 1) * nz });
+        used[c] += colw[t];
+    }
+    if (dealt < (size_t)n_cta) return lockstep_runs(w, nz, n_cta);      // not even one full wave
+    if (dealt == order.size()) return runs;
+    // the pool: positions of the columns order[dealt..], column after column
     double pool = 0.0;
-    for (long long q = q0; q < q1; ++q) pool += w[q];
+    for (size_t p = dealt; p < order.size(); ++p) pool += colw[order[p]];
     // level: sum_c max(0, level - used[c]) = pool
     std::vector<double> u(used);
     std::sort(u.begin(), u.end());
@@ -1158,23 +1168,27 @@ Runs wave_runs(const std::vector<double> &w, int nz, int n_cta)
         level = (pool + below) / m;
         if (m == n_cta || level <= u[m]) break;
     }
-    long long q = q0;
+    int last_c = -1;
+    for (int c = 0; c < n_cta; ++c) if (level - used[c] > 0.0) last_c = c;
+    size_t p = dealt;
+    int k = 0;                                   // next position: plane k of column order[p]
     double acc = 0.0, target = 0.0;
-    for (int c = 0; c < n_cta && q < q1; ++c) {
-        const double budget = std::max(0.0, level - used[c]);
+    for (int c = 0; c < n_cta && p < order.size(); ++c) {
+        const double budget = level - used[c];
         if (budget <= 0.0) continue;
         target += budget;
-        long long e = q;
-        while (e < q1 && (acc + w[e] <= target + 1e-9 * target || e == q)) acc += w[e++];
-        bool later = false;                      // the last CTA with a budget takes what is left
-        for (int c2 = c + 1; c2 < n_cta; ++c2) later |= level - used[c2] > 0.0;
-        if (!later) { while (e < q1) acc += w[e++]; }
-        for (long long a = q; a < e;) {
-            const long long b = std::min(e, (a / nz + 1) * nz);
-            runs[c].push_back({ a, b });
-            a = b;
+        bool first = true;
+        while (p < order.size()) {
+            const long long t = order[p];
+            const double x = w[t * nz + k];
+            if (c != last_c && !first && acc + x > target * (1.0 + 1e-9)) break;
+            const long long q = t * nz + k;
+            if (!runs[c].empty() && runs[c].back().second == q && k != 0) ++runs[c].back().second;
+            else runs[c].push_back({ q, q + 1 });
+            acc += x;
+            first = false;
+            if (++k == nz) { k = 0; ++p; }
         }
-        q = e;
     }
     return runs;
 }

@@ -97,23 +97,27 @@ def test_bad_arguments_are_rejected():
 
 
 def test_large_grids_march_whole_columns_in_waves():
-    """More columns than CTAs (C4): CTA c starts with the whole column c, then c + n_cta, ...: the n_cta columns of a
-    wave are y-consecutive and start at plane 0 together; only the pool that levels the costs is cut inside columns."""
+    """More columns than CTAs (C4): the columns without a y slab are dealt out whole, in sequence order, CTA c taking
+    the c-th, (c + n_cta)-th, ... of them, so the n_cta y-consecutive columns of a wave start at plane 0 together;
+    only the other columns (the pool that levels the costs) are cut inside."""
     b = _b()
     nx, ny, nz, d, tx, ty, n_cta = 800, 800, 600, 16, 200, 7, 148
     nty = -(-ny // ty)
     segs = b.fdtd_debug_partition(nx, ny, nz, d, tx, ty, n_cta, 1.0, 0.8, True)
+    col = lambda s: (s[0] // tx) * nty + s[1] // ty
+    slab = lambda j0: j0 <= d or j0 + ty >= ny - d
+    cheap = [t for t in range(4 * nty) if not slab((t % nty) * ty)]
     per_cta = collections.defaultdict(list)
     for s in segs:
         per_cta[s[0]].append(s[1:])
-    waves = 0
+    whole = 0
     for c in range(n_cta):
-        col = lambda s: (s[0] // tx) * nty + s[1] // ty
-        first = per_cta[c][0]
-        assert col(first) == c and first[2:] == (0, nz)
         w = 0
-        while w < len(per_cta[c]) and per_cta[c][w][2:] == (0, nz) and col(per_cta[c][w]) == c + w * n_cta:
+        while w < len(per_cta[c]) and per_cta[c][w][2:] == (0, nz):
+            assert col(per_cta[c][w]) == cheap[c + w * n_cta]
             w += 1
-        waves = w if c == 0 else waves
-        assert w == waves
-    assert waves >= 2
+        assert w >= 2
+        whole += w
+        for s in per_cta[c][w:]:                              # what follows is pool work: columns with a y slab
+            assert slab(s[1])
+    assert whole == len(cheap)                                # every cheap column is marched whole: 440 of 460
