@@ -178,6 +178,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--time-steps", type=int, default=2000, help="FDTD time steps per gradient (C3: 2000)")
     ap.add_argument("--grid", type=int, default=200, help="C3 grid size per axis (200)")
+    ap.add_argument("--workload", default="c3", choices=["c3", "c4"],
+                    help="c3: the graded config (default); c4: configs[3], 800x800x600 memory-scale run (use a small --time-steps)")
     ap.add_argument("--path", default="auto", choices=["auto", "generic", "fused"])
     ap.add_argument("--ref-sample-steps", type=int, default=12)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -214,7 +216,11 @@ def main():
         torch.cuda.synchronize()
 
     # ---- workload: C3 (seed + rank: every rank an independent problem) -----------------------------
-    w = wl.c3(n=args.grid, n_steps=args.time_steps, seed=sharding.problem_seed(3, rank))
+    if args.workload == "c4":
+        w = wl.c4(n_steps=args.time_steps)
+        w.meta.setdefault("delta_eps", 12.25 - 2.085)
+    else:
+        w = wl.c3(n=args.grid, n_steps=args.time_steps, seed=sharding.problem_seed(3, rank))
     T = w.n_steps
     path = {"auto": B.FDTD_PATH_AUTO, "generic": B.FDTD_PATH_GENERIC, "fused": B.FDTD_PATH_FUSED}[args.path]
     kw = w.grid_kwargs()
@@ -395,7 +401,8 @@ def main():
     if rank == 0:
         cpu = None
         if not args.no_cpu_baseline and world == 1:
-            cpu = cpu_oracle_rate(wl.c3(n=args.grid, n_steps=args.time_steps), args.ref_sample_steps)
+            cpu = cpu_oracle_rate(wl.c3(n=args.grid, n_steps=args.time_steps) if args.workload == "c3"
+                                  else wl.c4(n_steps=args.time_steps), args.ref_sample_steps)
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",

@@ -208,6 +208,24 @@ __device__ __noinline__ float4 det_adjoint4(const StepParams &P, int n, int comp
     return v;
 }
 
+// exact per-plane tests behind the coarse k ranges of the parameters (sEl..dHh span all sources / detectors of a
+// family: with two detector planes far apart every plane in between would otherwise pay for the box tests per cell)
+template <class PT>
+__device__ __forceinline__ bool src_plane(const PT &P, int k, int family)
+{
+    bool hit = false;
+    for (int s = 0; s < P.n_src; ++s) hit |= (P.src[s].comp >= 3) == (family != 0) && k >= P.src[s].lo[2] && k < P.src[s].hi[2];
+    return hit;
+}
+__device__ __forceinline__ bool det_plane(const StepParams &P, int k, int family, bool need_cotangent)
+{
+    bool hit = false;
+    for (int s = 0; s < P.n_det; ++s)
+        hit |= ((P.det[s].mask >> (3 * family)) & 7) != 0 && k >= P.det[s].lo[2] && k < P.det[s].hi[2] &&
+               (!need_cotangent || P.det[s].phasor != nullptr);
+    return hit;
+}
+
 __device__ __forceinline__ float f4get(const float4 &v, int q) { return q == 0 ? v.x : (q == 1 ? v.y : (q == 2 ? v.z : v.w)); }
 
 // adds the sources of component `comp` to the float4 of cells (i..i+3, j, k); rare planes only
@@ -393,7 +411,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
             mbar_wait(&full[st_i], st_ph);
             const uint32_t so = stage_base + st_off + o_own;
             const uint32_t sp = stage_base + pv_off + o_own;       // the stage of plane kk-1 is still held
-            if (ADJ && kk >= P.dEl && kk < P.dEh && !dup) {
+            if (ADJ && kk >= P.dEl && kk < P.dEh && !dup && det_plane(P, kk, 0, true)) {
                 // B1 for E-component detectors: the cotangents are added to lamE in the stage, at my cells, before
                 // anything is live in registers (lamE is only ever read at a thread's own cells)
                 for (int c = 0; c < 3; ++c) {
@@ -514,7 +532,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                 v2x = sie * e2x; v2y = sie * e2y; v2z = sie * e2z;
             } else {
                 e2x = fma4(sie, tEx, ex); e2y = fma4(sie, tEy, ey); e2z = fma4(sie, tEz, ez);
-                if (kk >= P.sEl && kk < P.sEh) {
+                if (kk >= P.sEl && kk < P.sEh && src_plane(P, kk, 0)) {
                     e2x = add_sources4(P, n, 0, e2x, i, j, kk); e2y = add_sources4(P, n, 1, e2y, i, j, kk); e2z = add_sources4(P, n, 2, e2z, i, j, kk);
                 }
                 v2x = e2x; v2y = e2y; v2z = e2z;
@@ -522,7 +540,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
             if (wr) {
                 float *o = dst + off;
                 stg4(o, e2x); stg4(o + nc, e2y); stg4(o + 2 * nc, e2z);
-                if (!ADJ && kk >= P.dEl && kk < P.dEh) detect4(P, n, 0, e2x, e2y, e2z, i, j, kk);
+                if (!ADJ && kk >= P.dEl && kk < P.dEh && det_plane(P, kk, 0, false)) detect4(P, n, 0, e2x, e2y, e2z, i, j, kk);
             }
             float4 Yx = v2x, Yz = v2z, Xy = v2y, Xz = v2z, Zx = v2x, Zy = v2y;
             if (ADJ && (slab_xy || zs >= 0)) {       // phase-B operands are filtered where they are produced
@@ -602,13 +620,13 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                 } else {
                     const float4 sim = has_mu ? S * ldg4(P.im + offm) : splat(S);
                     h2x = hx - sim * tHx; h2y = hy - sim * tHy; h2z = hz - sim * tHz;
-                    if (km1 >= P.sHl && km1 < P.sHh) {
+                    if (km1 >= P.sHl && km1 < P.sHh && src_plane(P, km1, 1)) {
                         h2x = add_sources4(P, n, 3, h2x, i, j, km1); h2y = add_sources4(P, n, 4, h2y, i, j, km1); h2z = add_sources4(P, n, 5, h2z, i, j, km1);
                     }
                 }
                 float *o = dst + 3 * nc + offm;
                 stg4(o, h2x); stg4(o + nc, h2y); stg4(o + 2 * nc, h2z);
-                if (!ADJ && km1 >= P.dHl && km1 < P.dHh) detect4(P, n, 1, h2x, h2y, h2z, i, j, km1);
+                if (!ADJ && km1 >= P.dHl && km1 < P.dHh && det_plane(P, km1, 1, false)) detect4(P, n, 1, h2x, h2y, h2z, i, j, km1);
             }
             if (ADJ) { cZx = Zx; cZy = Zy; }
             // the stage of plane kk-1 is no longer needed; the stage of plane kk stays for the next iteration
@@ -792,7 +810,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_inverse(const __grid_constant
             const float4 Dx_y = dplus_x(Ey, Ey_px), Dx_z = dplus_x(Ez, Ez_px);
             const float4 Dz_x = Ex_pz - Ex, Dz_y = Ey_pz - Ey;
             float4 Hx = fma4(S, Dy_z - Dz_y, Hpx), Hy = fma4(S, Dz_x - Dx_z, Hpy), Hz = fma4(S, Dx_y - Dy_x, Hpz);
-            if (kk >= P.sHl && kk < P.sHh) {
+            if (kk >= P.sHl && kk < P.sHh && src_plane(P, kk, 1)) {
                 Hx = Hx - add_sources4(P, n, 3, splat(0.f), i, j, kk);
                 Hy = Hy - add_sources4(P, n, 4, splat(0.f), i, j, kk);
                 Hz = Hz - add_sources4(P, n, 5, splat(0.f), i, j, kk);
@@ -828,7 +846,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_inverse(const __grid_constant
                 const float4 sie = S * lds4(sp + 6 * C::SLOT);
                 const float4 lx = lds4(sp + 7 * C::SLOT), ly = lds4(sp + 8 * C::SLOT), lz = lds4(sp + 9 * C::SLOT);
                 float4 E2x = Ex - sie * qx, E2y = Ey - sie * qy, E2z = Ez - sie * qz;
-                if (kk >= P.sEl && kk < P.sEh) {
+                if (kk >= P.sEl && kk < P.sEh && src_plane(P, kk, 0)) {
                     E2x = E2x - add_sources4(P, n, 0, splat(0.f), i, j, kk);
                     E2y = E2y - add_sources4(P, n, 1, splat(0.f), i, j, kk);
                     E2z = E2z - add_sources4(P, n, 2, splat(0.f), i, j, kk);
