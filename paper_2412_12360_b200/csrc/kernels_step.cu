@@ -154,29 +154,6 @@ __device__ __noinline__ float source_at(const PT &P, int n, int comp, int i, int
     return acc;
 }
 
-// running DFT of component `comp` (value v) at cell (i,j,k): P_f += v (cos - i sin)
-__device__ __noinline__ void detect_cell(const StepParams &P, int n, int comp, float v, int i, int j, int k)
-{
-    for (int s = 0; s < P.n_det; ++s) {
-        const DetectorDev &q = P.det[s];
-        if (!((q.mask >> comp) & 1)) continue;
-        if (i < q.lo[0] || i >= q.hi[0] || j < q.lo[1] || j >= q.hi[1] || k < q.lo[2] || k >= q.hi[2]) continue;
-        const int bx = q.hi[0] - q.lo[0], by = q.hi[1] - q.lo[1], bz = q.hi[2] - q.lo[2];
-        const long long bc = (long long)bx * by * bz;
-        const long long cell = ((long long)(k - q.lo[2]) * by + (j - q.lo[1])) * bx + (i - q.lo[0]);
-        int ci = 0;
-        for (int c = 0; c < comp; ++c) ci += (q.mask >> c) & 1;
-        const float *csn = P.cs + ((long long)n * P.total_freq + q.cs_off) * 2;
-        for (int f = 0; f < q.n_freq; ++f) {
-            float2 *ph = reinterpret_cast<float2 *>(q.phasor) + ((long long)f * q.ncomp + ci) * bc + cell;
-            float2 acc = *ph;
-            acc.x += v * __ldg(csn + 2 * f);
-            acc.y -= v * __ldg(csn + 2 * f + 1);
-            *ph = acc;
-        }
-    }
-}
-
 // adjoint of the running DFT (B1) at cell (i,j,k) of component `comp`: sum_f Gr cos - Gi sin, with the caller's
 // phasor cotangents in det[].phasor (NULL: no cotangent for that detector)
 __device__ __noinline__ float det_adjoint_at(const StepParams &P, int n, int comp, int i, int j, int k)
@@ -211,19 +188,18 @@ __device__ __noinline__ float4 det_adjoint4(const StepParams &P, int n, int comp
 // exact per-plane tests behind the coarse k ranges of the parameters (sEl..dHh span all sources / detectors of a
 // family: with two detector planes far apart every plane in between would otherwise pay for the box tests per cell)
 template <class PT>
-__device__ __forceinline__ bool src_plane(const PT &P, int k, int family)
+__device__ __forceinline__ int src_mask(const PT &P, int k)      // bit c: some source of component c has cells on plane k
 {
-    bool hit = false;
-    for (int s = 0; s < P.n_src; ++s) hit |= (P.src[s].comp >= 3) == (family != 0) && k >= P.src[s].lo[2] && k < P.src[s].hi[2];
-    return hit;
+    int m = 0;
+    for (int s = 0; s < P.n_src; ++s) if (k >= P.src[s].lo[2] && k < P.src[s].hi[2]) m |= 1 << P.src[s].comp;
+    return m;
 }
-__device__ __forceinline__ bool det_plane(const StepParams &P, int k, int family, bool need_cotangent)
+__device__ __forceinline__ int det_mask(const StepParams &P, int k, bool need_cotangent)   // bit c: a detector of component c on plane k
 {
-    bool hit = false;
+    int m = 0;
     for (int s = 0; s < P.n_det; ++s)
-        hit |= ((P.det[s].mask >> (3 * family)) & 7) != 0 && k >= P.det[s].lo[2] && k < P.det[s].hi[2] &&
-               (!need_cotangent || P.det[s].phasor != nullptr);
-    return hit;
+        if (k >= P.det[s].lo[2] && k < P.det[s].hi[2] && (!need_cotangent || P.det[s].phasor != nullptr)) m |= P.det[s].mask;
+    return m;
 }
 
 __device__ __forceinline__ float f4get(const float4 &v, int q) { return q == 0 ? v.x : (q == 1 ? v.y : (q == 2 ? v.z : v.w)); }
@@ -238,14 +214,47 @@ __device__ __noinline__ float4 add_sources4(const PT &P, int n, int comp, float4
     v.w += source_at(P, n, comp, i + 3, j, k);
     return v;
 }
-__device__ __noinline__ void detect4(const StepParams &P, int n, int family, float4 vx, float4 vy, float4 vz, int i, int j, int k)
+// running DFT of component `comp` at the cells (i..i+3, j, k): two float4 read-modify-writes per frequency when the
+// four cells are inside the box and their phasors 16-byte aligned, cell by cell otherwise
+__device__ __noinline__ void detect_comp4(const StepParams &P, int n, int comp, float4 v, int i, int j, int k)
 {
+    for (int s = 0; s < P.n_det; ++s) {
+        const DetectorDev &q = P.det[s];
+        if (!((q.mask >> comp) & 1)) continue;
+        if (j < q.lo[1] || j >= q.hi[1] || k < q.lo[2] || k >= q.hi[2] || i + 3 < q.lo[0] || i >= q.hi[0]) continue;
+        const int bx = q.hi[0] - q.lo[0], by = q.hi[1] - q.lo[1], bz = q.hi[2] - q.lo[2];
+        const long long bc = (long long)bx * by * bz;
+        const long long cell = ((long long)(k - q.lo[2]) * by + (j - q.lo[1])) * bx + (i - q.lo[0]);
+        int ci = 0;
+        for (int c = 0; c < comp; ++c) ci += (q.mask >> c) & 1;
+        const float *csn = P.cs + ((long long)n * P.total_freq + q.cs_off) * 2;
+        const bool whole = i >= q.lo[0] && i + 3 < q.hi[0];
+        for (int f = 0; f < q.n_freq; ++f) {
+            const float c = __ldg(csn + 2 * f), sn = __ldg(csn + 2 * f + 1);
+            float2 *ph = reinterpret_cast<float2 *>(q.phasor) + ((long long)f * q.ncomp + ci) * bc + cell;
+            if (whole && (reinterpret_cast<unsigned long long>(ph) & 15ull) == 0) {
+                float4 a = ld4(reinterpret_cast<const float *>(ph)), b = ld4(reinterpret_cast<const float *>(ph + 2));
+                a.x += v.x * c; a.y -= v.x * sn; a.z += v.y * c; a.w -= v.y * sn;
+                b.x += v.z * c; b.y -= v.z * sn; b.z += v.w * c; b.w -= v.w * sn;
+                stg4(reinterpret_cast<float *>(ph), a); stg4(reinterpret_cast<float *>(ph + 2), b);
+            } else {
 #pragma unroll
-    for (int q = 0; q < 4; ++q) {
-        detect_cell(P, n, 3 * family + 0, f4get(vx, q), i + q, j, k);
-        detect_cell(P, n, 3 * family + 1, f4get(vy, q), i + q, j, k);
-        detect_cell(P, n, 3 * family + 2, f4get(vz, q), i + q, j, k);
+                for (int e = 0; e < 4; ++e) {
+                    if (i + e < q.lo[0] || i + e >= q.hi[0]) continue;
+                    float2 acc = ph[e];
+                    const float x = f4get(v, e);
+                    acc.x += x * c; acc.y -= x * sn;
+                    ph[e] = acc;
+                }
+            }
+        }
     }
+}
+__device__ __forceinline__ void detect4(const StepParams &P, int n, int family, int dm, float4 vx, float4 vy, float4 vz, int i, int j, int k)
+{
+    if ((dm >> (3 * family)) & 1) detect_comp4(P, n, 3 * family + 0, vx, i, j, k);
+    if ((dm >> (3 * family)) & 2) detect_comp4(P, n, 3 * family + 1, vy, i, j, k);
+    if ((dm >> (3 * family)) & 4) detect_comp4(P, n, 3 * family + 2, vz, i, j, k);
 }
 
 // ================================================================================================
@@ -411,14 +420,16 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
             mbar_wait(&full[st_i], st_ph);
             const uint32_t so = stage_base + st_off + o_own;
             const uint32_t sp = stage_base + pv_off + o_own;       // the stage of plane kk-1 is still held
-            if (ADJ && kk >= P.dEl && kk < P.dEh && !dup && det_plane(P, kk, 0, true)) {
+            if (ADJ && kk >= P.dEl && kk < P.dEh && !dup) {
                 // B1 for E-component detectors: the cotangents are added to lamE in the stage, at my cells, before
                 // anything is live in registers (lamE is only ever read at a thread's own cells)
+                const int dm = det_mask(P, kk, true);
                 for (int c = 0; c < 3; ++c) {
+                    if (!((dm >> c) & 1)) continue;
                     const uint32_t se = so + (3 + c) * C::SLOT;
                     sts4(se, det_adjoint4(P, n, c, lds4(se), i, j, kk));
                 }
-                fence_proxy_async();
+                if (dm & 7) fence_proxy_async();
             }
             const uint32_t xs0 = stage_base + st_off + 7 * C::SLOT; // x-slab state boxes of this stage
             const float4 fx = lds4(so), fy = lds4(so + C::SLOT), fz = lds4(so + 2 * C::SLOT);
@@ -532,15 +543,18 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                 v2x = sie * e2x; v2y = sie * e2y; v2z = sie * e2z;
             } else {
                 e2x = fma4(sie, tEx, ex); e2y = fma4(sie, tEy, ey); e2z = fma4(sie, tEz, ez);
-                if (kk >= P.sEl && kk < P.sEh && src_plane(P, kk, 0)) {
-                    e2x = add_sources4(P, n, 0, e2x, i, j, kk); e2y = add_sources4(P, n, 1, e2y, i, j, kk); e2z = add_sources4(P, n, 2, e2z, i, j, kk);
+                if (kk >= P.sEl && kk < P.sEh) {
+                    const int sm = src_mask(P, kk);
+                    if (sm & 1) e2x = add_sources4(P, n, 0, e2x, i, j, kk);
+                    if (sm & 2) e2y = add_sources4(P, n, 1, e2y, i, j, kk);
+                    if (sm & 4) e2z = add_sources4(P, n, 2, e2z, i, j, kk);
                 }
                 v2x = e2x; v2y = e2y; v2z = e2z;
             }
             if (wr) {
                 float *o = dst + off;
                 stg4(o, e2x); stg4(o + nc, e2y); stg4(o + 2 * nc, e2z);
-                if (!ADJ && kk >= P.dEl && kk < P.dEh && det_plane(P, kk, 0, false)) detect4(P, n, 0, e2x, e2y, e2z, i, j, kk);
+                if (!ADJ && kk >= P.dEl && kk < P.dEh) detect4(P, n, 0, det_mask(P, kk, false), e2x, e2y, e2z, i, j, kk);
             }
             float4 Yx = v2x, Yz = v2z, Xy = v2y, Xz = v2z, Zx = v2x, Zy = v2y;
             if (ADJ && (slab_xy || zs >= 0)) {       // phase-B operands are filtered where they are produced
@@ -620,13 +634,16 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                 } else {
                     const float4 sim = has_mu ? S * ldg4(P.im + offm) : splat(S);
                     h2x = hx - sim * tHx; h2y = hy - sim * tHy; h2z = hz - sim * tHz;
-                    if (km1 >= P.sHl && km1 < P.sHh && src_plane(P, km1, 1)) {
-                        h2x = add_sources4(P, n, 3, h2x, i, j, km1); h2y = add_sources4(P, n, 4, h2y, i, j, km1); h2z = add_sources4(P, n, 5, h2z, i, j, km1);
+                    if (km1 >= P.sHl && km1 < P.sHh) {
+                        const int sm = src_mask(P, km1);
+                        if (sm & 8) h2x = add_sources4(P, n, 3, h2x, i, j, km1);
+                        if (sm & 16) h2y = add_sources4(P, n, 4, h2y, i, j, km1);
+                        if (sm & 32) h2z = add_sources4(P, n, 5, h2z, i, j, km1);
                     }
                 }
                 float *o = dst + 3 * nc + offm;
                 stg4(o, h2x); stg4(o + nc, h2y); stg4(o + 2 * nc, h2z);
-                if (!ADJ && km1 >= P.dHl && km1 < P.dHh && det_plane(P, km1, 1, false)) detect4(P, n, 1, h2x, h2y, h2z, i, j, km1);
+                if (!ADJ && km1 >= P.dHl && km1 < P.dHh) detect4(P, n, 1, det_mask(P, km1, false), h2x, h2y, h2z, i, j, km1);
             }
             if (ADJ) { cZx = Zx; cZy = Zy; }
             // the stage of plane kk-1 is no longer needed; the stage of plane kk stays for the next iteration
@@ -810,10 +827,11 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_inverse(const __grid_constant
             const float4 Dx_y = dplus_x(Ey, Ey_px), Dx_z = dplus_x(Ez, Ez_px);
             const float4 Dz_x = Ex_pz - Ex, Dz_y = Ey_pz - Ey;
             float4 Hx = fma4(S, Dy_z - Dz_y, Hpx), Hy = fma4(S, Dz_x - Dx_z, Hpy), Hz = fma4(S, Dx_y - Dy_x, Hpz);
-            if (kk >= P.sHl && kk < P.sHh && src_plane(P, kk, 1)) {
-                Hx = Hx - add_sources4(P, n, 3, splat(0.f), i, j, kk);
-                Hy = Hy - add_sources4(P, n, 4, splat(0.f), i, j, kk);
-                Hz = Hz - add_sources4(P, n, 5, splat(0.f), i, j, kk);
+            if (kk >= P.sHl && kk < P.sHh) {
+                const int sm = src_mask(P, kk);
+                if (sm & 8) Hx = Hx - add_sources4(P, n, 3, splat(0.f), i, j, kk);
+                if (sm & 16) Hy = Hy - add_sources4(P, n, 4, splat(0.f), i, j, kk);
+                if (sm & 32) Hz = Hz - add_sources4(P, n, 5, splat(0.f), i, j, kk);
             }
             // outside I the volume's own value stands (the recorded pre-step H at index lo-1)
             Hx = sel4(m0 && inz, m1 && inz, m2 && inz, m3 && inz, Hx, Hpx);
@@ -846,10 +864,11 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_inverse(const __grid_constant
                 const float4 sie = S * lds4(sp + 6 * C::SLOT);
                 const float4 lx = lds4(sp + 7 * C::SLOT), ly = lds4(sp + 8 * C::SLOT), lz = lds4(sp + 9 * C::SLOT);
                 float4 E2x = Ex - sie * qx, E2y = Ey - sie * qy, E2z = Ez - sie * qz;
-                if (kk >= P.sEl && kk < P.sEh && src_plane(P, kk, 0)) {
-                    E2x = E2x - add_sources4(P, n, 0, splat(0.f), i, j, kk);
-                    E2y = E2y - add_sources4(P, n, 1, splat(0.f), i, j, kk);
-                    E2z = E2z - add_sources4(P, n, 2, splat(0.f), i, j, kk);
+                if (kk >= P.sEl && kk < P.sEh) {
+                    const int sm = src_mask(P, kk);
+                    if (sm & 1) E2x = E2x - add_sources4(P, n, 0, splat(0.f), i, j, kk);
+                    if (sm & 2) E2y = E2y - add_sources4(P, n, 1, splat(0.f), i, j, kk);
+                    if (sm & 4) E2z = E2z - add_sources4(P, n, 2, splat(0.f), i, j, kk);
                 }
                 float *o = dst + off;
                 st_masked(o, E2x, mall, m0, m1, m2, m3);
