@@ -154,34 +154,40 @@ __device__ __noinline__ float source_at(const PT &P, int n, int comp, int i, int
     return acc;
 }
 
-// adjoint of the running DFT (B1) at cell (i,j,k) of component `comp`: sum_f Gr cos - Gi sin, with the caller's
-// phasor cotangents in det[].phasor (NULL: no cotangent for that detector)
-__device__ __noinline__ float det_adjoint_at(const StepParams &P, int n, int comp, int i, int j, int k)
+// adjoint of the running DFT (B1) at the cells (i..i+3, j, k) of component `comp`: v += sum_f Gr cos - Gi sin, with the
+// caller's phasor cotangents in det[].phasor (NULL: no cotangent for that detector)
+__device__ __noinline__ float4 det_adjoint4(const StepParams &P, int n, int comp, float4 v, int i, int j, int k)
 {
-    float acc = 0.f;
     for (int s = 0; s < P.n_det; ++s) {
         const DetectorDev &q = P.det[s];
         if (!q.phasor || !((q.mask >> comp) & 1)) continue;
-        if (i < q.lo[0] || i >= q.hi[0] || j < q.lo[1] || j >= q.hi[1] || k < q.lo[2] || k >= q.hi[2]) continue;
+        if (j < q.lo[1] || j >= q.hi[1] || k < q.lo[2] || k >= q.hi[2] || i + 3 < q.lo[0] || i >= q.hi[0]) continue;
         const int bx = q.hi[0] - q.lo[0], by = q.hi[1] - q.lo[1], bz = q.hi[2] - q.lo[2];
         const long long bc = (long long)bx * by * bz;
         const long long cell = ((long long)(k - q.lo[2]) * by + (j - q.lo[1])) * bx + (i - q.lo[0]);
         int ci = 0;
         for (int c = 0; c < comp; ++c) ci += (q.mask >> c) & 1;
         const float *csn = P.cs + ((long long)n * P.total_freq + q.cs_off) * 2;
+        const bool whole = i >= q.lo[0] && i + 3 < q.hi[0];
         for (int f = 0; f < q.n_freq; ++f) {
-            const float2 Gq = __ldg(reinterpret_cast<const float2 *>(q.phasor) + ((long long)f * q.ncomp + ci) * bc + cell);
-            acc += Gq.x * __ldg(csn + 2 * f) - Gq.y * __ldg(csn + 2 * f + 1);
+            const float c = __ldg(csn + 2 * f), sn = __ldg(csn + 2 * f + 1);
+            const float2 *ph = reinterpret_cast<const float2 *>(q.phasor) + ((long long)f * q.ncomp + ci) * bc + cell;
+            if (whole && (reinterpret_cast<unsigned long long>(ph) & 15ull) == 0) {
+                const float4 a = ldg4(reinterpret_cast<const float *>(ph)), b = ldg4(reinterpret_cast<const float *>(ph + 2));
+                v.x += a.x * c - a.y * sn; v.y += a.z * c - a.w * sn;
+                v.z += b.x * c - b.y * sn; v.w += b.z * c - b.w * sn;
+            } else {
+                float add[4] = { 0.f, 0.f, 0.f, 0.f };
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    if (i + e < q.lo[0] || i + e >= q.hi[0]) continue;
+                    const float2 Gq = __ldg(ph + e);
+                    add[e] = Gq.x * c - Gq.y * sn;
+                }
+                v.x += add[0]; v.y += add[1]; v.z += add[2]; v.w += add[3];
+            }
         }
     }
-    return acc;
-}
-__device__ __noinline__ float4 det_adjoint4(const StepParams &P, int n, int comp, float4 v, int i, int j, int k)
-{
-    v.x += det_adjoint_at(P, n, comp, i + 0, j, k);
-    v.y += det_adjoint_at(P, n, comp, i + 1, j, k);
-    v.z += det_adjoint_at(P, n, comp, i + 2, j, k);
-    v.w += det_adjoint_at(P, n, comp, i + 3, j, k);
     return v;
 }
 
