@@ -46,7 +46,10 @@
  * Gauss law, forward-N/inverse-N recovery, tape == reversible gradient,
  * gradient vs central finite differences, adjoint dot-product identity,
  * CPML vs big-box, late-time decay, linearity/null tests, the paper's
- * Table 2 step counts (Courant convention).
+ * Table 2 step counts (Courant convention); CPML coefficients a, b against
+ * the zero-frequency limit and the low-frequency response of ref. 7's
+ * stretch factor; the rho chain rule (B6) against a central finite
+ * difference of the loss with respect to rho.
  * Parity unpinned: agreement with the paper's own FDTDX outputs (no numbers,
  * code, geometry or data are available) and the specific CPML constants /
  * DFT normalisation FDTDX uses.
@@ -774,4 +777,27 @@ int orc_backward_tape(orc_state *st, const REAL *ie, const REAL *im,
     if (dL_dfields0) memcpy(dL_dfields0, lam, 6 * nc * sizeof(REAL));
     free(lam);
     return 0;
+}
+
+/* ------------------------------------------------------------------------ */
+/* B6: chain rule to the design parameters (reading R20).    */
+/* On a design box the permittivity is eps = eps_bg + delta_eps * rho, the   */
+/* solver's input is ie = 1/eps, hence                                       */
+/*   d(ie)/d(rho) = -delta_eps / eps^2 = -delta_eps * ie^2                   */
+/*   dL/drho[cell] = g[cell] * d(ie)/d(rho)[cell],   g = dL/d(inv_eps).      */
+/* out is box-shaped [k][j][i].  Pinned by a central finite difference of L  */
+/* with respect to rho (tests/test_oracle_pins.py), not by this formula.     */
+/* ------------------------------------------------------------------------ */
+void orc_grad_rho(const orc_desc *D, const REAL *g, const REAL *ie, double delta_eps,
+                  const int lo[3], const int hi[3], REAL *out)
+{
+    const int bx = hi[0] - lo[0], by = hi[1] - lo[1];
+    for (int k = lo[2]; k < hi[2]; ++k)
+        for (int j = lo[1]; j < hi[1]; ++j)
+            for (int i = lo[0]; i < hi[0]; ++i) {
+                const size_t p = IDX(i, j, k);
+                const size_t c = ((size_t)(k - lo[2]) * by + (j - lo[1])) * bx + (i - lo[0]);
+                const REAL dinv = -(REAL)delta_eps * ie[p] * ie[p];
+                out[c] = g[p] * dinv;
+            }
 }

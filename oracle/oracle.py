@@ -94,6 +94,8 @@ def _lib(tag: str):
         L.orc_backward_tape.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p,
                                         C.c_void_p, C.c_int, C.c_void_p, C.c_void_p,
                                         C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_grad_rho.argtypes = [C.POINTER(_Desc), C.c_void_p, C.c_void_p, C.c_double,
+                                   C.POINTER(C.c_int), C.POINTER(C.c_int), C.c_void_p]
         L.orc_set_ftz.argtypes = [C.c_int]
         L.orc_num_threads.restype = C.c_int
         _LIBS[tag] = L
@@ -299,6 +301,15 @@ class Oracle:
                                       int(n_steps), _ptr(tape), _ptr(g), _ptr(lam0))
         assert rc == 0, rc
         return g, lam0
+
+    def grad_rho(self, g, inv_eps, delta_eps, lo, hi):
+        """B6 (reading R20): dL/drho on the design box [lo, hi) from g = dL/d(inv_eps); box-shaped [k][j][i]."""
+        g = self.arr(g, self.shape)
+        ie = self.arr(inv_eps, self.shape)
+        out = np.zeros((hi[2] - lo[2], hi[1] - lo[1], hi[0] - lo[0]), dtype=self.dtype)
+        self.L.orc_grad_rho(C.byref(self.desc), _ptr(g), _ptr(ie), float(delta_eps),
+                            (C.c_int * 3)(*lo), (C.c_int * 3)(*hi), _ptr(out))
+        return out
 
     def set_ftz(self, on=True):
         self.L.orc_set_ftz(int(on))

@@ -456,3 +456,92 @@ def test_cpml_tables_structure():
     b2, a2, k2 = o2.cpml_table(2, 0)
     assert np.all(k2 == 1) and np.allclose(a2[:d], b2[:d] - 1)
     assert math.isclose(b2[0], math.exp(-(3.2 / math.sqrt(2.085)) * S), rel_tol=1e-14)
+
+
+# ----------------------------------------------------------------------------- CPML coefficients a, b
+def _cpml_profile(n, d, half, m=3.0, sigma_max=0.8 * 4.0, kappa_max=3.0, alpha_max=0.05, alpha_m=1.0):
+    """sigma~, kappa, alpha~ of reading R8 at the table positions (x = p, or p + 1/2 when `half`), recomputed here."""
+    x = np.arange(n, dtype=np.float64) + (0.5 if half else 0.0)
+    rho = np.maximum(0.0, np.maximum(d - x, x - (n - d)))
+    r = rho / d
+    inside = rho > 0
+    sig = np.where(inside, sigma_max * r ** m, 0.0)
+    kap = np.where(inside, 1.0 + (kappa_max - 1.0) * r ** m, 1.0)
+    alp = np.where(inside, alpha_max * (1.0 - r) ** alpha_m, 0.0)
+    return inside, sig, kap, alp
+
+
+@pytest.mark.parametrize("kappa_max,alpha_max", [(3.0, 0.05), (1.0, 0.0), (2.0, 0.3)])
+def test_cpml_zero_frequency_limit_of_the_stretch_factor(kappa_max, alpha_max):
+    """PAPER.md L72 (CPML, ref. 7): the stretched derivative is d/s with s(w) = kappa + sigma/(alpha + i w eps0).
+    A constant input d drives psi to a d/(1-b), so the recursion's DC gain 1/kappa + a/(1-b) must equal
+    1/s(0) = 1/(kappa + sigma~/alpha~) = alpha~/(sigma~ + kappa alpha~)  (0 where alpha~ = 0), at every PML position
+    of both staggerings.  A kappa dropped from a's denominator, or a sign slip, fails this."""
+    n, d = 30, 8
+    o = Oracle(n, n + 2, n + 4, S, pml_cells=d, pml_kappa_max=kappa_max, pml_alpha_max=alpha_max)
+    seen_alpha_zero = seen_alpha_pos = False
+    for axis, na in enumerate((n, n + 2, n + 4)):
+        for half in (0, 1):
+            b, a, ik = o.cpml_table(axis, half)
+            inside, sig, kap, alp = _cpml_profile(na, d, half, kappa_max=kappa_max, alpha_max=alpha_max)
+            assert inside.sum() in (2 * d, 2 * d - 1)
+            dc = ik + np.where(inside, a / np.where(inside, 1.0 - b, 1.0), 0.0)
+            want = np.where(inside, alp / np.where(inside, sig + kap * alp, 1.0), 1.0)
+            assert np.max(np.abs(dc - want)) < 1e-13, (axis, half)
+            seen_alpha_zero |= bool(np.any(inside & (alp == 0)))
+            seen_alpha_pos |= bool(np.any(inside & (alp > 0)))
+    assert seen_alpha_zero and (seen_alpha_pos or alpha_max == 0)
+
+
+def test_cpml_coefficients_are_the_integrated_impulse_response():
+    """Ref. 7's recursive convolution: 1/s(w) = 1/kappa + FT[zeta], zeta(t) = -(sigma~ S/kappa^2) exp(-(sigma~/kappa + alpha~) S t)
+    (t in steps; (sigma/eps0) dt = sigma~ S), and psi_n = sum_m Z(m) d_{n-m} with Z(m) the integral of zeta over [m, m+1].
+    The tables must satisfy a = Z(0) and a b = Z(1): checked by Gauss-Legendre quadrature of zeta, which pins a and b
+    (exponent, the factor S, kappa in both places) without retyping their closed forms."""
+    n, d, kmax, amax = 26, 7, 3.0, 0.05
+    o = Oracle(n, n, n, S, pml_cells=d, pml_kappa_max=kmax, pml_alpha_max=amax, pml_eps_bg=2.085)
+    xg, wg = np.polynomial.legendre.leggauss(24)
+    for half in (0, 1):
+        b, a, ik = o.cpml_table(1, half)
+        inside, sig, kap, alp = _cpml_profile(n, d, half, sigma_max=0.8 * 4.0 / math.sqrt(2.085), kappa_max=kmax, alpha_max=amax)
+        for p in np.nonzero(inside)[0]:
+            zeta = lambda t: -(sig[p] * S / kap[p] ** 2) * np.exp(-(sig[p] / kap[p] + alp[p]) * S * t)
+            Z0 = 0.5 * np.sum(wg * zeta(0.5 * (xg + 1.0)))
+            Z1 = 0.5 * np.sum(wg * zeta(1.0 + 0.5 * (xg + 1.0)))
+            assert abs(a[p] - Z0) < 1e-13 and abs(a[p] * b[p] - Z1) < 1e-13, (half, p, a[p], Z0)
+            assert abs(ik[p] - 1.0 / kap[p]) < 1e-15
+
+
+# ----------------------------------------------------------------------------- B6
+def test_b6_rho_chain_rule_against_finite_differences():
+    """SURVEY 8(a) B6 / reading R20: eps = eps_bg + delta_eps rho on a design box, solver input inv_eps = 1/eps.
+    dL/drho from the oracle (time-reversed gradient, then orc_grad_rho) against central finite differences of the
+    loss with respect to single rho voxels on the tiny CPML grid (box offset from the origin, inside I)."""
+    w = wl.tiny_pml(n_steps=30)
+    shape = (w.nz, w.ny, w.nx)
+    d = w.pml_cells
+    lo, hi = (d + 1, d + 1, d + 1), (w.nx - d - 1, w.ny - d, w.nz - d - 1)          # (i,j,k), inside I = [d, N-d)
+    box = (slice(lo[2], hi[2]), slice(lo[1], hi[1]), slice(lo[0], hi[0]))
+    eps_bg, delta_eps = 1.5, 2.5
+    rho = _rng(17).random((hi[2] - lo[2], hi[1] - lo[1], hi[0] - lo[0]))
+    wfield = _rng(18).random((6,) + shape)
+
+    def inv_eps_of(rho_):
+        ie = w.inv_eps.astype(np.float64).copy()
+        ie[box] = 1.0 / (eps_bg + delta_eps * rho_)
+        return ie
+
+    ie = inv_eps_of(rho)
+    o, f, out, L, dLp, dLf = _run_loss(w, ie, wfield, record=True)
+    g, _ = o.backward(f, ie, w.meta["inv_mu"], w.sources, w.detectors, dLp, dLf, w.n_steps, out["rec"])
+    dL_drho = o.grad_rho(g, ie, delta_eps, lo, hi)
+    assert dL_drho.shape == rho.shape
+    scale = np.max(np.abs(dL_drho))
+    assert scale > 0
+    h = 1e-6
+    for v in [(0, 0, 0), (1, 2, 3), (rho.shape[0] - 1, rho.shape[1] - 1, rho.shape[2] - 1), (2, 0, 1)]:
+        rp, rm = rho.copy(), rho.copy()
+        rp[v] += h
+        rm[v] -= h
+        fd = (_run_loss(w, inv_eps_of(rp), wfield)[3] - _run_loss(w, inv_eps_of(rm), wfield)[3]) / (2 * h)
+        assert abs(fd - dL_drho[v]) < 2e-6 * scale + 1e-6 * abs(fd), (v, fd, dL_drho[v])
