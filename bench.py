@@ -1,20 +1,28 @@
 #!/usr/bin/env python
-"""bench.py -- Yee cell-updates/s of the FDTD hot path on B200 (BASELINE.json metric).
+"""bench.py -- Yee cell-updates/s of the FDTD hot path on B200 (BASELINE.json metric; SURVEY.md 8(d)).
 
-One "step" = one whole pass of the hot path over one synthetic problem: fdtd_forward with
-interface recording (F1..F8) + the caller's loss cotangent + fdtd_backward (B0..B5) + the
-rho chain rule (B6) on the graded config C3 (200^3, 12-cell CPML, 2000 time steps, 864k design
-voxels).  value = cells * n_time_steps * K / (time of K steps), summed over ranks.
+One "step" = one whole pass of the hot path over one synthetic problem: fdtd_forward with interface
+recording (F1..F8) + the caller's loss cotangent + fdtd_backward (B0..B5) + the rho chain rule (B6).
+Default workload: the graded config C3 (200^3, 12-cell CPML, 2000 time steps, 864k design voxels).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--time-steps T]
+    value  = cells * n_time_steps * K / (time of K steps), summed over ranks, with record=1: the recorder on
+             the PML / interior interface, the whole interior reconstructed (t_fwd(record=1) +
+             t_bwd, 161 B/cell/step on C3);
+    fwd    = cells * n_time_steps / t_fwd(record=0);
+    n1_design_box_recorder = the same gradient with record=2 (faces of the design box
+             recorded, only that box reconstructed; 135 B/cell/step on C3), a named extra beside `value`.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload c3|c4|c5] [--grid N] [--time-steps T] [--record 1|2|both]
 
 N > 1 (torchrun): every rank runs an independent problem (seed + rank), no data-path collective
-("weak" scaling over independent inverse-design problems; DESIGN.md section 9).
+("weak" scaling over independent inverse-design problems; DESIGN.md section 10).
 --impl reference times the CPU oracle (oracle/, fp32 build, all host cores) on a bounded sample.
 """
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
 import statistics
@@ -27,8 +35,17 @@ from pathlib import Path
 ROOT = Path(__file__).resolve().parent
 sys.path.insert(0, str(ROOT))
 
-METRIC = "Yee cell-updates/s, forward + time-reversed backward (C3 gradient)"
+METRIC = "Yee cell-updates/s, forward(record=1) + time-reversed backward (gradient)"
 UNIT = "Mcells/s"
+KERNEL_SOURCES = ("kernels_step.cu", "kernels_generic.cu", "fused_common.cuh", "fdtd_internal.h")
+
+
+def kernel_source_hash() -> str:
+    """sha256 over the kernel sources: profiles/traffic.json records the hash of the build its ncu capture was taken on."""
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES:
+        h.update((ROOT / "paper_2412_12360_b200" / "csrc" / name).read_bytes())
+    return h.hexdigest()
 
 
 # ------------------------------------------------------------------------------------------------
@@ -50,9 +67,9 @@ def algorithmic_bytes(w, grad_cells: int, recording: bool, has_mu: bool = False,
         "fused_forward_step": cells * (52 + mu) + slab * 32 + 2 * rec,
         # fused adjoint step (B2+B5): 6 R + 6 W cotangents + ie over the grid, adjoint psi R/W on slabs; the face
         # injection of the reverse sweep runs beside it and is timed with it
-        "fused_adjoint_step": cells * 52 + slab * 32 + 2 * rec,
-        # fused inverse step (B3+B4) over I: R E',H' (6), ie, lamE' (3), W E,H (6); g R/W on the grad box
-        "fused_inverse_step": inter * 64 + grad_cells * 8,
+        "fused_adjoint_step": cells * (52 + mu) + slab * 32 + 2 * rec,
+        # fused inverse step (B3+B4) over the box: R E',H' (6), ie, lamE' (3), W E,H (6); g R/W on the grad box
+        "fused_inverse_step": inter * (64 + mu) + grad_cells * 8,
         "update_E": cells * 40 + slab * 16,
         "update_H": cells * (36 + mu) + slab * 16,
         "adjoint_H": cells * (36 + mu) + slab * 16,
@@ -62,6 +79,20 @@ def algorithmic_bytes(w, grad_cells: int, recording: bool, has_mu: bool = False,
         "record_faces": 2 * 4 * face,
         "inject_faces": 2 * 4 * face,
     }
+
+
+def whole_job_bytes_per_cell_step(w, grad_cells: int, rbox=None) -> dict:
+    """SURVEY 8(d) whole-job figures per cell and time step: forward alone (6 R + 6 W + inv_eps + psi on the slabs), and
+    forward + adjoint pass + inverse pass + g, where the inverse pass counts 12 floats per box cell (R E', H'; W E, H):
+    inv_eps and lamE' are counted once, with the adjoint pass (13 + 12 + 2 floats; C3: 63.5 / 161.0).
+    The per-kernel figure of k_inverse (algorithmic_bytes) is 16 floats per box cell because as a launch of its own it
+    has to read inv_eps and lamE' again; the whole-job roofline is not credited with that re-read."""
+    a0 = algorithmic_bytes(w, grad_cells, recording=False)
+    d = w.pml_cells
+    bx, by, bz = rbox if rbox else (w.nx - 2 * d, w.ny - 2 * d, w.nz - 2 * d)
+    c = float(w.cells)
+    return {"fwd": a0["fused_forward_step"] / c,
+            "fwd_bwd": (2 * a0["fused_forward_step"] + bx * by * bz * 48 + grad_cells * 8) / c}
 
 
 # ------------------------------------------------------------------------------------------------
@@ -116,32 +147,63 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------
-def cpu_oracle_rate(w, sample_steps: int):
-    """Times the oracle as it stands (fp32 build, OpenMP over all host cores, FTZ on) on the first
-    `sample_steps` time steps of the workload: forward with recording + reversible backward."""
+def make_workload(args, rank: int = 0):
+    from paper_2412_12360_b200 import workloads as wl
+    from paper_2412_12360_b200 import sharding
+    if args.workload == "c4":
+        w = wl.c4(n_steps=args.time_steps or 5000)
+        w.meta.setdefault("delta_eps", 12.25 - 2.085)
+    elif args.workload == "c5":
+        w = wl.c5(args.grid or 256, n_steps=args.time_steps or 500)          # configs[4]: loss over I, gradient on all of I
+    else:
+        w = wl.c3(n=args.grid or 200, n_steps=args.time_steps or 2000, seed=sharding.problem_seed(3, rank))
+    return w
+
+
+def oracle_loss_cotangents(w, f, phasors):
+    """The caller's loss on the oracle side (numpy), same definitions as the GPU leg."""
+    import numpy as np
+    if w.loss == "phasor_power":
+        return [2.0 * P if i in w.loss_detectors else None for i, P in enumerate(phasors)], None
+    dLf = np.zeros_like(f)
+    d = w.pml_cells
+    sl = (slice(0, 3), slice(d, w.nz - d), slice(d, w.ny - d), slice(d, w.nx - d))
+    dLf[sl] = 2.0 * f[sl]
+    return None, dLf
+
+
+def cpu_oracle_rate(w, sample_steps: int, threads: int = 0):
+    """Times the oracle as it stands (fp32 build, OpenMP, FTZ on) on the first `sample_steps` time steps of the
+    workload: forward with recording + reversible backward.  threads = 0: all host cores."""
     import numpy as np
     from oracle.oracle import Oracle
     o = Oracle(**w.grid_kwargs(), dtype=np.float32)
+    all_cores = os.cpu_count() or 1
+    o.set_num_threads(threads if threads > 0 else all_cores)
     o.set_ftz(True)
     f = np.zeros((6, w.nz, w.ny, w.nx), dtype=np.float32)
     t0 = time.perf_counter()
     out = o.forward(f, w.inv_eps, None, w.sources, w.detectors, sample_steps, record=w.pml_cells > 0)
     t1 = time.perf_counter()
-    dLp = [2.0 * P if i in w.loss_detectors else None for i, P in enumerate(out["phasors"])]
-    o.backward(f, w.inv_eps, None, w.sources, w.detectors, dLp, None, sample_steps, out["rec"])
+    dLp, dLf = oracle_loss_cotangents(w, f, out["phasors"])
+    o.backward(f, w.inv_eps, None, w.sources, w.detectors, dLp, dLf, sample_steps, out["rec"])
     t2 = time.perf_counter()
     cells = w.cells * sample_steps
-    return {"value": cells / (t2 - t0) / 1e6, "fwd_value": cells / (t1 - t0) / 1e6, "unit": UNIT,
-            "cores": o.num_threads(), "kind": "oracle",
-            "sample": f"{w.name} {w.nx}x{w.ny}x{w.nz} grid, first {sample_steps} of {w.n_steps} time steps, "
-                      f"forward(record)+reversible backward, fp32 build of oracle/fdtd_oracle.c, OpenMP, FTZ"}
+    res = {"value": cells / (t2 - t0) / 1e6, "fwd_value": cells / (t1 - t0) / 1e6, "unit": UNIT,
+           "cores": o.num_threads(), "kind": "oracle",
+           "sample": f"{w.name} {w.nx}x{w.ny}x{w.nz} grid, first {sample_steps} of {w.n_steps} time steps, "
+                     f"forward(record)+reversible backward, fp32 build of oracle/fdtd_oracle.c, OpenMP, FTZ"}
+    o.set_num_threads(all_cores)
+    return res
 
 
 def workload_config(w, extra=None):
     cfg = {"workload": f"{w.name}: {w.nx}x{w.ny}x{w.nz} fp32 Yee grid, {w.pml_cells}-cell CPML, {w.n_steps} time steps, "
-                       f"forward(record)+reversible backward, grad box = design region",
+                       f"forward(record=1: PML/interior interface)+reversible backward over the whole interior, "
+                       + ("gradient on the design region" if w.design_lo else "gradient on the whole interior"),
            "time_steps": w.n_steps, "cells": w.cells,
-           "l2": "inputs larger than L2 (working set > 0.5 GB vs 126 MB L2); no flush needed"}
+           "l2": "inputs larger than L2 (working set > 0.5 GB vs 126 MB L2); no flush needed" if w.cells * 52 > 126e6
+                 else "grid fits in L2: fractions of the HBM roofline may exceed 1 (SURVEY 8(d))"}
     if extra:
         cfg.update(extra)
     return cfg
@@ -151,8 +213,7 @@ def run_reference(args, rank):
     """--impl reference: the CPU oracle on the host cores (bounded sample per step)."""
     if rank != 0:
         return
-    from paper_2412_12360_b200 import workloads as wl
-    w = wl.c3(n_steps=args.time_steps)
+    w = make_workload(args)
     sample = args.ref_sample_steps
     for _ in range(args.warmup):
         cpu_oracle_rate(w, max(1, sample // 4))
@@ -176,16 +237,18 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--time-steps", type=int, default=2000, help="FDTD time steps per gradient (C3: 2000)")
-    ap.add_argument("--grid", type=int, default=200, help="C3 grid size per axis (200)")
-    ap.add_argument("--workload", default="c3", choices=["c3", "c4"],
-                    help="c3: the graded config (default); c4: configs[3], 800x800x600 memory-scale run (use a small --time-steps)")
+    ap.add_argument("--time-steps", type=int, default=0, help="FDTD time steps per gradient (default: the config's: C3 2000, C4 5000, C5 500)")
+    ap.add_argument("--grid", type=int, default=0, help="grid size per axis: C3 recipe scaled to N^3 (default 200), C5 N (default 256)")
+    ap.add_argument("--workload", default="c3", choices=["c3", "c4", "c5"],
+                    help="c3: the graded config (default); c4: configs[3], 800x800x600 memory-scale run; c5: configs[4], the size sweep")
     ap.add_argument("--path", default="auto", choices=["auto", "generic", "fused"])
     ap.add_argument("--ref-sample-steps", type=int, default=12)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--record", type=int, default=2, choices=[1, 2],
-                    help="1: record the PML/interior interface, reconstruct the interior; 2: record the faces of the design box, reconstruct that box only")
+    ap.add_argument("--record", default="", choices=["", "1", "2", "both"],
+                    help="1: `value` only (record the PML/interior interface, reconstruct the interior); 2: `value` on the "
+                         "design-box recorder instead (labelled); both (default where there is a design box and memory allows): "
+                         "`value` on record=1 and the record=2 figure beside it")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -215,19 +278,28 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- workload: C3 (seed + rank: every rank an independent problem) -----------------------------
-    if args.workload == "c4":
-        w = wl.c4(n_steps=args.time_steps)
-        w.meta.setdefault("delta_eps", 12.25 - 2.085)
-    else:
-        w = wl.c3(n=args.grid, n_steps=args.time_steps, seed=sharding.problem_seed(3, rank))
+    # ---- workload (seed + rank: every rank an independent problem) ---------------------------------
+    w = make_workload(args, rank)
     T = w.n_steps
+    has_box = w.design_lo is not None
+    rec_arg = args.record or ("both" if has_box and args.workload != "c4" else ("2" if args.workload == "c4" else "1"))
+    if not has_box:
+        rec_arg = "1"
+    main_record = 2 if rec_arg == "2" else 1
     path = {"auto": B.FDTD_PATH_AUTO, "generic": B.FDTD_PATH_GENERIC, "fused": B.FDTD_PATH_FUSED}[args.path]
-    kw = w.grid_kwargs()
-    kw.update(max_steps=T, record=args.record, grad_lo=w.design_lo, grad_hi=w.design_hi, path=path)
-    grid = B.Grid(**kw)
-    kw_f = dict(kw); kw_f.update(record=False)
-    grid_f = B.Grid(**kw_f)                                   # forward-only grid (no recorder)
+    d = w.pml_cells
+    dlo, dhi = (w.design_lo, w.design_hi) if has_box else ((d, d, d), (w.nx - d, w.ny - d, w.nz - d))
+
+    def make_grid(record, staging=False):
+        kw = w.grid_kwargs()
+        kw.update(max_steps=T, record=record, path=path, flags=B.FDTD_FLAG_HOST_STAGING if staging else 0)
+        if has_box:
+            kw.update(grad_lo=dlo, grad_hi=dhi)
+        return B.Grid(**kw)
+
+    grid = make_grid(main_record, staging=not args.no_e2e)          # the `value` grid
+    grid2 = make_grid(2) if rec_arg == "both" else None             # N1 extra: design-box recorder
+    grid_f = make_grid(0)                                           # forward-only grid (no recorder)
     stream = torch.cuda.Stream()
     dev = torch.device("cuda", local_rank)
     ie = torch.as_tensor(w.inv_eps).to(dev)
@@ -235,12 +307,20 @@ def main():
     for s in w.sources:                                        # resident descriptors
         s.waveform = torch.as_tensor(s.waveform).to(dev)
         s.profile = None if s.profile is None else torch.as_tensor(s.profile).to(dev)
-    phasors = [torch.zeros(d.phasor_shape, dtype=torch.float32, device=dev) for d in w.detectors]
+    phasors = [torch.zeros(dt.phasor_shape, dtype=torch.float32, device=dev) for dt in w.detectors]
     grad = torch.empty((w.nz, w.ny, w.nx), dtype=torch.float32, device=dev)
-    dlo, dhi = w.design_lo, w.design_hi
-    drho = torch.empty((dhi[2] - dlo[2], dhi[1] - dlo[1], dhi[0] - dlo[0]), dtype=torch.float32, device=dev)
-    grad_cells = drho.numel()
-    delta_eps = float(w.meta["delta_eps"])
+    drho = torch.empty((dhi[2] - dlo[2], dhi[1] - dlo[1], dhi[0] - dlo[0]), dtype=torch.float32, device=dev) if has_box else None
+    grad_cells = (dhi[0] - dlo[0]) * (dhi[1] - dlo[1]) * (dhi[2] - dlo[2])
+    delta_eps = float(w.meta.get("delta_eps", 0.0))
+    dLf_buf = torch.zeros_like(fields) if w.loss != "phasor_power" else None
+    inter = (slice(0, 3), slice(d, w.nz - d), slice(d, w.ny - d), slice(d, w.nx - d))
+
+    def loss_cotangents():
+        """The caller's loss (torch ops on the caller's side of the ABI): phasor power or sum E^2 over I."""
+        if w.loss == "phasor_power":
+            return [2.0 * P if i in w.loss_detectors else None for i, P in enumerate(phasors)], None
+        dLf_buf[inter] = 2.0 * fields[inter]
+        return None, dLf_buf
 
     def gradient_step(g):
         """One pass of the whole hot path, inputs resident in HBM."""
@@ -248,9 +328,10 @@ def main():
         for P in phasors:
             P.zero_()
         g.forward(fields, ie, None, w.sources, w.detectors, T, phasors=phasors)
-        dLp = [2.0 * P if i in w.loss_detectors else None for i, P in enumerate(phasors)]   # caller's loss
-        g.backward(fields, ie, None, w.sources, w.detectors, dLp, None, T, out=grad)
-        B.fdtd_grad_rho(g.h, grad, ie, delta_eps, dlo, dhi, drho, g.stream())
+        dLp, dLf = loss_cotangents()
+        g.backward(fields, ie, None, w.sources, w.detectors, dLp, dLf, T, out=grad)
+        if has_box:
+            B.fdtd_grad_rho(g.h, grad, ie, delta_eps, dlo, dhi, drho, g.stream())
 
     def forward_only(g):
         fields.zero_()
@@ -268,6 +349,11 @@ def main():
         barrier()
         return sharding.max_over_ranks(e0.elapsed_time(e1), device=dev)
 
+    def loss_value():
+        if w.loss == "phasor_power":
+            return float(sum((P.double() ** 2).sum() for i, P in enumerate(phasors) if i in w.loss_detectors))
+        return None
+
     with torch.cuda.stream(stream):
         for _ in range(args.warmup):
             gradient_step(grid)
@@ -277,8 +363,18 @@ def main():
         ms_total = timed(lambda: gradient_step(grid), args.steps)
         clocks = sampler.stop()
         launches = grid.info().kernel_launches - l0
-        loss = float(sum((P.double() ** 2).sum() for i, P in enumerate(phasors) if i in w.loss_detectors))
-        gnorm = float(drho.double().abs().max())
+        loss = loss_value()
+        gnorm = float((drho if has_box else grad).double().abs().max())
+
+        # N1 extra: the same gradient with the design-box recorder (record=2)
+        n1 = None
+        if grid2 is not None:
+            reps2 = max(1, min(args.steps, 3))
+            for _ in range(min(args.warmup, 2)):
+                gradient_step(grid2)
+            ms2 = timed(lambda: gradient_step(grid2), reps2)
+            n1 = {"value": sharding.whole_job_rate(w.cells * T, reps2, ms2, world), "unit": UNIT, "ms_per_step": ms2 / reps2,
+                  "max_abs_dL_drho": float(drho.double().abs().max()), "loss": loss_value()}
 
         # forward-only (record=0) rate, same workload
         for _ in range(min(args.warmup, 2)):
@@ -286,14 +382,14 @@ def main():
         ms_fwd = timed(lambda: forward_only(grid_f), max(1, args.steps))
 
         # adjoint sweep only (dL_dinv_eps = NULL: one k_step<adjoint> launch per time step), same cotangent seed
-        dLp_t = [2.0 * P if i in w.loss_detectors else None for i, P in enumerate(phasors)]
+        dLp_t, dLf_t = loss_cotangents()
 
         def adjoint_only(g):
-            g.backward(fields, ie, None, w.sources, w.detectors, dLp_t, None, T, want_grad=False)
+            g.backward(fields, ie, None, w.sources, w.detectors, dLp_t, dLf_t, T, want_grad=False)
 
         adjoint_only(grid_f)
-        ms_adj = timed(lambda: adjoint_only(grid_f), max(1, min(args.steps, 3)))
         reps_adj = max(1, min(args.steps, 3))
+        ms_adj = timed(lambda: adjoint_only(grid_f), reps_adj)
 
         # ---- per-kernel roofline: one more pass with every step kernel bracketed by CUDA events --------
         B.fdtd_set_profiling(grid.h, True)
@@ -312,8 +408,9 @@ def main():
         peak, peak_src = float(json.loads(peaks_file.read_text())["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     else:
         peak, peak_src = 6650.0, "fallback (B200_PROFILING.md)"
-    rbox = tuple(dhi[a] - dlo[a] for a in range(3)) if args.record == 2 else None
-    alg = algorithmic_bytes(w, grad_cells, recording=True, rbox=rbox)
+    dbox = tuple(dhi[a] - dlo[a] for a in range(3))
+    rbox_main = dbox if (main_record == 2 and has_box) else None
+    alg = algorithmic_bytes(w, grad_cells, recording=True, rbox=rbox_main)
     kernels = {}
     for name, (n, ms) in prof.items():
         if name in alg and n:
@@ -325,16 +422,25 @@ def main():
     tot_ms = sum(ms for _, ms in prof.values()) or 1.0
     for name, (n, ms) in prof.items():
         kernels[name]["share_of_step"] = ms / tot_ms
-    info_path_fused = grid.info().path == 2
+    info = grid.info()
+    info_path_fused = info.path == 2
     dom = max((k for k in kernels if "achieved_gbs" in kernels[k]), key=lambda k: prof[k][1], default=None)
     roofline = None
     if dom:
-        traffic = None
-        tf = ROOT / "profiles" / "traffic.json"      # dram bytes per launch from the committed ncu --set full capture
+        # dram bytes per launch from the committed ncu --set full capture; refused when the kernel sources changed since
+        traffic, traffic_note = None, "no profiles/traffic.json"
+        tf = ROOT / "profiles" / "traffic.json"
         if tf.exists():
-            traffic = json.loads(tf.read_text()).get(dom)
+            tj = json.loads(tf.read_text())
+            if tj.get("kernel_source_sha256") != kernel_source_hash():
+                traffic_note = "profiles/traffic.json was captured on other kernel sources (hash mismatch): not reported"
+            elif tj.get("workload") not in (None, w.name) or (tj.get("grid") not in (None, [w.nx, w.ny, w.nz])):
+                traffic_note = "profiles/traffic.json was captured on another workload: not reported"
+            else:
+                traffic, traffic_note = tj.get(dom), tj.get("how", "ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum per launch")
         roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["achieved_gbs"], "peak": peak,
                     "peak_source": peak_src, "unit": "GB/s", "frac": kernels[dom]["frac"], "traffic": traffic,
+                    "traffic_note": traffic_note,
                     "alg_bytes_per_launch": alg[dom], "avg_launch_us": kernels[dom]["avg_us"],
                     "frac_of_8000": kernels[dom]["achieved_gbs"] / 8000.0}
         # the same kernel template inside the replayed CUDA graph (no events between launches): the forward-only
@@ -345,7 +451,7 @@ def main():
             roofline["forward_step_in_graph"] = {"avg_launch_us": us, "alg_bytes_per_launch": fb,
                                                  "achieved": fb / us / 1e3, "frac": fb / us / 1e3 / peak}
             # likewise the adjoint-sweep-only pass: one k_step<adjoint> launch per time step (its time also holds the
-            # cotangent seed and the copy of the result: 6 volumes each, once per 2000 launches)
+            # cotangent seed and the copy of the result: 6 volumes each, once per T launches)
             ab = algorithmic_bytes(w, grad_cells, recording=False)["fused_adjoint_step"]
             us = ms_adj / reps_adj / T * 1e3
             roofline["adjoint_step_in_graph"] = {"avg_launch_us": us, "alg_bytes_per_launch": ab,
@@ -360,14 +466,29 @@ def main():
                                 alg_bytes_per_launch=g_["alg_bytes_per_launch"], frac_of_8000=g_["achieved"] / 8000.0,
                                 method=f"{ing}: CUDA events around a pass of {T} back-to-back launches of this kernel "
                                        "in the replayed graph, time / launches")
+        # whole-job fractions: algorithmic B/cell/step x rate against the measured peak and the 8000 GB/s bar
+        bpc = whole_job_bytes_per_cell_step(w, grad_cells, rbox=rbox_main)
+        wj = {"fwd": {"bytes_per_cell_step": bpc["fwd"], "achieved": bpc["fwd"] * fwd_value / world / 1e3},
+              f"fwd_bwd_record{main_record}": {"bytes_per_cell_step": bpc["fwd_bwd"], "achieved": bpc["fwd_bwd"] * value / world / 1e3}}
+        if n1 is not None:
+            b2 = whole_job_bytes_per_cell_step(w, grad_cells, rbox=dbox)["fwd_bwd"]
+            wj["fwd_bwd_record2"] = {"bytes_per_cell_step": b2, "achieved": b2 * n1["value"] / world / 1e3}
+            n1["bytes_per_cell_step"] = b2
+        for v in wj.values():
+            v["frac"] = v["achieved"] / peak
+            v["frac_of_8000"] = v["achieved"] / 8000.0
+        roofline["whole_job"] = wj
 
     # ---- end to end through the host-buffer C ABI (pinned host memory, H2D/D2H inside the timed region) ----
     e2e = None
     if not args.no_e2e:
         h_ie = torch.as_tensor(w.inv_eps).pin_memory()
         h_grad = torch.empty((w.nz, w.ny, w.nx), dtype=torch.float32).pin_memory()
-        h_ph = [torch.zeros(d.phasor_shape, dtype=torch.float32).pin_memory() for d in w.detectors]
-        h_cot = [torch.zeros(d.phasor_shape, dtype=torch.float32).pin_memory() for d in w.detectors]
+        h_ph = [torch.zeros(dt.phasor_shape, dtype=torch.float32).pin_memory() for dt in w.detectors]
+        h_cot = [torch.zeros(dt.phasor_shape, dtype=torch.float32).pin_memory() for dt in w.detectors]
+        field_loss = w.loss != "phasor_power"
+        h_fields = torch.zeros((6, w.nz, w.ny, w.nx), dtype=torch.float32).pin_memory() if field_loss else None
+        h_dLf = torch.zeros((6, w.nz, w.ny, w.nx), dtype=torch.float32).pin_memory() if field_loss else None
         host_src = [wl.Source(s.component, s.lo, s.hi, s.waveform.cpu().numpy(),
                               None if s.profile is None else s.profile.cpu().numpy()) for s in w.sources]
         sarr, ns, k1 = grid.marshal_sources(host_src, host=True)
@@ -377,50 +498,68 @@ def main():
         for i in range(nd):
             cot[i] = h_cot[i].data_ptr() if i in w.loss_detectors else None
         sp = C.c_void_p(stream.cuda_stream)
-        h2d = h_ie.numel() * 4 * 2 + sum(p.numel() * 4 for p in h_ph) + sum(h_cot[i].numel() * 4 for i in w.loss_detectors)
+        vol = h_ie.numel() * 4
+        h2d = vol * 2 + sum(p.numel() * 4 for p in h_ph) + sum(h_cot[i].numel() * 4 for i in w.loss_detectors)
         h2d += sum(s.waveform.size * 4 + (0 if s.profile is None else s.profile.size * 4) for s in host_src) * 2
-        d2h = h_grad.numel() * 4 + sum(p.numel() * 4 for p in h_ph)
+        d2h = vol + sum(p.numel() * 4 for p in h_ph)
+        if field_loss:            # the final state goes to the host for the caller's loss, its cotangent comes back
+            h2d += 6 * vol * 2
+            d2h += 6 * vol
 
         def e2e_step():
             for P in h_ph:
                 P.zero_()
-            B.fdtd_forward_host(grid.h, None, h_ie, None, sarr, ns, darr, nd, T, sp)
+            if field_loss:
+                h_fields.zero_()
+            B.fdtd_forward_host(grid.h, h_fields, h_ie, None, sarr, ns, darr, nd, T, sp)
             for i in w.loss_detectors:
                 torch.mul(h_ph[i], 2.0, out=h_cot[i])                      # caller's loss cotangent on the host
-            B.fdtd_backward_host(grid.h, None, h_ie, None, sarr, ns, darr, nd, cot, None, T, h_grad, None, sp)
+            if field_loss:
+                h_dLf[inter] = 2.0 * h_fields[inter]
+            B.fdtd_backward_host(grid.h, None, h_ie, None, sarr, ns, darr, nd, cot if nd else None, h_dLf, T, h_grad, None, sp)
 
-        e2e_step()
-        t0 = time.perf_counter()
-        ms_e2e = timed(e2e_step, max(1, min(args.steps, 3)))
-        reps = max(1, min(args.steps, 3))
+        with torch.cuda.stream(stream):
+            e2e_step()
+            reps = max(1, min(args.steps, 3))
+            ms_e2e = timed(e2e_step, reps)
         e2e = {"value": world * cells_steps * reps / (ms_e2e * 1e-3) / 1e6, "unit": UNIT,
                "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "ms_per_step": ms_e2e / reps,
-               "api": "fdtd_forward_host + fdtd_backward_host (pinned host buffers)"}
+               "api": "fdtd_forward_host + fdtd_backward_host (pinned host buffers, staging allocated by fdtd_create_grid)"}
 
     info = grid.info()
     if rank == 0:
         cpu = None
         if not args.no_cpu_baseline and world == 1:
-            cpu = cpu_oracle_rate(wl.c3(n=args.grid, n_steps=args.time_steps) if args.workload == "c3"
-                                  else wl.c4(n_steps=args.time_steps), args.ref_sample_steps)
-        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            wc = make_workload(args)
+            cpu = cpu_oracle_rate(wc, args.ref_sample_steps)
+            one = cpu_oracle_rate(wc, max(2, args.ref_sample_steps // 4), threads=1)
+            cpu["one_thread"] = {"value": one["value"], "fwd_value": one["fwd_value"], "unit": UNIT, "cores": 1,
+                                 "sample_time_steps": max(2, args.ref_sample_steps // 4)}
+        rec_names = {1: "PML/interior interface, record=1 (SURVEY 8(d))", 2: "faces of the design box, record=2 (SURVEY 8(f) N1)"}
+        out = {"metric": METRIC if main_record == 1 else METRIC.replace("record=1", "record=2"),
+               "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                "config": workload_config(w, {"path": {1: "generic", 2: "fused"}[info.path],
                                              "tile": [info.tile_x, info.tile_y, info.tile_z],
                                              "parallelism": f"independent problems x{world}",
-                                             "partition": "lock-step runs (DESIGN.md section 8)",
+                                             "partition": B.PARTITION_NAMES.get(int(info.partition), str(info.partition)),
                                              "reverse_sweep": "grouped launches" if info.pipelined_inverse_ctas else "sequential",
-                                             "recorder": "faces of the design box, record=2 (SURVEY 8(f) N1)" if args.record == 2
-                                             else "PML/interior interface, record=1"}),
+                                             "recorder": rec_names[main_record],
+                                             "recorder_bytes": int(info.recorder_bytes), "scratch_bytes": int(info.scratch_bytes)}),
                "fwd": {"value": fwd_value, "unit": UNIT, "ms_per_pass": ms_fwd / max(1, args.steps),
                        "what": "forward only, record=0, same workload"},
+               "n1_design_box_recorder": n1,
                "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
                "roofline": roofline, "kernels": kernels, "cpu_baseline": cpu,
-               "check": {"loss": loss, "max_abs_dL_drho": gnorm}}
+               "check": {"loss": loss, "max_abs_grad": gnorm,
+                         "device_bytes": {"caller_torch_peak": int(torch.cuda.max_memory_allocated()),
+                                          "grid_recorder": int(info.recorder_bytes), "grid_scratch": int(info.scratch_bytes)}}}
         print(json.dumps(out))
     grid.close()
     grid_f.close()
+    if grid2 is not None:
+        grid2.close()
     if world > 1:
         dist.destroy_process_group()
 

@@ -32,10 +32,34 @@
  *   Pointers marked HOST are ordinary host memory read during the call.  The grid object owns
  *   only scratch: CPML tables, psi slabs, cotangent fields, ping-pong copies, the recorder.
  *
+ *   Everything the entry points need is allocated by fdtd_create_grid: psi slabs, the recorder and (record != 0)
+ *   the cotangent volumes and their psi slabs, the fused path's ping-pong volumes, the DFT phase table for up to
+ *   16 frequencies x max_steps, and with FDTD_FLAG_HOST_STAGING the staging buffers of the *_host entry points.
+ *   Allocated on first use instead (cudaMalloc inside the call): the cotangent volumes when fdtd_backward runs
+ *   on a grid created with record == 0 (adjoint sweep only), a larger phase table when a call passes more than 16
+ *   frequencies in total, the *_host staging buffers without the flag (and those of inv_mu / dL_dfields, which
+ *   are optional arguments, in any case).
+ *
  * Execution
  *   All work is enqueued on `cuda_stream` (a cudaStream_t passed as void*, NULL = legacy default
- *   stream).  The device entry points do not synchronise the host with the device and copy
- *   nothing device->host.  The *_host entry points (below) copy host<->device and synchronise.
+ *   stream).  The device entry points never wait for kernels and copy nothing device->host.  They may wait for
+ *   the host->device upload of a small host-built table of the PREVIOUS call on the same grid (the DFT phase
+ *   table, the TMA descriptors: pinned staging that is about to be rewritten), which is over unless the calls
+ *   follow each other within microseconds.  fdtd_create_grid is synchronous: on the fused path it also times
+ *   the step kernels on scratch volumes (calibration of the work partition: ~30 launches per kernel, a
+ *   temporary allocation of 7 volumes, cudaDeviceSynchronize).  The *_host entry points (below) copy
+ *   host<->device and synchronise the stream.
+ *
+ * Kernel paths
+ *   FDTD_PATH_AUTO picks the fused TMA kernels (one kernel per time step forward, adjoint step + inverse step
+ *   per reverse time step) when ALL of these hold, else the generic one-thread-per-cell kernels:
+ *     - not periodic; nx % 4 == 0; nx >= 2*roundup4(pml_cells); fewer than 2^31 - 4*nx*ny cells;
+ *     - a compiled tile shape fits in shared memory and the driver provides cuTensorMapEncodeTiled.
+ *   On a fused grid a single call still runs on the generic kernels when it passes more than 4 sources or
+ *   more than 4 detectors (the fused kernels' parameter block has 4 slots each; under FDTD_PATH_FUSED such a
+ *   call fails with EINVAL).  In fdtd_backward, detectors with a cotangent on an H component are injected
+ *   by a small kernel per detector and step instead of inside the adjoint step kernel.  inv_mu is taken
+ *   by both paths in both directions.  Results of the two paths agree to rounding (different summation order).
  *
  * Errors
  *   Every function returns FDTD_OK (0) or a negative code; fdtd_last_error() returns a
@@ -68,6 +92,10 @@ extern "C" {
 #define FDTD_PATH_GENERIC  1   /* one-thread-per-cell kernels (periodic grids, odd sizes, debugging)  */
 #define FDTD_PATH_FUSED    2   /* fused kernels; create_grid fails with EINVAL if not applicable      */
 
+/* fdtd_grid_desc.flags */
+#define FDTD_FLAG_HOST_STAGING  1   /* allocate the staging buffers of fdtd_forward_host / fdtd_backward_host
+                                       (fields, inv_eps, and the gradient when record != 0) in fdtd_create_grid */
+
 typedef struct fdtd_grid fdtd_grid;      /* opaque */
 
 /* Grid descriptor.  A zero in any CPML constant selects its default (reading R8). */
@@ -90,7 +118,8 @@ typedef struct {
     int32_t grad_lo[3];        /* half-open (i,j,k) box on which dL_dinv_eps is wanted;             */
     int32_t grad_hi[3];        /*   all zero => the whole interior I.  Always clipped to I.         */
     int32_t path;              /* FDTD_PATH_*                                                       */
-    int32_t reserved[7];       /* must be zero                                                      */
+    int32_t flags;             /* FDTD_FLAG_* bits                                                  */
+    int32_t reserved[6];       /* must be zero                                                      */
 } fdtd_grid_desc;
 
 /* Additive source patch (reading R10/R11): during step n,
@@ -175,8 +204,14 @@ typedef struct {
     int64_t scratch_bytes;           /* all other device bytes owned by the grid                     */
     int64_t record_floats_per_step;  /* recorder stride in floats                                    */
     int64_t pipelined_inverse_ctas;  /* CTAs of the inverse step in the pipelined reverse sweep; 0: sequential */
-    int64_t reserved[3];
+    int64_t fused_step_launches;     /* launches of the fused step kernel (forward + adjoint) so far         */
+    int64_t fused_inverse_launches;  /* launches of the fused inverse step kernel so far                     */
+    int64_t partition;               /* fused path: FDTD_PARTITION_* of the step kernels' work split         */
 } fdtd_grid_info;
+#define FDTD_PARTITION_NONE        0   /* generic path                                                    */
+#define FDTD_PARTITION_CONTIGUOUS  1   /* the (column, plane) sequence cut into contiguous runs           */
+#define FDTD_PARTITION_LOCKSTEP    2   /* columns of one cost class get identical cuts */
+#define FDTD_PARTITION_WAVES       3   /* whole columns dealt out in waves, the rest cut to level the CTAs */
 FDTD_API int fdtd_get_info(const fdtd_grid *grid, fdtd_grid_info *info);
 
 /* Per-kernel timing for roofline reports.  While profiling is enabled the per-step kernels are

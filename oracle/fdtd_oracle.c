@@ -162,6 +162,16 @@ int orc_num_threads(void)
 #endif
 }
 
+/* threads the OpenMP loops use from now on (bench.py times the oracle with all cores and with 1 thread) */
+void orc_set_num_threads(int n)
+{
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
 int orc_sizeof_real(void) { return (int)sizeof(REAL); }
 
 /* ------------------------------------------------------------------------ */

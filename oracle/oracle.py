@@ -98,6 +98,7 @@ def _lib(tag: str):
                                    C.POINTER(C.c_int), C.POINTER(C.c_int), C.c_void_p]
         L.orc_set_ftz.argtypes = [C.c_int]
         L.orc_num_threads.restype = C.c_int
+        L.orc_set_num_threads.argtypes = [C.c_int]
         _LIBS[tag] = L
     return _LIBS[tag]
 
@@ -313,6 +314,9 @@ class Oracle:
 
     def set_ftz(self, on=True):
         self.L.orc_set_ftz(int(on))
+
+    def set_num_threads(self, n):
+        self.L.orc_set_num_threads(int(n))
 
     def num_threads(self):
         return int(self.L.orc_num_threads())

@@ -20,6 +20,8 @@ LIB_PATH = _HERE / "libfdtd_b200.so"
 
 FDTD_OK, FDTD_EINVAL, FDTD_ENOMEM, FDTD_ECUDA, FDTD_ESTATE = 0, -1, -2, -3, -4
 FDTD_PATH_AUTO, FDTD_PATH_GENERIC, FDTD_PATH_FUSED = 0, 1, 2
+FDTD_FLAG_HOST_STAGING = 1
+PARTITION_NAMES = {0: "none (generic kernels)", 1: "contiguous runs", 2: "lock-step runs", 3: "waves of whole columns + levelled pool"}
 
 
 class fdtd_grid_desc(C.Structure):
@@ -29,7 +31,7 @@ class fdtd_grid_desc(C.Structure):
                 ("pml_alpha_max", C.c_float), ("pml_alpha_m", C.c_float), ("pml_eps_bg", C.c_float),
                 ("max_steps", C.c_int32), ("record", C.c_int32),
                 ("grad_lo", C.c_int32 * 3), ("grad_hi", C.c_int32 * 3),
-                ("path", C.c_int32), ("reserved", C.c_int32 * 7)]
+                ("path", C.c_int32), ("flags", C.c_int32), ("reserved", C.c_int32 * 6)]
 
 
 class fdtd_source(C.Structure):
@@ -46,7 +48,7 @@ class fdtd_grid_info(C.Structure):
     _fields_ = [("path", C.c_int32), ("tile_x", C.c_int32), ("tile_y", C.c_int32), ("tile_z", C.c_int32),
                 ("kernel_launches", C.c_int64), ("recorder_bytes", C.c_int64), ("scratch_bytes", C.c_int64),
                 ("record_floats_per_step", C.c_int64), ("pipelined_inverse_ctas", C.c_int64),
-                ("reserved", C.c_int64 * 3)]
+                ("fused_step_launches", C.c_int64), ("fused_inverse_launches", C.c_int64), ("partition", C.c_int64)]
 
 
 FDTD_PROF_CLASSES = 16
@@ -201,13 +203,13 @@ def fdtd_backward_host(grid, h_fields, h_inv_eps, h_inv_mu, src, n_src, det, n_d
 # --------------------------------------------------------------------------------------------
 def make_desc(nx, ny, nz, courant, periodic=False, pml_cells=0, pml_m=0.0, pml_sigma_scale=0.0,
               pml_kappa_max=0.0, pml_alpha_max=0.0, pml_alpha_m=0.0, pml_eps_bg=0.0, max_steps=0,
-              record=False, grad_lo=None, grad_hi=None, path=FDTD_PATH_AUTO) -> fdtd_grid_desc:
+              record=False, grad_lo=None, grad_hi=None, path=FDTD_PATH_AUTO, flags=0) -> fdtd_grid_desc:
     d = fdtd_grid_desc()
     d.nx, d.ny, d.nz, d.courant = nx, ny, nz, courant
     d.periodic, d.pml_cells = int(bool(periodic)), pml_cells
     d.pml_m, d.pml_sigma_scale, d.pml_kappa_max = pml_m, pml_sigma_scale, pml_kappa_max
     d.pml_alpha_max, d.pml_alpha_m, d.pml_eps_bg = pml_alpha_max, pml_alpha_m, pml_eps_bg
-    d.max_steps, d.record, d.path = max_steps, int(record), path
+    d.max_steps, d.record, d.path, d.flags = max_steps, int(record), path, int(flags)
     if grad_lo is not None:
         d.grad_lo[:] = list(grad_lo)
         d.grad_hi[:] = list(grad_hi)

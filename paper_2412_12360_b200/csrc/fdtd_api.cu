@@ -1,5 +1,5 @@
 // fdtd_api.cu -- the C ABI of include/fdtd.h: validation, the grid object, host orchestration.
-// Every step of the path runs in the kernels of kernels_generic.cu / kernels_fused_*.cu; this
+// Every step of the path runs in the kernels of kernels_generic.cu / kernels_step.cu; this
 // file only owns memory, builds tables and enqueues launches (through CUDA graphs).
 #include <cmath>
 #include <cstdio>
@@ -91,6 +91,8 @@ bool box_ok(const Dims &G, const int32_t lo[3], const int32_t hi[3])
 
 int popcount6(int m) { int n = 0; for (int c = 0; c < 6; ++c) n += (m >> c) & 1; return n; }
 
+constexpr int CS_PREALLOC_FREQ = 16;     // frequencies (summed over the detectors) the (cos, sin) table is sized for at create time
+
 }  // namespace
 
 // ================================================================================================
@@ -160,7 +162,8 @@ extern "C" int fdtd_create_grid(const fdtd_grid_desc *desc, fdtd_grid **out)
     if (desc->max_steps < 0) return fail(FDTD_EINVAL, "max_steps must be >= 0");
     if (desc->record < 0 || desc->record > 2) return fail(FDTD_EINVAL, "record must be 0, 1 or 2");
     if (desc->path < 0 || desc->path > 2) return fail(FDTD_EINVAL, "unknown path");
-    for (int q = 0; q < 7; ++q) if (desc->reserved[q]) return fail(FDTD_EINVAL, "reserved fields must be zero");
+    for (int q = 0; q < 6; ++q) if (desc->reserved[q]) return fail(FDTD_EINVAL, "reserved fields must be zero");
+    if (desc->flags & ~FDTD_FLAG_HOST_STAGING) return fail(FDTD_EINVAL, "unknown bit in flags");
     if (desc->pml_m < 0 || desc->pml_sigma_scale < 0 || desc->pml_kappa_max < 0 || desc->pml_alpha_max < 0 ||
         desc->pml_alpha_m < 0 || desc->pml_eps_bg < 0)
         return fail(FDTD_EINVAL, "CPML constants must be >= 0");
@@ -253,10 +256,16 @@ extern "C" int fdtd_create_grid(const fdtd_grid_desc *desc, fdtd_grid **out)
         if (e != cudaSuccess) return bail(cuda_fail(e, "cudaEventCreate"));
     }
     g->path = FDTD_PATH_GENERIC;
-    rc = fused_setup(g);          // may switch g->path to FDTD_PATH_FUSED (kernels_fused_*.cu)
+    rc = fused_setup(g);          // may switch g->path to FDTD_PATH_FUSED (kernels_step.cu)
     if (rc) return bail(rc);
     if (desc->path == FDTD_PATH_FUSED && g->path != FDTD_PATH_FUSED)
         return bail(fail(FDTD_EINVAL, "FDTD_PATH_FUSED requested but the grid does not qualify: " + g->fused_why_not));
+    // everything the entry points need is allocated here (include/fdtd.h "Memory / ownership"): a recording grid will
+    // run fdtd_backward, so its cotangent volumes exist from the start; the (cos, sin) table is sized for
+    // CS_PREALLOC_FREQ frequencies; the staging buffers of the *_host entry points when the flag asks for them
+    if (desc->record && (rc = g->ensure_backward_buffers())) return bail(rc);
+    if (desc->max_steps > 0 && (rc = g->reserve_cs_table((size_t)desc->max_steps * CS_PREALLOC_FREQ * 2))) return bail(rc);
+    if ((desc->flags & FDTD_FLAG_HOST_STAGING) && (rc = g->ensure_host_buffers(false, desc->record != 0))) return bail(rc);
     *out = g;
     return FDTD_OK;
 }
@@ -353,6 +362,9 @@ extern "C" int fdtd_get_info(const fdtd_grid *g, fdtd_grid_info *info)
     info->scratch_bytes = g->scratch_bytes;
     info->record_floats_per_step = g->R.stride;
     info->pipelined_inverse_ctas = g->pipelined_inverse_ctas;
+    info->fused_step_launches = g->fused_step_launches;
+    info->fused_inverse_launches = g->fused_inverse_launches;
+    info->partition = g->path == FDTD_PATH_FUSED ? g->partition : FDTD_PARTITION_NONE;
     return FDTD_OK;
 }
 
@@ -409,22 +421,33 @@ int translate(const fdtd_detector *det, int n_det, std::vector<DetectorDev> &out
     return tot;
 }
 
+}  // namespace
+
+// device + pinned host capacity of the (cos, sin) table; earlier uploads have to be finished before the old buffers go
+int fdtd_grid::reserve_cs_table(size_t floats)
+{
+    if (floats <= cs_cap) return FDTD_OK;
+    CK(cudaEventSynchronize(table_done));
+    if (h_cs) { cudaFreeHost(h_cs); h_cs = nullptr; }
+    CK(cudaMallocHost((void **)&h_cs, floats * sizeof(float)));
+    int rc = alloc((void **)&d_cs, floats * sizeof(float));
+    if (rc) return rc;
+    cs_cap = floats;
+    return FDTD_OK;
+}
+
+namespace {
+
 // (cos, sin) of omega_f*(n+1) for n < n_steps, fp64 on the host, stored fp32 (reading R13)
 int upload_cs_table(fdtd_grid *g, const fdtd_detector *det, int n_det, int total_freq, int n_steps, cudaStream_t st)
 {
     if (total_freq == 0 || n_steps == 0) return FDTD_OK;
     const size_t need = (size_t)n_steps * total_freq * 2;
-    if (need > g->cs_cap) {
-        // grow (device + pinned host); previous copies have to be finished first
-        CK(cudaEventSynchronize(g->table_done));
-        if (g->h_cs) { cudaFreeHost(g->h_cs); g->h_cs = nullptr; }
-        const size_t cap = (size_t)std::max(n_steps, g->desc.max_steps) * total_freq * 2;
-        CK(cudaMallocHost((void **)&g->h_cs, cap * sizeof(float)));
-        int rc = g->alloc((void **)&g->d_cs, cap * sizeof(float));
+    if (need > g->cs_cap) {       // more than CS_PREALLOC_FREQ frequencies: grow
+        int rc = g->reserve_cs_table((size_t)std::max(n_steps, g->desc.max_steps) * total_freq * 2);
         if (rc) return rc;
-        g->cs_cap = cap;
     }
-    CK(cudaEventSynchronize(g->table_done));
+    CK(cudaEventSynchronize(g->table_done));      // the previous call's upload has left the pinned staging table
     int f0 = 0;
     for (int s = 0; s < n_det; ++s) {
         for (int q = 0; q < det[s].n_freq; ++q) {
@@ -451,8 +474,10 @@ int run_steps(fdtd_grid *g, fdtd_grid::GraphCache &gc, const std::string &key, i
     if (n_steps == 0) return FDTD_OK;
     if (g->profiling) {
         g->step_par = 0;
+        const long long s0 = g->enq_step, i0 = g->enq_inv;
         for (int n = 0; n < n_steps; ++n) { enqueue(st); g->step_par ^= 1; }
         g->kernel_launches += (long long)n_steps * launches_per_step;
+        g->fused_step_launches += g->enq_step - s0; g->fused_inverse_launches += g->enq_inv - i0;
         return FDTD_OK;
     }
     static const int env_unroll = getenv("FDTD_GRAPH_UNROLL") ? std::max(2, atoi(getenv("FDTD_GRAPH_UNROLL")) / 2 * 2) : 0;
@@ -468,7 +493,9 @@ int run_steps(fdtd_grid *g, fdtd_grid::GraphCache &gc, const std::string &key, i
             CK(cudaStreamBeginCapture(g->cap_stream, cudaStreamCaptureModeThreadLocal));
             g->prof_capturing = true;
             g->step_par = which == 2 ? 1 : 0;
+            const long long s0 = g->enq_step, i0 = g->enq_inv;
             for (int r = 0; r < reps; ++r) { enqueue(g->cap_stream); g->step_par ^= 1; }
+            if (which == 1) { gc.step_per = g->enq_step - s0; gc.inv_per = g->enq_inv - i0; }   // fused kernels per time step
             g->prof_capturing = false;
             cudaError_t e = cudaStreamEndCapture(g->cap_stream, &graph);
             if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture");
@@ -485,6 +512,7 @@ int run_steps(fdtd_grid *g, fdtd_grid::GraphCache &gc, const std::string &key, i
     while (left > 0) { CK(cudaGraphLaunch(gc.exec_tail[par], st)); par ^= 1; --left; }
     CK(cudaEventRecord(gc.done, st));
     g->kernel_launches += (long long)n_steps * launches_per_step;
+    g->fused_step_launches += n_steps * gc.step_per; g->fused_inverse_launches += n_steps * gc.inv_per;
     return FDTD_OK;
 }
 
@@ -537,13 +565,18 @@ extern "C" int fdtd_forward(fdtd_grid *g, float *fields, const float *inv_eps, c
     if ((rc = upload_cs_table(g, det, n_det, total_freq, n_steps, st))) return rc;
     launch_set_step(g->d_step, 0, st);                   // step 0 reads slot 0
 
-    if (g->path == FDTD_PATH_FUSED) {
+    // more descriptors than the fused kernels' parameter block holds: this call runs on the generic kernels (same
+    // psi slabs, same recorder layout, so a fused or generic fdtd_backward can follow)
+    const bool fused_call = g->path == FDTD_PATH_FUSED && n_src <= FDTD_FUSED_MAX_SRC && n_det <= FDTD_FUSED_MAX_DET;
+    if (g->path == FDTD_PATH_FUSED && !fused_call && g->desc.path == FDTD_PATH_FUSED)
+        return fail(FDTD_EINVAL, "FDTD_PATH_FUSED takes at most 4 sources and 4 detectors per call (FDTD_PATH_AUTO falls back to the generic kernels)");
+    if (fused_call) {
         rc = fused_forward(g, fields, inv_eps, inv_mu, S, D, total_freq, n_steps, recording, st);
         if (rc) return rc;
     } else {
         if ((rc = g->zero_psi(g->psiE[0], st)) || (rc = g->zero_psi(g->psiH[0], st))) return rc;
         const int launches = 3 + n_src + n_det + (recording ? 1 : 0);
-        const std::string key = make_key("gf", fields, inv_eps, inv_mu, g->rec, nullptr, S, D, recording);
+        const std::string key = make_key("gf", fields, inv_eps, inv_mu, g->rec, g->d_cs, S, D, recording);
         rc = run_steps(g, g->fwd_graph, key, n_steps, launches, st, [&](cudaStream_t cs) {
             { ProfScope p(g, fdtd_grid::PC_UPDATE_E, cs); launch_update_E(G, g->T, fields, inv_eps, g->psiE[0], cs); }
             { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
@@ -573,7 +606,7 @@ int fdtd_grid::ensure_backward_buffers()
     if ((rc = alloc((void **)&lam, (size_t)G.nc * 6 * sizeof(float)))) return rc;
     for (int q = 0; q < 2; ++q)
         if ((rc = alloc_psi(lpsiE[q])) || (rc = alloc_psi(lpsiH[q]))) return rc;
-    return FDTD_OK;
+    return fused ? fused_alloc_backward(this) : FDTD_OK;
 }
 
 extern "C" int fdtd_backward(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
@@ -607,14 +640,18 @@ extern "C" int fdtd_backward(fdtd_grid *g, float *fields, const float *inv_eps, 
     launch_set_step(g->d_step, std::max(n_steps - 1, 0), st);   // the first reverse step reads slot 0
     const bool want_grad = dL_dinv_eps != nullptr;              // false: adjoint sweep only (B1, B2, B5)
 
-    if (g->path == FDTD_PATH_FUSED && g->fused_backward_ready && !inv_mu) {
-        rc = fused_backward(g, fields, inv_eps, inv_mu, S, D, total_freq, n_steps, dL_dinv_eps, st);
+    if (g->path == FDTD_PATH_FUSED && g->fused_backward_ready) {
+        // seeded_H: the H part of the seed can be non-zero (it is scaled by inv_mu for the sweep)
+        rc = fused_backward(g, fields, inv_eps, inv_mu, S, D, total_freq, n_steps, dL_dinv_eps, dL_dfields != nullptr, st);
         if (rc) return rc;
+        // the fused sweep carried im lamH in the H part (kernels_step.cu); the cotangent of state 0 is lamH
+        if (inv_mu && dL_dfields0) launch_scale_H(G, g->lam, inv_mu, true, st);
     } else {
         int n_adj = 0;
         for (const DetectorDev &dt : D) if (dt.phasor) ++n_adj;
         const int launches = want_grad ? 5 + n_adj + n_src + (G.d > 0 ? 1 : 0) : 3 + n_adj;
-        const std::string key = make_key("gb", fields, inv_eps, inv_mu, g->rec, dL_dinv_eps, S, D, 0);
+        std::string key = make_key("gb", fields, inv_eps, inv_mu, g->rec, dL_dinv_eps, S, D, 0);
+        key.append((const char *)&g->d_cs, sizeof(g->d_cs));
         rc = run_steps(g, g->bwd_graph, key, n_steps, launches, st, [&](cudaStream_t cs) {
             { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
               for (const DetectorDev &dt : D) if (dt.phasor) launch_detector_adjoint(G, g->lam, dt, g->d_cs, total_freq, g->step_in(), cs); }
@@ -633,7 +670,7 @@ extern "C" int fdtd_backward(fdtd_grid *g, float *fields, const float *inv_eps, 
         });
         if (rc) return rc;
     }
-    if (dL_dfields0) CK(cudaMemcpyAsync(dL_dfields0, g->lam_result ? g->lam_result : g->lam, 6 * vol, cudaMemcpyDeviceToDevice, st));
+    if (dL_dfields0) CK(cudaMemcpyAsync(dL_dfields0, g->lam, 6 * vol, cudaMemcpyDeviceToDevice, st));
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "fdtd_backward launch");
     return FDTD_OK;
@@ -669,13 +706,14 @@ size_t box_cells(const int32_t lo[3], const int32_t hi[3])
 
 }  // namespace
 
-int fdtd_grid::ensure_host_buffers(bool need_mu)
+int fdtd_grid::ensure_host_buffers(bool need_mu, bool need_grad)
 {
     int rc;
     const size_t vol = (size_t)G.nc * sizeof(float);
     if (!hb_fields && (rc = alloc((void **)&hb_fields, 6 * vol))) return rc;
     if (!hb_ie && (rc = alloc((void **)&hb_ie, vol))) return rc;
     if (need_mu && !hb_im && (rc = alloc((void **)&hb_im, vol))) return rc;
+    if (need_grad && !hb_grad && (rc = alloc((void **)&hb_grad, vol))) return rc;
     return FDTD_OK;
 }
 
@@ -738,7 +776,7 @@ extern "C" int fdtd_forward_host(fdtd_grid *g, float *h_fields, const float *h_i
     for (int s = 0; s < n_src; ++s) if (!box_ok(g->G, h_src[s].lo, h_src[s].hi) || !h_src[s].waveform) return fail(FDTD_EINVAL, "fdtd_forward_host: bad source");
     for (int s = 0; s < n_det; ++s) if (!box_ok(g->G, h_det[s].lo, h_det[s].hi) || !h_det[s].phasor || h_det[s].n_freq < 1) return fail(FDTD_EINVAL, "fdtd_forward_host: bad detector");
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    int rc = g->ensure_host_buffers(h_inv_mu != nullptr);
+    int rc = g->ensure_host_buffers(h_inv_mu != nullptr, false);
     if (rc) return rc;
     const size_t vol = (size_t)g->G.nc * sizeof(float);
     if (h_fields) CK(cudaMemcpyAsync(g->hb_fields, h_fields, 6 * vol, cudaMemcpyHostToDevice, st));
@@ -769,10 +807,9 @@ extern "C" int fdtd_backward_host(fdtd_grid *g, float *h_fields, const float *h_
     for (int s = 0; s < n_det; ++s) if (!box_ok(g->G, h_det[s].lo, h_det[s].hi) || h_det[s].n_freq < 1) return fail(FDTD_EINVAL, "fdtd_backward_host: bad detector");
     if (!h_fields && !g->hb_fields) return fail(FDTD_ESTATE, "fdtd_backward_host: no state left by fdtd_forward_host");
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    int rc = g->ensure_host_buffers(h_inv_mu != nullptr);
+    int rc = g->ensure_host_buffers(h_inv_mu != nullptr, true);
     if (rc) return rc;
     const size_t vol = (size_t)g->G.nc * sizeof(float);
-    if (!g->hb_grad && (rc = g->alloc((void **)&g->hb_grad, vol))) return rc;
     if ((h_dL_dfields || h_dL_dfields0) && !g->hb_cotf && (rc = g->alloc((void **)&g->hb_cotf, 6 * vol))) return rc;
     if (h_fields) CK(cudaMemcpyAsync(g->hb_fields, h_fields, 6 * vol, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(g->hb_ie, h_inv_eps, vol, cudaMemcpyHostToDevice, st));

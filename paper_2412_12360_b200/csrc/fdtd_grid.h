@@ -4,7 +4,11 @@
 #include <vector>
 #include "fdtd_internal.h"
 
-struct FusedState;   // kernels_fused.cu
+struct FusedState;   // kernels_step.cu
+
+// descriptor slots of the fused step kernels' parameter block; a call with more sources or detectors runs on the
+// generic kernels (FDTD_PATH_AUTO) -- see include/fdtd.h "Kernel paths"
+constexpr int FDTD_FUSED_MAX_SRC = 4, FDTD_FUSED_MAX_DET = 4;
 
 struct fdtd_grid {
     fdtd_grid_desc desc{};
@@ -30,7 +34,6 @@ struct fdtd_grid {
     fdtd::PsiSet psiE[2]{}, psiH[2]{};     // primal psi ([1] only used by the fused path's ping-pong)
     fdtd::PsiSet lpsiE[2]{}, lpsiH[2]{};   // psi cotangents, ping-ponged by step parity
     float *lam = nullptr;                  // cotangent fields [6][nz][ny][nx]
-    float *lam_result = nullptr;           // where the final cotangent lives if not in `lam` (fused path)
     float *rec = nullptr;                  // interface recorder
     int recorded_steps = -1;               // n_steps of the last recorded forward, or -1
     float *d_cs = nullptr;                 // per-step (cos, sin) table
@@ -49,6 +52,7 @@ struct fdtd_grid {
         std::string key;
         cudaGraphExec_t exec_main = nullptr, exec_tail[2] = { nullptr, nullptr };   // tail: one step, per counter slot
         cudaEvent_t done = nullptr;
+        long long step_per = 0, inv_per = 0;   // fused step / inverse kernels per time step in this graph
     } fwd_graph, bwd_graph;
     cudaStream_t cap_stream = nullptr;
     // fork / join of the launches that run beside a step kernel (recorder, inverse step, face injection): the side
@@ -56,6 +60,9 @@ struct fdtd_grid {
     cudaStream_t side_stream[2] = { nullptr, nullptr };
     cudaEvent_t fork_ev = nullptr, join_ev[2] = { nullptr, nullptr };
     long long kernel_launches = 0;
+    long long fused_step_launches = 0, fused_inverse_launches = 0;   // counted as they are enqueued (graph nodes x replays)
+    int partition = FDTD_PARTITION_NONE;
+    long long enq_step = 0, enq_inv = 0;   // bumped by every enqueue of a fused step / inverse kernel (run_steps turns them into launch counts)
 
     FusedState *fused = nullptr;
 
@@ -76,20 +83,22 @@ struct fdtd_grid {
     int alloc_psi(fdtd::PsiSet &s);
     int zero_psi(const fdtd::PsiSet &s, cudaStream_t st);
     int ensure_backward_buffers();
-    int ensure_host_buffers(bool need_mu);
+    int ensure_host_buffers(bool need_mu, bool need_grad);
+    int reserve_cs_table(size_t floats);
     void drop_graphs();
 };
 
-// fused TMA path (kernels_fused.cu).  fused_setup decides whether the grid qualifies and, if so,
+// fused TMA path (kernels_step.cu).  fused_setup decides whether the grid qualifies and, if so,
 // sets g->path = FDTD_PATH_FUSED; otherwise it records the reason in g->fused_why_not.
 int fused_setup(fdtd_grid *g);
 void fused_teardown(fdtd_grid *g);
+int fused_alloc_backward(fdtd_grid *g);    // second cotangent volume of the ping-pong
 int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
                   const std::vector<fdtd::SourceDev> &S, const std::vector<fdtd::DetectorDev> &D,
                   int total_freq, int n_steps, bool recording, cudaStream_t st);
 int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
                    const std::vector<fdtd::SourceDev> &S, const std::vector<fdtd::DetectorDev> &D,
-                   int total_freq, int n_steps, float *dL_dinv_eps, cudaStream_t st);
+                   int total_freq, int n_steps, float *dL_dinv_eps, bool seeded_H, cudaStream_t st);
 
 // RAII span: brackets the launches made in its lifetime with two events when profiling is on
 struct ProfScope {

@@ -134,7 +134,10 @@ void launch_inv_E_grad(const Dims &G, float *fields, const float *ie, const floa
 // fused path: cotangent volumes are ping-ponged by step parity
 void launch_inv_E_grad_pp(const Dims &G, float *fields, const float *ie, const float *lamA, const float *lamB,
                           const int *step, float *g, cudaStream_t st);
+// im != NULL: the H part of the volumes holds im lamH, so H-component cotangents are scaled by im at their cell
 void launch_detector_adjoint_pp(const Dims &G, float *lamA, float *lamB, const DetectorDev &dt, const float *cs_table,
-                                int total_freq, const int *step, cudaStream_t st);
+                                int total_freq, const int *step, const float *im, cudaStream_t st);
+// H part of a cotangent volume: lamH *= im (inverse = false) or lamH /= im (inverse = true)
+void launch_scale_H(const Dims &G, float *lam, const float *im, bool inverse, cudaStream_t st);
 
 }  // namespace fdtd

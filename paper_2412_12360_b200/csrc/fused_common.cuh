@@ -15,36 +15,7 @@ namespace fdtd {
 struct Segment {
     int i0, j0;       // tile origin
     int k0, k1;       // planes [k0, k1) owned by this segment
-    int flags;        // SEG_X_LO | SEG_X_HI | SEG_Y_LO | SEG_Y_HI : which CPML slabs the tile touches
-    int xbase;        // first x of the x-slab psi box (see kernels_fused.cu)
-    int pad[2];
 };
-enum { SEG_X_LO = 1, SEG_X_HI = 2, SEG_Y_LO = 4, SEG_Y_HI = 8 };
-
-// logical arrays of one pipeline stage
-enum StageArray {
-    SA_EX = 0, SA_EY, SA_EZ, SA_HX, SA_HY, SA_HZ, SA_IE, SA_IM,
-    SA_PE_Y0, SA_PE_Y1,     // psi_E of the y axis: psiE_x0, psiE_z1
-    SA_PE_Z0, SA_PE_Z1,     // psi_E of the z axis: psiE_y0, psiE_x1
-    SA_PH_Y0, SA_PH_Y1,     // psi_H of the y axis: psiH_x0, psiH_z1      (lagging plane)
-    SA_PH_Z0, SA_PH_Z1,     // psi_H of the z axis: psiH_y0, psiH_x1      (lagging plane)
-    SA_PE_X0, SA_PE_X1,     // psi_E of the x axis: psiE_z0, psiE_y1      (narrow boxes)
-    SA_PH_X0, SA_PH_X1,     // psi_H of the x axis: psiH_z0, psiH_y1      (narrow boxes, lagging plane)
-    SA_COUNT
-};
-
-// tensor-map table (device memory, 64 B aligned entries); index helpers
-enum {
-    TM_FIELD = 0,                 // + set*6 + comp                     (12)
-    TM_IE = 12, TM_IM = 13,
-    TM_PSI = 14,                  // + set*20 + family*10 + local       (40)
-    TM_COUNT = 54
-};
-// local index inside a (set, family) block of 10 maps:
-//   0,1: x axis arrays (c=z,s=0),(c=y,s=1) low view ; 2,3: same, high view
-//   4,5: y axis arrays (c=x,s=0),(c=z,s=1) low view ; 6,7: same, high view
-//   8,9: z axis arrays (c=y,s=0),(c=x,s=1)
-__host__ __device__ inline int tm_psi(int set, int family, int local) { return TM_PSI + set * 20 + family * 10 + local; }
 
 // ------------------------------------------------------------------------------------------------
 // PTX wrappers

@@ -4,6 +4,7 @@
 // They serve periodic grids and sizes the fused TMA kernels do not take, and they are the
 // simple statement the fused kernels are cross-checked against on the GPU.
 // Formulas: include/fdtd.h (conventions) and DESIGN.md section 2; Eq. 1-2, L72, L84.
+#include <algorithm>
 #include "fdtd_internal.h"
 
 namespace fdtd {
@@ -121,7 +122,8 @@ __global__ void k_add_source(Dims G, float *__restrict__ f, SourceDev s, const i
 // cs_table: [max_steps][total_freq][2] = (cos, sin) of omega_f*(n+1), built on the host in fp64 (R13)
 template <bool ADJ>
 __global__ void k_detector(Dims G, float *__restrict__ f, DetectorDev dt, const float *__restrict__ cs,
-                           int total_freq, const int *__restrict__ step, float *__restrict__ f2, int par_off)
+                           int total_freq, const int *__restrict__ step, float *__restrict__ f2, int par_off,
+                           const float *__restrict__ med_H)
 {
     if (f2 && ((*step + par_off) & 1)) f = f2;       // ping-pong volumes of the fused path
     const int bx = dt.hi[0] - dt.lo[0], by = dt.hi[1] - dt.lo[1], bz = dt.hi[2] - dt.lo[2];
@@ -149,9 +151,19 @@ __global__ void k_detector(Dims G, float *__restrict__ f, DetectorDev dt, const 
                 const float2 Gq = __ldg(reinterpret_cast<const float2 *>(dt.phasor) + ((long long)q * dt.ncomp + ci) * bc + t);
                 acc += Gq.x * __ldg(csn + 2 * q) - Gq.y * __ldg(csn + 2 * q + 1);
             }
+            if (med_H && c >= 3) acc *= __ldg(med_H + p);
             f[c * G.nc + p] += acc;
         }
         ++ci;
+    }
+}
+
+// lamH <-> im lamH on the three H volumes (fused reverse sweep with inv_mu)
+__global__ void k_scale_H(float *__restrict__ lamH, const float *__restrict__ im, long long nc, bool inverse)
+{
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < 3 * nc; t += (long long)gridDim.x * blockDim.x) {
+        const float m = __ldg(im + t % nc);
+        lamH[t] = inverse ? lamH[t] / m : lamH[t] * m;
     }
 }
 
@@ -470,22 +482,28 @@ void launch_detector(const Dims &G, const float *fields, const DetectorDev &dt, 
                      int total_freq, const int *step, cudaStream_t st)
 {
     const long long n = (long long)(dt.hi[0] - dt.lo[0]) * (dt.hi[1] - dt.lo[1]) * (dt.hi[2] - dt.lo[2]);
-    k_detector<false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(G, const_cast<float *>(fields), dt, cs_table, total_freq, step, nullptr, 0);
+    k_detector<false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(G, const_cast<float *>(fields), dt, cs_table, total_freq, step, nullptr, 0, nullptr);
 }
 
 void launch_detector_adjoint(const Dims &G, float *lam, const DetectorDev &dt, const float *cs_table,
                              int total_freq, const int *step, cudaStream_t st)
 {
     const long long n = (long long)(dt.hi[0] - dt.lo[0]) * (dt.hi[1] - dt.lo[1]) * (dt.hi[2] - dt.lo[2]);
-    k_detector<true><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(G, lam, dt, cs_table, total_freq, step, nullptr, 0);
+    k_detector<true><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(G, lam, dt, cs_table, total_freq, step, nullptr, 0, nullptr);
 }
 
 // reverse step n of the fused path injects into the volume it is about to read: buffer (n+1)&1
 void launch_detector_adjoint_pp(const Dims &G, float *lamA, float *lamB, const DetectorDev &dt, const float *cs_table,
-                                int total_freq, const int *step, cudaStream_t st)
+                                int total_freq, const int *step, const float *im, cudaStream_t st)
 {
     const long long n = (long long)(dt.hi[0] - dt.lo[0]) * (dt.hi[1] - dt.lo[1]) * (dt.hi[2] - dt.lo[2]);
-    k_detector<true><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(G, lamA, dt, cs_table, total_freq, step, lamB, 1);
+    k_detector<true><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(G, lamA, dt, cs_table, total_freq, step, lamB, 1, im);
+}
+
+void launch_scale_H(const Dims &G, float *lam, const float *im, bool inverse, cudaStream_t st)
+{
+    const long long n = 3 * G.nc;
+    k_scale_H<<<(unsigned)std::min<long long>((n + 255) / 256, 1 << 20), 256, 0, st>>>(lam + 3 * G.nc, im, G.nc, inverse);
 }
 
 void launch_record(const Dims &G, const RecLayout &R, const float *fields_H, const float *fields_E,

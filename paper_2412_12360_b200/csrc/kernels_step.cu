@@ -12,9 +12,9 @@
 //   * only the three arrays that are differenced in phase A (the H-type operand F) need neighbours: one
 //     producer thread streams their boxes (one-cell halo, 16-byte aligned in x) global -> shared with TMA
 //     (cp.async.bulk.tensor; the zero fill outside the grid IS the zero-pad wall convention R7) through a
-//     ring of NST stages with full/empty mbarriers.  Everything a thread only needs at its own cells
-//     (E-type target, inv_eps, CPML states) is read straight from global memory as float4, the E-type
-//     target and inv_eps one plane ahead;
+//     ring of NST stages with full/empty mbarriers.  The E-type target, inv_eps and the x-slab CPML states
+//     travel in the same stage (seven boxes plus four narrow ones); only the y / z slab CPML states (and inv_mu)
+//     are read straight from global memory as float4 at a thread's own cells;
 //   * consumer warps are 8 x 4 patches of float4 threads (128 B contiguous per patch row), so CPML slab
 //     code is executed by the few warps that touch a slab.  Plane kk, phase A: the E-type update of plane
 //     kk on the tile plus a +x halo column and a +y halo row (recomputed, not exchanged between CTAs),
@@ -41,7 +41,7 @@ using namespace fdtd;
 
 namespace {
 
-constexpr int MAX_SRC = 4, MAX_DET = 4;
+constexpr int MAX_SRC = FDTD_FUSED_MAX_SRC, MAX_DET = FDTD_FUSED_MAX_DET;
 // timing experiments (wrong results): build with -DFDTD_TIMING_EXPERIMENTS and set FDTD_DBG to a bit mask:
 // 1 no global stores, 2 no phase B, 4 no barrier, 8 load pipeline only, 16 no CPML, 32/64/128 no x/y/z slab code
 #ifdef FDTD_TIMING_EXPERIMENTS
@@ -267,7 +267,7 @@ __device__ __forceinline__ void detect4(const StepParams &P, int n, int family, 
 // The step kernel.  Names follow the forward step: "F" is the H-type operand of phase A, "e" the
 // E-type target, "v" the phase-A result that phase B differences, "h" the H-type target.
 //   forward : e' = e + S ie curl-(F = H)            v = e'            h' = h - S im curl+(v)
-//   adjoint : e' = e - S curl-(F = lamH)   (im = 1) v = S ie e'       h' = h + curl+(v)
+//   adjoint : e' = e - S curl-(F = im lamH)         v = S ie e'       h' = h + im curl+(v)     (h = im lamH)
 // curl with CPML: t_x = Dy_z - Dz_y, t_y = Dz_x - Dx_z, t_z = Dx_y - Dy_x, where D<a>_<c> is the
 // (filtered) difference of component c along axis a; its state array is
 //   Dy_z p[0][0]   Dz_y p[0][1]   Dz_x p[1][0]   Dx_z p[1][1]   Dx_y p[2][0]   Dy_x p[2][1].
@@ -392,7 +392,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
     const long long nc = G.nc;
     const int plane = G.ny * G.nx;
     const bool pml = G.d > 0 && !DBG(16);
-    const bool has_mu = !ADJ && P.im != nullptr;
+    const bool has_mu = P.im != nullptr;
     const int pz = plane, py = 2 * G.d * G.nx, px = G.ny * 2 * G.dpx;      // plane pitch of the z / y / x state arrays
 
     const float4 Z4 = splat(0.f);
@@ -636,7 +636,10 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                 const float4 hx = lds4(sp), hy = lds4(sp + C::SLOT), hz = lds4(sp + 2 * C::SLOT);
                 float4 h2x, h2y, h2z;
                 if (ADJ) {
-                    h2x = hx + tHx; h2y = hy + tHy; h2z = hz + tHz;
+                    // with inv_mu the H part of the cotangent volumes holds Lambda_H = im lamH (fused_backward): phase A
+                    // differences it as it is, and the transpose of the E update lands in it scaled by im at my cells
+                    if (has_mu) { const float4 m = ldg4(P.im + offm); h2x = fma4(m, tHx, hx); h2y = fma4(m, tHy, hy); h2z = fma4(m, tHz, hz); }
+                    else { h2x = hx + tHx; h2y = hy + tHy; h2z = hz + tHz; }
                 } else {
                     const float4 sim = has_mu ? S * ldg4(P.im + offm) : splat(S);
                     h2x = hx - sim * tHx; h2y = hy - sim * tHy; h2z = hz - sim * tHz;
@@ -709,6 +712,7 @@ struct InvParams {
     const int *seg_begin;          // [n_cta + 1]
     float *buf[2];                 // primal ping-pong volumes
     float *grad;                   // dL/d inv_eps, accumulated
+    const float *im;               // inv_mu or NULL (= 1)
     const int *step;
     int bias, n_steps;             // this launch inverts step n = *step + bias; nothing to do if n >= n_steps (see enqueue_bwd)
     int nst, stage;
@@ -832,7 +836,9 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_inverse(const __grid_constant
             const float4 Dy_z = Ez_py - Ez, Dy_x = Ex_py - Ex;
             const float4 Dx_y = dplus_x(Ey, Ey_px), Dx_z = dplus_x(Ez, Ez_px);
             const float4 Dz_x = Ex_pz - Ex, Dz_y = Ey_pz - Ey;
-            float4 Hx = fma4(S, Dy_z - Dz_y, Hpx), Hy = fma4(S, Dz_x - Dx_z, Hpy), Hz = fma4(S, Dx_y - Dy_x, Hpz);
+            // S im at my cells (halo threads included: whatever they produce outside I is discarded below)
+            const float4 sim = (P.im && many && inz) ? S * ldg4(P.im + kk * plane + own_xy) : splat(S);
+            float4 Hx = fma4(sim, Dy_z - Dz_y, Hpx), Hy = fma4(sim, Dz_x - Dx_z, Hpy), Hz = fma4(sim, Dx_y - Dy_x, Hpz);
             if (kk >= P.sHl && kk < P.sHh) {
                 const int sm = src_mask(P, kk);
                 if (sm & 8) Hx = Hx - add_sources4(P, n, 3, splat(0.f), i, j, kk);
@@ -1107,8 +1113,11 @@ typedef std::vector<std::vector<std::pair<long long, long long>>> Runs;
 // The plain split: the whole sequence cut into n_cta contiguous runs.  Neighbouring columns are then marched
 // with arbitrary plane offsets, so the halo rows a tile shares with its y neighbours miss L2 (measured on C3:
 // +76 MB of DRAM reads per launch, +27 % over the lock-step split below).
+thread_local int t_partition_kind = FDTD_PARTITION_NONE;    // what the last make_runs() on this thread produced
+
 Runs contiguous_runs(const std::vector<double> &w, int nz, int n_cta)
 {
+    t_partition_kind = FDTD_PARTITION_CONTIGUOUS;
     const std::vector<long long> cut = equal_cost_cuts(w, n_cta);
     Runs runs(n_cta);
     for (int c = 0; c < n_cta; ++c)
@@ -1163,6 +1172,7 @@ Runs lockstep_runs(const std::vector<double> &w, int nz, int n_cta)
             runs.push_back(run);
         }
     }
+    t_partition_kind = FDTD_PARTITION_LOCKSTEP;
     return runs;
 }
 
@@ -1198,6 +1208,7 @@ Runs wave_runs(const std::vector<double> &w, int nz, int n_cta)
         used[c] += colw[t];
     }
     if (dealt < (size_t)n_cta) return lockstep_runs(w, nz, n_cta);      // not even one full wave
+    t_partition_kind = FDTD_PARTITION_WAVES;
     if (dealt == order.size()) return runs;
     // the pool: positions of the columns order[dealt..], column after column
     double pool = 0.0;
@@ -1364,6 +1375,7 @@ int fused_setup(fdtd_grid *g)
     std::vector<Segment> all;
     std::vector<int> begins;
     segments_from_runs(nty, G.nz, F->TX, F->TY, 0, 0, 0, make_runs(model_cost(G, F->TX, F->TY, wy, wz), G.nz, n_cta), all, begins);
+    g->partition = t_partition_kind;
     F->seg_cap = (size_t)n_cta + (size_t)ntx * nty + 8;        // a run adds at most one segment per column boundary
     const size_t stride = F->seg_cap;
     for (int q = 0; q < 2; ++q) {
@@ -1493,6 +1505,13 @@ int fused_setup(fdtd_grid *g)
     g->tile_z = (int)std::min<long long>(G.nz, total / n_cta);
     if (!getenv("FDTD_NO_CALIBRATE") && total >= 8LL * n_cta) return calibrate(g);
     return FDTD_OK;
+}
+
+int fused_alloc_backward(fdtd_grid *g)
+{
+    FusedState *F = g->fused;
+    if (!F || F->lamB) return FDTD_OK;
+    return g->alloc((void **)&F->lamB, (size_t)g->G.nc * 6 * sizeof(float));
 }
 
 void fused_teardown(fdtd_grid *g)
@@ -1652,7 +1671,7 @@ static int calibrate(fdtd_grid *g)
                 for (const std::pair<long long, long long> &r : runs[c]) for (long long q = r.first; q < r.second; ++q) w[q] *= scale;
             }
             average_classes(w, cls, G.nz);
-            if (span < best) { best = span; best_runs = runs; best_fb = w; }
+            if (span < best) { best = span; best_runs = runs; best_fb = w; if (mode == 0) g->partition = t_partition_kind; }
         }
         if (best_runs.empty()) return done(fdtd_fail(FDTD_ECUDA, "calibration: no partition fits the segment table"));
         segments_from_runs(nty, G.nz, F->TX, F->TY, 0, 0, 0, best_runs, segs, begins);
@@ -1709,10 +1728,11 @@ void enqueue_fwd(void *vctx, cudaStream_t cs)
     }
     F->tile->launch_fwd(Q, F->n_cta, F->smem, cs);
     if (c->recording) join_side(g, cs, 1);
+    ++g->enq_step;
 }
 
 struct BwdCtx {
-    fdtd_grid *g; StepParams P; InvParams I; bool fused_inv; bool fused_det; bool pipelined; bool want_grad; float *bufB; float *fields; const float *ie; float *grad; float *lamA; float *lamB;
+    fdtd_grid *g; StepParams P; InvParams I; bool fused_inv; bool fused_det; bool pipelined; bool want_grad; float *bufB; float *fields; const float *ie; const float *im; float *grad; float *lamA; float *lamB;
     const std::vector<SourceDev> *S; const std::vector<DetectorDev> *D; int total_freq;
 };
 // Reverse step n.  One kernel after the other: B1 (detector cotangents into the volume about to be read), B2+B5
@@ -1742,11 +1762,12 @@ void enqueue_bwd(void *vctx, cudaStream_t cs)
         if (G.d > 0) launch_inject_pipe(G, g->R, c->fields, c->bufB, g->rec, g->step_in(), g->side_stream[1]);
         F->tile->launch_adj(Q, F->n_adj, F->smem, cs);
         join_side(g, cs, n_side);
+        ++g->enq_step; ++g->enq_inv;
         return;
     }
     if (!c->fused_det) { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
       for (const DetectorDev &dt : *c->D)
-          if (dt.phasor) launch_detector_adjoint_pp(G, c->lamA, c->lamB, dt, g->d_cs, c->total_freq, g->step_in(), cs); }
+          if (dt.phasor) launch_detector_adjoint_pp(G, c->lamA, c->lamB, dt, g->d_cs, c->total_freq, g->step_in(), c->im, cs); }
     // the face injection (it writes cells of the primal volume, which the adjoint step never touches) runs beside it
     const bool side_inject = c->fused_inv && G.d > 0;       // fused_inv implies want_grad
     { ProfScope p(g, fdtd_grid::PC_FUSED_BWD, cs);
@@ -1755,18 +1776,20 @@ void enqueue_bwd(void *vctx, cudaStream_t cs)
           launch_inject_pipe(G, g->R, c->fields, c->bufB, g->rec, g->step_in(), g->side_stream[0]);
       }
       F->tile->launch_adj(Q, F->n_adj, F->smem, cs);
+      ++g->enq_step;
       if (side_inject) join_side(g, cs, 1); }
     if (c->fused_inv) {
         InvParams J = c->I;
         J.step = g->step_in();
         { ProfScope p(g, fdtd_grid::PC_FUSED_INV, cs); F->itile->launch_inv(J, F->in_cta, F->ismem, cs); }
+        ++g->enq_inv;
         return;
     }
     if (!c->want_grad) return;
     { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
       for (const SourceDev &s : *c->S) if (s.comp >= 3) launch_add_source(G, c->fields, s, g->step_in(), -1.f, cs); }
     if (G.d > 0) { ProfScope p(g, fdtd_grid::PC_INJECT, cs); launch_inject(G, g->R, c->fields, g->rec, g->step_in(), cs); }
-    { ProfScope p(g, fdtd_grid::PC_INV_H, cs); launch_inv_H(G, c->fields, nullptr, cs); }
+    { ProfScope p(g, fdtd_grid::PC_INV_H, cs); launch_inv_H(G, c->fields, c->im, cs); }
     { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
       for (const SourceDev &s : *c->S) if (s.comp < 3) launch_add_source(G, c->fields, s, g->step_in(), -1.f, cs); }
     { ProfScope p(g, fdtd_grid::PC_INV_E_GRAD, cs);
@@ -1826,14 +1849,15 @@ int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float
 // result is back in volume 0 = g->lam.
 int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
                    const std::vector<SourceDev> &S, const std::vector<DetectorDev> &D, int total_freq, int n_steps,
-                   float *dL_dinv_eps, cudaStream_t st)
+                   float *dL_dinv_eps, bool seeded_H, cudaStream_t st)
 {
     FusedState *F = g->fused;
-    if (inv_mu) return fdtd_fail(FDTD_ESTATE, "fused backward does not take inv_mu");
     const size_t vol6 = (size_t)g->G.nc * 6 * sizeof(float);
     int rc;
-    if (!F->lamB && (rc = g->alloc((void **)&F->lamB, vol6))) return rc;
+    if ((rc = fused_alloc_backward(g))) return rc;
     if ((rc = build_maps(g, 1, g->lam, F->lamB, inv_eps, st))) return rc;
+    // with inv_mu the sweep runs on Lambda_H = im lamH (see k_step); fdtd_backward scales the result back
+    if (inv_mu && seeded_H) launch_scale_H(g->G, g->lam, inv_mu, false, st);
     if (n_steps & 1) {
         cudaError_t e = cudaMemcpyAsync(F->lamB, g->lam, vol6, cudaMemcpyDeviceToDevice, st);
         if (e != cudaSuccess) { (void)cudaGetLastError(); return fdtd_fail(FDTD_ECUDA, cudaGetErrorString(e)); }
@@ -1845,7 +1869,7 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     for (const DetectorDev &dt : D) if (dt.phasor && (dt.mask >> 3)) fused_det = false;
     // while profiling (events around every launch) the kernels run one after the other, so each is timed alone
     const bool pipelined = fused_inv && fused_det && F->n_inv_p > 0 && !g->profiling;
-    BwdCtx ctx{ g, F->sp, F->ip, fused_inv, fused_det, pipelined, want_grad, F->bufB, fields, inv_eps, dL_dinv_eps, g->lam, F->lamB, &S, &D, total_freq };
+    BwdCtx ctx{ g, F->sp, F->ip, fused_inv, fused_det, pipelined, want_grad, F->bufB, fields, inv_eps, inv_mu, dL_dinv_eps, g->lam, F->lamB, &S, &D, total_freq };
     if (fused_inv) {
         // reverse step n reads primal volume (n+1)&1 and writes n&1: state n_steps must sit in volume n_steps&1
         if ((rc = build_inv_maps(g, fields, F->bufB, inv_eps, g->lam, F->lamB, st))) return rc;
@@ -1855,7 +1879,7 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
         }
         InvParams &I = ctx.I;
         I.maps = F->d_maps[2]; I.lmaps = F->d_maps[2] + 13;
-        I.buf[0] = fields; I.buf[1] = F->bufB; I.grad = dL_dinv_eps;
+        I.buf[0] = fields; I.buf[1] = F->bufB; I.grad = dL_dinv_eps; I.im = inv_mu;
         I.n_src = (int)S.size();
         I.sEl = I.sHl = 1 << 30; I.sEh = I.sHh = -1;
         for (size_t q = 0; q < S.size(); ++q) {
@@ -1869,7 +1893,7 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     P.maps = F->d_maps[1];
     P.segs = F->d_segs[1]; P.seg_begin = F->d_seg_begin[1];
     P.buf[0] = g->lam; P.buf[1] = F->lamB;
-    P.ie = inv_eps; P.im = nullptr;
+    P.ie = inv_eps; P.im = inv_mu;
     for (int q = 0; q < 2; ++q) { P.psiE[q] = g->lpsiE[q]; P.psiH[q] = g->lpsiH[q]; }
     P.n_src = 0; P.n_det = 0; P.total_freq = total_freq;
     P.sEl = P.sHl = P.dEl = P.dHl = 1 << 30; P.sEh = P.sHh = P.dEh = P.dHh = -1;
@@ -1901,5 +1925,6 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     J.step = g->d_step + (n_steps & 1);
     { ProfScope p(g, fdtd_grid::PC_FUSED_INV, st); F->itile->launch_inv(J, F->in_cta, F->ismem, st); }
     g->kernel_launches += 1;
+    g->fused_inverse_launches += 1;
     return FDTD_OK;
 }

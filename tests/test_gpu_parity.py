@@ -61,11 +61,11 @@ def loss_cotangents(w, fields, phasors, interior_only=False):
     return None, None
 
 
-def run_oracle(w, n_steps=None, backward=True, f0=None):
+def run_oracle(w, n_steps=None, backward=True, f0=None, dtype=np.float64):
     from oracle.oracle import Oracle
     n = w.n_steps if n_steps is None else n_steps
-    o = Oracle(**w.grid_kwargs())
-    f = np.zeros((6, w.nz, w.ny, w.nx)) if f0 is None else f0.astype(np.float64).copy()
+    o = Oracle(**w.grid_kwargs(), dtype=dtype)
+    f = np.zeros((6, w.nz, w.ny, w.nx), dtype=dtype) if f0 is None else f0.astype(dtype).copy()
     out = o.forward(f, w.inv_eps, w.meta.get("inv_mu"), w.sources, w.detectors, n, record=backward and w.pml_cells > 0)
     res = {"fields": f.copy(), "phasors": out["phasors"]}
     if backward:
@@ -75,7 +75,7 @@ def run_oracle(w, n_steps=None, backward=True, f0=None):
     return res
 
 
-def run_gpu(B, w, path, n_steps=None, backward=True, f0=None, grad_box=None, record_mode=1):
+def run_gpu(B, w, path, n_steps=None, backward=True, f0=None, grad_box=None, record_mode=1, rho_box=None):
     import torch
     n = w.n_steps if n_steps is None else n_steps
     kw = w.grid_kwargs()
@@ -94,8 +94,13 @@ def run_gpu(B, w, path, n_steps=None, backward=True, f0=None, grad_box=None, rec
     if backward:
         dLp, dLf = loss_cotangents(w, f, ph)
         grad, lam0 = g.backward(f, ie, im, w.sources, w.detectors, dLp, dLf, n, want_dL_dfields0=True)
+        if rho_box is not None:            # B6 through the ABI: dL/drho on the design box
+            lo, hi = rho_box
+            drho = torch.empty((hi[2] - lo[2], hi[1] - lo[1], hi[0] - lo[0]), dtype=torch.float32, device="cuda")
+            B.fdtd_grad_rho(g.h, grad, ie, float(w.meta["delta_eps"]), lo, hi, drho, g.stream())
+            res["dL_drho"] = drho.cpu().numpy()
         torch.cuda.synchronize()
-        res.update(grad=grad.cpu().numpy(), lam0=lam0.cpu().numpy(), state0=f.cpu().numpy())
+        res.update(grad=grad.cpu().numpy(), lam0=lam0.cpu().numpy(), state0=f.cpu().numpy(), info=g.info())
     g.close()
     return res
 
@@ -150,9 +155,18 @@ def test_c3_mini_all_paths(B, kappa, alpha):
     forward fields + phasors + reversible gradient + cotangent of state 0, every kernel path."""
     w = wl.c3_mini(kappa_max=kappa, alpha_max=alpha)
     ref = run_oracle(w)
+    # conditioning of the workload itself: the fp32 build of the oracle against its fp64 build (the pulse has
+    # crossed the detector plane by the end of the run, so the gradient is not dominated by cancellation)
+    ref32 = run_oracle(w, dtype=np.float32)
+    cond = relerr(ref32["grad"], ref["grad"])
+    print("c3-mini oracle fp32 vs fp64: gradient", cond, "phasor", relerr(ref32["phasors"][0], ref["phasors"][0]))
+    assert cond <= 1e-4
+    assert np.max(np.abs(ref["phasors"][0])) > 0.2 * np.max(np.abs(ref["fields"]))      # the pulse did reach the detector
     for path in paths(B, w):
         gpu = run_gpu(B, w, path)
         assert gpu["info"].path == path
+        if path == B.FDTD_PATH_FUSED:
+            assert gpu["info"].fused_step_launches == 2 * w.n_steps and gpu["info"].fused_inverse_launches >= w.n_steps
         print("c3-mini path", path, compare(w, gpu, ref))
 
 
@@ -163,7 +177,86 @@ def test_c3_mini_with_inv_mu_and_h_source(B):
     w.sources.append(wl.Source(3, (20, 12, 14), (30, 20, 16), (0.3 * wl.gaussian_sine(80, 20, 8, 10)).astype(np.float32)))
     ref = run_oracle(w)
     for path in paths(B, w):
-        print("c3-mini mu", path, compare(w, run_gpu(B, w, path), ref))
+        gpu = run_gpu(B, w, path)
+        print("c3-mini mu", path, compare(w, gpu, ref))
+        if path == B.FDTD_PATH_FUSED:       # inv_mu goes through the fused adjoint and inverse kernels, not the generic ones
+            assert gpu["info"].pipelined_inverse_ctas > 0
+            assert gpu["info"].fused_step_launches == 2 * w.n_steps and gpu["info"].fused_inverse_launches == w.n_steps
+    # the same with an E-only loss detector: the pipelined (grouped) reverse sweep carries inv_mu too
+    w.detectors[0] = wl.Detector(1 << 1, w.detectors[0].lo, w.detectors[0].hi, w.detectors[0].omega)
+    ref = run_oracle(w)
+    gpu = run_gpu(B, w, B.FDTD_PATH_FUSED)
+    print("c3-mini mu, pipelined", compare(w, gpu, ref))
+    assert gpu["info"].fused_inverse_launches == w.n_steps + 1      # step n_steps (empty) .. 1 in the groups, step 0 after the loop
+
+
+def test_fused_inverse_subtracts_h_sources(B):
+    """SURVEY B3 (`H' - srcH_n`): an H-component source inside the interior, inv_mu = NULL and an E-only loss
+    detector, so the whole reverse sweep runs in the fused kernels (pipelined groups): k_inverse has to take the
+    H source out again before it inverts the H update."""
+    w = wl.c3_mini(nx=64, ny=40, nz=36, d=6, n_steps=90)
+    w.detectors[0] = wl.Detector(1 << 1, w.detectors[0].lo, w.detectors[0].hi, w.detectors[0].omega)
+    w.sources.append(wl.Source(4, (18, 10, 12), (31, 19, 15), (0.4 * wl.gaussian_sine(90, 25, 8, 10)).astype(np.float32)))
+    w.sources.append(wl.Source(5, (40, 22, 20), (41, 23, 21), (0.3 * wl.gaussian_sine(90, 20, 7, 9)).astype(np.float32)))
+    ref = run_oracle(w)
+    for path in paths(B, w):
+        gpu = run_gpu(B, w, path)
+        print("H sources", path, compare(w, gpu, ref))
+        if path == B.FDTD_PATH_FUSED:
+            assert gpu["info"].fused_inverse_launches == w.n_steps + 1
+    # teeth: without the H sources the reconstructed state differs by far more than the tolerance
+    w0 = wl.c3_mini(nx=64, ny=40, nz=36, d=6, n_steps=90)
+    w0.detectors[0] = w.detectors[0]
+    assert relerr(run_oracle(w0)["fields"], ref["fields"]) > 1e-2
+
+
+def test_fused_path_with_prime_ny_nz(B):
+    """Ragged tails with no common factor with any tile height: ny = 53, nz = 47 (nx = 88 as the float4 rows need)."""
+    w = wl.c3_mini(nx=88, ny=53, nz=47, d=8, n_steps=100, kappa_max=3.0, alpha_max=0.05)
+    ref = run_oracle(w)
+    for path in paths(B, w):
+        gpu = run_gpu(B, w, path)
+        assert gpu["info"].path == path
+        print("prime ny nz", path, compare(w, gpu, ref))
+
+
+def test_more_descriptors_than_the_fused_kernels_hold(B):
+    """include/fdtd.h "Kernel paths": 5 sources and 5 detectors on a grid that qualifies for the fused kernels.  Under
+    FDTD_PATH_AUTO the forward call runs on the generic kernels and the reverse sweep degrades per feature; the
+    result matches the oracle.  FDTD_PATH_FUSED refuses the call with EINVAL."""
+    w = wl.c3_mini(nx=64, ny=40, nz=36, d=6, n_steps=70)
+    d0 = w.detectors[0]
+    for q in range(4):
+        w.sources.append(wl.Source(q % 3, (10 + 9 * q, 9 + 3 * q, 9 + 4 * q), (14 + 9 * q, 12 + 3 * q, 10 + 4 * q),
+                                   (0.2 * wl.gaussian_sine(70, 15 + 3 * q, 6, 9 + q)).astype(np.float32)))
+        w.detectors.append(wl.Detector(1 << (q % 3), (8, 8, 12 + 3 * q), (56, 32, 13 + 3 * q), [wl.omega_ppw(11 + q)]))
+    w.loss_detectors = (0, 2, 4)
+    assert len(w.sources) == 5 and len(w.detectors) == 5
+    ref = run_oracle(w)
+    gpu = run_gpu(B, w, B.FDTD_PATH_AUTO)
+    assert gpu["info"].path == B.FDTD_PATH_FUSED          # the grid itself is a fused grid
+    print("5 sources, 5 detectors", compare(w, gpu, ref))
+    with pytest.raises(B.FdtdError) as ei:
+        run_gpu(B, w, B.FDTD_PATH_FUSED)
+    assert ei.value.code == B.FDTD_EINVAL
+
+
+def test_b6_grad_rho_parity(B):
+    """SURVEY 8(a) B6 / R20 through the ABI: fdtd_grad_rho on the design box (offset from the origin) against the
+    oracle's orc_grad_rho applied to the oracle's gradient, element by element, every kernel path."""
+    w = wl.c3_mini()
+    lo, hi = w.design_lo, w.design_hi
+    assert min(lo) > 0
+    from oracle.oracle import Oracle
+    ref = run_oracle(w)
+    ref_drho = Oracle(**w.grid_kwargs()).grad_rho(ref["grad"], w.inv_eps, w.meta["delta_eps"], lo, hi)
+    assert ref_drho.shape == w.meta["rho"].shape and np.max(np.abs(ref_drho)) > 0
+    for path in paths(B, w):
+        for rmode, gbox in ((1, None), (2, (lo, hi))):
+            gpu = run_gpu(B, w, path, rho_box=(lo, hi), grad_box=gbox, record_mode=rmode)
+            e = relerr(gpu["dL_drho"], ref_drho)
+            print("B6 dL/drho", path, "record", rmode, e)
+            assert gpu["dL_drho"].shape == ref_drho.shape and e <= TOL_GRAD
 
 
 def test_c2_fields_at_100_200_and_phasor_at_1000(B):
@@ -321,13 +414,26 @@ def test_c3_full_size_truncated_in_the_bench_configuration(B):
     and the loss is sum E^2 at the final state, so fields, gradient and cotangents are non-trivial."""
     w = wl.c3(n_steps=40, source_k=66)
     w.loss = "final_E2"
-    ref = run_oracle(w)
+    # a seeded random initial state (amplitude 0.1, all six components, every cell): every CPML slab, edge and corner
+    # cell of the 200 x 7 lock-step configuration is compared on non-zero values
+    f0 = (0.1 * np.random.default_rng(40).standard_normal((6, w.nz, w.ny, w.nx))).astype(np.float32)
+    ref = run_oracle(w, f0=f0)
     lo, hi = w.design_lo, w.design_hi
     box = (slice(lo[2], hi[2]), slice(lo[1], hi[1]), slice(lo[0], hi[0]))
     assert np.max(np.abs(ref["grad"][box])) > 0
     scale = np.max(np.abs(ref["fields"]))
+    d = w.pml_cells
+    regions = 0
+    for rz in (slice(0, d), slice(d, w.nz - d), slice(w.nz - d, w.nz)):
+        for ry in (slice(0, d), slice(d, w.ny - d), slice(w.ny - d, w.ny)):
+            for rx in (slice(0, d), slice(d, w.nx - d), slice(w.nx - d, w.nx)):
+                for c in range(6):         # reference fields and state-0 cotangents are non-zero in all 27 regions
+                    assert np.max(np.abs(ref["fields"][c][rz, ry, rx])) > 1e-3 * scale
+                    assert np.max(np.abs(ref["lam0"][c][rz, ry, rx])) > 0
+                regions += 1
+    assert regions == 27
     for mode in (2, 1):
-        gpu = run_gpu(B, w, B.FDTD_PATH_FUSED, grad_box=(lo, hi), record_mode=mode)
+        gpu = run_gpu(B, w, B.FDTD_PATH_FUSED, grad_box=(lo, hi), record_mode=mode, f0=f0)
         assert gpu["info"].path == B.FDTD_PATH_FUSED
         eE, eH = relerr(gpu["fields"][:3], ref["fields"][:3]), relerr(gpu["fields"][3:], ref["fields"][3:])
         eG, eL = relerr(gpu["grad"][box], ref["grad"][box]), relerr(gpu["lam0"], ref["lam0"])
