@@ -245,6 +245,8 @@ def main():
     ap.add_argument("--ref-sample-steps", type=int, default=12)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--lean", action="store_true",
+                    help="memory-scale runs: no second (forward-only) grid, hence no forward-only and adjoint-only passes")
     ap.add_argument("--record", default="", choices=["", "1", "2", "both"],
                     help="1: `value` only (record the PML/interior interface, reconstruct the interior); 2: `value` on the "
                          "design-box recorder instead (labelled); both (default where there is a design box and memory allows): "
@@ -299,7 +301,7 @@ def main():
 
     grid = make_grid(main_record, staging=not args.no_e2e)          # the `value` grid
     grid2 = make_grid(2) if rec_arg == "both" else None             # N1 extra: design-box recorder
-    grid_f = make_grid(0)                                           # forward-only grid (no recorder)
+    grid_f = None if args.lean else make_grid(0)                    # forward-only grid (no recorder)
     stream = torch.cuda.Stream()
     dev = torch.device("cuda", local_rank)
     ie = torch.as_tensor(w.inv_eps).to(dev)
@@ -376,20 +378,22 @@ def main():
             n1 = {"value": sharding.whole_job_rate(w.cells * T, reps2, ms2, world), "unit": UNIT, "ms_per_step": ms2 / reps2,
                   "max_abs_dL_drho": float(drho.double().abs().max()), "loss": loss_value()}
 
-        # forward-only (record=0) rate, same workload
-        for _ in range(min(args.warmup, 2)):
-            forward_only(grid_f)
-        ms_fwd = timed(lambda: forward_only(grid_f), max(1, args.steps))
-
-        # adjoint sweep only (dL_dinv_eps = NULL: one k_step<adjoint> launch per time step), same cotangent seed
-        dLp_t, dLf_t = loss_cotangents()
-
-        def adjoint_only(g):
-            g.backward(fields, ie, None, w.sources, w.detectors, dLp_t, dLf_t, T, want_grad=False)
-
-        adjoint_only(grid_f)
+        ms_fwd = ms_adj = None
         reps_adj = max(1, min(args.steps, 3))
-        ms_adj = timed(lambda: adjoint_only(grid_f), reps_adj)
+        if grid_f is not None:
+            # forward-only (record=0) rate, same workload
+            for _ in range(min(args.warmup, 2)):
+                forward_only(grid_f)
+            ms_fwd = timed(lambda: forward_only(grid_f), max(1, args.steps))
+
+            # adjoint sweep only (dL_dinv_eps = NULL: one k_step<adjoint> launch per time step), same cotangent seed
+            dLp_t, dLf_t = loss_cotangents()
+
+            def adjoint_only(g):
+                g.backward(fields, ie, None, w.sources, w.detectors, dLp_t, dLf_t, T, want_grad=False)
+
+            adjoint_only(grid_f)
+            ms_adj = timed(lambda: adjoint_only(grid_f), reps_adj)
 
         # ---- per-kernel roofline: one more pass with every step kernel bracketed by CUDA events --------
         B.fdtd_set_profiling(grid.h, True)
@@ -401,7 +405,7 @@ def main():
 
     cells_steps = w.cells * T
     value = sharding.whole_job_rate(cells_steps, args.steps, ms_total, world)
-    fwd_value = sharding.whole_job_rate(cells_steps, max(1, args.steps), ms_fwd, world)
+    fwd_value = sharding.whole_job_rate(cells_steps, max(1, args.steps), ms_fwd, world) if ms_fwd else None
 
     peaks_file = ROOT / "MEASURED_PEAKS.json"
     if peaks_file.exists():
@@ -445,7 +449,7 @@ def main():
                     "frac_of_8000": kernels[dom]["achieved_gbs"] / 8000.0}
         # the same kernel template inside the replayed CUDA graph (no events between launches): the forward-only
         # pass is one k_step launch per time step, so its time / launches is that kernel's launch-to-launch period
-        if info_path_fused:
+        if info_path_fused and ms_fwd:
             fb = algorithmic_bytes(w, grad_cells, recording=False)["fused_forward_step"]
             us = ms_fwd / max(1, args.steps) / T * 1e3
             roofline["forward_step_in_graph"] = {"avg_launch_us": us, "alg_bytes_per_launch": fb,
@@ -468,8 +472,9 @@ def main():
                                        "in the replayed graph, time / launches")
         # whole-job fractions: algorithmic B/cell/step x rate against the measured peak and the 8000 GB/s bar
         bpc = whole_job_bytes_per_cell_step(w, grad_cells, rbox=rbox_main)
-        wj = {"fwd": {"bytes_per_cell_step": bpc["fwd"], "achieved": bpc["fwd"] * fwd_value / world / 1e3},
-              f"fwd_bwd_record{main_record}": {"bytes_per_cell_step": bpc["fwd_bwd"], "achieved": bpc["fwd_bwd"] * value / world / 1e3}}
+        wj = {f"fwd_bwd_record{main_record}": {"bytes_per_cell_step": bpc["fwd_bwd"], "achieved": bpc["fwd_bwd"] * value / world / 1e3}}
+        if fwd_value:
+            wj["fwd"] = {"bytes_per_cell_step": bpc["fwd"], "achieved": bpc["fwd"] * fwd_value / world / 1e3}
         if n1 is not None:
             b2 = whole_job_bytes_per_cell_step(w, grad_cells, rbox=dbox)["fwd_bwd"]
             wj["fwd_bwd_record2"] = {"bytes_per_cell_step": b2, "achieved": b2 * n1["value"] / world / 1e3}
@@ -548,7 +553,7 @@ def main():
                                              "recorder": rec_names[main_record],
                                              "recorder_bytes": int(info.recorder_bytes), "scratch_bytes": int(info.scratch_bytes)}),
                "fwd": {"value": fwd_value, "unit": UNIT, "ms_per_pass": ms_fwd / max(1, args.steps),
-                       "what": "forward only, record=0, same workload"},
+                       "what": "forward only, record=0, same workload"} if ms_fwd else None,
                "n1_design_box_recorder": n1,
                "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
                "roofline": roofline, "kernels": kernels, "cpu_baseline": cpu,
@@ -557,7 +562,8 @@ def main():
                                           "grid_recorder": int(info.recorder_bytes), "grid_scratch": int(info.scratch_bytes)}}}
         print(json.dumps(out))
     grid.close()
-    grid_f.close()
+    if grid_f is not None:
+        grid_f.close()
     if grid2 is not None:
         grid2.close()
     if world > 1:

@@ -503,14 +503,121 @@ static void record_faces(const orc_desc *D, const REAL *fields, size_t nc, REAL 
 }
 
 /* ------------------------------------------------------------------------ */
-/* forward driver: n_steps of  [O0r] O1 O2 [O2r] O3 O4 O5                   */
+/* N2 ("access to intermediate fields, energy,     */
+/* Poynting flux", L70 interpolation off by default): time-domain detectors. */
+/* Reading R23: a time-domain detector fires after step n when               */
+/* (n+1) % stride == 0, record index q = (n+1)/stride - 1, on the state      */
+/* (E^{n+1}, H^{n+3/2}) -- the same time stamp as the DFT detectors (R13):   */
+/*   kind 0 SNAPSHOT: out[q][ci][cell] = F_c[cell] for every c in mask       */
+/*   kind 1 ENERGY  : out[q] = sum_cells 1/2 (sum_c E_c^2/ie + H_c^2/im)     */
+/*                    (eta0-normalised H, energy in units of eps0 dx^3; the   */
+/*                    six components are taken at the same index, no          */
+/*                    co-location, as the paper's default)                    */
+/* ------------------------------------------------------------------------ */
+typedef struct {
+    int kind;              /* 0 snapshot, 1 energy                             */
+    int mask;              /* snapshot: components; energy: ignored            */
+    int lo[3], hi[3];
+    int stride;            /* >= 1                                             */
+    REAL *out;             /* snapshot [n_rec][n_comp][cells]; energy [n_rec]  */
+} orc_tdetector;
+
+static void time_detect(const orc_desc *D, const REAL *fields, size_t nc, const REAL *ie, const REAL *im,
+                        const orc_tdetector *td, int n_td, int n)
+{
+    for (int s = 0; s < n_td; ++s) {
+        const orc_tdetector *q = &td[s];
+        if ((n + 1) % q->stride != 0) continue;
+        const size_t rec_i = (size_t)((n + 1) / q->stride - 1);
+        const int bx = q->hi[0] - q->lo[0], by = q->hi[1] - q->lo[1], bz = q->hi[2] - q->lo[2];
+        const size_t bc = (size_t)bx * by * bz;
+        if (q->kind == 0) {
+            const int ncomp = popcount6(q->mask);
+            int ci = 0;
+            for (int c = 0; c < 6; ++c) {
+                if (!((q->mask >> c) & 1)) continue;
+                REAL *out = q->out + (rec_i * ncomp + ci) * bc;
+                for (int k = q->lo[2]; k < q->hi[2]; ++k)
+                    for (int j = q->lo[1]; j < q->hi[1]; ++j)
+                        for (int i = q->lo[0]; i < q->hi[0]; ++i)
+                            out[((size_t)(k - q->lo[2]) * by + (j - q->lo[1])) * bx + (i - q->lo[0])] = fields[(size_t)c * nc + IDX(i, j, k)];
+                ++ci;
+            }
+        } else {
+            double acc = 0.0;
+            for (int k = q->lo[2]; k < q->hi[2]; ++k)
+                for (int j = q->lo[1]; j < q->hi[1]; ++j)
+                    for (int i = q->lo[0]; i < q->hi[0]; ++i) {
+                        const size_t p = IDX(i, j, k);
+                        double e2 = 0.0, h2 = 0.0;
+                        for (int c = 0; c < 3; ++c) {
+                            e2 += (double)fields[(size_t)c * nc + p] * fields[(size_t)c * nc + p];
+                            h2 += (double)fields[(size_t)(3 + c) * nc + p] * fields[(size_t)(3 + c) * nc + p];
+                        }
+                        acc += 0.5 * (e2 / (double)ie[p] + h2 / (im ? (double)im[p] : 1.0));
+                    }
+            q->out[rec_i] = (REAL)acc;
+        }
+    }
+}
+
+/* transpose of time_detect at reverse step n, with G = dL/d out:                               */
+/*   snapshot: lam F_c[cell] += G[q][ci][cell]                                                  */
+/*   energy  : lam E_c += G[q] E_c/ie ; lam H_c += G[q] H_c/im  (primal state after step n: the  */
+/*             detector box must lie inside the reconstruction box I), and the explicit          */
+/*             dependence on ie:  g[cell] += G[q] * (-1/2) sum_c E_c^2 / ie^2                     */
+static void time_detect_adjoint(const orc_desc *D, REAL *lam, const REAL *fields, size_t nc, const REAL *ie, const REAL *im,
+                                const orc_tdetector *td, int n_td, const REAL *const *dL_dout, REAL *g, int n)
+{
+    if (!dL_dout) return;
+    for (int s = 0; s < n_td; ++s) {
+        const orc_tdetector *q = &td[s];
+        const REAL *G = dL_dout[s];
+        if (!G || (n + 1) % q->stride != 0) continue;
+        const size_t rec_i = (size_t)((n + 1) / q->stride - 1);
+        const int bx = q->hi[0] - q->lo[0], by = q->hi[1] - q->lo[1], bz = q->hi[2] - q->lo[2];
+        const size_t bc = (size_t)bx * by * bz;
+        if (q->kind == 0) {
+            const int ncomp = popcount6(q->mask);
+            int ci = 0;
+            for (int c = 0; c < 6; ++c) {
+                if (!((q->mask >> c) & 1)) continue;
+                const REAL *Gp = G + (rec_i * ncomp + ci) * bc;
+                for (int k = q->lo[2]; k < q->hi[2]; ++k)
+                    for (int j = q->lo[1]; j < q->hi[1]; ++j)
+                        for (int i = q->lo[0]; i < q->hi[0]; ++i)
+                            lam[(size_t)c * nc + IDX(i, j, k)] += Gp[((size_t)(k - q->lo[2]) * by + (j - q->lo[1])) * bx + (i - q->lo[0])];
+                ++ci;
+            }
+        } else {
+            const REAL Gq = G[rec_i];
+            for (int k = q->lo[2]; k < q->hi[2]; ++k)
+                for (int j = q->lo[1]; j < q->hi[1]; ++j)
+                    for (int i = q->lo[0]; i < q->hi[0]; ++i) {
+                        const size_t p = IDX(i, j, k);
+                        REAL e2 = (REAL)0;
+                        for (int c = 0; c < 3; ++c) {
+                            const REAL E = fields[(size_t)c * nc + p], H = fields[(size_t)(3 + c) * nc + p];
+                            lam[(size_t)c * nc + p] += Gq * E / ie[p];
+                            lam[(size_t)(3 + c) * nc + p] += Gq * H / (im ? im[p] : (REAL)1);
+                            e2 += E * E;
+                        }
+                        if (g) g[p] += Gq * (REAL)(-0.5) * e2 / (ie[p] * ie[p]);
+                    }
+        }
+    }
+}
+
+/* ------------------------------------------------------------------------ */
+/* forward driver: n_steps of  [O0r] O1 O2 [O2r] O3 O4 O5 [time detectors]  */
 /* rec   : NULL or n_steps * orc_record_stride() REALs                      */
 /* tape  : NULL or n_steps * 3 * cells REALs (bracket of every E update)    */
 /* psi is NOT reset here (callers use orc_zero_psi; R21)                    */
 /* ------------------------------------------------------------------------ */
-int orc_forward(orc_state *st, REAL *fields, const REAL *ie, const REAL *im,
-                const orc_source *src, int n_src, const orc_detector *det, int n_det,
-                int n_steps, REAL *rec, REAL *tape)
+int orc_forward_td(orc_state *st, REAL *fields, const REAL *ie, const REAL *im,
+                   const orc_source *src, int n_src, const orc_detector *det, int n_det,
+                   const orc_tdetector *td, int n_td,
+                   int n_steps, REAL *rec, REAL *tape)
 {
     const orc_desc *D = &st->D;
     const size_t nc = st->nc;
@@ -523,8 +630,16 @@ int orc_forward(orc_state *st, REAL *fields, const REAL *ie, const REAL *im,
         orc_step_H(st, fields, im);                                              /* O3  */
         add_sources(D, fields, nc, src, n_src, n, 1, (REAL)1);                   /* O4  */
         detect(D, fields, nc, det, n_det, n);                                    /* O5  */
+        time_detect(D, fields, nc, ie, im, td, n_td, n);                         /* N2  */
     }
     return 0;
+}
+
+int orc_forward(orc_state *st, REAL *fields, const REAL *ie, const REAL *im,
+                const orc_source *src, int n_src, const orc_detector *det, int n_det,
+                int n_steps, REAL *rec, REAL *tape)
+{
+    return orc_forward_td(st, fields, ie, im, src, n_src, det, n_det, NULL, 0, n_steps, rec, tape);
 }
 
 /* ------------------------------------------------------------------------ */
@@ -728,10 +843,12 @@ void orc_inv_E_grad(orc_state *st, REAL *fields, const REAL *ie, const REAL *lam
 /* fields: in = state n_steps (valid on I), out = reconstructed state 0 on I */
 /* g (cells) and dL_dfields0 (6*cells, may be NULL) are outputs.             */
 /* ------------------------------------------------------------------------ */
-int orc_backward(orc_state *st, REAL *fields, const REAL *ie, const REAL *im,
-                 const orc_source *src, int n_src, const orc_detector *det, int n_det,
-                 const REAL *const *dL_dphasor, const REAL *dL_dfields,
-                 int n_steps, const REAL *rec, REAL *g, REAL *dL_dfields0)
+int orc_backward_td(orc_state *st, REAL *fields, const REAL *ie, const REAL *im,
+                    const orc_source *src, int n_src, const orc_detector *det, int n_det,
+                    const REAL *const *dL_dphasor,
+                    const orc_tdetector *td, int n_td, const REAL *const *dL_dtd,
+                    const REAL *dL_dfields,
+                    int n_steps, const REAL *rec, REAL *g, REAL *dL_dfields0)
 {
     const orc_desc *D = &st->D;
     const size_t nc = st->nc;
@@ -744,6 +861,7 @@ int orc_backward(orc_state *st, REAL *fields, const REAL *ie, const REAL *im,
     memset(g, 0, nc * sizeof(REAL));
     for (int n = n_steps - 1; n >= 0; --n) {
         const REAL *rec_n = rec ? rec + (size_t)n * rs : NULL;
+        time_detect_adjoint(D, lam, fields, nc, ie, im, td, n_td, dL_dtd, g, n);   /* N2^T (primal state after step n) */
         detect_adjoint(D, lam, nc, det, n_det, dL_dphasor, n);           /* B1  */
         orc_adj_H(st, lam, im);                                          /* B2  */
         add_sources(D, fields, nc, src, n_src, n, 1, (REAL)-1);          /* undo O4 */
@@ -755,6 +873,15 @@ int orc_backward(orc_state *st, REAL *fields, const REAL *ie, const REAL *im,
     if (dL_dfields0) memcpy(dL_dfields0, lam, 6 * nc * sizeof(REAL));
     free(lam);
     return 0;
+}
+
+int orc_backward(orc_state *st, REAL *fields, const REAL *ie, const REAL *im,
+                 const orc_source *src, int n_src, const orc_detector *det, int n_det,
+                 const REAL *const *dL_dphasor, const REAL *dL_dfields,
+                 int n_steps, const REAL *rec, REAL *g, REAL *dL_dfields0)
+{
+    return orc_backward_td(st, fields, ie, im, src, n_src, det, n_det, dL_dphasor, NULL, 0, NULL, dL_dfields,
+                           n_steps, rec, g, dL_dfields0);
 }
 
 /* ------------------------------------------------------------------------ */
@@ -810,4 +937,141 @@ void orc_grad_rho(const orc_desc *D, const REAL *g, const REAL *ie, double delta
                 const REAL dinv = -(REAL)delta_eps * ie[p] * ie[p];
                 out[c] = g[p] * dinv;
             }
+}
+
+/* ------------------------------------------------------------------------ */
+/* N2: Poynting flux through a plane from the DFT phasors (PAPER.md L68      */
+/* "Poynting flux", L148 Fig. 5 "fraction of Poynting flux"; L70 "Yee        */
+/* interpolation", off by default).  Reading R24:                            */
+/* the detector box is a slab normal to `axis` a whose mask holds the four   */
+/* tangential components E_b, E_c, H_b, H_c (b = a+1, c = a+2 mod 3); for    */
+/* every frequency                                                           */
+/*   flux_f = 1/2 sum_cells Re( E_b conj(H_c) - E_c conj(H_b) )     (n = +e_a)*/
+/* interpolate = 0: slab one plane thick, phasors multiplied as accumulated  */
+/*   (same index, same phase stamp w (n+1): the paper's default);            */
+/* interpolate = 1: slab two planes thick (indices p-1, p along a); E from   */
+/*   plane p; H co-located with it in space, Hbar = (H[p-1] + H[p])/2 (H_c   */
+/*   sits half a cell above E_b along a and at the same in-plane position),  */
+/*   and in time, H~ = exp(-i w/2) Hbar (H is stamped half a step late).     */
+/* ------------------------------------------------------------------------ */
+static int comp_slot(int mask, int comp)
+{
+    int ci = 0;
+    for (int c = 0; c < comp; ++c) ci += (mask >> c) & 1;
+    return ci;
+}
+
+/* flux[n_freq] out; vjp: dL_dflux[n_freq] in, dL_dphasor (laid out like phasor) written */
+static int flux_impl(const orc_detector *q, const REAL *phasor, int axis, int interpolate,
+                     REAL *flux, const REAL *dL_dflux, REAL *dL_dphasor)
+{
+    const int a = axis, b = (a + 1) % 3, c = (a + 2) % 3;
+    const int need = (1 << b) | (1 << c) | (1 << (3 + b)) | (1 << (3 + c));
+    if ((q->mask & need) != need) return -1;
+    const int ext[3] = { q->hi[0] - q->lo[0], q->hi[1] - q->lo[1], q->hi[2] - q->lo[2] };
+    if (ext[a] != (interpolate ? 2 : 1)) return -1;
+    const size_t bc = (size_t)ext[0] * ext[1] * ext[2];
+    const int ncomp = popcount6(q->mask);
+    const int sEb = comp_slot(q->mask, b), sEc = comp_slot(q->mask, c);
+    const int sHb = comp_slot(q->mask, 3 + b), sHc = comp_slot(q->mask, 3 + c);
+    const int t1 = ext[a] - 1;                       /* plane of E (and of the upper H) inside the box */
+    if (dL_dphasor) memset(dL_dphasor, 0, (size_t)q->n_freq * ncomp * bc * 2 * sizeof(REAL));
+    for (int f = 0; f < q->n_freq; ++f) {
+        const double cw = interpolate ? cos(0.5 * q->omega[f]) : 1.0, sw = interpolate ? sin(0.5 * q->omega[f]) : 0.0;
+        const REAL *P = phasor + (size_t)f * ncomp * bc * 2;
+        REAL *dP = dL_dphasor ? dL_dphasor + (size_t)f * ncomp * bc * 2 : NULL;
+        double acc = 0.0;
+        int pos[3];
+        for (pos[2] = 0; pos[2] < ext[2]; ++pos[2])
+            for (pos[1] = 0; pos[1] < ext[1]; ++pos[1])
+                for (pos[0] = 0; pos[0] < ext[0]; ++pos[0]) {
+                    if (pos[a] != t1) continue;
+                    const size_t cell = ((size_t)pos[2] * ext[1] + pos[1]) * ext[0] + pos[0];
+                    int pm[3] = { pos[0], pos[1], pos[2] };
+                    pm[a] -= 1;
+                    const size_t cellm = interpolate ? ((size_t)pm[2] * ext[1] + pm[1]) * ext[0] + pm[0] : cell;
+                    /* pair 0: E_b with H_c (sign +), pair 1: E_c with H_b (sign -) */
+                    for (int pr = 0; pr < 2; ++pr) {
+                        const int sE = pr ? sEc : sEb, sH = pr ? sHb : sHc;
+                        const double sg = pr ? -1.0 : 1.0;
+                        const REAL *E = P + ((size_t)sE * bc + cell) * 2;
+                        const REAL *H1 = P + ((size_t)sH * bc + cell) * 2, *H0 = P + ((size_t)sH * bc + cellm) * 2;
+                        const double hr = interpolate ? 0.5 * ((double)H0[0] + H1[0]) : (double)H1[0];
+                        const double hi = interpolate ? 0.5 * ((double)H0[1] + H1[1]) : (double)H1[1];
+                        const double tr = hr * cw + hi * sw, ti = hi * cw - hr * sw;      /* H~ = exp(-i w/2) Hbar */
+                        acc += sg * 0.5 * ((double)E[0] * tr + (double)E[1] * ti);
+                        if (dP) {
+                            const double G = sg * 0.5 * (double)dL_dflux[f];
+                            REAL *dE = dP + ((size_t)sE * bc + cell) * 2;
+                            dE[0] += (REAL)(G * tr); dE[1] += (REAL)(G * ti);
+                            const double dtr = G * (double)E[0], dti = G * (double)E[1];
+                            const double dhr = dtr * cw - dti * sw, dhi = dtr * sw + dti * cw;
+                            REAL *d1 = dP + ((size_t)sH * bc + cell) * 2;
+                            if (interpolate) {
+                                REAL *d0 = dP + ((size_t)sH * bc + cellm) * 2;
+                                d1[0] += (REAL)(0.5 * dhr); d1[1] += (REAL)(0.5 * dhi);
+                                d0[0] += (REAL)(0.5 * dhr); d0[1] += (REAL)(0.5 * dhi);
+                            } else {
+                                d1[0] += (REAL)dhr; d1[1] += (REAL)dhi;
+                            }
+                        }
+                    }
+                }
+        if (flux) flux[f] = (REAL)acc;
+    }
+    return 0;
+}
+
+int orc_flux(const orc_detector *q, const REAL *phasor, int axis, int interpolate, REAL *flux)
+{
+    return flux_impl(q, phasor, axis, interpolate, flux, NULL, NULL);
+}
+
+int orc_flux_vjp(const orc_detector *q, const REAL *phasor, int axis, int interpolate,
+                 const REAL *dL_dflux, REAL *dL_dphasor)
+{
+    return flux_impl(q, phasor, axis, interpolate, NULL, dL_dflux, dL_dphasor);
+}
+
+/* ------------------------------------------------------------------------ */
+/* N2: one-directional plane source = Total-Field/Scattered-Field interface  */
+/* ("Total-Field Scattered-Field", L130).  Reading R25.         */
+/* A plane wave travelling along axis a (dir = +1 / -1), E polarised along   */
+/* `pol` = b != a, its H along the third axis c, in a medium that is uniform */
+/* (eps_r, mu_r) on the planes the interface touches.  With                  */
+/*   sgn = +1 if a == b+1 (mod 3), -1 if a == b+2                            */
+/* the updates of 8.0 restricted to this wave are the 1-D leapfrog           */
+/*   e[m] += sgn S ie (h[m] - h[m-1]) ;  h[m] += sgn S im (e[m+1] - e[m]).   */
+/* The incident wave is generated on an auxiliary 1-D grid of exactly that   */
+/* form (same S, same medium, hard source e[0] = base[n], long enough that   */
+/* its far wall is out of causal reach), so it carries the 3-D grid's own    */
+/* numerical dispersion and the field behind the interface cancels to        */
+/* rounding.  Interface at plane p0 (aux node m0 = 2), total-field side =    */
+/* the side the wave travels to.  The two additive patches (R10/R11) are     */
+/*   E_b on plane p0            : wE[n] = -sgn S ie h_aux^{n+1/2}[m0-1]      */
+/*   H_c on plane p0-1 (dir +1) : wH[n] = -sgn S im e_aux^{n+1}[m0]          */
+/*   H_c on plane p0   (dir -1) : wH[n] = +sgn S im e_aux^{n+1}[m0]          */
+/* (for dir = -1 the aux axis is the mirror image; mirroring flips h).       */
+/* Returns the H component (3 + c) and writes *h_plane_offset = -1 or 0.     */
+/* ------------------------------------------------------------------------ */
+int orc_tfsf_plane(double S, double eps_r, double mu_r, int axis, int pol, int dir,
+                   int n_steps, const double *base, double *wE, double *wH, int *h_plane_offset)
+{
+    if (axis < 0 || axis > 2 || pol < 0 || pol > 2 || pol == axis || (dir != 1 && dir != -1)) return -1;
+    const int a = axis, b = pol, c = 3 - a - b;
+    const double sgn = (a == (b + 1) % 3) ? 1.0 : -1.0;
+    const double ie = 1.0 / eps_r, im = 1.0 / mu_r;
+    const int m0 = 2, L = m0 + n_steps / 2 + 16;
+    double *e = (double *)calloc((size_t)L + 1, sizeof(double)), *h = (double *)calloc((size_t)L + 1, sizeof(double));
+    if (!e || !h) { free(e); free(h); return -2; }
+    for (int n = 0; n < n_steps; ++n) {
+        wE[n] = -sgn * S * ie * h[m0 - 1];
+        for (int m = L - 1; m >= 1; --m) e[m] += sgn * S * ie * (h[m] - h[m - 1]);
+        e[0] = base[n];
+        wH[n] = (dir > 0 ? -1.0 : 1.0) * sgn * S * im * e[m0];
+        for (int m = 0; m < L - 1; ++m) h[m] += sgn * S * im * (e[m + 1] - e[m]);
+    }
+    free(e); free(h);
+    if (h_plane_offset) *h_plane_offset = dir > 0 ? -1 : 0;
+    return 3 + c;
 }

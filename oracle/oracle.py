@@ -51,6 +51,11 @@ class _Source(C.Structure):
                 ("profile", C.c_void_p), ("waveform", C.c_void_p)]
 
 
+class _TDetector(C.Structure):
+    _fields_ = [("kind", C.c_int), ("mask", C.c_int), ("lo", C.c_int * 3), ("hi", C.c_int * 3),
+                ("stride", C.c_int), ("out", C.c_void_p)]
+
+
 class _Detector(C.Structure):
     _fields_ = [("mask", C.c_int), ("lo", C.c_int * 3), ("hi", C.c_int * 3),
                 ("n_freq", C.c_int), ("omega", C.c_void_p), ("phasor", C.c_void_p)]
@@ -90,6 +95,22 @@ def _lib(tag: str):
                                    C.c_void_p, C.c_int, C.c_void_p, C.c_int,
                                    C.c_void_p, C.c_void_p, C.c_int, C.c_void_p,
                                    C.c_void_p, C.c_void_p]
+        L.orc_forward_td.restype = C.c_int
+        L.orc_forward_td.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                     C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p, C.c_int,
+                                     C.c_int, C.c_void_p, C.c_void_p]
+        L.orc_backward_td.restype = C.c_int
+        L.orc_backward_td.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                      C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p,
+                                      C.c_void_p, C.c_int, C.c_void_p,
+                                      C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_flux.restype = C.c_int
+        L.orc_flux.argtypes = [C.POINTER(_Detector), C.c_void_p, C.c_int, C.c_int, C.c_void_p]
+        L.orc_flux_vjp.restype = C.c_int
+        L.orc_flux_vjp.argtypes = [C.POINTER(_Detector), C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
+        L.orc_tfsf_plane.restype = C.c_int
+        L.orc_tfsf_plane.argtypes = [C.c_double, C.c_double, C.c_double, C.c_int, C.c_int, C.c_int, C.c_int,
+                                     C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_int)]
         L.orc_backward_tape.restype = C.c_int
         L.orc_backward_tape.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p,
                                         C.c_void_p, C.c_int, C.c_void_p, C.c_void_p,
@@ -211,6 +232,27 @@ class Oracle:
         return arr, n, keep
 
     @staticmethod
+    def tdet_shape(td, n_steps):
+        """Output shape of a time-domain detector (kind 'snapshot' | 'energy', component_mask, lo, hi, stride)."""
+        n_rec = n_steps // td.stride
+        if td.kind == "energy":
+            return (n_rec,)
+        ncomp = bin(int(td.component_mask) & 63).count("1")
+        return (n_rec, ncomp, td.hi[2] - td.lo[2], td.hi[1] - td.lo[1], td.hi[0] - td.lo[0])
+
+    def _tdetectors(self, tdets, outs):
+        n = len(tdets)
+        arr = (_TDetector * max(n, 1))()
+        for idx, (s, q) in enumerate(zip(arr, tdets)):
+            s.kind = 1 if q.kind == "energy" else 0
+            s.mask = int(q.component_mask)
+            s.lo[:] = list(q.lo)
+            s.hi[:] = list(q.hi)
+            s.stride = int(q.stride)
+            s.out = None if outs is None else outs[idx].ctypes.data
+        return arr, n
+
+    @staticmethod
     def phasor_shape(det):
         ncomp = bin(int(det.component_mask) & 63).count("1")
         bz, by, bx = (det.hi[2] - det.lo[2], det.hi[1] - det.lo[1], det.hi[0] - det.lo[0])
@@ -237,7 +279,7 @@ class Oracle:
 
     # ---- drivers ------------------------------------------------------------
     def forward(self, fields, inv_eps, inv_mu=None, sources=(), detectors=(), n_steps=0,
-                record=False, tape=False, phasors=None, reset_psi=True):
+                record=False, tape=False, phasors=None, reset_psi=True, time_detectors=()):
         """Runs n_steps in place on `fields` (dtype self.dtype, shape [6,nz,ny,nx]).
 
         Returns dict(phasors=[...], rec=array|None, tape=array|None)."""
@@ -252,13 +294,15 @@ class Oracle:
         darr, nd, k2 = self._detectors(detectors, phasors)
         rec = np.zeros((n_steps, self.record_stride()), dtype=self.dtype) if record else None
         tp = np.zeros((n_steps, 3) + self.shape, dtype=self.dtype) if tape else None
-        rc = self.L.orc_forward(self.h, _ptr(fields), _ptr(ie), _ptr(im), sarr, ns, darr, nd,
-                                int(n_steps), _ptr(rec), _ptr(tp))
+        touts = [np.zeros(self.tdet_shape(t, n_steps), dtype=self.dtype) for t in time_detectors]
+        tarr, nt = self._tdetectors(time_detectors, touts)
+        rc = self.L.orc_forward_td(self.h, _ptr(fields), _ptr(ie), _ptr(im), sarr, ns, darr, nd, tarr, nt,
+                                   int(n_steps), _ptr(rec), _ptr(tp))
         assert rc == 0, rc
-        return {"phasors": phasors, "rec": rec, "tape": tp}
+        return {"phasors": phasors, "rec": rec, "tape": tp, "time_outputs": touts}
 
     def backward(self, fields, inv_eps, inv_mu=None, sources=(), detectors=(),
-                 dL_dphasor=None, dL_dfields=None, n_steps=0, rec=None):
+                 dL_dphasor=None, dL_dfields=None, n_steps=0, rec=None, time_detectors=(), dL_dtime=None):
         """Time-reversed gradient.  `fields` (state n_steps) is overwritten by the
         reconstructed state 0 on I.  Returns (g, dL_dfields0)."""
         assert fields.dtype == self.dtype and fields.flags.c_contiguous
@@ -277,10 +321,48 @@ class Oracle:
         dLf = self.arr(dL_dfields)
         g = np.zeros(self.shape, dtype=self.dtype)
         lam0 = np.zeros((6,) + self.shape, dtype=self.dtype)
-        rc = self.L.orc_backward(self.h, _ptr(fields), _ptr(ie), _ptr(im), sarr, ns, darr, nd,
-                                 gp, _ptr(dLf), int(n_steps), _ptr(rec), _ptr(g), _ptr(lam0))
+        tarr, nt = self._tdetectors(time_detectors, None)
+        tp = None
+        if dL_dtime is not None:
+            tp = (C.c_void_p * max(nt, 1))()
+            for i, G in enumerate(dL_dtime):
+                Ga = self.arr(G)
+                keep.append(Ga)
+                tp[i] = None if Ga is None else Ga.ctypes.data
+        rc = self.L.orc_backward_td(self.h, _ptr(fields), _ptr(ie), _ptr(im), sarr, ns, darr, nd, gp,
+                                    tarr, nt, tp, _ptr(dLf), int(n_steps), _ptr(rec), _ptr(g), _ptr(lam0))
         assert rc == 0, rc
         return g, lam0
+
+    # ---- N2: flux from phasors, TFSF plane source ----------------------------
+    def flux(self, det, phasor, axis, interpolate=False):
+        """Poynting flux through the detector's plane along +axis for every frequency (reading R24)."""
+        P = self.arr(phasor)
+        darr, nd, k2 = self._detectors([det], [P])
+        out = np.zeros(len(det.omega), dtype=self.dtype)
+        rc = self.L.orc_flux(darr, _ptr(P), int(axis), int(bool(interpolate)), _ptr(out))
+        assert rc == 0, rc
+        return out
+
+    def flux_vjp(self, det, phasor, axis, interpolate, dL_dflux):
+        P = self.arr(phasor)
+        darr, nd, k2 = self._detectors([det], [P])
+        G = self.arr(dL_dflux)
+        out = np.zeros_like(P)
+        rc = self.L.orc_flux_vjp(darr, _ptr(P), int(axis), int(bool(interpolate)), _ptr(G), _ptr(out))
+        assert rc == 0, rc
+        return out
+
+    def tfsf_plane(self, courant, eps_r, mu_r, axis, pol, direction, base):
+        """Waveforms of the E patch and the H patch of a one-directional plane source (reading R25).
+        Returns (wE, wH, h_component, h_plane_offset); all fp64."""
+        base = np.ascontiguousarray(base, dtype=np.float64)
+        wE, wH = np.zeros_like(base), np.zeros_like(base)
+        off = C.c_int(0)
+        hc = self.L.orc_tfsf_plane(float(courant), float(eps_r), float(mu_r), int(axis), int(pol), int(direction),
+                                   base.size, _ptr(base), _ptr(wE), _ptr(wH), C.byref(off))
+        assert hc >= 3, hc
+        return wE, wH, hc, off.value
 
     def backward_tape(self, inv_eps, inv_mu=None, detectors=(), dL_dphasor=None,
                       dL_dfields=None, n_steps=0, tape=None):

@@ -56,6 +56,23 @@ class Detector:
 
 
 @dataclass
+class TimeDetector:
+    """Time-domain detector: fires after every `stride`-th step.
+    kind 'snapshot': the components of component_mask on the box; 'energy': the electromagnetic energy in the box."""
+    kind: str
+    lo: Tuple[int, int, int]
+    hi: Tuple[int, int, int]
+    stride: int = 1
+    component_mask: int = 0
+
+    def out_shape(self, n_steps: int):
+        n_rec = n_steps // self.stride
+        if self.kind == "energy":
+            return (n_rec,)
+        return (n_rec, bin(self.component_mask & 63).count("1"), self.hi[2] - self.lo[2], self.hi[1] - self.lo[1], self.hi[0] - self.lo[0])
+
+
+@dataclass
 class Workload:
     name: str
     nx: int

@@ -489,19 +489,23 @@ def test_c3_full_length_self_consistency(B):
 
 def test_c4_full_size_self_consistency(B):
     """configs[3] at its full 800 x 800 x 600 size (384 M cells; maximum size, 6 nc > 2^31 elements) in the
-    bench launch configuration (fused kernels, record=2), truncated to 24 steps with the source plane moved next
-    to the design box.  The oracle cannot run this size in seconds, so the checks are properties that hold at
-    any size: a directional central finite difference of the loss against <dL/d inv_eps, delta>, and the
-    reconstructed state 0 (true value 0) on the design box."""
+    bench launch configuration (fused kernels, record=2).  The oracle cannot run this size in seconds, so the
+    checks are properties that hold at any size: a directional central finite difference of the loss against
+    <dL/d inv_eps, delta>, and the reconstructed state 0 (true value 0) on the design box.
+    Default: truncated to 24 steps with the source plane moved next to the design box and the loss on the final
+    fields.  FDTD_C4_STEPS=5000 runs the config as BASELINE.json states it (source at k = 40, loss = phasor power on
+    the far plane; ~4 GPU-minutes; result recorded in profiles/r2_c4_full.md)."""
     import torch
     free, _ = torch.cuda.mem_get_info()
     if free < 100e9:
         pytest.skip("needs ~100 GB of device memory")
-    n = 24
+    n = int(os.environ.get("FDTD_C4_STEPS", "24"))
+    full = n > 1000
     w = wl.c4(n_steps=n)
     d, lo, hi = w.pml_cells, w.design_lo, w.design_hi
-    s0 = w.sources[0]
-    w.sources[0] = wl.Source(s0.component, (d, d, lo[2] - 4), (w.nx - d, w.ny - d, lo[2] - 3), s0.waveform, s0.profile)
+    if not full:
+        s0 = w.sources[0]
+        w.sources[0] = wl.Source(s0.component, (d, d, lo[2] - 4), (w.nx - d, w.ny - d, lo[2] - 3), s0.waveform, s0.profile)
     kw = w.grid_kwargs()
     kw.update(max_steps=n, record=2, grad_lo=lo, grad_hi=hi, path=B.FDTD_PATH_FUSED)
     g = B.Grid(**kw)
@@ -509,29 +513,45 @@ def test_c4_full_size_self_consistency(B):
     ie = torch.as_tensor(w.inv_eps).cuda()
     box = (slice(lo[2], hi[2]), slice(lo[1], hi[1]), slice(lo[0], hi[0]))
     f = torch.zeros((6, w.nz, w.ny, w.nx), dtype=torch.float32, device="cuda")
+    fmax = 1.0
+    if full:
+        g.forward(f, ie, None, w.sources, w.detectors, 700)
+        fmax = float(f.abs().max())                          # field scale while the pulse is inside the grid
 
     def loss_of(ie_t):
         f.zero_()
-        g.forward(f, ie_t, None, w.sources, w.detectors, n)
-        return float((f[:3].double() ** 2).sum())
+        ph = g.forward(f, ie_t, None, w.sources, w.detectors, n)
+        if full:
+            return ph, float(sum((P.double() ** 2).sum() for i, P in enumerate(ph) if i in w.loss_detectors))
+        return ph, float((f[:3].double() ** 2).sum())
 
-    L0 = loss_of(ie)
+    ph, L0 = loss_of(ie)
     assert np.isfinite(L0) and L0 > 0
-    fmax = float(f.abs().max())
-    dLf = torch.zeros_like(f)
-    dLf[:3] = 2.0 * f[:3]
-    grad, _ = g.backward(f, ie, None, w.sources, w.detectors, None, dLf, n)
+    if full:
+        dLp = [2.0 * P if i in w.loss_detectors else None for i, P in enumerate(ph)]
+        grad, _ = g.backward(f, ie, None, w.sources, w.detectors, dLp, None, n)
+    else:
+        fmax = float(f.abs().max())
+        dLf = torch.zeros_like(f)
+        dLf[:3] = 2.0 * f[:3]
+        grad, _ = g.backward(f, ie, None, w.sources, w.detectors, None, dLf, n)
+        del dLf
     torch.cuda.synchronize()
-    del dLf
     resid = max(float(f[c][box].abs().max()) for c in range(6)) / fmax
-    gen = torch.Generator(device="cuda").manual_seed(4)
     delta = torch.zeros_like(ie)
-    delta[box] = torch.randint(0, 2, delta[box].shape, generator=gen, device="cuda").float() * 2 - 1
+    if full:
+        delta[box] = torch.sign(grad[box])
+        h = 2e-4
+    else:
+        gen = torch.Generator(device="cuda").manual_seed(4)
+        delta[box] = torch.randint(0, 2, delta[box].shape, generator=gen, device="cuda").float() * 2 - 1
+        h = 2e-3
     an = float((grad.double() * delta.double()).sum())
-    h = 2e-3
-    fd = (loss_of(ie + h * delta) - loss_of(ie - h * delta)) / (2 * h)
+    fd = (loss_of(ie + h * delta)[1] - loss_of(ie - h * delta)[1]) / (2 * h)
+    info = g.info()
     g.close()
-    print("C4 full size: L", L0, "directional derivative analytic", an, "finite difference", fd, "state-0 residue", resid)
+    print("C4 full size:", n, "steps, L", L0, "directional derivative analytic", an, "finite difference", fd, "state-0 residue", resid,
+          "recorder bytes", info.recorder_bytes, "grid scratch bytes", info.scratch_bytes, "torch peak bytes", torch.cuda.max_memory_allocated())
     assert abs(fd - an) <= 2e-2 * abs(an)
     assert resid <= 1e-4
     grad[box] = 0

@@ -1,0 +1,236 @@
+"""Pins for the N2 part of the CPU oracle (Poynting-flux / energy / snapshot detectors, one-directional
+TFSF plane source).  As in test_oracle_pins.py each test checks the oracle against
+something the mathematics fixes, not against itself or the CUDA path:
+
+N2-a  flux of the exact discrete plane-wave eigenmode (P1) in closed form, with and without Yee co-location
+N2-b  flux VJP against central finite differences (the flux is a quadratic form of the phasors: exact)
+N2-c  energy of the eigenmode in closed form; energy / snapshot detectors against block-wise stepping
+N2-d  gradient of a loss on energy and snapshot outputs against central finite differences (tiny CPML grid)
+N2-e  TFSF plane source: nothing behind the interface (to rounding), every (axis, polarisation, direction);
+      backward flux <= 1e-12 of the forward flux
+"""
+import math
+
+import numpy as np
+import pytest
+
+from oracle.oracle import Oracle
+from paper_2412_12360_b200 import workloads as wl
+
+S = wl.COURANT
+
+
+def _stag(shape, comp, is_H):
+    nz, ny, nx = shape
+    off = [0.0, 0.0, 0.0]
+    if is_H:
+        off[(comp + 1) % 3] = 0.5
+        off[(comp + 2) % 3] = 0.5
+    else:
+        off[comp] = 0.5
+    x = np.arange(nx, dtype=np.float64)[None, None, :] + off[0]
+    y = np.arange(ny, dtype=np.float64)[None, :, None] + off[1]
+    z = np.arange(nz, dtype=np.float64)[:, None, None] + off[2]
+    return x, y, z
+
+
+def _eigenmode(dims, mvec, M, pol_seed):
+    """Exact plane-wave eigenmode of the leapfrog (pin P1) whose frequency is exactly 2 pi / M: the permittivity is
+    chosen so that sin^2(w/2) = (S^2/eps) sum sin^2(k_a/2) holds with w = 2 pi / M."""
+    nx, ny, nz = dims
+    shape = (nz, ny, nx)
+    k = np.array([2 * math.pi * mvec[0] / nx, 2 * math.pi * mvec[1] / ny, 2 * math.pi * mvec[2] / nz])
+    w = 2.0 * math.pi / M
+    eps_r = S * S * np.sum(np.sin(k / 2.0) ** 2) / math.sin(w / 2.0) ** 2
+    assert eps_r > 1.0
+    K = 2.0 * np.sin(k / 2.0)
+    r = np.random.default_rng(pol_seed).standard_normal(3)
+    A = r - K * (r @ K) / (K @ K)
+    Bv = S * np.cross(K, A) / (2.0 * math.sin(w / 2.0))
+
+    def state(n):
+        f = np.zeros((6,) + shape)
+        for c in range(3):
+            x, y, z = _stag(shape, c, False)
+            f[c] = A[c] * np.cos(k[0] * x + k[1] * y + k[2] * z - w * n)
+            x, y, z = _stag(shape, c, True)
+            f[3 + c] = Bv[c] * np.cos(k[0] * x + k[1] * y + k[2] * z - w * (n + 0.5))
+        return f
+
+    return shape, k, w, eps_r, A, Bv, state
+
+
+# ----------------------------------------------------------------------------- N2-a
+@pytest.mark.parametrize("dims,mvec,axis,M", [((16, 12, 8), (0, 0, 1), 2, 16), ((16, 12, 8), (1, 0, 1), 2, 16),
+                                              ((16, 12, 8), (2, 1, 0), 0, 16), ((10, 12, 8), (1, 2, -1), 1, 12)])
+def test_n2a_flux_of_the_exact_plane_wave(dims, mvec, axis, M):
+    """For E_c = A_c cos(k.r - w t), H_c = B_c cos(k.r_H - w (t + 1/2)) and a run over whole periods (w N = 2 pi q), the
+    DFT phasors are (N/2) A e^{-i theta_E} and (N/2) B e^{-i (theta_H - w/2)} exactly, hence per plane cell
+      co-located : 1/2 Re(E_b conj H~_c - E_c conj H~_b) = (N/2)^2 cos(k_a/2) (A_b B_c - A_c B_b) / 2
+      raw        :                                         (N/2)^2 cos((k_a - w)/2) (A_b B_c - A_c B_b) / 2
+    (E_b and H_c share their in-plane position on the Yee grid; they differ by half a cell along a and half a step)."""
+    q = 3
+    shape, k, w, eps_r, A, Bv, state = _eigenmode(dims, mvec, M, pol_seed=axis)
+    nx, ny, nz = dims
+    N = M * q
+    a, b, c = axis, (axis + 1) % 3, (axis + 2) % 3
+    p = 5
+    for interpolate in (True, False):
+        lo, hi = [0, 0, 0], [nx, ny, nz]
+        lo[a], hi[a] = (p - 1 if interpolate else p), p + 1
+        det = wl.Detector((1 << b) | (1 << c) | (1 << (3 + b)) | (1 << (3 + c)), tuple(lo), tuple(hi), [w])
+        det.omega = [w]                                       # exact (the dataclass rounds omega to fp32 for the GPU's sake)
+        o = Oracle(nx, ny, nz, S, periodic=True)
+        f = state(0)
+        out = o.forward(f, np.full(shape, 1.0 / eps_r), detectors=[det], n_steps=N)
+        assert np.max(np.abs(f - state(N))) < 1e-11            # still the eigenmode (P1)
+        flux = o.flux(det, out["phasors"][0], a, interpolate)
+        cells = nx * ny * nz // dims[a]
+        geom = math.cos(k[a] / 2.0) if interpolate else math.cos((k[a] - w) / 2.0)
+        want = cells * (N / 2.0) ** 2 * 0.5 * geom * (A[b] * Bv[c] - A[c] * Bv[b])
+        assert abs(want) > 1.0
+        assert abs(flux[0] - want) < 1e-10 * abs(want), (interpolate, flux[0], want)
+    # sanity of the sign convention: the flux along +a has the sign of k_a (the wave travels along +k)
+    assert np.sign(want) == np.sign(k[a])
+
+
+# ----------------------------------------------------------------------------- N2-b
+@pytest.mark.parametrize("interpolate", [False, True])
+def test_n2b_flux_vjp_against_finite_differences(interpolate):
+    rng = np.random.default_rng(12)
+    a = 1
+    lo, hi = (2, 3 if interpolate else 4, 1), (7, 5, 5)
+    det = wl.Detector(0b111101, lo, hi, [0.31, 0.47])         # Ex, Ez, Hx, Hy, Hz (and the unused Hy): tangential to y = Ex, Ez, Hx, Hz
+    o = Oracle(12, 10, 8, S, periodic=True)
+    P = rng.standard_normal(det.phasor_shape)
+    G = rng.standard_normal(2)
+    vjp = o.flux_vjp(det, P, a, interpolate, G)
+    assert vjp.shape == P.shape
+    h = 1e-5
+    idx = [tuple(rng.integers(0, s) for s in P.shape) for _ in range(40)]
+    for t in idx:
+        Pp, Pm = P.copy(), P.copy()
+        Pp[t] += h
+        Pm[t] -= h
+        fd = float(G @ (o.flux(det, Pp, a, interpolate) - o.flux(det, Pm, a, interpolate))) / (2 * h)
+        assert abs(fd - vjp[t]) < 1e-8 * max(1.0, abs(fd)), (t, fd, vjp[t])
+    # components that do not enter the flux (the normal ones; E on the lower plane when co-locating) get no cotangent
+    comps = [c for c in range(6) if (det.component_mask >> c) & 1]
+    assert np.all(vjp[:, comps.index(4)] == 0)                # Hy is normal to the plane
+    if interpolate:
+        assert np.all(vjp[:, comps.index(0), :, 0] == 0) and np.any(vjp[:, comps.index(3), :, 0] != 0)
+
+
+# ----------------------------------------------------------------------------- N2-c
+def test_n2c_energy_of_the_eigenmode_and_blockwise_consistency():
+    """Energy detector: for the plane-wave eigenmode the sum of cos^2 over whole spatial periods is cells/2 for every
+    component at every time, so U = (cells/4) (eps |A|^2 + |B|^2) exactly.  Snapshot detector: equals the state reached
+    by stepping in blocks."""
+    dims, mvec = (16, 12, 8), (1, 0, 1)
+    shape, k, w, eps_r, A, Bv, state = _eigenmode(dims, mvec, 16, pol_seed=7)
+    nx, ny, nz = dims
+    ie = np.full(shape, 1.0 / eps_r)
+    td = [wl.TimeDetector("energy", (0, 0, 0), (nx, ny, nz), stride=1),
+          wl.TimeDetector("snapshot", (3, 2, 1), (9, 7, 6), stride=5, component_mask=0b100110)]
+    o = Oracle(nx, ny, nz, S, periodic=True)
+    f = state(0)
+    out = o.forward(f, ie, n_steps=23, time_detectors=td)
+    U, snap = out["time_outputs"]
+    want = nx * ny * nz / 4.0 * (eps_r * (A @ A) + Bv @ Bv)
+    assert U.shape == (23,) and np.max(np.abs(U - want)) < 1e-11 * want
+    assert snap.shape == (4, 3, 5, 5, 6)
+    g = state(0)
+    for q in range(4):
+        o.forward(g, ie, n_steps=5)
+        for ci, c in enumerate((1, 2, 5)):
+            assert np.array_equal(snap[q, ci], g[c, 1:6, 2:7, 3:9])
+
+
+# ----------------------------------------------------------------------------- N2-d
+def test_n2d_gradient_through_energy_and_snapshot_detectors():
+    """Loss = sum_q a_q U_q + sum W snapshot^2 on the tiny CPML grid (every term: kappa, alpha, inv_mu, E and H sources):
+    the time-reversed gradient -- transposed detectors injected into the cotangents, plus the explicit dependence of the
+    energy on inv_eps -- against central finite differences of the loss with respect to single inv_eps voxels."""
+    w = wl.tiny_pml(n_steps=30)
+    d = w.pml_cells
+    shape = (w.nz, w.ny, w.nx)
+    ie = w.inv_eps.astype(np.float64)
+    td = [wl.TimeDetector("energy", (d, d, d), (w.nx - d, w.ny - d, w.nz - d), stride=3),
+          wl.TimeDetector("snapshot", (d + 1, d, d + 1), (w.nx - d, w.ny - d - 1, w.nz - d), stride=4, component_mask=0b011011)]
+    rng = np.random.default_rng(5)
+    aq = rng.standard_normal(td[0].out_shape(w.n_steps))
+    Wq = rng.standard_normal(td[1].out_shape(w.n_steps))
+
+    def loss(ie_, want_grad=False):
+        o = Oracle(**w.grid_kwargs())
+        f = np.zeros((6,) + shape)
+        out = o.forward(f, ie_, w.meta["inv_mu"], w.sources, [], w.n_steps, record=want_grad, time_detectors=td)
+        U, snap = out["time_outputs"]
+        L = float(aq @ U + np.sum(Wq * snap * snap))
+        if not want_grad:
+            return L
+        g, _ = o.backward(f, ie_, w.meta["inv_mu"], w.sources, [], None, None, w.n_steps, out["rec"],
+                          time_detectors=td, dL_dtime=[aq, 2.0 * Wq * snap])
+        return L, g
+
+    L, g = loss(ie, True)
+    scale = np.max(np.abs(g))
+    assert scale > 0
+    h = 1e-6
+    for v in [(w.nz // 2, w.ny // 2, w.nx // 2), (d, d, d), (w.nz - d - 1, w.ny - d - 1, w.nx - d - 1), (d + 1, d + 2, d + 3)]:
+        ip, im_ = ie.copy(), ie.copy()
+        ip[v] += h
+        im_[v] -= h
+        fd = (loss(ip) - loss(im_)) / (2 * h)
+        assert abs(fd - g[v]) < 2e-6 * scale + 1e-6 * abs(fd), (v, fd, g[v])
+
+
+# ----------------------------------------------------------------------------- N2-e
+@pytest.mark.parametrize("axis,pol", [(0, 1), (0, 2), (1, 0), (1, 2), (2, 0), (2, 1)])
+@pytest.mark.parametrize("direction", [1, -1])
+def test_n2e_tfsf_plane_source_is_one_directional(axis, pol, direction):
+    """The E patch + H patch pair launches a plane wave to one side only: in a periodic uniform box the field behind
+    the interface stays at rounding level while the wave in front has the source's amplitude, and the DFT flux behind
+    is <= 1e-12 of the flux in front.  (Run shorter than the numerical domain of dependence needs to wrap around.)"""
+    n_long, n_steps, p0 = 96, 70, 48
+    dims = [6, 5, 4]
+    dims[axis] = n_long
+    nx, ny, nz = dims
+    shape = (nz, ny, nx)
+    eps_r, mu_r = 2.25, 1.0
+    ppw = 14.0
+    base = wl.gaussian_sine(n_steps, 24, 7, ppw).astype(np.float64)
+    o = Oracle(nx, ny, nz, S, periodic=True)
+    wE, wH, hcomp, hoff = o.tfsf_plane(S, eps_r, mu_r, axis, pol, direction, base)
+    lo, hi = [0, 0, 0], [nx, ny, nz]
+    lo[axis], hi[axis] = p0, p0 + 1
+    srcE = wl.Source(pol, tuple(lo), tuple(hi), wE)
+    lo[axis], hi[axis] = p0 + hoff, p0 + hoff + 1
+    srcH = wl.Source(hcomp, tuple(lo), tuple(hi), wH)
+    b, c = (axis + 1) % 3, (axis + 2) % 3
+    mask = (1 << b) | (1 << c) | (1 << (3 + b)) | (1 << (3 + c))
+    om = wl.omega_ppw(ppw)
+
+    def plane_det(p):
+        lo, hi = [0, 0, 0], [nx, ny, nz]
+        lo[axis], hi[axis] = p - 1, p + 1
+        return wl.Detector(mask, tuple(lo), tuple(hi), [om])
+
+    dets = [plane_det(p0 + 12 * direction), plane_det(p0 - 12 * direction)]       # in front / behind
+    f = np.zeros((6,) + shape)
+    out = o.forward(f, np.full(shape, 1.0 / eps_r), None, [srcE, srcH], dets, n_steps)
+    ax_np = 3 - axis                                           # numpy axis of `axis` in [c, z, y, x]
+    idx = np.arange(n_long)
+    behind_E = idx < p0 if direction > 0 else idx > p0
+    behind_H = idx < p0 if direction > 0 else idx >= p0
+    front = np.max(np.abs(np.compress(~behind_E, f[:3], axis=ax_np)))
+    assert front > 0.2 * np.max(np.abs(base))
+    assert np.max(np.abs(np.compress(behind_E, f[:3], axis=ax_np))) < 1e-13 * front
+    assert np.max(np.abs(np.compress(behind_H, f[3:], axis=ax_np))) < 1e-13 * front
+    fl_front = o.flux(dets[0], out["phasors"][0], axis, True)[0]
+    fl_back = o.flux(dets[1], out["phasors"][1], axis, True)[0]
+    assert fl_front * direction > 0                            # energy flows the way the wave travels
+    assert abs(fl_back) <= 1e-12 * abs(fl_front)
+    # only the polarisation asked for (and its H partner) is excited
+    others = [q for q in range(6) if q not in (pol, hcomp)]
+    assert np.max(np.abs(f[others])) == 0.0
