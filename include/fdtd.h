@@ -189,6 +189,73 @@ FDTD_API int fdtd_backward(fdtd_grid *grid, float *fields, const float *inv_eps,
 FDTD_API int fdtd_grad_rho(fdtd_grid *grid, const float *dL_dinv_eps, const float *inv_eps, float delta_eps,
                            const int32_t lo[3], const int32_t hi[3], float *dL_drho, void *cuda_stream);
 
+/* ------------------------------------------------------------------------------------------
+ * N2 -- the paper's source / detector set beyond the running DFT.
+ *
+ * Time-domain detectors ("access to intermediate fields, energy, Poynting flux"; L70: the six
+ * components are taken at the same index, no Yee co-location, the paper's default; reading R23).
+ * A detector fires after step n when (n+1) % stride == 0, record index q = (n+1)/stride - 1, on the state
+ * (E^{n+1}, H^{n+3/2}) -- the time stamp of the DFT detectors:
+ *   FDTD_TD_SNAPSHOT: out[q][ci][cell] = F_c[cell] for every component c of component_mask (ci counts the set bits);
+ *   FDTD_TD_ENERGY  : out[q] = sum_cells 1/2 (sum_c E_c^2 / inv_eps + H_c^2 / inv_mu)   (eta0-normalised H).
+ * out: DEVICE, snapshot [n_steps/stride][n_comp][box cells ordered k,j,i], energy [n_steps/stride]; written, not
+ * accumulated.  In fdtd_backward_td the matching cotangent dL/d out has the same layout; the energy detector's
+ * transpose reads the reconstructed primal fields, so its box must lie inside the reconstruction box (the
+ * interior I, or the gradient box with record == 2) and dL_dinv_eps must be requested; it also adds the explicit
+ * dependence on inv_eps, dL/d out[q] * (-1/2) sum_c E_c^2 / inv_eps^2, to dL_dinv_eps. */
+#define FDTD_TD_SNAPSHOT 0
+#define FDTD_TD_ENERGY   1
+typedef struct {
+    int32_t kind;              /* FDTD_TD_*                                                          */
+    int32_t component_mask;    /* snapshot: bit c set => component c; energy: ignored               */
+    int32_t lo[3], hi[3];      /* half-open box in (i,j,k), inside the grid, non-empty              */
+    int32_t stride;            /* >= 1                                                              */
+    float  *out;               /* DEVICE (see above).  Ignored by fdtd_backward_td.                 */
+} fdtd_time_detector;
+
+/* fdtd_forward / fdtd_backward with time-domain detectors (td: HOST array of n_td descriptors; dL_dtd: HOST array
+ * of n_td DEVICE pointers, the array or any entry may be NULL).  With n_td == 0 they are fdtd_forward /
+ * fdtd_backward.  Each detector adds one small kernel launch per time step. */
+FDTD_API int fdtd_forward_td(fdtd_grid *grid, float *fields, const float *inv_eps, const float *inv_mu,
+                    const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
+                    const fdtd_time_detector *td, int32_t n_td, int32_t n_steps, void *cuda_stream);
+FDTD_API int fdtd_backward_td(fdtd_grid *grid, float *fields, const float *inv_eps, const float *inv_mu,
+                     const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
+                     const float *const *dL_dphasor,
+                     const fdtd_time_detector *td, int32_t n_td, const float *const *dL_dtd,
+                     const float *dL_dfields, int32_t n_steps, float *dL_dinv_eps, float *dL_dfields0,
+                     void *cuda_stream);
+
+/* Poynting flux through a plane from the phasors of a DFT detector (Fig. 5 "fraction of
+ * Poynting flux"; L70 Yee interpolation, off by default; reading R24).  The detector box is a slab normal to
+ * `axis` a whose component_mask holds the four tangential components E_b, E_c, H_b, H_c (b = a+1, c = a+2 mod 3):
+ *   flux[f] = 1/2 sum_cells Re( E_b conj(H_c) - E_c conj(H_b) )          (normal +e_a)
+ * interpolate == 0: slab one plane thick, the phasors as accumulated (same index, same phase stamp);
+ * interpolate == 1: slab two planes thick (p-1, p along a); E from plane p, H co-located with it in space,
+ *   (H[p-1] + H[p])/2, and in time, multiplied by exp(-i omega_f / 2) (H is stamped half a step late).
+ * det: HOST descriptor (geometry, mask, n_freq, omega; its phasor field is ignored); phasor: DEVICE, laid out as
+ * fdtd_detector.phasor; flux: DEVICE [n_freq], written.  fdtd_flux_vjp writes dL_dphasor (DEVICE, same layout as
+ * phasor, zero where the flux does not depend on it) from dL_dflux (DEVICE [n_freq]); pass it to fdtd_backward.
+ * Errors: EINVAL if the mask lacks a tangential component or the slab thickness does not match. */
+FDTD_API int fdtd_flux(fdtd_grid *grid, const fdtd_detector *det, const float *phasor, int32_t axis, int32_t interpolate,
+              float *flux, void *cuda_stream);
+FDTD_API int fdtd_flux_vjp(fdtd_grid *grid, const fdtd_detector *det, const float *phasor, int32_t axis, int32_t interpolate,
+                  const float *dL_dflux, float *dL_dphasor, void *cuda_stream);
+
+/* One-directional plane source = Total-Field/Scattered-Field interface (reading R25).
+ * A plane wave travelling along `axis` a in direction dir = +1 / -1, E polarised along pol = b != a, its H along the
+ * third axis c, in a medium that is uniform (eps_r, mu_r) on the planes the interface touches.  The incident wave is
+ * generated on an auxiliary 1-D grid with the 3-D grid's own update (same S, same medium, hard source
+ * e[0] = base[n]), so it carries the grid's numerical dispersion and the field behind the interface cancels to
+ * rounding.  Outputs the waveforms of the two additive patches (fdtd_source) that realise the interface at plane p0:
+ *   E_b on plane p0, waveform wE;   H_c (component *h_component) on plane p0 + *h_plane_offset, waveform wH
+ * (total-field side = the side the wave travels to; the caller supplies the transverse profile).
+ * base, wE, wH: DEVICE, n_steps floats each; one kernel on cuda_stream, no grid needed.
+ * Errors: EINVAL for bad axis / pol / dir or n_steps > 50000 (the auxiliary grid lives in shared memory). */
+FDTD_API int fdtd_tfsf_plane(float courant, float eps_r, float mu_r, int32_t axis, int32_t pol, int32_t dir, int32_t n_steps,
+                    const float *base, float *wE, float *wH, int32_t *h_component, int32_t *h_plane_offset,
+                    void *cuda_stream);
+
 /* Frees the grid and everything it owns (synchronises the device first).  NULL is a no-op. */
 FDTD_API int fdtd_destroy(fdtd_grid *grid);
 

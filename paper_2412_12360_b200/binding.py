@@ -44,6 +44,14 @@ class fdtd_detector(C.Structure):
                 ("n_freq", C.c_int32), ("omega", C.POINTER(C.c_float)), ("phasor", C.c_void_p)]
 
 
+class fdtd_time_detector(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("component_mask", C.c_int32), ("lo", C.c_int32 * 3), ("hi", C.c_int32 * 3),
+                ("stride", C.c_int32), ("out", C.c_void_p)]
+
+
+FDTD_TD_SNAPSHOT, FDTD_TD_ENERGY = 0, 1
+
+
 class fdtd_grid_info(C.Structure):
     _fields_ = [("path", C.c_int32), ("tile_x", C.c_int32), ("tile_y", C.c_int32), ("tile_z", C.c_int32),
                 ("kernel_launches", C.c_int64), ("recorder_bytes", C.c_int64), ("scratch_bytes", C.c_int64),
@@ -61,7 +69,8 @@ class fdtd_profile(C.Structure):
 
 
 EXPORTS = ("fdtd_grad_rho", "fdtd_set_profiling", "fdtd_get_profile", "fdtd_create_grid", "fdtd_forward", "fdtd_backward", "fdtd_destroy", "fdtd_last_error",
-           "fdtd_get_info", "fdtd_version", "fdtd_forward_host", "fdtd_backward_host", "fdtd_debug_partition")
+           "fdtd_get_info", "fdtd_version", "fdtd_forward_host", "fdtd_backward_host", "fdtd_debug_partition",
+           "fdtd_forward_td", "fdtd_backward_td", "fdtd_flux", "fdtd_flux_vjp", "fdtd_tfsf_plane")
 
 
 def _load():
@@ -75,6 +84,19 @@ def _load():
     L.fdtd_create_grid.argtypes = [C.POINTER(fdtd_grid_desc), C.POINTER(vp)]
     L.fdtd_forward.restype = C.c_int
     L.fdtd_forward.argtypes = [vp, vp, vp, vp, C.POINTER(fdtd_source), i32, C.POINTER(fdtd_detector), i32, i32, vp]
+    L.fdtd_forward_td.restype = C.c_int
+    L.fdtd_forward_td.argtypes = [vp, vp, vp, vp, C.POINTER(fdtd_source), i32, C.POINTER(fdtd_detector), i32,
+                                  C.POINTER(fdtd_time_detector), i32, i32, vp]
+    L.fdtd_backward_td.restype = C.c_int
+    L.fdtd_backward_td.argtypes = [vp, vp, vp, vp, C.POINTER(fdtd_source), i32, C.POINTER(fdtd_detector), i32,
+                                   C.POINTER(vp), C.POINTER(fdtd_time_detector), i32, C.POINTER(vp), vp, i32, vp, vp, vp]
+    L.fdtd_flux.restype = C.c_int
+    L.fdtd_flux.argtypes = [vp, C.POINTER(fdtd_detector), vp, i32, i32, vp, vp]
+    L.fdtd_flux_vjp.restype = C.c_int
+    L.fdtd_flux_vjp.argtypes = [vp, C.POINTER(fdtd_detector), vp, i32, i32, vp, vp, vp]
+    L.fdtd_tfsf_plane.restype = C.c_int
+    L.fdtd_tfsf_plane.argtypes = [C.c_float, C.c_float, C.c_float, i32, i32, i32, i32, vp, vp, vp,
+                                  C.POINTER(i32), C.POINTER(i32), vp]
     L.fdtd_backward.restype = C.c_int
     L.fdtd_backward.argtypes = [vp, vp, vp, vp, C.POINTER(fdtd_source), i32, C.POINTER(fdtd_detector), i32,
                                 C.POINTER(vp), vp, i32, vp, vp, vp]
@@ -186,6 +208,32 @@ def fdtd_backward(grid, fields, inv_eps, inv_mu, src, n_src, det, n_det, dL_dpha
                             dL_dphasor, _ptr(dL_dfields), n_steps, _ptr(dL_dinv_eps), _ptr(dL_dfields0), stream))
 
 
+def fdtd_forward_td(grid, fields, inv_eps, inv_mu, src, n_src, det, n_det, td, n_td, n_steps, stream) -> None:
+    _check(_L.fdtd_forward_td(grid, _ptr(fields), _ptr(inv_eps), _ptr(inv_mu), src, n_src, det, n_det, td, n_td, n_steps, stream))
+
+
+def fdtd_backward_td(grid, fields, inv_eps, inv_mu, src, n_src, det, n_det, dL_dphasor, td, n_td, dL_dtd, dL_dfields,
+                     n_steps, dL_dinv_eps, dL_dfields0, stream) -> None:
+    _check(_L.fdtd_backward_td(grid, _ptr(fields), _ptr(inv_eps), _ptr(inv_mu), src, n_src, det, n_det, dL_dphasor,
+                               td, n_td, dL_dtd, _ptr(dL_dfields), n_steps, _ptr(dL_dinv_eps), _ptr(dL_dfields0), stream))
+
+
+def fdtd_flux(grid, det, phasor, axis, interpolate, flux, stream) -> None:
+    _check(_L.fdtd_flux(grid, det, _ptr(phasor), int(axis), int(bool(interpolate)), _ptr(flux), stream))
+
+
+def fdtd_flux_vjp(grid, det, phasor, axis, interpolate, dL_dflux, dL_dphasor, stream) -> None:
+    _check(_L.fdtd_flux_vjp(grid, det, _ptr(phasor), int(axis), int(bool(interpolate)), _ptr(dL_dflux), _ptr(dL_dphasor), stream))
+
+
+def fdtd_tfsf_plane(courant, eps_r, mu_r, axis, pol, direction, n_steps, base, wE, wH, stream):
+    """Returns (h_component, h_plane_offset); wE / wH (device, n_steps floats) are written."""
+    hc, off = C.c_int32(0), C.c_int32(0)
+    _check(_L.fdtd_tfsf_plane(float(courant), float(eps_r), float(mu_r), int(axis), int(pol), int(direction), int(n_steps),
+                              _ptr(base), _ptr(wE), _ptr(wH), C.byref(hc), C.byref(off), stream))
+    return hc.value, off.value
+
+
 def fdtd_forward_host(grid, h_fields, h_inv_eps, h_inv_mu, src, n_src, det, n_det, n_steps, stream) -> None:
     _check(_L.fdtd_forward_host(grid, _ptr(h_fields), _ptr(h_inv_eps), _ptr(h_inv_mu), src, n_src, det, n_det,
                                 n_steps, stream))
@@ -284,23 +332,62 @@ class Grid:
             s.phasor = None if phasors is None else _ptr(phasors[idx])
         return arr, n, keep
 
+    def marshal_time_detectors(self, tdets, outs):
+        n = len(tdets)
+        arr = (fdtd_time_detector * max(n, 1))()
+        for idx, (s, q) in enumerate(zip(arr, tdets)):
+            s.kind = FDTD_TD_ENERGY if q.kind == "energy" else FDTD_TD_SNAPSHOT
+            s.component_mask = int(q.component_mask)
+            s.lo[:] = list(q.lo)
+            s.hi[:] = list(q.hi)
+            s.stride = int(q.stride)
+            s.out = None if outs is None else _ptr(outs[idx])
+        return arr, n
+
     def stream(self):
         return C.c_void_p(self.torch.cuda.current_stream().cuda_stream)
 
+    # -- N2: flux from phasors, TFSF plane source ------------------------------------------------
+    def flux(self, det, phasor, axis, interpolate=False):
+        darr, nd, k = self.marshal_detectors([det], None)
+        out = self.torch.empty(len(det.omega), dtype=self.torch.float32, device="cuda")
+        fdtd_flux(self.h, darr, phasor, axis, interpolate, out, self.stream())
+        return out
+
+    def flux_vjp(self, det, phasor, axis, interpolate, dL_dflux):
+        darr, nd, k = self.marshal_detectors([det], None)
+        out = self.torch.empty_like(phasor)
+        fdtd_flux_vjp(self.h, darr, phasor, axis, interpolate, self._dev(dL_dflux), out, self.stream())
+        return out
+
+    def tfsf_plane(self, eps_r, mu_r, axis, pol, direction, base):
+        """(wE, wH, h_component, h_plane_offset) of a one-directional plane source; wE / wH are cuda tensors."""
+        b = self._dev(base)
+        wE, wH = self.torch.empty_like(b), self.torch.empty_like(b)
+        hc, off = fdtd_tfsf_plane(self.desc.courant, eps_r, mu_r, axis, pol, direction, b.numel(), b, wE, wH, self.stream())
+        return wE, wH, hc, off
+
     # -- device entry points ---------------------------------------------------------------------
-    def forward(self, fields, inv_eps, inv_mu=None, sources=(), detectors=(), n_steps=0, phasors=None):
-        """fields: cuda float32 [6,nz,ny,nx], updated in place.  Returns the phasor tensors."""
+    def forward(self, fields, inv_eps, inv_mu=None, sources=(), detectors=(), n_steps=0, phasors=None, time_detectors=()):
+        """fields: cuda float32 [6,nz,ny,nx], updated in place.  Returns the phasor tensors; the outputs of the
+        time-domain detectors are left in self.time_outputs."""
         torch = self.torch
         if phasors is None:
             phasors = [torch.zeros(d.phasor_shape, dtype=torch.float32, device="cuda") for d in detectors]
         sarr, ns, k1 = self.marshal_sources(sources)
         darr, nd, k2 = self.marshal_detectors(detectors, phasors)
-        fdtd_forward(self.h, fields, inv_eps, inv_mu, sarr, ns, darr, nd, int(n_steps), self.stream())
+        if time_detectors:
+            self.time_outputs = [torch.zeros(t.out_shape(int(n_steps)), dtype=torch.float32, device="cuda") for t in time_detectors]
+            tarr, nt = self.marshal_time_detectors(time_detectors, self.time_outputs)
+            fdtd_forward_td(self.h, fields, inv_eps, inv_mu, sarr, ns, darr, nd, tarr, nt, int(n_steps), self.stream())
+        else:
+            self.time_outputs = []
+            fdtd_forward(self.h, fields, inv_eps, inv_mu, sarr, ns, darr, nd, int(n_steps), self.stream())
         self._keep = [k1, k2, sarr, darr]
         return phasors
 
     def backward(self, fields, inv_eps, inv_mu=None, sources=(), detectors=(), dL_dphasor=None,
-                 dL_dfields=None, n_steps=0, want_dL_dfields0=False, out=None, want_grad=True):
+                 dL_dfields=None, n_steps=0, want_dL_dfields0=False, out=None, want_grad=True, time_detectors=(), dL_dtime=None):
         """want_grad=False: adjoint sweep only (dL_dinv_eps = NULL): returns (None, cotangent of state 0)."""
         torch = self.torch
         sarr, ns, k1 = self.marshal_sources(sources)
@@ -312,7 +399,15 @@ class Grid:
                 cot[i] = _ptr(G)
         g = None if not want_grad else (out if out is not None else torch.empty(self.shape, dtype=torch.float32, device="cuda"))
         lam0 = torch.empty((6,) + self.shape, dtype=torch.float32, device="cuda") if (want_dL_dfields0 or not want_grad) else None
-        fdtd_backward(self.h, fields, inv_eps, inv_mu, sarr, ns, darr, nd, cot, dL_dfields, int(n_steps),
-                      g, lam0, self.stream())
-        self._keep = [k1, k2, sarr, darr, cot, dL_dphasor]
+        if time_detectors:
+            tarr, nt = self.marshal_time_detectors(time_detectors, None)
+            tcot = (C.c_void_p * max(nt, 1))()
+            for i, G in enumerate(dL_dtime or []):
+                tcot[i] = _ptr(G)
+            fdtd_backward_td(self.h, fields, inv_eps, inv_mu, sarr, ns, darr, nd, cot, tarr, nt, tcot, dL_dfields,
+                             int(n_steps), g, lam0, self.stream())
+        else:
+            fdtd_backward(self.h, fields, inv_eps, inv_mu, sarr, ns, darr, nd, cot, dL_dfields, int(n_steps),
+                          g, lam0, self.stream())
+        self._keep = [k1, k2, sarr, darr, cot, dL_dphasor, dL_dtime]
         return g, lam0

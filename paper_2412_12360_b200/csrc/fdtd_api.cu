@@ -237,6 +237,8 @@ extern "C" int fdtd_create_grid(const fdtd_grid_desc *desc, fdtd_grid **out)
         g->h_tables = h;
     }
     if ((rc = g->alloc((void **)&g->d_step, 64))) return bail(rc);
+    if ((rc = g->alloc((void **)&g->red.partial, RED_BLOCKS * sizeof(double))) || (rc = g->alloc((void **)&g->red.ticket, 64))) return bail(rc);
+    if (cudaMemset(g->red.ticket, 0, 64) != cudaSuccess) return bail(cuda_fail(cudaGetLastError(), "cudaMemset"));
     if ((rc = g->alloc_psi(g->psiE[0])) || (rc = g->alloc_psi(g->psiH[0]))) return bail(rc);
     if (desc->record && G.d > 0 && desc->max_steps > 0) {
         const size_t bytes = (size_t)g->R.stride * sizeof(float) * (size_t)desc->max_steps;
@@ -421,6 +423,28 @@ int translate(const fdtd_detector *det, int n_det, std::vector<DetectorDev> &out
     return tot;
 }
 
+int translate_td(fdtd_grid *g, const fdtd_time_detector *td, int n_td, int n_steps, std::vector<TimeDetDev> &out, const char *who)
+{
+    out.clear();
+    if (n_td < 0 || (n_td && !td)) return fail(FDTD_EINVAL, std::string(who) + ": bad time-detector array");
+    out.resize(n_td);
+    for (int s = 0; s < n_td; ++s) {
+        if (td[s].kind != FDTD_TD_SNAPSHOT && td[s].kind != FDTD_TD_ENERGY) return fail(FDTD_EINVAL, "time detector kind must be FDTD_TD_SNAPSHOT or FDTD_TD_ENERGY");
+        if (td[s].kind == FDTD_TD_SNAPSHOT && (td[s].component_mask <= 0 || td[s].component_mask > 63))
+            return fail(FDTD_EINVAL, "snapshot detector component_mask must be 1..63");
+        if (!box_ok(g->G, td[s].lo, td[s].hi)) return fail(FDTD_EINVAL, "time detector box outside the grid or empty");
+        if (td[s].stride < 1) return fail(FDTD_EINVAL, "time detector stride must be >= 1");
+        out[s].kind = td[s].kind;
+        out[s].mask = td[s].kind == FDTD_TD_SNAPSHOT ? td[s].component_mask : 0;
+        out[s].ncomp = popcount6(out[s].mask);
+        for (int a = 0; a < 3; ++a) { out[s].lo[a] = td[s].lo[a]; out[s].hi[a] = td[s].hi[a]; }
+        out[s].stride = td[s].stride;
+        out[s].out = td[s].out;
+    }
+    (void)n_steps;
+    return FDTD_OK;
+}
+
 }  // namespace
 
 // device + pinned host capacity of the (cos, sin) table; earlier uploads have to be finished before the old buffers go
@@ -550,6 +574,13 @@ extern "C" int fdtd_forward(fdtd_grid *g, float *fields, const float *inv_eps, c
                             const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
                             int32_t n_steps, void *cuda_stream)
 {
+    return fdtd_forward_td(g, fields, inv_eps, inv_mu, src, n_src, det, n_det, nullptr, 0, n_steps, cuda_stream);
+}
+
+extern "C" int fdtd_forward_td(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
+                               const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
+                               const fdtd_time_detector *td, int32_t n_td, int32_t n_steps, void *cuda_stream)
+{
     int rc = check_common(g, fields, inv_eps, src, n_src, det, n_det, n_steps, "fdtd_forward");
     if (rc) return rc;
     for (int s = 0; s < n_det; ++s)
@@ -558,6 +589,9 @@ extern "C" int fdtd_forward(fdtd_grid *g, float *fields, const float *inv_eps, c
     const Dims &G = g->G;
     std::vector<SourceDev> S;
     std::vector<DetectorDev> D;
+    std::vector<TimeDetDev> TD;
+    if ((rc = translate_td(g, td, n_td, n_steps, TD, "fdtd_forward_td"))) return rc;
+    for (const TimeDetDev &q : TD) if (!q.out) return fail(FDTD_EINVAL, "fdtd_forward_td: time detector out is NULL");
     translate(src, n_src, S);
     const int total_freq = translate(det, n_det, D);
     const bool recording = g->desc.record && G.d > 0;
@@ -571,12 +605,13 @@ extern "C" int fdtd_forward(fdtd_grid *g, float *fields, const float *inv_eps, c
     if (g->path == FDTD_PATH_FUSED && !fused_call && g->desc.path == FDTD_PATH_FUSED)
         return fail(FDTD_EINVAL, "FDTD_PATH_FUSED takes at most 4 sources and 4 detectors per call (FDTD_PATH_AUTO falls back to the generic kernels)");
     if (fused_call) {
-        rc = fused_forward(g, fields, inv_eps, inv_mu, S, D, total_freq, n_steps, recording, st);
+        rc = fused_forward(g, fields, inv_eps, inv_mu, S, D, TD, total_freq, n_steps, recording, st);
         if (rc) return rc;
     } else {
         if ((rc = g->zero_psi(g->psiE[0], st)) || (rc = g->zero_psi(g->psiH[0], st))) return rc;
-        const int launches = 3 + n_src + n_det + (recording ? 1 : 0);
-        const std::string key = make_key("gf", fields, inv_eps, inv_mu, g->rec, g->d_cs, S, D, recording);
+        const int launches = 3 + n_src + n_det + n_td + (recording ? 1 : 0);
+        std::string key = make_key("gf", fields, inv_eps, inv_mu, g->rec, g->d_cs, S, D, recording);
+        if (!TD.empty()) key.append((const char *)TD.data(), TD.size() * sizeof(TimeDetDev));
         rc = run_steps(g, g->fwd_graph, key, n_steps, launches, st, [&](cudaStream_t cs) {
             { ProfScope p(g, fdtd_grid::PC_UPDATE_E, cs); launch_update_E(G, g->T, fields, inv_eps, g->psiE[0], cs); }
             { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
@@ -585,7 +620,8 @@ extern "C" int fdtd_forward(fdtd_grid *g, float *fields, const float *inv_eps, c
             { ProfScope p(g, fdtd_grid::PC_UPDATE_H, cs); launch_update_H(G, g->T, fields, inv_mu, g->psiH[0], cs); }
             { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
               for (const SourceDev &s : S) if (s.comp >= 3) launch_add_source(G, fields, s, g->step_in(), 1.f, cs);
-              for (const DetectorDev &dt : D) launch_detector(G, fields, dt, g->d_cs, total_freq, g->step_in(), cs); }
+              for (const DetectorDev &dt : D) launch_detector(G, fields, dt, g->d_cs, total_freq, g->step_in(), cs);
+              for (const TimeDetDev &q : TD) launch_time_detect(G, fields, nullptr, 0, inv_eps, inv_mu, q, g->red, g->step_in(), cs); }
             { ProfScope p(g, fdtd_grid::PC_OTHER, cs); launch_next_step(g->step_in(), g->step_out(), 1, cs); }
         });
         if (rc) return rc;
@@ -614,6 +650,17 @@ extern "C" int fdtd_backward(fdtd_grid *g, float *fields, const float *inv_eps, 
                              const float *const *dL_dphasor, const float *dL_dfields,
                              int32_t n_steps, float *dL_dinv_eps, float *dL_dfields0, void *cuda_stream)
 {
+    return fdtd_backward_td(g, fields, inv_eps, inv_mu, src, n_src, det, n_det, dL_dphasor, nullptr, 0, nullptr, dL_dfields,
+                            n_steps, dL_dinv_eps, dL_dfields0, cuda_stream);
+}
+
+extern "C" int fdtd_backward_td(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
+                                const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
+                                const float *const *dL_dphasor,
+                                const fdtd_time_detector *td, int32_t n_td, const float *const *dL_dtd,
+                                const float *dL_dfields, int32_t n_steps, float *dL_dinv_eps, float *dL_dfields0,
+                                void *cuda_stream)
+{
     int rc = check_common(g, fields, inv_eps, src, n_src, det, n_det, n_steps, "fdtd_backward");
     if (rc) return rc;
     if (!dL_dinv_eps && !dL_dfields0) return fail(FDTD_EINVAL, "fdtd_backward: dL_dinv_eps or dL_dfields0 is required");
@@ -623,6 +670,20 @@ extern "C" int fdtd_backward(fdtd_grid *g, float *fields, const float *inv_eps, 
     cudaStream_t st = (cudaStream_t)cuda_stream;
     std::vector<SourceDev> S;
     std::vector<DetectorDev> D;
+    // time-domain detectors: only those with a cotangent take part; `out` carries the cotangent from here on
+    std::vector<TimeDetDev> TDall, TD;
+    if ((rc = translate_td(g, td, n_td, n_steps, TDall, "fdtd_backward_td"))) return rc;
+    for (int s = 0; s < n_td; ++s) {
+        if (!dL_dtd || !dL_dtd[s]) continue;
+        TimeDetDev q = TDall[s];
+        q.out = const_cast<float *>(dL_dtd[s]);
+        if (q.kind == FDTD_TD_ENERGY) {
+            if (!dL_dinv_eps) return fail(FDTD_EINVAL, "fdtd_backward_td: the energy detector's transpose needs the reconstructed fields (request dL_dinv_eps)");
+            for (int a = 0; a < 3; ++a)
+                if (q.lo[a] < G.lo[a] || q.hi[a] > G.hi[a]) return fail(FDTD_EINVAL, "fdtd_backward_td: energy detector box outside the reconstruction box");
+        }
+        TD.push_back(q);
+    }
     translate(src, n_src, S);
     const int total_freq = translate(det, n_det, D);
     for (int s = 0; s < n_det; ++s)
@@ -642,18 +703,22 @@ extern "C" int fdtd_backward(fdtd_grid *g, float *fields, const float *inv_eps, 
 
     if (g->path == FDTD_PATH_FUSED && g->fused_backward_ready) {
         // seeded_H: the H part of the seed can be non-zero (it is scaled by inv_mu for the sweep)
-        rc = fused_backward(g, fields, inv_eps, inv_mu, S, D, total_freq, n_steps, dL_dinv_eps, dL_dfields != nullptr, st);
+        rc = fused_backward(g, fields, inv_eps, inv_mu, S, D, TD, total_freq, n_steps, dL_dinv_eps, dL_dfields != nullptr, st);
         if (rc) return rc;
         // the fused sweep carried im lamH in the H part (kernels_step.cu); the cotangent of state 0 is lamH
         if (inv_mu && dL_dfields0) launch_scale_H(G, g->lam, inv_mu, true, st);
     } else {
         int n_adj = 0;
         for (const DetectorDev &dt : D) if (dt.phasor) ++n_adj;
-        const int launches = want_grad ? 5 + n_adj + n_src + (G.d > 0 ? 1 : 0) : 3 + n_adj;
+        const int launches = (want_grad ? 5 + n_adj + n_src + (G.d > 0 ? 1 : 0) : 3 + n_adj) + (int)TD.size();
         std::string key = make_key("gb", fields, inv_eps, inv_mu, g->rec, dL_dinv_eps, S, D, 0);
         key.append((const char *)&g->d_cs, sizeof(g->d_cs));
+        if (!TD.empty()) key.append((const char *)TD.data(), TD.size() * sizeof(TimeDetDev));
         rc = run_steps(g, g->bwd_graph, key, n_steps, launches, st, [&](cudaStream_t cs) {
             { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
+              // N2 transposes first: they act on the state after step n, before anything of reverse step n
+              for (const TimeDetDev &q : TD)
+                  launch_time_detect_adjoint(G, g->lam, nullptr, fields, nullptr, 0, inv_eps, inv_mu, false, q, dL_dinv_eps, g->step_in(), cs);
               for (const DetectorDev &dt : D) if (dt.phasor) launch_detector_adjoint(G, g->lam, dt, g->d_cs, total_freq, g->step_in(), cs); }
             { ProfScope p(g, fdtd_grid::PC_ADJ_H, cs); launch_adj_H(G, g->T, g->lam, inv_mu, g->lpsiH[0], g->lpsiH[1], g->step_in(), cs); }
             if (want_grad) {
@@ -685,6 +750,83 @@ extern "C" int fdtd_grad_rho(fdtd_grid *g, const float *dL_dinv_eps, const float
     g->kernel_launches += 1;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "fdtd_grad_rho launch");
+    return FDTD_OK;
+}
+
+// ================================================================================================
+// N2: flux from phasors, TFSF plane source (kernels_n2.cu)
+// ================================================================================================
+namespace {
+int flux_common(fdtd_grid *g, const fdtd_detector *det, const float *phasor, int axis, int interpolate, DetectorDev &dt, const char *who)
+{
+    if (!g || !det || !phasor) return fail(FDTD_EINVAL, std::string(who) + ": NULL argument");
+    if (axis < 0 || axis > 2) return fail(FDTD_EINVAL, std::string(who) + ": axis must be 0..2");
+    if (det->component_mask <= 0 || det->component_mask > 63 || !box_ok(g->G, det->lo, det->hi) || det->n_freq < 1 || !det->omega)
+        return fail(FDTD_EINVAL, std::string(who) + ": bad detector descriptor");
+    std::vector<DetectorDev> D;
+    translate(det, 1, D);
+    dt = D[0];
+    const int b = (axis + 1) % 3, c = (axis + 2) % 3;
+    const int need = (1 << b) | (1 << c) | (1 << (3 + b)) | (1 << (3 + c));
+    if ((dt.mask & need) != need) return fail(FDTD_EINVAL, std::string(who) + ": the detector lacks a tangential component of the plane");
+    if (dt.hi[axis] - dt.lo[axis] != (interpolate ? 2 : 1))
+        return fail(FDTD_EINVAL, std::string(who) + ": the box must be 1 plane thick along the axis (2 with interpolation)");
+    return FDTD_OK;
+}
+}  // namespace
+
+extern "C" int fdtd_flux(fdtd_grid *g, const fdtd_detector *det, const float *phasor, int32_t axis, int32_t interpolate,
+                         float *flux, void *cuda_stream)
+{
+    DetectorDev dt;
+    int rc = flux_common(g, det, phasor, axis, interpolate, dt, "fdtd_flux");
+    if (rc) return rc;
+    if (!flux) return fail(FDTD_EINVAL, "fdtd_flux: flux is NULL");
+    for (int f = 0; f < dt.n_freq; ++f)
+        launch_flux(dt, phasor, axis, interpolate ? 1 : 0, f, (float)std::cos(0.5 * (double)det->omega[f]),
+                    (float)std::sin(0.5 * (double)det->omega[f]), flux, g->red, (cudaStream_t)cuda_stream);
+    g->kernel_launches += dt.n_freq;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "fdtd_flux launch");
+    return FDTD_OK;
+}
+
+extern "C" int fdtd_flux_vjp(fdtd_grid *g, const fdtd_detector *det, const float *phasor, int32_t axis, int32_t interpolate,
+                             const float *dL_dflux, float *dL_dphasor, void *cuda_stream)
+{
+    DetectorDev dt;
+    int rc = flux_common(g, det, phasor, axis, interpolate, dt, "fdtd_flux_vjp");
+    if (rc) return rc;
+    if (!dL_dflux || !dL_dphasor) return fail(FDTD_EINVAL, "fdtd_flux_vjp: NULL argument");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t bytes = (size_t)dt.n_freq * dt.ncomp * (size_t)(dt.hi[0] - dt.lo[0]) * (dt.hi[1] - dt.lo[1]) * (dt.hi[2] - dt.lo[2]) * 2 * sizeof(float);
+    CK(cudaMemsetAsync(dL_dphasor, 0, bytes, st));
+    for (int f = 0; f < dt.n_freq; ++f)
+        launch_flux_vjp(dt, phasor, axis, interpolate ? 1 : 0, f, (float)std::cos(0.5 * (double)det->omega[f]),
+                        (float)std::sin(0.5 * (double)det->omega[f]), dL_dflux, dL_dphasor, st);
+    g->kernel_launches += dt.n_freq;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "fdtd_flux_vjp launch");
+    return FDTD_OK;
+}
+
+extern "C" int fdtd_tfsf_plane(float courant, float eps_r, float mu_r, int32_t axis, int32_t pol, int32_t dir, int32_t n_steps,
+                               const float *base, float *wE, float *wH, int32_t *h_component, int32_t *h_plane_offset,
+                               void *cuda_stream)
+{
+    if (axis < 0 || axis > 2 || pol < 0 || pol > 2 || pol == axis || (dir != 1 && dir != -1))
+        return fail(FDTD_EINVAL, "fdtd_tfsf_plane: need axis, pol in 0..2, pol != axis, dir = +1 or -1");
+    if (!(courant > 0.f) || !(eps_r > 0.f) || !(mu_r > 0.f)) return fail(FDTD_EINVAL, "fdtd_tfsf_plane: courant, eps_r, mu_r must be > 0");
+    if (n_steps < 0 || n_steps > 50000) return fail(FDTD_EINVAL, "fdtd_tfsf_plane: need 0 <= n_steps <= 50000");
+    if (n_steps && (!base || !wE || !wH)) return fail(FDTD_EINVAL, "fdtd_tfsf_plane: NULL argument");
+    const int c = 3 - axis - pol;
+    const float sgn = (axis == (pol + 1) % 3) ? 1.f : -1.f;
+    if (h_component) *h_component = 3 + c;
+    if (h_plane_offset) *h_plane_offset = dir > 0 ? -1 : 0;
+    if (n_steps == 0) return FDTD_OK;
+    cudaError_t e = launch_tfsf_aux(courant, 1.f / eps_r, 1.f / mu_r, sgn, dir > 0 ? 1.f : -1.f, n_steps, base, wE, wH,
+                                    (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(e, "fdtd_tfsf_plane launch");
     return FDTD_OK;
 }
 

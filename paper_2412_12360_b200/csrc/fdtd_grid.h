@@ -40,6 +40,7 @@ struct fdtd_grid {
     float *h_cs = nullptr;                 // pinned staging of the same
     size_t cs_cap = 0;
     cudaEvent_t table_done = nullptr;
+    fdtd::ReduceScratch red{};             // block partials + ticket of the N2 reductions (energy, flux)
 
     // host-buffer entry points
     float *hb_fields = nullptr, *hb_ie = nullptr, *hb_im = nullptr, *hb_grad = nullptr, *hb_cotf = nullptr;
@@ -95,10 +96,11 @@ void fused_teardown(fdtd_grid *g);
 int fused_alloc_backward(fdtd_grid *g);    // second cotangent volume of the ping-pong
 int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
                   const std::vector<fdtd::SourceDev> &S, const std::vector<fdtd::DetectorDev> &D,
-                  int total_freq, int n_steps, bool recording, cudaStream_t st);
+                  const std::vector<fdtd::TimeDetDev> &TD, int total_freq, int n_steps, bool recording, cudaStream_t st);
 int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
                    const std::vector<fdtd::SourceDev> &S, const std::vector<fdtd::DetectorDev> &D,
-                   int total_freq, int n_steps, float *dL_dinv_eps, bool seeded_H, cudaStream_t st);
+                   const std::vector<fdtd::TimeDetDev> &TD, int total_freq, int n_steps, float *dL_dinv_eps, bool seeded_H,
+                   cudaStream_t st);
 
 // RAII span: brackets the launches made in its lifetime with two events when profiling is on
 struct ProfScope {

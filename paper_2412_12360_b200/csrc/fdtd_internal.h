@@ -140,4 +140,40 @@ void launch_detector_adjoint_pp(const Dims &G, float *lamA, float *lamB, const D
 // H part of a cotangent volume: lamH *= im (inverse = false) or lamH /= im (inverse = true)
 void launch_scale_H(const Dims &G, float *lam, const float *im, bool inverse, cudaStream_t st);
 
+// ----------------------------------------------------------------------------------------------
+// N2: time-domain detectors, Poynting flux from phasors, TFSF plane source
+// -- kernels_n2.cu.  A time-domain detector fires after step n when (n+1) % stride == 0 (record index
+// (n+1)/stride - 1); the kernels read n from *step and return at once on the other steps, so the per-step launch
+// sequence stays replayable.
+// ----------------------------------------------------------------------------------------------
+struct TimeDetDev {
+    int kind;                 // 0 snapshot, 1 energy
+    int mask, ncomp;
+    int lo[3], hi[3];
+    int stride;
+    float *out;               // forward: written;  backward: cotangent (may be NULL)
+};
+struct ReduceScratch {        // block partials + ticket of the last-block-done reductions (grid owned)
+    double *partial;          // [RED_BLOCKS]
+    unsigned int *ticket;
+};
+constexpr int RED_BLOCKS = 1024;
+// volA / volB: the state after step n sits in volA, or (fused ping-pong, volB != NULL) in the volume of parity
+// (n + par_off) & 1 (0: volA)
+void launch_time_detect(const Dims &G, const float *volA, const float *volB, int par_off, const float *ie, const float *im,
+                        const TimeDetDev &td, const ReduceScratch &rs, const int *step, cudaStream_t st);
+// transpose at reverse step n: cotangent volume lamA / lamB and primal volume fA / fB picked by parity like above;
+// scaled_H: the H part of the cotangent volumes holds im lamH; g: dL/d inv_eps or NULL
+void launch_time_detect_adjoint(const Dims &G, float *lamA, float *lamB, const float *fA, const float *fB, int par_off,
+                                const float *ie, const float *im, bool scaled_H, const TimeDetDev &td, float *g,
+                                const int *step, cudaStream_t st);
+// flux_f = 1/2 sum Re(E_b conj(H_c) - E_c conj(H_b)) on the plane (reading R24); cw, sw = cos, sin(omega_f / 2)
+void launch_flux(const DetectorDev &dt, const float *phasor, int axis, int interpolate, int f, float cw, float sw,
+                 float *flux, const ReduceScratch &rs, cudaStream_t st);
+void launch_flux_vjp(const DetectorDev &dt, const float *phasor, int axis, int interpolate, int f, float cw, float sw,
+                     const float *dL_dflux, float *dL_dphasor, cudaStream_t st);
+// auxiliary 1-D leapfrog of the TFSF plane source (reading R25); returns cudaErrorInvalidValue when n_steps is too large
+cudaError_t launch_tfsf_aux(float S, float ie, float im, float sgn, float dir_sign, int n_steps, const float *base,
+                            float *wE, float *wH, cudaStream_t st);
+
 }  // namespace fdtd

@@ -1710,6 +1710,7 @@ void join_side(fdtd_grid *g, cudaStream_t cs, int n_side)
 
 struct FwdCtx {
     fdtd_grid *g; StepParams P; bool recording; float *A; float *B; int n_steps;
+    const std::vector<TimeDetDev> *TD; const float *ie; const float *im;
 };
 // forward step n; with the recorder on, k_record_pipe runs beside it on a side stream: both only read buffer n&1
 // (pre-step H of step n -> rec[n], E' of step n-1 -> rec[n-1]); the step after next overwrites that buffer, so the
@@ -1728,12 +1729,15 @@ void enqueue_fwd(void *vctx, cudaStream_t cs)
     }
     F->tile->launch_fwd(Q, F->n_cta, F->smem, cs);
     if (c->recording) join_side(g, cs, 1);
+    // N2: time-domain detectors on the state step n just wrote (volume (n+1)&1)
+    for (const TimeDetDev &q : *c->TD) launch_time_detect(g->G, c->A, c->B, 1, c->ie, c->im, q, g->red, g->step_in(), cs);
     ++g->enq_step;
 }
 
 struct BwdCtx {
     fdtd_grid *g; StepParams P; InvParams I; bool fused_inv; bool fused_det; bool pipelined; bool want_grad; float *bufB; float *fields; const float *ie; const float *im; float *grad; float *lamA; float *lamB;
     const std::vector<SourceDev> *S; const std::vector<DetectorDev> *D; int total_freq;
+    const std::vector<TimeDetDev> *TD;
 };
 // Reverse step n.  One kernel after the other: B1 (detector cotangents into the volume about to be read), B2+B5
 // (fused adjoint step), face injection, then the primal inverse step B3+B4 with lamE' taken from the volume the
@@ -1765,6 +1769,12 @@ void enqueue_bwd(void *vctx, cudaStream_t cs)
         ++g->enq_step; ++g->enq_inv;
         return;
     }
+    // N2 transposes first: they act on the state after step n (primal volume (n+1)&1 when the fused inverse step
+    // ping-pongs, else `fields`), into the cotangent volume the adjoint step is about to read ((n+1)&1)
+    if (!c->TD->empty()) { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
+      for (const TimeDetDev &q : *c->TD)
+          launch_time_detect_adjoint(G, c->lamA, c->lamB, c->fields, c->fused_inv ? c->bufB : nullptr, 1, c->ie, c->im,
+                                     c->im != nullptr, q, c->grad, g->step_in(), cs); }
     if (!c->fused_det) { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
       for (const DetectorDev &dt : *c->D)
           if (dt.phasor) launch_detector_adjoint_pp(G, c->lamA, c->lamB, dt, g->d_cs, c->total_freq, g->step_in(), c->im, cs); }
@@ -1798,8 +1808,8 @@ void enqueue_bwd(void *vctx, cudaStream_t cs)
 }  // namespace
 
 int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
-                  const std::vector<SourceDev> &S, const std::vector<DetectorDev> &D, int total_freq, int n_steps,
-                  bool recording, cudaStream_t st)
+                  const std::vector<SourceDev> &S, const std::vector<DetectorDev> &D, const std::vector<TimeDetDev> &TD,
+                  int total_freq, int n_steps, bool recording, cudaStream_t st)
 {
     FusedState *F = g->fused;
     if ((int)S.size() > MAX_SRC || (int)D.size() > MAX_DET)
@@ -1808,7 +1818,7 @@ int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float
     if (rc) return rc;
     for (int q = 0; q < 2; ++q)
         if ((rc = g->zero_psi(g->psiE[q], st)) || (rc = g->zero_psi(g->psiH[q], st))) return rc;
-    FwdCtx ctx{ g, F->sp, recording, fields, F->bufB, n_steps };
+    FwdCtx ctx{ g, F->sp, recording, fields, F->bufB, n_steps, &TD, inv_eps, inv_mu };
     StepParams &P = ctx.P;
     P.maps = F->d_maps[0];
     P.buf[0] = fields; P.buf[1] = F->bufB;
@@ -1831,7 +1841,8 @@ int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float
     key.append((const char *)&P, sizeof(P));
     key.push_back(recording ? 1 : 0);
     key.append((const char *)&n_steps, recording ? sizeof(n_steps) : 0);
-    rc = fdtd_run_steps_fwd(g, key, n_steps, 1 + (recording ? 1 : 0), st, enqueue_fwd, &ctx);
+    if (!TD.empty()) key.append((const char *)TD.data(), TD.size() * sizeof(TimeDetDev));
+    rc = fdtd_run_steps_fwd(g, key, n_steps, 1 + (recording ? 1 : 0) + (int)TD.size(), st, enqueue_fwd, &ctx);
     if (rc) return rc;
     if (recording) {      // E' of the last step; step p read counter slot p&1, so the count n_steps sits in slot n_steps&1
         ProfScope p(g, fdtd_grid::PC_RECORD, st);
@@ -1848,8 +1859,8 @@ int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float
 // The cotangent seed is in g->lam; reverse step n reads volume (n+1)&1 and writes n&1, so after step 0 the
 // result is back in volume 0 = g->lam.
 int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
-                   const std::vector<SourceDev> &S, const std::vector<DetectorDev> &D, int total_freq, int n_steps,
-                   float *dL_dinv_eps, bool seeded_H, cudaStream_t st)
+                   const std::vector<SourceDev> &S, const std::vector<DetectorDev> &D, const std::vector<TimeDetDev> &TD,
+                   int total_freq, int n_steps, float *dL_dinv_eps, bool seeded_H, cudaStream_t st)
 {
     FusedState *F = g->fused;
     const size_t vol6 = (size_t)g->G.nc * 6 * sizeof(float);
@@ -1868,8 +1879,9 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     bool fused_det = (int)D.size() <= MAX_DET;
     for (const DetectorDev &dt : D) if (dt.phasor && (dt.mask >> 3)) fused_det = false;
     // while profiling (events around every launch) the kernels run one after the other, so each is timed alone
-    const bool pipelined = fused_inv && fused_det && F->n_inv_p > 0 && !g->profiling;
-    BwdCtx ctx{ g, F->sp, F->ip, fused_inv, fused_det, pipelined, want_grad, F->bufB, fields, inv_eps, inv_mu, dL_dinv_eps, g->lam, F->lamB, &S, &D, total_freq };
+    // (time-domain detector transposes read the primal state after step n, which the pipelined sweep is still writing)
+    const bool pipelined = fused_inv && fused_det && F->n_inv_p > 0 && !g->profiling && TD.empty();
+    BwdCtx ctx{ g, F->sp, F->ip, fused_inv, fused_det, pipelined, want_grad, F->bufB, fields, inv_eps, inv_mu, dL_dinv_eps, g->lam, F->lamB, &S, &D, total_freq, &TD };
     if (fused_inv) {
         // reverse step n reads primal volume (n+1)&1 and writes n&1: state n_steps must sit in volume n_steps&1
         if ((rc = build_inv_maps(g, fields, F->bufB, inv_eps, g->lam, F->lamB, st))) return rc;
@@ -1914,9 +1926,10 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     key.append((const char *)&dL_dinv_eps, sizeof(dL_dinv_eps));
     if (!S.empty()) key.append((const char *)S.data(), S.size() * sizeof(SourceDev));
     if (!D.empty()) key.append((const char *)D.data(), D.size() * sizeof(DetectorDev));
+    if (!TD.empty()) key.append((const char *)TD.data(), TD.size() * sizeof(TimeDetDev));
     const int n_inj = g->G.d > 0 ? 1 : 0;
-    const int launches = !want_grad ? 1 + (fused_det ? 0 : n_adj)
-                         : (fused_inv ? 2 + (fused_det ? 0 : n_adj) + n_inj : 3 + (fused_det ? 0 : n_adj) + (int)S.size() + n_inj);
+    const int launches = (int)TD.size() + (!want_grad ? 1 + (fused_det ? 0 : n_adj)
+                         : (fused_inv ? 2 + (fused_det ? 0 : n_adj) + n_inj : 3 + (fused_det ? 0 : n_adj) + (int)S.size() + n_inj));
     rc = fdtd_run_steps_bwd(g, key, n_steps, launches, st, enqueue_bwd, &ctx);
     if (rc || !pipelined) return rc;
     // inverse step 0 on every SM; reverse step p read counter slot p&1 (p counted from the end), so -1 sits in slot n_steps&1

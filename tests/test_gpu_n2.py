@@ -1,0 +1,205 @@
+"""GPU parity for SURVEY 8(f) N2: time-domain snapshot / energy detectors and their
+transposes, Poynting flux from phasors with and without Yee co-location and its VJP, the one-directional TFSF plane
+source -- the CUDA path through the C ABI against the fp64 oracle on the same seeded inputs (readings R23-R25).
+Tolerances as in test_gpu_parity.py: fields 1e-5, phasor-level quantities 1e-4, gradients 1e-3 (R19 metric)."""
+import numpy as np
+import pytest
+
+from paper_2412_12360_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL_FIELD, TOL_PHASOR, TOL_GRAD = 1e-5, 1e-4, 1e-3
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device")
+    from paper_2412_12360_b200 import binding
+    return binding
+
+
+def relerr(x, ref):
+    ref = np.asarray(ref, dtype=np.float64)
+    x = np.asarray(x, dtype=np.float64)
+    den = np.max(np.abs(ref))
+    return float(np.max(np.abs(x - ref)) / den) if den > 0 else float(np.max(np.abs(x)))
+
+
+def _time_detector_case(B, w, path, td, record_mode=1, grad_box=None):
+    """Forward with time-domain detectors, loss linear in their outputs (fixed seeded weights), backward."""
+    import torch
+    from oracle.oracle import Oracle
+    rng = np.random.default_rng(11)
+    cots = [rng.standard_normal(t.out_shape(w.n_steps)).astype(np.float32) for t in td]
+    im = w.meta.get("inv_mu")
+    # oracle
+    o = Oracle(**w.grid_kwargs())
+    fr = np.zeros((6, w.nz, w.ny, w.nx))
+    out = o.forward(fr, w.inv_eps, im, w.sources, [], w.n_steps, record=True, time_detectors=td)
+    g_ref, lam_ref = o.backward(fr, w.inv_eps, im, w.sources, [], None, None, w.n_steps, out["rec"],
+                                time_detectors=td, dL_dtime=cots)
+    # GPU
+    kw = w.grid_kwargs()
+    kw.update(max_steps=w.n_steps, record=record_mode, path=path)
+    if grad_box:
+        kw.update(grad_lo=grad_box[0], grad_hi=grad_box[1])
+    g = B.Grid(**kw)
+    f = torch.zeros((6, w.nz, w.ny, w.nx), device="cuda")
+    ie = torch.as_tensor(w.inv_eps).cuda()
+    imt = None if im is None else torch.as_tensor(im).cuda()
+    g.forward(f, ie, imt, w.sources, [], w.n_steps, time_detectors=td)
+    torch.cuda.synchronize()
+    for t, got, want in zip(td, g.time_outputs, out["time_outputs"]):
+        e = relerr(got.cpu().numpy(), want)
+        assert e <= (TOL_PHASOR if t.kind == "energy" else TOL_FIELD), (t.kind, e)
+    grad, lam0 = g.backward(f, ie, imt, w.sources, [], None, None, w.n_steps, want_dL_dfields0=True,
+                            time_detectors=td, dL_dtime=[torch.as_tensor(c).cuda() for c in cots])
+    torch.cuda.synchronize()
+    info = g.info()
+    gg, ll = grad.cpu().numpy(), lam0.cpu().numpy()
+    g.close()
+    if grad_box:
+        lo, hi = grad_box
+        mask = np.zeros_like(g_ref, dtype=bool)
+        mask[lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0]] = True
+        g_ref = np.where(mask, g_ref, 0.0)
+    eg, el = relerr(gg, g_ref), relerr(ll, lam_ref)
+    assert eg <= TOL_GRAD and el <= TOL_GRAD, (eg, el)
+    return info
+
+
+def test_time_detectors_tiny_every_term(B):
+    """Tiny CPML grid with kappa, alpha, inv_mu, E and H sources (generic kernels: nx % 4 != 0)."""
+    w = wl.tiny_pml(n_steps=30)
+    d = w.pml_cells
+    td = [wl.TimeDetector("energy", (d, d, d), (w.nx - d, w.ny - d, w.nz - d), stride=3),
+          wl.TimeDetector("snapshot", (d + 1, d, d + 1), (w.nx - d, w.ny - d - 1, w.nz - d), stride=4, component_mask=0b011011)]
+    _time_detector_case(B, w, B.FDTD_PATH_GENERIC, td)
+
+
+@pytest.mark.parametrize("with_mu", [False, True])
+@pytest.mark.parametrize("record_mode", [1, 2])
+def test_time_detectors_on_the_fused_path(B, with_mu, record_mode):
+    """C3 miniature on the fused kernels (ping-pong volumes, im lamH carried by the sweep when inv_mu is given):
+    an energy detector inside the reconstruction box, a snapshot detector that reaches into the PML."""
+    w = wl.c3_mini(n_steps=90)
+    if with_mu:
+        rng = np.random.default_rng(5)
+        w.meta["inv_mu"] = (1.0 / (1.0 + 0.5 * rng.random((w.nz, w.ny, w.nx), dtype=np.float32))).astype(np.float32)
+    lo, hi = w.design_lo, w.design_hi
+    td = [wl.TimeDetector("energy", lo, hi, stride=7),
+          wl.TimeDetector("snapshot", (2, 3, lo[2]), (w.nx - 6, w.ny - 2, lo[2] + 2), stride=10, component_mask=0b101101)]
+    info = _time_detector_case(B, w, B.FDTD_PATH_FUSED, td, record_mode=record_mode, grad_box=(lo, hi))
+    assert info.path == B.FDTD_PATH_FUSED
+
+
+def _flux_detector(w, axis, p, thick):
+    d = w.pml_cells
+    lo, hi = [d, d, d], [w.nx - d, w.ny - d, w.nz - d]
+    lo[axis], hi[axis] = p - (thick - 1), p + 1
+    b, c = (axis + 1) % 3, (axis + 2) % 3
+    mask = (1 << b) | (1 << c) | (1 << (3 + b)) | (1 << (3 + c)) | (1 << axis)      # one extra component: slots are not 0..3
+    return wl.Detector(mask, tuple(lo), tuple(hi), [wl.omega_ppw(12), wl.omega_ppw(17)])
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+@pytest.mark.parametrize("interpolate", [False, True])
+def test_flux_and_its_vjp(B, axis, interpolate):
+    """Flux through a plane normal to every axis from the phasors the GPU accumulated, and the VJP that turns
+    dL/dflux into the phasor cotangent, against the oracle's statement of reading R24 on the same phasors."""
+    import torch
+    from oracle.oracle import Oracle
+    w = wl.c3_mini(nx=40, ny=36, nz=32, d=6, n_steps=80)
+    det = _flux_detector(w, axis, [26, 22, 20][axis], 2 if interpolate else 1)
+    g = B.Grid(**{**w.grid_kwargs(), "max_steps": w.n_steps})
+    f = torch.zeros((6, w.nz, w.ny, w.nx), device="cuda")
+    ie = torch.as_tensor(w.inv_eps).cuda()
+    ph = g.forward(f, ie, None, w.sources, [det], w.n_steps)[0]
+    fl = g.flux(det, ph, axis, interpolate)
+    Gf = np.array([0.7, -1.3], dtype=np.float32)
+    dP = g.flux_vjp(det, ph, axis, interpolate, Gf)
+    torch.cuda.synchronize()
+    o = Oracle(**w.grid_kwargs())
+    P = ph.cpu().numpy().astype(np.float64)
+    fl_ref = o.flux(det, P, axis, interpolate)
+    dP_ref = o.flux_vjp(det, P, axis, interpolate, Gf.astype(np.float64))
+    g.close()
+    assert np.max(np.abs(fl_ref)) > 0
+    # the flux is a difference of two products summed over the plane: error relative to the sum of magnitudes' scale
+    assert relerr(fl.cpu().numpy(), fl_ref) <= TOL_PHASOR, (fl.cpu().numpy(), fl_ref)
+    assert relerr(dP.cpu().numpy(), dP_ref) <= TOL_FIELD
+
+
+def test_flux_rejects_a_detector_without_the_tangential_components(B):
+    import torch
+    w = wl.c3_mini(nx=40, ny=36, nz=32, d=6, n_steps=4)
+    det = wl.Detector(0b000011, (6, 6, 20), (34, 30, 21), [0.3])
+    g = B.Grid(**{**w.grid_kwargs(), "max_steps": 4})
+    ph = torch.zeros(det.phasor_shape, device="cuda")
+    with pytest.raises(B.FdtdError) as e:
+        g.flux(det, ph, 2, False)
+    assert e.value.code == B.FDTD_EINVAL
+    det2 = _flux_detector(w, 2, 20, 1)
+    with pytest.raises(B.FdtdError):
+        g.flux(det2, torch.zeros(det2.phasor_shape, device="cuda"), 2, True)       # needs two planes
+    g.close()
+
+
+@pytest.mark.parametrize("axis,pol,direction", [(2, 1, 1), (2, 0, -1), (0, 2, 1), (1, 0, -1)])
+def test_tfsf_plane_source(B, axis, pol, direction):
+    """The helper's two waveforms against the oracle's auxiliary grid, then the pair of patches in a 3-D run on the
+    GPU: fields equal the oracle's run, the wave leaves to one side only (backward flux <= 1e-5 of the forward flux;
+    fp32 rounding in place of the oracle's 1e-12)."""
+    import torch
+    from oracle.oracle import Oracle
+    n_long, n_steps, p0 = 96, 70, 48
+    dims = [8, 6, 5]
+    dims[axis] = n_long
+    if axis != 0:
+        dims[0] = 8
+    nx, ny, nz = dims
+    eps_r, mu_r, ppw = 2.25, 1.0, 14.0
+    base = wl.gaussian_sine(n_steps, 24, 7, ppw)
+    o = Oracle(nx, ny, nz, wl.COURANT, periodic=True)
+    wE_r, wH_r, hc_r, off_r = o.tfsf_plane(wl.COURANT, eps_r, mu_r, axis, pol, direction, base.astype(np.float64))
+    g = B.Grid(nx=nx, ny=ny, nz=nz, courant=wl.COURANT, periodic=True, max_steps=n_steps)
+    wE, wH, hc, off = g.tfsf_plane(eps_r, mu_r, axis, pol, direction, base)
+    torch.cuda.synchronize()
+    assert (hc, off) == (hc_r, off_r)
+    assert relerr(wE.cpu().numpy(), wE_r) <= TOL_FIELD and relerr(wH.cpu().numpy(), wH_r) <= TOL_FIELD
+
+    def patches(we, wh):
+        lo, hi = [0, 0, 0], [nx, ny, nz]
+        lo[axis], hi[axis] = p0, p0 + 1
+        sE = wl.Source(pol, tuple(lo), tuple(hi), we)
+        lo[axis], hi[axis] = p0 + off, p0 + off + 1
+        return [sE, wl.Source(hc, tuple(lo), tuple(hi), wh)]
+
+    b, c = (axis + 1) % 3, (axis + 2) % 3
+    mask = (1 << b) | (1 << c) | (1 << (3 + b)) | (1 << (3 + c))
+
+    def plane_det(p):
+        lo, hi = [0, 0, 0], [nx, ny, nz]
+        lo[axis], hi[axis] = p - 1, p + 1
+        return wl.Detector(mask, tuple(lo), tuple(hi), [wl.omega_ppw(ppw)])
+
+    dets = [plane_det(p0 + 12 * direction), plane_det(p0 - 12 * direction)]
+    ie = np.full((nz, ny, nx), 1.0 / eps_r, dtype=np.float32)
+    fr = np.zeros((6, nz, ny, nx))
+    o.forward(fr, ie, None, patches(wE_r.astype(np.float32), wH_r.astype(np.float32)), dets, n_steps)
+    f = torch.zeros((6, nz, ny, nx), device="cuda")
+    ph = g.forward(f, torch.as_tensor(ie).cuda(), None, patches(wE, wH), dets, n_steps)
+    fl_front = float(g.flux(dets[0], ph[0], axis, True)[0])
+    fl_back = float(g.flux(dets[1], ph[1], axis, True)[0])
+    torch.cuda.synchronize()
+    fg = f.cpu().numpy()
+    g.close()
+    assert relerr(fg[:3], fr[:3]) <= TOL_FIELD and relerr(fg[3:], fr[3:]) <= TOL_FIELD
+    assert fl_front * direction > 0 and abs(fl_back) <= 1e-5 * abs(fl_front), (fl_front, fl_back)
+    idx = np.arange(n_long)
+    behind = idx < p0 - 1 if direction > 0 else idx > p0 + 1
+    front = np.max(np.abs(fg[:3]))
+    assert np.max(np.abs(np.compress(behind, fg, axis=3 - axis))) <= 1e-5 * front
