@@ -96,6 +96,12 @@ extern "C" {
 #define FDTD_FLAG_HOST_STAGING  1   /* allocate the staging buffers of fdtd_forward_host / fdtd_backward_host
                                        (fields, inv_eps, and the gradient when record != 0) in fdtd_create_grid */
 
+#define FDTD_FLAG_RECORDER_FP16  2   /* SURVEY 8(f) N1, reduced-precision recorder: the interface values are stored as
+                                       fp16 (round to nearest) instead of fp32, halving the recorder (C3: 2.97 -> 1.49 GB,
+                                       C4: 117 -> 58 GB).  An approximation, off by default: the reconstructed fields carry
+                                       the rounding (2^-11 relative per recorded value); the gradient error this costs is
+                                       measured in tests/test_gpu_parity.py and stated in DESIGN.md.                       */
+
 typedef struct fdtd_grid fdtd_grid;      /* opaque */
 
 /* Grid descriptor.  A zero in any CPML constant selects its default (reading R8). */

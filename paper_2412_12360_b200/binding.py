@@ -20,7 +20,7 @@ LIB_PATH = _HERE / "libfdtd_b200.so"
 
 FDTD_OK, FDTD_EINVAL, FDTD_ENOMEM, FDTD_ECUDA, FDTD_ESTATE = 0, -1, -2, -3, -4
 FDTD_PATH_AUTO, FDTD_PATH_GENERIC, FDTD_PATH_FUSED = 0, 1, 2
-FDTD_FLAG_HOST_STAGING = 1
+FDTD_FLAG_HOST_STAGING, FDTD_FLAG_RECORDER_FP16 = 1, 2
 PARTITION_NAMES = {0: "none (generic kernels)", 1: "contiguous runs", 2: "lock-step runs", 3: "waves of whole columns + levelled pool"}
 
 

@@ -163,7 +163,7 @@ extern "C" int fdtd_create_grid(const fdtd_grid_desc *desc, fdtd_grid **out)
     if (desc->record < 0 || desc->record > 2) return fail(FDTD_EINVAL, "record must be 0, 1 or 2");
     if (desc->path < 0 || desc->path > 2) return fail(FDTD_EINVAL, "unknown path");
     for (int q = 0; q < 6; ++q) if (desc->reserved[q]) return fail(FDTD_EINVAL, "reserved fields must be zero");
-    if (desc->flags & ~FDTD_FLAG_HOST_STAGING) return fail(FDTD_EINVAL, "unknown bit in flags");
+    if (desc->flags & ~(FDTD_FLAG_HOST_STAGING | FDTD_FLAG_RECORDER_FP16)) return fail(FDTD_EINVAL, "unknown bit in flags");
     if (desc->pml_m < 0 || desc->pml_sigma_scale < 0 || desc->pml_kappa_max < 0 || desc->pml_alpha_max < 0 ||
         desc->pml_alpha_m < 0 || desc->pml_eps_bg < 0)
         return fail(FDTD_EINVAL, "CPML constants must be >= 0");
@@ -203,6 +203,7 @@ extern "C" int fdtd_create_grid(const fdtd_grid_desc *desc, fdtd_grid **out)
         }
     }
     make_rec_layout(G, g->R);
+    g->R.half = (desc->flags & FDTD_FLAG_RECORDER_FP16) ? 1 : 0;
 
     int rc = FDTD_OK;
     auto bail = [&](int code) { std::string keep = g_err; fdtd_destroy(g); g_err = keep; return code; };
@@ -241,7 +242,7 @@ extern "C" int fdtd_create_grid(const fdtd_grid_desc *desc, fdtd_grid **out)
     if (cudaMemset(g->red.ticket, 0, 64) != cudaSuccess) return bail(cuda_fail(cudaGetLastError(), "cudaMemset"));
     if ((rc = g->alloc_psi(g->psiE[0])) || (rc = g->alloc_psi(g->psiH[0]))) return bail(rc);
     if (desc->record && G.d > 0 && desc->max_steps > 0) {
-        const size_t bytes = (size_t)g->R.stride * sizeof(float) * (size_t)desc->max_steps;
+        const size_t bytes = (size_t)g->R.stride * (g->R.half ? 2 : sizeof(float)) * (size_t)desc->max_steps;
         if ((rc = g->alloc((void **)&g->rec, bytes, true))) return bail(rc);
     }
     {

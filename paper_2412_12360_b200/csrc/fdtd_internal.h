@@ -75,7 +75,8 @@ struct RecLayout {
     long long off[3][2][2];   // [axis][side 0=low,1=high][which]
     long long cells[3];       // face cells per axis
     int fast[3], slow[3];     // the two in-face axes
-    long long stride;         // floats per step (multiple of 32)
+    long long stride;         // elements per step (multiple of 32)
+    int half;                 // 1: elements are fp16 (FDTD_FLAG_RECORDER_FP16), 0: fp32
 };
 
 struct SourceDev {

@@ -5,6 +5,7 @@
 // simple statement the fused kernels are cross-checked against on the GPU.
 // Formulas: include/fdtd.h (conventions) and DESIGN.md section 2; Eq. 1-2, L72, L84.
 #include <algorithm>
+#include <cuda_fp16.h>
 #include "fdtd_internal.h"
 
 namespace fdtd {
@@ -169,6 +170,16 @@ __global__ void k_scale_H(float *__restrict__ lamH, const float *__restrict__ im
 
 // ------------------------------------------------------------------------------------------ F8
 // One thread per float of a step's record.  INJECT=false: fields -> rec[n]; true: rec[n] -> fields.
+// recorder element idx: fp32, or fp16 when the grid was created with FDTD_FLAG_RECORDER_FP16
+__device__ __forceinline__ void rec_store(float *rec, long long idx, float v, int half)
+{
+    if (half) reinterpret_cast<__half *>(rec)[idx] = __float2half_rn(v); else rec[idx] = v;
+}
+__device__ __forceinline__ float rec_load(const float *rec, long long idx, int half)
+{
+    return half ? __half2float(reinterpret_cast<const __half *>(rec)[idx]) : __ldg(rec + idx);
+}
+
 // PP=true (fused ping-pong path): fH/fE are the two field buffers A/B; step n read buffer n&1 (pre-step H)
 // and wrote buffer (n+1)&1 (E'); for INJECT the target is buffer (n+1)&1 (the state the reverse step reads).
 template <bool INJECT, bool PP>
@@ -205,11 +216,11 @@ __global__ void k_record(Dims G, RecLayout R, const float *__restrict__ fH, cons
     pos[sl] = G.lo[sl] + (int)(local / nf);
     const int comp = (a + 1 + which) % 3;
     const long long p = lin(G, pos[0], pos[1], pos[2]);
-    float *r = rec + (long long)(*step) * R.stride + t;
+    const long long r = (long long)(*step) * R.stride + t;
     if (!INJECT) {
-        *r = side ? __ldg(fE + comp * G.nc + p) : __ldg(fH + (3 + comp) * G.nc + p);
+        rec_store(rec, r, side ? __ldg(fE + comp * G.nc + p) : __ldg(fH + (3 + comp) * G.nc + p), R.half);
     } else {
-        fout[(side ? comp : 3 + comp) * G.nc + p] = *r;
+        fout[(side ? comp : 3 + comp) * G.nc + p] = rec_load(rec, r, R.half);
     }
 }
 
@@ -245,7 +256,7 @@ __global__ void __launch_bounds__(128, 16) k_record_pipe(Dims G, RecLayout R, co
     pos[sl] = G.lo[sl] + (int)(local / nf);
     const int comp = (a + 1 + which) % 3;
     const long long p = lin(G, pos[0], pos[1], pos[2]);
-    rec[(long long)(side ? n - 1 : n) * R.stride + t] = __ldg(f + (side ? comp : 3 + comp) * G.nc + p);
+    rec_store(rec, (long long)(side ? n - 1 : n) * R.stride + t, __ldg(f + (side ? comp : 3 + comp) * G.nc + p), R.half);
 }
 
 // Face injection of the fused reverse sweep, run beside adjoint step n: rec[n] -> buffer (n+1)&1, the volume
@@ -276,7 +287,7 @@ __global__ void __launch_bounds__(128, 16) k_inject_pipe(Dims G, RecLayout R, fl
     pos[fa] = G.lo[fa] + (int)(local % nf);
     pos[sl] = G.lo[sl] + (int)(local / nf);
     const int comp = (a + 1 + which) % 3;
-    f[(side ? comp : 3 + comp) * G.nc + lin(G, pos[0], pos[1], pos[2])] = __ldg(rec + (long long)n * R.stride + t);
+    f[(side ? comp : 3 + comp) * G.nc + lin(G, pos[0], pos[1], pos[2])] = rec_load(rec, (long long)n * R.stride + t, R.half);
 }
 
 __global__ void k_advance(int *step, int delta) { *step += delta; }

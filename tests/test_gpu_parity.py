@@ -75,11 +75,11 @@ def run_oracle(w, n_steps=None, backward=True, f0=None, dtype=np.float64):
     return res
 
 
-def run_gpu(B, w, path, n_steps=None, backward=True, f0=None, grad_box=None, record_mode=1, rho_box=None):
+def run_gpu(B, w, path, n_steps=None, backward=True, f0=None, grad_box=None, record_mode=1, rho_box=None, flags=0):
     import torch
     n = w.n_steps if n_steps is None else n_steps
     kw = w.grid_kwargs()
-    kw.update(max_steps=n, record=record_mode if (backward and w.pml_cells > 0) else 0, path=path)
+    kw.update(max_steps=n, record=record_mode if (backward and w.pml_cells > 0) else 0, path=path, flags=flags)
     if grad_box:
         kw.update(grad_lo=grad_box[0], grad_hi=grad_box[1])
     g = B.Grid(**kw)
@@ -346,6 +346,27 @@ def test_gradient_box_recorder(B):
             mask = np.ones_like(gpu["grad"], bool)
             mask[box] = False
             assert np.all(gpu["grad"][mask] == 0)
+
+
+@pytest.mark.parametrize("record_mode", [1, 2])
+def test_reduced_precision_recorder(B, record_mode):
+    """SURVEY 8(f) N1, reduced-precision recorder (FDTD_FLAG_RECORDER_FP16): half the recorder bytes; the interface
+    values re-imposed in the reverse sweep carry fp16 rounding (2^-11 relative), so the reconstructed fields and the
+    gradient are approximate.  The gradient must stay within the north-star 1e-3 of the fp64 oracle on the C3
+    miniature (both kernel paths); the measured error is printed beside the fp32 recorder's."""
+    w = wl.c3_mini(n_steps=200)
+    ref = run_oracle(w)
+    box = (w.design_lo, w.design_hi)
+    gref = np.zeros_like(ref["grad"])
+    sl = (slice(box[0][2], box[1][2]), slice(box[0][1], box[1][1]), slice(box[0][0], box[1][0]))
+    gref[sl] = ref["grad"][sl]
+    for path in paths(B, w):
+        e32 = relerr(run_gpu(B, w, path, grad_box=box, record_mode=record_mode)["grad"], gref)
+        r16 = run_gpu(B, w, path, grad_box=box, record_mode=record_mode, flags=B.FDTD_FLAG_RECORDER_FP16)
+        e16 = relerr(r16["grad"], gref)
+        print(f"recorder fp32 / fp16, record={record_mode}, path={path}: gradient error {e32:.2e} / {e16:.2e}")
+        assert r16["info"].recorder_bytes == r16["info"].record_floats_per_step * 2 * w.n_steps      # 2 bytes per value
+        assert e16 <= TOL_GRAD, (e32, e16)
 
 
 def test_pipelined_reverse_sweep_is_the_same_computation(B, monkeypatch):
