@@ -125,7 +125,13 @@ typedef struct {
     int32_t grad_hi[3];        /*   all zero => the whole interior I.  Always clipped to I.         */
     int32_t path;              /* FDTD_PATH_*                                                       */
     int32_t flags;             /* FDTD_FLAG_* bits                                                  */
-    int32_t reserved[6];       /* must be zero                                                      */
+    /* z-slab sub-grid (one simulation over several GPUs).  z_global == 0:
+     * an ordinary grid.  Otherwise this grid holds the planes [z_offset, z_offset + nz) of a grid of z_global planes:
+     * z_ghost_lo (0 or 1) ghost plane below and z_ghost_hi (0 or 1) above the planes it owns; the CPML tables, the
+     * interior box and the recorder faces follow the GLOBAL position (an internal cut is recorded like a PML face, so
+     * the reverse sweep's inverse step needs no exchange).  See "Domain decomposition" below. */
+    int32_t z_global, z_offset, z_ghost_lo, z_ghost_hi;
+    int32_t reserved[2];       /* must be zero                                                      */
 } fdtd_grid_desc;
 
 /* Additive source patch (reading R10/R11): during step n,
@@ -261,6 +267,52 @@ FDTD_API int fdtd_flux_vjp(fdtd_grid *grid, const fdtd_detector *det, const floa
 FDTD_API int fdtd_tfsf_plane(float courant, float eps_r, float mu_r, int32_t axis, int32_t pol, int32_t dir, int32_t n_steps,
                     const float *base, float *wE, float *wH, int32_t *h_component, int32_t *h_plane_offset,
                     void *cuda_stream);
+
+/* ------------------------------------------------------------------------------------------
+ * N3 -- domain decomposition along z (2.3 B cells over 4 GPUs).
+ *
+ * One simulation of z_global planes is cut into slabs of xy planes; each slab is a grid of its own (one per GPU /
+ * process) created with z_global / z_offset / z_ghost_lo / z_ghost_hi.  A slab owns the planes
+ * [z_offset + z_ghost_lo, z_offset + nz - z_ghost_hi) and carries one ghost plane on every side that is a cut:
+ *   ghost below (local plane 0)     : holds the H-type components of the lower neighbour's top plane, imported;
+ *   ghost above (local plane nz - 1): a replica of the upper neighbour's bottom plane -- its E-type components are
+ *                                     updated here redundantly (bit-identical arithmetic), its H-type components are
+ *                                     imported.  Everything else computed on ghost planes is overwritten or unused.
+ * Protocol: advance all slabs by one step (fdtd_forward_range(n, n+1)), then every slab exports its lowest and its
+ * highest owned plane (fdtd_halo_export: the three H-type components, [3][ny][nx]) and imports its neighbours'
+ * (fdtd_halo_import); one exchange per full step, 3 nx ny floats per neighbour and direction.  The adjoint sweep
+ * (fdtd_backward_range(n+1, n)) exchanges the H-type cotangents the same way (which = 1).  The primal inverse step of
+ * the reverse sweep needs NO exchange: the interior box of a slab is the global interior restricted to its own
+ * planes, and a cut is recorded like a PML face (tangential H of the ghost plane below before the step, tangential E'
+ * of the ghost plane above after the E update), so every slab reconstructs its own planes from its own record.
+ * Inputs per slab: inv_eps / inv_mu / dL_dfields are the local planes (ghosts included) of the global volumes;
+ * sources are clipped to the local planes (ghosts included: the replica needs them); detectors are clipped to the
+ * owned planes in fdtd_forward_range and to the local planes (with the matching slice of the cotangent) in
+ * fdtd_backward_range.  All slabs must run the same kernel path.  On owned planes the fields, the phasors and the
+ * cotangents are bit-identical to the undivided grid; dL_dinv_eps agrees to the rounding of the time reversal (next
+ * to a cut the inverse step reads the recorded value where the undivided grid reads its reconstructed neighbour:
+ * a few 1e-8 of the maximum; tests/test_gpu_subgrid.py).  Time-domain detectors are not available on range calls.
+ *
+ * fdtd_forward_range: steps n_begin .. n_end-1 of a run of n_total steps (n_begin == 0 starts a run: psi = 0; later
+ *   calls must continue where the previous one ended, else ESTATE).  Between the calls of a sequence `fields` may be
+ *   stale (the fused path keeps state n in its own second volume when n is odd); the call with n_end == n_total
+ *   leaves state n_total in `fields`.  fdtd_forward is fdtd_forward_range(0, n_steps, n_steps).
+ * fdtd_backward_range: reverse steps n_hi-1 .. n_lo (n_hi == n_total starts: B0 seeds from dL_dfields, zeroes
+ *   dL_dinv_eps; n_lo == 0 ends: dL_dfields0 is written).  The same pointers must be passed to every call of a sequence.
+ * fdtd_halo_export / fdtd_halo_import: which = 0 the fields holding state n (after fdtd_forward_range(.., n, ..)),
+ *   which = 1 the cotangents after reverse step n (after fdtd_backward_range(.., n, ..)); side 0 = low end, 1 = high
+ *   end; out / in: DEVICE [3][ny][nx].  Plane copies on cuda_stream.  The seed of the reverse sweep needs no exchange:
+ *   dL_dfields is given on the local planes, ghosts included. */
+FDTD_API int fdtd_forward_range(fdtd_grid *grid, float *fields, const float *inv_eps, const float *inv_mu,
+                       const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
+                       int32_t n_begin, int32_t n_end, int32_t n_total, void *cuda_stream);
+FDTD_API int fdtd_backward_range(fdtd_grid *grid, float *fields, const float *inv_eps, const float *inv_mu,
+                        const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
+                        const float *const *dL_dphasor, const float *dL_dfields,
+                        int32_t n_hi, int32_t n_lo, int32_t n_total, float *dL_dinv_eps, float *dL_dfields0,
+                        void *cuda_stream);
+FDTD_API int fdtd_halo_export(fdtd_grid *grid, float *fields, int32_t which, int32_t n, int32_t side, float *out, void *cuda_stream);
+FDTD_API int fdtd_halo_import(fdtd_grid *grid, float *fields, int32_t which, int32_t n, int32_t side, const float *in, void *cuda_stream);
 
 /* Frees the grid and everything it owns (synchronises the device first).  NULL is a no-op. */
 FDTD_API int fdtd_destroy(fdtd_grid *grid);

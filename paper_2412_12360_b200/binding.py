@@ -31,7 +31,9 @@ class fdtd_grid_desc(C.Structure):
                 ("pml_alpha_max", C.c_float), ("pml_alpha_m", C.c_float), ("pml_eps_bg", C.c_float),
                 ("max_steps", C.c_int32), ("record", C.c_int32),
                 ("grad_lo", C.c_int32 * 3), ("grad_hi", C.c_int32 * 3),
-                ("path", C.c_int32), ("flags", C.c_int32), ("reserved", C.c_int32 * 6)]
+                ("path", C.c_int32), ("flags", C.c_int32),
+                ("z_global", C.c_int32), ("z_offset", C.c_int32), ("z_ghost_lo", C.c_int32), ("z_ghost_hi", C.c_int32),
+                ("reserved", C.c_int32 * 2)]
 
 
 class fdtd_source(C.Structure):
@@ -70,7 +72,8 @@ class fdtd_profile(C.Structure):
 
 EXPORTS = ("fdtd_grad_rho", "fdtd_set_profiling", "fdtd_get_profile", "fdtd_create_grid", "fdtd_forward", "fdtd_backward", "fdtd_destroy", "fdtd_last_error",
            "fdtd_get_info", "fdtd_version", "fdtd_forward_host", "fdtd_backward_host", "fdtd_debug_partition",
-           "fdtd_forward_td", "fdtd_backward_td", "fdtd_flux", "fdtd_flux_vjp", "fdtd_tfsf_plane")
+           "fdtd_forward_td", "fdtd_backward_td", "fdtd_flux", "fdtd_flux_vjp", "fdtd_tfsf_plane",
+           "fdtd_forward_range", "fdtd_backward_range", "fdtd_halo_export", "fdtd_halo_import")
 
 
 def _load():
@@ -90,6 +93,15 @@ def _load():
     L.fdtd_backward_td.restype = C.c_int
     L.fdtd_backward_td.argtypes = [vp, vp, vp, vp, C.POINTER(fdtd_source), i32, C.POINTER(fdtd_detector), i32,
                                    C.POINTER(vp), C.POINTER(fdtd_time_detector), i32, C.POINTER(vp), vp, i32, vp, vp, vp]
+    L.fdtd_forward_range.restype = C.c_int
+    L.fdtd_forward_range.argtypes = [vp, vp, vp, vp, C.POINTER(fdtd_source), i32, C.POINTER(fdtd_detector), i32, i32, i32, i32, vp]
+    L.fdtd_backward_range.restype = C.c_int
+    L.fdtd_backward_range.argtypes = [vp, vp, vp, vp, C.POINTER(fdtd_source), i32, C.POINTER(fdtd_detector), i32,
+                                      C.POINTER(vp), vp, i32, i32, i32, vp, vp, vp]
+    L.fdtd_halo_export.restype = C.c_int
+    L.fdtd_halo_export.argtypes = [vp, vp, i32, i32, i32, vp, vp]
+    L.fdtd_halo_import.restype = C.c_int
+    L.fdtd_halo_import.argtypes = [vp, vp, i32, i32, i32, vp, vp]
     L.fdtd_flux.restype = C.c_int
     L.fdtd_flux.argtypes = [vp, C.POINTER(fdtd_detector), vp, i32, i32, vp, vp]
     L.fdtd_flux_vjp.restype = C.c_int
@@ -218,6 +230,25 @@ def fdtd_backward_td(grid, fields, inv_eps, inv_mu, src, n_src, det, n_det, dL_d
                                td, n_td, dL_dtd, _ptr(dL_dfields), n_steps, _ptr(dL_dinv_eps), _ptr(dL_dfields0), stream))
 
 
+def fdtd_forward_range(grid, fields, inv_eps, inv_mu, src, n_src, det, n_det, n_begin, n_end, n_total, stream) -> None:
+    _check(_L.fdtd_forward_range(grid, _ptr(fields), _ptr(inv_eps), _ptr(inv_mu), src, n_src, det, n_det,
+                                 int(n_begin), int(n_end), int(n_total), stream))
+
+
+def fdtd_backward_range(grid, fields, inv_eps, inv_mu, src, n_src, det, n_det, dL_dphasor, dL_dfields, n_hi, n_lo, n_total,
+                        dL_dinv_eps, dL_dfields0, stream) -> None:
+    _check(_L.fdtd_backward_range(grid, _ptr(fields), _ptr(inv_eps), _ptr(inv_mu), src, n_src, det, n_det, dL_dphasor,
+                                  _ptr(dL_dfields), int(n_hi), int(n_lo), int(n_total), _ptr(dL_dinv_eps), _ptr(dL_dfields0), stream))
+
+
+def fdtd_halo_export(grid, fields, which, n, side, out, stream) -> None:
+    _check(_L.fdtd_halo_export(grid, _ptr(fields), int(which), int(n), int(side), _ptr(out), stream))
+
+
+def fdtd_halo_import(grid, fields, which, n, side, buf, stream) -> None:
+    _check(_L.fdtd_halo_import(grid, _ptr(fields), int(which), int(n), int(side), _ptr(buf), stream))
+
+
 def fdtd_flux(grid, det, phasor, axis, interpolate, flux, stream) -> None:
     _check(_L.fdtd_flux(grid, det, _ptr(phasor), int(axis), int(bool(interpolate)), _ptr(flux), stream))
 
@@ -251,13 +282,15 @@ def fdtd_backward_host(grid, h_fields, h_inv_eps, h_inv_mu, src, n_src, det, n_d
 # --------------------------------------------------------------------------------------------
 def make_desc(nx, ny, nz, courant, periodic=False, pml_cells=0, pml_m=0.0, pml_sigma_scale=0.0,
               pml_kappa_max=0.0, pml_alpha_max=0.0, pml_alpha_m=0.0, pml_eps_bg=0.0, max_steps=0,
-              record=False, grad_lo=None, grad_hi=None, path=FDTD_PATH_AUTO, flags=0) -> fdtd_grid_desc:
+              record=False, grad_lo=None, grad_hi=None, path=FDTD_PATH_AUTO, flags=0,
+              z_global=0, z_offset=0, z_ghost_lo=0, z_ghost_hi=0) -> fdtd_grid_desc:
     d = fdtd_grid_desc()
     d.nx, d.ny, d.nz, d.courant = nx, ny, nz, courant
     d.periodic, d.pml_cells = int(bool(periodic)), pml_cells
     d.pml_m, d.pml_sigma_scale, d.pml_kappa_max = pml_m, pml_sigma_scale, pml_kappa_max
     d.pml_alpha_max, d.pml_alpha_m, d.pml_eps_bg = pml_alpha_max, pml_alpha_m, pml_eps_bg
     d.max_steps, d.record, d.path, d.flags = max_steps, int(record), path, int(flags)
+    d.z_global, d.z_offset, d.z_ghost_lo, d.z_ghost_hi = int(z_global), int(z_offset), int(z_ghost_lo), int(z_ghost_hi)
     if grad_lo is not None:
         d.grad_lo[:] = list(grad_lo)
         d.grad_hi[:] = list(grad_hi)

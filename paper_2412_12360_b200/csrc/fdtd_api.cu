@@ -156,13 +156,26 @@ extern "C" int fdtd_create_grid(const fdtd_grid_desc *desc, fdtd_grid **out)
         return fail(FDTD_EINVAL, "courant must satisfy 0 < S < 1/sqrt(3)");
     if (desc->pml_cells < 0) return fail(FDTD_EINVAL, "pml_cells must be >= 0");
     if (desc->periodic && desc->pml_cells != 0) return fail(FDTD_EINVAL, "a periodic grid cannot have a PML");
-    const int mn = std::min(desc->nx, std::min(desc->ny, desc->nz));
+    const bool sub = desc->z_global != 0;
+    if (sub) {
+        if (desc->periodic) return fail(FDTD_EINVAL, "a z-slab sub-grid cannot be periodic");
+        if (desc->z_ghost_lo < 0 || desc->z_ghost_lo > 1 || desc->z_ghost_hi < 0 || desc->z_ghost_hi > 1)
+            return fail(FDTD_EINVAL, "z_ghost_lo / z_ghost_hi must be 0 or 1");
+        if (desc->z_offset < 0 || desc->z_offset + desc->nz > desc->z_global || desc->nz - desc->z_ghost_lo - desc->z_ghost_hi < 1)
+            return fail(FDTD_EINVAL, "sub-grid planes [z_offset, z_offset + nz) must lie inside [0, z_global) and own at least one plane");
+        if ((desc->z_ghost_lo == 0) != (desc->z_offset == 0) || (desc->z_ghost_hi == 0) != (desc->z_offset + desc->nz == desc->z_global))
+            return fail(FDTD_EINVAL, "a sub-grid has a ghost plane exactly where it does not touch the end of the global grid");
+    } else if (desc->z_offset || desc->z_ghost_lo || desc->z_ghost_hi) {
+        return fail(FDTD_EINVAL, "z_offset / z_ghost_* need z_global");
+    }
+    const int nz_full = sub ? desc->z_global : desc->nz;
+    const int mn = std::min(desc->nx, std::min(desc->ny, nz_full));
     if (desc->pml_cells > 0 && 2 * desc->pml_cells + 2 > mn)
         return fail(FDTD_EINVAL, "need 2*pml_cells + 2 <= min(nx,ny,nz)");
     if (desc->max_steps < 0) return fail(FDTD_EINVAL, "max_steps must be >= 0");
     if (desc->record < 0 || desc->record > 2) return fail(FDTD_EINVAL, "record must be 0, 1 or 2");
     if (desc->path < 0 || desc->path > 2) return fail(FDTD_EINVAL, "unknown path");
-    for (int q = 0; q < 6; ++q) if (desc->reserved[q]) return fail(FDTD_EINVAL, "reserved fields must be zero");
+    for (int q = 0; q < 2; ++q) if (desc->reserved[q]) return fail(FDTD_EINVAL, "reserved fields must be zero");
     if (desc->flags & ~(FDTD_FLAG_HOST_STAGING | FDTD_FLAG_RECORDER_FP16)) return fail(FDTD_EINVAL, "unknown bit in flags");
     if (desc->pml_m < 0 || desc->pml_sigma_scale < 0 || desc->pml_kappa_max < 0 || desc->pml_alpha_max < 0 ||
         desc->pml_alpha_m < 0 || desc->pml_eps_bg < 0)
@@ -181,6 +194,16 @@ extern "C" int fdtd_create_grid(const fdtd_grid_desc *desc, fdtd_grid **out)
     const int dp4 = (G.d + 3) / 4 * 4;
     G.dpx = (G.nx % 4 == 0 && G.nx >= 2 * dp4) ? dp4 : G.d;
     for (int a = 0; a < 3; ++a) { G.lo[a] = G.d; G.hi[a] = dim_of(G, a) - G.d; }
+    G.zoff = sub ? desc->z_offset : 0; G.nzg = nz_full;
+    G.zl = std::min(G.nz, std::max(0, G.d - G.zoff));
+    G.zh = std::min(G.nz, std::max(0, G.zoff + G.nz - (G.nzg - G.d)));
+    if (sub) {
+        // interior box along z: the global interior restricted to the planes this sub-grid owns (local indices)
+        const int own_lo = G.zoff + desc->z_ghost_lo, own_hi = G.zoff + G.nz - desc->z_ghost_hi;
+        G.lo[2] = std::max(G.d, own_lo) - G.zoff;
+        G.hi[2] = std::min(G.nzg - G.d, own_hi) - G.zoff;
+        if (G.hi[2] <= G.lo[2]) { delete g; return fail(FDTD_EINVAL, "a sub-grid must own at least one plane of the interior"); }
+    }
     bool all_zero = true;
     for (int a = 0; a < 3; ++a) if (desc->grad_lo[a] || desc->grad_hi[a]) all_zero = false;
     for (int a = 0; a < 3; ++a) {
@@ -228,6 +251,11 @@ extern "C" int fdtd_create_grid(const fdtd_grid_desc *desc, fdtd_grid **out)
             for (int a = 0; a < 3; ++a) {
                 const int n = dim_of(G, a), np = padded(n);
                 for (int q = 0; q < np; ++q) { h[off + q] = 1.f; h[off + np + q] = 0.f; h[off + 2 * np + q] = 1.f; }
+                if (a == 2 && sub) {      // the planes [zoff, zoff + nz) of the global table
+                    std::vector<float> tb(G.nzg), ta(G.nzg), tk(G.nzg);
+                    make_table(G.nzg, G.d, fam, (double)G.S, m, smax, km, (double)desc->pml_alpha_max, am, tb.data(), ta.data(), tk.data());
+                    for (int q = 0; q < n; ++q) { h[off + q] = tb[G.zoff + q]; h[off + np + q] = ta[G.zoff + q]; h[off + 2 * np + q] = tk[G.zoff + q]; }
+                } else
                 make_table(n, G.d, fam, (double)G.S, m, smax, km, (double)desc->pml_alpha_max, am,
                            &h[off], &h[off + np], &h[off + 2 * np]);
                 g->T.b[fam][a] = dev + off; g->T.a[fam][a] = dev + off + np; g->T.ik[fam][a] = dev + off + 2 * np;
@@ -467,6 +495,12 @@ namespace {
 int upload_cs_table(fdtd_grid *g, const fdtd_detector *det, int n_det, int total_freq, int n_steps, cudaStream_t st)
 {
     if (total_freq == 0 || n_steps == 0) return FDTD_OK;
+    // the same frequencies and step count as the table on the device (the calls of a range sequence): nothing to do
+    std::vector<float> ck;
+    ck.push_back((float)n_steps);
+    for (int s = 0; s < n_det; ++s) for (int q = 0; q < det[s].n_freq; ++q) ck.push_back(det[s].omega[q]);
+    if (ck == g->cs_key) return FDTD_OK;
+    g->cs_key.clear();
     const size_t need = (size_t)n_steps * total_freq * 2;
     if (need > g->cs_cap) {       // more than CS_PREALLOC_FREQ frequencies: grow
         int rc = g->reserve_cs_table((size_t)std::max(n_steps, g->desc.max_steps) * total_freq * 2);
@@ -487,6 +521,7 @@ int upload_cs_table(fdtd_grid *g, const fdtd_detector *det, int n_det, int total
     }
     CK(cudaMemcpyAsync(g->d_cs, g->h_cs, need * sizeof(float), cudaMemcpyHostToDevice, st));
     CK(cudaEventRecord(g->table_done, st));
+    g->cs_key = ck;
     return FDTD_OK;
 }
 
@@ -578,10 +613,32 @@ extern "C" int fdtd_forward(fdtd_grid *g, float *fields, const float *inv_eps, c
     return fdtd_forward_td(g, fields, inv_eps, inv_mu, src, n_src, det, n_det, nullptr, 0, n_steps, cuda_stream);
 }
 
+static int forward_impl(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
+                        const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
+                        const fdtd_time_detector *td, int32_t n_td, int n_begin, int n_end, int n_total, void *cuda_stream);
+
 extern "C" int fdtd_forward_td(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
                                const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
                                const fdtd_time_detector *td, int32_t n_td, int32_t n_steps, void *cuda_stream)
 {
+    return forward_impl(g, fields, inv_eps, inv_mu, src, n_src, det, n_det, td, n_td, 0, n_steps, n_steps, cuda_stream);
+}
+
+extern "C" int fdtd_forward_range(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
+                                  const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
+                                  int32_t n_begin, int32_t n_end, int32_t n_total, void *cuda_stream)
+{
+    if (n_begin < 0 || n_end < n_begin || n_total < n_end) return fail(FDTD_EINVAL, "fdtd_forward_range: need 0 <= n_begin <= n_end <= n_total");
+    if (g && n_begin != 0 && g->fwd_pos != n_begin) return fail(FDTD_ESTATE, "fdtd_forward_range: n_begin does not continue the previous range");
+    return forward_impl(g, fields, inv_eps, inv_mu, src, n_src, det, n_det, nullptr, 0, n_begin, n_end, n_total, cuda_stream);
+}
+
+// steps n_begin .. n_end-1 of a run of n_total steps (fdtd_forward: 0 .. n_steps-1)
+static int forward_impl(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
+                        const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
+                        const fdtd_time_detector *td, int32_t n_td, int n_begin, int n_end, int n_total, void *cuda_stream)
+{
+    const int n_steps = n_total;
     int rc = check_common(g, fields, inv_eps, src, n_src, det, n_det, n_steps, "fdtd_forward");
     if (rc) return rc;
     for (int s = 0; s < n_det; ++s)
@@ -597,8 +654,9 @@ extern "C" int fdtd_forward_td(fdtd_grid *g, float *fields, const float *inv_eps
     const int total_freq = translate(det, n_det, D);
     const bool recording = g->desc.record && G.d > 0;
     g->recorded_steps = -1;
+    g->fwd_pos = -1;
     if ((rc = upload_cs_table(g, det, n_det, total_freq, n_steps, st))) return rc;
-    launch_set_step(g->d_step, 0, st);                   // step 0 reads slot 0
+    launch_set_step(g->d_step, n_begin, st);             // the first step of the call reads slot 0
 
     // more descriptors than the fused kernels' parameter block holds: this call runs on the generic kernels (same
     // psi slabs, same recorder layout, so a fused or generic fdtd_backward can follow)
@@ -606,14 +664,14 @@ extern "C" int fdtd_forward_td(fdtd_grid *g, float *fields, const float *inv_eps
     if (g->path == FDTD_PATH_FUSED && !fused_call && g->desc.path == FDTD_PATH_FUSED)
         return fail(FDTD_EINVAL, "FDTD_PATH_FUSED takes at most 4 sources and 4 detectors per call (FDTD_PATH_AUTO falls back to the generic kernels)");
     if (fused_call) {
-        rc = fused_forward(g, fields, inv_eps, inv_mu, S, D, TD, total_freq, n_steps, recording, st);
+        rc = fused_forward(g, fields, inv_eps, inv_mu, S, D, TD, total_freq, n_begin, n_end, n_total, recording, st);
         if (rc) return rc;
     } else {
-        if ((rc = g->zero_psi(g->psiE[0], st)) || (rc = g->zero_psi(g->psiH[0], st))) return rc;
+        if (n_begin == 0 && ((rc = g->zero_psi(g->psiE[0], st)) || (rc = g->zero_psi(g->psiH[0], st)))) return rc;
         const int launches = 3 + n_src + n_det + n_td + (recording ? 1 : 0);
         std::string key = make_key("gf", fields, inv_eps, inv_mu, g->rec, g->d_cs, S, D, recording);
         if (!TD.empty()) key.append((const char *)TD.data(), TD.size() * sizeof(TimeDetDev));
-        rc = run_steps(g, g->fwd_graph, key, n_steps, launches, st, [&](cudaStream_t cs) {
+        rc = run_steps(g, g->fwd_graph, key, n_end - n_begin, launches, st, [&](cudaStream_t cs) {
             { ProfScope p(g, fdtd_grid::PC_UPDATE_E, cs); launch_update_E(G, g->T, fields, inv_eps, g->psiE[0], cs); }
             { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
               for (const SourceDev &s : S) if (s.comp < 3) launch_add_source(G, fields, s, g->step_in(), 1.f, cs); }
@@ -629,7 +687,9 @@ extern "C" int fdtd_forward_td(fdtd_grid *g, float *fields, const float *inv_eps
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "fdtd_forward launch");
-    if (recording) g->recorded_steps = n_steps;
+    g->fwd_pos = n_end;
+    g->fwd_fused = fused_call;
+    if (recording && n_end == n_total) g->recorded_steps = n_steps;
     return FDTD_OK;
 }
 
@@ -655,6 +715,13 @@ extern "C" int fdtd_backward(fdtd_grid *g, float *fields, const float *inv_eps, 
                             n_steps, dL_dinv_eps, dL_dfields0, cuda_stream);
 }
 
+static int backward_impl(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
+                         const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
+                         const float *const *dL_dphasor,
+                         const fdtd_time_detector *td, int32_t n_td, const float *const *dL_dtd,
+                         const float *dL_dfields, int n_hi, int n_lo, int n_total, float *dL_dinv_eps, float *dL_dfields0,
+                         void *cuda_stream);
+
 extern "C" int fdtd_backward_td(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
                                 const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
                                 const float *const *dL_dphasor,
@@ -662,6 +729,33 @@ extern "C" int fdtd_backward_td(fdtd_grid *g, float *fields, const float *inv_ep
                                 const float *dL_dfields, int32_t n_steps, float *dL_dinv_eps, float *dL_dfields0,
                                 void *cuda_stream)
 {
+    return backward_impl(g, fields, inv_eps, inv_mu, src, n_src, det, n_det, dL_dphasor, td, n_td, dL_dtd, dL_dfields,
+                         n_steps, 0, n_steps, dL_dinv_eps, dL_dfields0, cuda_stream);
+}
+
+extern "C" int fdtd_backward_range(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
+                                   const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
+                                   const float *const *dL_dphasor, const float *dL_dfields,
+                                   int32_t n_hi, int32_t n_lo, int32_t n_total, float *dL_dinv_eps, float *dL_dfields0,
+                                   void *cuda_stream)
+{
+    if (n_lo < 0 || n_hi < n_lo || n_total < n_hi) return fail(FDTD_EINVAL, "fdtd_backward_range: need 0 <= n_lo <= n_hi <= n_total");
+    if (g && n_hi != n_total && g->bwd_pos != n_hi) return fail(FDTD_ESTATE, "fdtd_backward_range: n_hi does not continue the previous range");
+    return backward_impl(g, fields, inv_eps, inv_mu, src, n_src, det, n_det, dL_dphasor, nullptr, 0, nullptr, dL_dfields,
+                         n_hi, n_lo, n_total, dL_dinv_eps, dL_dfields0, cuda_stream);
+}
+
+// reverse steps n_hi-1 .. n_lo of a run of n_total steps (fdtd_backward: n_steps-1 .. 0); the cotangent seed (B0) is
+// placed by the call with n_hi == n_total, dL_dfields0 is written by the call with n_lo == 0
+static int backward_impl(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
+                         const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
+                         const float *const *dL_dphasor,
+                         const fdtd_time_detector *td, int32_t n_td, const float *const *dL_dtd,
+                         const float *dL_dfields, int n_hi, int n_lo, int n_total, float *dL_dinv_eps, float *dL_dfields0,
+                         void *cuda_stream)
+{
+    const int n_steps = n_total;
+    const bool first = n_hi == n_total, last = n_lo == 0;
     int rc = check_common(g, fields, inv_eps, src, n_src, det, n_det, n_steps, "fdtd_backward");
     if (rc) return rc;
     if (!dL_dinv_eps && !dL_dfields0) return fail(FDTD_EINVAL, "fdtd_backward: dL_dinv_eps or dL_dfields0 is required");
@@ -694,20 +788,24 @@ extern "C" int fdtd_backward_td(fdtd_grid *g, float *fields, const float *inv_ep
 
     // B0: seed cotangents
     const size_t vol = (size_t)G.nc * sizeof(float);
-    if (dL_dfields) CK(cudaMemcpyAsync(g->lam, dL_dfields, 6 * vol, cudaMemcpyDeviceToDevice, st));
-    else            CK(cudaMemsetAsync(g->lam, 0, 6 * vol, st));
-    for (int q = 0; q < 2; ++q)
-        if ((rc = g->zero_psi(g->lpsiE[q], st)) || (rc = g->zero_psi(g->lpsiH[q], st))) return rc;
-    if (dL_dinv_eps) CK(cudaMemsetAsync(dL_dinv_eps, 0, vol, st));
-    launch_set_step(g->d_step, std::max(n_steps - 1, 0), st);   // the first reverse step reads slot 0
+    g->bwd_pos = -1;
+    if (first) {
+        if (dL_dfields) CK(cudaMemcpyAsync(g->lam, dL_dfields, 6 * vol, cudaMemcpyDeviceToDevice, st));
+        else            CK(cudaMemsetAsync(g->lam, 0, 6 * vol, st));
+        for (int q = 0; q < 2; ++q)
+            if ((rc = g->zero_psi(g->lpsiE[q], st)) || (rc = g->zero_psi(g->lpsiH[q], st))) return rc;
+        if (dL_dinv_eps) CK(cudaMemsetAsync(dL_dinv_eps, 0, vol, st));
+    }
+    launch_set_step(g->d_step, std::max(n_hi - 1, 0), st);      // the first reverse step of the call reads slot 0
     const bool want_grad = dL_dinv_eps != nullptr;              // false: adjoint sweep only (B1, B2, B5)
+    const bool fused_call = g->path == FDTD_PATH_FUSED && g->fused_backward_ready;
 
-    if (g->path == FDTD_PATH_FUSED && g->fused_backward_ready) {
+    if (fused_call) {
         // seeded_H: the H part of the seed can be non-zero (it is scaled by inv_mu for the sweep)
-        rc = fused_backward(g, fields, inv_eps, inv_mu, S, D, TD, total_freq, n_steps, dL_dinv_eps, dL_dfields != nullptr, st);
+        rc = fused_backward(g, fields, inv_eps, inv_mu, S, D, TD, total_freq, n_hi, n_lo, n_total, dL_dinv_eps, dL_dfields != nullptr, st);
         if (rc) return rc;
         // the fused sweep carried im lamH in the H part (kernels_step.cu); the cotangent of state 0 is lamH
-        if (inv_mu && dL_dfields0) launch_scale_H(G, g->lam, inv_mu, true, st);
+        if (last && inv_mu && dL_dfields0) launch_scale_H(G, g->lam, inv_mu, true, st);
     } else {
         int n_adj = 0;
         for (const DetectorDev &dt : D) if (dt.phasor) ++n_adj;
@@ -715,7 +813,7 @@ extern "C" int fdtd_backward_td(fdtd_grid *g, float *fields, const float *inv_ep
         std::string key = make_key("gb", fields, inv_eps, inv_mu, g->rec, dL_dinv_eps, S, D, 0);
         key.append((const char *)&g->d_cs, sizeof(g->d_cs));
         if (!TD.empty()) key.append((const char *)TD.data(), TD.size() * sizeof(TimeDetDev));
-        rc = run_steps(g, g->bwd_graph, key, n_steps, launches, st, [&](cudaStream_t cs) {
+        rc = run_steps(g, g->bwd_graph, key, n_hi - n_lo, launches, st, [&](cudaStream_t cs) {
             { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
               // N2 transposes first: they act on the state after step n, before anything of reverse step n
               for (const TimeDetDev &q : TD)
@@ -736,9 +834,11 @@ extern "C" int fdtd_backward_td(fdtd_grid *g, float *fields, const float *inv_ep
         });
         if (rc) return rc;
     }
-    if (dL_dfields0) CK(cudaMemcpyAsync(dL_dfields0, g->lam, 6 * vol, cudaMemcpyDeviceToDevice, st));
+    if (last && dL_dfields0) CK(cudaMemcpyAsync(dL_dfields0, g->lam, 6 * vol, cudaMemcpyDeviceToDevice, st));
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "fdtd_backward launch");
+    g->bwd_pos = n_lo;
+    g->bwd_fused = fused_call;
     return FDTD_OK;
 }
 
@@ -751,6 +851,52 @@ extern "C" int fdtd_grad_rho(fdtd_grid *g, const float *dL_dinv_eps, const float
     g->kernel_launches += 1;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "fdtd_grad_rho launch");
+    return FDTD_OK;
+}
+
+// ================================================================================================
+// N3: halo planes of a z-slab sub-grid (include/fdtd.h "Domain decomposition")
+// ================================================================================================
+namespace {
+// volume that holds state n: primal (which = 0) or cotangents (which = 1)
+int halo_volume(fdtd_grid *g, float *fields, int which, int n, float **vol, const char *who)
+{
+    if (!g) return fail(FDTD_EINVAL, std::string(who) + ": NULL grid");
+    if (which != 0 && which != 1) return fail(FDTD_EINVAL, std::string(who) + ": which must be 0 (fields) or 1 (cotangents)");
+    if (which == 0 && !fields) return fail(FDTD_EINVAL, std::string(who) + ": fields is NULL");
+    if (which == 1 && !g->lam) return fail(FDTD_ESTATE, std::string(who) + ": no cotangent volumes yet (call fdtd_backward_range first)");
+    const bool fused = which == 0 ? g->fwd_fused : g->bwd_fused;
+    *vol = fused ? fused_volume(g, fields, which, n) : (which == 0 ? fields : g->lam);
+    return FDTD_OK;
+}
+}  // namespace
+
+extern "C" int fdtd_halo_export(fdtd_grid *g, float *fields, int32_t which, int32_t n, int32_t side, float *out, void *cuda_stream)
+{
+    float *vol = nullptr;
+    int rc = halo_volume(g, fields, which, n, &vol, "fdtd_halo_export");
+    if (rc) return rc;
+    if (!out || (side != 0 && side != 1)) return fail(FDTD_EINVAL, "fdtd_halo_export: bad argument");
+    const Dims &G = g->G;
+    const int k = side ? G.nz - 1 - g->desc.z_ghost_hi : g->desc.z_ghost_lo;        // highest / lowest owned plane
+    const size_t plane = (size_t)G.nx * G.ny;
+    for (int c = 0; c < 3; ++c)
+        CK(cudaMemcpyAsync(out + c * plane, vol + (3 + c) * G.nc + (size_t)k * plane, plane * sizeof(float), cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
+    return FDTD_OK;
+}
+
+extern "C" int fdtd_halo_import(fdtd_grid *g, float *fields, int32_t which, int32_t n, int32_t side, const float *in, void *cuda_stream)
+{
+    float *vol = nullptr;
+    int rc = halo_volume(g, fields, which, n, &vol, "fdtd_halo_import");
+    if (rc) return rc;
+    if (!in || (side != 0 && side != 1)) return fail(FDTD_EINVAL, "fdtd_halo_import: bad argument");
+    if (side ? !g->desc.z_ghost_hi : !g->desc.z_ghost_lo) return fail(FDTD_EINVAL, "fdtd_halo_import: the grid has no ghost plane on that side");
+    const Dims &G = g->G;
+    const int k = side ? G.nz - 1 : 0;
+    const size_t plane = (size_t)G.nx * G.ny;
+    for (int c = 0; c < 3; ++c)
+        CK(cudaMemcpyAsync(vol + (3 + c) * G.nc + (size_t)k * plane, in + c * plane, plane * sizeof(float), cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
     return FDTD_OK;
 }
 

@@ -36,9 +36,12 @@ struct fdtd_grid {
     float *lam = nullptr;                  // cotangent fields [6][nz][ny][nx]
     float *rec = nullptr;                  // interface recorder
     int recorded_steps = -1;               // n_steps of the last recorded forward, or -1
+    int fwd_pos = -1, bwd_pos = -1;        // fdtd_forward_range / fdtd_backward_range: the state index the last call left
+    bool fwd_fused = false, bwd_fused = false;   // which kernels the last (range) call ran on: where its state lives
     float *d_cs = nullptr;                 // per-step (cos, sin) table
     float *h_cs = nullptr;                 // pinned staging of the same
     size_t cs_cap = 0;
+    std::vector<float> cs_key;             // n_steps and the frequencies of the table on the device
     cudaEvent_t table_done = nullptr;
     fdtd::ReduceScratch red{};             // block partials + ticket of the N2 reductions (energy, flux)
 
@@ -96,11 +99,14 @@ void fused_teardown(fdtd_grid *g);
 int fused_alloc_backward(fdtd_grid *g);    // second cotangent volume of the ping-pong
 int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
                   const std::vector<fdtd::SourceDev> &S, const std::vector<fdtd::DetectorDev> &D,
-                  const std::vector<fdtd::TimeDetDev> &TD, int total_freq, int n_steps, bool recording, cudaStream_t st);
+                  const std::vector<fdtd::TimeDetDev> &TD, int total_freq, int n_begin, int n_end, int n_total, bool recording,
+                  cudaStream_t st);
 int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
                    const std::vector<fdtd::SourceDev> &S, const std::vector<fdtd::DetectorDev> &D,
-                   const std::vector<fdtd::TimeDetDev> &TD, int total_freq, int n_steps, float *dL_dinv_eps, bool seeded_H,
-                   cudaStream_t st);
+                   const std::vector<fdtd::TimeDetDev> &TD, int total_freq, int n_hi, int n_lo, int n_total, float *dL_dinv_eps,
+                   bool seeded_H, cudaStream_t st);
+// the volume that holds state n of the fused path's ping-pong: which = 0 primal (fields / second buffer), 1 cotangents
+float *fused_volume(fdtd_grid *g, float *fields, int which, int n);
 
 // RAII span: brackets the launches made in its lifetime with two events when profiling is on
 struct ProfScope {

@@ -20,7 +20,20 @@ struct Dims {
     long long nc;     // cells
     int lo[3], hi[3]; // interior box I
     int glo[3], ghi[3]; // gradient box (already clipped to I)
+    // z-slab sub-grid: the local planes are global planes [zoff, zoff + nz) of a grid of nzg
+    // planes; zl / zh = how many of the first / last local planes lie in the global low / high z CPML slab (d / d on
+    // an ordinary grid).  CPML tables are stored per local plane; the z-slab psi arrays keep 2 d planes.
+    int zoff, nzg, zl, zh;
 };
+
+// slab-compact plane of local plane k in a z-slab psi array ([0, zl) low slab, [2 d - zh, 2 d) high slab), or -1
+__host__ __device__ inline int zslab_pos(const Dims &G, int k)
+{
+    if (k < 0 || k >= G.nz) return -1;
+    if (k < G.zl) return k;
+    if (k >= G.nz - G.zh) return 2 * G.d - G.zh + (k - (G.nz - G.zh));
+    return -1;
+}
 
 // CPML tables on the device: [family 0=E 1=H][axis] -> pointer to N_axis floats
 struct Tables {
@@ -59,8 +72,8 @@ __host__ __device__ inline long long psi_index(const Dims &G, int axis, int i, i
         if (j < G.d) s = j; else if (j >= G.ny - G.d) s = j - (G.ny - 2 * G.d); else return -1;
         return ((long long)k * (2 * G.d) + s) * G.nx + i;
     } else {
-        int s;
-        if (k < G.d) s = k; else if (k >= G.nz - G.d) s = k - (G.nz - 2 * G.d); else return -1;
+        const int s = zslab_pos(G, k);
+        if (s < 0) return -1;
         return ((long long)s * G.ny + j) * G.nx + i;
     }
 }

@@ -315,7 +315,8 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
         const int ax = q < YO ? 0 : (q < ZO ? 1 : 2);
         const int sc = q - (ax == 0 ? 0 : (ax == 1 ? YO : ZO));
         const int w = ax == 0 ? G.dpx : G.d, N = ax == 0 ? G.nx : (ax == 1 ? G.ny : G.nz);
-        const int pos = sc < w ? sc : N - 2 * w + sc;
+        // (on a z-slab sub-grid the entries between the zl low and the zh high planes are never read: clamp)
+        const int pos = min(max(sc < w ? sc : N - 2 * w + sc, 0), N - 1);
         const float *src = kind == 0 ? P.T.b[fam][ax] : (kind == 1 ? P.T.a[fam][ax] : P.T.ik[fam][ax]);
         tabs[e] = __ldg(src + pos) - (kind == 2 ? 1.f : 0.f);
     }
@@ -403,6 +404,9 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
     int pv_i = 0;                 // the stage that holds the previous plane
     uint32_t pv_off = 0;
     float4 cgx = Z4, cgy = Z4, cZx = Z4, cZy = Z4;   // adjoint: z-filtered operands of the previous plane at my cells
+    // forward: F of the previous plane at my cells (= the H-type target of phase B) travels in registers, so a stage is
+    // released as soon as its own plane is done and the ring of NST stages keeps one more plane in flight
+    float4 pFx = Z4, pFy = Z4, pFz = Z4;
     for (int sg = seg_lo; sg < seg_hi; ++sg) {
         const Segment Sg = segs[sg];
         const int i = Sg.i0 + 4 * tx, j = Sg.j0 + ty;
@@ -422,7 +426,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
 
         // ---------------------------------------------------------------- one plane (phase A of kk, phase B of kk-1)
         auto plane_step = [&](const int kk, const bool doB) {
-            const int zs = (pml && !DBG(128)) ? slab_pos(kk, G.nz, G.d) : -1;
+            const int zs = (pml && !DBG(128)) ? zslab_pos(G, kk) : -1;
             mbar_wait(&full[st_i], st_ph);
             const uint32_t so = stage_base + st_off + o_own;
             const uint32_t sp = stage_base + pv_off + o_own;       // the stage of plane kk-1 is still held
@@ -455,14 +459,14 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
             float4 Dx_y = dminus_x(fy, fy_mx), Dx_z = dminus_x(fz, fz_mx);
             float4 Dz_x, Dz_y;
             if (pml && ing) {
-                const int zs2 = slab_pos(kk + FDTD_PF_DIST, G.nz, G.d);
+                const int zs2 = zslab_pos(G, kk + FDTD_PF_DIST);
                 if (zs2 >= 0) {
                     const int q = zs2 * pz + own_xy;
                     pf_l2(qAi.p[1][0] + q); pf_l2(qAi.p[0][1] + q); pf_l2(qBi.p[1][0] + q); pf_l2(qBi.p[0][1] + q);
                 }
             }
             if (!ADJ) {
-                Dz_x = fx - lds4(sp); Dz_y = fy - lds4(sp + C::SLOT);
+                Dz_x = fx - pFx; Dz_y = fy - pFy;
                 if (slab_xy || zs >= 0) {
                     if (zs >= 0 && ing) {
                         const float b = TB1(FA, 0, ZO + zs), a = TB1(FA, 1, ZO + zs), km = TB1(FA, 2, ZO + zs);
@@ -604,7 +608,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                 float4 Dz_y = Zy - (ADJ ? cZy : oXy), Dz_x = Zx - (ADJ ? cZx : oYx);
                 float4 Dx_z = dplus_x(oXz, Xz_px), Dx_y = dplus_x(oXy, Xy_px);
                 const int offm = off - plane;
-                const int zsm = (!ADJ && pml && !DBG(128)) ? slab_pos(km1, G.nz, G.d) : -1;
+                const int zsm = (!ADJ && pml && !DBG(128)) ? zslab_pos(G, km1) : -1;
                 if (!ADJ && (slab_xy || zsm >= 0)) {
                     if (zsm >= 0) {
                         const float b = TB1(FB, 0, ZO + zsm), a = TB1(FB, 1, ZO + zsm), km = TB1(FB, 2, ZO + zsm);
@@ -633,7 +637,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                     }
                 }
                 const float4 tHx = Dy_z - Dz_y, tHy = Dz_x - Dx_z, tHz = Dx_y - Dy_x;
-                const float4 hx = lds4(sp), hy = lds4(sp + C::SLOT), hz = lds4(sp + 2 * C::SLOT);
+                const float4 hx = ADJ ? lds4(sp) : pFx, hy = ADJ ? lds4(sp + C::SLOT) : pFy, hz = ADJ ? lds4(sp + 2 * C::SLOT) : pFz;
                 float4 h2x, h2y, h2z;
                 if (ADJ) {
                     // with inv_mu the H part of the cotangent volumes holds Lambda_H = im lamH (fused_backward): phase A
@@ -654,10 +658,11 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                 stg4(o, h2x); stg4(o + nc, h2y); stg4(o + 2 * nc, h2z);
                 if (!ADJ && km1 >= P.dHl && km1 < P.dHh) detect4(P, n, 1, det_mask(P, km1, false), h2x, h2y, h2z, i, j, km1);
             }
-            if (ADJ) { cZx = Zx; cZy = Zy; }
-            // the stage of plane kk-1 is no longer needed; the stage of plane kk stays for the next iteration
+            if (ADJ) { cZx = Zx; cZy = Zy; } else { pFx = fx; pFy = fy; pFz = fz; }
+            // adjoint: the stage of plane kk-1 is no longer needed, the stage of plane kk stays for the next iteration;
+            // forward: nothing of plane kk is read from its stage again
             __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[pv_i]);
+            if (lane == 0) mbar_arrive(&empty[ADJ ? pv_i : st_i]);
             pv_i = st_i; pv_off = st_off;
             st_off += P.stage;
             if (++st_i == nst) { st_i = 0; st_off = 0; st_ph ^= 1; }
@@ -672,7 +677,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                 const uint32_t so = stage_base + st_off + o_own;
                 cgx = lds4(so); cgy = lds4(so + C::SLOT);
                 if (pml) {
-                    const int zs = slab_pos(kk, G.nz, G.d);
+                    const int zs = zslab_pos(G, kk);
                     if (zs >= 0 && ing) {
                         const float b = TB1(FA, 0, ZO + zs), a = TB1(FA, 1, ZO + zs), km = TB1(FA, 2, ZO + zs);
                         const int oz = zs * pz + own_xy;
@@ -682,14 +687,22 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                     }
                 }
             }
+            if (!ADJ) {
+                const uint32_t so = stage_base + st_off + o_own;
+                pFx = lds4(so); pFy = lds4(so + C::SLOT); pFz = lds4(so + 2 * C::SLOT);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty[st_i]);
+            }
             pv_i = st_i; pv_off = st_off;
             st_off += P.stage;
             if (++st_i == nst) { st_i = 0; st_off = 0; st_ph ^= 1; }
         }
         plane_step(Sg.k0, false);
         for (int kk = Sg.k0 + 1; kk <= k1; ++kk) plane_step(kk, true);
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&empty[pv_i]);      // the stage of plane k1
+        if (ADJ) {
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[pv_i]);      // the stage of plane k1
+        }
     }
     if (P.dbg_t && threadIdx.x == 0) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); P.dbg_t[2 * blockIdx.x + 1] = t; }
 }
@@ -1809,14 +1822,17 @@ void enqueue_bwd(void *vctx, cudaStream_t cs)
 
 int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
                   const std::vector<SourceDev> &S, const std::vector<DetectorDev> &D, const std::vector<TimeDetDev> &TD,
-                  int total_freq, int n_steps, bool recording, cudaStream_t st)
+                  int total_freq, int n_begin, int n_end, int n_total, bool recording, cudaStream_t st)
 {
+    // steps n_begin .. n_end-1 of a run of n_total; state n lives in volume n&1 (0: fields, 1: the grid's copy) between
+    // the calls of a range sequence and is brought back to `fields` by the call that ends the run
+    const int n_steps = n_total, n_count = n_end - n_begin;
     FusedState *F = g->fused;
     if ((int)S.size() > MAX_SRC || (int)D.size() > MAX_DET)
         return fdtd_fail(FDTD_EINVAL, "the fused path takes at most 4 sources and 4 detectors (use FDTD_PATH_GENERIC)");
     int rc = build_maps(g, 0, fields, F->bufB, inv_eps, st);
     if (rc) return rc;
-    for (int q = 0; q < 2; ++q)
+    for (int q = 0; q < 2 && n_begin == 0; ++q)
         if ((rc = g->zero_psi(g->psiE[q], st)) || (rc = g->zero_psi(g->psiH[q], st))) return rc;
     FwdCtx ctx{ g, F->sp, recording, fields, F->bufB, n_steps, &TD, inv_eps, inv_mu };
     StepParams &P = ctx.P;
@@ -1842,11 +1858,12 @@ int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float
     key.push_back(recording ? 1 : 0);
     key.append((const char *)&n_steps, recording ? sizeof(n_steps) : 0);
     if (!TD.empty()) key.append((const char *)TD.data(), TD.size() * sizeof(TimeDetDev));
-    rc = fdtd_run_steps_fwd(g, key, n_steps, 1 + (recording ? 1 : 0) + (int)TD.size(), st, enqueue_fwd, &ctx);
+    rc = fdtd_run_steps_fwd(g, key, n_count, 1 + (recording ? 1 : 0) + (int)TD.size(), st, enqueue_fwd, &ctx);
     if (rc) return rc;
-    if (recording) {      // E' of the last step; step p read counter slot p&1, so the count n_steps sits in slot n_steps&1
+    if (n_end != n_total) return FDTD_OK;
+    if (recording) {      // E' of the last step; the p-th step of the call read counter slot p&1, so the count sits in slot n_count&1
         ProfScope p(g, fdtd_grid::PC_RECORD, st);
-        launch_record_pipe(g->G, g->R, fields, F->bufB, g->rec, g->d_step + (n_steps & 1), n_steps, st);
+        launch_record_pipe(g->G, g->R, fields, F->bufB, g->rec, g->d_step + (n_count & 1), n_steps, st);
         g->kernel_launches += 1;
     }
     if (n_steps & 1) {
@@ -1860,16 +1877,21 @@ int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float
 // result is back in volume 0 = g->lam.
 int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
                    const std::vector<SourceDev> &S, const std::vector<DetectorDev> &D, const std::vector<TimeDetDev> &TD,
-                   int total_freq, int n_steps, float *dL_dinv_eps, bool seeded_H, cudaStream_t st)
+                   int total_freq, int n_hi, int n_lo, int n_total, float *dL_dinv_eps, bool seeded_H, cudaStream_t st)
 {
+    // reverse steps n_hi-1 .. n_lo of a run of n_total (fdtd_backward: n_steps-1 .. 0).  Between the calls of a range
+    // sequence the cotangents after reverse step n live in volume n&1 (0: g->lam) and the reconstructed state n in
+    // primal volume n&1 (0: fields); the seed and state n_total are placed by the call that starts at n_total.
+    const int n_steps = n_total, n_count = n_hi - n_lo;
+    const bool first = n_hi == n_total, whole = first && n_lo == 0;
     FusedState *F = g->fused;
     const size_t vol6 = (size_t)g->G.nc * 6 * sizeof(float);
     int rc;
     if ((rc = fused_alloc_backward(g))) return rc;
     if ((rc = build_maps(g, 1, g->lam, F->lamB, inv_eps, st))) return rc;
     // with inv_mu the sweep runs on Lambda_H = im lamH (see k_step); fdtd_backward scales the result back
-    if (inv_mu && seeded_H) launch_scale_H(g->G, g->lam, inv_mu, false, st);
-    if (n_steps & 1) {
+    if (first && inv_mu && seeded_H) launch_scale_H(g->G, g->lam, inv_mu, false, st);
+    if (first && (n_steps & 1)) {
         cudaError_t e = cudaMemcpyAsync(F->lamB, g->lam, vol6, cudaMemcpyDeviceToDevice, st);
         if (e != cudaSuccess) { (void)cudaGetLastError(); return fdtd_fail(FDTD_ECUDA, cudaGetErrorString(e)); }
     }
@@ -1880,12 +1902,12 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     for (const DetectorDev &dt : D) if (dt.phasor && (dt.mask >> 3)) fused_det = false;
     // while profiling (events around every launch) the kernels run one after the other, so each is timed alone
     // (time-domain detector transposes read the primal state after step n, which the pipelined sweep is still writing)
-    const bool pipelined = fused_inv && fused_det && F->n_inv_p > 0 && !g->profiling && TD.empty();
+    const bool pipelined = fused_inv && fused_det && F->n_inv_p > 0 && !g->profiling && TD.empty() && whole;
     BwdCtx ctx{ g, F->sp, F->ip, fused_inv, fused_det, pipelined, want_grad, F->bufB, fields, inv_eps, inv_mu, dL_dinv_eps, g->lam, F->lamB, &S, &D, total_freq, &TD };
     if (fused_inv) {
         // reverse step n reads primal volume (n+1)&1 and writes n&1: state n_steps must sit in volume n_steps&1
         if ((rc = build_inv_maps(g, fields, F->bufB, inv_eps, g->lam, F->lamB, st))) return rc;
-        if (n_steps & 1) {
+        if (first && (n_steps & 1)) {
             cudaError_t e = cudaMemcpyAsync(F->bufB, fields, vol6, cudaMemcpyDeviceToDevice, st);
             if (e != cudaSuccess) { (void)cudaGetLastError(); return fdtd_fail(FDTD_ECUDA, cudaGetErrorString(e)); }
         }
@@ -1930,7 +1952,7 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     const int n_inj = g->G.d > 0 ? 1 : 0;
     const int launches = (int)TD.size() + (!want_grad ? 1 + (fused_det ? 0 : n_adj)
                          : (fused_inv ? 2 + (fused_det ? 0 : n_adj) + n_inj : 3 + (fused_det ? 0 : n_adj) + (int)S.size() + n_inj));
-    rc = fdtd_run_steps_bwd(g, key, n_steps, launches, st, enqueue_bwd, &ctx);
+    rc = fdtd_run_steps_bwd(g, key, n_count, launches, st, enqueue_bwd, &ctx);
     if (rc || !pipelined) return rc;
     // inverse step 0 on every SM; reverse step p read counter slot p&1 (p counted from the end), so -1 sits in slot n_steps&1
     InvParams J = ctx.I;
@@ -1940,4 +1962,11 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     g->kernel_launches += 1;
     g->fused_inverse_launches += 1;
     return FDTD_OK;
+}
+
+float *fused_volume(fdtd_grid *g, float *fields, int which, int n)
+{
+    FusedState *F = g->fused;
+    if (which == 0) return (n & 1) ? F->bufB : fields;
+    return (n & 1) ? F->lamB : g->lam;
 }

@@ -24,3 +24,231 @@ def max_over_ranks(ms_local: float, device=None) -> float:
 def whole_job_rate(cells_steps_per_rank: int, reps: int, ms_max: float, world: int) -> float:
     """Mcells/s summed over ranks: every rank processed cells_steps_per_rank * reps cell updates in ms_max."""
     return world * cells_steps_per_rank * reps / (ms_max * 1e-3) / 1e6
+
+
+# --------------------------------------------------------------------------------------------------------------
+# Domain decomposition of ONE grid into z slabs (SURVEY 8(e), 8(f) N3; include/fdtd.h "Domain decomposition";
+# PAPER.md L116-118).  Host logic only: which planes a rank holds, how the inputs are cut, which planes travel.
+# --------------------------------------------------------------------------------------------------------------
+from dataclasses import dataclass, replace as _replace
+from typing import List, Optional, Sequence, Tuple
+
+
+@dataclass(frozen=True)
+class ZSlab:
+    """Planes of rank `rank` of `world`: owns [k_lo, k_hi), stores [z_offset, z_offset + nz) (one ghost plane per cut)."""
+    rank: int
+    world: int
+    nz_global: int
+    k_lo: int
+    k_hi: int
+
+    @property
+    def ghost_lo(self) -> int:
+        return 0 if self.k_lo == 0 else 1
+
+    @property
+    def ghost_hi(self) -> int:
+        return 0 if self.k_hi == self.nz_global else 1
+
+    @property
+    def z_offset(self) -> int:
+        return self.k_lo - self.ghost_lo
+
+    @property
+    def nz(self) -> int:
+        return self.k_hi - self.k_lo + self.ghost_lo + self.ghost_hi
+
+    def grid_kwargs(self) -> dict:
+        return dict(nz=self.nz, z_global=self.nz_global, z_offset=self.z_offset, z_ghost_lo=self.ghost_lo, z_ghost_hi=self.ghost_hi)
+
+    def local_planes(self) -> slice:
+        return slice(self.z_offset, self.z_offset + self.nz)
+
+    def owned_local(self) -> slice:
+        """The owned planes in local indices."""
+        return slice(self.ghost_lo, self.nz - self.ghost_hi)
+
+
+def z_slabs(nz_global: int, world: int, pml_cells: int = 0, cuts: Optional[Sequence[int]] = None) -> List[ZSlab]:
+    """Cuts [0, nz_global) into `world` slabs of (nearly) equal plane counts, or at the given cut planes.  Every slab
+    must own at least one plane of the interior [pml_cells, nz_global - pml_cells)."""
+    if cuts is None:
+        cuts = [round(nz_global * r / world) for r in range(1, world)]
+    edges = [0, *cuts, nz_global]
+    if len(edges) != world + 1 or any(b <= a for a, b in zip(edges, edges[1:])):
+        raise ValueError(f"bad cuts {cuts} for {world} slabs of {nz_global} planes")
+    slabs = [ZSlab(r, world, nz_global, edges[r], edges[r + 1]) for r in range(world)]
+    for s in slabs:
+        if min(s.k_hi, nz_global - pml_cells) <= max(s.k_lo, pml_cells):
+            raise ValueError(f"slab {s.rank} owns no interior plane")
+    return slabs
+
+
+def _clip_box(lo, hi, k0: int, k1: int, shift: int):
+    """Box (lo, hi) clipped to global planes [k0, k1) and shifted to local plane indices; None if empty."""
+    a, b = max(lo[2], k0), min(hi[2], k1)
+    if b <= a:
+        return None
+    return (lo[0], lo[1], a - shift), (hi[0], hi[1], b - shift), (a - lo[2], b - lo[2])
+
+
+def local_sources(sources, slab: ZSlab):
+    """Sources clipped to the local planes (ghosts included: the E replica on the ghost plane above needs them)."""
+    out = []
+    for s in sources:
+        c = _clip_box(s.lo, s.hi, slab.z_offset, slab.z_offset + slab.nz, slab.z_offset)
+        if c is None:
+            continue
+        lo, hi, (a, b) = c
+        prof = None if s.profile is None else s.profile[a:b]
+        out.append(_replace(s, lo=lo, hi=hi, profile=prof))
+    return out
+
+
+def local_detectors(detectors, slab: ZSlab, with_ghosts: bool):
+    """[(index of the global detector, local detector, slice of its box planes)]: clipped to the owned planes
+    (forward) or to all local planes (backward: the cotangent injection must reach the ghost planes too)."""
+    k0, k1 = (slab.z_offset, slab.z_offset + slab.nz) if with_ghosts else (slab.k_lo, slab.k_hi)
+    out = []
+    for idx, d in enumerate(detectors):
+        c = _clip_box(d.lo, d.hi, k0, k1, slab.z_offset)
+        if c is None:
+            continue
+        lo, hi, (a, b) = c
+        out.append((idx, _replace(d, lo=lo, hi=hi), slice(a, b)))
+    return out
+
+
+def exchange_halos_dist(slab: ZSlab, send_down, send_up, recv_below, recv_above, group=None):
+    """One halo exchange over torch.distributed point-to-point (NCCL on GPU tensors, gloo on CPU tensors):
+    my lowest owned plane goes to rank-1 (its ghost above), my highest owned plane to rank+1 (its ghost below)."""
+    ops = []
+    if slab.ghost_lo:
+        ops.append(dist.P2POp(dist.isend, send_down, slab.rank - 1, group))
+        ops.append(dist.P2POp(dist.irecv, recv_below, slab.rank - 1, group))
+    if slab.ghost_hi:
+        ops.append(dist.P2POp(dist.isend, send_up, slab.rank + 1, group))
+        ops.append(dist.P2POp(dist.irecv, recv_above, slab.rank + 1, group))
+    if ops:
+        for req in dist.batch_isend_irecv(ops):
+            req.wait()
+
+
+class SlabRunner:
+    """One z slab of a workload on the current CUDA device: the local grid, the local slices of the inputs and the halo
+    buffers.  Marshalling only -- every step runs in the library (fdtd_forward_range / fdtd_backward_range /
+    fdtd_halo_export / fdtd_halo_import)."""
+
+    def __init__(self, B, w, slab: ZSlab, n_total: int, record: int = 1, path=None, flags: int = 0):
+        import numpy as np
+        self.B, self.w, self.slab, self.n_total = B, w, slab, n_total
+        t = self.torch = torch
+        kw = w.grid_kwargs()
+        kw.update(slab.grid_kwargs())
+        kw.update(max_steps=n_total, record=record if w.pml_cells > 0 else 0, flags=flags)
+        if path is not None:
+            kw.update(path=path)
+        self.grid = B.Grid(**kw)
+        zs = slab.local_planes()
+        self.ie = t.as_tensor(np.ascontiguousarray(w.inv_eps[zs])).cuda()
+        im = w.meta.get("inv_mu")
+        self.im = None if im is None else t.as_tensor(np.ascontiguousarray(im[zs])).cuda()
+        self.fields = t.zeros((6, slab.nz, w.ny, w.nx), dtype=t.float32, device="cuda")
+        self.sources = local_sources(w.sources, slab)
+        self.det_fwd = local_detectors(w.detectors, slab, with_ghosts=False)
+        self.det_bwd = local_detectors(w.detectors, slab, with_ghosts=True)
+        self.phasors = [t.zeros(d.phasor_shape, dtype=t.float32, device="cuda") for _, d, _ in self.det_fwd]
+        g = self.grid
+        self.sarr, self.ns, self._k1 = g.marshal_sources(self.sources)
+        self.darr, self.nd, self._k2 = g.marshal_detectors([d for _, d, _ in self.det_fwd], self.phasors)
+        self.darr_b, self.nd_b, self._k3 = g.marshal_detectors([d for _, d, _ in self.det_bwd], None)
+        plane = (3, w.ny, w.nx)
+        self.send_down, self.send_up = t.empty(plane, device="cuda"), t.empty(plane, device="cuda")
+        self.recv_below, self.recv_above = t.empty(plane, device="cuda"), t.empty(plane, device="cuda")
+        self.grad = self.lam0 = self._cot = self._dLf = None
+
+    def close(self):
+        self.grid.close()
+
+    # ---- forward ------------------------------------------------------------------------------------------
+    def forward_steps(self, n_begin: int, n_end: int):
+        self.B.fdtd_forward_range(self.grid.h, self.fields, self.ie, self.im, self.sarr, self.ns, self.darr, self.nd,
+                                  n_begin, n_end, self.n_total, self.grid.stream())
+
+    def export_halos(self, which: int, n: int):
+        B, g = self.B, self.grid
+        if self.slab.ghost_lo:
+            B.fdtd_halo_export(g.h, self.fields, which, n, 0, self.send_down, g.stream())
+        if self.slab.ghost_hi:
+            B.fdtd_halo_export(g.h, self.fields, which, n, 1, self.send_up, g.stream())
+
+    def import_halos(self, which: int, n: int, from_below=None, from_above=None):
+        B, g = self.B, self.grid
+        if self.slab.ghost_lo:
+            B.fdtd_halo_import(g.h, self.fields, which, n, 0, self.recv_below if from_below is None else from_below, g.stream())
+        if self.slab.ghost_hi:
+            B.fdtd_halo_import(g.h, self.fields, which, n, 1, self.recv_above if from_above is None else from_above, g.stream())
+
+    # ---- backward -----------------------------------------------------------------------------------------
+    def set_cotangents(self, dL_dphasor_global=None, dL_dfields_global=None):
+        """Cotangents given on the GLOBAL boxes / volume (device tensors); this slab takes its planes, ghosts included."""
+        import ctypes as C
+        t = self.torch
+        self._cot_keep = []
+        cot = (C.c_void_p * max(self.nd_b, 1))()
+        for q, (idx, d, sl) in enumerate(self.det_bwd):
+            G = None if dL_dphasor_global is None else dL_dphasor_global[idx]
+            if G is not None:
+                G = G[:, :, sl].contiguous()
+                self._cot_keep.append(G)
+                cot[q] = G.data_ptr()
+        self._cot = cot
+        self._dLf = None if dL_dfields_global is None else dL_dfields_global[:, self.slab.local_planes()].contiguous()
+        self.grad = t.empty((self.slab.nz, self.w.ny, self.w.nx), dtype=t.float32, device="cuda")
+        self.lam0 = t.empty((6, self.slab.nz, self.w.ny, self.w.nx), dtype=t.float32, device="cuda")
+
+    def backward_steps(self, n_hi: int, n_lo: int, want_grad: bool = True):
+        self.B.fdtd_backward_range(self.grid.h, self.fields, self.ie, self.im, self.sarr, self.ns, self.darr_b, self.nd_b,
+                                   self._cot, self._dLf, n_hi, n_lo, self.n_total, self.grad if want_grad else None,
+                                   self.lam0, self.grid.stream())
+
+
+def run_slabs_lockstep(runners: List["SlabRunner"], n_total: int, direction: str = "forward"):
+    """Advances the slabs of one process in lock step, one exchange per step (the single-device form of the protocol
+    of include/fdtd.h; across processes every rank runs the same loop with exchange_halos_dist in the middle)."""
+    def swap(which, n):
+        for r in runners:
+            r.export_halos(which, n)
+        for q, r in enumerate(runners):
+            r.import_halos(which, n, from_below=runners[q - 1].send_up if r.slab.ghost_lo else None,
+                           from_above=runners[q + 1].send_down if r.slab.ghost_hi else None)
+    if direction == "forward":
+        for n in range(n_total):
+            for r in runners:
+                r.forward_steps(n, n + 1)
+            if n + 1 < n_total:
+                swap(0, n + 1)
+    else:
+        for n in range(n_total - 1, -1, -1):
+            for r in runners:
+                r.backward_steps(n + 1, n)
+            if n > 0:
+                swap(1, n)
+
+
+def run_slab_distributed(runner: "SlabRunner", n_total: int, direction: str = "forward", group=None):
+    """The same loop for one rank of a torch.distributed job (one slab per GPU, NCCL point-to-point)."""
+    which = 0 if direction == "forward" else 1
+    steps = range(n_total) if direction == "forward" else range(n_total - 1, -1, -1)
+    for n in steps:
+        if direction == "forward":
+            runner.forward_steps(n, n + 1)
+            state, more = n + 1, n + 1 < n_total
+        else:
+            runner.backward_steps(n + 1, n)
+            state, more = n, n > 0
+        if more:
+            runner.export_halos(which, state)
+            exchange_halos_dist(runner.slab, runner.send_down, runner.send_up, runner.recv_below, runner.recv_above, group)
+            runner.import_halos(which, state)

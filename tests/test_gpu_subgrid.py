@@ -1,0 +1,113 @@
+"""Domain decomposition along z (include/fdtd.h "Domain decomposition") on ONE
+device: the slabs of a grid advanced in lock step with one halo exchange per step must reproduce the undivided grid
+BIT FOR BIT on the planes they own -- fields, phasors, cotangent of state 0 -- on both kernel paths (the per-cell
+arithmetic does not depend on where a cell sits in its grid).  The gradient agrees to the rounding of the time
+reversal: next to a cut a slab's inverse step reads the RECORDED interface value (the forward run's, exact) where
+the undivided grid reads its own reconstructed neighbour (equal up to the reconstruction's fp32 rounding), so
+dL/d inv_eps differs by a few 1e-8 of its maximum (bound asserted: 1e-6; the oracle tolerance is 1e-3).  The
+undivided grid itself is checked against the oracle in test_gpu_parity.py."""
+import numpy as np
+import pytest
+
+from paper_2412_12360_b200 import sharding, workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device")
+    from paper_2412_12360_b200 import binding
+    return binding
+
+
+def _single(B, w, path, n, dLf_fn=None):
+    import torch
+    kw = w.grid_kwargs()
+    kw.update(max_steps=n, record=1, path=path)
+    g = B.Grid(**kw)
+    f = torch.zeros((6, w.nz, w.ny, w.nx), device="cuda")
+    ie = torch.as_tensor(w.inv_eps).cuda()
+    im = None if w.meta.get("inv_mu") is None else torch.as_tensor(w.meta["inv_mu"]).cuda()
+    ph = g.forward(f, ie, im, w.sources, w.detectors, n)
+    torch.cuda.synchronize()
+    fields = f.cpu().numpy()
+    dLp = [2.0 * P for P in ph]
+    dLf = torch.zeros_like(f)
+    dLf[:3] = 0.5 * f[:3]
+    dLf[3:] = -0.25 * f[3:]
+    grad, lam0 = g.backward(f, ie, im, w.sources, w.detectors, dLp, dLf, n, want_dL_dfields0=True)
+    torch.cuda.synchronize()
+    res = dict(fields=fields, phasors=[p.cpu().numpy() for p in ph], grad=grad.cpu().numpy(), lam0=lam0.cpu().numpy(),
+               dLp=dLp, dLf=dLf, path=g.info().path)
+    g.close()
+    return res
+
+
+def _slabs(B, w, path, n, cuts, ref):
+    import torch
+    slabs = sharding.z_slabs(w.nz, len(cuts) + 1, w.pml_cells, cuts)
+    runners = [sharding.SlabRunner(B, w, s, n, record=1, path=path) for s in slabs]
+    sharding.run_slabs_lockstep(runners, n, "forward")
+    torch.cuda.synchronize()
+    fields = np.zeros_like(ref["fields"])
+    phasors = [np.zeros_like(p) for p in ref["phasors"]]
+    for r in runners:
+        own = r.slab.owned_local()
+        fields[:, r.slab.k_lo:r.slab.k_hi] = r.fields[:, own].cpu().numpy()
+        for (idx, d, sl), P in zip(r.det_fwd, r.phasors):
+            phasors[idx][:, :, sl] = P.cpu().numpy()
+    for r in runners:
+        r.set_cotangents(ref["dLp"], ref["dLf"])
+    sharding.run_slabs_lockstep(runners, n, "backward")
+    torch.cuda.synchronize()
+    grad, lam0 = np.zeros_like(ref["grad"]), np.zeros_like(ref["lam0"])
+    for r in runners:
+        own = r.slab.owned_local()
+        grad[r.slab.k_lo:r.slab.k_hi] = r.grad[own].cpu().numpy()
+        lam0[:, r.slab.k_lo:r.slab.k_hi] = r.lam0[:, own].cpu().numpy()
+    paths = {r.grid.info().path for r in runners}
+    for r in runners:
+        r.close()
+    return dict(fields=fields, phasors=phasors, grad=grad, lam0=lam0, paths=paths)
+
+
+@pytest.mark.parametrize("path_name", ["generic", "fused"])
+@pytest.mark.parametrize("cuts", [(21,), (13, 33), (9, 20, 35)])
+def test_z_slabs_in_lock_step_reproduce_the_single_grid_bitwise(B, path_name, cuts):
+    """C3 miniature with kappa / alpha CPML, inv_mu, an extra H source; cuts through the design box, next to the
+    detector plane (k = 33) and (9, 35: d = 8) next to a z CPML slab; odd step count (the fused
+    ping-pong ends in its second volume)."""
+    path = B.FDTD_PATH_GENERIC if path_name == "generic" else B.FDTD_PATH_FUSED
+    n = 37
+    w = wl.c3_mini(n_steps=n, kappa_max=3.0, alpha_max=0.05)
+    rng = np.random.default_rng(3)
+    w.meta["inv_mu"] = (1.0 / (1.0 + 0.5 * rng.random((w.nz, w.ny, w.nx), dtype=np.float32))).astype(np.float32)
+    w.sources.append(wl.Source(3, (20, 12, 22), (60, 40, 23), (0.3 * wl.gaussian_sine(n, 12, 5, 11)).astype(np.float32)))
+    w.detectors.append(wl.Detector((1 << 1) | (1 << 5), (10, 10, 18), (70, 40, 24), [wl.omega_ppw(12)]))   # a box across the cuts
+    ref = _single(B, w, path, n)
+    assert ref["path"] == path
+    got = _slabs(B, w, path, n, list(cuts), ref)
+    assert got["paths"] == {path}
+    assert np.max(np.abs(ref["grad"])) > 0 and np.max(np.abs(ref["lam0"])) > 0
+    assert np.array_equal(got["fields"], ref["fields"])
+    for P, Pr in zip(got["phasors"], ref["phasors"]):
+        assert np.max(np.abs(Pr)) > 0 and np.array_equal(P, Pr)
+    assert np.array_equal(got["lam0"], ref["lam0"])
+    err = float(np.max(np.abs(got["grad"].astype(np.float64) - ref["grad"])) / np.max(np.abs(ref["grad"])))
+    print(f"z slabs {cuts} {path_name}: fields, phasors, lam0 bit-identical; gradient differs by {err:.1e} of its maximum")
+    assert err <= 1e-6
+
+
+def test_subgrid_descriptor_checks(B):
+    w = wl.c3_mini(n_steps=4)
+    kw = w.grid_kwargs()
+    for bad in (dict(nz=10, z_global=44, z_offset=0, z_ghost_lo=1, z_ghost_hi=1),      # ghost below at the global bottom
+                dict(nz=10, z_global=44, z_offset=10, z_ghost_lo=1, z_ghost_hi=0),      # missing ghost above
+                dict(nz=6, z_global=44, z_offset=0, z_ghost_lo=0, z_ghost_hi=1),        # owns no interior plane (d = 8)
+                dict(nz=10, z_global=0, z_offset=3)):
+        with pytest.raises(B.FdtdError) as e:
+            B.Grid(**{**kw, **bad, "max_steps": 4})
+        assert e.value.code == B.FDTD_EINVAL
