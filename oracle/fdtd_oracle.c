@@ -767,6 +767,37 @@ static REAL E_plus(const orc_desc *D, const REAL *const E[3], const REAL *rec_n,
     return at(D, E[comp], pos[0], pos[1], pos[2]);
 }
 
+/* N4 ("dL/d inv_mu"; Eq. 1): the H update H'_c = H_c - S im C_c(E') depends on im   */
+/* at its own cell only, so  dL/d im[p] = sum_n sum_c lamH'_c[p] * (-S C_c(E')[p]),  lamH' = cotangent of the       */
+/* post-step H (the cotangent as it stands after B1, before B5).  Like dL/d inv_eps it is formed on the interior I  */
+/* only (reading R17), where C = curl+ E' has no psi term and the primal fields are reconstructed.  Same loop as     */
+/* orc_inv_H with the accumulation added; lam = NULL or g_mu = NULL: orc_inv_H itself.                               */
+void orc_inv_H_grad(orc_state *st, REAL *fields, const REAL *im, const REAL *rec_n, const REAL *lam, REAL *g_mu)
+{
+    const orc_desc *D = &st->D;
+    const REAL S = (REAL)D->S;
+    const size_t nc = st->nc;
+    const REAL *E[3] = { fields, fields + nc, fields + 2 * nc };
+    REAL *H[3] = { fields + 3 * nc, fields + 4 * nc, fields + 5 * nc };
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (int k = lo_I(D, 2); k < hi_I(D, 2); ++k)
+        for (int j = lo_I(D, 1); j < hi_I(D, 1); ++j)
+            for (int i = lo_I(D, 0); i < hi_I(D, 0); ++i) {
+                const size_t p = IDX(i, j, k);
+                REAL acc = (REAL)0;
+                for (int c = 0; c < 3; ++c) {
+                    const int a = (c + 1) % 3, b = (c + 2) % 3;
+                    REAL d1 = E_plus(D, E, rec_n, b, a, i, j, k) - E[b][p];
+                    REAL d2 = E_plus(D, E, rec_n, a, b, i, j, k) - E[a][p];
+                    if (lam && g_mu) acc += lam[(size_t)(3 + c) * nc + p] * (d1 - d2);
+                    H[c][p] += S * (im ? im[p] : (REAL)1) * (d1 - d2);
+                }
+                if (lam && g_mu) g_mu[p] -= S * acc;
+            }
+}
+
 void orc_inv_H(orc_state *st, REAL *fields, const REAL *im, const REAL *rec_n)
 {
     const orc_desc *D = &st->D;
@@ -843,12 +874,31 @@ void orc_inv_E_grad(orc_state *st, REAL *fields, const REAL *ie, const REAL *lam
 /* fields: in = state n_steps (valid on I), out = reconstructed state 0 on I */
 /* g (cells) and dL_dfields0 (6*cells, may be NULL) are outputs.             */
 /* ------------------------------------------------------------------------ */
+int orc_backward_mu(orc_state *st, REAL *fields, const REAL *ie, const REAL *im,
+                    const orc_source *src, int n_src, const orc_detector *det, int n_det,
+                    const REAL *const *dL_dphasor,
+                    const orc_tdetector *td, int n_td, const REAL *const *dL_dtd,
+                    const REAL *dL_dfields,
+                    int n_steps, const REAL *rec, REAL *g, REAL *dL_dfields0, REAL *g_mu);
+
 int orc_backward_td(orc_state *st, REAL *fields, const REAL *ie, const REAL *im,
                     const orc_source *src, int n_src, const orc_detector *det, int n_det,
                     const REAL *const *dL_dphasor,
                     const orc_tdetector *td, int n_td, const REAL *const *dL_dtd,
                     const REAL *dL_dfields,
                     int n_steps, const REAL *rec, REAL *g, REAL *dL_dfields0)
+{
+    return orc_backward_mu(st, fields, ie, im, src, n_src, det, n_det, dL_dphasor, td, n_td, dL_dtd, dL_dfields,
+                           n_steps, rec, g, dL_dfields0, NULL);
+}
+
+/* the reverse driver; g_mu (cells, may be NULL): dL/d inv_mu on I (N4) */
+int orc_backward_mu(orc_state *st, REAL *fields, const REAL *ie, const REAL *im,
+                    const orc_source *src, int n_src, const orc_detector *det, int n_det,
+                    const REAL *const *dL_dphasor,
+                    const orc_tdetector *td, int n_td, const REAL *const *dL_dtd,
+                    const REAL *dL_dfields,
+                    int n_steps, const REAL *rec, REAL *g, REAL *dL_dfields0, REAL *g_mu)
 {
     const orc_desc *D = &st->D;
     const size_t nc = st->nc;
@@ -859,13 +909,14 @@ int orc_backward_td(orc_state *st, REAL *fields, const REAL *ie, const REAL *im,
     if (dL_dfields) memcpy(lam, dL_dfields, 6 * nc * sizeof(REAL));      /* B0 */
     orc_zero_lpsi(st);
     memset(g, 0, nc * sizeof(REAL));
+    if (g_mu) memset(g_mu, 0, nc * sizeof(REAL));
     for (int n = n_steps - 1; n >= 0; --n) {
         const REAL *rec_n = rec ? rec + (size_t)n * rs : NULL;
         time_detect_adjoint(D, lam, fields, nc, ie, im, td, n_td, dL_dtd, g, n);   /* N2^T (primal state after step n) */
         detect_adjoint(D, lam, nc, det, n_det, dL_dphasor, n);           /* B1  */
         orc_adj_H(st, lam, im);                                          /* B2  */
         add_sources(D, fields, nc, src, n_src, n, 1, (REAL)-1);          /* undo O4 */
-        orc_inv_H(st, fields, im, rec_n);                                /* O6c */
+        orc_inv_H_grad(st, fields, im, rec_n, lam, g_mu);                /* O6c (+ N4: dL/d inv_mu) */
         add_sources(D, fields, nc, src, n_src, n, 0, (REAL)-1);          /* undo O2 */
         orc_inv_E_grad(st, fields, ie, lam, g, rec_n);                   /* O7a */
         orc_adj_E(st, lam, ie);                                          /* B5  */

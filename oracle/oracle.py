@@ -99,6 +99,11 @@ def _lib(tag: str):
         L.orc_forward_td.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                      C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p, C.c_int,
                                      C.c_int, C.c_void_p, C.c_void_p]
+        L.orc_backward_mu.restype = C.c_int
+        L.orc_backward_mu.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                      C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p,
+                                      C.c_void_p, C.c_int, C.c_void_p,
+                                      C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_backward_td.restype = C.c_int
         L.orc_backward_td.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                       C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p,
@@ -302,9 +307,10 @@ class Oracle:
         return {"phasors": phasors, "rec": rec, "tape": tp, "time_outputs": touts}
 
     def backward(self, fields, inv_eps, inv_mu=None, sources=(), detectors=(),
-                 dL_dphasor=None, dL_dfields=None, n_steps=0, rec=None, time_detectors=(), dL_dtime=None):
+                 dL_dphasor=None, dL_dfields=None, n_steps=0, rec=None, time_detectors=(), dL_dtime=None,
+                 want_grad_mu=False):
         """Time-reversed gradient.  `fields` (state n_steps) is overwritten by the
-        reconstructed state 0 on I.  Returns (g, dL_dfields0)."""
+        reconstructed state 0 on I.  Returns (g, dL_dfields0), or (g, dL_dfields0, dL/d inv_mu) with want_grad_mu (N4)."""
         assert fields.dtype == self.dtype and fields.flags.c_contiguous
         ie = self.arr(inv_eps, self.shape)
         im = self.arr(inv_mu, self.shape)
@@ -329,10 +335,11 @@ class Oracle:
                 Ga = self.arr(G)
                 keep.append(Ga)
                 tp[i] = None if Ga is None else Ga.ctypes.data
-        rc = self.L.orc_backward_td(self.h, _ptr(fields), _ptr(ie), _ptr(im), sarr, ns, darr, nd, gp,
-                                    tarr, nt, tp, _ptr(dLf), int(n_steps), _ptr(rec), _ptr(g), _ptr(lam0))
+        g_mu = np.zeros(self.shape, dtype=self.dtype) if want_grad_mu else None
+        rc = self.L.orc_backward_mu(self.h, _ptr(fields), _ptr(ie), _ptr(im), sarr, ns, darr, nd, gp,
+                                    tarr, nt, tp, _ptr(dLf), int(n_steps), _ptr(rec), _ptr(g), _ptr(lam0), _ptr(g_mu))
         assert rc == 0, rc
-        return g, lam0
+        return (g, lam0, g_mu) if want_grad_mu else (g, lam0)
 
     # ---- N2: flux from phasors, TFSF plane source ----------------------------
     def flux(self, det, phasor, axis, interpolate=False):

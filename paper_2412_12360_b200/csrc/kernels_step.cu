@@ -1414,7 +1414,8 @@ int fused_setup(fdtd_grid *g)
         for (int q = 0; q < kNumTiles; ++q) {
             const TileImpl &t = kTiles[q];
             if (iTX && (t.TX != iTX || t.TY != iTY)) continue;
-            const int nst = std::min(MAX_ST, (smem_cap - t.ring_bytes - tail_bytes - 1024) / (t.stage / 7 * 10));
+            int nst = std::min(MAX_ST, (smem_cap - t.ring_bytes - tail_bytes - 1024) / (t.stage / 7 * 10));
+            if (const char *e = getenv("FDTD_INST")) nst = std::min(nst, atoi(e));
             if (nst < 3) continue;
             const long long ntx = (nx_i + t.TX - 1) / t.TX, nty = (ny_i + t.TY - 1) / t.TY;
             const double eff = ((double)(G.hi[0] - G.lo[0]) / 4 * ny_i) / ((double)ntx * nty * t.ncw * 32);

@@ -234,3 +234,43 @@ def test_n2e_tfsf_plane_source_is_one_directional(axis, pol, direction):
     # only the polarisation asked for (and its H partner) is excited
     others = [q for q in range(6) if q not in (pol, hcomp)]
     assert np.max(np.abs(f[others])) == 0.0
+
+
+# ----------------------------------------------------------------------------- N4
+def test_n4_gradient_with_respect_to_inv_mu():
+    """SURVEY 8(f) N4 (dL/d inv_mu; Eq. 1): the time-reversed sweep's dL/d inv_mu on the interior against
+    central finite differences of the loss with respect to single inv_mu voxels, on the tiny CPML grid with every term
+    (kappa, alpha, random inv_eps and inv_mu, E and H sources, DFT loss on Ey and Hx)."""
+    w = wl.tiny_pml(n_steps=30)
+    d = w.pml_cells
+    shape = (w.nz, w.ny, w.nx)
+    ie = w.inv_eps.astype(np.float64)
+    im0 = w.meta["inv_mu"].astype(np.float64)
+
+    def loss(im_, want_grad=False):
+        o = Oracle(**w.grid_kwargs())
+        f = np.zeros((6,) + shape)
+        out = o.forward(f, ie, im_, w.sources, w.detectors, w.n_steps, record=want_grad)
+        P = out["phasors"][0]
+        L = float(np.sum(P * P)) + 0.5 * float(np.sum(f[3:] ** 2))
+        if not want_grad:
+            return L
+        dLf = np.zeros_like(f)
+        dLf[3:] = f[3:]
+        g, _, g_mu = o.backward(f, ie, im_, w.sources, w.detectors, [2.0 * P], dLf, w.n_steps, out["rec"], want_grad_mu=True)
+        return L, g_mu
+
+    L, g_mu = loss(im0, True)
+    scale = np.max(np.abs(g_mu))
+    assert scale > 0
+    outside = np.ones(shape, dtype=bool)
+    outside[d:w.nz - d, d:w.ny - d, d:w.nx - d] = False
+    assert np.all(g_mu[outside] == 0.0)                       # formed on the interior only (R17)
+    h = 1e-6
+    for v in [(w.nz // 2, w.ny // 2, w.nx // 2), (d, d, d), (w.nz - d - 1, w.ny - d - 1, w.nx - d - 1), (d + 1, d + 2, d + 3),
+              (w.nz // 2, w.ny // 2, w.nx // 2 + 1)]:
+        ip, im_ = im0.copy(), im0.copy()
+        ip[v] += h
+        im_[v] -= h
+        fd = (loss(ip) - loss(im_)) / (2 * h)
+        assert abs(fd - g_mu[v]) < 2e-6 * scale + 1e-6 * abs(fd), (v, fd, g_mu[v])
