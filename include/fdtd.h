@@ -194,6 +194,17 @@ FDTD_API int fdtd_backward(fdtd_grid *grid, float *fields, const float *inv_eps,
                   int32_t n_steps, float *dL_dinv_eps, float *dL_dfields0,
                   void *cuda_stream);
 
+/* N4: fdtd_backward that also returns dL/d inv_mu (Eq. 1: the H update depends on
+ * inv_mu at its own cell), dL_dinv_mu[p] = sum_n sum_c lamH'_c[p] * (-S (curl+ E')_c[p]) with lamH' the cotangent of
+ * the post-step H.  DEVICE [nz][ny][nx], OUT, zero-filled by the library, non-zero only on the reconstruction box
+ * (like dL_dinv_eps it needs the reconstructed fields, so dL_dinv_eps must be requested too).  NULL: fdtd_backward.
+ * On the fused path the inverse step then runs on the generic kernels (the adjoint step stays fused).
+ * Not built (N4 remainder): one inv_eps volume per E component, lossy / dispersive media with a checkpointed reverse sweep. */
+FDTD_API int fdtd_backward_mu(fdtd_grid *grid, float *fields, const float *inv_eps, const float *inv_mu,
+                     const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
+                     const float *const *dL_dphasor, const float *dL_dfields,
+                     int32_t n_steps, float *dL_dinv_eps, float *dL_dinv_mu, float *dL_dfields0, void *cuda_stream);
+
 /* B6, chain rule to design parameters (once per gradient, not per step): for a design box whose
  * permittivity is eps = eps_bg + delta_eps*rho (reading R20),
  *   dL_drho[cell] = dL_dinv_eps[cell] * d(1/eps)/drho = -dL_dinv_eps[cell] * delta_eps * inv_eps[cell]^2.

@@ -73,7 +73,7 @@ class fdtd_profile(C.Structure):
 EXPORTS = ("fdtd_grad_rho", "fdtd_set_profiling", "fdtd_get_profile", "fdtd_create_grid", "fdtd_forward", "fdtd_backward", "fdtd_destroy", "fdtd_last_error",
            "fdtd_get_info", "fdtd_version", "fdtd_forward_host", "fdtd_backward_host", "fdtd_debug_partition",
            "fdtd_forward_td", "fdtd_backward_td", "fdtd_flux", "fdtd_flux_vjp", "fdtd_tfsf_plane",
-           "fdtd_forward_range", "fdtd_backward_range", "fdtd_halo_export", "fdtd_halo_import")
+           "fdtd_forward_range", "fdtd_backward_range", "fdtd_halo_export", "fdtd_halo_import", "fdtd_backward_mu")
 
 
 def _load():
@@ -98,6 +98,9 @@ def _load():
     L.fdtd_backward_range.restype = C.c_int
     L.fdtd_backward_range.argtypes = [vp, vp, vp, vp, C.POINTER(fdtd_source), i32, C.POINTER(fdtd_detector), i32,
                                       C.POINTER(vp), vp, i32, i32, i32, vp, vp, vp]
+    L.fdtd_backward_mu.restype = C.c_int
+    L.fdtd_backward_mu.argtypes = [vp, vp, vp, vp, C.POINTER(fdtd_source), i32, C.POINTER(fdtd_detector), i32,
+                                   C.POINTER(vp), vp, i32, vp, vp, vp, vp]
     L.fdtd_halo_export.restype = C.c_int
     L.fdtd_halo_export.argtypes = [vp, vp, i32, i32, i32, vp, vp]
     L.fdtd_halo_import.restype = C.c_int
@@ -239,6 +242,12 @@ def fdtd_backward_range(grid, fields, inv_eps, inv_mu, src, n_src, det, n_det, d
                         dL_dinv_eps, dL_dfields0, stream) -> None:
     _check(_L.fdtd_backward_range(grid, _ptr(fields), _ptr(inv_eps), _ptr(inv_mu), src, n_src, det, n_det, dL_dphasor,
                                   _ptr(dL_dfields), int(n_hi), int(n_lo), int(n_total), _ptr(dL_dinv_eps), _ptr(dL_dfields0), stream))
+
+
+def fdtd_backward_mu(grid, fields, inv_eps, inv_mu, src, n_src, det, n_det, dL_dphasor, dL_dfields, n_steps,
+                     dL_dinv_eps, dL_dinv_mu, dL_dfields0, stream) -> None:
+    _check(_L.fdtd_backward_mu(grid, _ptr(fields), _ptr(inv_eps), _ptr(inv_mu), src, n_src, det, n_det, dL_dphasor,
+                               _ptr(dL_dfields), n_steps, _ptr(dL_dinv_eps), _ptr(dL_dinv_mu), _ptr(dL_dfields0), stream))
 
 
 def fdtd_halo_export(grid, fields, which, n, side, out, stream) -> None:
@@ -420,7 +429,7 @@ class Grid:
         return phasors
 
     def backward(self, fields, inv_eps, inv_mu=None, sources=(), detectors=(), dL_dphasor=None,
-                 dL_dfields=None, n_steps=0, want_dL_dfields0=False, out=None, want_grad=True, time_detectors=(), dL_dtime=None):
+                 dL_dfields=None, n_steps=0, want_dL_dfields0=False, out=None, want_grad=True, time_detectors=(), dL_dtime=None, grad_mu=None):
         """want_grad=False: adjoint sweep only (dL_dinv_eps = NULL): returns (None, cotangent of state 0)."""
         torch = self.torch
         sarr, ns, k1 = self.marshal_sources(sources)
@@ -432,7 +441,10 @@ class Grid:
                 cot[i] = _ptr(G)
         g = None if not want_grad else (out if out is not None else torch.empty(self.shape, dtype=torch.float32, device="cuda"))
         lam0 = torch.empty((6,) + self.shape, dtype=torch.float32, device="cuda") if (want_dL_dfields0 or not want_grad) else None
-        if time_detectors:
+        if grad_mu is not None:          # N4: dL/d inv_mu into the caller's volume
+            fdtd_backward_mu(self.h, fields, inv_eps, inv_mu, sarr, ns, darr, nd, cot, dL_dfields, int(n_steps),
+                             g, grad_mu, lam0, self.stream())
+        elif time_detectors:
             tarr, nt = self.marshal_time_detectors(time_detectors, None)
             tcot = (C.c_void_p * max(nt, 1))()
             for i, G in enumerate(dL_dtime or []):

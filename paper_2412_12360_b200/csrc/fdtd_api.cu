@@ -720,7 +720,17 @@ static int backward_impl(fdtd_grid *g, float *fields, const float *inv_eps, cons
                          const float *const *dL_dphasor,
                          const fdtd_time_detector *td, int32_t n_td, const float *const *dL_dtd,
                          const float *dL_dfields, int n_hi, int n_lo, int n_total, float *dL_dinv_eps, float *dL_dfields0,
-                         void *cuda_stream);
+                         void *cuda_stream, float *dL_dinv_mu = nullptr);
+
+extern "C" int fdtd_backward_mu(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
+                                const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
+                                const float *const *dL_dphasor, const float *dL_dfields,
+                                int32_t n_steps, float *dL_dinv_eps, float *dL_dinv_mu, float *dL_dfields0, void *cuda_stream)
+{
+    if (dL_dinv_mu && !dL_dinv_eps) return fail(FDTD_EINVAL, "fdtd_backward_mu: dL_dinv_mu needs the reconstructed fields (request dL_dinv_eps too)");
+    return backward_impl(g, fields, inv_eps, inv_mu, src, n_src, det, n_det, dL_dphasor, nullptr, 0, nullptr, dL_dfields,
+                         n_steps, 0, n_steps, dL_dinv_eps, dL_dfields0, cuda_stream, dL_dinv_mu);
+}
 
 extern "C" int fdtd_backward_td(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
                                 const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
@@ -752,7 +762,7 @@ static int backward_impl(fdtd_grid *g, float *fields, const float *inv_eps, cons
                          const float *const *dL_dphasor,
                          const fdtd_time_detector *td, int32_t n_td, const float *const *dL_dtd,
                          const float *dL_dfields, int n_hi, int n_lo, int n_total, float *dL_dinv_eps, float *dL_dfields0,
-                         void *cuda_stream)
+                         void *cuda_stream, float *dL_dinv_mu)
 {
     const int n_steps = n_total;
     const bool first = n_hi == n_total, last = n_lo == 0;
@@ -795,6 +805,7 @@ static int backward_impl(fdtd_grid *g, float *fields, const float *inv_eps, cons
         for (int q = 0; q < 2; ++q)
             if ((rc = g->zero_psi(g->lpsiE[q], st)) || (rc = g->zero_psi(g->lpsiH[q], st))) return rc;
         if (dL_dinv_eps) CK(cudaMemsetAsync(dL_dinv_eps, 0, vol, st));
+        if (dL_dinv_mu) CK(cudaMemsetAsync(dL_dinv_mu, 0, vol, st));
     }
     launch_set_step(g->d_step, std::max(n_hi - 1, 0), st);      // the first reverse step of the call reads slot 0
     const bool want_grad = dL_dinv_eps != nullptr;              // false: adjoint sweep only (B1, B2, B5)
@@ -802,7 +813,7 @@ static int backward_impl(fdtd_grid *g, float *fields, const float *inv_eps, cons
 
     if (fused_call) {
         // seeded_H: the H part of the seed can be non-zero (it is scaled by inv_mu for the sweep)
-        rc = fused_backward(g, fields, inv_eps, inv_mu, S, D, TD, total_freq, n_hi, n_lo, n_total, dL_dinv_eps, dL_dfields != nullptr, st);
+        rc = fused_backward(g, fields, inv_eps, inv_mu, S, D, TD, total_freq, n_hi, n_lo, n_total, dL_dinv_eps, dL_dfields != nullptr, st, dL_dinv_mu);
         if (rc) return rc;
         // the fused sweep carried im lamH in the H part (kernels_step.cu); the cotangent of state 0 is lamH
         if (last && inv_mu && dL_dfields0) launch_scale_H(G, g->lam, inv_mu, true, st);
@@ -812,6 +823,7 @@ static int backward_impl(fdtd_grid *g, float *fields, const float *inv_eps, cons
         const int launches = (want_grad ? 5 + n_adj + n_src + (G.d > 0 ? 1 : 0) : 3 + n_adj) + (int)TD.size();
         std::string key = make_key("gb", fields, inv_eps, inv_mu, g->rec, dL_dinv_eps, S, D, 0);
         key.append((const char *)&g->d_cs, sizeof(g->d_cs));
+        key.append((const char *)&dL_dinv_mu, sizeof(dL_dinv_mu));
         if (!TD.empty()) key.append((const char *)TD.data(), TD.size() * sizeof(TimeDetDev));
         rc = run_steps(g, g->bwd_graph, key, n_hi - n_lo, launches, st, [&](cudaStream_t cs) {
             { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
@@ -824,7 +836,7 @@ static int backward_impl(fdtd_grid *g, float *fields, const float *inv_eps, cons
             { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
               for (const SourceDev &s : S) if (s.comp >= 3) launch_add_source(G, fields, s, g->step_in(), -1.f, cs); }
             if (G.d > 0) { ProfScope p(g, fdtd_grid::PC_INJECT, cs); launch_inject(G, g->R, fields, g->rec, g->step_in(), cs); }
-            { ProfScope p(g, fdtd_grid::PC_INV_H, cs); launch_inv_H(G, fields, inv_mu, cs); }
+            { ProfScope p(g, fdtd_grid::PC_INV_H, cs); launch_inv_H(G, fields, inv_mu, cs, g->lam, nullptr, nullptr, false, dL_dinv_mu); }
             { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
               for (const SourceDev &s : S) if (s.comp < 3) launch_add_source(G, fields, s, g->step_in(), -1.f, cs); }
             { ProfScope p(g, fdtd_grid::PC_INV_E_GRAD, cs); launch_inv_E_grad(G, fields, inv_eps, g->lam, dL_dinv_eps, cs); }

@@ -104,7 +104,7 @@ int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float
 int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
                    const std::vector<fdtd::SourceDev> &S, const std::vector<fdtd::DetectorDev> &D,
                    const std::vector<fdtd::TimeDetDev> &TD, int total_freq, int n_hi, int n_lo, int n_total, float *dL_dinv_eps,
-                   bool seeded_H, cudaStream_t st);
+                   bool seeded_H, cudaStream_t st, float *dL_dinv_mu = nullptr);
 // the volume that holds state n of the fused path's ping-pong: which = 0 primal (fields / second buffer), 1 cotangents
 float *fused_volume(fdtd_grid *g, float *fields, int which, int n);
 

@@ -143,7 +143,10 @@ void launch_adj_E(const Dims &G, const Tables &T, float *lam, const float *ie, P
                   const int *step, cudaStream_t st);
 void launch_grad_rho(const Dims &G, const float *g, const float *ie, float delta_eps, const int lo[3], const int hi[3],
                      float *out, cudaStream_t st);
-void launch_inv_H(const Dims &G, float *fields, const float *im, cudaStream_t st);
+// N4: with g_mu, dL/d inv_mu is accumulated from the cotangent of the post-step H (the H part of lam, or of the
+// fused sweep's volume (n+1)&1 of lam / lam2, which holds im lamH when `scaled`)
+void launch_inv_H(const Dims &G, float *fields, const float *im, cudaStream_t st, const float *lam = nullptr,
+                  const float *lam2 = nullptr, const int *step = nullptr, bool scaled = false, float *g_mu = nullptr);
 void launch_inv_E_grad(const Dims &G, float *fields, const float *ie, const float *lam, float *g, cudaStream_t st);
 // fused path: cotangent volumes are ping-ponged by step parity
 void launch_inv_E_grad_pp(const Dims &G, float *fields, const float *ie, const float *lamA, const float *lamB,

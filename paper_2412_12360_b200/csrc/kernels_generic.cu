@@ -411,12 +411,19 @@ __global__ void __launch_bounds__(BX *BY) k_adjoint(Dims G, Tables T, float *__r
 // ------------------------------------------------------------------------------------------ B3
 // inverse H step on I:  H = H' + S im curl+ E'   (sources already subtracted; the E' operand at
 // index N_a-d was injected from the record)
+// N4 (dL/d inv_mu): with lam and g_mu, g_mu -= S sum_c lamH'_c (curl+ E')_c, lamH' = the cotangent of the post-step H:
+// the H part of `lam`, or of lam2 when the fused sweep's volume (n+1)&1 is the odd one; scaled: that part holds im lamH'.
 template <bool PER>
-__global__ void __launch_bounds__(BX *BY) k_inv_H(Dims G, float *__restrict__ f, const float *__restrict__ im)
+__global__ void __launch_bounds__(BX *BY) k_inv_H(Dims G, float *__restrict__ f, const float *__restrict__ im,
+                                                  const float *__restrict__ lam, const float *__restrict__ lam2,
+                                                  const int *__restrict__ step, int scaled, float *__restrict__ g_mu)
 {
     CELL_IJK();
     if (i < G.lo[0] || i >= G.hi[0] || j < G.lo[1] || j >= G.hi[1] || k < G.lo[2] || k >= G.hi[2]) return;
-    const float sim = G.S * (im ? __ldg(im + p) : 1.f);
+    const float m = im ? __ldg(im + p) : 1.f;
+    const float sim = G.S * m;
+    if (lam2 && ((*step + 1) & 1)) lam = lam2;
+    float acc = 0.f;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         const int a = (c + 1) % 3, b = (c + 2) % 3;
@@ -424,7 +431,9 @@ __global__ void __launch_bounds__(BX *BY) k_inv_H(Dims G, float *__restrict__ f,
         const float d1 = fetch<PER>(G, Eb, i + (a == 0), j + (a == 1), k + (a == 2)) - Eb[p];
         const float d2 = fetch<PER>(G, Ea, i + (b == 0), j + (b == 1), k + (b == 2)) - Ea[p];
         f[(3 + c) * G.nc + p] += sim * (d1 - d2);
+        if (g_mu) acc = fmaf(lam[(3 + c) * G.nc + p], d1 - d2, acc);
     }
+    if (g_mu) g_mu[p] -= G.S * (scaled ? acc / m : acc);
 }
 
 // ------------------------------------------------------------------------------------------ B4
@@ -584,10 +593,11 @@ void launch_grad_rho(const Dims &G, const float *g, const float *ie, float delta
     k_grad_rho<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(G, g, ie, delta_eps, lo[0], lo[1], lo[2], bx, by, bz, out);
 }
 
-void launch_inv_H(const Dims &G, float *fields, const float *im, cudaStream_t st)
+void launch_inv_H(const Dims &G, float *fields, const float *im, cudaStream_t st, const float *lam, const float *lam2,
+                  const int *step, bool scaled, float *g_mu)
 {
-    if (G.periodic) k_inv_H<true><<<vol_grid(G), vol_block(), 0, st>>>(G, fields, im);
-    else            k_inv_H<false><<<vol_grid(G), vol_block(), 0, st>>>(G, fields, im);
+    if (G.periodic) k_inv_H<true><<<vol_grid(G), vol_block(), 0, st>>>(G, fields, im, lam, lam2, step, scaled ? 1 : 0, g_mu);
+    else            k_inv_H<false><<<vol_grid(G), vol_block(), 0, st>>>(G, fields, im, lam, lam2, step, scaled ? 1 : 0, g_mu);
 }
 
 void launch_inv_E_grad(const Dims &G, float *fields, const float *ie, const float *lam, float *g, cudaStream_t st)

@@ -1751,7 +1751,7 @@ void enqueue_fwd(void *vctx, cudaStream_t cs)
 struct BwdCtx {
     fdtd_grid *g; StepParams P; InvParams I; bool fused_inv; bool fused_det; bool pipelined; bool want_grad; float *bufB; float *fields; const float *ie; const float *im; float *grad; float *lamA; float *lamB;
     const std::vector<SourceDev> *S; const std::vector<DetectorDev> *D; int total_freq;
-    const std::vector<TimeDetDev> *TD;
+    const std::vector<TimeDetDev> *TD; float *grad_mu;
 };
 // Reverse step n.  One kernel after the other: B1 (detector cotangents into the volume about to be read), B2+B5
 // (fused adjoint step), face injection, then the primal inverse step B3+B4 with lamE' taken from the volume the
@@ -1813,7 +1813,9 @@ void enqueue_bwd(void *vctx, cudaStream_t cs)
     { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
       for (const SourceDev &s : *c->S) if (s.comp >= 3) launch_add_source(G, c->fields, s, g->step_in(), -1.f, cs); }
     if (G.d > 0) { ProfScope p(g, fdtd_grid::PC_INJECT, cs); launch_inject(G, g->R, c->fields, g->rec, g->step_in(), cs); }
-    { ProfScope p(g, fdtd_grid::PC_INV_H, cs); launch_inv_H(G, c->fields, c->im, cs); }
+    // N4: the cotangent of the post-step H is still in the volume adjoint step n read, (n+1)&1 (scaled by im with inv_mu)
+    { ProfScope p(g, fdtd_grid::PC_INV_H, cs);
+      launch_inv_H(G, c->fields, c->im, cs, c->lamA, c->lamB, g->step_in(), c->im != nullptr, c->grad_mu); }
     { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
       for (const SourceDev &s : *c->S) if (s.comp < 3) launch_add_source(G, c->fields, s, g->step_in(), -1.f, cs); }
     { ProfScope p(g, fdtd_grid::PC_INV_E_GRAD, cs);
@@ -1878,7 +1880,8 @@ int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float
 // result is back in volume 0 = g->lam.
 int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
                    const std::vector<SourceDev> &S, const std::vector<DetectorDev> &D, const std::vector<TimeDetDev> &TD,
-                   int total_freq, int n_hi, int n_lo, int n_total, float *dL_dinv_eps, bool seeded_H, cudaStream_t st)
+                   int total_freq, int n_hi, int n_lo, int n_total, float *dL_dinv_eps, bool seeded_H, cudaStream_t st,
+                   float *dL_dinv_mu)
 {
     // reverse steps n_hi-1 .. n_lo of a run of n_total (fdtd_backward: n_steps-1 .. 0).  Between the calls of a range
     // sequence the cotangents after reverse step n live in volume n&1 (0: g->lam) and the reconstructed state n in
@@ -1897,14 +1900,15 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
         if (e != cudaSuccess) { (void)cudaGetLastError(); return fdtd_fail(FDTD_ECUDA, cudaGetErrorString(e)); }
     }
     const bool want_grad = dL_dinv_eps != nullptr;      // false: adjoint sweep only, the primal volumes are not touched
-    const bool fused_inv = want_grad && F->itile != nullptr && (int)S.size() <= MAX_SRC && !getenv("FDTD_GENERIC_INVERSE");
+    // N4: dL/d inv_mu is formed by the generic inverse H kernel (the fused inverse step's stage has no room for lamH)
+    const bool fused_inv = want_grad && F->itile != nullptr && (int)S.size() <= MAX_SRC && !getenv("FDTD_GENERIC_INVERSE") && !dL_dinv_mu;
     // B1 inside the adjoint kernel when every detector with a cotangent is on E components (else a kernel per detector)
     bool fused_det = (int)D.size() <= MAX_DET;
     for (const DetectorDev &dt : D) if (dt.phasor && (dt.mask >> 3)) fused_det = false;
     // while profiling (events around every launch) the kernels run one after the other, so each is timed alone
     // (time-domain detector transposes read the primal state after step n, which the pipelined sweep is still writing)
     const bool pipelined = fused_inv && fused_det && F->n_inv_p > 0 && !g->profiling && TD.empty() && whole;
-    BwdCtx ctx{ g, F->sp, F->ip, fused_inv, fused_det, pipelined, want_grad, F->bufB, fields, inv_eps, inv_mu, dL_dinv_eps, g->lam, F->lamB, &S, &D, total_freq, &TD };
+    BwdCtx ctx{ g, F->sp, F->ip, fused_inv, fused_det, pipelined, want_grad, F->bufB, fields, inv_eps, inv_mu, dL_dinv_eps, g->lam, F->lamB, &S, &D, total_freq, &TD, dL_dinv_mu };
     if (fused_inv) {
         // reverse step n reads primal volume (n+1)&1 and writes n&1: state n_steps must sit in volume n_steps&1
         if ((rc = build_inv_maps(g, fields, F->bufB, inv_eps, g->lam, F->lamB, st))) return rc;
@@ -1947,6 +1951,7 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     if (fused_inv) key.append((const char *)&ctx.I, sizeof(ctx.I));
     key.append((const char *)&fields, sizeof(fields));
     key.append((const char *)&dL_dinv_eps, sizeof(dL_dinv_eps));
+    key.append((const char *)&dL_dinv_mu, sizeof(dL_dinv_mu));
     if (!S.empty()) key.append((const char *)S.data(), S.size() * sizeof(SourceDev));
     if (!D.empty()) key.append((const char *)D.data(), D.size() * sizeof(DetectorDev));
     if (!TD.empty()) key.append((const char *)TD.data(), TD.size() * sizeof(TimeDetDev));
