@@ -1648,6 +1648,8 @@ static int calibrate(fdtd_grid *g)
     static const double cand[][2] = { { 1.0, 0.8 }, { 0.75, 0.55 }, { 0.75, 0.8 }, { 0.75, 1.05 }, { 1.0, 0.55 }, { 1.0, 1.05 },
                                       { 0.5, 0.8 }, { 0.5, 1.05 }, { 1.25, 0.8 }, { 1.25, 1.05 }, { 1.0, 0.3 }, { 0.75, 0.3 } };
     const int n_grid = G.d > 0 ? (int)(sizeof(cand) / sizeof(cand[0])) : 1;
+    // (round 2: chaining up to ten damped feedback rounds after the candidates was measured and dropped -- the spans stay
+    // at 94-100 us forward and get worse, 104-106 us, for the adjoint kernel: profiles/r2_bound_experiments.md)
     const int cal_iters = getenv("FDTD_CAL_ITERS") ? std::max(1, atoi(getenv("FDTD_CAL_ITERS"))) : n_grid + 2;
     for (int mode = 0; mode < 2; ++mode) {
         const int n_cta = mode ? F->n_adj : F->n_cta;
@@ -1694,6 +1696,22 @@ static int calibrate(fdtd_grid *g)
             return done(fdtd_fail(FDTD_ECUDA, "calibration: upload of the segment table failed"));
         F->calibrated_us[mode] = best;
         if (getenv("FDTD_VERBOSE")) fprintf(stderr, "fdtd: calibrated %s step kernel: %.1f us per launch\n", mode ? "adjoint" : "forward", best);
+        if (getenv("FDTD_VERBOSE") && atoi(getenv("FDTD_VERBOSE")) > 2) {
+            // per-CTA durations of four successive launches of the final partition: is a slow CTA slow every time?
+            std::vector<std::vector<double>> dur(4, std::vector<double>(n_cta));
+            for (int rep = 0; rep < 4; ++rep) {
+                if (mode) F->tile->launch_adj(P, n_cta, F->smem, 0); else F->tile->launch_fwd(P, n_cta, F->smem, 0);
+                cudaDeviceSynchronize();
+                cudaMemcpy(t.data(), F->d_cta_t, 2 * (size_t)n_cta * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
+                for (int c = 0; c < n_cta; ++c) dur[rep][c] = (double)(t[2 * c + 1] - t[2 * c]) * 1e-3;
+            }
+            for (int c = 0; c < n_cta; ++c) {
+                double cost = 0.0;
+                for (const std::pair<long long, long long> &r : best_runs[c]) cost += (double)(r.second - r.first);
+                fprintf(stderr, "fdtd:   cta %3d planes %5.0f segs %zu durations %.1f %.1f %.1f %.1f\n", c, cost, best_runs[c].size(),
+                        dur[0][c], dur[1][c], dur[2][c], dur[3][c]);
+            }
+        }
     }
     cudaMemset(F->bufB, 0, 6 * vol);
     return done(FDTD_OK);
