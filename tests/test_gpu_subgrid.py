@@ -111,3 +111,49 @@ def test_subgrid_descriptor_checks(B):
         with pytest.raises(B.FdtdError) as e:
             B.Grid(**{**kw, **bad, "max_steps": 4})
         assert e.value.code == B.FDTD_EINVAL
+
+
+@pytest.mark.parametrize("path_name", ["generic", "fused"])
+def test_a_run_in_pieces_is_the_same_run(B, path_name):
+    """fdtd_forward_range / fdtd_backward_range on an ordinary grid: a run cut into pieces of odd and even lengths (the
+    fused ping-pong changes volume with every step) gives bit for bit what fdtd_forward / fdtd_backward give; a piece that
+    does not continue the previous one is ESTATE."""
+    import torch
+    path = B.FDTD_PATH_GENERIC if path_name == "generic" else B.FDTD_PATH_FUSED
+    n = 23
+    w = wl.c3_mini(n_steps=n, kappa_max=3.0, alpha_max=0.05)
+    ref = _single(B, w, path, n)
+    slab = sharding.ZSlab(0, 1, w.nz, 0, w.nz)                  # the whole grid as one "slab": no ghosts, no exchange
+    r = sharding.SlabRunner(B, w, slab, n, record=1, path=path)
+    r.grid.close()
+    kw = w.grid_kwargs()
+    kw.update(max_steps=n, record=1, path=path)
+    r.grid = B.Grid(**kw)                                       # an ordinary grid (z_global = 0) behind the same runner
+    r.sarr, r.ns, r._k1 = r.grid.marshal_sources(r.sources)
+    r.darr, r.nd, r._k2 = r.grid.marshal_detectors([d for _, d, _ in r.det_fwd], r.phasors)
+    r.darr_b, r.nd_b, r._k3 = r.grid.marshal_detectors([d for _, d, _ in r.det_bwd], None)
+    for a, b in [(0, 5), (5, 6), (6, 20), (20, 23)]:
+        r.forward_steps(a, b)
+    with pytest.raises(B.FdtdError) as e:
+        r.forward_steps(7, 9)
+    assert e.value.code == B.FDTD_ESTATE
+    torch.cuda.synchronize()
+    assert np.array_equal(r.fields.cpu().numpy(), ref["fields"])
+    for P, Pr in zip(r.phasors, ref["phasors"]):
+        assert np.array_equal(P.cpu().numpy(), Pr)
+    # a new run may start at any time (n_begin = 0: psi reset, state taken from `fields`)
+    for P in r.phasors:
+        P.zero_()
+    r.fields.zero_()
+    for a, b in [(0, 1), (1, 8), (8, 23)]:
+        r.forward_steps(a, b)
+    torch.cuda.synchronize()
+    for P, Pr in zip(r.phasors, ref["phasors"]):
+        assert np.array_equal(P.cpu().numpy(), Pr)
+    r.set_cotangents(ref["dLp"], ref["dLf"])
+    for a, b in [(23, 22), (22, 15), (15, 14), (14, 0)]:
+        r.backward_steps(a, b)
+    torch.cuda.synchronize()
+    assert np.array_equal(r.lam0.cpu().numpy(), ref["lam0"])
+    assert np.array_equal(r.grad.cpu().numpy(), ref["grad"])
+    r.close()
