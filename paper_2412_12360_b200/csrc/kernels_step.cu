@@ -92,6 +92,12 @@ struct Cfg {
     static constexpr int RING_ARR = RW * RP;                            // floats of one ring array
     static constexpr int RING_SLOT = 4 * RING_ARR;                      // Yx, Yz, Xy, Xz
     static constexpr int RING_BYTES = (2 * RING_SLOT * 4 + 127) / 128 * 128;
+    // inverse step kernel: three box shapes per stage (see k_inverse)
+    static constexpr int BW = TX + 4, BROWS = TY + 1;                  // H' and E'(kk+1): my cells, minus-side halo threads included
+    static constexpr int BOXB_BYTES = BW * BROWS * 4, SLOTB = (BOXB_BYTES + 127) / 128 * 128;
+    static constexpr int BOXC_BYTES = TX * TY * 4, SLOTC = (BOXC_BYTES + 127) / 128 * 128;     // inv_eps, lamE': owned cells only
+    static constexpr int ISTAGE = 3 * SLOT + 5 * SLOTB + 4 * SLOTC;
+    static constexpr int IRING_BYTES = (2 * 3 * RING_ARR * 4 + 127) / 128 * 128;              // H_x, H_y, H_z, two planes
 };
 
 __device__ __forceinline__ float4 lds4(uint32_t addr)
@@ -715,12 +721,17 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
 // Reads primal volume (n+1)&1 and cotangent volume n&1 (lamE' as the adjoint step left it), writes primal
 // volume n&1.  Same tiling as k_step with the halo on the minus side: thread column 0 / row 0 recompute H on
 // the cells left of / below the tile; cells outside I keep their (recorded or stale) values.
-// Stage slots: 0-2 E', 3-5 H', 6 inv_eps, 7-9 lamE'.
+// A stage holds everything plane kk needs, in three box shapes (round 2: the stage of plane kk+1 used to be read for
+// E'_x, E'_y at my cells, so two stages had to be resident and only one load was in flight; ncu showed the consumers
+// waiting for data, long_scoreboard 5.5 per issue):
+//   slots 0-2  E'_x,y,z(kk)          [TY+2][TX+8]   (+x / +y neighbours)
+//   slots 3-5  H'_x,y,z(kk)          [TY+1][TX+4]   (my cells, halo threads included)
+//   slots 6-7  E'_x, E'_y(kk+1)      [TY+1][TX+4]
+//   slots 8-11 inv_eps, lamE'_x,y,z  [TY][TX]       (owned cells)
 // ================================================================================================
 struct InvParams {
     Dims G;
-    const CUtensorMap *maps;       // primal table: [set][6], [12] inv_eps
-    const CUtensorMap *lmaps;      // lamE' components of cotangent volume `set`: [set][3]
+    const CUtensorMap *maps;       // [set][3] E' (shape A); [6 + set*5 + q] H'_x,y,z, E'_x, E'_y (shape B); [16] inv_eps, [17 + set*3 + c] lamE' (shape C)
     const Segment *segs;
     const int *seg_begin;          // [n_cta + 1]
     float *buf[2];                 // primal ping-pong volumes
@@ -754,13 +765,14 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_inverse(const __grid_constant
     const Dims &G = P.G;
     const uint32_t stage_base = smem_u32(smem);
     const uint32_t ring_base = stage_base + (uint32_t)P.nst * P.stage;
-    uint64_t *full = reinterpret_cast<uint64_t *>(smem + (size_t)P.nst * P.stage + C::RING_BYTES);
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + (size_t)P.nst * P.stage + C::IRING_BYTES);
     uint64_t *empty = full + MAX_ST;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n = *P.step + P.bias;
     if (n >= P.n_steps) return;
     const int rd = (n + 1) & 1, wv = n & 1;
     const int nst = P.nst;
+    constexpr uint32_t OB = 3 * C::SLOT, OD = OB + 3 * C::SLOTB, OC = OB + 5 * C::SLOTB;   // slot groups inside a stage
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < nst; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], C::NCW); }
@@ -772,26 +784,23 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_inverse(const __grid_constant
     // ============================================================================== producer
     if (warp == C::NCW) {
         if (lane != 0) return;
-        const CUtensorMap *M = P.maps + rd * 6, *Mie = P.maps + 12, *ML = P.lmaps + wv * 3;
+        const CUtensorMap *MA = P.maps + rd * 3, *MB = P.maps + 6 + rd * 5, *Mie = P.maps + 16, *ML = P.maps + 17 + wv * 3;
         int s = 0, use = 0;
         for (int sg = seg_lo; sg < seg_hi; ++sg) {
             const Segment S = P.segs[sg];
             const int x = S.i0 - 4, y = S.j0 - 1;
-            for (int kk = S.k0 - 1; kk <= S.k1; ++kk) {
+            for (int kk = S.k0 - 1; kk < S.k1; ++kk) {
                 if (use > 0) mbar_wait(&empty[s], (use - 1) & 1);
                 uint64_t *fb = &full[s];
                 uint8_t *st = smem + (size_t)s * P.stage;
-                const bool first = kk == S.k0 - 1, last = kk == S.k1;
-                mbar_expect_tx(fb, (last ? 2u : (first ? 6u : 10u)) * C::BOX_BYTES);
-                tma_load_3d(st, M, x, y, kk, fb);
-                tma_load_3d(st + C::SLOT, M + 1, x, y, kk, fb);
-                if (!last) {
-                    tma_load_3d(st + 2 * C::SLOT, M + 2, x, y, kk, fb);
-                    for (int c = 0; c < 3; ++c) tma_load_3d(st + (3 + c) * C::SLOT, M + 3 + c, x, y, kk, fb);
-                    if (!first) {
-                        tma_load_3d(st + 6 * C::SLOT, Mie, x, y, kk, fb);
-                        for (int c = 0; c < 3; ++c) tma_load_3d(st + (7 + c) * C::SLOT, ML + c, x, y, kk, fb);
-                    }
+                const bool first = kk == S.k0 - 1;       // only H of this plane is wanted: no inv_eps, no lamE'
+                mbar_expect_tx(fb, 3u * C::BOX_BYTES + 5u * C::BOXB_BYTES + (first ? 0u : 4u * C::BOXC_BYTES));
+                for (int c = 0; c < 3; ++c) tma_load_3d(st + c * C::SLOT, MA + c, x, y, kk, fb);
+                for (int c = 0; c < 3; ++c) tma_load_3d(st + OB + c * C::SLOTB, MB + c, x, y, kk, fb);
+                for (int c = 0; c < 2; ++c) tma_load_3d(st + OD + c * C::SLOTB, MB + 3 + c, x, y, kk + 1, fb);
+                if (!first) {
+                    tma_load_3d(st + OC, Mie, S.i0, S.j0, kk, fb);
+                    for (int c = 0; c < 3; ++c) tma_load_3d(st + OC + (1 + c) * C::SLOTC, ML + c, S.i0, S.j0, kk, fb);
                 }
                 if (++s == nst) { s = 0; ++use; }
             }
@@ -804,15 +813,17 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_inverse(const __grid_constant
     const bool dup = tx0 >= C::CW || ty0 >= C::RW;
     const int tx = min(tx0, C::CW - 1), ty = min(ty0, C::RW - 1);
     const bool inner = !dup && tx >= 1 && ty >= 1;                 // column 0 / row 0 are the halo threads
-    const uint32_t o_own = (ty * C::PW + 4 * tx) * 4;
+    const uint32_t oA = (ty * C::PW + 4 * tx) * 4;                 // my first cell inside a box of each shape
+    const uint32_t oB = (ty * C::BW + 4 * tx) * 4;
+    const uint32_t oC = (max(ty - 1, 0) * C::TX + 4 * max(tx - 1, 0)) * 4;
     const uint32_t r_own = (ty * C::RP + 4 * tx) * 4;
     float *dst = P.buf[wv];
     const float S = G.S;
     const long long nc = G.nc;
     const int plane = G.ny * G.nx;
 
-    int st_i = 0, pv_i = 0;
-    uint32_t st_ph = 0, st_off = 0, pv_off = 0;
+    int st_i = 0;
+    uint32_t st_ph = 0, st_off = 0;
     for (int sg = seg_lo; sg < seg_hi; ++sg) {
         const Segment Sg = P.segs[sg];
         const int i = Sg.i0 - 4 + 4 * tx, j = Sg.j0 - 1 + ty;
@@ -828,24 +839,18 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_inverse(const __grid_constant
         const int own_xy = j * G.nx + i;
         float4 cHx = splat(0.f), cHy = cHx;      // H_x, H_y of plane kk-1 at my cells
 
-        // the first plane's stage becomes the held one
-        mbar_wait(&full[st_i], st_ph);
-        pv_i = st_i; pv_off = st_off;
-        st_off += P.stage;
-        if (++st_i == nst) { st_i = 0; st_off = 0; st_ph ^= 1; }
-
         for (int kk = Sg.k0 - 1; kk < Sg.k1; ++kk) {
             const bool prolog = kk == Sg.k0 - 1;
             const bool inz = kk >= G.lo[2] && kk < G.hi[2];
-            mbar_wait(&full[st_i], st_ph);                          // plane kk+1 (E'_x, E'_y at my cells)
-            const uint32_t sp = stage_base + pv_off + o_own;        // plane kk
-            const uint32_t so = stage_base + st_off + o_own;
+            mbar_wait(&full[st_i], st_ph);
+            const uint32_t sb = stage_base + st_off;
+            const uint32_t sA = sb + oA, sB = sb + OB + oB, sD = sb + OD + oB, sC = sb + OC + oC;
             // ------------------------------------------------------------ H of plane kk
-            const float4 Ex = lds4(sp), Ey = lds4(sp + C::SLOT), Ez = lds4(sp + 2 * C::SLOT);
-            const float4 Ex_py = lds4(sp + C::ROWB), Ez_py = lds4(sp + 2 * C::SLOT + C::ROWB);
-            const float Ey_px = lds1(sp + C::SLOT + 16), Ez_px = lds1(sp + 2 * C::SLOT + 16);
-            const float4 Ex_pz = lds4(so), Ey_pz = lds4(so + C::SLOT);
-            const float4 Hpx = lds4(sp + 3 * C::SLOT), Hpy = lds4(sp + 4 * C::SLOT), Hpz = lds4(sp + 5 * C::SLOT);
+            const float4 Ex = lds4(sA), Ey = lds4(sA + C::SLOT), Ez = lds4(sA + 2 * C::SLOT);
+            const float4 Ex_py = lds4(sA + C::ROWB), Ez_py = lds4(sA + 2 * C::SLOT + C::ROWB);
+            const float Ey_px = lds1(sA + C::SLOT + 16), Ez_px = lds1(sA + 2 * C::SLOT + 16);
+            const float4 Ex_pz = lds4(sD), Ey_pz = lds4(sD + C::SLOTB);
+            const float4 Hpx = lds4(sB), Hpy = lds4(sB + C::SLOTB), Hpz = lds4(sB + 2 * C::SLOTB);
             const float4 Dy_z = Ez_py - Ez, Dy_x = Ex_py - Ex;
             const float4 Dx_y = dplus_x(Ey, Ey_px), Dx_z = dplus_x(Ez, Ez_px);
             const float4 Dz_x = Ex_pz - Ex, Dz_y = Ey_pz - Ey;
@@ -862,67 +867,58 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_inverse(const __grid_constant
             Hx = sel4(m0 && inz, m1 && inz, m2 && inz, m3 && inz, Hx, Hpx);
             Hy = sel4(m0 && inz, m1 && inz, m2 && inz, m3 && inz, Hy, Hpy);
             Hz = sel4(m0 && inz, m1 && inz, m2 && inz, m3 && inz, Hz, Hpz);
-            if (prolog) {
-                cHx = Hx; cHy = Hy;
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&empty[pv_i]);
-                pv_i = st_i; pv_off = st_off;
-                st_off += P.stage;
-                if (++st_i == nst) { st_i = 0; st_off = 0; st_ph ^= 1; }
-                continue;
-            }
-            const uint32_t rg = ring_base + (uint32_t)(kk & 1) * (C::RING_SLOT * 4) + r_own;
-            sts4(rg, Hx); sts4(rg + C::RING_ARR * 4, Hy); sts4(rg + 2 * C::RING_ARR * 4, Hz);
-            const int off = kk * plane + own_xy;
-            float4 gv = splat(0.f);
-            const bool gz = kk >= G.glo[2] && kk < G.ghi[2];
-            if (own_ok && gz && gall) gv = ld4(P.grad + off);
-            named_bar_sync(1, C::NCW * 32);
-            // ------------------------------------------------------------ q, gradient, E of plane kk
-            if (own_ok) {
-                const float4 Hx_my = lds4(rg - C::RP * 4), Hz_my = lds4(rg + 2 * C::RING_ARR * 4 - C::RP * 4);
-                const float Hy_mx = lds1(rg + C::RING_ARR * 4 - 4), Hz_mx = lds1(rg + 2 * C::RING_ARR * 4 - 4);
-                const float4 By_z = Hz - Hz_my, By_x = Hx - Hx_my;
-                const float4 Bx_y = dminus_x(Hy, Hy_mx), Bx_z = dminus_x(Hz, Hz_mx);
-                const float4 Bz_x = Hx - cHx, Bz_y = Hy - cHy;
-                const float4 qx = By_z - Bz_y, qy = Bz_x - Bx_z, qz = Bx_y - By_x;
-                const float4 sie = S * lds4(sp + 6 * C::SLOT);
-                const float4 lx = lds4(sp + 7 * C::SLOT), ly = lds4(sp + 8 * C::SLOT), lz = lds4(sp + 9 * C::SLOT);
-                float4 E2x = Ex - sie * qx, E2y = Ey - sie * qy, E2z = Ez - sie * qz;
-                if (kk >= P.sEl && kk < P.sEh) {
-                    const int sm = src_mask(P, kk);
-                    if (sm & 1) E2x = E2x - add_sources4(P, n, 0, splat(0.f), i, j, kk);
-                    if (sm & 2) E2y = E2y - add_sources4(P, n, 1, splat(0.f), i, j, kk);
-                    if (sm & 4) E2z = E2z - add_sources4(P, n, 2, splat(0.f), i, j, kk);
-                }
-                float *o = dst + off;
-                st_masked(o, E2x, mall, m0, m1, m2, m3);
-                st_masked(o + nc, E2y, mall, m0, m1, m2, m3);
-                st_masked(o + 2 * nc, E2z, mall, m0, m1, m2, m3);
-                st_masked(o + 3 * nc, Hx, mall, m0, m1, m2, m3);
-                st_masked(o + 4 * nc, Hy, mall, m0, m1, m2, m3);
-                st_masked(o + 5 * nc, Hz, mall, m0, m1, m2, m3);
-                if (gz && gany) {
-                    const float4 ga = S * fma4(lx, qx, fma4(ly, qy, lz * qz));
-                    if (gall) stg4(P.grad + off, gv + ga);
-                    else {
-                        float *gp = P.grad + off;
-                        if (g0) gp[0] += ga.x;
-                        if (g1) gp[1] += ga.y;
-                        if (g2) gp[2] += ga.z;
-                        if (g3) gp[3] += ga.w;
+            if (!prolog) {
+                const uint32_t rg = ring_base + (uint32_t)(kk & 1) * (3 * C::RING_ARR * 4) + r_own;
+                sts4(rg, Hx); sts4(rg + C::RING_ARR * 4, Hy); sts4(rg + 2 * C::RING_ARR * 4, Hz);
+                const int off = kk * plane + own_xy;
+                float4 gv = splat(0.f);
+                const bool gz = kk >= G.glo[2] && kk < G.ghi[2];
+                if (own_ok && gz && gall) gv = ld4(P.grad + off);
+                named_bar_sync(1, C::NCW * 32);
+                // ------------------------------------------------------------ q, gradient, E of plane kk
+                if (own_ok) {
+                    const float4 Hx_my = lds4(rg - C::RP * 4), Hz_my = lds4(rg + 2 * C::RING_ARR * 4 - C::RP * 4);
+                    const float Hy_mx = lds1(rg + C::RING_ARR * 4 - 4), Hz_mx = lds1(rg + 2 * C::RING_ARR * 4 - 4);
+                    const float4 By_z = Hz - Hz_my, By_x = Hx - Hx_my;
+                    const float4 Bx_y = dminus_x(Hy, Hy_mx), Bx_z = dminus_x(Hz, Hz_mx);
+                    const float4 Bz_x = Hx - cHx, Bz_y = Hy - cHy;
+                    const float4 qx = By_z - Bz_y, qy = Bz_x - Bx_z, qz = Bx_y - By_x;
+                    const float4 sie = S * lds4(sC);
+                    const float4 lx = lds4(sC + C::SLOTC), ly = lds4(sC + 2 * C::SLOTC), lz = lds4(sC + 3 * C::SLOTC);
+                    float4 E2x = Ex - sie * qx, E2y = Ey - sie * qy, E2z = Ez - sie * qz;
+                    if (kk >= P.sEl && kk < P.sEh) {
+                        const int sm = src_mask(P, kk);
+                        if (sm & 1) E2x = E2x - add_sources4(P, n, 0, splat(0.f), i, j, kk);
+                        if (sm & 2) E2y = E2y - add_sources4(P, n, 1, splat(0.f), i, j, kk);
+                        if (sm & 4) E2z = E2z - add_sources4(P, n, 2, splat(0.f), i, j, kk);
+                    }
+                    float *o = dst + off;
+                    st_masked(o, E2x, mall, m0, m1, m2, m3);
+                    st_masked(o + nc, E2y, mall, m0, m1, m2, m3);
+                    st_masked(o + 2 * nc, E2z, mall, m0, m1, m2, m3);
+                    st_masked(o + 3 * nc, Hx, mall, m0, m1, m2, m3);
+                    st_masked(o + 4 * nc, Hy, mall, m0, m1, m2, m3);
+                    st_masked(o + 5 * nc, Hz, mall, m0, m1, m2, m3);
+                    if (gz && gany) {
+                        const float4 ga = S * fma4(lx, qx, fma4(ly, qy, lz * qz));
+                        if (gall) stg4(P.grad + off, gv + ga);
+                        else {
+                            float *gp = P.grad + off;
+                            if (g0) gp[0] += ga.x;
+                            if (g1) gp[1] += ga.y;
+                            if (g2) gp[2] += ga.z;
+                            if (g3) gp[3] += ga.w;
+                        }
                     }
                 }
             }
             cHx = Hx; cHy = Hy;
+            // nothing of this plane is read from its stage again
             __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[pv_i]);
-            pv_i = st_i; pv_off = st_off;
+            if (lane == 0) mbar_arrive(&empty[st_i]);
             st_off += P.stage;
             if (++st_i == nst) { st_i = 0; st_off = 0; st_ph ^= 1; }
         }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&empty[pv_i]);      // the stage of plane k1
     }
 }
 
@@ -963,7 +959,7 @@ bool encode3d(CUtensorMap *out, const float *base, long long dx, long long dy, l
 
 // ---- the compiled tile shapes ----------------------------------------------------------------------
 struct TileImpl {
-    int TX, TY, threads, ncw, stage, ring_bytes;
+    int TX, TY, threads, ncw, stage, ring_bytes, istage, iring_bytes;
     void (*launch_fwd)(const StepParams &, int n_cta, size_t smem, cudaStream_t);
     void (*launch_adj)(const StepParams &, int n_cta, size_t smem, cudaStream_t);
     cudaError_t (*set_smem)(size_t);
@@ -1004,11 +1000,17 @@ template <class C> cudaError_t set_smem_impl(size_t smem)
     return e;
 }
 #define TILE(TX4, TY) { 4 * TX4, TY, Cfg<TX4, TY>::THREADS, Cfg<TX4, TY>::NCW, Cfg<TX4, TY>::STAGE, Cfg<TX4, TY>::RING_BYTES, \
+                        Cfg<TX4, TY>::ISTAGE, Cfg<TX4, TY>::IRING_BYTES, \
                         launch_fwd_impl<Cfg<TX4, TY>>, launch_adj_impl<Cfg<TX4, TY>>, set_smem_impl<Cfg<TX4, TY>>, \
                         launch_inv_impl<Cfg<TX4, TY>>, set_smem_inv_impl<Cfg<TX4, TY>> }
+// shapes compiled for the inverse step only (widths that cover common interiors without a ragged second tile column)
+#define ITILE(TX4, TY) { 4 * TX4, TY, Cfg<TX4, TY>::THREADS, Cfg<TX4, TY>::NCW, Cfg<TX4, TY>::STAGE, Cfg<TX4, TY>::RING_BYTES, \
+                         Cfg<TX4, TY>::ISTAGE, Cfg<TX4, TY>::IRING_BYTES, nullptr, nullptr, nullptr, \
+                         launch_inv_impl<Cfg<TX4, TY>>, set_smem_inv_impl<Cfg<TX4, TY>> }
 const TileImpl kTiles[] = {
     TILE(2, 3), TILE(4, 3), TILE(8, 7), TILE(16, 7), TILE(16, 15), TILE(25, 7), TILE(25, 11),
     TILE(32, 7), TILE(32, 11), TILE(50, 7), TILE(50, 11), TILE(62, 7),
+    ITILE(36, 7), ITILE(40, 7), ITILE(44, 7), ITILE(48, 7), ITILE(56, 7),
 };
 constexpr int kNumTiles = sizeof(kTiles) / sizeof(kTiles[0]);
 
@@ -1339,6 +1341,7 @@ int fused_setup(fdtd_grid *g)
     int best_nst = 0;
     for (int q = 0; q < kNumTiles; ++q) {
         const TileImpl &t = kTiles[q];
+        if (!t.launch_fwd) continue;                                 // inverse-only shape
         if (fTX && (t.TX != fTX || t.TY != fTY)) continue;
         const int xs_pitch = G.d > 0 ? (2 * G.dpx * (t.TY + 2) * 4 + 127) / 128 * 128 : 0;
         const int stage = t.stage + 4 * xs_pitch;
@@ -1364,8 +1367,8 @@ int fused_setup(fdtd_grid *g)
     if ((rc = g->alloc((void **)&F->bufB, (size_t)G.nc * 6 * sizeof(float)))) return rc;
     if ((rc = g->alloc_psi(g->psiE[1])) || (rc = g->alloc_psi(g->psiH[1]))) return rc;
     for (int q = 0; q < 3; ++q) {
-        if ((rc = g->alloc((void **)&F->d_maps[q], sizeof(CUtensorMap) * 21))) return rc;
-        if (cudaMallocHost((void **)&F->h_maps[q], sizeof(CUtensorMap) * 21) != cudaSuccess) {
+        if ((rc = g->alloc((void **)&F->d_maps[q], sizeof(CUtensorMap) * 24))) return rc;
+        if (cudaMallocHost((void **)&F->h_maps[q], sizeof(CUtensorMap) * 24) != cudaSuccess) {
             (void)cudaGetLastError();
             return fdtd_fail(FDTD_ENOMEM, "pinned tensor-map staging allocation failed");
         }
@@ -1414,9 +1417,11 @@ int fused_setup(fdtd_grid *g)
         for (int q = 0; q < kNumTiles; ++q) {
             const TileImpl &t = kTiles[q];
             if (iTX && (t.TX != iTX || t.TY != iTY)) continue;
-            int nst = std::min(MAX_ST, (smem_cap - t.ring_bytes - tail_bytes - 1024) / (t.stage / 7 * 10));
+            int nst = std::min(MAX_ST, (smem_cap - t.iring_bytes - tail_bytes - 1024) / t.istage);
             if (const char *e = getenv("FDTD_INST")) nst = std::min(nst, atoi(e));
-            if (nst < 3) continue;
+            // every stage is self-contained: one in use, the others in flight; two are enough (measured on C3: 100 x 11
+            // with 2 or 3 stages 92 us; 176 x 7, 192 x 7, 200 x 7 with 2 stages 84-86 us: one tile column over the box wins)
+            if (nst < 2) continue;
             const long long ntx = (nx_i + t.TX - 1) / t.TX, nty = (ny_i + t.TY - 1) / t.TY;
             const double eff = ((double)(G.hi[0] - G.lo[0]) / 4 * ny_i) / ((double)ntx * nty * t.ncw * 32);
             const double fill = std::min(1.0, (double)ntx * nty * nz_i / (8.0 * n_sm));
@@ -1442,8 +1447,8 @@ int fused_setup(fdtd_grid *g)
                 return fdtd_fail(FDTD_ECUDA, "upload of the inverse segment table failed");
             }
             F->itile = ib; F->inst = ib_nst; F->in_cta = in_cta;
-            const int istage = ib->stage / 7 * 10;
-            F->ismem = (size_t)ib_nst * istage + ib->ring_bytes + tail_bytes;
+            const int istage = ib->istage;
+            F->ismem = (size_t)ib_nst * istage + ib->iring_bytes + tail_bytes;
             InvParams &I = F->ip;
             I.G = G; I.segs = F->d_isegs; I.seg_begin = F->d_iseg_begin; I.step = g->d_step;
             I.nst = ib_nst; I.stage = istage;
@@ -1582,21 +1587,26 @@ int build_inv_maps(fdtd_grid *g, float *volA, float *volB, const float *ie, floa
     FusedState *F = g->fused;
     const Dims &G = g->G;
     if (F->maps_key[2][0] == volA && F->maps_key[2][1] == ie) return FDTD_OK;
-    const int PW = F->itile->TX + 8, ROWS = F->itile->TY + 2;
+    const int TXi = F->itile->TX, TYi = F->itile->TY;
     if (cudaEventSynchronize(F->maps_done) != cudaSuccess) { (void)cudaGetLastError(); }
     CUtensorMap *H = F->h_maps[2];
     bool ok = true;
     float *bufs[2] = { volA, volB }, *lams[2] = { lamA, lamB };
     const long long pl = (long long)G.nx * G.ny;
+    // three box shapes (see k_inverse): A [TY+2][TX+8], B [TY+1][TX+4], C [TY][TX]
     for (int set = 0; set < 2; ++set) {
-        for (int c = 0; c < 6; ++c)
-            ok &= encode3d(&H[set * 6 + c], bufs[set] + (long long)c * G.nc, G.nx, G.ny, G.nz, G.nx, pl, PW, ROWS);
         for (int c = 0; c < 3; ++c)
-            ok &= encode3d(&H[13 + set * 3 + c], lams[set] + (long long)c * G.nc, G.nx, G.ny, G.nz, G.nx, pl, PW, ROWS);
+            ok &= encode3d(&H[set * 3 + c], bufs[set] + (long long)c * G.nc, G.nx, G.ny, G.nz, G.nx, pl, TXi + 8, TYi + 2);
+        for (int q = 0; q < 5; ++q) {
+            const int comp = q < 3 ? 3 + q : q - 3;                  // H'_x, H'_y, H'_z, E'_x, E'_y
+            ok &= encode3d(&H[6 + set * 5 + q], bufs[set] + (long long)comp * G.nc, G.nx, G.ny, G.nz, G.nx, pl, TXi + 4, TYi + 1);
+        }
+        for (int c = 0; c < 3; ++c)
+            ok &= encode3d(&H[17 + set * 3 + c], lams[set] + (long long)c * G.nc, G.nx, G.ny, G.nz, G.nx, pl, TXi, TYi);
     }
-    ok &= encode3d(&H[12], ie, G.nx, G.ny, G.nz, G.nx, pl, PW, ROWS);
+    ok &= encode3d(&H[16], ie, G.nx, G.ny, G.nz, G.nx, pl, TXi, TYi);
     if (!ok) return fdtd_fail(FDTD_ECUDA, "cuTensorMapEncodeTiled failed");
-    cudaError_t e = cudaMemcpyAsync(F->d_maps[2], H, sizeof(CUtensorMap) * 19, cudaMemcpyHostToDevice, st);
+    cudaError_t e = cudaMemcpyAsync(F->d_maps[2], H, sizeof(CUtensorMap) * 23, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaEventRecord(F->maps_done, st);
     if (e != cudaSuccess) { (void)cudaGetLastError(); return fdtd_fail(FDTD_ECUDA, std::string("tensor map upload: ") + cudaGetErrorString(e)); }
     F->maps_key[2][0] = volA; F->maps_key[2][1] = ie;
@@ -1935,7 +1945,7 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
             if (e != cudaSuccess) { (void)cudaGetLastError(); return fdtd_fail(FDTD_ECUDA, cudaGetErrorString(e)); }
         }
         InvParams &I = ctx.I;
-        I.maps = F->d_maps[2]; I.lmaps = F->d_maps[2] + 13;
+        I.maps = F->d_maps[2];
         I.buf[0] = fields; I.buf[1] = F->bufB; I.grad = dL_dinv_eps; I.im = inv_mu;
         I.n_src = (int)S.size();
         I.sEl = I.sHl = 1 << 30; I.sEh = I.sHh = -1;
