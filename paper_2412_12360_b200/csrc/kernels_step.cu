@@ -12,7 +12,8 @@
 //   * only the three arrays that are differenced in phase A (the H-type operand F) need neighbours: one
 //     producer thread streams their boxes (one-cell halo, 16-byte aligned in x) global -> shared with TMA
 //     (cp.async.bulk.tensor; the zero fill outside the grid IS the zero-pad wall convention R7) through a
-//     ring of NST stages with full/empty mbarriers.  The E-type target, inv_eps and the x-slab CPML states
+//     ring of NST stages with full/empty mbarriers (a stage is released when its own plane is done: what the next
+//     plane needs of it -- F at a thread's own cells -- travels in registers).  The E-type target, inv_eps and the x-slab CPML states
 //     travel in the same stage (seven boxes plus four narrow ones); only the y / z slab CPML states (and inv_mu)
 //     are read straight from global memory as float4 at a thread's own cells;
 //   * consumer warps are 8 x 4 patches of float4 threads (128 B contiguous per patch row), so CPML slab
@@ -407,8 +408,6 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
     int st_i = 0;                 // pipeline stage of the next plane
     uint32_t st_ph = 0;           // its full-barrier parity
     uint32_t st_off = 0;          // st_i * STAGE
-    int pv_i = 0;                 // the stage that holds the previous plane
-    uint32_t pv_off = 0;
     float4 cgx = Z4, cgy = Z4, cZx = Z4, cZy = Z4;   // adjoint: z-filtered operands of the previous plane at my cells
     // forward: F of the previous plane at my cells (= the H-type target of phase B) travels in registers, so a stage is
     // released as soon as its own plane is done and the ring of NST stages keeps one more plane in flight
@@ -435,7 +434,6 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
             const int zs = (pml && !DBG(128)) ? zslab_pos(G, kk) : -1;
             mbar_wait(&full[st_i], st_ph);
             const uint32_t so = stage_base + st_off + o_own;
-            const uint32_t sp = stage_base + pv_off + o_own;       // the stage of plane kk-1 is still held
             if (ADJ && kk >= P.dEl && kk < P.dEh && !dup) {
                 // B1 for E-component detectors: the cotangents are added to lamE in the stage, at my cells, before
                 // anything is live in registers (lamE is only ever read at a thread's own cells)
@@ -643,7 +641,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                     }
                 }
                 const float4 tHx = Dy_z - Dz_y, tHy = Dz_x - Dx_z, tHz = Dx_y - Dy_x;
-                const float4 hx = ADJ ? lds4(sp) : pFx, hy = ADJ ? lds4(sp + C::SLOT) : pFy, hz = ADJ ? lds4(sp + 2 * C::SLOT) : pFz;
+                const float4 hx = pFx, hy = pFy, hz = pFz;
                 float4 h2x, h2y, h2z;
                 if (ADJ) {
                     // with inv_mu the H part of the cotangent volumes holds Lambda_H = im lamH (fused_backward): phase A
@@ -664,12 +662,11 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                 stg4(o, h2x); stg4(o + nc, h2y); stg4(o + 2 * nc, h2z);
                 if (!ADJ && km1 >= P.dHl && km1 < P.dHh) detect4(P, n, 1, det_mask(P, km1, false), h2x, h2y, h2z, i, j, km1);
             }
-            if (ADJ) { cZx = Zx; cZy = Zy; } else { pFx = fx; pFy = fy; pFz = fz; }
-            // adjoint: the stage of plane kk-1 is no longer needed, the stage of plane kk stays for the next iteration;
-            // forward: nothing of plane kk is read from its stage again
+            if (ADJ) { cZx = Zx; cZy = Zy; }
+            pFx = fx; pFy = fy; pFz = fz;
+            // nothing of plane kk is read from its stage again
             __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[ADJ ? pv_i : st_i]);
-            pv_i = st_i; pv_off = st_off;
+            if (lane == 0) mbar_arrive(&empty[st_i]);
             st_off += P.stage;
             if (++st_i == nst) { st_i = 0; st_off = 0; st_ph ^= 1; }
             if (!DBG(4)) named_bar_sync(1, C::NCW * 32);      // ring slot (kk-1)&1 may be overwritten in the next iteration
@@ -693,22 +690,17 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                     }
                 }
             }
-            if (!ADJ) {
+            {
                 const uint32_t so = stage_base + st_off + o_own;
                 pFx = lds4(so); pFy = lds4(so + C::SLOT); pFz = lds4(so + 2 * C::SLOT);
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&empty[st_i]);
             }
-            pv_i = st_i; pv_off = st_off;
             st_off += P.stage;
             if (++st_i == nst) { st_i = 0; st_off = 0; st_ph ^= 1; }
         }
         plane_step(Sg.k0, false);
         for (int kk = Sg.k0 + 1; kk <= k1; ++kk) plane_step(kk, true);
-        if (ADJ) {
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[pv_i]);      // the stage of plane k1
-        }
     }
     if (P.dbg_t && threadIdx.x == 0) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); P.dbg_t[2 * blockIdx.x + 1] = t; }
 }
