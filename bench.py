@@ -247,6 +247,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--lean", action="store_true",
                     help="memory-scale runs: no second (forward-only) grid, hence no forward-only and adjoint-only passes")
+    ap.add_argument("--recorder-fp16", action="store_true",
+                    help="SURVEY 8(f) N1: store the interface record as fp16 (FDTD_FLAG_RECORDER_FP16; an approximation, off by default)")
     ap.add_argument("--record", default="", choices=["", "1", "2", "both"],
                     help="1: `value` only (record the PML/interior interface, reconstruct the interior); 2: `value` on the "
                          "design-box recorder instead (labelled); both (default where there is a design box and memory allows): "
@@ -294,7 +296,8 @@ def main():
 
     def make_grid(record, staging=False):
         kw = w.grid_kwargs()
-        kw.update(max_steps=T, record=record, path=path, flags=B.FDTD_FLAG_HOST_STAGING if staging else 0)
+        kw.update(max_steps=T, record=record, path=path,
+                  flags=(B.FDTD_FLAG_HOST_STAGING if staging else 0) | (B.FDTD_FLAG_RECORDER_FP16 if args.recorder_fp16 else 0))
         if has_box:
             kw.update(grad_lo=dlo, grad_hi=dhi)
         return B.Grid(**kw)
@@ -550,7 +553,7 @@ def main():
                                              "parallelism": f"independent problems x{world}",
                                              "partition": B.PARTITION_NAMES.get(int(info.partition), str(info.partition)),
                                              "reverse_sweep": "grouped launches" if info.pipelined_inverse_ctas else "sequential",
-                                             "recorder": rec_names[main_record],
+                                             "recorder": rec_names[main_record] + (", fp16 (FDTD_FLAG_RECORDER_FP16)" if args.recorder_fp16 else ""),
                                              "recorder_bytes": int(info.recorder_bytes), "scratch_bytes": int(info.scratch_bytes)}),
                "fwd": {"value": fwd_value, "unit": UNIT, "ms_per_pass": ms_fwd / max(1, args.steps),
                        "what": "forward only, record=0, same workload"} if ms_fwd else None,

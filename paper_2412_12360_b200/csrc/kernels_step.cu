@@ -66,6 +66,7 @@ struct StepParams {
     int *step_next;                // the other slot: block 0 writes n + step_delta for the next step (or NULL)
     int step_delta;
     int nst;                       // pipeline stages
+    int hold;                      // 1: a stage is released one plane late (the consumers stay one plane closer to the loads)
     int stage;                     // bytes of one stage: 7 boxes + 4 x-slab state boxes
     int xs_bytes, xs_pitch;        // x-slab state box [ROWS][2*dpx]: exact bytes (TMA transaction) and 128-byte aligned pitch
     unsigned long long *dbg_t;     // timing experiments only (FDTD_DBG_TIMES): per-CTA start / end globaltimer
@@ -412,6 +413,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
     // forward: F of the previous plane at my cells (= the H-type target of phase B) travels in registers, so a stage is
     // released as soon as its own plane is done and the ring of NST stages keeps one more plane in flight
     float4 pFx = Z4, pFy = Z4, pFz = Z4;
+    int pv_i = 0;                 // P.hold: the stage of the previous plane
     for (int sg = seg_lo; sg < seg_hi; ++sg) {
         const Segment Sg = segs[sg];
         const int i = Sg.i0 + 4 * tx, j = Sg.j0 + ty;
@@ -664,9 +666,10 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
             }
             if (ADJ) { cZx = Zx; cZy = Zy; }
             pFx = fx; pFy = fy; pFz = fz;
-            // nothing of plane kk is read from its stage again
+            // nothing of plane kk is read from its stage again; with P.hold the stage of plane kk-1 goes instead
             __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[st_i]);
+            if (lane == 0) mbar_arrive(&empty[P.hold ? pv_i : st_i]);
+            pv_i = st_i;
             st_off += P.stage;
             if (++st_i == nst) { st_i = 0; st_off = 0; st_ph ^= 1; }
             if (!DBG(4)) named_bar_sync(1, C::NCW * 32);      // ring slot (kk-1)&1 may be overwritten in the next iteration
@@ -694,13 +697,18 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                 const uint32_t so = stage_base + st_off + o_own;
                 pFx = lds4(so); pFy = lds4(so + C::SLOT); pFz = lds4(so + 2 * C::SLOT);
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&empty[st_i]);
+                if (lane == 0 && !P.hold) mbar_arrive(&empty[st_i]);
             }
+            pv_i = st_i;
             st_off += P.stage;
             if (++st_i == nst) { st_i = 0; st_off = 0; st_ph ^= 1; }
         }
         plane_step(Sg.k0, false);
         for (int kk = Sg.k0 + 1; kk <= k1; ++kk) plane_step(kk, true);
+        if (P.hold) {
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[pv_i]);      // the stage of plane k1
+        }
     }
     if (P.dbg_t && threadIdx.x == 0) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); P.dbg_t[2 * blockIdx.x + 1] = t; }
 }
@@ -1502,6 +1510,11 @@ int fused_setup(fdtd_grid *g)
     P.n_rot = n_rot; P.seg_stride = (int)stride; P.n_cta = n_cta;
     P.step = g->d_step; P.step_next = nullptr; P.step_delta = 0;
     P.nst = F->nst;
+    // whole columns dealt out in waves (more tile columns than CTAs): the CTAs of a wave must stay on the same plane for the
+    // halo rows to be L2 hits, and a producer that runs a second plane ahead lets them drift: measured at 512^3, forward /
+    // adjoint 1494 / 1527 us held against 1700 / 1826 us released early; with lock-step runs (C3) early release wins, 97.8 /
+    // 103.8 against 98.6 / 106.4 us
+    P.hold = getenv("FDTD_HOLD") ? atoi(getenv("FDTD_HOLD")) : (g->partition == FDTD_PARTITION_WAVES ? 1 : 0);
     P.stage = stage_bytes; P.xs_bytes = xs_bytes; P.xs_pitch = xs_pitch;
     P.dbg = getenv("FDTD_DBG") ? atoi(getenv("FDTD_DBG")) : 0;
     P.dbg_t = nullptr;
