@@ -120,7 +120,10 @@ typedef struct {
     int32_t max_steps;         /* upper bound of n_steps; sizes the recorder when record != 0       */
     int32_t record;            /* 0: forward only; 1: record the PML/interior interface every step; */
                                /* 2: record the faces of the gradient box instead (pml_cells > 0):  */
-                               /*    fdtd_backward then reconstructs the fields on that box only    */
+                               /*    fdtd_backward then reconstructs the fields on that box only;   */
+                               /* 3: checkpointed reverse sweep: the  */
+                               /*    whole state every checkpoint_every steps, no inverse step -- see */
+                               /*    "Checkpointed reverse sweep" below                              */
     int32_t grad_lo[3];        /* half-open (i,j,k) box on which dL_dinv_eps is wanted;             */
     int32_t grad_hi[3];        /*   all zero => the whole interior I.  Always clipped to I.         */
     int32_t path;              /* FDTD_PATH_*                                                       */
@@ -131,7 +134,8 @@ typedef struct {
      * interior box and the recorder faces follow the GLOBAL position (an internal cut is recorded like a PML face, so
      * the reverse sweep's inverse step needs no exchange).  See "Domain decomposition" below. */
     int32_t z_global, z_offset, z_ghost_lo, z_ghost_hi;
-    int32_t reserved[2];       /* must be zero                                                      */
+    int32_t checkpoint_every;  /* record == 3: steps between checkpoints; 0 => about sqrt(max_steps)    */
+    int32_t reserved[1];       /* must be zero                                                      */
 } fdtd_grid_desc;
 
 /* Additive source patch (reading R10/R11): during step n,
@@ -204,6 +208,18 @@ FDTD_API int fdtd_backward_mu(fdtd_grid *grid, float *fields, const float *inv_e
                      const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
                      const float *const *dL_dphasor, const float *dL_dfields,
                      int32_t n_steps, float *dL_dinv_eps, float *dL_dinv_mu, float *dL_dfields0, void *cuda_stream);
+
+/* Checkpointed reverse sweep (record == 3, "checkpointing" as the alternative to time reversal).
+ * fdtd_forward stores the whole state (fields and CPML psi) every checkpoint_every steps.  fdtd_backward then works segment by
+ * segment from the last one: it restores the segment's checkpoint, runs the segment's forward steps again keeping
+ * dE = E' - E (sources subtracted) on the gradient box for each of them, and runs the segment's adjoint steps with
+ *   dL_dinv_eps[cell] += sum_c lamE'_c * dE_c / inv_eps      (= S lamE' . bracket of the E update: exact, no inverse step).
+ * Nothing is reconstructed backwards in time, so: the gradient box (grad_lo / grad_hi; all zero = the whole grid) may
+ * include PML cells, `fields` is scratch for the replay (unspecified on return), and the method does not rely on the update
+ * being invertible.  Costs one
+ * more forward pass; memory (max_steps / K) * (6 volumes + psi) + K * 3 * box cells floats (K = checkpoint_every).
+ * Same result as the time-reversed sweep on the interior to its reconstruction rounding; equals the plain reverse-mode
+ * derivative (the oracle's tape mode) on every cell.  Not available with time-domain detectors, range calls or sub-grids. */
 
 /* B6, chain rule to design parameters (once per gradient, not per step): for a design box whose
  * permittivity is eps = eps_bg + delta_eps*rho (reading R20),

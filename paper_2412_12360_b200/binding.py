@@ -33,7 +33,7 @@ class fdtd_grid_desc(C.Structure):
                 ("grad_lo", C.c_int32 * 3), ("grad_hi", C.c_int32 * 3),
                 ("path", C.c_int32), ("flags", C.c_int32),
                 ("z_global", C.c_int32), ("z_offset", C.c_int32), ("z_ghost_lo", C.c_int32), ("z_ghost_hi", C.c_int32),
-                ("reserved", C.c_int32 * 2)]
+                ("checkpoint_every", C.c_int32), ("reserved", C.c_int32 * 1)]
 
 
 class fdtd_source(C.Structure):
@@ -292,7 +292,7 @@ def fdtd_backward_host(grid, h_fields, h_inv_eps, h_inv_mu, src, n_src, det, n_d
 def make_desc(nx, ny, nz, courant, periodic=False, pml_cells=0, pml_m=0.0, pml_sigma_scale=0.0,
               pml_kappa_max=0.0, pml_alpha_max=0.0, pml_alpha_m=0.0, pml_eps_bg=0.0, max_steps=0,
               record=False, grad_lo=None, grad_hi=None, path=FDTD_PATH_AUTO, flags=0,
-              z_global=0, z_offset=0, z_ghost_lo=0, z_ghost_hi=0) -> fdtd_grid_desc:
+              z_global=0, z_offset=0, z_ghost_lo=0, z_ghost_hi=0, checkpoint_every=0) -> fdtd_grid_desc:
     d = fdtd_grid_desc()
     d.nx, d.ny, d.nz, d.courant = nx, ny, nz, courant
     d.periodic, d.pml_cells = int(bool(periodic)), pml_cells
@@ -300,6 +300,7 @@ def make_desc(nx, ny, nz, courant, periodic=False, pml_cells=0, pml_m=0.0, pml_s
     d.pml_alpha_max, d.pml_alpha_m, d.pml_eps_bg = pml_alpha_max, pml_alpha_m, pml_eps_bg
     d.max_steps, d.record, d.path, d.flags = max_steps, int(record), path, int(flags)
     d.z_global, d.z_offset, d.z_ghost_lo, d.z_ghost_hi = int(z_global), int(z_offset), int(z_ghost_lo), int(z_ghost_hi)
+    d.checkpoint_every = int(checkpoint_every)
     if grad_lo is not None:
         d.grad_lo[:] = list(grad_lo)
         d.grad_hi[:] = list(grad_hi)

@@ -173,9 +173,11 @@ extern "C" int fdtd_create_grid(const fdtd_grid_desc *desc, fdtd_grid **out)
     if (desc->pml_cells > 0 && 2 * desc->pml_cells + 2 > mn)
         return fail(FDTD_EINVAL, "need 2*pml_cells + 2 <= min(nx,ny,nz)");
     if (desc->max_steps < 0) return fail(FDTD_EINVAL, "max_steps must be >= 0");
-    if (desc->record < 0 || desc->record > 2) return fail(FDTD_EINVAL, "record must be 0, 1 or 2");
+    if (desc->record < 0 || desc->record > 3) return fail(FDTD_EINVAL, "record must be 0, 1, 2 or 3");
+    if (desc->checkpoint_every < 0) return fail(FDTD_EINVAL, "checkpoint_every must be >= 0");
+    if (desc->record == 3 && desc->z_global) return fail(FDTD_EINVAL, "the checkpointed reverse sweep is not available on a z-slab sub-grid");
     if (desc->path < 0 || desc->path > 2) return fail(FDTD_EINVAL, "unknown path");
-    for (int q = 0; q < 2; ++q) if (desc->reserved[q]) return fail(FDTD_EINVAL, "reserved fields must be zero");
+    if (desc->reserved[0]) return fail(FDTD_EINVAL, "reserved fields must be zero");
     if (desc->flags & ~(FDTD_FLAG_HOST_STAGING | FDTD_FLAG_RECORDER_FP16)) return fail(FDTD_EINVAL, "unknown bit in flags");
     if (desc->pml_m < 0 || desc->pml_sigma_scale < 0 || desc->pml_kappa_max < 0 || desc->pml_alpha_max < 0 ||
         desc->pml_alpha_m < 0 || desc->pml_eps_bg < 0)
@@ -217,6 +219,12 @@ extern "C" int fdtd_create_grid(const fdtd_grid_desc *desc, fdtd_grid **out)
             G.ghi[a] = std::max(G.glo[a], std::min(desc->grad_hi[a], G.hi[a]));
         }
     }
+    // record == 3 (checkpointed reverse sweep): no inverse step, so the gradient box is any box of the grid, PML included
+    if (desc->record == 3)
+        for (int a = 0; a < 3; ++a) {
+            G.glo[a] = all_zero ? 0 : desc->grad_lo[a];
+            G.ghi[a] = all_zero ? dim_of(G, a) : desc->grad_hi[a];
+        }
     // record == 2 (NEXT N1, design-box recorder): the reconstruction box shrinks from the interior I to the
     // gradient box -- the faces recorded, the inverse step and the reconstructed fields all follow G.lo / G.hi
     if (desc->record == 2 && G.d > 0) {
@@ -269,9 +277,21 @@ extern "C" int fdtd_create_grid(const fdtd_grid_desc *desc, fdtd_grid **out)
     if ((rc = g->alloc((void **)&g->red.partial, RED_BLOCKS * sizeof(double))) || (rc = g->alloc((void **)&g->red.ticket, 64))) return bail(rc);
     if (cudaMemset(g->red.ticket, 0, 64) != cudaSuccess) return bail(cuda_fail(cudaGetLastError(), "cudaMemset"));
     if ((rc = g->alloc_psi(g->psiE[0])) || (rc = g->alloc_psi(g->psiH[0]))) return bail(rc);
-    if (desc->record && G.d > 0 && desc->max_steps > 0) {
+    if ((desc->record == 1 || desc->record == 2) && G.d > 0 && desc->max_steps > 0) {
         const size_t bytes = (size_t)g->R.stride * (g->R.half ? 2 : sizeof(float)) * (size_t)desc->max_steps;
         if ((rc = g->alloc((void **)&g->rec, bytes, true))) return bail(rc);
+    }
+    if (desc->record == 3 && desc->max_steps > 0) {
+        // checkpoints of the whole state (6 volumes + the 12 psi arrays) every K steps, and dE = E' - E on the gradient box
+        // for the K steps of one segment; K defaults to ~sqrt(max_steps), which minimises their sum for a box of the grid's size
+        g->ck_every = desc->checkpoint_every > 0 ? desc->checkpoint_every : std::max(1, (int)std::lround(std::sqrt((double)desc->max_steps)));
+        g->ck_count = (desc->max_steps + g->ck_every - 1) / g->ck_every;
+        size_t psi_floats = 0;
+        for (int c = 0; c < 3; ++c) for (int q = 0; q < 2; ++q) psi_floats += (size_t)psi_elems(G, psi_axis(c, q));
+        g->ck_stride = 6 * (size_t)G.nc + 2 * psi_floats;
+        const size_t box = (size_t)(G.ghi[0] - G.glo[0]) * (G.ghi[1] - G.glo[1]) * (G.ghi[2] - G.glo[2]);
+        if ((rc = g->alloc((void **)&g->ckpt, g->ck_stride * g->ck_count * sizeof(float), true))) return bail(rc);
+        if ((rc = g->alloc((void **)&g->dE, 3 * box * (size_t)g->ck_every * sizeof(float), true))) return bail(rc);
     }
     {
         cudaError_t e = cudaStreamCreateWithFlags(&g->cap_stream, cudaStreamNonBlocking);
@@ -616,6 +636,56 @@ extern "C" int fdtd_forward(fdtd_grid *g, float *fields, const float *inv_eps, c
 static int forward_impl(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
                         const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
                         const fdtd_time_detector *td, int32_t n_td, int n_begin, int n_end, int n_total, void *cuda_stream);
+static int forward_core(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
+                        const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
+                        const fdtd_time_detector *td, int32_t n_td, int n_begin, int n_end, int n_total, void *cuda_stream);
+
+// record = 3: the whole state n (fields + the psi set state n lives in) to / from checkpoint slot idx
+static int copy_checkpoint(fdtd_grid *g, float *fields, bool fused, int n, int idx, bool restore, cudaStream_t st)
+{
+    const Dims &G = g->G;
+    float *ck = g->ckpt + (size_t)idx * g->ck_stride;
+    float *vol = fused ? fused_volume(g, fields, 0, n) : fields;
+    const int set = fused ? (n & 1) : 0;
+    auto cp = [&](float *dev, float *slot, size_t floats) -> cudaError_t {
+        return floats ? cudaMemcpyAsync(restore ? dev : slot, restore ? slot : dev, floats * sizeof(float), cudaMemcpyDeviceToDevice, st) : cudaSuccess;
+    };
+    CK(cp(vol, ck, 6 * (size_t)G.nc));
+    size_t off = 6 * (size_t)G.nc;
+    for (int fam = 0; fam < 2; ++fam)
+        for (int c = 0; c < 3; ++c)
+            for (int q = 0; q < 2; ++q) {
+                const size_t fl = (size_t)psi_elems(G, psi_axis(c, q));
+                CK(cp((fam ? g->psiH[set] : g->psiE[set]).p[c][q], ck + off, fl));
+                off += fl;
+            }
+    return FDTD_OK;
+}
+
+// fdtd_forward on a record = 3 grid: segment by segment, a checkpoint of the state in front of each
+static int forward_impl(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
+                        const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
+                        const fdtd_time_detector *td, int32_t n_td, int n_begin, int n_end, int n_total, void *cuda_stream)
+{
+    if (!g || g->desc.record != 3)
+        return forward_core(g, fields, inv_eps, inv_mu, src, n_src, det, n_det, td, n_td, n_begin, n_end, n_total, cuda_stream);
+    if (n_td) return fail(FDTD_EINVAL, "time-domain detectors are not available on a record = 3 grid");
+    if (n_begin != 0 || n_end != n_total) return fail(FDTD_EINVAL, "range calls are not available on a record = 3 grid");
+    if (!fields) return fail(FDTD_EINVAL, "fdtd_forward: fields and inv_eps are required");
+    const bool fused = g->path == FDTD_PATH_FUSED && n_src <= FDTD_FUSED_MAX_SRC && n_det <= FDTD_FUSED_MAX_DET;
+    const int K = g->ck_every;
+    int rc = FDTD_OK;
+    if (n_total == 0) return forward_core(g, fields, inv_eps, inv_mu, src, n_src, det, n_det, nullptr, 0, 0, 0, 0, cuda_stream);
+    if (n_total > g->desc.max_steps) return fail(FDTD_EINVAL, "fdtd_forward: need 0 <= n_steps <= max_steps");
+    for (int a = 0; a < n_total && !rc; a += K) {
+        const int b = std::min(n_total, a + K);
+        if (a > 0) rc = copy_checkpoint(g, fields, fused, a, a / K, false, (cudaStream_t)cuda_stream);   // (state 0 is restored by zeroing psi: slot 0 holds the fields only)
+        else CK(cudaMemcpyAsync(g->ckpt, fields, 6 * (size_t)g->G.nc * sizeof(float), cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
+        if (!rc) rc = forward_core(g, fields, inv_eps, inv_mu, src, n_src, det, n_det, nullptr, 0, a, b, n_total, cuda_stream);
+    }
+    if (!rc) g->recorded_steps = n_total;
+    return rc;
+}
 
 extern "C" int fdtd_forward_td(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
                                const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
@@ -634,7 +704,7 @@ extern "C" int fdtd_forward_range(fdtd_grid *g, float *fields, const float *inv_
 }
 
 // steps n_begin .. n_end-1 of a run of n_total steps (fdtd_forward: 0 .. n_steps-1)
-static int forward_impl(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
+static int forward_core(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
                         const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
                         const fdtd_time_detector *td, int32_t n_td, int n_begin, int n_end, int n_total, void *cuda_stream)
 {
@@ -652,7 +722,7 @@ static int forward_impl(fdtd_grid *g, float *fields, const float *inv_eps, const
     for (const TimeDetDev &q : TD) if (!q.out) return fail(FDTD_EINVAL, "fdtd_forward_td: time detector out is NULL");
     translate(src, n_src, S);
     const int total_freq = translate(det, n_det, D);
-    const bool recording = g->desc.record && G.d > 0;
+    const bool recording = (g->desc.record == 1 || g->desc.record == 2) && G.d > 0;
     g->recorded_steps = -1;
     g->fwd_pos = -1;
     if ((rc = upload_cs_table(g, det, n_det, total_freq, n_steps, st))) return rc;
@@ -755,8 +825,66 @@ extern "C" int fdtd_backward_range(fdtd_grid *g, float *fields, const float *inv
                          n_hi, n_lo, n_total, dL_dinv_eps, dL_dfields0, cuda_stream);
 }
 
-// reverse steps n_hi-1 .. n_lo of a run of n_total steps (fdtd_backward: n_steps-1 .. 0); the cotangent seed (B0) is
-// placed by the call with n_hi == n_total, dL_dfields0 is written by the call with n_lo == 0
+static int backward_core(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
+                         const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
+                         const float *const *dL_dphasor,
+                         const fdtd_time_detector *td, int32_t n_td, const float *const *dL_dtd,
+                         const float *dL_dfields, int n_hi, int n_lo, int n_total, float *dL_dinv_eps, float *dL_dfields0,
+                         void *cuda_stream, float *dL_dinv_mu, bool sweep_only);
+
+// record = 3: the reverse sweep from checkpoints, segment by segment from the last one --
+// restore the checkpoint, run the segment's forward steps again keeping dE = E' - E (sources subtracted) on the gradient box,
+// then the segment's adjoint steps, each followed by g += sum_c lamE'_c dE_c / inv_eps.  No inverse step.
+static int checkpointed_backward(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
+                                 const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
+                                 const float *const *dL_dphasor, const float *dL_dfields, int n_total,
+                                 float *dL_dinv_eps, float *dL_dfields0, void *cuda_stream)
+{
+    const Dims &G = g->G;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (g->recorded_steps != n_total) return fail(FDTD_ESTATE, "fdtd_backward: no matching checkpointed forward (need record=3 and the same n_steps)");
+    std::vector<SourceDev> S;
+    translate(src, n_src, S);
+    const bool fused_f = g->path == FDTD_PATH_FUSED && n_src <= FDTD_FUSED_MAX_SRC;      // the replay runs without detectors
+    const size_t vol = (size_t)G.nc * sizeof(float);
+    const size_t box = (size_t)(G.ghi[0] - G.glo[0]) * (G.ghi[1] - G.glo[1]) * (G.ghi[2] - G.glo[2]);
+    CK(cudaMemsetAsync(dL_dinv_eps, 0, vol, st));
+    const int K = g->ck_every;
+    int rc = FDTD_OK;
+    for (int a = (n_total - 1) / K * K; a >= 0 && n_total > 0; a -= K) {
+        const int b = std::min(n_total, a + K);
+        // ---- the segment's forward steps again, from its checkpoint
+        if (a > 0) { if ((rc = copy_checkpoint(g, fields, fused_f, a, a / K, true, st))) return rc; }
+        else CK(cudaMemcpyAsync(fields, g->ckpt, 6 * vol, cudaMemcpyDeviceToDevice, st));
+        for (int n = a; n < b; ++n) {
+            float *dE = g->dE + (size_t)(n - a) * 3 * box;
+            if (!fused_f) launch_dE_store(G, fields, nullptr, dE, 1, g->d_step, st);          // in-place step: -E before
+            g->replaying = true;
+            rc = forward_core(g, fields, inv_eps, inv_mu, src, n_src, nullptr, 0, nullptr, 0, n, n + 1, n_total, st);
+            g->replaying = false;
+            if (rc) return rc;
+            // the step's first launch read n from counter slot 0, which still holds it
+            if (fused_f) launch_dE_store(G, fields, fused_volume(g, fields, 0, 1), dE, 0, g->d_step, st);
+            else         launch_dE_store(G, fields, nullptr, dE, 2, g->d_step, st);
+            for (const SourceDev &q : S) if (q.comp < 3) launch_dE_source(G, dE, q, g->d_step, st);
+            g->kernel_launches += 2 + (fused_f ? 0 : 1);
+        }
+        // ---- the segment's adjoint steps, gradient from the stored dE
+        for (int n = b - 1; n >= a; --n) {
+            if ((rc = backward_core(g, fields, inv_eps, inv_mu, src, n_src, det, n_det, dL_dphasor, nullptr, 0, nullptr, dL_dfields,
+                                    n + 1, n, n_total, nullptr, dL_dfields0, st, nullptr, true))) return rc;
+            launch_grad_from_dE(G, g->lam, g->bwd_fused ? fused_volume(g, fields, 1, 1) : nullptr, g->dE + (size_t)(n - a) * 3 * box,
+                                inv_eps, dL_dinv_eps, g->d_step, st);
+            g->kernel_launches += 1;
+        }
+    }
+    // (`fields` was the replay's scratch: it ends at the state the first segment's replay left)
+    g->recorded_steps = n_total;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "fdtd_backward launch");
+    return FDTD_OK;
+}
+
 static int backward_impl(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
                          const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
                          const float *const *dL_dphasor,
@@ -764,11 +892,32 @@ static int backward_impl(fdtd_grid *g, float *fields, const float *inv_eps, cons
                          const float *dL_dfields, int n_hi, int n_lo, int n_total, float *dL_dinv_eps, float *dL_dfields0,
                          void *cuda_stream, float *dL_dinv_mu)
 {
+    if (g && g->desc.record == 3 && dL_dinv_eps) {
+        int rc = check_common(g, fields, inv_eps, src, n_src, det, n_det, n_total, "fdtd_backward");
+        if (rc) return rc;
+        if (n_td || dL_dinv_mu) return fail(FDTD_EINVAL, "time-domain detectors and dL_dinv_mu are not available on a record = 3 grid");
+        if (n_hi != n_total || n_lo != 0) return fail(FDTD_EINVAL, "range calls are not available on a record = 3 grid");
+        return checkpointed_backward(g, fields, inv_eps, inv_mu, src, n_src, det, n_det, dL_dphasor, dL_dfields, n_total,
+                                     dL_dinv_eps, dL_dfields0, cuda_stream);
+    }
+    return backward_core(g, fields, inv_eps, inv_mu, src, n_src, det, n_det, dL_dphasor, td, n_td, dL_dtd, dL_dfields, n_hi, n_lo,
+                         n_total, dL_dinv_eps, dL_dfields0, cuda_stream, dL_dinv_mu, false);
+}
+
+// reverse steps n_hi-1 .. n_lo of a run of n_total steps (fdtd_backward: n_steps-1 .. 0); the cotangent seed (B0) is
+// placed by the call with n_hi == n_total, dL_dfields0 is written by the call with n_lo == 0
+static int backward_core(fdtd_grid *g, float *fields, const float *inv_eps, const float *inv_mu,
+                         const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
+                         const float *const *dL_dphasor,
+                         const fdtd_time_detector *td, int32_t n_td, const float *const *dL_dtd,
+                         const float *dL_dfields, int n_hi, int n_lo, int n_total, float *dL_dinv_eps, float *dL_dfields0,
+                         void *cuda_stream, float *dL_dinv_mu, bool sweep_only)
+{
     const int n_steps = n_total;
     const bool first = n_hi == n_total, last = n_lo == 0;
     int rc = check_common(g, fields, inv_eps, src, n_src, det, n_det, n_steps, "fdtd_backward");
     if (rc) return rc;
-    if (!dL_dinv_eps && !dL_dfields0) return fail(FDTD_EINVAL, "fdtd_backward: dL_dinv_eps or dL_dfields0 is required");
+    if (!dL_dinv_eps && !dL_dfields0 && !sweep_only) return fail(FDTD_EINVAL, "fdtd_backward: dL_dinv_eps or dL_dfields0 is required");
     const Dims &G = g->G;
     if (dL_dinv_eps && G.d > 0 && (!g->desc.record || g->recorded_steps != n_steps))
         return fail(FDTD_ESTATE, "fdtd_backward: no matching recorded forward (need record=1 and the same n_steps)");

@@ -35,6 +35,10 @@ struct fdtd_grid {
     fdtd::PsiSet lpsiE[2]{}, lpsiH[2]{};   // psi cotangents, ping-ponged by step parity
     float *lam = nullptr;                  // cotangent fields [6][nz][ny][nx]
     float *rec = nullptr;                  // interface recorder
+    float *ckpt = nullptr, *dE = nullptr;  // record = 3: checkpoints [ck_count][ck_stride], dE [ck_every][3][box cells]
+    int ck_every = 0, ck_count = 0;
+    bool replaying = false;                // the checkpointed reverse sweep is re-running forward steps: the state stays in its ping-pong volume
+    size_t ck_stride = 0;
     int recorded_steps = -1;               // n_steps of the last recorded forward, or -1
     int fwd_pos = -1, bwd_pos = -1;        // fdtd_forward_range / fdtd_backward_range: the state index the last call left
     bool fwd_fused = false, bwd_fused = false;   // which kernels the last (range) call ran on: where its state lives

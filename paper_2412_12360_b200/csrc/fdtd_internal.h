@@ -148,6 +148,11 @@ void launch_grad_rho(const Dims &G, const float *g, const float *ie, float delta
 void launch_inv_H(const Dims &G, float *fields, const float *im, cudaStream_t st, const float *lam = nullptr,
                   const float *lam2 = nullptr, const int *step = nullptr, bool scaled = false, float *g_mu = nullptr);
 void launch_inv_E_grad(const Dims &G, float *fields, const float *ie, const float *lam, float *g, cudaStream_t st);
+// checkpointed reverse sweep (record = 3): dE = E' - E per replayed step on the gradient box, g += sum_c lamE'_c dE_c / ie
+void launch_dE_store(const Dims &G, const float *A, const float *B, float *dE, int mode, const int *step, cudaStream_t st);
+void launch_dE_source(const Dims &G, float *dE, const SourceDev &s, const int *step, cudaStream_t st);
+void launch_grad_from_dE(const Dims &G, const float *lamA, const float *lamB, const float *dE, const float *ie, float *g,
+                         const int *step, cudaStream_t st);
 // fused path: cotangent volumes are ping-ponged by step parity
 void launch_inv_E_grad_pp(const Dims &G, float *fields, const float *ie, const float *lamA, const float *lamB,
                           const int *step, float *g, cudaStream_t st);

@@ -600,6 +600,77 @@ void launch_inv_H(const Dims &G, float *fields, const float *im, cudaStream_t st
     else            k_inv_H<false><<<vol_grid(G), vol_block(), 0, st>>>(G, fields, im, lam, lam2, step, scaled ? 1 : 0, g_mu);
 }
 
+// ------------------------------------------------------------------------------------------ checkpointed reverse sweep
+// ("checkpointing": no inverse step.)  On the gradient box [glo, ghi) -- any box of the grid,
+// PML cells included -- the E update's dependence on inv_eps is  dE'_c/d ie = S * bracket_c = (E'_c - E_c - src_c) / ie,
+// so the replayed forward pass stores dE = E' - E per step and the adjoint sweep forms  g += sum_c lamE'_c dE_c / ie.
+// mode 0: dE = B_E - A_E (two volumes: the fused ping-pong, picked by the parity of *step);
+// mode 1: dE = -A_E (before an in-place step);  mode 2: dE += A_E (after it).
+__global__ void k_dE_store(Dims G, const float *__restrict__ A, const float *__restrict__ B, float *__restrict__ dE, int mode,
+                           const int *__restrict__ step)
+{
+    const int bx = G.ghi[0] - G.glo[0], by = G.ghi[1] - G.glo[1], bz = G.ghi[2] - G.glo[2];
+    const long long bc = (long long)bx * by * bz;
+    const float *En = A, *En1 = B;
+    if (mode == 0 && (*step & 1)) { En = B; En1 = A; }         // state n sits in volume n&1
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < bc; t += (long long)gridDim.x * blockDim.x) {
+        const int i = G.glo[0] + (int)(t % bx), j = G.glo[1] + (int)((t / bx) % by), k = G.glo[2] + (int)(t / ((long long)bx * by));
+        const long long p = lin(G, i, j, k);
+        for (int c = 0; c < 3; ++c) {
+            float *o = dE + c * bc + t;
+            if (mode == 0) *o = En1[c * G.nc + p] - En[c * G.nc + p];
+            else if (mode == 1) *o = -En[c * G.nc + p];
+            else *o += En[c * G.nc + p];
+        }
+    }
+}
+// dE_c -= profile * waveform[n] where an E source of component c overlaps the box
+__global__ void k_dE_source(Dims G, float *__restrict__ dE, SourceDev s, const int *__restrict__ step)
+{
+    const int bx = s.hi[0] - s.lo[0], by = s.hi[1] - s.lo[1], bz = s.hi[2] - s.lo[2];
+    const long long n_cells = (long long)bx * by * bz;
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n_cells) return;
+    const int i = s.lo[0] + (int)(t % bx), j = s.lo[1] + (int)((t / bx) % by), k = s.lo[2] + (int)(t / ((long long)bx * by));
+    if (i < G.glo[0] || i >= G.ghi[0] || j < G.glo[1] || j >= G.ghi[1] || k < G.glo[2] || k >= G.ghi[2]) return;
+    const int gx = G.ghi[0] - G.glo[0], gy = G.ghi[1] - G.glo[1], gz = G.ghi[2] - G.glo[2];
+    const long long q = ((long long)(k - G.glo[2]) * gy + (j - G.glo[1])) * gx + (i - G.glo[0]);
+    dE[(long long)s.comp * gx * gy * gz + q] -= (s.profile ? __ldg(s.profile + t) : 1.f) * __ldg(s.waveform + *step);
+}
+// g += sum_c lamE'_c dE_c / ie on the box; lamE' = the E part of the cotangent volume after reverse step n (volume n&1 of
+// lamA / lamB on the fused path, lamA alone otherwise)
+__global__ void k_grad_from_dE(Dims G, const float *__restrict__ lamA, const float *__restrict__ lamB, const float *__restrict__ dE,
+                               const float *__restrict__ ie, float *__restrict__ g, const int *__restrict__ step)
+{
+    const int bx = G.ghi[0] - G.glo[0], by = G.ghi[1] - G.glo[1], bz = G.ghi[2] - G.glo[2];
+    const long long bc = (long long)bx * by * bz;
+    const float *lam = (lamB && (*step & 1)) ? lamB : lamA;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < bc; t += (long long)gridDim.x * blockDim.x) {
+        const int i = G.glo[0] + (int)(t % bx), j = G.glo[1] + (int)((t / bx) % by), k = G.glo[2] + (int)(t / ((long long)bx * by));
+        const long long p = lin(G, i, j, k);
+        float acc = 0.f;
+        for (int c = 0; c < 3; ++c) acc = fmaf(lam[c * G.nc + p], dE[c * bc + t], acc);
+        g[p] += acc / __ldg(ie + p);
+    }
+}
+
+void launch_dE_store(const Dims &G, const float *A, const float *B, float *dE, int mode, const int *step, cudaStream_t st)
+{
+    const long long n = (long long)(G.ghi[0] - G.glo[0]) * (G.ghi[1] - G.glo[1]) * (G.ghi[2] - G.glo[2]);
+    k_dE_store<<<(unsigned)std::min<long long>((n + 255) / 256, 1 << 16), 256, 0, st>>>(G, A, B, dE, mode, step);
+}
+void launch_dE_source(const Dims &G, float *dE, const SourceDev &s, const int *step, cudaStream_t st)
+{
+    const long long n = (long long)(s.hi[0] - s.lo[0]) * (s.hi[1] - s.lo[1]) * (s.hi[2] - s.lo[2]);
+    k_dE_source<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(G, dE, s, step);
+}
+void launch_grad_from_dE(const Dims &G, const float *lamA, const float *lamB, const float *dE, const float *ie, float *g,
+                         const int *step, cudaStream_t st)
+{
+    const long long n = (long long)(G.ghi[0] - G.glo[0]) * (G.ghi[1] - G.glo[1]) * (G.ghi[2] - G.glo[2]);
+    k_grad_from_dE<<<(unsigned)std::min<long long>((n + 255) / 256, 1 << 16), 256, 0, st>>>(G, lamA, lamB, dE, ie, g, step);
+}
+
 void launch_inv_E_grad(const Dims &G, float *fields, const float *ie, const float *lam, float *g, cudaStream_t st)
 {
     if (G.periodic) k_inv_E_grad<true><<<vol_grid(G), vol_block(), 0, st>>>(G, fields, ie, lam, g, nullptr, nullptr);

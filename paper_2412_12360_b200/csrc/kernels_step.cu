@@ -1896,7 +1896,7 @@ int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float
     if (!TD.empty()) key.append((const char *)TD.data(), TD.size() * sizeof(TimeDetDev));
     rc = fdtd_run_steps_fwd(g, key, n_count, 1 + (recording ? 1 : 0) + (int)TD.size(), st, enqueue_fwd, &ctx);
     if (rc) return rc;
-    if (n_end != n_total) return FDTD_OK;
+    if (n_end != n_total || g->replaying) return FDTD_OK;      // (replaying: the checkpointed reverse sweep leaves the state in its volume)
     if (recording) {      // E' of the last step; the p-th step of the call read counter slot p&1, so the count sits in slot n_count&1
         ProfScope p(g, fdtd_grid::PC_RECORD, st);
         launch_record_pipe(g->G, g->R, fields, F->bufB, g->rec, g->d_step + (n_count & 1), n_steps, st);

@@ -245,3 +245,55 @@ def test_gradient_with_respect_to_inv_mu(B, case):
     g.close()
     assert np.max(np.abs(gmu_r)) > 0
     assert max(e) <= TOL_GRAD, e
+
+
+@pytest.mark.parametrize("case", ["tiny-generic", "mini-generic", "mini-fused", "mini-fused-odd"])
+def test_checkpointed_reverse_sweep(B, case):
+    """SURVEY 8(f) N4 / PAPER.md L82: record=3, the reverse sweep from checkpoints (no inverse step).  Its gradient is the
+    plain reverse-mode derivative on EVERY cell, PML included: compared with the oracle's tape mode (which stores every E-update
+    bracket) on the whole grid, and with the time-reversed sweep on the interior."""
+    import torch
+    from oracle.oracle import Oracle
+    if case.startswith("tiny"):
+        w = wl.tiny_pml(n_steps=30)
+        K = 7
+    else:
+        n = 61 if case.endswith("odd") else 60
+        w = wl.c3_mini(n_steps=n, kappa_max=3.0, alpha_max=0.05)
+        rng = np.random.default_rng(5)
+        w.meta["inv_mu"] = (1.0 / (1.0 + 0.5 * rng.random((w.nz, w.ny, w.nx), dtype=np.float32))).astype(np.float32)
+        # an E source inside the gradient box (its contribution to E' - E is not part of the bracket) and an H source
+        w.sources.append(wl.Source(2, (30, 20, 20), (50, 30, 22), (0.4 * wl.gaussian_sine(n, 20, 7, 10)).astype(np.float32)))
+        w.sources.append(wl.Source(4, (20, 12, 22), (60, 40, 23), (0.3 * wl.gaussian_sine(n, 25, 9, 11)).astype(np.float32)))
+        K = 0 if case.endswith("odd") else 16
+    path = B.FDTD_PATH_FUSED if "fused" in case else B.FDTD_PATH_GENERIC
+    im = w.meta["inv_mu"]
+    o = Oracle(**w.grid_kwargs())
+    fr = np.zeros((6, w.nz, w.ny, w.nx))
+    out = o.forward(fr, w.inv_eps, im, w.sources, w.detectors, w.n_steps, record=True, tape=True)
+    dLf_r = np.zeros_like(fr)
+    dLf_r[:3] = 0.5 * fr[:3]
+    dLp_r = [2.0 * P for P in out["phasors"]]
+    g_tape, lam_tape = o.backward_tape(w.inv_eps, im, w.detectors, dLp_r, dLf_r, w.n_steps, out["tape"])
+    kw = w.grid_kwargs()
+    kw.update(max_steps=w.n_steps, record=3, path=path, checkpoint_every=K)
+    g = B.Grid(**kw)
+    f = torch.zeros((6, w.nz, w.ny, w.nx), device="cuda")
+    ie, imt = torch.as_tensor(w.inv_eps).cuda(), torch.as_tensor(im).cuda()
+    ph = g.forward(f, ie, imt, w.sources, w.detectors, w.n_steps)
+    torch.cuda.synchronize()
+    assert relerr(f.cpu().numpy()[:3], fr[:3]) <= TOL_FIELD
+    dLf = torch.zeros_like(f)
+    dLf[:3] = 0.5 * f[:3]
+    grad, lam0 = g.backward(f, ie, imt, w.sources, w.detectors, [2.0 * P for P in ph], dLf, w.n_steps, want_dL_dfields0=True)
+    torch.cuda.synchronize()
+    info = g.info()
+    g.close()
+    assert info.path == path and info.recorder_bytes > 0
+    gg = grad.cpu().numpy()
+    d = w.pml_cells
+    pml = np.ones_like(g_tape, dtype=bool)
+    pml[d:w.nz - d, d:w.ny - d, d:w.nx - d] = False
+    assert np.max(np.abs(g_tape[pml])) > 1e-3 * np.max(np.abs(g_tape))          # the PML cells do carry gradient
+    assert relerr(gg, g_tape) <= TOL_GRAD and relerr(gg[pml], g_tape[pml]) <= TOL_GRAD, (relerr(gg, g_tape), relerr(gg[pml], g_tape[pml]))
+    assert relerr(lam0.cpu().numpy(), lam_tape) <= TOL_GRAD
