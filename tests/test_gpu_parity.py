@@ -508,6 +508,36 @@ def test_c3_full_length_self_consistency(B):
     assert float(grad.abs().max()) == 0.0
 
 
+def test_c3_full_length_time_reversal_equals_checkpointing(B):
+    """configs[2] at its full size and length: the gradient of the time-reversed sweep (record=2, the bench configuration; also
+    record=1) against the checkpointed sweep (record=3: no inverse step, nothing reconstructed), which is the
+    plain reverse-mode derivative.  Two independent routes to dL/d inv_eps over 2000 steps on 864 000 voxels: they must agree
+    to the rounding of the reconstruction (measured 7e-7 of the maximum; the oracle tolerance is 1e-3)."""
+    import torch
+    n = 2000
+    w = wl.c3(n_steps=n)
+    lo, hi = w.design_lo, w.design_hi
+    box = (slice(lo[2], hi[2]), slice(lo[1], hi[1]), slice(lo[0], hi[0]))
+    ie = torch.as_tensor(w.inv_eps).cuda()
+    grads = {}
+    for rec in (3, 2, 1):
+        kw = w.grid_kwargs()
+        kw.update(max_steps=n, record=rec, grad_lo=lo, grad_hi=hi, path=B.FDTD_PATH_FUSED)
+        g = B.Grid(**kw)
+        f = torch.zeros((6, w.nz, w.ny, w.nx), dtype=torch.float32, device="cuda")
+        ph = g.forward(f, ie, None, w.sources, w.detectors, n)
+        grad, _ = g.backward(f, ie, None, w.sources, w.detectors, [2.0 * P for P in ph], None, n)
+        torch.cuda.synchronize()
+        grads[rec] = grad[box].double().cpu().numpy()
+        g.close()
+    scale = np.max(np.abs(grads[3]))
+    assert scale > 0
+    for rec in (2, 1):
+        err = float(np.max(np.abs(grads[rec] - grads[3])) / scale)
+        print(f"C3 full length: time-reversed (record={rec}) vs checkpointed gradient: {err:.2e} of the maximum")
+        assert err <= 1e-5
+
+
 def test_c4_full_size_self_consistency(B):
     """configs[3] at its full 800 x 800 x 600 size (384 M cells; maximum size, 6 nc > 2^31 elements) in the
     bench launch configuration (fused kernels, record=2).  The oracle cannot run this size in seconds, so the
