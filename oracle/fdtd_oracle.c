@@ -104,6 +104,7 @@ typedef struct {
     REAL *psiE[3][2], *psiH[3][2];           /* primal psi, full volumes       */
     REAL *lpsiE[3][2], *lpsiH[3][2];         /* cotangents of psi              */
     REAL *tmp[3][2];                         /* scratch volumes for the adjoint */
+    const REAL *sigma;                       /* N4: normalised electric conductivity per voxel, or NULL (lossless) */
 } orc_state;
 
 #define NX (D->nx)
@@ -281,6 +282,17 @@ void orc_zero_lpsi(orc_state *st)
 }
 
 /* ------------------------------------------------------------------------ */
+/* N4 (SURVEY 8(f) N4 "conductive ... media where time reversal fails"; "reversible ... for lossless  */
+/* materials", L82 checkpointing as the alternative).  Reading R29: an electric conductivity sigma per voxel,        */
+/* normalised like the CPML's (sigma~ = sigma eta0 dx), enters Eq. 2 as  eps dE/dt = curl H - sigma E  and is         */
+/* discretised semi-implicitly (sigma E at the half step = sigma (E' + E)/2), the standard lossy Yee update:          */
+/*   beta = sigma~ S ie / 2,  Ca = (1 - beta)/(1 + beta),  Cb = 1/(1 + beta),   E'_c = Ca E_c + Cb S ie bracket_c     */
+/* (the same ie and sigma~ for the three components stored at the voxel, like R6).  sigma = NULL: Ca = Cb = 1.        */
+/* The inverse step is not defined for it (orc_backward refuses); gradients come from tape mode.                      */
+/* ------------------------------------------------------------------------ */
+void orc_set_sigma(orc_state *st, const REAL *sigma) { st->sigma = sigma; }
+
+/* ------------------------------------------------------------------------ */
 /* O1: E update (Eq. 2 discretised on the Yee grid; CPML psi_E recursion)   */
 /*   d1 = dm_a H_b, d2 = dm_b H_a                                           */
 /*   psiE_c0 = bE_a psiE_c0 + aE_a d1 ; psiE_c1 = bE_b psiE_c1 + aE_b d2    */
@@ -313,8 +325,18 @@ void orc_step_E(orc_state *st, REAL *fields, const REAL *ie, REAL *bracket)
                     st->psiE[c][0][p] = p0;
                     st->psiE[c][1][p] = p1;
                     REAL br = st->ikE[a][pos[a]] * d1 - st->ikE[b][pos[b]] * d2 + p0 - p1;
-                    if (bracket) bracket[(size_t)c * nc + p] = br;
-                    E[c][p] += S * ie[p] * br;
+                    if (!st->sigma) {
+                        if (bracket) bracket[(size_t)c * nc + p] = br;
+                        E[c][p] += S * ie[p] * br;
+                    } else {
+                        /* lossy update; `bracket` keeps its meaning dE'_c/d(ie) = S * bracket:                      */
+                        /*   dCa/d ie = -sigma S / (1+beta)^2,  dCb/d ie = -(sigma S / 2) / (1+beta)^2               */
+                        const REAL hs = (REAL)0.5 * st->sigma[p] * S, beta = hs * ie[p];
+                        const REAL Ca = ((REAL)1 - beta) / ((REAL)1 + beta), Cb = (REAL)1 / ((REAL)1 + beta);
+                        const REAL dCa = (REAL)-2 * hs * Cb * Cb, dCb = -hs * Cb * Cb;
+                        if (bracket) bracket[(size_t)c * nc + p] = (dCa * E[c][p] + (dCb * ie[p] + Cb) * S * br) / S;
+                        E[c][p] = Ca * E[c][p] + Cb * S * ie[p] * br;
+                    }
                 }
             }
 }
@@ -709,7 +731,7 @@ void orc_adj_E(orc_state *st, REAL *lam, const REAL *ie)
     const orc_desc *D = &st->D;
     const REAL S = (REAL)D->S;
     const size_t nc = st->nc;
-    const REAL *lE[3] = { lam, lam + nc, lam + 2 * nc };
+    REAL *lE[3] = { lam, lam + nc, lam + 2 * nc };
     REAL *lH[3] = { lam + 3 * nc, lam + 4 * nc, lam + 5 * nc };
 #ifdef _OPENMP
 #pragma omp parallel for schedule(static)
@@ -719,9 +741,13 @@ void orc_adj_E(orc_state *st, REAL *lam, const REAL *ie)
             for (int i = 0; i < NX; ++i) {
                 const size_t p = IDX(i, j, k);
                 const int pos[3] = { i, j, k };
+                /* N4, lossy update E' = Ca E + Cb S ie bracket: the bracket's cotangent is Cb S ie lamE', and E's is Ca lamE' */
+                const REAL beta = st->sigma ? (REAL)0.5 * st->sigma[p] * S * ie[p] : (REAL)0;
+                const REAL Ca = ((REAL)1 - beta) / ((REAL)1 + beta), Cb = (REAL)1 / ((REAL)1 + beta);
                 for (int c = 0; c < 3; ++c) {
                     const int a = (c + 1) % 3, b = (c + 2) % 3;
-                    REAL w = S * ie[p] * lE[c][p];
+                    REAL w = (st->sigma ? Cb : (REAL)1) * S * ie[p] * lE[c][p];
+                    if (st->sigma) lE[c][p] *= Ca;
                     REAL l0 = st->lpsiE[c][0][p] + w;
                     REAL l1 = st->lpsiE[c][1][p] - w;
                     st->tmp[c][0][p] = st->ikE[a][pos[a]] * w + st->aE[a][pos[a]] * l0;
@@ -904,6 +930,7 @@ int orc_backward_mu(orc_state *st, REAL *fields, const REAL *ie, const REAL *im,
     const size_t nc = st->nc;
     const size_t rs = orc_record_stride(D);
     if (D->d > 0 && !rec) return -4;
+    if (st->sigma) return -4;                 /* the inverse step is for lossless media */
     REAL *lam = zalloc(6 * nc);
     if (!lam) return -2;
     if (dL_dfields) memcpy(lam, dL_dfields, 6 * nc * sizeof(REAL));      /* B0 */

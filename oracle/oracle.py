@@ -206,6 +206,12 @@ class Oracle:
     def zero_lpsi(self):
         self.L.orc_zero_lpsi(self.h)
 
+    def set_sigma(self, sigma):
+        """N4 (reading R29): normalised electric conductivity per voxel for the lossy E update, or None (lossless)."""
+        self._sigma = self.arr(sigma, self.shape)
+        self.L.orc_set_sigma.argtypes = [C.c_void_p, C.c_void_p]
+        self.L.orc_set_sigma(self.h, _ptr(self._sigma))
+
     def _sources(self, sources):
         n = len(sources)
         arr = (_Source * max(n, 1))()

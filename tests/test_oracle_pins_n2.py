@@ -274,3 +274,91 @@ def test_n4_gradient_with_respect_to_inv_mu():
         im_[v] -= h
         fd = (loss(ip) - loss(im_)) / (2 * h)
         assert abs(fd - g_mu[v]) < 2e-6 * scale + 1e-6 * abs(fd), (v, fd, g_mu[v])
+
+
+# ----------------------------------------------------------------------------- N4: lossy media (reading R29)
+def test_n4_lossy_eigenmode_decays_as_the_closed_form_says():
+    """A plane wave in a uniform conductive medium, periodic box: with K^2 = sum_a 4 sin^2(k_a/2) the lossy leapfrog
+    E' = Ca E + Cb S ie curl- H, H' = H - S curl+ E' has the eigenvalue rho of
+        rho^2 - (1 + Ca - Cb S^2 ie K^2) rho + Ca = 0        (|rho|^2 = Ca: the decay per step)
+    for the transverse mode E^n = Re(rho^n e exp(i k.r_E)), H^{n+1/2} = Re(rho^n h exp(i k.r_H)),
+    h = -S rho (K+ x e) / (rho - 1), K+_a = 2 i sin(k_a/2) (staggered positions as in pin P1).  The oracle must follow it
+    to rounding; sigma = 0 must reproduce the lossless run bit for bit."""
+    nx, ny, nz = 12, 10, 8
+    shape = (nz, ny, nx)
+    mvec = (2, 1, 1)
+    k = np.array([2 * math.pi * mvec[0] / nx, 2 * math.pi * mvec[1] / ny, 2 * math.pi * mvec[2] / nz])
+    eps_r, sig = 2.25, 0.07
+    ie = 1.0 / eps_r
+    beta = 0.5 * sig * S * ie
+    Ca, Cb = (1 - beta) / (1 + beta), 1 / (1 + beta)
+    K2 = float(np.sum(4 * np.sin(k / 2) ** 2))
+    bq = 1 + Ca - Cb * S * S * ie * K2
+    rho = (bq + np.sqrt(complex(bq * bq - 4 * Ca))) / 2
+    assert abs(abs(rho) ** 2 - Ca) < 1e-14 and abs(rho) < 1
+    Kp = 2j * np.sin(k / 2)                       # symbol of the forward difference between the staggered positions
+    r = np.random.default_rng(3).standard_normal(3)
+    e = r - Kp * (r @ np.conj(Kp)) / K2           # transverse: Kp . e = 0 with the conjugate pairing of the staggered grid
+    e = e - np.conj(Kp) * (Kp @ e) / K2
+    h = -S * rho * np.cross(Kp, e) / (rho - 1)
+
+    def state(n):
+        f = np.zeros((6,) + shape)
+        for c in range(3):
+            x, y, z = _stag(shape, c, False)
+            f[c] = np.real(rho ** n * e[c] * np.exp(1j * (k[0] * x + k[1] * y + k[2] * z)))
+            x, y, z = _stag(shape, c, True)
+            f[3 + c] = np.real(rho ** n * h[c] * np.exp(1j * (k[0] * x + k[1] * y + k[2] * z)))
+        return f
+
+    o = Oracle(nx, ny, nz, S, periodic=True)
+    o.set_sigma(np.full(shape, sig))
+    f = state(0)
+    n = 57
+    o.forward(f, np.full(shape, ie), n_steps=n)
+    want = state(n)
+    assert np.max(np.abs(want)) > 0.05 * np.max(np.abs(state(0)))            # not yet decayed to nothing
+    assert np.max(np.abs(f - want)) < 1e-12 * np.max(np.abs(state(0)))
+    # sigma = 0: the lossless update, bit for bit
+    o0, o1 = Oracle(nx, ny, nz, S, periodic=True), Oracle(nx, ny, nz, S, periodic=True)
+    o1.set_sigma(np.zeros(shape))
+    f0, f1 = state(0), state(0)
+    o0.forward(f0, np.full(shape, ie), n_steps=9)
+    o1.forward(f1, np.full(shape, ie), n_steps=9)
+    assert np.array_equal(f0, f1)
+
+
+def test_n4_lossy_gradient_against_finite_differences():
+    """Tape-mode gradient with a random conductivity on the tiny CPML grid (every term) against central finite differences
+    in single inv_eps voxels (interior, PML, corner); the reversible sweep refuses a lossy medium."""
+    w = wl.tiny_pml(n_steps=30)
+    d = w.pml_cells
+    shape = (w.nz, w.ny, w.nx)
+    ie0 = w.inv_eps.astype(np.float64)
+    sig = 0.3 * np.random.default_rng(12).random(shape)
+
+    def loss(ie_, want_grad=False):
+        o = Oracle(**w.grid_kwargs())
+        o.set_sigma(sig)
+        f = np.zeros((6,) + shape)
+        out = o.forward(f, ie_, w.meta["inv_mu"], w.sources, w.detectors, w.n_steps, record=want_grad, tape=want_grad)
+        P = out["phasors"][0]
+        L = float(np.sum(P * P)) + 0.5 * float(np.sum(f[:3] ** 2))
+        if not want_grad:
+            return L
+        dLf = np.zeros_like(f)
+        dLf[:3] = f[:3]
+        g, _ = o.backward_tape(ie_, w.meta["inv_mu"], w.detectors, [2.0 * P], dLf, w.n_steps, out["tape"])
+        with pytest.raises(AssertionError):
+            o.backward(f, ie_, w.meta["inv_mu"], w.sources, w.detectors, [2.0 * P], dLf, w.n_steps, out["rec"])
+        return L, g
+
+    L, g = loss(ie0, True)
+    scale = np.max(np.abs(g))
+    h = 1e-6
+    for v in [(w.nz // 2, w.ny // 2, w.nx // 2), (d, d, d), (1, 2, 3), (0, 0, 0), (w.nz - 1, w.ny - 2, w.nx - 1), (d + 1, d + 2, d + 3)]:
+        ip, im_ = ie0.copy(), ie0.copy()
+        ip[v] += h
+        im_[v] -= h
+        fd = (loss(ip) - loss(im_)) / (2 * h)
+        assert abs(fd - g[v]) < 2e-6 * scale + 1e-6 * abs(fd), (v, fd, g[v])
