@@ -221,6 +221,15 @@ FDTD_API int fdtd_backward_mu(fdtd_grid *grid, float *fields, const float *inv_e
  * Same result as the time-reversed sweep on the interior to its reconstruction rounding; equals the plain reverse-mode
  * derivative (the oracle's tape mode) on every cell.  Not available with time-domain detectors, range calls or sub-grids. */
 
+/* N4, lossy media ("reversible ... for lossless materials"; reading R29): a normalised electric
+ * conductivity per voxel, sigma~ = sigma eta0 dx (DEVICE [nz][ny][nx], caller-owned, must stay valid while it is set; NULL
+ * removes it).  The E update becomes the semi-implicit lossy Yee update
+ *   beta = sigma~ S inv_eps / 2,   E'_c = (1 - beta)/(1 + beta) E_c + 1/(1 + beta) S inv_eps bracket_c .
+ * Such a step cannot be inverted stably, so the grid must have record == 0 (forward, adjoint sweep only) or record == 3 (the
+ * checkpointed reverse sweep, which then delivers dL_dinv_eps); ESTATE otherwise.  Runs on the generic kernels
+ * (FDTD_PATH_FUSED: EINVAL at the call). */
+FDTD_API int fdtd_set_conductivity(fdtd_grid *grid, const float *sigma);
+
 /* B6, chain rule to design parameters (once per gradient, not per step): for a design box whose
  * permittivity is eps = eps_bg + delta_eps*rho (reading R20),
  *   dL_drho[cell] = dL_dinv_eps[cell] * d(1/eps)/drho = -dL_dinv_eps[cell] * delta_eps * inv_eps[cell]^2.

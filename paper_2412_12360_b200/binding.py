@@ -73,7 +73,7 @@ class fdtd_profile(C.Structure):
 EXPORTS = ("fdtd_grad_rho", "fdtd_set_profiling", "fdtd_get_profile", "fdtd_create_grid", "fdtd_forward", "fdtd_backward", "fdtd_destroy", "fdtd_last_error",
            "fdtd_get_info", "fdtd_version", "fdtd_forward_host", "fdtd_backward_host", "fdtd_debug_partition",
            "fdtd_forward_td", "fdtd_backward_td", "fdtd_flux", "fdtd_flux_vjp", "fdtd_tfsf_plane",
-           "fdtd_forward_range", "fdtd_backward_range", "fdtd_halo_export", "fdtd_halo_import", "fdtd_backward_mu")
+           "fdtd_forward_range", "fdtd_backward_range", "fdtd_halo_export", "fdtd_halo_import", "fdtd_backward_mu", "fdtd_set_conductivity")
 
 
 def _load():
@@ -101,6 +101,8 @@ def _load():
     L.fdtd_backward_mu.restype = C.c_int
     L.fdtd_backward_mu.argtypes = [vp, vp, vp, vp, C.POINTER(fdtd_source), i32, C.POINTER(fdtd_detector), i32,
                                    C.POINTER(vp), vp, i32, vp, vp, vp, vp]
+    L.fdtd_set_conductivity.restype = C.c_int
+    L.fdtd_set_conductivity.argtypes = [vp, vp]
     L.fdtd_halo_export.restype = C.c_int
     L.fdtd_halo_export.argtypes = [vp, vp, i32, i32, i32, vp, vp]
     L.fdtd_halo_import.restype = C.c_int
@@ -389,6 +391,11 @@ class Grid:
 
     def stream(self):
         return C.c_void_p(self.torch.cuda.current_stream().cuda_stream)
+
+    def set_conductivity(self, sigma):
+        """N4: normalised electric conductivity per voxel (cuda tensor / array) or None; kept alive by this object."""
+        self._sigma = self._dev(sigma)
+        _check(_L.fdtd_set_conductivity(self.h, _ptr(self._sigma)))
 
     # -- N2: flux from phasors, TFSF plane source ------------------------------------------------
     def flux(self, det, phasor, axis, interpolate=False):

@@ -672,7 +672,7 @@ static int forward_impl(fdtd_grid *g, float *fields, const float *inv_eps, const
     if (n_td) return fail(FDTD_EINVAL, "time-domain detectors are not available on a record = 3 grid");
     if (n_begin != 0 || n_end != n_total) return fail(FDTD_EINVAL, "range calls are not available on a record = 3 grid");
     if (!fields) return fail(FDTD_EINVAL, "fdtd_forward: fields and inv_eps are required");
-    const bool fused = g->path == FDTD_PATH_FUSED && n_src <= FDTD_FUSED_MAX_SRC && n_det <= FDTD_FUSED_MAX_DET;
+    const bool fused = g->path == FDTD_PATH_FUSED && n_src <= FDTD_FUSED_MAX_SRC && n_det <= FDTD_FUSED_MAX_DET && !g->sigma;
     const int K = g->ck_every;
     int rc = FDTD_OK;
     if (n_total == 0) return forward_core(g, fields, inv_eps, inv_mu, src, n_src, det, n_det, nullptr, 0, 0, 0, 0, cuda_stream);
@@ -730,9 +730,11 @@ static int forward_core(fdtd_grid *g, float *fields, const float *inv_eps, const
 
     // more descriptors than the fused kernels' parameter block holds: this call runs on the generic kernels (same
     // psi slabs, same recorder layout, so a fused or generic fdtd_backward can follow)
-    const bool fused_call = g->path == FDTD_PATH_FUSED && n_src <= FDTD_FUSED_MAX_SRC && n_det <= FDTD_FUSED_MAX_DET;
+    // (a lossy medium, N4, also runs on the generic kernels)
+    const bool fused_call = g->path == FDTD_PATH_FUSED && n_src <= FDTD_FUSED_MAX_SRC && n_det <= FDTD_FUSED_MAX_DET && !g->sigma;
     if (g->path == FDTD_PATH_FUSED && !fused_call && g->desc.path == FDTD_PATH_FUSED)
-        return fail(FDTD_EINVAL, "FDTD_PATH_FUSED takes at most 4 sources and 4 detectors per call (FDTD_PATH_AUTO falls back to the generic kernels)");
+        return fail(FDTD_EINVAL, "FDTD_PATH_FUSED takes at most 4 sources and 4 detectors per call and no conductivity (FDTD_PATH_AUTO falls back to the generic kernels)");
+    if (g->sigma && recording) return fail(FDTD_ESTATE, "a lossy medium cannot be time-reversed (PAPER.md L84): use record = 0 or the checkpointed sweep, record = 3");
     if (fused_call) {
         rc = fused_forward(g, fields, inv_eps, inv_mu, S, D, TD, total_freq, n_begin, n_end, n_total, recording, st);
         if (rc) return rc;
@@ -741,8 +743,9 @@ static int forward_core(fdtd_grid *g, float *fields, const float *inv_eps, const
         const int launches = 3 + n_src + n_det + n_td + (recording ? 1 : 0);
         std::string key = make_key("gf", fields, inv_eps, inv_mu, g->rec, g->d_cs, S, D, recording);
         if (!TD.empty()) key.append((const char *)TD.data(), TD.size() * sizeof(TimeDetDev));
+        key.append((const char *)&g->sigma, sizeof(g->sigma));
         rc = run_steps(g, g->fwd_graph, key, n_end - n_begin, launches, st, [&](cudaStream_t cs) {
-            { ProfScope p(g, fdtd_grid::PC_UPDATE_E, cs); launch_update_E(G, g->T, fields, inv_eps, g->psiE[0], cs); }
+            { ProfScope p(g, fdtd_grid::PC_UPDATE_E, cs); launch_update_E(G, g->T, fields, inv_eps, g->psiE[0], cs, g->sigma); }
             { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
               for (const SourceDev &s : S) if (s.comp < 3) launch_add_source(G, fields, s, g->step_in(), 1.f, cs); }
             if (recording) { ProfScope p(g, fdtd_grid::PC_RECORD, cs); launch_record(G, g->R, fields, fields, g->rec, g->step_in(), cs); }
@@ -845,9 +848,8 @@ static int checkpointed_backward(fdtd_grid *g, float *fields, const float *inv_e
     if (g->recorded_steps != n_total) return fail(FDTD_ESTATE, "fdtd_backward: no matching checkpointed forward (need record=3 and the same n_steps)");
     std::vector<SourceDev> S;
     translate(src, n_src, S);
-    const bool fused_f = g->path == FDTD_PATH_FUSED && n_src <= FDTD_FUSED_MAX_SRC;      // the replay runs without detectors
+    const bool fused_f = g->path == FDTD_PATH_FUSED && n_src <= FDTD_FUSED_MAX_SRC && !g->sigma;      // the replay runs without detectors
     const size_t vol = (size_t)G.nc * sizeof(float);
-    const size_t box = (size_t)(G.ghi[0] - G.glo[0]) * (G.ghi[1] - G.glo[1]) * (G.ghi[2] - G.glo[2]);
     CK(cudaMemsetAsync(dL_dinv_eps, 0, vol, st));
     const int K = g->ck_every;
     int rc = FDTD_OK;
@@ -857,25 +859,32 @@ static int checkpointed_backward(fdtd_grid *g, float *fields, const float *inv_e
         if (a > 0) { if ((rc = copy_checkpoint(g, fields, fused_f, a, a / K, true, st))) return rc; }
         else CK(cudaMemcpyAsync(fields, g->ckpt, 6 * vol, cudaMemcpyDeviceToDevice, st));
         for (int n = a; n < b; ++n) {
-            float *dE = g->dE + (size_t)(n - a) * 3 * box;
-            if (!fused_f) launch_dE_store(G, fields, nullptr, dE, 1, g->d_step, st);          // in-place step: -E before
+            if (!fused_f) {                                   // in-place step: E before it (the counter slot the step will read)
+                launch_set_step(g->d_step, n, st);
+                launch_dE_store(G, fields, nullptr, g->dE, K, 1, inv_eps, g->sigma, g->d_step, st);
+            }
             g->replaying = true;
             rc = forward_core(g, fields, inv_eps, inv_mu, src, n_src, nullptr, 0, nullptr, 0, n, n + 1, n_total, st);
             g->replaying = false;
             if (rc) return rc;
             // the step's first launch read n from counter slot 0, which still holds it
-            if (fused_f) launch_dE_store(G, fields, fused_volume(g, fields, 0, 1), dE, 0, g->d_step, st);
-            else         launch_dE_store(G, fields, nullptr, dE, 2, g->d_step, st);
-            for (const SourceDev &q : S) if (q.comp < 3) launch_dE_source(G, dE, q, g->d_step, st);
-            g->kernel_launches += 2 + (fused_f ? 0 : 1);
+            if (fused_f) launch_dE_store(G, fields, fused_volume(g, fields, 0, 1), g->dE, K, 0, inv_eps, nullptr, g->d_step, st);
+            else         launch_dE_store(G, fields, nullptr, g->dE, K, 2, inv_eps, g->sigma, g->d_step, st);
+            for (const SourceDev &q : S) if (q.comp < 3) launch_dE_source(G, g->dE, K, q, inv_eps, g->sigma, g->d_step, st);
+            g->kernel_launches += 2 + (fused_f ? 0 : 2);
         }
-        // ---- the segment's adjoint steps, gradient from the stored dE
+        // ---- the segment's adjoint steps, gradient from the stored D (generic path: between its two adjoint kernels)
         for (int n = b - 1; n >= a; --n) {
-            if ((rc = backward_core(g, fields, inv_eps, inv_mu, src, n_src, det, n_det, dL_dphasor, nullptr, 0, nullptr, dL_dfields,
-                                    n + 1, n, n_total, nullptr, dL_dfields0, st, nullptr, true))) return rc;
-            launch_grad_from_dE(G, g->lam, g->bwd_fused ? fused_volume(g, fields, 1, 1) : nullptr, g->dE + (size_t)(n - a) * 3 * box,
-                                inv_eps, dL_dinv_eps, g->d_step, st);
-            g->kernel_launches += 1;
+            const bool fused_b = g->path == FDTD_PATH_FUSED && g->fused_backward_ready && !g->sigma;
+            g->ck_grad = fused_b ? nullptr : dL_dinv_eps;
+            rc = backward_core(g, fields, inv_eps, inv_mu, src, n_src, det, n_det, dL_dphasor, nullptr, 0, nullptr, dL_dfields,
+                               n + 1, n, n_total, nullptr, dL_dfields0, st, nullptr, true);
+            g->ck_grad = nullptr;
+            if (rc) return rc;
+            if (fused_b) {
+                launch_grad_from_dE(G, g->lam, fused_volume(g, fields, 1, 1), g->dE, K, dL_dinv_eps, g->d_step, st);
+                g->kernel_launches += 1;
+            }
         }
     }
     // (`fields` was the replay's scratch: it ends at the state the first segment's replay left)
@@ -958,7 +967,8 @@ static int backward_core(fdtd_grid *g, float *fields, const float *inv_eps, cons
     }
     launch_set_step(g->d_step, std::max(n_hi - 1, 0), st);      // the first reverse step of the call reads slot 0
     const bool want_grad = dL_dinv_eps != nullptr;              // false: adjoint sweep only (B1, B2, B5)
-    const bool fused_call = g->path == FDTD_PATH_FUSED && g->fused_backward_ready;
+    const bool fused_call = g->path == FDTD_PATH_FUSED && g->fused_backward_ready && !g->sigma;
+    if (g->sigma && want_grad) return fail(FDTD_ESTATE, "a lossy medium cannot be time-reversed (PAPER.md L84): its gradient comes from the checkpointed sweep (record = 3)");
 
     if (fused_call) {
         // seeded_H: the H part of the seed can be non-zero (it is scaled by inv_mu for the sweep)
@@ -969,10 +979,12 @@ static int backward_core(fdtd_grid *g, float *fields, const float *inv_eps, cons
     } else {
         int n_adj = 0;
         for (const DetectorDev &dt : D) if (dt.phasor) ++n_adj;
-        const int launches = (want_grad ? 5 + n_adj + n_src + (G.d > 0 ? 1 : 0) : 3 + n_adj) + (int)TD.size();
+        const int launches = (want_grad ? 5 + n_adj + n_src + (G.d > 0 ? 1 : 0) : 3 + n_adj) + (int)TD.size() + (g->ck_grad ? 1 : 0) + (g->sigma ? 1 : 0);
         std::string key = make_key("gb", fields, inv_eps, inv_mu, g->rec, dL_dinv_eps, S, D, 0);
         key.append((const char *)&g->d_cs, sizeof(g->d_cs));
         key.append((const char *)&dL_dinv_mu, sizeof(dL_dinv_mu));
+        key.append((const char *)&g->sigma, sizeof(g->sigma));
+        key.append((const char *)&g->ck_grad, sizeof(g->ck_grad));
         if (!TD.empty()) key.append((const char *)TD.data(), TD.size() * sizeof(TimeDetDev));
         rc = run_steps(g, g->bwd_graph, key, n_hi - n_lo, launches, st, [&](cudaStream_t cs) {
             { ProfScope p(g, fdtd_grid::PC_SRC_DET, cs);
@@ -990,7 +1002,10 @@ static int backward_core(fdtd_grid *g, float *fields, const float *inv_eps, cons
               for (const SourceDev &s : S) if (s.comp < 3) launch_add_source(G, fields, s, g->step_in(), -1.f, cs); }
             { ProfScope p(g, fdtd_grid::PC_INV_E_GRAD, cs); launch_inv_E_grad(G, fields, inv_eps, g->lam, dL_dinv_eps, cs); }
             }
-            { ProfScope p(g, fdtd_grid::PC_ADJ_E, cs); launch_adj_E(G, g->T, g->lam, inv_eps, g->lpsiE[0], g->lpsiE[1], g->step_in(), cs); }
+            // checkpointed sweep (record = 3): the gradient from the replay's D = dE'/d inv_eps, with lamE' as it stands here
+            if (g->ck_grad) { ProfScope p(g, fdtd_grid::PC_INV_E_GRAD, cs);
+              launch_grad_from_dE(G, g->lam, nullptr, g->dE, g->ck_every, g->ck_grad, g->step_in(), cs); }
+            { ProfScope p(g, fdtd_grid::PC_ADJ_E, cs); launch_adj_E(G, g->T, g->lam, inv_eps, g->lpsiE[0], g->lpsiE[1], g->step_in(), cs, g->sigma); }
             { ProfScope p(g, fdtd_grid::PC_OTHER, cs); launch_next_step(g->step_in(), g->step_out(), -1, cs); }
         });
         if (rc) return rc;
@@ -1000,6 +1015,15 @@ static int backward_core(fdtd_grid *g, float *fields, const float *inv_eps, cons
     if (e != cudaSuccess) return cuda_fail(e, "fdtd_backward launch");
     g->bwd_pos = n_lo;
     g->bwd_fused = fused_call;
+    return FDTD_OK;
+}
+
+extern "C" int fdtd_set_conductivity(fdtd_grid *g, const float *sigma)
+{
+    if (!g) return fail(FDTD_EINVAL, "fdtd_set_conductivity: NULL grid");
+    if (sigma && (g->desc.record == 1 || g->desc.record == 2))
+        return fail(FDTD_ESTATE, "a lossy medium cannot be time-reversed (PAPER.md L84): create the grid with record = 0 or record = 3");
+    g->sigma = sigma;
     return FDTD_OK;
 }
 

@@ -37,6 +37,8 @@ struct fdtd_grid {
     float *rec = nullptr;                  // interface recorder
     float *ckpt = nullptr, *dE = nullptr;  // record = 3: checkpoints [ck_count][ck_stride], dE [ck_every][3][box cells]
     int ck_every = 0, ck_count = 0;
+    float *ck_grad = nullptr;              // set while the checkpointed sweep runs an adjoint step on the generic kernels: g += lamE' . D there
+    const float *sigma = nullptr;          // N4: conductivity volume of the caller (fdtd_set_conductivity), or NULL
     bool replaying = false;                // the checkpointed reverse sweep is re-running forward steps: the state stays in its ping-pong volume
     size_t ck_stride = 0;
     int recorded_steps = -1;               // n_steps of the last recorded forward, or -1

@@ -112,7 +112,9 @@ struct DetectorDev {
 // All kernels read the current step index n from *step (device memory) so that the per-step
 // launch sequence is identical for every n and can be replayed from a CUDA graph.
 // ----------------------------------------------------------------------------------------------
-void launch_update_E(const Dims &G, const Tables &T, float *fields, const float *ie, PsiSet psiE, cudaStream_t st);
+// sigma: N4 (reading R29), normalised electric conductivity per voxel or NULL
+void launch_update_E(const Dims &G, const Tables &T, float *fields, const float *ie, PsiSet psiE, cudaStream_t st,
+                     const float *sigma = nullptr);
 void launch_update_H(const Dims &G, const Tables &T, float *fields, const float *im, PsiSet psiH, cudaStream_t st);
 void launch_add_source(const Dims &G, float *fields, const SourceDev &s, const int *step, float sign, cudaStream_t st);
 void launch_detector(const Dims &G, const float *fields, const DetectorDev &dt, const float *cs_table,
@@ -140,7 +142,7 @@ void launch_set_step(int *p, int v, cudaStream_t st);
 void launch_adj_H(const Dims &G, const Tables &T, float *lam, const float *im, PsiSet set0, PsiSet set1,
                   const int *step, cudaStream_t st);
 void launch_adj_E(const Dims &G, const Tables &T, float *lam, const float *ie, PsiSet set0, PsiSet set1,
-                  const int *step, cudaStream_t st);
+                  const int *step, cudaStream_t st, const float *sigma = nullptr);
 void launch_grad_rho(const Dims &G, const float *g, const float *ie, float delta_eps, const int lo[3], const int hi[3],
                      float *out, cudaStream_t st);
 // N4: with g_mu, dL/d inv_mu is accumulated from the cotangent of the post-step H (the H part of lam, or of the
@@ -148,10 +150,11 @@ void launch_grad_rho(const Dims &G, const float *g, const float *ie, float delta
 void launch_inv_H(const Dims &G, float *fields, const float *im, cudaStream_t st, const float *lam = nullptr,
                   const float *lam2 = nullptr, const int *step = nullptr, bool scaled = false, float *g_mu = nullptr);
 void launch_inv_E_grad(const Dims &G, float *fields, const float *ie, const float *lam, float *g, cudaStream_t st);
-// checkpointed reverse sweep (record = 3): dE = E' - E per replayed step on the gradient box, g += sum_c lamE'_c dE_c / ie
-void launch_dE_store(const Dims &G, const float *A, const float *B, float *dE, int mode, const int *step, cudaStream_t st);
-void launch_dE_source(const Dims &G, float *dE, const SourceDev &s, const int *step, cudaStream_t st);
-void launch_grad_from_dE(const Dims &G, const float *lamA, const float *lamB, const float *dE, const float *ie, float *g,
+// checkpointed reverse sweep (record = 3): D = dE'/d inv_eps per replayed step on the gradient box (slot n % K), g += sum_c lamE'_c D_c
+void launch_dE_store(const Dims &G, const float *A, const float *B, float *dE, int K, int mode, const float *ie, const float *sigma,
+                     const int *step, cudaStream_t st);
+void launch_dE_source(const Dims &G, float *dE, int K, const SourceDev &s, const float *ie, const float *sigma, const int *step, cudaStream_t st);
+void launch_grad_from_dE(const Dims &G, const float *lamA, const float *lamB, const float *dE, int K, float *g,
                          const int *step, cudaStream_t st);
 // fused path: cotangent volumes are ping-ponged by step parity
 void launch_inv_E_grad_pp(const Dims &G, float *fields, const float *ie, const float *lamA, const float *lamB,

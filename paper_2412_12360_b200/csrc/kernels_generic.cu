@@ -43,12 +43,16 @@ __device__ __forceinline__ float fetch(const Dims &G, const float *__restrict__ 
     (void)pos;
 
 // ------------------------------------------------------------------------------------------ F1+F2
+// N4 (reading R29): with a conductivity volume the update is E' = Ca E + Cb S ie bracket, beta = sigma S ie / 2,
+// Ca = (1 - beta)/(1 + beta), Cb = 1/(1 + beta)
 template <bool PER>
 __global__ void __launch_bounds__(BX *BY) k_update_E(Dims G, Tables T, float *__restrict__ f,
-                                                     const float *__restrict__ ie, PsiSet psi)
+                                                     const float *__restrict__ ie, PsiSet psi, const float *__restrict__ sigma)
 {
     CELL_IJK();
-    const float sie = G.S * __ldg(ie + p);
+    const float beta = sigma ? 0.5f * __ldg(sigma + p) * G.S * __ldg(ie + p) : 0.f;
+    const float Ca = (1.f - beta) / (1.f + beta), Cb = 1.f / (1.f + beta);
+    const float sie = (sigma ? Cb : 1.f) * G.S * __ldg(ie + p);
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         const int a = (c + 1) % 3, b = (c + 2) % 3;
@@ -70,7 +74,8 @@ __global__ void __launch_bounds__(BX *BY) k_update_E(Dims G, Tables T, float *__
                 t -= ps;
             }
         }
-        f[c * G.nc + p] += sie * t;
+        if (sigma) f[c * G.nc + p] = fmaf(Ca, f[c * G.nc + p], sie * t);
+        else f[c * G.nc + p] += sie * t;
     }
 }
 
@@ -156,6 +161,16 @@ __global__ void k_detector(Dims G, float *__restrict__ f, DetectorDev dt, const 
             f[c * G.nc + p] += acc;
         }
         ++ci;
+    }
+}
+
+// N4, lossy E update: lamE_c *= Ca after the adjoint of the E update
+__global__ void k_lossy_scale_E(Dims G, float *__restrict__ lam, const float *__restrict__ ie, const float *__restrict__ sigma)
+{
+    for (long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x; p < G.nc; p += (long long)gridDim.x * blockDim.x) {
+        const float beta = 0.5f * __ldg(sigma + p) * G.S * __ldg(ie + p);
+        const float Ca = (1.f - beta) / (1.f + beta);
+        lam[p] *= Ca; lam[G.nc + p] *= Ca; lam[2 * G.nc + p] *= Ca;
     }
 }
 
@@ -313,10 +328,13 @@ struct AdjCtx {
     const float *lam_src;    // 3 volumes (lamH for FAMILY 1, lamE for FAMILY 0)
     const float *med;        // inv_mu (may be NULL) or inv_eps
     const PsiSet &lin_;      // old psi cotangents
+    const float *sigma;      // FAMILY 0 only, lossy E update (N4): the bracket's cotangent is Cb S ie lamE'
     __device__ __forceinline__ float w(int c, long long q) const
     {
         const float m = med ? __ldg(med + q) : 1.f;
-        return (FAMILY ? -G.S : G.S) * m * __ldg(lam_src + c * G.nc + q);
+        float r = (FAMILY ? -G.S : G.S) * m * __ldg(lam_src + c * G.nc + q);
+        if (!FAMILY && sigma) r /= 1.f + 0.5f * __ldg(sigma + q) * G.S * m;
+        return r;
     }
     // g1 of component c at cell (i,j,k) (in range)
     __device__ __forceinline__ float g(int c, int s, int i, int j, int k, float *new_psi) const
@@ -342,7 +360,7 @@ struct AdjCtx {
 template <int FAMILY, bool PER>
 __global__ void __launch_bounds__(BX *BY) k_adjoint(Dims G, Tables T, float *__restrict__ lam,
                                                     const float *__restrict__ med, PsiSet set0, PsiSet set1,
-                                                    const int *__restrict__ step)
+                                                    const int *__restrict__ step, const float *__restrict__ sigma)
 {
     CELL_IJK();
     const int par = (*step) & 1;
@@ -350,7 +368,7 @@ __global__ void __launch_bounds__(BX *BY) k_adjoint(Dims G, Tables T, float *__r
     const PsiSet &pout = par ? set0 : set1;
     const float *src = lam + (FAMILY ? 3 : 0) * G.nc;
     float *dst = lam + (FAMILY ? 0 : 3) * G.nc;
-    AdjCtx<FAMILY> C{ G, T, src, med, pin };
+    AdjCtx<FAMILY> C{ G, T, src, med, pin, sigma };
     const int sgn = FAMILY ? -1 : +1;     // neighbour offset: p - e (H-update adjoint), p + e (E-update adjoint)
     // own-cell g values and psi-cotangent updates
     float g_own[3][2];
@@ -480,10 +498,10 @@ inline dim3 vol_block() { return dim3(BX, BY, 1); }
 
 }  // namespace
 
-void launch_update_E(const Dims &G, const Tables &T, float *fields, const float *ie, PsiSet psiE, cudaStream_t st)
+void launch_update_E(const Dims &G, const Tables &T, float *fields, const float *ie, PsiSet psiE, cudaStream_t st, const float *sigma)
 {
-    if (G.periodic) k_update_E<true><<<vol_grid(G), vol_block(), 0, st>>>(G, T, fields, ie, psiE);
-    else            k_update_E<false><<<vol_grid(G), vol_block(), 0, st>>>(G, T, fields, ie, psiE);
+    if (G.periodic) k_update_E<true><<<vol_grid(G), vol_block(), 0, st>>>(G, T, fields, ie, psiE, sigma);
+    else            k_update_E<false><<<vol_grid(G), vol_block(), 0, st>>>(G, T, fields, ie, psiE, sigma);
 }
 
 void launch_update_H(const Dims &G, const Tables &T, float *fields, const float *im, PsiSet psiH, cudaStream_t st)
@@ -574,15 +592,17 @@ void launch_set_step(int *p, int v, cudaStream_t st) { k_set_step<<<1, 1, 0, st>
 void launch_adj_H(const Dims &G, const Tables &T, float *lam, const float *im, PsiSet s0, PsiSet s1,
                   const int *step, cudaStream_t st)
 {
-    if (G.periodic) k_adjoint<1, true><<<vol_grid(G), vol_block(), 0, st>>>(G, T, lam, im, s0, s1, step);
-    else            k_adjoint<1, false><<<vol_grid(G), vol_block(), 0, st>>>(G, T, lam, im, s0, s1, step);
+    if (G.periodic) k_adjoint<1, true><<<vol_grid(G), vol_block(), 0, st>>>(G, T, lam, im, s0, s1, step, nullptr);
+    else            k_adjoint<1, false><<<vol_grid(G), vol_block(), 0, st>>>(G, T, lam, im, s0, s1, step, nullptr);
 }
 
 void launch_adj_E(const Dims &G, const Tables &T, float *lam, const float *ie, PsiSet s0, PsiSet s1,
-                  const int *step, cudaStream_t st)
+                  const int *step, cudaStream_t st, const float *sigma)
 {
-    if (G.periodic) k_adjoint<0, true><<<vol_grid(G), vol_block(), 0, st>>>(G, T, lam, ie, s0, s1, step);
-    else            k_adjoint<0, false><<<vol_grid(G), vol_block(), 0, st>>>(G, T, lam, ie, s0, s1, step);
+    if (G.periodic) k_adjoint<0, true><<<vol_grid(G), vol_block(), 0, st>>>(G, T, lam, ie, s0, s1, step, sigma);
+    else            k_adjoint<0, false><<<vol_grid(G), vol_block(), 0, st>>>(G, T, lam, ie, s0, s1, step, sigma);
+    // the cotangent of the pre-update E is Ca lamE' (the gather-form kernel reads its neighbours' lamE': scaled afterwards)
+    if (sigma) k_lossy_scale_E<<<(unsigned)std::min<long long>((G.nc + 255) / 256, 1 << 20), 256, 0, st>>>(G, lam, ie, sigma);
 }
 
 void launch_grad_rho(const Dims &G, const float *g, const float *ie, float delta_eps, const int lo[3], const int hi[3],
@@ -602,30 +622,38 @@ void launch_inv_H(const Dims &G, float *fields, const float *im, cudaStream_t st
 
 // ------------------------------------------------------------------------------------------ checkpointed reverse sweep
 // ("checkpointing": no inverse step.)  On the gradient box [glo, ghi) -- any box of the grid,
-// PML cells included -- the E update's dependence on inv_eps is  dE'_c/d ie = S * bracket_c = (E'_c - E_c - src_c) / ie,
-// so the replayed forward pass stores dE = E' - E per step and the adjoint sweep forms  g += sum_c lamE'_c dE_c / ie.
-// mode 0: dE = B_E - A_E (two volumes: the fused ping-pong, picked by the parity of *step);
-// mode 1: dE = -A_E (before an in-place step);  mode 2: dE += A_E (after it).
-__global__ void k_dE_store(Dims G, const float *__restrict__ A, const float *__restrict__ B, float *__restrict__ dE, int mode,
-                           const int *__restrict__ step)
+// PML cells included -- the replayed forward pass stores, per step, D_c = dE'_c / d inv_eps, and the adjoint sweep forms
+// g += sum_c lamE'_c D_c.  Lossless: E' = E + S ie bracket + src, so D = (E' - E - src) / ie.  Lossy (reading R29):
+// E' = Ca E + Cb S ie bracket + src, D = dCa E + F (E' - Ca E - src), F = (dCb ie + Cb) / (Cb ie),
+// dCa = -sigma S Cb^2, dCb = -(sigma S / 2) Cb^2.  The slot of step n in the buffer is n % K (K = steps per segment).
+// mode 0: state n in volume n&1 of (A, B), state n+1 in the other (the fused ping-pong; lossless only);
+// mode 1: before an in-place step, the slot takes E;  mode 2: after it, the slot becomes D.
+__global__ void k_dE_store(Dims G, const float *__restrict__ A, const float *__restrict__ B, float *__restrict__ dE, int K, int mode,
+                           const float *__restrict__ ie, const float *__restrict__ sigma, const int *__restrict__ step)
 {
     const int bx = G.ghi[0] - G.glo[0], by = G.ghi[1] - G.glo[1], bz = G.ghi[2] - G.glo[2];
     const long long bc = (long long)bx * by * bz;
+    const int n = *step;
+    dE += (long long)(n % K) * 3 * bc;
     const float *En = A, *En1 = B;
-    if (mode == 0 && (*step & 1)) { En = B; En1 = A; }         // state n sits in volume n&1
+    if (mode == 0 && (n & 1)) { En = B; En1 = A; }
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < bc; t += (long long)gridDim.x * blockDim.x) {
         const int i = G.glo[0] + (int)(t % bx), j = G.glo[1] + (int)((t / bx) % by), k = G.glo[2] + (int)(t / ((long long)bx * by));
         const long long p = lin(G, i, j, k);
+        const float e = __ldg(ie + p);
+        const float hs = sigma ? 0.5f * __ldg(sigma + p) * G.S : 0.f, Cb = 1.f / (1.f + hs * e), Ca = (1.f - hs * e) * Cb;
+        const float dCa = -2.f * hs * Cb * Cb, F = (-hs * Cb * Cb * e + Cb) / (Cb * e);
         for (int c = 0; c < 3; ++c) {
             float *o = dE + c * bc + t;
-            if (mode == 0) *o = En1[c * G.nc + p] - En[c * G.nc + p];
-            else if (mode == 1) *o = -En[c * G.nc + p];
-            else *o += En[c * G.nc + p];
+            if (mode == 0) *o = (En1[c * G.nc + p] - En[c * G.nc + p]) / e;
+            else if (mode == 1) *o = En[c * G.nc + p];
+            else { const float E0 = *o; *o = fmaf(dCa, E0, F * (En[c * G.nc + p] - Ca * E0)); }
         }
     }
 }
-// dE_c -= profile * waveform[n] where an E source of component c overlaps the box
-__global__ void k_dE_source(Dims G, float *__restrict__ dE, SourceDev s, const int *__restrict__ step)
+// D_c -= F profile * waveform[n] where an E source of component c overlaps the box
+__global__ void k_dE_source(Dims G, float *__restrict__ dE, int K, SourceDev s, const float *__restrict__ ie,
+                            const float *__restrict__ sigma, const int *__restrict__ step)
 {
     const int bx = s.hi[0] - s.lo[0], by = s.hi[1] - s.lo[1], bz = s.hi[2] - s.lo[2];
     const long long n_cells = (long long)bx * by * bz;
@@ -634,41 +662,50 @@ __global__ void k_dE_source(Dims G, float *__restrict__ dE, SourceDev s, const i
     const int i = s.lo[0] + (int)(t % bx), j = s.lo[1] + (int)((t / bx) % by), k = s.lo[2] + (int)(t / ((long long)bx * by));
     if (i < G.glo[0] || i >= G.ghi[0] || j < G.glo[1] || j >= G.ghi[1] || k < G.glo[2] || k >= G.ghi[2]) return;
     const int gx = G.ghi[0] - G.glo[0], gy = G.ghi[1] - G.glo[1], gz = G.ghi[2] - G.glo[2];
+    const long long bc = (long long)gx * gy * gz;
     const long long q = ((long long)(k - G.glo[2]) * gy + (j - G.glo[1])) * gx + (i - G.glo[0]);
-    dE[(long long)s.comp * gx * gy * gz + q] -= (s.profile ? __ldg(s.profile + t) : 1.f) * __ldg(s.waveform + *step);
+    const int n = *step;
+    const long long p = lin(G, i, j, k);
+    const float e = __ldg(ie + p);
+    const float hs = sigma ? 0.5f * __ldg(sigma + p) * G.S : 0.f, Cb = 1.f / (1.f + hs * e);
+    const float F = (-hs * Cb * Cb * e + Cb) / (Cb * e);
+    dE[(long long)(n % K) * 3 * bc + (long long)s.comp * bc + q] -= F * (s.profile ? __ldg(s.profile + t) : 1.f) * __ldg(s.waveform + n);
 }
-// g += sum_c lamE'_c dE_c / ie on the box; lamE' = the E part of the cotangent volume after reverse step n (volume n&1 of
-// lamA / lamB on the fused path, lamA alone otherwise)
-__global__ void k_grad_from_dE(Dims G, const float *__restrict__ lamA, const float *__restrict__ lamB, const float *__restrict__ dE,
-                               const float *__restrict__ ie, float *__restrict__ g, const int *__restrict__ step)
+// g += sum_c lamE'_c D_c on the box; lamE' = the E part of the cotangents after B1 + B2 of reverse step n: volume n&1 of
+// (lamA, lamB) after the fused adjoint step, lamA between the two adjoint kernels of the generic path
+__global__ void k_grad_from_dE(Dims G, const float *__restrict__ lamA, const float *__restrict__ lamB, const float *__restrict__ dE, int K,
+                               float *__restrict__ g, const int *__restrict__ step)
 {
     const int bx = G.ghi[0] - G.glo[0], by = G.ghi[1] - G.glo[1], bz = G.ghi[2] - G.glo[2];
     const long long bc = (long long)bx * by * bz;
-    const float *lam = (lamB && (*step & 1)) ? lamB : lamA;
+    const int n = *step;
+    dE += (long long)(n % K) * 3 * bc;
+    const float *lam = (lamB && (n & 1)) ? lamB : lamA;
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < bc; t += (long long)gridDim.x * blockDim.x) {
         const int i = G.glo[0] + (int)(t % bx), j = G.glo[1] + (int)((t / bx) % by), k = G.glo[2] + (int)(t / ((long long)bx * by));
         const long long p = lin(G, i, j, k);
         float acc = 0.f;
         for (int c = 0; c < 3; ++c) acc = fmaf(lam[c * G.nc + p], dE[c * bc + t], acc);
-        g[p] += acc / __ldg(ie + p);
+        g[p] += acc;
     }
 }
 
-void launch_dE_store(const Dims &G, const float *A, const float *B, float *dE, int mode, const int *step, cudaStream_t st)
+void launch_dE_store(const Dims &G, const float *A, const float *B, float *dE, int K, int mode, const float *ie, const float *sigma,
+                     const int *step, cudaStream_t st)
 {
     const long long n = (long long)(G.ghi[0] - G.glo[0]) * (G.ghi[1] - G.glo[1]) * (G.ghi[2] - G.glo[2]);
-    k_dE_store<<<(unsigned)std::min<long long>((n + 255) / 256, 1 << 16), 256, 0, st>>>(G, A, B, dE, mode, step);
+    k_dE_store<<<(unsigned)std::min<long long>((n + 255) / 256, 1 << 16), 256, 0, st>>>(G, A, B, dE, K, mode, ie, sigma, step);
 }
-void launch_dE_source(const Dims &G, float *dE, const SourceDev &s, const int *step, cudaStream_t st)
+void launch_dE_source(const Dims &G, float *dE, int K, const SourceDev &s, const float *ie, const float *sigma, const int *step, cudaStream_t st)
 {
     const long long n = (long long)(s.hi[0] - s.lo[0]) * (s.hi[1] - s.lo[1]) * (s.hi[2] - s.lo[2]);
-    k_dE_source<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(G, dE, s, step);
+    k_dE_source<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(G, dE, K, s, ie, sigma, step);
 }
-void launch_grad_from_dE(const Dims &G, const float *lamA, const float *lamB, const float *dE, const float *ie, float *g,
+void launch_grad_from_dE(const Dims &G, const float *lamA, const float *lamB, const float *dE, int K, float *g,
                          const int *step, cudaStream_t st)
 {
     const long long n = (long long)(G.ghi[0] - G.glo[0]) * (G.ghi[1] - G.glo[1]) * (G.ghi[2] - G.glo[2]);
-    k_grad_from_dE<<<(unsigned)std::min<long long>((n + 255) / 256, 1 << 16), 256, 0, st>>>(G, lamA, lamB, dE, ie, g, step);
+    k_grad_from_dE<<<(unsigned)std::min<long long>((n + 255) / 256, 1 << 16), 256, 0, st>>>(G, lamA, lamB, dE, K, g, step);
 }
 
 void launch_inv_E_grad(const Dims &G, float *fields, const float *ie, const float *lam, float *g, cudaStream_t st)

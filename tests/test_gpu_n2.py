@@ -297,3 +297,57 @@ def test_checkpointed_reverse_sweep(B, case):
     assert np.max(np.abs(g_tape[pml])) > 1e-3 * np.max(np.abs(g_tape))          # the PML cells do carry gradient
     assert relerr(gg, g_tape) <= TOL_GRAD and relerr(gg[pml], g_tape[pml]) <= TOL_GRAD, (relerr(gg, g_tape), relerr(gg[pml], g_tape[pml]))
     assert relerr(lam0.cpu().numpy(), lam_tape) <= TOL_GRAD
+
+
+@pytest.mark.parametrize("case", ["tiny", "mini"])
+def test_lossy_medium_forward_and_checkpointed_gradient(B, case):
+    """SURVEY 8(f) N4, reading R29: a random conductivity volume.  Forward fields and phasors against the oracle's lossy
+    update; the gradient from the checkpointed sweep (record=3; the only route: a lossy step cannot be time-reversed) and the
+    cotangent of state 0 against the oracle's tape mode, PML cells included.  On a grid that qualifies for the fused kernels
+    the calls fall back to the generic ones."""
+    import torch
+    from oracle.oracle import Oracle
+    if case == "tiny":
+        w = wl.tiny_pml(n_steps=30)
+    else:
+        w = wl.c3_mini(n_steps=70, kappa_max=3.0, alpha_max=0.05)
+        w.meta["inv_mu"] = None
+    shape = (w.nz, w.ny, w.nx)
+    sig = (0.25 * np.random.default_rng(12).random(shape, dtype=np.float32)).astype(np.float32)
+    im = w.meta["inv_mu"]
+    o = Oracle(**w.grid_kwargs())
+    o.set_sigma(sig)
+    fr = np.zeros((6,) + shape)
+    out = o.forward(fr, w.inv_eps, im, w.sources, w.detectors, w.n_steps, tape=True)
+    dLf_r = np.zeros_like(fr)
+    dLf_r[:3] = 0.5 * fr[:3]
+    g_tape, lam_tape = o.backward_tape(w.inv_eps, im, w.detectors, [2.0 * P for P in out["phasors"]], dLf_r, w.n_steps, out["tape"])
+    o0 = Oracle(**w.grid_kwargs())
+    f0 = np.zeros((6,) + shape)
+    o0.forward(f0, w.inv_eps, im, w.sources, w.detectors, w.n_steps)
+    assert relerr(fr[:3], f0[:3]) > 1e-2                      # the loss does change the fields
+    kw = w.grid_kwargs()
+    kw.update(max_steps=w.n_steps, record=3, checkpoint_every=9)
+    g = B.Grid(**kw)
+    g.set_conductivity(sig)
+    f = torch.zeros((6,) + shape, device="cuda")
+    ie = torch.as_tensor(w.inv_eps).cuda()
+    imt = None if im is None else torch.as_tensor(im).cuda()
+    ph = g.forward(f, ie, imt, w.sources, w.detectors, w.n_steps)
+    torch.cuda.synchronize()
+    fg = f.cpu().numpy()
+    assert relerr(fg[:3], fr[:3]) <= TOL_FIELD and relerr(fg[3:], fr[3:]) <= TOL_FIELD
+    for P, Pr in zip(ph, out["phasors"]):
+        assert relerr(P.cpu().numpy(), Pr) <= TOL_PHASOR
+    dLf = torch.zeros_like(f)
+    dLf[:3] = 0.5 * f[:3]
+    grad, lam0 = g.backward(f, ie, imt, w.sources, w.detectors, [2.0 * P for P in ph], dLf, w.n_steps, want_dL_dfields0=True)
+    torch.cuda.synchronize()
+    g.close()
+    assert relerr(grad.cpu().numpy(), g_tape) <= TOL_GRAD and relerr(lam0.cpu().numpy(), lam_tape) <= TOL_GRAD
+    # a recording grid refuses a lossy medium
+    g1 = B.Grid(**{**w.grid_kwargs(), "max_steps": 4, "record": 1})
+    with pytest.raises(B.FdtdError) as e:
+        g1.set_conductivity(sig)
+    assert e.value.code == B.FDTD_ESTATE
+    g1.close()
