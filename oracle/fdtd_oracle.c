@@ -105,7 +105,13 @@ typedef struct {
     REAL *lpsiE[3][2], *lpsiH[3][2];         /* cotangents of psi              */
     REAL *tmp[3][2];                         /* scratch volumes for the adjoint */
     const REAL *sigma;                       /* N4: normalised electric conductivity per voxel, or NULL (lossless) */
+    int aniso;                               /* N4: 1 = inv_eps (and its gradient) are three volumes, one per E component */
 } orc_state;
+
+/* N4 (SURVEY 8(f) N4 "per-component inv_eps (3 volumes / sub-pixel averaging)"), reading R30: with aniso set, inv_eps is      */
+/* [3][cells] and E_c is updated with inv_eps[c] at its own (staggered) position -- what sub-pixel smoothing of an interface     */
+/* produces -- instead of the one value per voxel of reading R6; the gradient is then [3][cells] as well.                        */
+#define IEC(c, p) ie[(st->aniso ? (size_t)(c) * nc : 0) + (p)]
 
 #define NX (D->nx)
 #define NY (D->ny)
@@ -291,6 +297,7 @@ void orc_zero_lpsi(orc_state *st)
 /* The inverse step is not defined for it (orc_backward refuses); gradients come from tape mode.                      */
 /* ------------------------------------------------------------------------ */
 void orc_set_sigma(orc_state *st, const REAL *sigma) { st->sigma = sigma; }
+void orc_set_aniso(orc_state *st, int aniso) { st->aniso = aniso ? 1 : 0; }
 
 /* ------------------------------------------------------------------------ */
 /* O1: E update (Eq. 2 discretised on the Yee grid; CPML psi_E recursion)   */
@@ -327,15 +334,15 @@ void orc_step_E(orc_state *st, REAL *fields, const REAL *ie, REAL *bracket)
                     REAL br = st->ikE[a][pos[a]] * d1 - st->ikE[b][pos[b]] * d2 + p0 - p1;
                     if (!st->sigma) {
                         if (bracket) bracket[(size_t)c * nc + p] = br;
-                        E[c][p] += S * ie[p] * br;
+                        E[c][p] += S * IEC(c, p) * br;
                     } else {
                         /* lossy update; `bracket` keeps its meaning dE'_c/d(ie) = S * bracket:                      */
                         /*   dCa/d ie = -sigma S / (1+beta)^2,  dCb/d ie = -(sigma S / 2) / (1+beta)^2               */
-                        const REAL hs = (REAL)0.5 * st->sigma[p] * S, beta = hs * ie[p];
+                        const REAL hs = (REAL)0.5 * st->sigma[p] * S, beta = hs * IEC(c, p);
                         const REAL Ca = ((REAL)1 - beta) / ((REAL)1 + beta), Cb = (REAL)1 / ((REAL)1 + beta);
                         const REAL dCa = (REAL)-2 * hs * Cb * Cb, dCb = -hs * Cb * Cb;
-                        if (bracket) bracket[(size_t)c * nc + p] = (dCa * E[c][p] + (dCb * ie[p] + Cb) * S * br) / S;
-                        E[c][p] = Ca * E[c][p] + Cb * S * ie[p] * br;
+                        if (bracket) bracket[(size_t)c * nc + p] = (dCa * E[c][p] + (dCb * IEC(c, p) + Cb) * S * br) / S;
+                        E[c][p] = Ca * E[c][p] + Cb * S * IEC(c, p) * br;
                     }
                 }
             }
@@ -644,6 +651,7 @@ int orc_forward_td(orc_state *st, REAL *fields, const REAL *ie, const REAL *im,
     const orc_desc *D = &st->D;
     const size_t nc = st->nc;
     const size_t rs = orc_record_stride(D);
+    for (int s = 0; s < n_td; ++s) if (st->aniso && td[s].kind == 1) return -1;    /* the energy detector is stated for one inv_eps per voxel */
     for (int n = 0; n < n_steps; ++n) {
         if (rec) record_faces(D, fields, nc, rec + (size_t)n * rs, 0);           /* O0r */
         orc_step_E(st, fields, ie, tape ? tape + (size_t)n * 3 * nc : NULL);     /* O1  */
@@ -742,11 +750,11 @@ void orc_adj_E(orc_state *st, REAL *lam, const REAL *ie)
                 const size_t p = IDX(i, j, k);
                 const int pos[3] = { i, j, k };
                 /* N4, lossy update E' = Ca E + Cb S ie bracket: the bracket's cotangent is Cb S ie lamE', and E's is Ca lamE' */
-                const REAL beta = st->sigma ? (REAL)0.5 * st->sigma[p] * S * ie[p] : (REAL)0;
-                const REAL Ca = ((REAL)1 - beta) / ((REAL)1 + beta), Cb = (REAL)1 / ((REAL)1 + beta);
                 for (int c = 0; c < 3; ++c) {
                     const int a = (c + 1) % 3, b = (c + 2) % 3;
-                    REAL w = (st->sigma ? Cb : (REAL)1) * S * ie[p] * lE[c][p];
+                    const REAL beta = st->sigma ? (REAL)0.5 * st->sigma[p] * S * IEC(c, p) : (REAL)0;
+                    const REAL Ca = ((REAL)1 - beta) / ((REAL)1 + beta), Cb = (REAL)1 / ((REAL)1 + beta);
+                    REAL w = (st->sigma ? Cb : (REAL)1) * S * IEC(c, p) * lE[c][p];
                     if (st->sigma) lE[c][p] *= Ca;
                     REAL l0 = st->lpsiE[c][0][p] + w;
                     REAL l1 = st->lpsiE[c][1][p] - w;
@@ -887,9 +895,10 @@ void orc_inv_E_grad(orc_state *st, REAL *fields, const REAL *ie, const REAL *lam
                     REAL d2 = H[a][p] - H_minus(D, H, rec_n, a, b, i, j, k);
                     REAL q = d1 - d2;
                     if (lam) acc += lam[(size_t)c * nc + p] * q;
-                    E[c][p] -= S * ie[p] * q;
+                    if (lam && g && st->aniso) g[(size_t)c * nc + p] += S * lam[(size_t)c * nc + p] * q;
+                    E[c][p] -= S * IEC(c, p) * q;
                 }
-                if (g) g[p] += S * acc;
+                if (g && !st->aniso) g[p] += S * acc;
             }
 }
 
@@ -935,7 +944,7 @@ int orc_backward_mu(orc_state *st, REAL *fields, const REAL *ie, const REAL *im,
     if (!lam) return -2;
     if (dL_dfields) memcpy(lam, dL_dfields, 6 * nc * sizeof(REAL));      /* B0 */
     orc_zero_lpsi(st);
-    memset(g, 0, nc * sizeof(REAL));
+    memset(g, 0, (st->aniso ? 3 : 1) * nc * sizeof(REAL));
     if (g_mu) memset(g_mu, 0, nc * sizeof(REAL));
     for (int n = n_steps - 1; n >= 0; --n) {
         const REAL *rec_n = rec ? rec + (size_t)n * rs : NULL;
@@ -979,14 +988,14 @@ int orc_backward_tape(orc_state *st, const REAL *ie, const REAL *im,
     if (!lam) return -2;
     if (dL_dfields) memcpy(lam, dL_dfields, 6 * nc * sizeof(REAL));
     orc_zero_lpsi(st);
-    memset(g, 0, nc * sizeof(REAL));
+    memset(g, 0, (st->aniso ? 3 : 1) * nc * sizeof(REAL));
     for (int n = n_steps - 1; n >= 0; --n) {
         const REAL *br = tape + (size_t)n * 3 * nc;
         detect_adjoint(D, lam, nc, det, n_det, dL_dphasor, n);
         orc_adj_H(st, lam, im);
         for (int c = 0; c < 3; ++c)
             for (size_t p = 0; p < nc; ++p)
-                g[p] += S * lam[(size_t)c * nc + p] * br[(size_t)c * nc + p];
+                g[(st->aniso ? (size_t)c * nc : 0) + p] += S * lam[(size_t)c * nc + p] * br[(size_t)c * nc + p];
         orc_adj_E(st, lam, ie);
     }
     if (dL_dfields0) memcpy(dL_dfields0, lam, 6 * nc * sizeof(REAL));

@@ -206,6 +206,18 @@ class Oracle:
     def zero_lpsi(self):
         self.L.orc_zero_lpsi(self.h)
 
+    def set_aniso(self, on=True):
+        """N4 (reading R30): inv_eps and its gradient become [3, nz, ny, nx], one volume per E component."""
+        self.aniso = bool(on)
+        self.L.orc_set_aniso.argtypes = [C.c_void_p, C.c_int]
+        self.L.orc_set_aniso(self.h, int(self.aniso))
+
+    def _ie(self, inv_eps):
+        return self.arr(inv_eps, ((3,) + self.shape) if getattr(self, "aniso", False) else self.shape)
+
+    def _gshape(self):
+        return ((3,) + self.shape) if getattr(self, "aniso", False) else self.shape
+
     def set_sigma(self, sigma):
         """N4 (reading R29): normalised electric conductivity per voxel for the lossy E update, or None (lossless)."""
         self._sigma = self.arr(sigma, self.shape)
@@ -295,7 +307,7 @@ class Oracle:
 
         Returns dict(phasors=[...], rec=array|None, tape=array|None)."""
         assert fields.dtype == self.dtype and fields.flags.c_contiguous
-        ie = self.arr(inv_eps, self.shape)
+        ie = self._ie(inv_eps)
         im = self.arr(inv_mu, self.shape)
         if reset_psi:
             self.zero_psi()
@@ -318,7 +330,7 @@ class Oracle:
         """Time-reversed gradient.  `fields` (state n_steps) is overwritten by the
         reconstructed state 0 on I.  Returns (g, dL_dfields0), or (g, dL_dfields0, dL/d inv_mu) with want_grad_mu (N4)."""
         assert fields.dtype == self.dtype and fields.flags.c_contiguous
-        ie = self.arr(inv_eps, self.shape)
+        ie = self._ie(inv_eps)
         im = self.arr(inv_mu, self.shape)
         sarr, ns, k1 = self._sources(sources)
         darr, nd, k2 = self._detectors(detectors, None)
@@ -331,7 +343,7 @@ class Oracle:
                 keep.append(Ga)
                 gp[i] = None if Ga is None else Ga.ctypes.data
         dLf = self.arr(dL_dfields)
-        g = np.zeros(self.shape, dtype=self.dtype)
+        g = np.zeros(self._gshape(), dtype=self.dtype)
         lam0 = np.zeros((6,) + self.shape, dtype=self.dtype)
         tarr, nt = self._tdetectors(time_detectors, None)
         tp = None
@@ -379,7 +391,7 @@ class Oracle:
 
     def backward_tape(self, inv_eps, inv_mu=None, detectors=(), dL_dphasor=None,
                       dL_dfields=None, n_steps=0, tape=None):
-        ie = self.arr(inv_eps, self.shape)
+        ie = self._ie(inv_eps)
         im = self.arr(inv_mu, self.shape)
         darr, nd, k2 = self._detectors(detectors, None)
         gp = None
@@ -391,7 +403,7 @@ class Oracle:
                 keep.append(Ga)
                 gp[i] = None if Ga is None else Ga.ctypes.data
         dLf = self.arr(dL_dfields)
-        g = np.zeros(self.shape, dtype=self.dtype)
+        g = np.zeros(self._gshape(), dtype=self.dtype)
         lam0 = np.zeros((6,) + self.shape, dtype=self.dtype)
         rc = self.L.orc_backward_tape(self.h, _ptr(ie), _ptr(im), darr, nd, gp, _ptr(dLf),
                                       int(n_steps), _ptr(tape), _ptr(g), _ptr(lam0))

@@ -362,3 +362,81 @@ def test_n4_lossy_gradient_against_finite_differences():
         im_[v] -= h
         fd = (loss(ip) - loss(im_)) / (2 * h)
         assert abs(fd - g[v]) < 2e-6 * scale + 1e-6 * abs(fd), (v, fd, g[v])
+
+
+# ----------------------------------------------------------------------------- N4: one inv_eps volume per E component (R30)
+def test_n4_per_component_inv_eps():
+    """(i) Three equal volumes reproduce the scalar run bit for bit and their three gradients sum to the scalar gradient;
+    (ii) a uniform diagonal-anisotropic periodic box carries the plane wave k || x, E || y at the speed eps_y alone fixes
+    (exact eigenmode, pin P1 with eps -> eps_y) -- eps_x, eps_z must not matter; (iii) tape-mode and time-reversed gradients
+    of the three volumes against central finite differences (tiny CPML grid, with a conductivity for the tape mode)."""
+    w = wl.tiny_pml(n_steps=30)
+    shape = (w.nz, w.ny, w.nx)
+    d = w.pml_cells
+    ie1 = w.inv_eps.astype(np.float64)
+    ie3 = np.stack([ie1, ie1, ie1])
+
+    def run(aniso, ie, sigma=None, mode="reversible"):
+        o = Oracle(**w.grid_kwargs())
+        if aniso:
+            o.set_aniso(True)
+        if sigma is not None:
+            o.set_sigma(sigma)
+        f = np.zeros((6,) + shape)
+        out = o.forward(f, ie, w.meta["inv_mu"], w.sources, w.detectors, w.n_steps, record=True, tape=(mode == "tape"))
+        P = out["phasors"][0]
+        L = float(np.sum(P * P)) + 0.5 * float(np.sum(f[:3] ** 2))
+        dLf = np.zeros_like(f)
+        dLf[:3] = f[:3]
+        fin = f.copy()
+        if mode == "tape":
+            g, _ = o.backward_tape(ie, w.meta["inv_mu"], w.detectors, [2.0 * P], dLf, w.n_steps, out["tape"])
+        elif mode == "reversible":
+            g, _ = o.backward(f, ie, w.meta["inv_mu"], w.sources, w.detectors, [2.0 * P], dLf, w.n_steps, out["rec"])
+        else:
+            g = None
+        return L, g, fin
+
+    L1, g1, f1 = run(False, ie1)
+    L3, g3, f3 = run(True, ie3)
+    assert np.array_equal(f1, f3) and L1 == L3
+    assert g3.shape == (3,) + shape and np.max(np.abs(g3.sum(0) - g1)) < 1e-12 * np.max(np.abs(g1))
+    # (iii) finite differences in single entries of the three volumes
+    rng = np.random.default_rng(4)
+    iea = ie3 * (0.8 + 0.4 * rng.random((3,) + shape))
+    sig = 0.2 * rng.random(shape)
+    for mode, sigma in (("reversible", None), ("tape", sig)):
+        L, g, _ = run(True, iea, sigma, mode)
+        scale = np.max(np.abs(g))
+        h = 1e-6
+        cells = [(0, w.nz // 2, w.ny // 2, w.nx // 2), (1, d, d, d), (2, w.nz - d - 1, w.ny - d - 1, w.nx - d - 1), (1, d + 1, d + 2, d + 3)]
+        if mode == "tape":
+            cells.append((2, 1, 2, 3))                 # a PML cell: only the tape mode has a gradient there
+        for v in cells:
+            ip, im_ = iea.copy(), iea.copy()
+            ip[v] += h
+            im_[v] -= h
+            fd = (run(True, ip, sigma, None)[0] - run(True, im_, sigma, None)[0]) / (2 * h)
+            assert abs(fd - g[v]) < 2e-6 * scale + 1e-6 * abs(fd), (mode, v, fd, g[v])
+    # (ii) exact eigenmode with k along x and E along y: only eps_y enters
+    nx, ny, nz = 16, 6, 5
+    sh = (nz, ny, nx)
+    kx = 2 * math.pi * 3 / nx
+    eps = np.array([5.0, 2.25, 9.0])
+    wq = 2 * math.asin(S / math.sqrt(eps[1]) * math.sin(kx / 2))
+    A = 0.7
+    Bz = S * (2 * math.sin(kx / 2)) * A / (2 * math.sin(wq / 2))      # P1: B = S (K x A) / (2 sin(w/2)), K = (Kx,0,0), A = (0,A,0)
+
+    def state(n):
+        f = np.zeros((6,) + sh)
+        x, y, z = _stag(sh, 1, False)
+        f[1] = A * np.cos(kx * x - wq * n) + 0 * y + 0 * z
+        x, y, z = _stag(sh, 2, True)
+        f[5] = Bz * np.cos(kx * x - wq * (n + 0.5)) + 0 * y + 0 * z
+        return f
+
+    o = Oracle(nx, ny, nz, S, periodic=True)
+    o.set_aniso(True)
+    f = state(0)
+    o.forward(f, np.stack([np.full(sh, 1.0 / e) for e in eps]), n_steps=41)
+    assert np.max(np.abs(f - state(41))) < 1e-12
