@@ -102,6 +102,11 @@ extern "C" {
                                        the rounding (2^-11 relative per recorded value); the gradient error this costs is
                                        measured in tests/test_gpu_parity.py and stated in DESIGN.md.                       */
 
+#define FDTD_FLAG_ANISO_EPS  4       /* SURVEY 8(f) N4, reading R30: inv_eps is [3][nz][ny][nx], one volume per E component (E_c is
+                                       updated with inv_eps[c] at its own staggered position: what sub-pixel smoothing of an
+                                       interface produces), and dL_dinv_eps is [3][nz][ny][nx] likewise.  Generic kernels only;
+                                       not with fdtd_grad_rho, the energy detector or the *_host entry points.               */
+
 typedef struct fdtd_grid fdtd_grid;      /* opaque */
 
 /* Grid descriptor.  A zero in any CPML constant selects its default (reading R8). */

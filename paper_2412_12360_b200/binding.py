@@ -20,7 +20,7 @@ LIB_PATH = _HERE / "libfdtd_b200.so"
 
 FDTD_OK, FDTD_EINVAL, FDTD_ENOMEM, FDTD_ECUDA, FDTD_ESTATE = 0, -1, -2, -3, -4
 FDTD_PATH_AUTO, FDTD_PATH_GENERIC, FDTD_PATH_FUSED = 0, 1, 2
-FDTD_FLAG_HOST_STAGING, FDTD_FLAG_RECORDER_FP16 = 1, 2
+FDTD_FLAG_HOST_STAGING, FDTD_FLAG_RECORDER_FP16, FDTD_FLAG_ANISO_EPS = 1, 2, 4
 PARTITION_NAMES = {0: "none (generic kernels)", 1: "contiguous runs", 2: "lock-step runs", 3: "waves of whole columns + levelled pool"}
 
 
@@ -447,7 +447,8 @@ class Grid:
             cot = (C.c_void_p * max(nd, 1))()
             for i, G in enumerate(dL_dphasor):
                 cot[i] = _ptr(G)
-        g = None if not want_grad else (out if out is not None else torch.empty(self.shape, dtype=torch.float32, device="cuda"))
+        gshape = ((3,) + self.shape) if (self.desc.flags & FDTD_FLAG_ANISO_EPS) else self.shape
+        g = None if not want_grad else (out if out is not None else torch.empty(gshape, dtype=torch.float32, device="cuda"))
         lam0 = torch.empty((6,) + self.shape, dtype=torch.float32, device="cuda") if (want_dL_dfields0 or not want_grad) else None
         if grad_mu is not None:          # N4: dL/d inv_mu into the caller's volume
             fdtd_backward_mu(self.h, fields, inv_eps, inv_mu, sarr, ns, darr, nd, cot, dL_dfields, int(n_steps),

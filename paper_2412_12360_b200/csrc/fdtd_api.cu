@@ -178,7 +178,11 @@ extern "C" int fdtd_create_grid(const fdtd_grid_desc *desc, fdtd_grid **out)
     if (desc->record == 3 && desc->z_global) return fail(FDTD_EINVAL, "the checkpointed reverse sweep is not available on a z-slab sub-grid");
     if (desc->path < 0 || desc->path > 2) return fail(FDTD_EINVAL, "unknown path");
     if (desc->reserved[0]) return fail(FDTD_EINVAL, "reserved fields must be zero");
-    if (desc->flags & ~(FDTD_FLAG_HOST_STAGING | FDTD_FLAG_RECORDER_FP16)) return fail(FDTD_EINVAL, "unknown bit in flags");
+    if (desc->flags & ~(FDTD_FLAG_HOST_STAGING | FDTD_FLAG_RECORDER_FP16 | FDTD_FLAG_ANISO_EPS)) return fail(FDTD_EINVAL, "unknown bit in flags");
+    if ((desc->flags & FDTD_FLAG_ANISO_EPS) && desc->path == FDTD_PATH_FUSED)
+        return fail(FDTD_EINVAL, "FDTD_FLAG_ANISO_EPS runs on the generic kernels (use FDTD_PATH_AUTO or FDTD_PATH_GENERIC)");
+    if ((desc->flags & FDTD_FLAG_ANISO_EPS) && (desc->flags & FDTD_FLAG_HOST_STAGING))
+        return fail(FDTD_EINVAL, "the host-buffer entry points take one inv_eps volume (no FDTD_FLAG_ANISO_EPS)");
     if (desc->pml_m < 0 || desc->pml_sigma_scale < 0 || desc->pml_kappa_max < 0 || desc->pml_alpha_max < 0 ||
         desc->pml_alpha_m < 0 || desc->pml_eps_bg < 0)
         return fail(FDTD_EINVAL, "CPML constants must be >= 0");
@@ -196,6 +200,7 @@ extern "C" int fdtd_create_grid(const fdtd_grid_desc *desc, fdtd_grid **out)
     const int dp4 = (G.d + 3) / 4 * 4;
     G.dpx = (G.nx % 4 == 0 && G.nx >= 2 * dp4) ? dp4 : G.d;
     for (int a = 0; a < 3; ++a) { G.lo[a] = G.d; G.hi[a] = dim_of(G, a) - G.d; }
+    G.aniso = (desc->flags & FDTD_FLAG_ANISO_EPS) ? 1 : 0;
     G.zoff = sub ? desc->z_offset : 0; G.nzg = nz_full;
     G.zl = std::min(G.nz, std::max(0, G.d - G.zoff));
     G.zh = std::min(G.nz, std::max(0, G.zoff + G.nz - (G.nzg - G.d)));
@@ -483,6 +488,7 @@ int translate_td(fdtd_grid *g, const fdtd_time_detector *td, int n_td, int n_ste
             return fail(FDTD_EINVAL, "snapshot detector component_mask must be 1..63");
         if (!box_ok(g->G, td[s].lo, td[s].hi)) return fail(FDTD_EINVAL, "time detector box outside the grid or empty");
         if (td[s].stride < 1) return fail(FDTD_EINVAL, "time detector stride must be >= 1");
+        if (td[s].kind == FDTD_TD_ENERGY && g->G.aniso) return fail(FDTD_EINVAL, "the energy detector is stated for one inv_eps per voxel (no FDTD_FLAG_ANISO_EPS)");
         out[s].kind = td[s].kind;
         out[s].mask = td[s].kind == FDTD_TD_SNAPSHOT ? td[s].component_mask : 0;
         out[s].ncomp = popcount6(out[s].mask);
@@ -850,7 +856,7 @@ static int checkpointed_backward(fdtd_grid *g, float *fields, const float *inv_e
     translate(src, n_src, S);
     const bool fused_f = g->path == FDTD_PATH_FUSED && n_src <= FDTD_FUSED_MAX_SRC && !g->sigma;      // the replay runs without detectors
     const size_t vol = (size_t)G.nc * sizeof(float);
-    CK(cudaMemsetAsync(dL_dinv_eps, 0, vol, st));
+    CK(cudaMemsetAsync(dL_dinv_eps, 0, (G.aniso ? 3 : 1) * vol, st));
     const int K = g->ck_every;
     int rc = FDTD_OK;
     for (int a = (n_total - 1) / K * K; a >= 0 && n_total > 0; a -= K) {
@@ -962,7 +968,7 @@ static int backward_core(fdtd_grid *g, float *fields, const float *inv_eps, cons
         else            CK(cudaMemsetAsync(g->lam, 0, 6 * vol, st));
         for (int q = 0; q < 2; ++q)
             if ((rc = g->zero_psi(g->lpsiE[q], st)) || (rc = g->zero_psi(g->lpsiH[q], st))) return rc;
-        if (dL_dinv_eps) CK(cudaMemsetAsync(dL_dinv_eps, 0, vol, st));
+        if (dL_dinv_eps) CK(cudaMemsetAsync(dL_dinv_eps, 0, (G.aniso ? 3 : 1) * vol, st));
         if (dL_dinv_mu) CK(cudaMemsetAsync(dL_dinv_mu, 0, vol, st));
     }
     launch_set_step(g->d_step, std::max(n_hi - 1, 0), st);      // the first reverse step of the call reads slot 0
@@ -1032,6 +1038,7 @@ extern "C" int fdtd_grad_rho(fdtd_grid *g, const float *dL_dinv_eps, const float
 {
     if (!g || !dL_dinv_eps || !inv_eps || !lo || !hi || !dL_drho) return fail(FDTD_EINVAL, "fdtd_grad_rho: NULL argument");
     if (!box_ok(g->G, lo, hi)) return fail(FDTD_EINVAL, "fdtd_grad_rho: box outside the grid or empty");
+    if (g->G.aniso) return fail(FDTD_EINVAL, "fdtd_grad_rho is stated for one inv_eps per voxel (no FDTD_FLAG_ANISO_EPS)");
     launch_grad_rho(g->G, dL_dinv_eps, inv_eps, delta_eps, lo, hi, dL_drho, (cudaStream_t)cuda_stream);
     g->kernel_launches += 1;
     cudaError_t e = cudaGetLastError();

@@ -50,12 +50,13 @@ __global__ void __launch_bounds__(BX *BY) k_update_E(Dims G, Tables T, float *__
                                                      const float *__restrict__ ie, PsiSet psi, const float *__restrict__ sigma)
 {
     CELL_IJK();
-    const float beta = sigma ? 0.5f * __ldg(sigma + p) * G.S * __ldg(ie + p) : 0.f;
-    const float Ca = (1.f - beta) / (1.f + beta), Cb = 1.f / (1.f + beta);
-    const float sie = (sigma ? Cb : 1.f) * G.S * __ldg(ie + p);
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         const int a = (c + 1) % 3, b = (c + 2) % 3;
+        const float e = __ldg(ie + (G.aniso ? c * G.nc : 0) + p);            // reading R30: one volume per component when aniso
+        const float beta = sigma ? 0.5f * __ldg(sigma + p) * G.S * e : 0.f;
+        const float Ca = (1.f - beta) / (1.f + beta), Cb = 1.f / (1.f + beta);
+        const float sie = (sigma ? Cb : 1.f) * G.S * e;
         const float *Hb = f + (3 + b) * G.nc, *Ha = f + (3 + a) * G.nc;
         const float d1 = Hb[p] - fetch<PER>(G, Hb, i - (a == 0), j - (a == 1), k - (a == 2));
         const float d2 = Ha[p] - fetch<PER>(G, Ha, i - (b == 0), j - (b == 1), k - (b == 2));
@@ -168,9 +169,10 @@ __global__ void k_detector(Dims G, float *__restrict__ f, DetectorDev dt, const 
 __global__ void k_lossy_scale_E(Dims G, float *__restrict__ lam, const float *__restrict__ ie, const float *__restrict__ sigma)
 {
     for (long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x; p < G.nc; p += (long long)gridDim.x * blockDim.x) {
-        const float beta = 0.5f * __ldg(sigma + p) * G.S * __ldg(ie + p);
-        const float Ca = (1.f - beta) / (1.f + beta);
-        lam[p] *= Ca; lam[G.nc + p] *= Ca; lam[2 * G.nc + p] *= Ca;
+        for (int c = 0; c < 3; ++c) {
+            const float beta = 0.5f * __ldg(sigma + p) * G.S * __ldg(ie + (G.aniso ? c * G.nc : 0) + p);
+            lam[c * G.nc + p] *= (1.f - beta) / (1.f + beta);
+        }
     }
 }
 
@@ -331,7 +333,7 @@ struct AdjCtx {
     const float *sigma;      // FAMILY 0 only, lossy E update (N4): the bracket's cotangent is Cb S ie lamE'
     __device__ __forceinline__ float w(int c, long long q) const
     {
-        const float m = med ? __ldg(med + q) : 1.f;
+        const float m = med ? __ldg(med + ((!FAMILY && G.aniso) ? c * G.nc : 0) + q) : 1.f;
         float r = (FAMILY ? -G.S : G.S) * m * __ldg(lam_src + c * G.nc + q);
         if (!FAMILY && sigma) r /= 1.f + 0.5f * __ldg(sigma + q) * G.S * m;
         return r;
@@ -465,7 +467,7 @@ __global__ void __launch_bounds__(BX *BY) k_inv_E_grad(Dims G, float *__restrict
     CELL_IJK();
     if (lam2 && ((*step) & 1)) lam = lam2;           // ping-pong cotangents of the fused path: lamE' of step n is in buffer n&1
     if (i < G.lo[0] || i >= G.hi[0] || j < G.lo[1] || j >= G.hi[1] || k < G.lo[2] || k >= G.hi[2]) return;
-    const float sie = G.S * __ldg(ie + p);
+    const bool ing = i >= G.glo[0] && i < G.ghi[0] && j >= G.glo[1] && j < G.ghi[1] && k >= G.glo[2] && k < G.ghi[2];
     float acc = 0.f;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
@@ -474,11 +476,12 @@ __global__ void __launch_bounds__(BX *BY) k_inv_E_grad(Dims G, float *__restrict
         const float d1 = Hb[p] - fetch<PER>(G, Hb, i - (a == 0), j - (a == 1), k - (a == 2));
         const float d2 = Ha[p] - fetch<PER>(G, Ha, i - (b == 0), j - (b == 1), k - (b == 2));
         const float q = d1 - d2;
-        acc += __ldg(lam + c * G.nc + p) * q;
-        f[c * G.nc + p] -= sie * q;
+        const float lq = __ldg(lam + c * G.nc + p) * q;
+        acc += lq;
+        if (G.aniso && ing) g[c * G.nc + p] += G.S * lq;                   // reading R30: one gradient volume per component
+        f[c * G.nc + p] -= G.S * __ldg(ie + (G.aniso ? c * G.nc : 0) + p) * q;
     }
-    if (i >= G.glo[0] && i < G.ghi[0] && j >= G.glo[1] && j < G.ghi[1] && k >= G.glo[2] && k < G.ghi[2])
-        g[p] += G.S * acc;
+    if (!G.aniso && ing) g[p] += G.S * acc;
 }
 
 // ------------------------------------------------------------------------------------------ B6
@@ -640,10 +643,10 @@ __global__ void k_dE_store(Dims G, const float *__restrict__ A, const float *__r
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < bc; t += (long long)gridDim.x * blockDim.x) {
         const int i = G.glo[0] + (int)(t % bx), j = G.glo[1] + (int)((t / bx) % by), k = G.glo[2] + (int)(t / ((long long)bx * by));
         const long long p = lin(G, i, j, k);
-        const float e = __ldg(ie + p);
-        const float hs = sigma ? 0.5f * __ldg(sigma + p) * G.S : 0.f, Cb = 1.f / (1.f + hs * e), Ca = (1.f - hs * e) * Cb;
-        const float dCa = -2.f * hs * Cb * Cb, F = (-hs * Cb * Cb * e + Cb) / (Cb * e);
         for (int c = 0; c < 3; ++c) {
+            const float e = __ldg(ie + (G.aniso ? c * G.nc : 0) + p);
+            const float hs = sigma ? 0.5f * __ldg(sigma + p) * G.S : 0.f, Cb = 1.f / (1.f + hs * e), Ca = (1.f - hs * e) * Cb;
+            const float dCa = -2.f * hs * Cb * Cb, F = (-hs * Cb * Cb * e + Cb) / (Cb * e);
             float *o = dE + c * bc + t;
             if (mode == 0) *o = (En1[c * G.nc + p] - En[c * G.nc + p]) / e;
             else if (mode == 1) *o = En[c * G.nc + p];
@@ -666,7 +669,7 @@ __global__ void k_dE_source(Dims G, float *__restrict__ dE, int K, SourceDev s, 
     const long long q = ((long long)(k - G.glo[2]) * gy + (j - G.glo[1])) * gx + (i - G.glo[0]);
     const int n = *step;
     const long long p = lin(G, i, j, k);
-    const float e = __ldg(ie + p);
+    const float e = __ldg(ie + (G.aniso ? s.comp * G.nc : 0) + p);
     const float hs = sigma ? 0.5f * __ldg(sigma + p) * G.S : 0.f, Cb = 1.f / (1.f + hs * e);
     const float F = (-hs * Cb * Cb * e + Cb) / (Cb * e);
     dE[(long long)(n % K) * 3 * bc + (long long)s.comp * bc + q] -= F * (s.profile ? __ldg(s.profile + t) : 1.f) * __ldg(s.waveform + n);
@@ -685,8 +688,11 @@ __global__ void k_grad_from_dE(Dims G, const float *__restrict__ lamA, const flo
         const int i = G.glo[0] + (int)(t % bx), j = G.glo[1] + (int)((t / bx) % by), k = G.glo[2] + (int)(t / ((long long)bx * by));
         const long long p = lin(G, i, j, k);
         float acc = 0.f;
-        for (int c = 0; c < 3; ++c) acc = fmaf(lam[c * G.nc + p], dE[c * bc + t], acc);
-        g[p] += acc;
+        for (int c = 0; c < 3; ++c) {
+            const float v = lam[c * G.nc + p] * dE[c * bc + t];
+            if (G.aniso) g[c * G.nc + p] += v; else acc += v;
+        }
+        if (!G.aniso) g[p] += acc;
     }
 }
 

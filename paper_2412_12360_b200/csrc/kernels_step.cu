@@ -1320,6 +1320,7 @@ int fused_setup(fdtd_grid *g)
     const Dims &G = g->G;
     if (g->desc.path == FDTD_PATH_GENERIC) { g->fused_why_not = "generic path requested"; return FDTD_OK; }
     if (G.periodic) { g->fused_why_not = "periodic grids use the generic kernels"; return FDTD_OK; }
+    if (G.aniso) { g->fused_why_not = "per-component inv_eps (FDTD_FLAG_ANISO_EPS) uses the generic kernels"; return FDTD_OK; }
     if (G.nx % 4) { g->fused_why_not = "nx is not a multiple of 4"; return FDTD_OK; }
     if (G.d > 0 && (G.dpx % 4)) { g->fused_why_not = "x-slab psi storage is not float4 aligned (nx < 2*roundup4(d))"; return FDTD_OK; }
     if (G.nc >= (1LL << 31) - 4LL * G.nx * G.ny) { g->fused_why_not = "more than 2^31 cells (32-bit plane offsets)"; return FDTD_OK; }

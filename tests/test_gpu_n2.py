@@ -351,3 +351,57 @@ def test_lossy_medium_forward_and_checkpointed_gradient(B, case):
         g1.set_conductivity(sig)
     assert e.value.code == B.FDTD_ESTATE
     g1.close()
+
+
+@pytest.mark.parametrize("case", ["tiny-reversible", "mini-reversible", "mini-checkpointed-lossy"])
+def test_per_component_inv_eps(B, case):
+    """SURVEY 8(f) N4, reading R30 (FDTD_FLAG_ANISO_EPS): three inv_eps volumes, three gradient volumes.  Fields, phasors and the
+    time-reversed gradient against the oracle; with a conductivity, the checkpointed gradient against the oracle's tape mode."""
+    import torch
+    from oracle.oracle import Oracle
+    w = wl.tiny_pml(n_steps=30) if case.startswith("tiny") else wl.c3_mini(n_steps=70, kappa_max=3.0, alpha_max=0.05)
+    shape = (w.nz, w.ny, w.nx)
+    rng = np.random.default_rng(4)
+    ie3 = (np.stack([w.inv_eps] * 3) * (0.8 + 0.4 * rng.random((3,) + shape, dtype=np.float32))).astype(np.float32)
+    lossy = case.endswith("lossy")
+    sig = (0.2 * rng.random(shape, dtype=np.float32)).astype(np.float32) if lossy else None
+    im = w.meta.get("inv_mu")
+    o = Oracle(**w.grid_kwargs())
+    o.set_aniso(True)
+    if lossy:
+        o.set_sigma(sig)
+    fr = np.zeros((6,) + shape)
+    out = o.forward(fr, ie3, im, w.sources, w.detectors, w.n_steps, record=not lossy, tape=lossy)
+    dLf_r = np.zeros_like(fr)
+    dLf_r[:3] = 0.5 * fr[:3]
+    dLp_r = [2.0 * P for P in out["phasors"]]
+    fin = fr.copy()
+    if lossy:
+        g_r, lam_r = o.backward_tape(ie3, im, w.detectors, dLp_r, dLf_r, w.n_steps, out["tape"])
+    else:
+        g_r, lam_r = o.backward(fr, ie3, im, w.sources, w.detectors, dLp_r, dLf_r, w.n_steps, out["rec"])
+    kw = w.grid_kwargs()
+    kw.update(max_steps=w.n_steps, record=3 if lossy else 1, flags=B.FDTD_FLAG_ANISO_EPS)
+    g = B.Grid(**kw)
+    assert g.info().path == B.FDTD_PATH_GENERIC
+    if lossy:
+        g.set_conductivity(sig)
+    f = torch.zeros((6,) + shape, device="cuda")
+    ie = torch.as_tensor(ie3).cuda()
+    imt = None if im is None else torch.as_tensor(im).cuda()
+    ph = g.forward(f, ie, imt, w.sources, w.detectors, w.n_steps)
+    torch.cuda.synchronize()
+    fg = f.cpu().numpy()
+    assert relerr(fg[:3], fin[:3]) <= TOL_FIELD and relerr(fg[3:], fin[3:]) <= TOL_FIELD
+    for P, Pr in zip(ph, out["phasors"]):
+        assert relerr(P.cpu().numpy(), Pr) <= TOL_PHASOR
+    dLf = torch.zeros_like(f)
+    dLf[:3] = 0.5 * f[:3]
+    grad, lam0 = g.backward(f, ie, imt, w.sources, w.detectors, [2.0 * P for P in ph], dLf, w.n_steps, want_dL_dfields0=True)
+    torch.cuda.synchronize()
+    g.close()
+    assert tuple(grad.shape) == (3,) + shape
+    gg = grad.cpu().numpy()
+    for c in range(3):
+        assert np.max(np.abs(g_r[c])) > 0
+    assert relerr(gg, g_r) <= TOL_GRAD and relerr(lam0.cpu().numpy(), lam_r) <= TOL_GRAD
