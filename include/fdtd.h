@@ -2,7 +2,7 @@
  * fdtd.h -- C ABI of the B200-native FDTD hot path (arXiv 2412.12360, "FDTDX").
  *
  * What the library computes (citations: /root/reference/PAPER.md line numbers; the
- * discretisation choices the paper leaves open are the readings R1..R22 of DESIGN.md):
+ * discretisation choices the paper leaves open are the readings R1..R30 of DESIGN.md):
  *
  *   forward  : n_steps of the Yee-grid leapfrog (Eq. 1-2; Yee staggering L68):
  *              E update with per-voxel inverse permittivity and CPML psi_E recursion (L72),

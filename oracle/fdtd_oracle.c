@@ -22,7 +22,7 @@
  *                      volume ... saved for every time step"
  * Everything below that level (index convention, normalisation, CPML grading,
  * DFT phase stamp, what the recorder stores) is silent in the paper; the
- * readings R1..R22 are listed in DESIGN.md section 3 and followed literally here.
+ * readings R1..R30 are listed in DESIGN.md section 3 and followed literally here.
  *
  * Conventions:
  *   grid nx*ny*nz, x fastest: lin = (k*ny + j)*nx + i
@@ -50,6 +50,12 @@
  * the zero-frequency limit and the low-frequency response of ref. 7's
  * stretch factor; the rho chain rule (B6) against a central finite
  * difference of the loss with respect to rho.
+ * NEXT rows (tests/test_oracle_pins_n2.py): flux and energy of the exact
+ * eigenmode in closed form, detector transposes and flux VJP against finite
+ * differences, one-directionality of the TFSF plane source (N2); dL/d inv_mu,
+ * the lossy update (closed-form eigenvalue of a plane wave in a conductive
+ * box) and one inv_eps per E component (exact eigenmode of a diagonal-
+ * anisotropic box) with their gradients against finite differences (N4).
  * Parity unpinned: agreement with the paper's own FDTDX outputs (no numbers,
  * code, geometry or data are available) and the specific CPML constants /
  * DFT normalisation FDTDX uses.
