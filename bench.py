@@ -231,6 +231,62 @@ def run_reference(args, rank):
 
 
 # ------------------------------------------------------------------------------------------------
+def run_decomposed(args, rank, world, local_rank, barrier):
+    """--decompose z: one grid, `world` z slabs, one halo exchange per time step (include/fdtd.h "Domain decomposition").
+    Forward pass and adjoint sweep of the whole grid; value = cells * time_steps / time, strong scaling."""
+    import torch
+    from paper_2412_12360_b200 import binding as B
+    from paper_2412_12360_b200 import sharding
+    w = make_workload(args)                                   # the same problem on every rank: each takes its slab
+    T = args.time_steps or min(w.n_steps, 200)
+    slab = sharding.z_slabs(w.nz, world, w.pml_cells)[rank]
+    r = sharding.SlabRunner(B, w, slab, T, record=0)
+    dev = torch.device("cuda", local_rank)
+    seed = torch.zeros((6, w.nz, w.ny, w.nx), dtype=torch.float32, device=dev)
+    seed[1, w.nz // 2] = 1.0                                  # a fixed cotangent seed for the adjoint sweep
+
+    def fwd():
+        r.fields.zero_()
+        for P in r.phasors:
+            P.zero_()
+        sharding.run_slab_distributed(r, T, "forward")
+
+    def adj():
+        r.set_cotangents(None, seed)
+        sharding.run_slab_distributed(r, T, "backward")
+
+    def timed(fn, reps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        barrier()
+        return sharding.max_over_ranks(e0.elapsed_time(e1), device=dev)
+
+    for _ in range(args.warmup):
+        fwd()
+    ms_f = timed(fwd, args.steps)
+    r.want_grad = False                                       # adjoint sweep only (dL_dinv_eps = NULL)
+    adj()
+    ms_a = timed(adj, max(1, min(args.steps, 3)))
+    info = r.grid.info()
+    if rank == 0:
+        cs = w.cells * T
+        print(json.dumps({"metric": "Yee cell-updates/s, forward pass of ONE grid cut into z slabs (strong scaling)",
+                          "value": cs * args.steps / (ms_f * 1e-3) / 1e6, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                          "warmup": args.warmup, "ms_per_step": ms_f / args.steps, "higher_is_better": True, "scaling": "strong",
+                          "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                          "config": workload_config(w, {"time_steps": T, "parallelism": f"z slabs x{world}, one halo exchange per time step "
+                                                        "(3 planes of nx*ny floats per neighbour and direction)",
+                                                        "slab_planes": slab.nz, "path": {1: "generic", 2: "fused"}[info.path]}),
+                          "adjoint_sweep": {"value": cs * max(1, min(args.steps, 3)) / (ms_a * 1e-3) / 1e6, "unit": UNIT},
+                          "gpu_launches": int(info.kernel_launches)}))
+    r.close()
+
+
+# ------------------------------------------------------------------------------------------------
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -247,6 +303,10 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--lean", action="store_true",
                     help="memory-scale runs: no second (forward-only) grid, hence no forward-only and adjoint-only passes")
+    ap.add_argument("--decompose", default="", choices=["", "z"],
+                    help="z: ONE grid cut into z slabs, one per rank (SURVEY 8(e) / 8(f) N3; sharding.run_slab_distributed, NCCL "
+                         "point-to-point halo exchange once per time step); times the forward pass and the adjoint sweep of the whole "
+                         "grid (strong scaling).  Not measured on more than one GPU in this build: see DESIGN.md section 10")
     ap.add_argument("--recorder-fp16", action="store_true",
                     help="SURVEY 8(f) N1: store the interface record as fp16 (FDTD_FLAG_RECORDER_FP16; an approximation, off by default)")
     ap.add_argument("--record", default="", choices=["", "1", "2", "both"],
@@ -281,6 +341,12 @@ def main():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
+
+    if args.decompose == "z":
+        run_decomposed(args, rank, world, local_rank, barrier)
+        if world > 1:
+            dist.destroy_process_group()
+        return
 
     # ---- workload (seed + rank: every rank an independent problem) ---------------------------------
     w = make_workload(args, rank)

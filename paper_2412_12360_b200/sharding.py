@@ -167,6 +167,7 @@ class SlabRunner:
         self.send_down, self.send_up = t.empty(plane, device="cuda"), t.empty(plane, device="cuda")
         self.recv_below, self.recv_above = t.empty(plane, device="cuda"), t.empty(plane, device="cuda")
         self.grad = self.lam0 = self._cot = self._dLf = None
+        self.want_grad = True          # False: the reverse steps are adjoint steps only (no gradient, nothing reconstructed)
 
     def close(self):
         self.grid.close()
@@ -208,9 +209,9 @@ class SlabRunner:
         self.grad = t.empty((self.slab.nz, self.w.ny, self.w.nx), dtype=t.float32, device="cuda")
         self.lam0 = t.empty((6, self.slab.nz, self.w.ny, self.w.nx), dtype=t.float32, device="cuda")
 
-    def backward_steps(self, n_hi: int, n_lo: int, want_grad: bool = True):
+    def backward_steps(self, n_hi: int, n_lo: int):
         self.B.fdtd_backward_range(self.grid.h, self.fields, self.ie, self.im, self.sarr, self.ns, self.darr_b, self.nd_b,
-                                   self._cot, self._dLf, n_hi, n_lo, self.n_total, self.grad if want_grad else None,
+                                   self._cot, self._dLf, n_hi, n_lo, self.n_total, self.grad if self.want_grad else None,
                                    self.lam0, self.grid.stream())
 
 
