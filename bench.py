@@ -286,6 +286,41 @@ def run_decomposed(args, rank, world, local_rank, barrier):
     r.close()
 
 
+def run_probe(args):
+    """bench.py --probe: what the memory system gives for the step kernel's bytes and traversal, without its arithmetic."""
+    import torch
+    from paper_2412_12360_b200 import binding as B
+    N = args.grid or 200
+    vin = torch.rand((7, N, N, N), device="cuda")
+    vout = torch.empty((6, N, N, N), device="cuda")
+    st = torch.cuda.current_stream().cuda_stream
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    peaks_file = ROOT / "MEASURED_PEAKS.json"
+    if peaks_file.exists():
+        peaks = {"hbm_gbs": float(json.loads(peaks_file.read_text())["hbm_gbs"]), "source": "measured (MEASURED_PEAKS.json hbm_gbs)"}
+    else:
+        peaks = {"hbm_gbs": 6650.0, "source": "fallback (B200_PROFILING.md)"}
+    rows = []
+
+    def one(label, pattern, tile_y=0, runs=1, unroll=1, blocks=0, threads=256):
+        gbs = B.fdtd_probe_bandwidth(pattern, N, N, N, tile_y, runs, unroll, blocks, threads, 20, vin, vout, st)
+        us = 13 * 4 * N ** 3 * (runs if pattern == 0 else 1) / gbs / 1e3
+        rows.append({"probe": label, "GB/s": round(gbs, 1), "us": round(us, 1), "frac_of_peak": round(gbs / peaks["hbm_gbs"], 3)})
+
+    for b in (4, 8, 16):
+        one(f"stream {sms * b}x256", 0, blocks=sms * b, threads=256)
+    if 13 * 4 * N ** 3 < 60e6:                  # fits in L2: many passes per launch = the L2 <-> SM rate of this mix
+        one(f"stream {sms * 8}x256, 20 passes per launch (L2 resident)", 0, runs=20, blocks=sms * 8, threads=256)
+        one(f"stream {sms * 8}x512, 20 passes per launch (L2 resident)", 0, runs=20, blocks=sms * 8, threads=512)
+    for ty, runs, u, th in ((7, 5, 1, 384), (7, 5, 2, 384), (7, 5, 4, 384), (7, 10, 1, 384), (7, 10, 2, 384), (7, 20, 2, 384),
+                            (14, 10, 2, 512), (28, 20, 2, 512)):
+        nb = (N + ty - 1) // ty * runs
+        one(f"tile {N}x{ty} runs={runs} unroll={u} ({nb} blocks x {th}, {nb / sms:.2f}/SM)", 1, ty, runs, u, threads=th)
+    print(json.dumps({"probe": "7 volumes read + 6 written, float4 per thread, no arithmetic (fdtd_probe_bandwidth)",
+                      "grid": [N, N, N], "bytes_per_launch": 13 * 4 * N ** 3, "peak_hbm_gbs": peaks["hbm_gbs"],
+                      "peak_source": peaks["source"], "rows": rows}))
+
+
 # ------------------------------------------------------------------------------------------------
 def main():
     ap = argparse.ArgumentParser()
@@ -313,6 +348,10 @@ def main():
                     help="1: `value` only (record the PML/interior interface, reconstruct the interior); 2: `value` on the "
                          "design-box recorder instead (labelled); both (default where there is a design box and memory allows): "
                          "`value` on record=1 and the record=2 figure beside it")
+    ap.add_argument("--probe", action="store_true",
+                    help="no FDTD: the bandwidth probes of fdtd_probe_bandwidth (the step kernel's 7 volumes read + 6 written "
+                         "without its arithmetic, streaming and in the step kernel's tile-column traversal) on the --grid size "
+                         "(default 200), one JSON line; DESIGN.md section 8")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -341,6 +380,13 @@ def main():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
+
+    if args.probe:
+        if rank == 0:
+            run_probe(args)
+        if world > 1:
+            dist.destroy_process_group()
+        return
 
     if args.decompose == "z":
         run_decomposed(args, rank, world, local_rank, barrier)

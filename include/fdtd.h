@@ -407,6 +407,15 @@ FDTD_API int fdtd_get_profile(fdtd_grid *grid, fdtd_profile *out);
 FDTD_API int fdtd_debug_partition(int32_t nx, int32_t ny, int32_t nz, int32_t d, int32_t tile_x, int32_t tile_y,
                          int32_t n_cta, double wy, double wz, int32_t lockstep, int32_t *segments, int32_t cap);
 
+/* Bandwidth probe for the roofline discussion (bench.py --probe; not on the hot path): moves the step kernel's bytes -- 7 volumes
+ * read, 6 written, float4 per thread -- without its arithmetic.  pattern 0: grid-stride streaming with `blocks` x `threads`, `runs` passes over the volumes per launch;
+ * pattern 1: the step kernel's traversal, a block per (tile column of tile_y whole-x rows, run of nz / runs planes), `unroll`
+ * (1, 2, 4) planes in flight per iteration.  in: DEVICE 7 * nx*ny*nz floats, out: DEVICE 6 * nx*ny*nz floats.  Synchronous: times
+ * `reps` launches with CUDA events after 3 warm-up launches; *gbs = 13 volumes * reps / time in GB/s. */
+FDTD_API int fdtd_probe_bandwidth(int32_t pattern, int32_t nx, int32_t ny, int32_t nz, int32_t tile_y, int32_t runs, int32_t unroll,
+                         int32_t blocks, int32_t threads, int32_t reps, const float *in, float *out, double *gbs,
+                         void *cuda_stream);
+
 /* Library version string, e.g. "fdtd-b200 0.1 sm_100a". */
 FDTD_API const char *fdtd_version(void);
 

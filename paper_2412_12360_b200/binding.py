@@ -73,7 +73,7 @@ class fdtd_profile(C.Structure):
 EXPORTS = ("fdtd_grad_rho", "fdtd_set_profiling", "fdtd_get_profile", "fdtd_create_grid", "fdtd_forward", "fdtd_backward", "fdtd_destroy", "fdtd_last_error",
            "fdtd_get_info", "fdtd_version", "fdtd_forward_host", "fdtd_backward_host", "fdtd_debug_partition",
            "fdtd_forward_td", "fdtd_backward_td", "fdtd_flux", "fdtd_flux_vjp", "fdtd_tfsf_plane",
-           "fdtd_forward_range", "fdtd_backward_range", "fdtd_halo_export", "fdtd_halo_import", "fdtd_backward_mu", "fdtd_set_conductivity")
+           "fdtd_forward_range", "fdtd_backward_range", "fdtd_halo_export", "fdtd_halo_import", "fdtd_backward_mu", "fdtd_set_conductivity", "fdtd_probe_bandwidth")
 
 
 def _load():
@@ -250,6 +250,16 @@ def fdtd_backward_mu(grid, fields, inv_eps, inv_mu, src, n_src, det, n_det, dL_d
                      dL_dinv_eps, dL_dinv_mu, dL_dfields0, stream) -> None:
     _check(_L.fdtd_backward_mu(grid, _ptr(fields), _ptr(inv_eps), _ptr(inv_mu), src, n_src, det, n_det, dL_dphasor,
                                _ptr(dL_dfields), n_steps, _ptr(dL_dinv_eps), _ptr(dL_dinv_mu), _ptr(dL_dfields0), stream))
+
+
+def fdtd_probe_bandwidth(pattern, nx, ny, nz, tile_y, runs, unroll, blocks, threads, reps, vin, vout, stream) -> float:
+    """GB/s of the 7-read / 6-write probe (include/fdtd.h); vin: 7 volumes, vout: 6 volumes (cuda tensors)."""
+    _L.fdtd_probe_bandwidth.restype = C.c_int
+    _L.fdtd_probe_bandwidth.argtypes = [C.c_int32] * 10 + [C.c_void_p, C.c_void_p, C.POINTER(C.c_double), C.c_void_p]
+    out = C.c_double(0.0)
+    _check(_L.fdtd_probe_bandwidth(pattern, nx, ny, nz, tile_y, runs, unroll, blocks, threads, reps, _ptr(vin), _ptr(vout),
+                                   C.byref(out), stream))
+    return out.value
 
 
 def fdtd_halo_export(grid, fields, which, n, side, out, stream) -> None:
