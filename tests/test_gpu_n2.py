@@ -405,3 +405,27 @@ def test_per_component_inv_eps(B, case):
     for c in range(3):
         assert np.max(np.abs(g_r[c])) > 0
     assert relerr(gg, g_r) <= TOL_GRAD and relerr(lam0.cpu().numpy(), lam_r) <= TOL_GRAD
+
+
+def test_bandwidth_probe_touches_every_cell(B):
+    """bench.py --probe: the probe kernels (include/fdtd.h fdtd_probe_bandwidth) must move ALL of the 7 + 6 volumes, or the rate they
+    report is not the rate of the step kernel's bytes: out[c] = in[c] + 0.5 * in[6] * in[(c + 1) % 6] on every cell, for the
+    streaming pattern and for the tile-column traversal with a ragged last tile column, ragged runs and every unroll."""
+    import torch
+    nx, ny, nz = 40, 23, 19
+    vin = torch.rand((7, nz, ny, nx), device="cuda")
+    want = torch.stack([vin[c] + 0.5 * vin[6] * vin[(c + 1) % 6] for c in range(6)])
+    st = torch.cuda.current_stream().cuda_stream
+    for pattern, ty, runs, unroll, blocks, threads in ((0, 0, 1, 1, 7, 64), (0, 0, 3, 1, 300, 256), (1, 7, 5, 1, 0, 96), (1, 7, 4, 2, 0, 384),
+                                                       (1, 5, 19, 4, 0, 64), (1, 30, 1, 2, 0, 512)):
+        vout = torch.full((6, nz, ny, nx), float("nan"), device="cuda")
+        gbs = B.fdtd_probe_bandwidth(pattern, nx, ny, nz, ty, runs, unroll, blocks, threads, 2, vin, vout, st)
+        assert gbs > 0
+        assert torch.allclose(vout, want, rtol=1e-6, atol=1e-7), (pattern, ty, runs, unroll)     # fused multiply-add vs two roundings; NaN = not written
+    for bad in (dict(nx=42), dict(threads=100), dict(pattern=2), dict(pattern=1, unroll=3), dict(pattern=1, runs=nz + 1), dict(pattern=0, blocks=0)):
+        a = dict(pattern=0, nx=nx, ny=ny, nz=nz, tile_y=7, runs=2, unroll=1, blocks=8, threads=128)
+        a.update(bad)
+        with pytest.raises(B.FdtdError) as e:
+            B.fdtd_probe_bandwidth(a["pattern"], a["nx"], a["ny"], a["nz"], a["tile_y"], a["runs"], a["unroll"], a["blocks"], a["threads"], 1, vin,
+                                   torch.empty_like(want), st)
+        assert e.value.code == B.FDTD_EINVAL
