@@ -286,6 +286,82 @@ def run_decomposed(args, rank, world, local_rank, barrier):
     r.close()
 
 
+def run_n4(args):
+    """bench.py --n4: the SURVEY 8(f) N4 variants on C3's grid and recipe, timed like `value` (CUDA events around whole gradient
+    passes, inputs resident): per-component inv_eps, dL/d inv_mu, the checkpointed reverse sweep and a lossy medium.  One JSON line."""
+    import math
+    import numpy as np
+    import torch
+    from paper_2412_12360_b200 import binding as B
+    args.time_steps = args.time_steps or 600
+    w = make_workload(args, 0)
+    T = w.n_steps
+    dev = torch.device("cuda", 0)
+    stream = torch.cuda.Stream()
+    shape = (w.nz, w.ny, w.nx)
+    rng = np.random.default_rng(5)
+    ie = torch.as_tensor(w.inv_eps).to(dev)
+    ie3 = torch.stack([ie * float(a) for a in (1.0, 0.95, 1.05)]).contiguous()
+    im = torch.as_tensor((1.0 / (1.0 + 0.2 * rng.random(shape, dtype=np.float32))).astype(np.float32)).to(dev)
+    sig = torch.as_tensor((0.02 * rng.random(shape, dtype=np.float32)).astype(np.float32)).to(dev)
+    for q in w.sources:
+        q.waveform = torch.as_tensor(q.waveform).to(dev)
+        q.profile = None if q.profile is None else torch.as_tensor(q.profile).to(dev)
+    K = max(1, int(round(math.sqrt(T))))
+    fields = torch.zeros((6,) + shape, dtype=torch.float32, device=dev)
+    phasors = [torch.zeros(dt.phasor_shape, dtype=torch.float32, device=dev) for dt in w.detectors]
+    reps = max(1, min(args.steps, 3))
+    rows = {}
+
+    def case(name, record, flags=0, eps=ie, mu=None, sigma=None, grad_mu=False, ck=0):
+        kw = w.grid_kwargs()
+        kw.update(max_steps=T, record=record, flags=flags, checkpoint_every=ck)
+        g = B.Grid(**kw)
+        if sigma is not None:
+            g.set_conductivity(sigma)
+        gm = torch.empty(shape, dtype=torch.float32, device=dev) if grad_mu else None
+
+        def fwd():
+            fields.zero_()
+            for P in phasors:
+                P.zero_()
+            g.forward(fields, eps, mu, w.sources, w.detectors, T, phasors=phasors)
+
+        def grad():
+            fwd()
+            dLp = [2.0 * P if i in w.loss_detectors else None for i, P in enumerate(phasors)]
+            return g.backward(fields, eps, mu, w.sources, w.detectors, dLp, None, T, grad_mu=gm)[0]
+
+        def timed(fn):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            fn()
+            torch.cuda.synchronize()
+            e0.record(stream)
+            for _ in range(reps):
+                out = fn()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            return e0.elapsed_time(e1) / reps, out
+
+        with torch.cuda.stream(stream):
+            ms_f, _ = timed(fwd)
+            ms_g, gr = timed(grad)
+            info = g.info()
+            rows[name] = {"path": {B.FDTD_PATH_FUSED: "fused", B.FDTD_PATH_GENERIC: "generic"}[info.path],
+                          "forward_Mcells_s": round(w.cells * T / ms_f / 1e3, 1), "forward_us_per_time_step": round(1e3 * ms_f / T, 1),
+                          "gradient_Mcells_s": round(w.cells * T / ms_g / 1e3, 1), "gradient_us_per_time_step": round(1e3 * ms_g / T, 1),
+                          "recorder_GB": round(info.recorder_bytes / 1e9, 2), "max_abs_grad": float(gr.double().abs().max())}
+        g.close()
+
+    case("isotropic, time-reversed (record=1): the contract's path", 1)
+    case("inv_mu volume + dL/d inv_mu (fdtd_backward_mu)", 1, mu=im, grad_mu=True)
+    case("per-component inv_eps (FDTD_FLAG_ANISO_EPS), time-reversed", 1, flags=B.FDTD_FLAG_ANISO_EPS, eps=ie3)
+    case(f"isotropic, checkpointed reverse sweep (record=3, every {K} steps)", 3, ck=K)
+    case(f"lossy medium (fdtd_set_conductivity), checkpointed reverse sweep (record=3, every {K} steps)", 3, sigma=sig, ck=K)
+    print(json.dumps({"n4": "SURVEY 8(f) N4 variants on C3's grid and recipe", "grid": list(shape[::-1]), "time_steps": T,
+                      "passes_timed": reps, "unit": "Mcells/s = cells * time steps / time of forward (or forward + backward)", "rows": rows}))
+
+
 def run_probe(args):
     """bench.py --probe: what the memory system gives for the step kernel's bytes and traversal, without its arithmetic."""
     import torch
@@ -348,6 +424,9 @@ def main():
                     help="1: `value` only (record the PML/interior interface, reconstruct the interior); 2: `value` on the "
                          "design-box recorder instead (labelled); both (default where there is a design box and memory allows): "
                          "`value` on record=1 and the record=2 figure beside it")
+    ap.add_argument("--n4", action="store_true",
+                    help="SURVEY 8(f) N4 variants on C3 (per-component inv_eps, dL/d inv_mu, checkpointed sweep, lossy medium): forward "
+                         "and gradient rates, one JSON line (--time-steps, default 600)")
     ap.add_argument("--probe", action="store_true",
                     help="no FDTD: the bandwidth probes of fdtd_probe_bandwidth (the step kernel's 7 volumes read + 6 written "
                          "without its arithmetic, streaming and in the step kernel's tile-column traversal) on the --grid size "
@@ -381,9 +460,9 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    if args.probe:
+    if args.probe or args.n4:
         if rank == 0:
-            run_probe(args)
+            (run_probe if args.probe else run_n4)(args)
         if world > 1:
             dist.destroy_process_group()
         return
