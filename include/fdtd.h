@@ -58,8 +58,11 @@
  *   On a fused grid a single call still runs on the generic kernels when it passes more than 4 sources or
  *   more than 4 detectors (the fused kernels' parameter block has 4 slots each; under FDTD_PATH_FUSED such a
  *   call fails with EINVAL).  In fdtd_backward, detectors with a cotangent on an H component are injected
- *   by a small kernel per detector and step instead of inside the adjoint step kernel.  inv_mu is taken
- *   by both paths in both directions.  Results of the two paths agree to rounding (different summation order).
+ *   by a small kernel per detector and step instead of inside the adjoint step kernel.  inv_mu, one inv_eps per
+ *   component (FDTD_FLAG_ANISO_EPS) and a conductivity (fdtd_set_conductivity) are taken by both paths in both
+ *   directions: the fused step kernels have a second instance that reads them at a thread's own cells.
+ *   Results of the two paths agree to rounding (different summation order; the fused lossy step forms 1 / (1 + beta)
+ *   with the hardware reciprocal, one unit in the last place).
  *
  * Errors
  *   Every function returns FDTD_OK (0) or a negative code; fdtd_last_error() returns a
@@ -104,7 +107,7 @@ extern "C" {
 
 #define FDTD_FLAG_ANISO_EPS  4       /* SURVEY 8(f) N4, reading R30: inv_eps is [3][nz][ny][nx], one volume per E component (E_c is
                                        updated with inv_eps[c] at its own staggered position: what sub-pixel smoothing of an
-                                       interface produces), and dL_dinv_eps is [3][nz][ny][nx] likewise.  Generic kernels only;
+                                       interface produces), and dL_dinv_eps is [3][nz][ny][nx] likewise.  Both kernel paths;
                                        not with fdtd_grad_rho, the energy detector or the *_host entry points.               */
 
 typedef struct fdtd_grid fdtd_grid;      /* opaque */
@@ -231,8 +234,9 @@ FDTD_API int fdtd_backward_mu(fdtd_grid *grid, float *fields, const float *inv_e
  * removes it).  The E update becomes the semi-implicit lossy Yee update
  *   beta = sigma~ S inv_eps / 2,   E'_c = (1 - beta)/(1 + beta) E_c + 1/(1 + beta) S inv_eps bracket_c .
  * Such a step cannot be inverted stably, so the grid must have record == 0 (forward, adjoint sweep only) or record == 3 (the
- * checkpointed reverse sweep, which then delivers dL_dinv_eps); ESTATE otherwise.  Runs on the generic kernels
- * (FDTD_PATH_FUSED: EINVAL at the call). */
+ * checkpointed reverse sweep, which then delivers dL_dinv_eps); ESTATE otherwise.  Both kernel paths take it (the fused step
+ * kernels read sigma~ at a thread's own cells).  On a fused record == 3 grid the first call that sets a conductivity allocates
+ * three scratch volumes (the adjoint step leaves lamE' there before scaling it by (1 - beta)/(1 + beta)); ENOMEM if that fails. */
 FDTD_API int fdtd_set_conductivity(fdtd_grid *grid, const float *sigma);
 
 /* B6, chain rule to design parameters (once per gradient, not per step): for a design box whose

@@ -179,8 +179,6 @@ extern "C" int fdtd_create_grid(const fdtd_grid_desc *desc, fdtd_grid **out)
     if (desc->path < 0 || desc->path > 2) return fail(FDTD_EINVAL, "unknown path");
     if (desc->reserved[0]) return fail(FDTD_EINVAL, "reserved fields must be zero");
     if (desc->flags & ~(FDTD_FLAG_HOST_STAGING | FDTD_FLAG_RECORDER_FP16 | FDTD_FLAG_ANISO_EPS)) return fail(FDTD_EINVAL, "unknown bit in flags");
-    if ((desc->flags & FDTD_FLAG_ANISO_EPS) && desc->path == FDTD_PATH_FUSED)
-        return fail(FDTD_EINVAL, "FDTD_FLAG_ANISO_EPS runs on the generic kernels (use FDTD_PATH_AUTO or FDTD_PATH_GENERIC)");
     if ((desc->flags & FDTD_FLAG_ANISO_EPS) && (desc->flags & FDTD_FLAG_HOST_STAGING))
         return fail(FDTD_EINVAL, "the host-buffer entry points take one inv_eps volume (no FDTD_FLAG_ANISO_EPS)");
     if (desc->pml_m < 0 || desc->pml_sigma_scale < 0 || desc->pml_kappa_max < 0 || desc->pml_alpha_max < 0 ||
@@ -678,7 +676,7 @@ static int forward_impl(fdtd_grid *g, float *fields, const float *inv_eps, const
     if (n_td) return fail(FDTD_EINVAL, "time-domain detectors are not available on a record = 3 grid");
     if (n_begin != 0 || n_end != n_total) return fail(FDTD_EINVAL, "range calls are not available on a record = 3 grid");
     if (!fields) return fail(FDTD_EINVAL, "fdtd_forward: fields and inv_eps are required");
-    const bool fused = g->path == FDTD_PATH_FUSED && n_src <= FDTD_FUSED_MAX_SRC && n_det <= FDTD_FUSED_MAX_DET && !g->sigma;
+    const bool fused = g->path == FDTD_PATH_FUSED && n_src <= FDTD_FUSED_MAX_SRC && n_det <= FDTD_FUSED_MAX_DET;
     const int K = g->ck_every;
     int rc = FDTD_OK;
     if (n_total == 0) return forward_core(g, fields, inv_eps, inv_mu, src, n_src, det, n_det, nullptr, 0, 0, 0, 0, cuda_stream);
@@ -737,7 +735,7 @@ static int forward_core(fdtd_grid *g, float *fields, const float *inv_eps, const
     // more descriptors than the fused kernels' parameter block holds: this call runs on the generic kernels (same
     // psi slabs, same recorder layout, so a fused or generic fdtd_backward can follow)
     // (a lossy medium, N4, also runs on the generic kernels)
-    const bool fused_call = g->path == FDTD_PATH_FUSED && n_src <= FDTD_FUSED_MAX_SRC && n_det <= FDTD_FUSED_MAX_DET && !g->sigma;
+    const bool fused_call = g->path == FDTD_PATH_FUSED && n_src <= FDTD_FUSED_MAX_SRC && n_det <= FDTD_FUSED_MAX_DET;
     if (g->path == FDTD_PATH_FUSED && !fused_call && g->desc.path == FDTD_PATH_FUSED)
         return fail(FDTD_EINVAL, "FDTD_PATH_FUSED takes at most 4 sources and 4 detectors per call and no conductivity (FDTD_PATH_AUTO falls back to the generic kernels)");
     if (g->sigma && recording) return fail(FDTD_ESTATE, "a lossy medium cannot be time-reversed (PAPER.md L84): use record = 0 or the checkpointed sweep, record = 3");
@@ -854,7 +852,7 @@ static int checkpointed_backward(fdtd_grid *g, float *fields, const float *inv_e
     if (g->recorded_steps != n_total) return fail(FDTD_ESTATE, "fdtd_backward: no matching checkpointed forward (need record=3 and the same n_steps)");
     std::vector<SourceDev> S;
     translate(src, n_src, S);
-    const bool fused_f = g->path == FDTD_PATH_FUSED && n_src <= FDTD_FUSED_MAX_SRC && !g->sigma;      // the replay runs without detectors
+    const bool fused_f = g->path == FDTD_PATH_FUSED && n_src <= FDTD_FUSED_MAX_SRC;      // the replay runs without detectors
     const size_t vol = (size_t)G.nc * sizeof(float);
     CK(cudaMemsetAsync(dL_dinv_eps, 0, (G.aniso ? 3 : 1) * vol, st));
     const int K = g->ck_every;
@@ -874,21 +872,25 @@ static int checkpointed_backward(fdtd_grid *g, float *fields, const float *inv_e
             g->replaying = false;
             if (rc) return rc;
             // the step's first launch read n from counter slot 0, which still holds it
-            if (fused_f) launch_dE_store(G, fields, fused_volume(g, fields, 0, 1), g->dE, K, 0, inv_eps, nullptr, g->d_step, st);
+            if (fused_f) launch_dE_store(G, fields, fused_volume(g, fields, 0, 1), g->dE, K, 0, inv_eps, g->sigma, g->d_step, st);
             else         launch_dE_store(G, fields, nullptr, g->dE, K, 2, inv_eps, g->sigma, g->d_step, st);
             for (const SourceDev &q : S) if (q.comp < 3) launch_dE_source(G, g->dE, K, q, inv_eps, g->sigma, g->d_step, st);
             g->kernel_launches += 2 + (fused_f ? 0 : 2);
         }
         // ---- the segment's adjoint steps, gradient from the stored D (generic path: between its two adjoint kernels)
         for (int n = b - 1; n >= a; --n) {
-            const bool fused_b = g->path == FDTD_PATH_FUSED && g->fused_backward_ready && !g->sigma;
+            const bool fused_b = g->path == FDTD_PATH_FUSED && g->fused_backward_ready && (!g->sigma || g->e2buf);
             g->ck_grad = fused_b ? nullptr : dL_dinv_eps;
+            g->ck_e2 = fused_b && g->sigma ? g->e2buf : nullptr;
             rc = backward_core(g, fields, inv_eps, inv_mu, src, n_src, det, n_det, dL_dphasor, nullptr, 0, nullptr, dL_dfields,
                                n + 1, n, n_total, nullptr, dL_dfields0, st, nullptr, true);
             g->ck_grad = nullptr;
+            float *const e2 = g->ck_e2;
+            g->ck_e2 = nullptr;
             if (rc) return rc;
             if (fused_b) {
-                launch_grad_from_dE(G, g->lam, fused_volume(g, fields, 1, 1), g->dE, K, dL_dinv_eps, g->d_step, st);
+                // lossy: the volume holds lamE = Ca lamE'; the adjoint step left lamE' itself in the scratch volumes
+                launch_grad_from_dE(G, e2 ? e2 : g->lam, e2 ? e2 : fused_volume(g, fields, 1, 1), g->dE, K, dL_dinv_eps, g->d_step, st);
                 g->kernel_launches += 1;
             }
         }
@@ -973,7 +975,7 @@ static int backward_core(fdtd_grid *g, float *fields, const float *inv_eps, cons
     }
     launch_set_step(g->d_step, std::max(n_hi - 1, 0), st);      // the first reverse step of the call reads slot 0
     const bool want_grad = dL_dinv_eps != nullptr;              // false: adjoint sweep only (B1, B2, B5)
-    const bool fused_call = g->path == FDTD_PATH_FUSED && g->fused_backward_ready && !g->sigma;
+    const bool fused_call = g->path == FDTD_PATH_FUSED && g->fused_backward_ready && (!g->sigma || !sweep_only || g->ck_e2);
     if (g->sigma && want_grad) return fail(FDTD_ESTATE, "a lossy medium cannot be time-reversed (PAPER.md L84): its gradient comes from the checkpointed sweep (record = 3)");
 
     if (fused_call) {
@@ -1029,6 +1031,12 @@ extern "C" int fdtd_set_conductivity(fdtd_grid *g, const float *sigma)
     if (!g) return fail(FDTD_EINVAL, "fdtd_set_conductivity: NULL grid");
     if (sigma && (g->desc.record == 1 || g->desc.record == 2))
         return fail(FDTD_ESTATE, "a lossy medium cannot be time-reversed (PAPER.md L84): create the grid with record = 0 or record = 3");
+    // fused record = 3 grid: the lossy adjoint step leaves lamE' (before its scaling by Ca) in three scratch volumes for the
+    // checkpointed sweep's gradient; allocated by the first call that sets a conductivity
+    if (sigma && g->desc.record == 3 && g->path == FDTD_PATH_FUSED && !g->e2buf) {
+        int rc = g->alloc((void **)&g->e2buf, 3 * (size_t)g->G.nc * sizeof(float));
+        if (rc) return rc;
+    }
     g->sigma = sigma;
     return FDTD_OK;
 }

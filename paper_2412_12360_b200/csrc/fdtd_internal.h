@@ -24,7 +24,7 @@ struct Dims {
     // planes; zl / zh = how many of the first / last local planes lie in the global low / high z CPML slab (d / d on
     // an ordinary grid).  CPML tables are stored per local plane; the z-slab psi arrays keep 2 d planes.
     int zoff, nzg, zl, zh;
-    int aniso;        // N4 (reading R30): inv_eps and dL/d inv_eps are [3][nc], one volume per E component (generic kernels only)
+    int aniso;        // N4 (reading R30): inv_eps and dL/d inv_eps are [3][nc], one volume per E component
 };
 
 // slab-compact plane of local plane k in a z-slab psi array ([0, zl) low slab, [2 d - zh, 2 d) high slab), or -1

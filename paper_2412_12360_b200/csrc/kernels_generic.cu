@@ -629,7 +629,7 @@ void launch_inv_H(const Dims &G, float *fields, const float *im, cudaStream_t st
 // g += sum_c lamE'_c D_c.  Lossless: E' = E + S ie bracket + src, so D = (E' - E - src) / ie.  Lossy (reading R29):
 // E' = Ca E + Cb S ie bracket + src, D = dCa E + F (E' - Ca E - src), F = (dCb ie + Cb) / (Cb ie),
 // dCa = -sigma S Cb^2, dCb = -(sigma S / 2) Cb^2.  The slot of step n in the buffer is n % K (K = steps per segment).
-// mode 0: state n in volume n&1 of (A, B), state n+1 in the other (the fused ping-pong; lossless only);
+// mode 0: state n in volume n&1 of (A, B), state n+1 in the other (the fused ping-pong);
 // mode 1: before an in-place step, the slot takes E;  mode 2: after it, the slot becomes D.
 __global__ void k_dE_store(Dims G, const float *__restrict__ A, const float *__restrict__ B, float *__restrict__ dE, int K, int mode,
                            const float *__restrict__ ie, const float *__restrict__ sigma, const int *__restrict__ step)
@@ -648,7 +648,8 @@ __global__ void k_dE_store(Dims G, const float *__restrict__ A, const float *__r
             const float hs = sigma ? 0.5f * __ldg(sigma + p) * G.S : 0.f, Cb = 1.f / (1.f + hs * e), Ca = (1.f - hs * e) * Cb;
             const float dCa = -2.f * hs * Cb * Cb, F = (-hs * Cb * Cb * e + Cb) / (Cb * e);
             float *o = dE + c * bc + t;
-            if (mode == 0) *o = (En1[c * G.nc + p] - En[c * G.nc + p]) / e;
+            if (mode == 0 && !sigma) *o = (En1[c * G.nc + p] - En[c * G.nc + p]) / e;
+            else if (mode == 0) { const float E0 = En[c * G.nc + p]; *o = fmaf(dCa, E0, F * (En1[c * G.nc + p] - Ca * E0)); }
             else if (mode == 1) *o = En[c * G.nc + p];
             else { const float E0 = *o; *o = fmaf(dCa, E0, F * (En[c * G.nc + p] - Ca * E0)); }
         }

@@ -1,7 +1,8 @@
 // kernels_step.cu -- fused z-marching step kernels of the hot path (DESIGN.md sections 7-8):
 //
-//   k_step<C, false>  forward step : E update + H update + CPML psi + sources + detectors   (F1-F7)
-//   k_step<C, true>   adjoint step : transpose of the H update, then of the E update, adjoint CPML (B2+B5)
+//   k_step<C, false, N4>  forward step : E update + H update + CPML psi + sources + detectors   (F1-F7)
+//   k_step<C, true, N4>   adjoint step : transpose of the H update, then of the E update, adjoint CPML (B2+B5)
+//   (N4 = true: the instance with the operands beyond the contract's path -- inv_mu, three inv_eps volumes, a conductivity)
 //
 // PAPER.md: Eq. 1-2 (L64-66) for the curl updates, L72 for the CPML, L78-84 for the VJP.
 //
@@ -61,6 +62,8 @@ struct StepParams {
     int n_rot, seg_stride, n_cta;
     float *buf[2];                 // ping-pong volumes, [6][nc] each
     const float *ie, *im;
+    const float *sigma;            // N4 (reading R29): normalised conductivity volume or NULL.  With G.aniso (R30) `ie` is [3][nc]
+    float *e2_out;                 // lossy adjoint step in the checkpointed sweep: lamE' before its scaling by Ca, [3][nc], or NULL
     PsiSet psiE[2], psiH[2];       // CPML states of the E-type / H-type update, ping-pong
     const int *step;               // the slot of the two-slot step counter this step reads
     int *step_next;                // the other slot: block 0 writes n + step_delta for the next step (or NULL)
@@ -121,6 +124,9 @@ __device__ __forceinline__ void sts4(uint32_t addr, float4 v)
 __device__ __forceinline__ float4 ldg4(const float *p) { return __ldg(reinterpret_cast<const float4 *>(p)); }
 __device__ __forceinline__ float4 ld4(const float *p) { return *reinterpret_cast<const float4 *>(p); }
 __device__ __forceinline__ void stg4(float *p, float4 v) { *reinterpret_cast<float4 *>(p) = v; }
+// 1 / a to one unit in the last place (MUFU.RCP; the IEEE division's slow-path calls cost the step kernel its registers)
+__device__ __forceinline__ float rcp1(float a) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r; }
+__device__ __forceinline__ float4 rcp4(float4 a) { return make_float4(rcp1(a.x), rcp1(a.y), rcp1(a.z), rcp1(a.w)); }
 __device__ __forceinline__ float4 fma4(float4 a, float4 b, float4 c)
 {
     return make_float4(fmaf(a.x, b.x, c.x), fmaf(a.y, b.y, c.y), fmaf(a.z, b.z, c.z), fmaf(a.w, b.w, c.w));
@@ -291,11 +297,14 @@ __device__ __forceinline__ void pf_l2(const float *p)
     asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
 #endif
 }
+__device__ __forceinline__ void pf_l1(const float *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 #ifndef FDTD_PF_DIST
 #define FDTD_PF_DIST 1
 #endif
 
-template <class C, bool ADJ>
+// N4 = true: the instance that takes the operands beyond the contract's path, read by LDG at a thread's own cells: an inv_mu
+// volume (P.im), three inv_eps volumes (G.aniso), a conductivity (P.sigma).  The contract's path runs N4 = false.
+template <class C, bool ADJ, bool N4>
 __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ StepParams P)
 {
     extern __shared__ __align__(1024) uint8_t smem[];
@@ -401,7 +410,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
     const long long nc = G.nc;
     const int plane = G.ny * G.nx;
     const bool pml = G.d > 0 && !DBG(16);
-    const bool has_mu = P.im != nullptr;
+    const bool has_mu = N4 && P.im != nullptr;      // (the N4 = false instance is launched without inv_mu)
     const int pz = plane, py = 2 * G.d * G.nx, px = G.ny * 2 * G.dpx;      // plane pitch of the z / y / x state arrays
 
     const float4 Z4 = splat(0.f);
@@ -434,6 +443,12 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
         // ---------------------------------------------------------------- one plane (phase A of kk, phase B of kk-1)
         auto plane_step = [&](const int kk, const bool doB) {
             const int zs = (pml && !DBG(128)) ? zslab_pos(G, kk) : -1;
+            if (N4 && ing && kk < G.nz) {      // the operands that come by LDG at my cells: on their way while the stage lands
+                const float *q = P.ie + (kk * (G.ny * G.nx) + own_xy);
+                if (G.aniso) { pf_l1(q + G.nc); pf_l1(q + 2 * G.nc); }
+                if (P.sigma) pf_l1(P.sigma + (kk * (G.ny * G.nx) + own_xy));
+            }
+            if (has_mu && own_ok && doB) pf_l1(P.im + ((kk - 1) * (G.ny * G.nx) + own_xy));     // phase B's inv_mu, likewise
             mbar_wait(&full[st_i], st_ph);
             const uint32_t so = stage_base + st_off + o_own;
             if (ADJ && kk >= P.dEl && kk < P.dEh && !dup) {
@@ -553,12 +568,29 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
             const float4 tEx = Dy_z - Dz_y, tEy = Dz_x - Dx_z, tEz = Dx_y - Dy_x;
             const float4 ex = lds4(so + 3 * C::SLOT), ey = lds4(so + 4 * C::SLOT), ez = lds4(so + 5 * C::SLOT);
             const float4 sie = S * lds4(so + 6 * C::SLOT);
+            // N4: one inv_eps volume per component (R30: the stage holds component x, y and z come by LDG at my cells) and / or
+            // a conductivity (R29: E' = Ca E + Cb S ie bracket, beta = sigma S ie / 2, Ca = (1 - beta) / (1 + beta), Cb = 1 / (1 + beta))
+            const bool n4 = N4 && (G.aniso || P.sigma != nullptr);
+            float4 siy = sie, siz = sie, six = sie, cax = splat(1.f), cay = cax, caz = cax;
+            if (n4) {
+                const bool ld_ok = ing && kin;
+                if (G.aniso && ld_ok) { siy = S * ldg4(P.ie + nc + off); siz = S * ldg4(P.ie + 2 * nc + off); }
+                if (N4 && P.sigma) {
+                    const float4 hs = ld_ok ? 0.5f * ldg4(P.sigma + off) : Z4;
+                    const float4 bx = hs * six, by = hs * siy, bz = hs * siz;
+                    const float4 cbx = rcp4(splat(1.f) + bx), cby = rcp4(splat(1.f) + by), cbz = rcp4(splat(1.f) + bz);
+                    cax = (splat(1.f) - bx) * cbx; cay = (splat(1.f) - by) * cby; caz = (splat(1.f) - bz) * cbz;
+                    six = six * cbx; siy = siy * cby; siz = siz * cbz;
+                }
+            }
             float4 e2x, e2y, e2z, v2x, v2y, v2z;
             if (ADJ) {
                 e2x = fma4(-S, tEx, ex); e2y = fma4(-S, tEy, ey); e2z = fma4(-S, tEz, ez);
-                v2x = sie * e2x; v2y = sie * e2y; v2z = sie * e2z;
+                if (n4) { v2x = six * e2x; v2y = siy * e2y; v2z = siz * e2z; }
+                else { v2x = sie * e2x; v2y = sie * e2y; v2z = sie * e2z; }
             } else {
-                e2x = fma4(sie, tEx, ex); e2y = fma4(sie, tEy, ey); e2z = fma4(sie, tEz, ez);
+                if (n4) { e2x = fma4(cax, ex, six * tEx); e2y = fma4(cay, ey, siy * tEy); e2z = fma4(caz, ez, siz * tEz); }
+                else { e2x = fma4(sie, tEx, ex); e2y = fma4(sie, tEy, ey); e2z = fma4(sie, tEz, ez); }
                 if (kk >= P.sEl && kk < P.sEh) {
                     const int sm = src_mask(P, kk);
                     if (sm & 1) e2x = add_sources4(P, n, 0, e2x, i, j, kk);
@@ -569,7 +601,12 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
             }
             if (wr) {
                 float *o = dst + off;
-                stg4(o, e2x); stg4(o + nc, e2y); stg4(o + 2 * nc, e2z);
+                if (ADJ && N4 && P.sigma) {    // lamE of the earlier step is Ca lamE'; the checkpointed sweep's gradient wants lamE' itself
+                    if (P.e2_out) { float *q = P.e2_out + off; stg4(q, e2x); stg4(q + nc, e2y); stg4(q + 2 * nc, e2z); }
+                    stg4(o, cax * e2x); stg4(o + nc, cay * e2y); stg4(o + 2 * nc, caz * e2z);
+                } else {
+                    stg4(o, e2x); stg4(o + nc, e2y); stg4(o + 2 * nc, e2z);
+                }
                 if (!ADJ && kk >= P.dEl && kk < P.dEh) detect4(P, n, 0, det_mask(P, kk, false), e2x, e2y, e2z, i, j, kk);
             }
             float4 Yx = v2x, Yz = v2z, Xy = v2y, Xz = v2z, Zx = v2x, Zy = v2y;
@@ -735,8 +772,9 @@ struct InvParams {
     const Segment *segs;
     const int *seg_begin;          // [n_cta + 1]
     float *buf[2];                 // primal ping-pong volumes
-    float *grad;                   // dL/d inv_eps, accumulated
+    float *grad;                   // dL/d inv_eps, accumulated ([3][nc] with G.aniso)
     const float *im;               // inv_mu or NULL (= 1)
+    const float *ie;               // inv_eps (G.aniso: [3][nc]; components y, z come by LDG at my cells)
     const int *step;
     int bias, n_steps;             // this launch inverts step n = *step + bias; nothing to do if n >= n_steps (see enqueue_bwd)
     int nst, stage;
@@ -873,7 +911,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_inverse(const __grid_constant
                 const int off = kk * plane + own_xy;
                 float4 gv = splat(0.f);
                 const bool gz = kk >= G.glo[2] && kk < G.ghi[2];
-                if (own_ok && gz && gall) gv = ld4(P.grad + off);
+                if (own_ok && gz && gall && !G.aniso) gv = ld4(P.grad + off);
                 named_bar_sync(1, C::NCW * 32);
                 // ------------------------------------------------------------ q, gradient, E of plane kk
                 if (own_ok) {
@@ -885,7 +923,9 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_inverse(const __grid_constant
                     const float4 qx = By_z - Bz_y, qy = Bz_x - Bx_z, qz = Bx_y - By_x;
                     const float4 sie = S * lds4(sC);
                     const float4 lx = lds4(sC + C::SLOTC), ly = lds4(sC + 2 * C::SLOTC), lz = lds4(sC + 3 * C::SLOTC);
-                    float4 E2x = Ex - sie * qx, E2y = Ey - sie * qy, E2z = Ez - sie * qz;
+                    float4 siy = sie, siz = sie;
+                    if (G.aniso) { siy = S * ldg4(P.ie + nc + off); siz = S * ldg4(P.ie + 2 * nc + off); }
+                    float4 E2x = Ex - sie * qx, E2y = Ey - siy * qy, E2z = Ez - siz * qz;
                     if (kk >= P.sEl && kk < P.sEh) {
                         const int sm = src_mask(P, kk);
                         if (sm & 1) E2x = E2x - add_sources4(P, n, 0, splat(0.f), i, j, kk);
@@ -899,7 +939,19 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_inverse(const __grid_constant
                     st_masked(o + 3 * nc, Hx, mall, m0, m1, m2, m3);
                     st_masked(o + 4 * nc, Hy, mall, m0, m1, m2, m3);
                     st_masked(o + 5 * nc, Hz, mall, m0, m1, m2, m3);
-                    if (gz && gany) {
+                    if (gz && gany && G.aniso) {               // reading R30: one gradient volume per component
+                        const float4 gc[3] = { S * (lx * qx), S * (ly * qy), S * (lz * qz) };
+                        for (int c = 0; c < 3; ++c) {
+                            float *gp = P.grad + c * nc + off;
+                            if (gall) stg4(gp, ld4(gp) + gc[c]);
+                            else {
+                                if (g0) gp[0] += gc[c].x;
+                                if (g1) gp[1] += gc[c].y;
+                                if (g2) gp[2] += gc[c].z;
+                                if (g3) gp[3] += gc[c].w;
+                            }
+                        }
+                    } else if (gz && gany) {
                         const float4 ga = S * fma4(lx, qx, fma4(ly, qy, lz * qz));
                         if (gall) stg4(P.grad + off, gv + ga);
                         else {
@@ -986,17 +1038,24 @@ template <class C, bool ADJ> void launch_step_impl(const StepParams &P, int n_ct
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
-    cudaLaunchKernelEx(&cfg, k_step<C, ADJ>, P);
+    if (P.G.aniso || P.sigma || P.im) cudaLaunchKernelEx(&cfg, k_step<C, ADJ, true>, P);
+    else cudaLaunchKernelEx(&cfg, k_step<C, ADJ, false>, P);
 }
 template <class C> void launch_fwd_impl(const StepParams &P, int n_cta, size_t smem, cudaStream_t st) { launch_step_impl<C, false>(P, n_cta, smem, st); }
 template <class C> void launch_adj_impl(const StepParams &P, int n_cta, size_t smem, cudaStream_t st) { launch_step_impl<C, true>(P, n_cta, smem, st); }
+template <class K> cudaError_t set_smem_kernel(K kernel, size_t smem)
+{
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    // the same shared-memory carve-out for every kernel of the time loop: no L1 / shared reconfiguration between launches
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    return e;
+}
 template <class C> cudaError_t set_smem_impl(size_t smem)
 {
-    cudaError_t e = cudaFuncSetAttribute(k_step<C, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step<C, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    // the same shared-memory carve-out for every kernel of the time loop: no L1 / shared reconfiguration between launches
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step<C, false>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step<C, true>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    cudaError_t e = set_smem_kernel(k_step<C, false, false>, smem);
+    if (e == cudaSuccess) e = set_smem_kernel(k_step<C, true, false>, smem);
+    if (e == cudaSuccess) e = set_smem_kernel(k_step<C, false, true>, smem);
+    if (e == cudaSuccess) e = set_smem_kernel(k_step<C, true, true>, smem);
     return e;
 }
 #define TILE(TX4, TY) { 4 * TX4, TY, Cfg<TX4, TY>::THREADS, Cfg<TX4, TY>::NCW, Cfg<TX4, TY>::STAGE, Cfg<TX4, TY>::RING_BYTES, \
@@ -1320,7 +1379,6 @@ int fused_setup(fdtd_grid *g)
     const Dims &G = g->G;
     if (g->desc.path == FDTD_PATH_GENERIC) { g->fused_why_not = "generic path requested"; return FDTD_OK; }
     if (G.periodic) { g->fused_why_not = "periodic grids use the generic kernels"; return FDTD_OK; }
-    if (G.aniso) { g->fused_why_not = "per-component inv_eps (FDTD_FLAG_ANISO_EPS) uses the generic kernels"; return FDTD_OK; }
     if (G.nx % 4) { g->fused_why_not = "nx is not a multiple of 4"; return FDTD_OK; }
     if (G.d > 0 && (G.dpx % 4)) { g->fused_why_not = "x-slab psi storage is not float4 aligned (nx < 2*roundup4(d))"; return FDTD_OK; }
     if (G.nc >= (1LL << 31) - 4LL * G.nx * G.ny) { g->fused_why_not = "more than 2^31 cells (32-bit plane offsets)"; return FDTD_OK; }
@@ -1631,13 +1689,13 @@ static int calibrate(fdtd_grid *g)
     const Dims &G = g->G;
     const size_t vol = (size_t)G.nc * sizeof(float);
     float *T = nullptr, *tie = nullptr;
-    if (cudaMalloc((void **)&T, 6 * vol) != cudaSuccess || cudaMalloc((void **)&tie, vol) != cudaSuccess) {
+    if (cudaMalloc((void **)&T, 6 * vol) != cudaSuccess || cudaMalloc((void **)&tie, (G.aniso ? 3 : 1) * vol) != cudaSuccess) {
         (void)cudaGetLastError();
         if (T) cudaFree(T);
         return FDTD_OK;                                   // no room for the scratch volumes: keep the model's cuts
     }
     auto done = [&](int rc) { cudaFree(T); cudaFree(tie); F->maps_key[0][0] = nullptr; return rc; };
-    cudaMemset(T, 0, 6 * vol); cudaMemset(F->bufB, 0, 6 * vol); cudaMemset(tie, 0, vol);
+    cudaMemset(T, 0, 6 * vol); cudaMemset(F->bufB, 0, 6 * vol); cudaMemset(tie, 0, (G.aniso ? 3 : 1) * vol);
     cudaMemset(g->d_step, 0, sizeof(int));
     int rc;
     for (int q = 0; q < 2; ++q)
@@ -1875,7 +1933,7 @@ int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float
     StepParams &P = ctx.P;
     P.maps = F->d_maps[0];
     P.buf[0] = fields; P.buf[1] = F->bufB;
-    P.ie = inv_eps; P.im = inv_mu;
+    P.ie = inv_eps; P.im = inv_mu; P.sigma = g->sigma; P.e2_out = nullptr;
     for (int q = 0; q < 2; ++q) { P.psiE[q] = g->psiE[q]; P.psiH[q] = g->psiH[q]; }
     P.n_src = (int)S.size(); P.n_det = (int)D.size(); P.total_freq = total_freq;
     for (size_t q = 0; q < S.size(); ++q) P.src[q] = S[q];
@@ -1952,7 +2010,7 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
         }
         InvParams &I = ctx.I;
         I.maps = F->d_maps[2];
-        I.buf[0] = fields; I.buf[1] = F->bufB; I.grad = dL_dinv_eps; I.im = inv_mu;
+        I.buf[0] = fields; I.buf[1] = F->bufB; I.grad = dL_dinv_eps; I.im = inv_mu; I.ie = inv_eps;
         I.n_src = (int)S.size();
         I.sEl = I.sHl = 1 << 30; I.sEh = I.sHh = -1;
         for (size_t q = 0; q < S.size(); ++q) {
@@ -1966,7 +2024,7 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     P.maps = F->d_maps[1];
     P.segs = F->d_segs[1]; P.seg_begin = F->d_seg_begin[1];
     P.buf[0] = g->lam; P.buf[1] = F->lamB;
-    P.ie = inv_eps; P.im = inv_mu;
+    P.ie = inv_eps; P.im = inv_mu; P.sigma = g->sigma; P.e2_out = g->sigma ? g->ck_e2 : nullptr;
     for (int q = 0; q < 2; ++q) { P.psiE[q] = g->lpsiE[q]; P.psiH[q] = g->lpsiH[q]; }
     P.n_src = 0; P.n_det = 0; P.total_freq = total_freq;
     P.sEl = P.sHl = P.dEl = P.dHl = 1 << 30; P.sEh = P.sHh = P.dEh = P.dHh = -1;

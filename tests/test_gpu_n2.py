@@ -299,19 +299,23 @@ def test_checkpointed_reverse_sweep(B, case):
     assert relerr(lam0.cpu().numpy(), lam_tape) <= TOL_GRAD
 
 
-@pytest.mark.parametrize("case", ["tiny", "mini"])
+@pytest.mark.parametrize("case", ["tiny", "mini-generic", "mini-fused", "mini-fused-mu"])
 def test_lossy_medium_forward_and_checkpointed_gradient(B, case):
     """SURVEY 8(f) N4, reading R29: a random conductivity volume.  Forward fields and phasors against the oracle's lossy
     update; the gradient from the checkpointed sweep (record=3; the only route: a lossy step cannot be time-reversed) and the
-    cotangent of state 0 against the oracle's tape mode, PML cells included.  On a grid that qualifies for the fused kernels
-    the calls fall back to the generic ones."""
+    cotangent of state 0 against the oracle's tape mode, PML cells included.  Both kernel paths (the fused step kernels read
+    the conductivity at a thread's own cells; the fused adjoint step leaves lamE' before its scaling by Ca in scratch volumes)."""
     import torch
     from oracle.oracle import Oracle
+    path = B.FDTD_PATH_FUSED if "fused" in case else B.FDTD_PATH_GENERIC
     if case == "tiny":
         w = wl.tiny_pml(n_steps=30)
     else:
         w = wl.c3_mini(n_steps=70, kappa_max=3.0, alpha_max=0.05)
-        w.meta["inv_mu"] = None
+        if not case.endswith("mu"):
+            w.meta["inv_mu"] = None
+        else:
+            w.meta["inv_mu"] = (1.0 / (1.0 + 0.5 * np.random.default_rng(8).random((w.nz, w.ny, w.nx), dtype=np.float32))).astype(np.float32)
     shape = (w.nz, w.ny, w.nx)
     sig = (0.25 * np.random.default_rng(12).random(shape, dtype=np.float32)).astype(np.float32)
     im = w.meta["inv_mu"]
@@ -327,8 +331,9 @@ def test_lossy_medium_forward_and_checkpointed_gradient(B, case):
     o0.forward(f0, w.inv_eps, im, w.sources, w.detectors, w.n_steps)
     assert relerr(fr[:3], f0[:3]) > 1e-2                      # the loss does change the fields
     kw = w.grid_kwargs()
-    kw.update(max_steps=w.n_steps, record=3, checkpoint_every=9)
+    kw.update(max_steps=w.n_steps, record=3, checkpoint_every=9, path=path)
     g = B.Grid(**kw)
+    assert g.info().path == path
     g.set_conductivity(sig)
     f = torch.zeros((6,) + shape, device="cuda")
     ie = torch.as_tensor(w.inv_eps).cuda()
@@ -343,7 +348,10 @@ def test_lossy_medium_forward_and_checkpointed_gradient(B, case):
     dLf[:3] = 0.5 * f[:3]
     grad, lam0 = g.backward(f, ie, imt, w.sources, w.detectors, [2.0 * P for P in ph], dLf, w.n_steps, want_dL_dfields0=True)
     torch.cuda.synchronize()
+    info = g.info()
     g.close()
+    # forward + replayed forward + adjoint sweep, each w.n_steps launches of the fused step kernel
+    assert info.fused_step_launches == (3 * w.n_steps if path == B.FDTD_PATH_FUSED else 0)
     assert relerr(grad.cpu().numpy(), g_tape) <= TOL_GRAD and relerr(lam0.cpu().numpy(), lam_tape) <= TOL_GRAD
     # a recording grid refuses a lossy medium
     g1 = B.Grid(**{**w.grid_kwargs(), "max_steps": 4, "record": 1})
@@ -353,7 +361,8 @@ def test_lossy_medium_forward_and_checkpointed_gradient(B, case):
     g1.close()
 
 
-@pytest.mark.parametrize("case", ["tiny-reversible", "mini-reversible", "mini-checkpointed-lossy"])
+@pytest.mark.parametrize("case", ["tiny-reversible", "mini-reversible", "mini-checkpointed-lossy", "mini-fused-reversible",
+                                  "mini-fused-checkpointed-lossy", "mini-fused-reversible-box"])
 def test_per_component_inv_eps(B, case):
     """SURVEY 8(f) N4, reading R30 (FDTD_FLAG_ANISO_EPS): three inv_eps volumes, three gradient volumes.  Fields, phasors and the
     time-reversed gradient against the oracle; with a conductivity, the checkpointed gradient against the oracle's tape mode."""
@@ -381,9 +390,12 @@ def test_per_component_inv_eps(B, case):
     else:
         g_r, lam_r = o.backward(fr, ie3, im, w.sources, w.detectors, dLp_r, dLf_r, w.n_steps, out["rec"])
     kw = w.grid_kwargs()
-    kw.update(max_steps=w.n_steps, record=3 if lossy else 1, flags=B.FDTD_FLAG_ANISO_EPS)
+    path = B.FDTD_PATH_FUSED if "fused" in case else B.FDTD_PATH_GENERIC
+    kw.update(max_steps=w.n_steps, record=3 if lossy else 1, flags=B.FDTD_FLAG_ANISO_EPS, path=path)
+    if case.endswith("box"):            # the design-box recorder (record=2): the fused inverse step masks the box edges
+        kw.update(record=2, grad_lo=w.design_lo, grad_hi=w.design_hi)
     g = B.Grid(**kw)
-    assert g.info().path == B.FDTD_PATH_GENERIC
+    assert g.info().path == path
     if lossy:
         g.set_conductivity(sig)
     f = torch.zeros((6,) + shape, device="cuda")
@@ -399,12 +411,25 @@ def test_per_component_inv_eps(B, case):
     dLf[:3] = 0.5 * f[:3]
     grad, lam0 = g.backward(f, ie, imt, w.sources, w.detectors, [2.0 * P for P in ph], dLf, w.n_steps, want_dL_dfields0=True)
     torch.cuda.synchronize()
+    info = g.info()
     g.close()
+    if path == B.FDTD_PATH_FUSED:
+        assert info.fused_step_launches == (3 if lossy else 2) * w.n_steps
+        assert info.fused_inverse_launches == (0 if lossy else w.n_steps)
+    else:
+        assert info.fused_step_launches == 0
     assert tuple(grad.shape) == (3,) + shape
     gg = grad.cpu().numpy()
     for c in range(3):
         assert np.max(np.abs(g_r[c])) > 0
-    assert relerr(gg, g_r) <= TOL_GRAD and relerr(lam0.cpu().numpy(), lam_r) <= TOL_GRAD
+    if case.endswith("box"):
+        lo, hi = w.design_lo, w.design_hi
+        box = (slice(None), slice(lo[2], hi[2]), slice(lo[1], hi[1]), slice(lo[0], hi[0]))
+        assert np.max(np.abs(g_r[box])) > 0
+        assert relerr(gg[box], g_r[box]) <= TOL_GRAD
+    else:
+        assert relerr(gg, g_r) <= TOL_GRAD
+    assert relerr(lam0.cpu().numpy(), lam_r) <= TOL_GRAD
 
 
 def test_bandwidth_probe_touches_every_cell(B):
