@@ -315,7 +315,7 @@ def run_n4(args):
 
     def case(name, record, flags=0, eps=ie, mu=None, sigma=None, grad_mu=False, ck=0):
         kw = w.grid_kwargs()
-        kw.update(max_steps=T, record=record, flags=flags, checkpoint_every=ck)
+        kw.update(max_steps=T, record=record, flags=flags, checkpoint_every=ck, grad_lo=w.design_lo, grad_hi=w.design_hi)   # gradient on the design region, as `value`
         g = B.Grid(**kw)
         if sigma is not None:
             g.set_conductivity(sigma)

@@ -210,8 +210,8 @@ FDTD_API int fdtd_backward(fdtd_grid *grid, float *fields, const float *inv_eps,
  * inv_mu at its own cell), dL_dinv_mu[p] = sum_n sum_c lamH'_c[p] * (-S (curl+ E')_c[p]) with lamH' the cotangent of
  * the post-step H.  DEVICE [nz][ny][nx], OUT, zero-filled by the library, non-zero only on the reconstruction box
  * (like dL_dinv_eps it needs the reconstructed fields, so dL_dinv_eps must be requested too).  NULL: fdtd_backward.
- * On the fused path the inverse step then runs on the generic kernels (the adjoint step stays fused).
- * Not built (N4 remainder): one inv_eps volume per E component, lossy / dispersive media with a checkpointed reverse sweep. */
+ * On the fused path the fused inverse step forms it (lamH' read at a thread's own cells); the inverse step of step n then has to
+ * run before adjoint step n-1, so the two are launched one after the other instead of side by side. */
 FDTD_API int fdtd_backward_mu(fdtd_grid *grid, float *fields, const float *inv_eps, const float *inv_mu,
                      const fdtd_source *src, int32_t n_src, const fdtd_detector *det, int32_t n_det,
                      const float *const *dL_dphasor, const float *dL_dfields,

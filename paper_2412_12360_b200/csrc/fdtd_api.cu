@@ -734,10 +734,9 @@ static int forward_core(fdtd_grid *g, float *fields, const float *inv_eps, const
 
     // more descriptors than the fused kernels' parameter block holds: this call runs on the generic kernels (same
     // psi slabs, same recorder layout, so a fused or generic fdtd_backward can follow)
-    // (a lossy medium, N4, also runs on the generic kernels)
     const bool fused_call = g->path == FDTD_PATH_FUSED && n_src <= FDTD_FUSED_MAX_SRC && n_det <= FDTD_FUSED_MAX_DET;
     if (g->path == FDTD_PATH_FUSED && !fused_call && g->desc.path == FDTD_PATH_FUSED)
-        return fail(FDTD_EINVAL, "FDTD_PATH_FUSED takes at most 4 sources and 4 detectors per call and no conductivity (FDTD_PATH_AUTO falls back to the generic kernels)");
+        return fail(FDTD_EINVAL, "FDTD_PATH_FUSED takes at most 4 sources and 4 detectors per call (FDTD_PATH_AUTO falls back to the generic kernels)");
     if (g->sigma && recording) return fail(FDTD_ESTATE, "a lossy medium cannot be time-reversed (PAPER.md L84): use record = 0 or the checkpointed sweep, record = 3");
     if (fused_call) {
         rc = fused_forward(g, fields, inv_eps, inv_mu, S, D, TD, total_freq, n_begin, n_end, n_total, recording, st);
@@ -857,41 +856,49 @@ static int checkpointed_backward(fdtd_grid *g, float *fields, const float *inv_e
     CK(cudaMemsetAsync(dL_dinv_eps, 0, (G.aniso ? 3 : 1) * vol, st));
     const int K = g->ck_every;
     int rc = FDTD_OK;
+    const bool fused_b = g->path == FDTD_PATH_FUSED && g->fused_backward_ready && (!g->sigma || g->e2buf);
     for (int a = (n_total - 1) / K * K; a >= 0 && n_total > 0; a -= K) {
         const int b = std::min(n_total, a + K);
         // ---- the segment's forward steps again, from its checkpoint
         if (a > 0) { if ((rc = copy_checkpoint(g, fields, fused_f, a, a / K, true, st))) return rc; }
         else CK(cudaMemcpyAsync(fields, g->ckpt, 6 * vol, cudaMemcpyDeviceToDevice, st));
-        for (int n = a; n < b; ++n) {
-            if (!fused_f) {                                   // in-place step: E before it (the counter slot the step will read)
+        if (fused_f) {
+            // one call for the segment: the D store runs after every step inside the replayed graph (enqueue_fwd)
+            g->replaying = true; g->ck_store = true;
+            rc = forward_core(g, fields, inv_eps, inv_mu, src, n_src, nullptr, 0, nullptr, 0, a, b, n_total, st);
+            g->replaying = false; g->ck_store = false;
+            if (rc) return rc;
+        } else {
+            for (int n = a; n < b; ++n) {
+                // in-place step: E before it (the counter slot the step will read), D after it
                 launch_set_step(g->d_step, n, st);
                 launch_dE_store(G, fields, nullptr, g->dE, K, 1, inv_eps, g->sigma, g->d_step, st);
+                g->replaying = true;
+                rc = forward_core(g, fields, inv_eps, inv_mu, src, n_src, nullptr, 0, nullptr, 0, n, n + 1, n_total, st);
+                g->replaying = false;
+                if (rc) return rc;
+                // the step's first launch read n from counter slot 0, which still holds it
+                launch_dE_store(G, fields, nullptr, g->dE, K, 2, inv_eps, g->sigma, g->d_step, st);
+                for (const SourceDev &q : S) if (q.comp < 3) launch_dE_source(G, g->dE, K, q, inv_eps, g->sigma, g->d_step, st);
+                g->kernel_launches += 4;
             }
-            g->replaying = true;
-            rc = forward_core(g, fields, inv_eps, inv_mu, src, n_src, nullptr, 0, nullptr, 0, n, n + 1, n_total, st);
-            g->replaying = false;
-            if (rc) return rc;
-            // the step's first launch read n from counter slot 0, which still holds it
-            if (fused_f) launch_dE_store(G, fields, fused_volume(g, fields, 0, 1), g->dE, K, 0, inv_eps, g->sigma, g->d_step, st);
-            else         launch_dE_store(G, fields, nullptr, g->dE, K, 2, inv_eps, g->sigma, g->d_step, st);
-            for (const SourceDev &q : S) if (q.comp < 3) launch_dE_source(G, g->dE, K, q, inv_eps, g->sigma, g->d_step, st);
-            g->kernel_launches += 2 + (fused_f ? 0 : 2);
         }
-        // ---- the segment's adjoint steps, gradient from the stored D (generic path: between its two adjoint kernels)
-        for (int n = b - 1; n >= a; --n) {
-            const bool fused_b = g->path == FDTD_PATH_FUSED && g->fused_backward_ready && (!g->sigma || g->e2buf);
-            g->ck_grad = fused_b ? nullptr : dL_dinv_eps;
-            g->ck_e2 = fused_b && g->sigma ? g->e2buf : nullptr;
+        // ---- the segment's adjoint steps, gradient from the stored D
+        if (fused_b) {
+            // one call for the segment: g += lamE' . D runs after every adjoint step inside the replayed graph (enqueue_bwd)
+            g->ck_gradhook = dL_dinv_eps;
+            g->ck_e2 = g->sigma ? g->e2buf : nullptr;
             rc = backward_core(g, fields, inv_eps, inv_mu, src, n_src, det, n_det, dL_dphasor, nullptr, 0, nullptr, dL_dfields,
-                               n + 1, n, n_total, nullptr, dL_dfields0, st, nullptr, true);
-            g->ck_grad = nullptr;
-            float *const e2 = g->ck_e2;
-            g->ck_e2 = nullptr;
+                               b, a, n_total, nullptr, dL_dfields0, st, nullptr, true);
+            g->ck_gradhook = nullptr; g->ck_e2 = nullptr;
             if (rc) return rc;
-            if (fused_b) {
-                // lossy: the volume holds lamE = Ca lamE'; the adjoint step left lamE' itself in the scratch volumes
-                launch_grad_from_dE(G, e2 ? e2 : g->lam, e2 ? e2 : fused_volume(g, fields, 1, 1), g->dE, K, dL_dinv_eps, g->d_step, st);
-                g->kernel_launches += 1;
+        } else {
+            for (int n = b - 1; n >= a; --n) {       // generic path: the gradient kernel sits between its two adjoint kernels
+                g->ck_grad = dL_dinv_eps;
+                rc = backward_core(g, fields, inv_eps, inv_mu, src, n_src, det, n_det, dL_dphasor, nullptr, 0, nullptr, dL_dfields,
+                                   n + 1, n, n_total, nullptr, dL_dfields0, st, nullptr, true);
+                g->ck_grad = nullptr;
+                if (rc) return rc;
             }
         }
     }

@@ -39,6 +39,8 @@ struct fdtd_grid {
     int ck_every = 0, ck_count = 0;
     float *e2buf = nullptr;                // lossy medium on a fused record = 3 grid: lamE' before its scaling by Ca, [3][nc] (fdtd_set_conductivity)
     float *ck_e2 = nullptr;                // = e2buf while the checkpointed sweep runs a fused adjoint step of a lossy medium
+    bool ck_store = false;                 // set while the checkpointed sweep replays a segment on the fused kernels: D = dE'/d inv_eps after every step
+    float *ck_gradhook = nullptr;          // set while it runs the segment's fused adjoint steps: g += lamE' . D after every step
     float *ck_grad = nullptr;              // set while the checkpointed sweep runs an adjoint step on the generic kernels: g += lamE' . D there
     const float *sigma = nullptr;          // N4: conductivity volume of the caller (fdtd_set_conductivity), or NULL
     bool replaying = false;                // the checkpointed reverse sweep is re-running forward steps: the state stays in its ping-pong volume

@@ -775,6 +775,8 @@ struct InvParams {
     float *grad;                   // dL/d inv_eps, accumulated ([3][nc] with G.aniso)
     const float *im;               // inv_mu or NULL (= 1)
     const float *ie;               // inv_eps (G.aniso: [3][nc]; components y, z come by LDG at my cells)
+    float *gmu;                    // N4: dL/d inv_mu, accumulated (g_mu -= S sum_c lamH'_c (curl+ E')_c), or NULL
+    const float *lamH[2];          // ... the H part of the cotangent volumes: lamH' of step n is in volume (n+1)&1 (im lamH' with inv_mu)
     const int *step;
     int bias, n_steps;             // this launch inverts step n = *step + bias; nothing to do if n >= n_steps (see enqueue_bwd)
     int nst, stage;
@@ -900,6 +902,23 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_inverse(const __grid_constant
                 if (sm & 8) Hx = Hx - add_sources4(P, n, 3, splat(0.f), i, j, kk);
                 if (sm & 16) Hy = Hy - add_sources4(P, n, 4, splat(0.f), i, j, kk);
                 if (sm & 32) Hz = Hz - add_sources4(P, n, 5, splat(0.f), i, j, kk);
+            }
+            if (P.gmu && !prolog && own_ok && inz) {          // N4, dL/d inv_mu at my cells of I (sequential sweep only: see fused_backward)
+                const int off = kk * plane + own_xy;
+                const float *lh = P.lamH[(n + 1) & 1] + off;
+                float4 a = ldg4(lh) * (Dy_z - Dz_y);
+                a = fma4(ldg4(lh + nc), Dz_x - Dx_z, a);
+                a = fma4(ldg4(lh + 2 * nc), Dx_y - Dy_x, a);
+                if (P.im) a = a * (S * rcp4(sim));                // the volume holds im lamH': a / im = a S / (S im)
+                a = S * a;
+                float *gp = P.gmu + off;
+                if (mall) stg4(gp, ld4(gp) - a);
+                else {
+                    if (m0) gp[0] -= a.x;
+                    if (m1) gp[1] -= a.y;
+                    if (m2) gp[2] -= a.z;
+                    if (m3) gp[3] -= a.w;
+                }
             }
             // outside I the volume's own value stands (the recorded pre-step H at index lo-1)
             Hx = sel4(m0 && inz, m1 && inz, m2 && inz, m3 && inz, Hx, Hpx);
@@ -1837,6 +1856,12 @@ void enqueue_fwd(void *vctx, cudaStream_t cs)
     if (c->recording) join_side(g, cs, 1);
     // N2: time-domain detectors on the state step n just wrote (volume (n+1)&1)
     for (const TimeDetDev &q : *c->TD) launch_time_detect(g->G, c->A, c->B, 1, c->ie, c->im, q, g->red, g->step_in(), cs);
+    // N4, replay of a segment in the checkpointed reverse sweep: D = dE'/d inv_eps of step n from the two volumes
+    if (g->ck_store) {
+        launch_dE_store(g->G, c->A, c->B, g->dE, g->ck_every, 0, c->ie, g->sigma, g->step_in(), cs);
+        for (int q = 0; q < c->P.n_src; ++q)
+            if (c->P.src[q].comp < 3) launch_dE_source(g->G, g->dE, g->ck_every, c->P.src[q], c->ie, g->sigma, g->step_in(), cs);
+    }
     ++g->enq_step;
 }
 
@@ -1894,6 +1919,10 @@ void enqueue_bwd(void *vctx, cudaStream_t cs)
       F->tile->launch_adj(Q, F->n_adj, F->smem, cs);
       ++g->enq_step;
       if (side_inject) join_side(g, cs, 1); }
+    // N4, checkpointed reverse sweep: g += lamE' . D with lamE' in the volume the adjoint step just wrote (n&1), or, for a
+    // lossy medium (the volume holds Ca lamE'), in the scratch volumes
+    if (g->ck_gradhook) { ProfScope p(g, fdtd_grid::PC_INV_E_GRAD, cs);
+      launch_grad_from_dE(G, Q.e2_out ? Q.e2_out : c->lamA, Q.e2_out ? Q.e2_out : c->lamB, g->dE, g->ck_every, g->ck_gradhook, g->step_in(), cs); }
     if (c->fused_inv) {
         InvParams J = c->I;
         J.step = g->step_in();
@@ -1953,7 +1982,10 @@ int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float
     key.push_back(recording ? 1 : 0);
     key.append((const char *)&n_steps, recording ? sizeof(n_steps) : 0);
     if (!TD.empty()) key.append((const char *)TD.data(), TD.size() * sizeof(TimeDetDev));
-    rc = fdtd_run_steps_fwd(g, key, n_count, 1 + (recording ? 1 : 0) + (int)TD.size(), st, enqueue_fwd, &ctx);
+    int n_store = 0;
+    if (g->ck_store) { n_store = 1; for (const SourceDev &q : S) if (q.comp < 3) ++n_store; }
+    key.push_back((char)n_store);
+    rc = fdtd_run_steps_fwd(g, key, n_count, 1 + (recording ? 1 : 0) + (int)TD.size() + n_store, st, enqueue_fwd, &ctx);
     if (rc) return rc;
     if (n_end != n_total || g->replaying) return FDTD_OK;      // (replaying: the checkpointed reverse sweep leaves the state in its volume)
     if (recording) {      // E' of the last step; the p-th step of the call read counter slot p&1, so the count sits in slot n_count&1
@@ -1992,14 +2024,15 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
         if (e != cudaSuccess) { (void)cudaGetLastError(); return fdtd_fail(FDTD_ECUDA, cudaGetErrorString(e)); }
     }
     const bool want_grad = dL_dinv_eps != nullptr;      // false: adjoint sweep only, the primal volumes are not touched
-    // N4: dL/d inv_mu is formed by the generic inverse H kernel (the fused inverse step's stage has no room for lamH)
-    const bool fused_inv = want_grad && F->itile != nullptr && (int)S.size() <= MAX_SRC && !getenv("FDTD_GENERIC_INVERSE") && !dL_dinv_mu;
+    // N4: dL/d inv_mu is formed in the inverse step from lamH' of volume (n+1)&1, which adjoint step n-1 overwrites: the
+    // inverse step of step n must then run before adjoint step n-1 (no pipelined sweep)
+    const bool fused_inv = want_grad && F->itile != nullptr && (int)S.size() <= MAX_SRC && !getenv("FDTD_GENERIC_INVERSE");
     // B1 inside the adjoint kernel when every detector with a cotangent is on E components (else a kernel per detector)
     bool fused_det = (int)D.size() <= MAX_DET;
     for (const DetectorDev &dt : D) if (dt.phasor && (dt.mask >> 3)) fused_det = false;
     // while profiling (events around every launch) the kernels run one after the other, so each is timed alone
     // (time-domain detector transposes read the primal state after step n, which the pipelined sweep is still writing)
-    const bool pipelined = fused_inv && fused_det && F->n_inv_p > 0 && !g->profiling && TD.empty() && whole;
+    const bool pipelined = fused_inv && fused_det && F->n_inv_p > 0 && !g->profiling && TD.empty() && whole && !dL_dinv_mu;
     BwdCtx ctx{ g, F->sp, F->ip, fused_inv, fused_det, pipelined, want_grad, F->bufB, fields, inv_eps, inv_mu, dL_dinv_eps, g->lam, F->lamB, &S, &D, total_freq, &TD, dL_dinv_mu };
     if (fused_inv) {
         // reverse step n reads primal volume (n+1)&1 and writes n&1: state n_steps must sit in volume n_steps&1
@@ -2011,6 +2044,7 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
         InvParams &I = ctx.I;
         I.maps = F->d_maps[2];
         I.buf[0] = fields; I.buf[1] = F->bufB; I.grad = dL_dinv_eps; I.im = inv_mu; I.ie = inv_eps;
+        I.gmu = dL_dinv_mu; I.lamH[0] = g->lam + 3 * (size_t)g->G.nc; I.lamH[1] = F->lamB + 3 * (size_t)g->G.nc;
         I.n_src = (int)S.size();
         I.sEl = I.sHl = 1 << 30; I.sEh = I.sHh = -1;
         for (size_t q = 0; q < S.size(); ++q) {
@@ -2044,11 +2078,12 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     key.append((const char *)&fields, sizeof(fields));
     key.append((const char *)&dL_dinv_eps, sizeof(dL_dinv_eps));
     key.append((const char *)&dL_dinv_mu, sizeof(dL_dinv_mu));
+    key.append((const char *)&g->ck_gradhook, sizeof(g->ck_gradhook));
     if (!S.empty()) key.append((const char *)S.data(), S.size() * sizeof(SourceDev));
     if (!D.empty()) key.append((const char *)D.data(), D.size() * sizeof(DetectorDev));
     if (!TD.empty()) key.append((const char *)TD.data(), TD.size() * sizeof(TimeDetDev));
     const int n_inj = g->G.d > 0 ? 1 : 0;
-    const int launches = (int)TD.size() + (!want_grad ? 1 + (fused_det ? 0 : n_adj)
+    const int launches = (int)TD.size() + (g->ck_gradhook ? 1 : 0) + (!want_grad ? 1 + (fused_det ? 0 : n_adj)
                          : (fused_inv ? 2 + (fused_det ? 0 : n_adj) + n_inj : 3 + (fused_det ? 0 : n_adj) + (int)S.size() + n_inj));
     rc = fdtd_run_steps_bwd(g, key, n_count, launches, st, enqueue_bwd, &ctx);
     if (rc || !pipelined) return rc;

@@ -206,7 +206,7 @@ def test_tfsf_plane_source(B, axis, pol, direction):
 
 
 # ----------------------------------------------------------------------------------------------------------- N4
-@pytest.mark.parametrize("case", ["tiny-generic", "mini-generic", "mini-fused"])
+@pytest.mark.parametrize("case", ["tiny-generic", "mini-generic", "mini-fused", "mini-nomu-odd-fused"])
 def test_gradient_with_respect_to_inv_mu(B, case):
     """dL/d inv_mu through fdtd_backward_mu against the oracle (loss on phasors and on the final H, so the
     cotangent of H is seeded; every CPML term on the tiny grid; the fused sweep carries im lamH)."""
@@ -215,10 +215,11 @@ def test_gradient_with_respect_to_inv_mu(B, case):
     if case.startswith("tiny"):
         w = wl.tiny_pml(n_steps=30)
     else:
-        w = wl.c3_mini(n_steps=120, kappa_max=3.0, alpha_max=0.05)
+        ns = 121 if "odd" in case else 120
+        w = wl.c3_mini(n_steps=ns, kappa_max=3.0, alpha_max=0.05)
         rng = np.random.default_rng(5)
-        w.meta["inv_mu"] = (1.0 / (1.0 + 0.5 * rng.random((w.nz, w.ny, w.nx), dtype=np.float32))).astype(np.float32)
-        w.sources.append(wl.Source(4, (20, 12, 22), (60, 40, 23), (0.3 * wl.gaussian_sine(120, 40, 12, 11)).astype(np.float32)))
+        w.meta["inv_mu"] = None if "nomu" in case else (1.0 / (1.0 + 0.5 * rng.random((w.nz, w.ny, w.nx), dtype=np.float32))).astype(np.float32)
+        w.sources.append(wl.Source(4, (20, 12, 22), (60, 40, 23), (0.3 * wl.gaussian_sine(ns, 40, 12, 11)).astype(np.float32)))
     path = B.FDTD_PATH_FUSED if case.endswith("fused") else B.FDTD_PATH_GENERIC
     im = w.meta["inv_mu"]
     o = Oracle(**w.grid_kwargs())
@@ -232,7 +233,7 @@ def test_gradient_with_respect_to_inv_mu(B, case):
     kw.update(max_steps=w.n_steps, record=1, path=path)
     g = B.Grid(**kw)
     f = torch.zeros((6, w.nz, w.ny, w.nx), device="cuda")
-    ie, imt = torch.as_tensor(w.inv_eps).cuda(), torch.as_tensor(im).cuda()
+    ie, imt = torch.as_tensor(w.inv_eps).cuda(), (None if im is None else torch.as_tensor(im).cuda())
     ph = g.forward(f, ie, imt, w.sources, w.detectors, w.n_steps)
     dLf = torch.zeros_like(f)
     dLf[3:] = f[3:]
@@ -240,7 +241,10 @@ def test_gradient_with_respect_to_inv_mu(B, case):
     grad, lam0 = g.backward(f, ie, imt, w.sources, w.detectors, [2.0 * P for P in ph], dLf, w.n_steps,
                             want_dL_dfields0=True, grad_mu=gmu)
     torch.cuda.synchronize()
-    assert g.info().path == path
+    info = g.info()
+    assert info.path == path
+    # fused: dL/d inv_mu is formed inside the fused inverse step (one launch per reverse step, and inverse step 0)
+    assert info.fused_inverse_launches == (w.n_steps if path == B.FDTD_PATH_FUSED else 0)
     e = (relerr(gmu.cpu().numpy(), gmu_r), relerr(grad.cpu().numpy(), g_r), relerr(lam0.cpu().numpy(), lam_r))
     g.close()
     assert np.max(np.abs(gmu_r)) > 0
