@@ -357,6 +357,19 @@ def test_lossy_medium_forward_and_checkpointed_gradient(B, case):
     # forward + replayed forward + adjoint sweep, each w.n_steps launches of the fused step kernel
     assert info.fused_step_launches == (3 * w.n_steps if path == B.FDTD_PATH_FUSED else 0)
     assert relerr(grad.cpu().numpy(), g_tape) <= TOL_GRAD and relerr(lam0.cpu().numpy(), lam_tape) <= TOL_GRAD
+    # record = 0: forward and the adjoint sweep alone (no gradient, nothing to reverse) take the lossy medium as well
+    g0 = B.Grid(**{**w.grid_kwargs(), "max_steps": w.n_steps, "record": 0, "path": path})
+    g0.set_conductivity(sig)
+    f0g = torch.zeros((6,) + shape, device="cuda")
+    ph0 = g0.forward(f0g, ie, imt, w.sources, w.detectors, w.n_steps)
+    dLf0 = torch.zeros_like(f0g)
+    dLf0[:3] = 0.5 * f0g[:3]
+    _, lam00 = g0.backward(f0g, ie, imt, w.sources, w.detectors, [2.0 * P for P in ph0], dLf0, w.n_steps, want_grad=False)
+    torch.cuda.synchronize()
+    info0 = g0.info()
+    g0.close()
+    assert info0.fused_step_launches == (2 * w.n_steps if path == B.FDTD_PATH_FUSED else 0)
+    assert relerr(f0g.cpu().numpy(), fr) <= TOL_FIELD and relerr(lam00.cpu().numpy(), lam_tape) <= TOL_GRAD
     # a recording grid refuses a lossy medium
     g1 = B.Grid(**{**w.grid_kwargs(), "max_steps": 4, "record": 1})
     with pytest.raises(B.FdtdError) as e:
