@@ -91,6 +91,7 @@ struct Cfg {
     static constexpr int PW = TX + 8, ROWS = TY + 2;
     static constexpr int ROWB = PW * 4;                                 // box row pitch in bytes
     static constexpr int BOX_BYTES = PW * ROWS * 4;                     // TMA transaction bytes of one box
+    static constexpr int BOXE_BYTES = PW * (ROWS - 1) * 4;              // ... of an own-cell array of the step kernel (e, inv_eps): no row below the tile
     static constexpr int SLOT = (BOX_BYTES + 127) / 128 * 128;
     static constexpr int STAGE = 7 * SLOT;                               // F x3, e x3, inv_eps
     static constexpr int RP = 4 * CW;                                   // ring row pitch (floats)
@@ -370,15 +371,16 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                 uint8_t *st = smem + (size_t)s * P.stage;
                 const bool prolog = kk == S.k0 - 1;
                 const bool xs = G.d > 0 && !prolog;
-                mbar_expect_tx(fb, (prolog ? 3u : 7u) * C::BOX_BYTES + (xs ? 4u * P.xs_bytes : 0u));
+                mbar_expect_tx(fb, 3u * C::BOX_BYTES + (prolog ? 0u : 4u * C::BOXE_BYTES) + (xs ? 4u * P.xs_bytes : 0u));
                 tma_load_3d(st, M + 3, x, y, kk, fb);
                 tma_load_3d(st + C::SLOT, M + 4, x, y, kk, fb);
                 tma_load_3d(st + 2 * C::SLOT, M + 5, x, y, kk, fb);
                 if (!prolog) {
-                    tma_load_3d(st + 3 * C::SLOT, M + 0, x, y, kk, fb);
-                    tma_load_3d(st + 4 * C::SLOT, M + 1, x, y, kk, fb);
-                    tma_load_3d(st + 5 * C::SLOT, M + 2, x, y, kk, fb);
-                    tma_load_3d(st + 6 * C::SLOT, Mie, x, y, kk, fb);
+                    // e and inv_eps are read at a thread's own cells only (rows j0 .. j0 + TY): their boxes start one row later
+                    tma_load_3d(st + 3 * C::SLOT, M + 0, x, y + 1, kk, fb);
+                    tma_load_3d(st + 4 * C::SLOT, M + 1, x, y + 1, kk, fb);
+                    tma_load_3d(st + 5 * C::SLOT, M + 2, x, y + 1, kk, fb);
+                    tma_load_3d(st + 6 * C::SLOT, Mie, x, y + 1, kk, fb);
                 }
                 if (xs) {      // phase A states of plane kk; phase B states of plane kk-1 (forward) / kk (adjoint)
                     const CUtensorMap *MA = P.maps + 13 + par * 4 + FA * 2, *MB = P.maps + 13 + par * 4 + FB * 2;
@@ -457,7 +459,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                 const int dm = det_mask(P, kk, true);
                 for (int c = 0; c < 3; ++c) {
                     if (!((dm >> c) & 1)) continue;
-                    const uint32_t se = so + (3 + c) * C::SLOT;
+                    const uint32_t se = so - C::ROWB + (3 + c) * C::SLOT;
                     sts4(se, det_adjoint4(P, n, c, lds4(se), i, j, kk));
                 }
                 if (dm & 7) fence_proxy_async();
@@ -566,8 +568,9 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                 cgx = gx; cgy = gy;
             }
             const float4 tEx = Dy_z - Dz_y, tEy = Dz_x - Dx_z, tEz = Dx_y - Dy_x;
-            const float4 ex = lds4(so + 3 * C::SLOT), ey = lds4(so + 4 * C::SLOT), ez = lds4(so + 5 * C::SLOT);
-            const float4 sie = S * lds4(so + 6 * C::SLOT);
+            const uint32_t soe = so - C::ROWB;           // my cells inside a box of e / inv_eps (no row below the tile)
+            const float4 ex = lds4(soe + 3 * C::SLOT), ey = lds4(soe + 4 * C::SLOT), ez = lds4(soe + 5 * C::SLOT);
+            const float4 sie = S * lds4(soe + 6 * C::SLOT);
             // N4: one inv_eps volume per component (R30: the stage holds component x, y and z come by LDG at my cells) and / or
             // a conductivity (R29: E' = Ca E + Cb S ie bracket, beta = sigma S ie / 2, Ca = (1 - beta) / (1 + beta), Cb = 1 / (1 + beta))
             const bool n4 = N4 && (G.aniso || P.sigma != nullptr);
@@ -1640,11 +1643,13 @@ int build_maps(fdtd_grid *g, int which, float *volA, float *volB, const float *i
     CUtensorMap *H = F->h_maps[which];
     bool ok = true;
     float *bufs[2] = { volA, volB };
+    // components 3-5 (the H-type operand F of phase A) are differenced: boxes with the row below the tile; components 0-2 and
+    // inv_eps are read at a thread's own cells only: one row less
     for (int set = 0; set < 2; ++set)
         for (int c = 0; c < 6; ++c)
             ok &= encode3d(&H[set * 6 + c], bufs[set] + (long long)c * G.nc, G.nx, G.ny, G.nz, G.nx,
-                           (long long)G.nx * G.ny, PW, ROWS);
-    ok &= encode3d(&H[12], ie, G.nx, G.ny, G.nz, G.nx, (long long)G.nx * G.ny, PW, ROWS);
+                           (long long)G.nx * G.ny, PW, c < 3 ? ROWS - 1 : ROWS);
+    ok &= encode3d(&H[12], ie, G.nx, G.ny, G.nz, G.nx, (long long)G.nx * G.ny, PW, ROWS - 1);
     if (G.d > 0) {
         // x-slab states (c=z,s=0) and (c=y,s=1): layout [nz][ny][2*dpx], box = whole storage rows of the tile's rows
         for (int set = 0; set < 2; ++set)
