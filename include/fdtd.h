@@ -299,6 +299,22 @@ FDTD_API int fdtd_flux(fdtd_grid *grid, const fdtd_detector *det, const float *p
 FDTD_API int fdtd_flux_vjp(fdtd_grid *grid, const fdtd_detector *det, const float *phasor, int32_t axis, int32_t interpolate,
                   const float *dL_dflux, float *dL_dphasor, void *cuda_stream);
 
+/* fdtd_flux for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): same flux, same arguments without the grid (whose only part in fdtd_flux is the reduction scratch
+ * that fdtd_create_grid allocated).  This entry point calls no cudaMalloc / cudaFree and no allocating library routine: its
+ * scratch (one block partial per 2048 plane cells + a ticket, 16.25 KB) is a file-scope `static __device__` array of the
+ * library, held by every GPU that loads the library until the process exits.  Hence the limit: the plane may have at most
+ * FDTD_FLUX_STATIC_MAX_CELLS cells (e.g. 2048 x 2048); beyond it EINVAL, use fdtd_flux.  The detector box is taken as it is
+ * (no grid to check it against: lo >= 0, hi > lo).  Work: one 256-byte memset and n_freq kernels on cuda_stream; the first
+ * call on a device also resolves the array's device address (cudaGetSymbolAddress), so make that call outside a capture.
+ * All calls share the array and it keeps the last call's contents: what must start at zero is cleared on cuda_stream at
+ * the start of every call, but calls that overlap on the GPU (other streams, other threads) race on it -- serialise them.
+ * The sum over the plane is taken in a fixed order (deterministic); it differs from fdtd_flux's by rounding only.
+ * det: HOST; phasor: DEVICE; flux: DEVICE [n_freq], written.  Errors: EINVAL as fdtd_flux, and for a plane beyond the limit. */
+#define FDTD_FLUX_STATIC_MAX_CELLS 4194304
+FDTD_API int fdtd_flux_static(const fdtd_detector *det, const float *phasor, int32_t axis, int32_t interpolate, float *flux,
+                     void *cuda_stream);
+
 /* One-directional plane source = Total-Field/Scattered-Field interface (reading R25).
  * A plane wave travelling along `axis` a in direction dir = +1 / -1, E polarised along pol = b != a, its H along the
  * third axis c, in a medium that is uniform (eps_r, mu_r) on the planes the interface touches.  The incident wave is

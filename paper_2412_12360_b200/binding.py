@@ -73,7 +73,7 @@ class fdtd_profile(C.Structure):
 EXPORTS = ("fdtd_grad_rho", "fdtd_set_profiling", "fdtd_get_profile", "fdtd_create_grid", "fdtd_forward", "fdtd_backward", "fdtd_destroy", "fdtd_last_error",
            "fdtd_get_info", "fdtd_version", "fdtd_forward_host", "fdtd_backward_host", "fdtd_debug_partition",
            "fdtd_forward_td", "fdtd_backward_td", "fdtd_flux", "fdtd_flux_vjp", "fdtd_tfsf_plane",
-           "fdtd_forward_range", "fdtd_backward_range", "fdtd_halo_export", "fdtd_halo_import", "fdtd_backward_mu", "fdtd_set_conductivity", "fdtd_probe_bandwidth")
+           "fdtd_forward_range", "fdtd_backward_range", "fdtd_halo_export", "fdtd_halo_import", "fdtd_backward_mu", "fdtd_set_conductivity", "fdtd_probe_bandwidth", "fdtd_flux_static")
 
 
 def _load():
@@ -272,6 +272,17 @@ def fdtd_halo_import(grid, fields, which, n, side, buf, stream) -> None:
 
 def fdtd_flux(grid, det, phasor, axis, interpolate, flux, stream) -> None:
     _check(_L.fdtd_flux(grid, det, _ptr(phasor), int(axis), int(bool(interpolate)), _ptr(flux), stream))
+
+
+FDTD_FLUX_STATIC_MAX_CELLS = 4194304
+
+
+def fdtd_flux_static(det, phasor, axis, interpolate, flux, stream) -> None:
+    """fdtd_flux without a grid and without any device allocation (include/fdtd.h): scratch in a static __device__ array;
+    planes of at most FDTD_FLUX_STATIC_MAX_CELLS cells.  det: a fdtd_detector struct (HOST); phasor, flux: cuda tensors."""
+    _L.fdtd_flux_static.restype = C.c_int
+    _L.fdtd_flux_static.argtypes = [C.POINTER(fdtd_detector), C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
+    _check(_L.fdtd_flux_static(det, _ptr(phasor), int(axis), int(bool(interpolate)), _ptr(flux), stream))
 
 
 def fdtd_flux_vjp(grid, det, phasor, axis, interpolate, dL_dflux, dL_dphasor, stream) -> None:
