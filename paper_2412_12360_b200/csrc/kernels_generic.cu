@@ -243,68 +243,67 @@ __global__ void k_record(Dims G, RecLayout R, const float *__restrict__ fH, cons
 
 // Pipelined recorder of the fused path: runs beside forward step n and reads the buffer that step reads
 // (n&1): pre-step H at lo-1 -> rec[n] (n < n_steps), E' at hi, written by step n-1, -> rec[n-1] (n >= 1).
-// 128 threads x <= 32 registers and no shared memory, so a block fits beside a resident k_step CTA.
-__global__ void __launch_bounds__(128, 16) k_record_pipe(Dims G, RecLayout R, const float *__restrict__ A,
+// 128 threads x <= 32 registers and no shared memory, so a block fits beside a resident k_step CTA and shares its issue
+// slots: the kernel is kept short in instructions (grid.y = the record's segment, 32-bit index arithmetic, PIPE_U elements
+// per thread with their loads in flight together).
+#ifndef FDTD_PIPE_U
+#define FDTD_PIPE_U 2
+#endif
+constexpr int PIPE_U = FDTD_PIPE_U;
+
+struct PipeSeg {               // segment blockIdx.y of a step's record
+    long long base;            // volume offset (component included) of the segment's first face cell
+    long long off;             // offset of the segment inside a step's record
+    unsigned cells, nf;        // face cells; extent of the fast in-face axis
+    long long sf, ss;          // volume strides of the fast / slow in-face axis
+    int side;                  // 0: low face (H at lo-1), 1: high face (E' at hi)
+};
+struct PipeTable { PipeSeg s[12]; long long stride; int half; };
+
+__global__ void __launch_bounds__(128, 16) k_record_pipe(const __grid_constant__ PipeTable T, const float *__restrict__ A,
                                                          const float *__restrict__ B, float *__restrict__ rec,
                                                          const int *__restrict__ step, int n_steps)
 {
-    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= R.stride) return;
     const int n = *step;
-    const float *f = (n & 1) ? B : A;
-    int a = 0, side = 0, which = 0;
-    long long local = -1;
+    const PipeSeg &q = T.s[blockIdx.y];
+    if (q.side ? n < 1 : n >= n_steps) return;
+    const float *f = ((n & 1) ? B : A) + q.base;
+    const unsigned l0 = blockIdx.x * (128u * PIPE_U) + threadIdx.x;
+    float v[PIPE_U];
 #pragma unroll
-    for (int aa = 0; aa < 3; ++aa)
+    for (int u = 0; u < PIPE_U; ++u) {
+        const unsigned l = l0 + u * 128u;
+        v[u] = l < q.cells ? __ldg(f + (l % q.nf) * q.sf + (l / q.nf) * q.ss) : 0.f;
+    }
+    const long long r0 = (long long)(q.side ? n - 1 : n) * T.stride + q.off;
 #pragma unroll
-        for (int ss = 0; ss < 2; ++ss)
-#pragma unroll
-            for (int ww = 0; ww < 2; ++ww) {
-                const long long o = R.off[aa][ss][ww];
-                if (t >= o && t < o + R.cells[aa]) { a = aa; side = ss; which = ww; local = t - o; }
-            }
-    if (local < 0) return;   // padding
-    if (side ? n < 1 : n >= n_steps) return;
-    const int fa = R.fast[a], sl = R.slow[a];
-    const int nf = G.hi[fa] - G.lo[fa];
-    int pos[3];
-    pos[a] = side ? G.hi[a] : G.lo[a] - 1;
-    pos[fa] = G.lo[fa] + (int)(local % nf);
-    pos[sl] = G.lo[sl] + (int)(local / nf);
-    const int comp = (a + 1 + which) % 3;
-    const long long p = lin(G, pos[0], pos[1], pos[2]);
-    rec_store(rec, (long long)(side ? n - 1 : n) * R.stride + t, __ldg(f + (side ? comp : 3 + comp) * G.nc + p), R.half);
+    for (int u = 0; u < PIPE_U; ++u) {
+        const unsigned l = l0 + u * 128u;
+        if (l < q.cells) rec_store(rec, r0 + l, v[u], T.half);
+    }
 }
 
 // Face injection of the fused reverse sweep, run beside adjoint step n: rec[n] -> buffer (n+1)&1, the volume
 // the inverse step n reads (pre-step H at lo-1, E' at hi).  Sized like k_record_pipe to fit beside a k_step CTA.
-__global__ void __launch_bounds__(128, 16) k_inject_pipe(Dims G, RecLayout R, float *__restrict__ A, float *__restrict__ B,
+__global__ void __launch_bounds__(128, 16) k_inject_pipe(const __grid_constant__ PipeTable T, float *__restrict__ A, float *__restrict__ B,
                                                          const float *__restrict__ rec, const int *__restrict__ step)
 {
-    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= R.stride) return;
     const int n = *step;
-    float *f = (n & 1) ? A : B;
-    int a = 0, side = 0, which = 0;
-    long long local = -1;
+    const PipeSeg &q = T.s[blockIdx.y];
+    float *f = ((n & 1) ? A : B) + q.base;
+    const unsigned l0 = blockIdx.x * (128u * PIPE_U) + threadIdx.x;
+    const long long r0 = (long long)n * T.stride + q.off;
+    float v[PIPE_U];
 #pragma unroll
-    for (int aa = 0; aa < 3; ++aa)
+    for (int u = 0; u < PIPE_U; ++u) {
+        const unsigned l = l0 + u * 128u;
+        v[u] = l < q.cells ? rec_load(rec, r0 + l, T.half) : 0.f;
+    }
 #pragma unroll
-        for (int ss = 0; ss < 2; ++ss)
-#pragma unroll
-            for (int ww = 0; ww < 2; ++ww) {
-                const long long o = R.off[aa][ss][ww];
-                if (t >= o && t < o + R.cells[aa]) { a = aa; side = ss; which = ww; local = t - o; }
-            }
-    if (local < 0) return;   // padding
-    const int fa = R.fast[a], sl = R.slow[a];
-    const int nf = G.hi[fa] - G.lo[fa];
-    int pos[3];
-    pos[a] = side ? G.hi[a] : G.lo[a] - 1;
-    pos[fa] = G.lo[fa] + (int)(local % nf);
-    pos[sl] = G.lo[sl] + (int)(local / nf);
-    const int comp = (a + 1 + which) % 3;
-    f[(side ? comp : 3 + comp) * G.nc + lin(G, pos[0], pos[1], pos[2])] = rec_load(rec, (long long)n * R.stride + t, R.half);
+    for (int u = 0; u < PIPE_U; ++u) {
+        const unsigned l = l0 + u * 128u;
+        if (l < q.cells) f[(l % q.nf) * q.sf + (l / q.nf) * q.ss] = v[u];
+    }
 }
 
 __global__ void k_advance(int *step, int delta) { *step += delta; }
@@ -561,18 +560,43 @@ void launch_record_pp(const Dims &G, const RecLayout &R, const float *bufA, cons
     k_record<false, true><<<(unsigned)((R.stride + 255) / 256), 256, 0, st>>>(G, R, bufA, bufB, nullptr, rec, step);
 }
 
+// grid of the pipe kernels: x = blocks over the largest face, y = the 12 segments of a step's record
+static dim3 pipe_grid(const RecLayout &R)
+{
+    const long long c = std::max(R.cells[0], std::max(R.cells[1], R.cells[2]));
+    return dim3((unsigned)((c + 128 * PIPE_U - 1) / (128 * PIPE_U)), 12, 1);
+}
+static PipeTable pipe_table(const Dims &G, const RecLayout &R)
+{
+    PipeTable T;
+    const long long str[3] = { 1, G.nx, (long long)G.nx * G.ny };
+    for (int seg = 0; seg < 12; ++seg) {
+        const int a = seg >> 2, side = (seg >> 1) & 1, which = seg & 1;
+        const int fa = R.fast[a], sl = R.slow[a], comp = (a + 1 + which) % 3;
+        PipeSeg &q = T.s[seg];
+        q.side = side;
+        q.cells = (unsigned)R.cells[a];
+        q.nf = (unsigned)(G.hi[fa] - G.lo[fa]);
+        q.sf = str[fa]; q.ss = str[sl];
+        q.base = (long long)(side ? comp : 3 + comp) * G.nc + (side ? G.hi[a] : G.lo[a] - 1) * str[a] + G.lo[fa] * str[fa] + G.lo[sl] * str[sl];
+        q.off = R.off[a][side][which];
+    }
+    T.stride = R.stride; T.half = R.half;
+    return T;
+}
+
 void launch_record_pipe(const Dims &G, const RecLayout &R, const float *bufA, const float *bufB, float *rec,
                         const int *step, int n_steps, cudaStream_t st)
 {
     if (R.stride == 0) return;
-    k_record_pipe<<<(unsigned)((R.stride + 127) / 128), 128, 0, st>>>(G, R, bufA, bufB, rec, step, n_steps);
+    k_record_pipe<<<pipe_grid(R), 128, 0, st>>>(pipe_table(G, R), bufA, bufB, rec, step, n_steps);
 }
 
 void launch_inject_pipe(const Dims &G, const RecLayout &R, float *bufA, float *bufB, const float *rec,
                         const int *step, cudaStream_t st)
 {
     if (R.stride == 0) return;
-    k_inject_pipe<<<(unsigned)((R.stride + 127) / 128), 128, 0, st>>>(G, R, bufA, bufB, rec, step);
+    k_inject_pipe<<<pipe_grid(R), 128, 0, st>>>(pipe_table(G, R), bufA, bufB, rec, step);
 }
 
 void launch_inject_pp(const Dims &G, const RecLayout &R, float *bufA, float *bufB, const float *rec,
