@@ -68,8 +68,8 @@ def algorithmic_bytes(w, grad_cells: int, recording: bool, has_mu: bool = False,
         # fused adjoint step (B2+B5): 6 R + 6 W cotangents + ie over the grid, adjoint psi R/W on slabs; the face
         # injection of the reverse sweep runs beside it and is timed with it
         "fused_adjoint_step": cells * (52 + mu) + slab * 32 + 2 * rec,
-        # fused inverse step (B3+B4) over the box: R E',H' (6), ie, lamE' (3), W E,H (6); g R/W on the grad box
-        "fused_inverse_step": inter * (64 + mu) + grad_cells * 8,
+        # fused inverse step (B3+B4) over the box: R E',H' (6), ie, W E,H (6); on the grad box also R lamE' (3) and g R/W
+        "fused_inverse_step": inter * (52 + mu) + grad_cells * 20,
         "update_E": cells * 40 + slab * 16,
         "update_H": cells * (36 + mu) + slab * 16,
         "adjoint_H": cells * (36 + mu) + slab * 16,
@@ -85,8 +85,9 @@ def whole_job_bytes_per_cell_step(w, grad_cells: int, rbox=None) -> dict:
     """SURVEY 8(d) whole-job figures per cell and time step: forward alone (6 R + 6 W + inv_eps + psi on the slabs), and
     forward + adjoint pass + inverse pass + g, where the inverse pass counts 12 floats per box cell (R E', H'; W E, H):
     inv_eps and lamE' are counted once, with the adjoint pass (13 + 12 + 2 floats; C3: 63.5 / 161.0).
-    The per-kernel figure of k_inverse (algorithmic_bytes) is 16 floats per box cell because as a launch of its own it
-    has to read inv_eps and lamE' again; the whole-job roofline is not credited with that re-read."""
+    The per-kernel figure of k_inverse (algorithmic_bytes) is 13 floats per box cell and 16 on the gradient box because as a
+    launch of its own it has to read inv_eps and (where the gradient is formed) lamE' again; the whole-job roofline is not
+    credited with that re-read."""
     a0 = algorithmic_bytes(w, grad_cells, recording=False)
     d = w.pml_cells
     bx, by, bz = rbox if rbox else (w.nx - 2 * d, w.ny - 2 * d, w.nz - 2 * d)

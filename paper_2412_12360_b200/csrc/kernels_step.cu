@@ -837,13 +837,16 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_inverse(const __grid_constant
                 uint64_t *fb = &full[s];
                 uint8_t *st = smem + (size_t)s * P.stage;
                 const bool first = kk == S.k0 - 1;       // only H of this plane is wanted: no inv_eps, no lamE'
-                mbar_expect_tx(fb, 3u * C::BOX_BYTES + 5u * C::BOXB_BYTES + (first ? 0u : 4u * C::BOXC_BYTES));
+                // lamE' only enters the gradient: planes and tiles outside the gradient box do not load it
+                const bool lam = !first && kk >= G.glo[2] && kk < G.ghi[2] && S.i0 < G.ghi[0] && S.i0 + C::TX > G.glo[0] &&
+                                 S.j0 < G.ghi[1] && S.j0 + C::TY > G.glo[1];
+                mbar_expect_tx(fb, 3u * C::BOX_BYTES + 5u * C::BOXB_BYTES + (first ? 0u : (lam ? 4u : 1u) * C::BOXC_BYTES));
                 for (int c = 0; c < 3; ++c) tma_load_3d(st + c * C::SLOT, MA + c, x, y, kk, fb);
                 for (int c = 0; c < 3; ++c) tma_load_3d(st + OB + c * C::SLOTB, MB + c, x, y, kk, fb);
                 for (int c = 0; c < 2; ++c) tma_load_3d(st + OD + c * C::SLOTB, MB + 3 + c, x, y, kk + 1, fb);
                 if (!first) {
                     tma_load_3d(st + OC, Mie, S.i0, S.j0, kk, fb);
-                    for (int c = 0; c < 3; ++c) tma_load_3d(st + OC + (1 + c) * C::SLOTC, ML + c, S.i0, S.j0, kk, fb);
+                    if (lam) for (int c = 0; c < 3; ++c) tma_load_3d(st + OC + (1 + c) * C::SLOTC, ML + c, S.i0, S.j0, kk, fb);
                 }
                 if (++s == nst) { s = 0; ++use; }
             }
