@@ -375,6 +375,37 @@ FDTD_API int fdtd_backward_range(fdtd_grid *grid, float *fields, const float *in
 FDTD_API int fdtd_halo_export(fdtd_grid *grid, float *fields, int32_t which, int32_t n, int32_t side, float *out, void *cuda_stream);
 FDTD_API int fdtd_halo_import(fdtd_grid *grid, float *fields, int32_t which, int32_t n, int32_t side, const float *in, void *cuda_stream);
 
+/* Peer stores: the exchange fused into the step kernel.  With a neighbour
+ * attached, the fused step kernel that produces the H-type components of a slab's lowest / highest owned plane stores
+ * them a second time, straight into the ghost plane of the neighbour's volume (same-process pointers, peer-mapped
+ * pointers of another GPU, or pointers opened from another process's handle: plain stores over NVLink), and leaves the
+ * H-type components of its own ghost plane on that side to the neighbour's kernel.  No plane copies, no
+ * fdtd_halo_export / _import: what is left of the exchange is ordering -- all slabs finish step n before any starts
+ * step n+1 (one stream in one process; a neighbour token or barrier across processes).  Fields, phasors and
+ * cotangents stay bit-identical to the undivided grid (tests/test_gpu_subgrid.py).
+ *
+ * fdtd_halo_volumes: the two volumes of this grid's ping-pong that hold state n (n even: *vol0, n odd: *vol1);
+ *   which = 0 the primal fields (`fields` is the pointer the range calls are given, *vol0 == fields), which = 1 the
+ *   cotangents (allocated here if no reverse sweep ran yet).  DEVICE pointers, [6][nz][ny][nx], owned by the caller
+ *   (fields) / the grid (the rest); they stay valid until fdtd_destroy.  ESTATE on a grid that runs the generic kernels.
+ * fdtd_halo_attach: side 0 = the neighbour below, 1 = above; peer_vol0 / peer_vol1 = that neighbour's
+ *   fdtd_halo_volumes of the same `which`, peer_nz its local plane count (ghosts included).  Both NULL detaches.  The
+ *   grid must have a cut on that side and run the fused kernels (ESTATE otherwise); the neighbour must attach this
+ *   grid in turn (a ghost plane on an attached side is written by the neighbour only).  While a neighbour is attached
+ *   a range call must advance exactly one step (EINVAL otherwise) and the caller orders the steps of the slabs as
+ *   stated above; a call that would run on the generic kernels (more than 4 sources / detectors) returns ESTATE.
+ * fdtd_ipc_export / fdtd_ipc_open / fdtd_ipc_close: cudaIpcGetMemHandle / OpenMemHandle / CloseMemHandle behind this ABI,
+ *   so that ranks can hand their volumes to each other without a CUDA binding of their own.  handle: HOST, 64 bytes;
+ *   offset: the pointer's offset inside the allocation the handle names (a caching allocator hands out interior
+ *   pointers).  fdtd_ipc_open returns the pointer itself (base + offset), valid in the calling process until
+ *   fdtd_ipc_close(ptr, offset).  Volumes obtained from cudaMalloc (PyTorch's default allocator, this library) qualify;
+ *   stream-ordered pools and expandable segments do not (ECUDA). */
+FDTD_API int fdtd_halo_volumes(fdtd_grid *grid, float *fields, int32_t which, float **vol0, float **vol1);
+FDTD_API int fdtd_halo_attach(fdtd_grid *grid, int32_t which, int32_t side, float *peer_vol0, float *peer_vol1, int32_t peer_nz);
+FDTD_API int fdtd_ipc_export(const void *dev_ptr, uint8_t handle[64], int64_t *offset);
+FDTD_API int fdtd_ipc_open(const uint8_t handle[64], int64_t offset, void **dev_ptr);
+FDTD_API int fdtd_ipc_close(void *dev_ptr, int64_t offset);
+
 /* Frees the grid and everything it owns (synchronises the device first).  NULL is a no-op. */
 FDTD_API int fdtd_destroy(fdtd_grid *grid);
 

@@ -73,7 +73,8 @@ class fdtd_profile(C.Structure):
 EXPORTS = ("fdtd_grad_rho", "fdtd_set_profiling", "fdtd_get_profile", "fdtd_create_grid", "fdtd_forward", "fdtd_backward", "fdtd_destroy", "fdtd_last_error",
            "fdtd_get_info", "fdtd_version", "fdtd_forward_host", "fdtd_backward_host", "fdtd_debug_partition",
            "fdtd_forward_td", "fdtd_backward_td", "fdtd_flux", "fdtd_flux_vjp", "fdtd_tfsf_plane",
-           "fdtd_forward_range", "fdtd_backward_range", "fdtd_halo_export", "fdtd_halo_import", "fdtd_backward_mu", "fdtd_set_conductivity", "fdtd_probe_bandwidth", "fdtd_flux_static")
+           "fdtd_forward_range", "fdtd_backward_range", "fdtd_halo_export", "fdtd_halo_import",
+           "fdtd_halo_volumes", "fdtd_halo_attach", "fdtd_ipc_export", "fdtd_ipc_open", "fdtd_ipc_close", "fdtd_backward_mu", "fdtd_set_conductivity", "fdtd_probe_bandwidth", "fdtd_flux_static")
 
 
 def _load():
@@ -107,6 +108,16 @@ def _load():
     L.fdtd_halo_export.argtypes = [vp, vp, i32, i32, i32, vp, vp]
     L.fdtd_halo_import.restype = C.c_int
     L.fdtd_halo_import.argtypes = [vp, vp, i32, i32, i32, vp, vp]
+    L.fdtd_halo_volumes.restype = C.c_int
+    L.fdtd_halo_volumes.argtypes = [vp, vp, i32, C.POINTER(vp), C.POINTER(vp)]
+    L.fdtd_halo_attach.restype = C.c_int
+    L.fdtd_halo_attach.argtypes = [vp, i32, i32, vp, vp, i32]
+    L.fdtd_ipc_export.restype = C.c_int
+    L.fdtd_ipc_export.argtypes = [vp, C.c_char_p, C.POINTER(C.c_int64)]
+    L.fdtd_ipc_open.restype = C.c_int
+    L.fdtd_ipc_open.argtypes = [C.c_char_p, C.c_int64, C.POINTER(vp)]
+    L.fdtd_ipc_close.restype = C.c_int
+    L.fdtd_ipc_close.argtypes = [vp, C.c_int64]
     L.fdtd_flux.restype = C.c_int
     L.fdtd_flux.argtypes = [vp, C.POINTER(fdtd_detector), vp, i32, i32, vp, vp]
     L.fdtd_flux_vjp.restype = C.c_int
@@ -268,6 +279,36 @@ def fdtd_halo_export(grid, fields, which, n, side, out, stream) -> None:
 
 def fdtd_halo_import(grid, fields, which, n, side, buf, stream) -> None:
     _check(_L.fdtd_halo_import(grid, _ptr(fields), int(which), int(n), int(side), _ptr(buf), stream))
+
+
+def fdtd_halo_volumes(grid, fields, which):
+    """(vol0, vol1): device addresses (int) of the two ping-pong volumes of the primal fields (which = 0) / cotangents (1)."""
+    a, b = C.c_void_p(), C.c_void_p()
+    _check(_L.fdtd_halo_volumes(grid, _ptr(fields), int(which), C.byref(a), C.byref(b)))
+    return int(a.value), int(b.value)
+
+
+def fdtd_halo_attach(grid, which, side, peer_vol0, peer_vol1, peer_nz) -> None:
+    """peer_vol0 / peer_vol1: device addresses (int) of the neighbour's fdtd_halo_volumes, or None / None to detach."""
+    _check(_L.fdtd_halo_attach(grid, int(which), int(side), C.c_void_p(peer_vol0), C.c_void_p(peer_vol1), int(peer_nz)))
+
+
+def fdtd_ipc_export(dev_ptr: int):
+    """(64-byte handle, offset) of a device address, to be opened by another process with fdtd_ipc_open."""
+    h = C.create_string_buffer(64)
+    off = C.c_int64(0)
+    _check(_L.fdtd_ipc_export(C.c_void_p(dev_ptr), h, C.byref(off)))
+    return h.raw, int(off.value)
+
+
+def fdtd_ipc_open(handle: bytes, offset: int) -> int:
+    p = C.c_void_p()
+    _check(_L.fdtd_ipc_open(C.create_string_buffer(handle, 64), int(offset), C.byref(p)))
+    return int(p.value)
+
+
+def fdtd_ipc_close(dev_ptr: int, offset: int) -> None:
+    _check(_L.fdtd_ipc_close(C.c_void_p(dev_ptr), int(offset)))
 
 
 def fdtd_flux(grid, det, phasor, axis, interpolate, flux, stream) -> None:

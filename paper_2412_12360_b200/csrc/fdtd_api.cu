@@ -738,6 +738,8 @@ static int forward_core(fdtd_grid *g, float *fields, const float *inv_eps, const
     if (g->path == FDTD_PATH_FUSED && !fused_call && g->desc.path == FDTD_PATH_FUSED)
         return fail(FDTD_EINVAL, "FDTD_PATH_FUSED takes at most 4 sources and 4 detectors per call (FDTD_PATH_AUTO falls back to the generic kernels)");
     if (g->sigma && recording) return fail(FDTD_ESTATE, "a lossy medium cannot be time-reversed (PAPER.md L84): use record = 0 or the checkpointed sweep, record = 3");
+    if (!fused_call && (g->peer[0][0].vol[0] || g->peer[0][1].vol[0]))
+        return fail(FDTD_ESTATE, "fdtd_forward: neighbours are attached (fdtd_halo_attach) but this call runs on the generic kernels");
     if (fused_call) {
         rc = fused_forward(g, fields, inv_eps, inv_mu, S, D, TD, total_freq, n_begin, n_end, n_total, recording, st);
         if (rc) return rc;
@@ -972,9 +974,13 @@ static int backward_core(fdtd_grid *g, float *fields, const float *inv_eps, cons
     // B0: seed cotangents
     const size_t vol = (size_t)G.nc * sizeof(float);
     g->bwd_pos = -1;
+    const bool fused_call = g->path == FDTD_PATH_FUSED && g->fused_backward_ready && (!g->sigma || !sweep_only || g->ck_e2);
     if (first) {
-        if (dL_dfields) CK(cudaMemcpyAsync(g->lam, dL_dfields, 6 * vol, cudaMemcpyDeviceToDevice, st));
-        else            CK(cudaMemsetAsync(g->lam, 0, 6 * vol, st));
+        // the fused sweep ping-pongs: the cotangent of state n lives in volume n&1, so the seed goes where state n_steps lives
+        if (fused_call && (rc = fused_alloc_backward(g))) return rc;
+        float *seed = fused_call ? fused_volume(g, fields, 1, n_steps) : g->lam;
+        if (dL_dfields) CK(cudaMemcpyAsync(seed, dL_dfields, 6 * vol, cudaMemcpyDeviceToDevice, st));
+        else            CK(cudaMemsetAsync(seed, 0, 6 * vol, st));
         for (int q = 0; q < 2; ++q)
             if ((rc = g->zero_psi(g->lpsiE[q], st)) || (rc = g->zero_psi(g->lpsiH[q], st))) return rc;
         if (dL_dinv_eps) CK(cudaMemsetAsync(dL_dinv_eps, 0, (G.aniso ? 3 : 1) * vol, st));
@@ -982,9 +988,10 @@ static int backward_core(fdtd_grid *g, float *fields, const float *inv_eps, cons
     }
     launch_set_step(g->d_step, std::max(n_hi - 1, 0), st);      // the first reverse step of the call reads slot 0
     const bool want_grad = dL_dinv_eps != nullptr;              // false: adjoint sweep only (B1, B2, B5)
-    const bool fused_call = g->path == FDTD_PATH_FUSED && g->fused_backward_ready && (!g->sigma || !sweep_only || g->ck_e2);
     if (g->sigma && want_grad) return fail(FDTD_ESTATE, "a lossy medium cannot be time-reversed (PAPER.md L84): its gradient comes from the checkpointed sweep (record = 3)");
 
+    if (!fused_call && (g->peer[1][0].vol[0] || g->peer[1][1].vol[0]))
+        return fail(FDTD_ESTATE, "fdtd_backward: neighbours are attached (fdtd_halo_attach) but this call runs on the generic kernels");
     if (fused_call) {
         // seeded_H: the H part of the seed can be non-zero (it is scaled by inv_mu for the sweep)
         rc = fused_backward(g, fields, inv_eps, inv_mu, S, D, TD, total_freq, n_hi, n_lo, n_total, dL_dinv_eps, dL_dfields != nullptr, st, dL_dinv_mu);
@@ -1104,6 +1111,84 @@ extern "C" int fdtd_halo_import(fdtd_grid *g, float *fields, int32_t which, int3
     const size_t plane = (size_t)G.nx * G.ny;
     for (int c = 0; c < 3; ++c)
         CK(cudaMemcpyAsync(vol + (3 + c) * G.nc + (size_t)k * plane, in + c * plane, plane * sizeof(float), cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
+    return FDTD_OK;
+}
+
+// N3 peer stores: the step kernels write the halo planes into the neighbour's volumes themselves
+extern "C" int fdtd_halo_volumes(fdtd_grid *g, float *fields, int32_t which, float **vol0, float **vol1)
+{
+    if (!g || !vol0 || !vol1) return fail(FDTD_EINVAL, "fdtd_halo_volumes: NULL argument");
+    if (which != 0 && which != 1) return fail(FDTD_EINVAL, "fdtd_halo_volumes: which must be 0 (fields) or 1 (cotangents)");
+    if (g->path != FDTD_PATH_FUSED) return fail(FDTD_ESTATE, "fdtd_halo_volumes: peer stores run on the fused kernels only (this grid: " + g->fused_why_not + ")");
+    if (which == 0 && !fields) return fail(FDTD_EINVAL, "fdtd_halo_volumes: fields is NULL");
+    if (which == 1) {
+        if (!g->fused_backward_ready) return fail(FDTD_ESTATE, "fdtd_halo_volumes: this grid's reverse sweep runs on the generic kernels");
+        int rc = g->ensure_backward_buffers();
+        if (rc) return rc;
+    }
+    *vol0 = fused_volume(g, fields, which, 0);
+    *vol1 = fused_volume(g, fields, which, 1);
+    return FDTD_OK;
+}
+
+extern "C" int fdtd_halo_attach(fdtd_grid *g, int32_t which, int32_t side, float *peer_vol0, float *peer_vol1, int32_t peer_nz)
+{
+    if (!g) return fail(FDTD_EINVAL, "fdtd_halo_attach: NULL grid");
+    if ((which != 0 && which != 1) || (side != 0 && side != 1)) return fail(FDTD_EINVAL, "fdtd_halo_attach: which and side must be 0 or 1");
+    fdtd_grid::PeerLink &L = g->peer[which][side];
+    if (!peer_vol0 && !peer_vol1) { L = fdtd_grid::PeerLink{}; return FDTD_OK; }      // detach
+    if (!peer_vol0 || !peer_vol1) return fail(FDTD_EINVAL, "fdtd_halo_attach: both volumes of the neighbour are needed");
+    if (g->path != FDTD_PATH_FUSED || (which == 1 && !g->fused_backward_ready))
+        return fail(FDTD_ESTATE, "fdtd_halo_attach: peer stores run on the fused kernels only");
+    if (side ? !g->desc.z_ghost_hi : !g->desc.z_ghost_lo) return fail(FDTD_EINVAL, "fdtd_halo_attach: the grid has no cut on that side");
+    if (peer_nz < 3) return fail(FDTD_EINVAL, "fdtd_halo_attach: peer_nz is the neighbour's local plane count (>= 3: a ghost plane, an owned plane, ...)");
+    // my lowest owned plane is the neighbour-below's ghost plane above (its last local plane); my highest owned plane is
+    // the neighbour-above's ghost plane below (its local plane 0)
+    const size_t plane = (size_t)g->G.nx * g->G.ny;
+    const long long pnc = (long long)peer_nz * (long long)plane;
+    const size_t k = side ? 0 : (size_t)peer_nz - 1;
+    L.vol[0] = peer_vol0 + 3 * pnc + k * plane;
+    L.vol[1] = peer_vol1 + 3 * pnc + k * plane;
+    L.nc = pnc;
+    return FDTD_OK;
+}
+
+// cudaIpc* behind the ABI, so that a binding needs no CUDA API of its own to hand a volume to another process
+extern "C" int fdtd_ipc_export(const void *dev_ptr, uint8_t handle[64], int64_t *offset)
+{
+    if (!dev_ptr || !handle || !offset) return fail(FDTD_EINVAL, "fdtd_ipc_export: NULL argument");
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "cudaIpcMemHandle_t is 64 bytes");
+    cudaIpcMemHandle_t h;
+    CK(cudaIpcGetMemHandle(&h, const_cast<void *>(dev_ptr)));
+    // the handle names the whole allocation; the pointer may sit inside it (a caching allocator's block)
+    typedef int (*range_fn)(unsigned long long *, size_t *, unsigned long long);      // CUresult cuMemGetAddressRange(CUdeviceptr *, size_t *, CUdeviceptr)
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuMemGetAddressRange", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn)
+        return fail(FDTD_ECUDA, "fdtd_ipc_export: cuMemGetAddressRange is not available");
+    unsigned long long base = 0;
+    size_t size = 0;
+    if (((range_fn)fn)(&base, &size, (unsigned long long)(uintptr_t)dev_ptr) != 0) return fail(FDTD_ECUDA, "fdtd_ipc_export: cuMemGetAddressRange failed");
+    memcpy(handle, &h, 64);
+    *offset = (int64_t)((unsigned long long)(uintptr_t)dev_ptr - base);
+    return FDTD_OK;
+}
+
+extern "C" int fdtd_ipc_open(const uint8_t handle[64], int64_t offset, void **dev_ptr)
+{
+    if (!handle || !dev_ptr || offset < 0) return fail(FDTD_EINVAL, "fdtd_ipc_open: bad argument");
+    cudaIpcMemHandle_t h;
+    memcpy(&h, handle, 64);
+    void *base = nullptr;
+    CK(cudaIpcOpenMemHandle(&base, h, cudaIpcMemLazyEnablePeerAccess));
+    *dev_ptr = (char *)base + offset;
+    return FDTD_OK;
+}
+
+extern "C" int fdtd_ipc_close(void *dev_ptr, int64_t offset)
+{
+    if (!dev_ptr) return FDTD_OK;
+    CK(cudaIpcCloseMemHandle((char *)dev_ptr - offset));
     return FDTD_OK;
 }
 

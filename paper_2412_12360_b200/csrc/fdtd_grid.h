@@ -80,6 +80,11 @@ struct fdtd_grid {
 
     FusedState *fused = nullptr;
 
+    // N3 peer stores (fdtd_halo_attach): [which: 0 primal, 1 cotangents][side: 0 below, 1 above].  vol[q] = component 3 of
+    // the plane of the neighbour's volume q that this grid's step kernel writes; nc = the neighbour's component stride
+    struct PeerLink { float *vol[2] = { nullptr, nullptr }; long long nc = 0; };
+    PeerLink peer[2][2];
+
     // per-kernel profiling (fdtd_set_profiling)
     enum ProfClass { PC_UPDATE_E, PC_UPDATE_H, PC_ADJ_H, PC_INV_H, PC_INV_E_GRAD, PC_ADJ_E,
                      PC_FUSED_FWD, PC_FUSED_BWD, PC_FUSED_INV, PC_RECORD, PC_INJECT, PC_SRC_DET, PC_OTHER, PC_COUNT };

@@ -79,6 +79,12 @@ struct StepParams {
     SourceDev src[MAX_SRC];
     DetectorDev det[MAX_DET];
     const float *cs;
+    // N3, peer stores (fdtd_halo_attach): the H-type result of my lowest / highest owned plane also goes straight into the
+    // ghost plane of the neighbouring slab's volume, and my own ghost planes on attached sides are left to the neighbour
+    int peer_on;                   // bit 0: a neighbour below is attached, bit 1: above
+    int own_lo, own_hi;            // lowest / highest owned plane (local index)
+    float *peer[2][2];             // [side][volume]: component 3 of the neighbour's ghost plane in its volume 0 / 1
+    long long peer_nc[2];          // the neighbour's component stride
 };
 
 template <int TX4_, int TY_>
@@ -701,7 +707,19 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_step(const __grid_constant__ 
                     }
                 }
                 float *o = dst + 3 * nc + offm;
-                stg4(o, h2x); stg4(o + nc, h2y); stg4(o + 2 * nc, h2z);
+                if (!P.peer_on) {
+                    stg4(o, h2x); stg4(o + nc, h2y); stg4(o + 2 * nc, h2z);
+                } else {
+                    // N3 with attached neighbours: a ghost plane's H-type components are written by the neighbour's kernel
+                    // (nothing of mine may land on them in the same step); my boundary planes go to the neighbour as well
+                    const bool ghost = ((P.peer_on & 1) && km1 == 0) || ((P.peer_on & 2) && km1 == G.nz - 1);
+                    if (!ghost) { stg4(o, h2x); stg4(o + nc, h2y); stg4(o + 2 * nc, h2z); }
+                    for (int sd = 0; sd < 2; ++sd) {
+                        if (!((P.peer_on >> sd) & 1) || km1 != (sd ? P.own_hi : P.own_lo)) continue;
+                        float *q = P.peer[sd][par ^ 1] + own_xy;
+                        stg4(q, h2x); stg4(q + P.peer_nc[sd], h2y); stg4(q + 2 * P.peer_nc[sd], h2z);
+                    }
+                }
                 if (!ADJ && km1 >= P.dHl && km1 < P.dHh) detect4(P, n, 1, det_mask(P, km1, false), h2x, h2y, h2z, i, j, km1);
             }
             if (ADJ) { cZx = Zx; cZy = Zy; }
@@ -1841,6 +1859,18 @@ void join_side(fdtd_grid *g, cudaStream_t cs, int n_side)
     }
 }
 
+// N3: the attached neighbours of the volumes this sweep writes (which = 0 primal, 1 cotangents)
+void set_peers(const fdtd_grid *g, int which, StepParams &P)
+{
+    P.peer_on = 0;
+    P.own_lo = g->desc.z_ghost_lo; P.own_hi = g->G.nz - 1 - g->desc.z_ghost_hi;
+    for (int sd = 0; sd < 2; ++sd) {
+        const fdtd_grid::PeerLink &L = g->peer[which][sd];
+        P.peer[sd][0] = L.vol[0]; P.peer[sd][1] = L.vol[1]; P.peer_nc[sd] = L.nc;
+        if (L.vol[0]) P.peer_on |= 1 << sd;
+    }
+}
+
 struct FwdCtx {
     fdtd_grid *g; StepParams P; bool recording; float *A; float *B; int n_steps;
     const std::vector<TimeDetDev> *TD; const float *ie; const float *im;
@@ -1976,6 +2006,8 @@ int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float
     for (size_t q = 0; q < S.size(); ++q) P.src[q] = S[q];
     for (size_t q = 0; q < D.size(); ++q) P.det[q] = D[q];
     P.cs = g->d_cs;
+    set_peers(g, 0, P);
+    if (P.peer_on && n_count > 1) return fdtd_fail(FDTD_EINVAL, "with attached neighbours (fdtd_halo_attach) a range call advances one step: the slabs synchronise after every step");
     P.sEl = P.sHl = P.dEl = P.dHl = 1 << 30; P.sEh = P.sHh = P.dEh = P.dHh = -1;
     for (const SourceDev &q : S) {
         if (q.comp < 3) { P.sEl = std::min(P.sEl, q.lo[2]); P.sEh = std::max(P.sEh, q.hi[2]); }
@@ -2026,11 +2058,10 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     if ((rc = fused_alloc_backward(g))) return rc;
     if ((rc = build_maps(g, 1, g->lam, F->lamB, inv_eps, st))) return rc;
     // with inv_mu the sweep runs on Lambda_H = im lamH (see k_step); fdtd_backward scales the result back
-    if (first && inv_mu && seeded_H) launch_scale_H(g->G, g->lam, inv_mu, false, st);
-    if (first && (n_steps & 1)) {
-        cudaError_t e = cudaMemcpyAsync(F->lamB, g->lam, vol6, cudaMemcpyDeviceToDevice, st);
-        if (e != cudaSuccess) { (void)cudaGetLastError(); return fdtd_fail(FDTD_ECUDA, cudaGetErrorString(e)); }
-    }
+    // (the seed sits in the volume of state n_steps already -- fdtd_api.cu seeds fused_volume(.., 1, n_steps) -- so that nothing
+    // is written to the other volume before the first step: with N3 peer stores a neighbour's first step may already have
+    // stored its boundary plane there)
+    if (first && inv_mu && seeded_H) launch_scale_H(g->G, (n_steps & 1) ? F->lamB : g->lam, inv_mu, false, st);
     const bool want_grad = dL_dinv_eps != nullptr;      // false: adjoint sweep only, the primal volumes are not touched
     // N4: dL/d inv_mu is formed in the inverse step from lamH' of volume (n+1)&1, which adjoint step n-1 overwrites: the
     // inverse step of step n must then run before adjoint step n-1 (no pipelined sweep)
@@ -2078,6 +2109,8 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
         }
     }
     P.cs = g->d_cs;
+    set_peers(g, 1, P);
+    if (P.peer_on && n_count > 1) return fdtd_fail(FDTD_EINVAL, "with attached neighbours (fdtd_halo_attach) a range call advances one step: the slabs synchronise after every step");
     int n_adj = 0;
     for (const DetectorDev &dt : D) if (dt.phasor) ++n_adj;
     std::string key(fused_inv ? "fB" : "fb");

@@ -191,6 +191,18 @@ class SlabRunner:
         if self.slab.ghost_hi:
             B.fdtd_halo_import(g.h, self.fields, which, n, 1, self.recv_above if from_above is None else from_above, g.stream())
 
+    # ---- peer stores: the step kernel writes the neighbour's ghost planes itself (include/fdtd.h "Peer stores") ----
+    def volumes(self, which: int):
+        """Device addresses of my two ping-pong volumes (which = 0 fields, 1 cotangents)."""
+        return self.B.fdtd_halo_volumes(self.grid.h, self.fields, which)
+
+    def attach(self, which: int, side: int, peer_vols, peer_nz: int):
+        self.B.fdtd_halo_attach(self.grid.h, which, side, peer_vols[0], peer_vols[1], peer_nz)
+
+    def detach(self, which: int):
+        for side in (0, 1):
+            self.B.fdtd_halo_attach(self.grid.h, which, side, None, None, 0)
+
     # ---- backward -----------------------------------------------------------------------------------------
     def set_cotangents(self, dL_dphasor_global=None, dL_dfields_global=None):
         """Cotangents given on the GLOBAL boxes / volume (device tensors); this slab takes its planes, ghosts included."""
@@ -215,9 +227,33 @@ class SlabRunner:
                                    self.lam0, self.grid.stream())
 
 
-def run_slabs_lockstep(runners: List["SlabRunner"], n_total: int, direction: str = "forward"):
+def attach_neighbours_local(runners: List["SlabRunner"], which: int):
+    """Slabs of one process: every runner gets its neighbours' volumes (plain device pointers)."""
+    vols = [r.volumes(which) for r in runners]
+    for q, r in enumerate(runners):
+        if r.slab.ghost_lo:
+            r.attach(which, 0, vols[q - 1], runners[q - 1].slab.nz)
+        if r.slab.ghost_hi:
+            r.attach(which, 1, vols[q + 1], runners[q + 1].slab.nz)
+
+
+def run_slabs_lockstep(runners: List["SlabRunner"], n_total: int, direction: str = "forward", peer: bool = False):
     """Advances the slabs of one process in lock step, one exchange per step (the single-device form of the protocol
-    of include/fdtd.h; across processes every rank runs the same loop with exchange_halos_dist in the middle)."""
+    of include/fdtd.h; across processes every rank runs the same loop with exchange_halos_dist in the middle).
+    peer = True: no exchange at all -- the step kernels store their boundary planes into the neighbours' volumes, and the
+    one stream all slabs share orders step n of every slab before step n+1 of any."""
+    which = 0 if direction == "forward" else 1
+    if peer:
+        attach_neighbours_local(runners, which)
+        try:
+            for n in (range(n_total) if direction == "forward" else range(n_total - 1, -1, -1)):
+                for r in runners:
+                    r.forward_steps(n, n + 1) if direction == "forward" else r.backward_steps(n + 1, n)
+        finally:
+            for r in runners:
+                r.detach(which)
+        return
+
     def swap(which, n):
         for r in runners:
             r.export_halos(which, n)
@@ -238,10 +274,74 @@ def run_slabs_lockstep(runners: List["SlabRunner"], n_total: int, direction: str
                 swap(1, n)
 
 
-def run_slab_distributed(runner: "SlabRunner", n_total: int, direction: str = "forward", group=None):
-    """The same loop for one rank of a torch.distributed job (one slab per GPU, NCCL point-to-point)."""
+class PeerLinks:
+    """One rank's view of its neighbours' volumes in a torch.distributed job: every rank publishes the CUDA IPC handles of
+    its two ping-pong volumes (fdtd_ipc_export), opens its neighbours' (fdtd_ipc_open: plain stores over NVLink when the
+    neighbour is another GPU) and attaches them (fdtd_halo_attach).  Host logic only."""
+
+    def __init__(self, runner: "SlabRunner", which: int, group=None):
+        B, slab = runner.B, runner.slab
+        self.runner, self.which, self.opened = runner, which, []
+        mine = [B.fdtd_ipc_export(v) for v in runner.volumes(which)]
+        table = [None] * slab.world
+        dist.all_gather_object(table, (slab.nz, mine), group=group)
+        for side, nb in ((0, slab.rank - 1), (1, slab.rank + 1)):
+            if not (slab.ghost_lo if side == 0 else slab.ghost_hi):
+                continue
+            nz_nb, handles = table[nb]
+            ptrs = [B.fdtd_ipc_open(h, off) for h, off in handles]
+            self.opened += [(p, off) for p, (_, off) in zip(ptrs, handles)]
+            runner.attach(which, side, ptrs, nz_nb)
+
+    def close(self):
+        self.runner.detach(self.which)
+        for p, off in self.opened:
+            self.runner.B.fdtd_ipc_close(p, off)
+        self.opened = []
+
+
+def neighbour_tokens(slab: ZSlab, token, scratch, group=None):
+    """The ordering that is left of the exchange with peer stores: a one-element message to and from every neighbour,
+    enqueued behind this rank's step (stream-ordered over NCCL; blocking over gloo).  When it has completed, the
+    neighbours have finished the step whose stores landed in my ghost planes, and they do not start the next one --
+    which stores into the volume my step was reading -- before I have finished mine."""
+    ops = []
+    for has, nb, q in ((slab.ghost_lo, slab.rank - 1, 0), (slab.ghost_hi, slab.rank + 1, 1)):
+        if has:
+            ops.append(dist.P2POp(dist.isend, token, nb, group))
+            ops.append(dist.P2POp(dist.irecv, scratch[q], nb, group))
+    if ops:
+        for req in dist.batch_isend_irecv(ops):
+            req.wait()
+
+
+def run_slab_distributed(runner: "SlabRunner", n_total: int, direction: str = "forward", group=None, peer: bool = False,
+                         host_sync: bool = False):
+    """The same loop for one rank of a torch.distributed job (one slab per GPU, NCCL point-to-point).
+    peer = True: the step kernels store the halo planes into the neighbours' volumes (PeerLinks); per step only a token
+    travels.  host_sync = True (tokens on CPU tensors, e.g. a gloo group): the stream is synchronised before the token
+    is sent -- for groups whose point-to-point calls are not stream-ordered."""
     which = 0 if direction == "forward" else 1
     steps = range(n_total) if direction == "forward" else range(n_total - 1, -1, -1)
+    if peer:
+        links = PeerLinks(runner, which, group)
+        dev = "cpu" if host_sync else "cuda"
+        token, scratch = torch.ones(1, device=dev), torch.zeros(2, 1, device=dev)
+        try:
+            dist.barrier(group=group)                  # every rank has attached before any kernel stores
+            for n in steps:
+                if direction == "forward":
+                    runner.forward_steps(n, n + 1)
+                else:
+                    runner.backward_steps(n + 1, n)
+                if host_sync:
+                    torch.cuda.current_stream().synchronize()
+                neighbour_tokens(runner.slab, token, scratch, group)
+            torch.cuda.current_stream().synchronize()
+            dist.barrier(group=group)                  # nobody closes a mapping a neighbour's kernel may still write
+        finally:
+            links.close()
+        return
     for n in steps:
         if direction == "forward":
             runner.forward_steps(n, n + 1)

@@ -46,11 +46,11 @@ def _single(B, w, path, n, dLf_fn=None):
     return res
 
 
-def _slabs(B, w, path, n, cuts, ref):
+def _slabs(B, w, path, n, cuts, ref, peer=False):
     import torch
     slabs = sharding.z_slabs(w.nz, len(cuts) + 1, w.pml_cells, cuts)
     runners = [sharding.SlabRunner(B, w, s, n, record=1, path=path) for s in slabs]
-    sharding.run_slabs_lockstep(runners, n, "forward")
+    sharding.run_slabs_lockstep(runners, n, "forward", peer=peer)
     torch.cuda.synchronize()
     fields = np.zeros_like(ref["fields"])
     phasors = [np.zeros_like(p) for p in ref["phasors"]]
@@ -61,7 +61,7 @@ def _slabs(B, w, path, n, cuts, ref):
             phasors[idx][:, :, sl] = P.cpu().numpy()
     for r in runners:
         r.set_cotangents(ref["dLp"], ref["dLf"])
-    sharding.run_slabs_lockstep(runners, n, "backward")
+    sharding.run_slabs_lockstep(runners, n, "backward", peer=peer)
     torch.cuda.synchronize()
     grad, lam0 = np.zeros_like(ref["grad"]), np.zeros_like(ref["lam0"])
     for r in runners:
@@ -99,6 +99,62 @@ def test_z_slabs_in_lock_step_reproduce_the_single_grid_bitwise(B, path_name, cu
     err = float(np.max(np.abs(got["grad"].astype(np.float64) - ref["grad"])) / np.max(np.abs(ref["grad"])))
     print(f"z slabs {cuts} {path_name}: fields, phasors, lam0 bit-identical; gradient differs by {err:.1e} of its maximum")
     assert err <= 1e-6
+
+
+@pytest.mark.parametrize("n", [37, 24])
+@pytest.mark.parametrize("cuts", [(21,), (9, 20, 35)])
+def test_peer_stores_replace_the_halo_exchange_bitwise(B, cuts, n):
+    """include/fdtd.h "Peer stores": with the neighbours attached (fdtd_halo_volumes / fdtd_halo_attach) the fused step
+    kernels write their boundary planes into the neighbours' ghost planes themselves and there is no fdtd_halo_export /
+    _import at all; the slabs still reproduce the undivided grid bit for bit (fields, phasors, cotangent of state 0) in
+    both directions, for an odd and an even step count (the seed of the reverse sweep lands in either volume of the
+    ping-pong).  Same workload as the exchange test above."""
+    path = B.FDTD_PATH_FUSED
+    w = wl.c3_mini(n_steps=n, kappa_max=3.0, alpha_max=0.05)
+    rng = np.random.default_rng(3)
+    w.meta["inv_mu"] = (1.0 / (1.0 + 0.5 * rng.random((w.nz, w.ny, w.nx), dtype=np.float32))).astype(np.float32)
+    w.sources.append(wl.Source(3, (20, 12, 22), (60, 40, 23), (0.3 * wl.gaussian_sine(n, 12, 5, 11)).astype(np.float32)))
+    w.detectors.append(wl.Detector((1 << 1) | (1 << 5), (10, 10, 18), (70, 40, 24), [wl.omega_ppw(12)]))
+    ref = _single(B, w, path, n)
+    got = _slabs(B, w, path, n, list(cuts), ref, peer=True)
+    assert got["paths"] == {path}
+    assert np.max(np.abs(ref["grad"])) > 0 and np.max(np.abs(ref["lam0"])) > 0
+    assert np.array_equal(got["fields"], ref["fields"])
+    for P, Pr in zip(got["phasors"], ref["phasors"]):
+        assert np.max(np.abs(Pr)) > 0 and np.array_equal(P, Pr)
+    assert np.array_equal(got["lam0"], ref["lam0"])
+    err = float(np.max(np.abs(got["grad"].astype(np.float64) - ref["grad"])) / np.max(np.abs(ref["grad"])))
+    print(f"peer stores, z slabs {cuts}, {n} steps: fields, phasors, lam0 bit-identical; gradient differs by {err:.1e} of its maximum")
+    assert err <= 1e-6
+
+
+def test_peer_store_argument_checks(B):
+    import torch
+    n = 4
+    w = wl.c3_mini(n_steps=n)
+    slabs = sharding.z_slabs(w.nz, 2, w.pml_cells, [21])
+    r0, r1 = (sharding.SlabRunner(B, w, s, n, record=1, path=B.FDTD_PATH_FUSED) for s in slabs)
+    v1 = r1.volumes(0)
+    assert v1[0] == r1.fields.data_ptr() and v1[1] != 0 and v1[1] != v1[0]
+    with pytest.raises(B.FdtdError) as e:          # slab 0 has no cut below
+        r0.attach(0, 0, v1, r1.slab.nz)
+    assert e.value.code == B.FDTD_EINVAL
+    with pytest.raises(B.FdtdError) as e:          # one volume only
+        B.fdtd_halo_attach(r0.grid.h, 0, 1, v1[0], None, r1.slab.nz)
+    assert e.value.code == B.FDTD_EINVAL
+    r0.attach(0, 1, v1, r1.slab.nz)
+    with pytest.raises(B.FdtdError) as e:          # attached: one step per call
+        r0.forward_steps(0, 2)
+    assert e.value.code == B.FDTD_EINVAL
+    r0.detach(0)
+    r0.forward_steps(0, 2)                          # detached: any range again
+    torch.cuda.synchronize()
+    g = sharding.SlabRunner(B, w, slabs[0], n, record=1, path=B.FDTD_PATH_GENERIC)
+    with pytest.raises(B.FdtdError) as e:          # the generic kernels have no peer stores
+        g.volumes(0)
+    assert e.value.code == B.FDTD_ESTATE
+    for r in (r0, r1, g):
+        r.close()
 
 
 def test_subgrid_descriptor_checks(B):
