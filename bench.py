@@ -246,15 +246,22 @@ def run_decomposed(args, rank, world, local_rank, barrier):
     seed = torch.zeros((6, w.nz, w.ny, w.nx), dtype=torch.float32, device=dev)
     seed[1, w.nz // 2] = 1.0                                  # a fixed cotangent seed for the adjoint sweep
 
+    # --halo peer: the fused step kernels store the halo planes into the neighbours' volumes (CUDA IPC mappings, opened
+    # once per direction outside the timed region); --halo nccl: plane copies + NCCL point-to-point between the launches
+    peer = args.halo == "peer" and r.grid.info().path == B.FDTD_PATH_FUSED
+    links = {0: sharding.PeerLinks(r, 0) if peer else False}
+
     def fwd():
         r.fields.zero_()
         for P in r.phasors:
             P.zero_()
-        sharding.run_slab_distributed(r, T, "forward")
+        sharding.run_slab_distributed(r, T, "forward", peer=links[0])
 
     def adj():
         r.set_cotangents(None, seed)
-        sharding.run_slab_distributed(r, T, "backward")
+        if 1 not in links:
+            links[1] = sharding.PeerLinks(r, 1) if peer else False
+        sharding.run_slab_distributed(r, T, "backward", peer=links[1])
 
     def timed(fn, reps):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -279,11 +286,15 @@ def run_decomposed(args, rank, world, local_rank, barrier):
                           "value": cs * args.steps / (ms_f * 1e-3) / 1e6, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                           "warmup": args.warmup, "ms_per_step": ms_f / args.steps, "higher_is_better": True, "scaling": "strong",
                           "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-                          "config": workload_config(w, {"time_steps": T, "parallelism": f"z slabs x{world}, one halo exchange per time step "
-                                                        "(3 planes of nx*ny floats per neighbour and direction)",
+                          "config": workload_config(w, {"time_steps": T, "parallelism": f"z slabs x{world}, " + (
+                                                            "halo planes stored by the step kernels into the neighbours' volumes (peer stores), one token per neighbour and step"
+                                                            if peer else "one halo exchange per time step (3 planes of nx*ny floats per neighbour and direction, NCCL point-to-point)"),
                                                         "slab_planes": slab.nz, "path": {1: "generic", 2: "fused"}[info.path]}),
                           "adjoint_sweep": {"value": cs * max(1, min(args.steps, 3)) / (ms_a * 1e-3) / 1e6, "unit": UNIT},
                           "gpu_launches": int(info.kernel_launches)}))
+    for l in links.values():
+        if l:
+            l.close()
     r.close()
 
 
@@ -419,6 +430,9 @@ def main():
                     help="z: ONE grid cut into z slabs, one per rank (SURVEY 8(e) / 8(f) N3; sharding.run_slab_distributed, NCCL "
                          "point-to-point halo exchange once per time step); times the forward pass and the adjoint sweep of the whole "
                          "grid (strong scaling).  Not measured on more than one GPU in this build: see DESIGN.md section 10")
+    ap.add_argument("--halo", default="peer", choices=["peer", "nccl"],
+                    help="--decompose z: peer = the fused step kernels store the halo planes into the neighbours' volumes (include/fdtd.h "
+                         "\"Peer stores\"; falls back to nccl on a grid that runs the generic kernels); nccl = plane copies + NCCL point-to-point")
     ap.add_argument("--recorder-fp16", action="store_true",
                     help="SURVEY 8(f) N1: store the interface record as fp16 (FDTD_FLAG_RECORDER_FP16; an approximation, off by default)")
     ap.add_argument("--record", default="", choices=["", "1", "2", "both"],

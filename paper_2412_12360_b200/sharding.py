@@ -282,6 +282,8 @@ class PeerLinks:
     def __init__(self, runner: "SlabRunner", which: int, group=None):
         B, slab = runner.B, runner.slab
         self.runner, self.which, self.opened = runner, which, []
+        if slab.world == 1:                                  # the whole grid on one rank: no neighbour, nothing to map
+            return
         mine = [B.fdtd_ipc_export(v) for v in runner.volumes(which)]
         table = [None] * slab.world
         dist.all_gather_object(table, (slab.nz, mine), group=group)
@@ -318,17 +320,21 @@ def neighbour_tokens(slab: ZSlab, token, scratch, group=None):
 def run_slab_distributed(runner: "SlabRunner", n_total: int, direction: str = "forward", group=None, peer: bool = False,
                          host_sync: bool = False):
     """The same loop for one rank of a torch.distributed job (one slab per GPU, NCCL point-to-point).
-    peer = True: the step kernels store the halo planes into the neighbours' volumes (PeerLinks); per step only a token
-    travels.  host_sync = True (tokens on CPU tensors, e.g. a gloo group): the stream is synchronised before the token
+    peer = True (or a PeerLinks built for this direction, to be reused over several runs): the step kernels store the halo
+    planes into the neighbours' volumes; per step only a token travels.  host_sync = True (tokens on CPU tensors, e.g. a gloo group): the stream is synchronised before the token
     is sent -- for groups whose point-to-point calls are not stream-ordered."""
     which = 0 if direction == "forward" else 1
     steps = range(n_total) if direction == "forward" else range(n_total - 1, -1, -1)
     if peer:
-        links = PeerLinks(runner, which, group)
+        own_links = not isinstance(peer, PeerLinks)         # peer = a PeerLinks of this direction: reused, the caller closes it
+        links = PeerLinks(runner, which, group) if own_links else peer
+        assert links.which == which
         dev = "cpu" if host_sync else "cuda"
         token, scratch = torch.ones(1, device=dev), torch.zeros(2, 1, device=dev)
         try:
-            dist.barrier(group=group)                  # every rank has attached before any kernel stores
+            multi = runner.slab.world > 1
+            if multi:
+                dist.barrier(group=group)              # every rank has attached before any kernel stores
             for n in steps:
                 if direction == "forward":
                     runner.forward_steps(n, n + 1)
@@ -338,9 +344,11 @@ def run_slab_distributed(runner: "SlabRunner", n_total: int, direction: str = "f
                     torch.cuda.current_stream().synchronize()
                 neighbour_tokens(runner.slab, token, scratch, group)
             torch.cuda.current_stream().synchronize()
-            dist.barrier(group=group)                  # nobody closes a mapping a neighbour's kernel may still write
+            if multi:
+                dist.barrier(group=group)              # nobody closes a mapping a neighbour's kernel may still write
         finally:
-            links.close()
+            if own_links:
+                links.close()
         return
     for n in steps:
         if direction == "forward":

@@ -128,6 +128,58 @@ def test_peer_stores_replace_the_halo_exchange_bitwise(B, cuts, n):
     assert err <= 1e-6
 
 
+def _ipc_worker(rank, world, port, out):
+    """One rank = one process with its own CUDA context on cuda:0: its slab, the neighbour's volumes opened from CUDA IPC
+    handles, tokens over gloo with a stream synchronisation before each (no kernel waits for another process's kernel)."""
+    import os
+    import torch
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        from paper_2412_12360_b200 import binding as B
+        torch.cuda.set_device(0)
+        n = 9
+        w = wl.c3_mini(n_steps=n, kappa_max=3.0, alpha_max=0.05)
+        ref = _single(B, w, B.FDTD_PATH_FUSED, n)
+        slab = sharding.z_slabs(w.nz, world, w.pml_cells, [21])[rank]
+        r = sharding.SlabRunner(B, w, slab, n, record=1, path=B.FDTD_PATH_FUSED)
+        sharding.run_slab_distributed(r, n, "forward", peer=True, host_sync=True)
+        torch.cuda.synchronize()
+        own = slab.owned_local()
+        ok_f = bool(np.array_equal(r.fields[:, own].cpu().numpy(), ref["fields"][:, slab.k_lo:slab.k_hi]))
+        ok_p = all(np.array_equal(P.cpu().numpy(), ref["phasors"][idx][:, :, sl]) for (idx, d, sl), P in zip(r.det_fwd, r.phasors))
+        r.set_cotangents(ref["dLp"], ref["dLf"])
+        sharding.run_slab_distributed(r, n, "backward", peer=True, host_sync=True)
+        torch.cuda.synchronize()
+        ok_l = bool(np.array_equal(r.lam0[:, own].cpu().numpy(), ref["lam0"][:, slab.k_lo:slab.k_hi]))
+        eg = float(np.max(np.abs(r.grad[own].cpu().numpy().astype(np.float64) - ref["grad"][slab.k_lo:slab.k_hi])) / np.max(np.abs(ref["grad"])))
+        out[rank] = (ok_f, ok_p, ok_l, eg, float(np.max(np.abs(ref["lam0"]))))
+        r.close()
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.timeout(600)
+def test_peer_stores_across_two_processes_through_cuda_ipc(B):
+    """The cross-process form of the peer stores (sharding.PeerLinks: fdtd_ipc_export / fdtd_ipc_open, then
+    fdtd_halo_attach) with two processes on the one device there is: each rank's kernels store into memory the OTHER
+    process allocated.  Bit-identical to the undivided grid again."""
+    import os
+    import torch.multiprocessing as mp
+    world, port = 2, 35500 + os.getpid() % 2000
+    with mp.Manager() as m:
+        out = m.dict()
+        mp.spawn(_ipc_worker, args=(world, port, out), nprocs=world, join=True)
+        res = dict(out)
+    assert set(res) == {0, 1}
+    for rank in range(world):
+        ok_f, ok_p, ok_l, eg, lmax = res[rank]
+        assert lmax > 0 and ok_f and ok_p and ok_l, (rank, res[rank])
+        assert eg <= 1e-6
+
+
 def test_peer_store_argument_checks(B):
     import torch
     n = 4

@@ -116,3 +116,33 @@ def test_halo_exchange_over_three_gloo_ranks():
     assert res[0] == (-1.0, 11.0)
     assert res[1] == (2.0, 21.0)
     assert res[2] == (12.0, -1.0)
+
+
+def _token_worker(rank, world, port, out):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    from paper_2412_12360_b200 import sharding
+    slab = sharding.z_slabs(30, world, 4)[rank]
+    token, scratch = torch.zeros(1), torch.full((2, 1), -1.0)
+    seen = []
+    for step in range(4):                                  # the token of step n must meet the neighbours' token of step n
+        token.fill_(100.0 * step + rank)
+        sharding.neighbour_tokens(slab, token, scratch)
+        seen.append((float(scratch[0, 0]), float(scratch[1, 0])))
+    out[rank] = seen
+    dist.destroy_process_group()
+
+
+def test_neighbour_tokens_over_three_gloo_ranks():
+    """What is left of the halo exchange with peer stores (include/fdtd.h "Peer stores"): one token to and from every
+    neighbour per step, paired step by step."""
+    world, port = 3, 33500 + os.getpid() % 2000
+    with mp.Manager() as m:
+        out = m.dict()
+        mp.spawn(_token_worker, args=(world, port, out), nprocs=world, join=True)
+        res = dict(out)
+    for step in range(4):
+        assert res[0][step] == (-1.0, 100.0 * step + 1)       # no neighbour below
+        assert res[1][step] == (100.0 * step + 0, 100.0 * step + 2)
+        assert res[2][step] == (100.0 * step + 1, -1.0)
