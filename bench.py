@@ -240,11 +240,59 @@ def run_decomposed(args, rank, world, local_rank, barrier):
     from paper_2412_12360_b200 import sharding
     w = make_workload(args)                                   # the same problem on every rank: each takes its slab
     T = args.time_steps or min(w.n_steps, 200)
-    slab = sharding.z_slabs(w.nz, world, w.pml_cells)[rank]
-    r = sharding.SlabRunner(B, w, slab, T, record=0)
     dev = torch.device("cuda", local_rank)
     seed = torch.zeros((6, w.nz, w.ny, w.nx), dtype=torch.float32, device=dev)
     seed[1, w.nz // 2] = 1.0                                  # a fixed cotangent seed for the adjoint sweep
+    if world == 1 and args.slabs > 1:
+        # one process, one device: the slabs in lock step on one stream (what the exchange costs in launches and copies,
+        # not a scaling figure: the slabs run one after the other)
+        runners = [sharding.SlabRunner(B, w, s, T, record=0) for s in sharding.z_slabs(w.nz, args.slabs, w.pml_cells)]
+        peer = args.halo == "peer" and all(q.grid.info().path == B.FDTD_PATH_FUSED for q in runners)
+
+        def fwd1():
+            for q in runners:
+                q.fields.zero_()
+                for P in q.phasors:
+                    P.zero_()
+            sharding.run_slabs_lockstep(runners, T, "forward", peer=peer)
+
+        def adj1():
+            for q in runners:
+                q.want_grad = False
+                q.set_cotangents(None, seed)
+            sharding.run_slabs_lockstep(runners, T, "backward", peer=peer)
+
+        def timed1(fn, reps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            for _ in range(reps):
+                fn()
+            e1.record()
+            torch.cuda.synchronize()
+            return e0.elapsed_time(e1)
+
+        for _ in range(args.warmup):
+            fwd1()
+        ms_f = timed1(fwd1, args.steps)
+        adj1()
+        ms_a = timed1(adj1, max(1, min(args.steps, 3)))
+        cs = w.cells * T
+        print(json.dumps({"metric": "Yee cell-updates/s, forward pass of ONE grid cut into z slabs run in lock step on ONE device",
+                          "value": cs * args.steps / (ms_f * 1e-3) / 1e6, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+                          "warmup": args.warmup, "ms_per_step": ms_f / args.steps, "higher_is_better": True, "scaling": "none (one device)",
+                          "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                          "config": workload_config(w, {"time_steps": T, "parallelism": f"{args.slabs} z slabs on one device, " + (
+                                                            "peer stores (no exchange launches)" if peer else "plane copies between the steps (fdtd_halo_export / _import)"),
+                                                        "slab_planes": [q.slab.nz for q in runners]}),
+                          "us_per_time_step": {"forward": 1e3 * ms_f / args.steps / T, "adjoint": 1e3 * ms_a / max(1, min(args.steps, 3)) / T},
+                          "adjoint_sweep": {"value": cs * max(1, min(args.steps, 3)) / (ms_a * 1e-3) / 1e6, "unit": UNIT},
+                          "gpu_launches": int(sum(q.grid.info().kernel_launches for q in runners))}))
+        for q in runners:
+            q.close()
+        return
+    slab = sharding.z_slabs(w.nz, world, w.pml_cells)[rank]
+    r = sharding.SlabRunner(B, w, slab, T, record=0)
 
     # --halo peer: the fused step kernels store the halo planes into the neighbours' volumes (CUDA IPC mappings, opened
     # once per direction outside the timed region); --halo nccl: plane copies + NCCL point-to-point between the launches
@@ -430,6 +478,9 @@ def main():
                     help="z: ONE grid cut into z slabs, one per rank (SURVEY 8(e) / 8(f) N3; sharding.run_slab_distributed, NCCL "
                          "point-to-point halo exchange once per time step); times the forward pass and the adjoint sweep of the whole "
                          "grid (strong scaling).  Not measured on more than one GPU in this build: see DESIGN.md section 10")
+    ap.add_argument("--slabs", type=int, default=0,
+                    help="--decompose z on ONE rank: cut the grid into this many z slabs and run them in lock step on the one device "
+                         "(sharding.run_slabs_lockstep): the cost of the exchange in launches and copies, with --halo peer | nccl (= plane copies)")
     ap.add_argument("--halo", default="peer", choices=["peer", "nccl"],
                     help="--decompose z: peer = the fused step kernels store the halo planes into the neighbours' volumes (include/fdtd.h "
                          "\"Peer stores\"; falls back to nccl on a grid that runs the generic kernels); nccl = plane copies + NCCL point-to-point")
