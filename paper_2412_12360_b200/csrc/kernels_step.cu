@@ -1483,7 +1483,10 @@ int fused_setup(fdtd_grid *g)
     // ---- segments ---------------------------------------------------------------------------------------------------
     const int ntx = (G.nx + F->TX - 1) / F->TX, nty = (G.ny + F->TY - 1) / F->TY;
     const long long total = (long long)ntx * nty * G.nz;
-    int n_cta = (int)std::min<long long>(n_sm, std::max<long long>(1, total / 6));
+    // one CTA per SM as soon as each gets two planes: a small grid is bound by the planes a CTA marches one after the other
+    // (~2 us each, latency), not by the prologue plane a shorter run adds (64^3, C2 / C5: 6 planes per run 17.5 / 19.1 us per
+    // forward / adjoint step, 4.3 planes per run on all 148 SMs 14.3 / 15.6 us; a second wave of CTAs: 18 / 22 us)
+    int n_cta = (int)std::min<long long>(n_sm, std::max<long long>(1, total / 2));
     if (const char *e = getenv("FDTD_NCTA")) n_cta = std::max(1, atoi(e));
     double wy = 1.0, wz = 0.8;                   // starting point of the cost model (measured on C3); see calibrate()
     if (const char *e = getenv("FDTD_WY")) wy = atof(e);
@@ -1535,7 +1538,7 @@ int fused_setup(fdtd_grid *g)
             // tiles start at row lo_y (their first halo row is lo_y - 1) and at column x0
             const int ntx = (nx_i + ib->TX - 1) / ib->TX, nty = (ny_i + ib->TY - 1) / ib->TY;
             const long long itotal = (long long)ntx * nty * nz_i;
-            int in_cta = (int)std::min<long long>(n_sm, std::max<long long>(1, itotal / 6));
+            int in_cta = (int)std::min<long long>(n_sm, std::max<long long>(1, itotal / 2));      // (64^3: 19.6 -> 14.8 us)
             if (const char *e = getenv("FDTD_INV_NCTA")) in_cta = std::max(1, atoi(e));
             std::vector<Segment> isegs;
             std::vector<int> ibeg;
