@@ -63,4 +63,9 @@ def test_null_arguments_are_einval():
     assert b._L.fdtd_forward(None, None, None, None, None, 0, None, 0, 0, None) == b.FDTD_EINVAL
     assert b._L.fdtd_get_info(None, None) == b.FDTD_EINVAL
     assert b._L.fdtd_destroy(None) == b.FDTD_OK
+    assert b._L.fdtd_halo_attach(None, 0, 0, None, None, 0) == b.FDTD_EINVAL
+    assert b._L.fdtd_halo_volumes(None, None, 0, None, None) == b.FDTD_EINVAL
+    assert b._L.fdtd_ipc_export(None, None, None) == b.FDTD_EINVAL
+    assert b._L.fdtd_ipc_open(None, 0, None) == b.FDTD_EINVAL
+    assert b._L.fdtd_ipc_close(None, 0) == b.FDTD_OK
     assert "NULL" in b.fdtd_last_error() or b.fdtd_last_error()
