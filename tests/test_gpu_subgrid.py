@@ -128,6 +128,25 @@ def test_peer_stores_replace_the_halo_exchange_bitwise(B, cuts, n):
     assert err <= 1e-6
 
 
+def test_c3_full_size_slabs_with_peer_stores_bitwise(B):
+    """C3 at its full size (200^3, d = 12: the 200 x 7 tiles and the calibrated lock-step partition of the bench, per slab) cut
+    at z = 87 and z = 140 -- through the design region -- with the halo planes stored by the step kernels: fields, phasors and
+    the cotangent of state 0 bit-identical to the undivided grid after 25 steps and 25 reverse steps."""
+    n = 25
+    w = wl.c3(n_steps=n)
+    ref = _single(B, w, B.FDTD_PATH_FUSED, n)
+    got = _slabs(B, w, B.FDTD_PATH_FUSED, n, [87, 140], ref, peer=True)
+    assert got["paths"] == {B.FDTD_PATH_FUSED}
+    assert np.max(np.abs(ref["fields"])) > 0 and np.max(np.abs(ref["lam0"])) > 0
+    assert np.array_equal(got["fields"], ref["fields"])
+    for P, Pr in zip(got["phasors"], ref["phasors"]):
+        assert np.array_equal(P, Pr)
+    assert np.array_equal(got["lam0"], ref["lam0"])
+    gmax = float(np.max(np.abs(ref["grad"])))
+    if gmax > 0:
+        assert float(np.max(np.abs(got["grad"].astype(np.float64) - ref["grad"]))) <= 1e-6 * gmax
+
+
 def _ipc_worker(rank, world, port, out):
     """One rank = one process with its own CUDA context on cuda:0: its slab, the neighbour's volumes opened from CUDA IPC
     handles, tokens over gloo with a stream synchronisation before each (no kernel waits for another process's kernel)."""
