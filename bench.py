@@ -247,7 +247,9 @@ def run_decomposed(args, rank, world, local_rank, barrier):
         # one process, one device: the slabs in lock step on one stream (what the exchange costs in launches and copies,
         # not a scaling figure: the slabs run one after the other)
         runners = [sharding.SlabRunner(B, w, s, T, record=0) for s in sharding.z_slabs(w.nz, args.slabs, w.pml_cells)]
-        peer = args.halo == "peer" and all(q.grid.info().path == B.FDTD_PATH_FUSED for q in runners)
+        peer = args.halo in ("peer", "flags") and all(q.grid.info().path == B.FDTD_PATH_FUSED for q in runners)
+        if peer and args.halo == "flags":
+            peer = "flags"                                    # + the wait / signal kernels (met at once on one stream)
 
         def fwd1():
             for q in runners:
@@ -283,7 +285,7 @@ def run_decomposed(args, rank, world, local_rank, barrier):
                           "warmup": args.warmup, "ms_per_step": ms_f / args.steps, "higher_is_better": True, "scaling": "none (one device)",
                           "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                           "config": workload_config(w, {"time_steps": T, "parallelism": f"{args.slabs} z slabs on one device, " + (
-                                                            "peer stores (no exchange launches)" if peer else "plane copies between the steps (fdtd_halo_export / _import)"),
+                                                            ("peer stores + device-side ordering kernels" if peer == "flags" else "peer stores (no exchange launches)") if peer else "plane copies between the steps (fdtd_halo_export / _import)"),
                                                         "slab_planes": [q.slab.nz for q in runners]}),
                           "us_per_time_step": {"forward": 1e3 * ms_f / args.steps / T, "adjoint": 1e3 * ms_a / max(1, min(args.steps, 3)) / T},
                           "adjoint_sweep": {"value": cs * max(1, min(args.steps, 3)) / (ms_a * 1e-3) / 1e6, "unit": UNIT},
@@ -296,8 +298,10 @@ def run_decomposed(args, rank, world, local_rank, barrier):
 
     # --halo peer: the fused step kernels store the halo planes into the neighbours' volumes (CUDA IPC mappings, opened
     # once per direction outside the timed region); --halo nccl: plane copies + NCCL point-to-point between the launches
-    peer = args.halo == "peer" and r.grid.info().path == B.FDTD_PATH_FUSED
-    links = {0: sharding.PeerLinks(r, 0) if peer else False}
+    # --halo flags: peer stores + the device-side ordering kernels (no token either; ranges of 64 steps per call)
+    peer = args.halo in ("peer", "flags") and r.grid.info().path == B.FDTD_PATH_FUSED
+    use_flags = args.halo == "flags"
+    links = {0: sharding.PeerLinks(r, 0, flags=use_flags) if peer else False}
 
     def fwd():
         r.fields.zero_()
@@ -308,7 +312,7 @@ def run_decomposed(args, rank, world, local_rank, barrier):
     def adj():
         r.set_cotangents(None, seed)
         if 1 not in links:
-            links[1] = sharding.PeerLinks(r, 1) if peer else False
+            links[1] = sharding.PeerLinks(r, 1, flags=use_flags) if peer else False
         sharding.run_slab_distributed(r, T, "backward", peer=links[1])
 
     def timed(fn, reps):
@@ -335,7 +339,7 @@ def run_decomposed(args, rank, world, local_rank, barrier):
                           "warmup": args.warmup, "ms_per_step": ms_f / args.steps, "higher_is_better": True, "scaling": "strong",
                           "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                           "config": workload_config(w, {"time_steps": T, "parallelism": f"z slabs x{world}, " + (
-                                                            "halo planes stored by the step kernels into the neighbours' volumes (peer stores), one token per neighbour and step"
+                                                            "halo planes stored by the step kernels into the neighbours' volumes (peer stores), " + ("ordered by flags on the device" if use_flags else "one token per neighbour and step")
                                                             if peer else "one halo exchange per time step (3 planes of nx*ny floats per neighbour and direction, NCCL point-to-point)"),
                                                         "slab_planes": slab.nz, "path": {1: "generic", 2: "fused"}[info.path]}),
                           "adjoint_sweep": {"value": cs * max(1, min(args.steps, 3)) / (ms_a * 1e-3) / 1e6, "unit": UNIT},
@@ -481,9 +485,11 @@ def main():
     ap.add_argument("--slabs", type=int, default=0,
                     help="--decompose z on ONE rank: cut the grid into this many z slabs and run them in lock step on the one device "
                          "(sharding.run_slabs_lockstep): the cost of the exchange in launches and copies, with --halo peer | nccl (= plane copies)")
-    ap.add_argument("--halo", default="peer", choices=["peer", "nccl"],
+    ap.add_argument("--halo", default="peer", choices=["peer", "flags", "nccl"],
                     help="--decompose z: peer = the fused step kernels store the halo planes into the neighbours' volumes (include/fdtd.h "
-                         "\"Peer stores\"; falls back to nccl on a grid that runs the generic kernels); nccl = plane copies + NCCL point-to-point")
+                         "\"Peer stores\"; falls back to nccl on a grid that runs the generic kernels), one token per neighbour and step; "
+                         "flags = peer stores ordered on the device (wait / signal kernels beside the step kernel, no token; one GPU per rank only); "
+                         "nccl = plane copies + NCCL point-to-point")
     ap.add_argument("--recorder-fp16", action="store_true",
                     help="SURVEY 8(f) N1: store the interface record as fp16 (FDTD_FLAG_RECORDER_FP16; an approximation, off by default)")
     ap.add_argument("--record", default="", choices=["", "1", "2", "both"],

@@ -392,14 +392,33 @@ FDTD_API int fdtd_halo_import(fdtd_grid *grid, float *fields, int32_t which, int
  *   fdtd_halo_volumes of the same `which`, peer_nz its local plane count (ghosts included).  Both NULL detaches.  The
  *   grid must have a cut on that side and run the fused kernels (ESTATE otherwise); the neighbour must attach this
  *   grid in turn (a ghost plane on an attached side is written by the neighbour only).  While a neighbour is attached
- *   a range call must advance exactly one step (EINVAL otherwise) and the caller orders the steps of the slabs as
- *   stated above; a call that would run on the generic kernels (more than 4 sources / detectors) returns ESTATE.
+ *   without flags (below) a range call must advance exactly one step (EINVAL otherwise) and the caller orders the steps
+ *   of the slabs as stated above; a call that would run on the generic kernels (more than 4 sources / detectors) returns ESTATE.
  * fdtd_ipc_export / fdtd_ipc_open / fdtd_ipc_close: cudaIpcGetMemHandle / OpenMemHandle / CloseMemHandle behind this ABI,
  *   so that ranks can hand their volumes to each other without a CUDA binding of their own.  handle: HOST, 64 bytes;
  *   offset: the pointer's offset inside the allocation the handle names (a caching allocator hands out interior
  *   pointers).  fdtd_ipc_open returns the pointer itself (base + offset), valid in the calling process until
  *   fdtd_ipc_close(ptr, offset).  Volumes obtained from cudaMalloc (PyTorch's default allocator, this library) qualify;
  *   stream-ordered pools and expandable segments do not (ECUDA). */
+/* Device-side ordering (csrc/halo_sync.cu): with flags attached on every attached side the slabs order their steps
+ * themselves -- before a step a one-thread kernel waits (ld.acquire.sys) until the slab's own flags show the state it is
+ * about to read, after a step another publishes the state reached in the neighbours' flags (st.release.sys) -- both as
+ * graph nodes beside the step kernel, so a range call may advance ANY number of steps and replays without the host; no
+ * token, no NCCL on the data path.  A wait passes when the flag shows the state wanted or the next one in the direction
+ * of time (a neighbour may be one state ahead, never two), so the value a previous run left behind does not pass: runs
+ * have at least 3 steps (EINVAL otherwise).  The slabs must then run concurrently (one GPU each): on ONE device the
+ * calls have to be issued step by step in slab order on one stream, so that every wait finds its flag already set.
+ * fdtd_halo_flags: this grid's two flags of `which` (DEVICE, int32[2]: [0] written by the neighbour below, [1] by the
+ *   neighbour above), allocated by the first call; owned by the grid.
+ * fdtd_halo_attach_flags: peer_flags = the fdtd_halo_flags pointer of the neighbour on `side` (same-process pointer or
+ *   opened from its IPC handle); needs fdtd_halo_attach on that side first and this grid's own fdtd_halo_flags (ESTATE
+ *   otherwise); NULL detaches the flag (fdtd_halo_attach(NULL, NULL) detaches both).
+ * fdtd_halo_sync_error: a wait gives up after FDTD_HALO_TIMEOUT_MS (environment, default 10000) instead of hanging the
+ *   device and raises a flag; this call reads and clears it (synchronous copy; *timed_out = 0: all waits were met,
+ *   else 1 + the state index that never came).  The results of such a run are invalid. */
+FDTD_API int fdtd_halo_flags(fdtd_grid *grid, int32_t which, int32_t **flags);
+FDTD_API int fdtd_halo_attach_flags(fdtd_grid *grid, int32_t which, int32_t side, int32_t *peer_flags);
+FDTD_API int fdtd_halo_sync_error(fdtd_grid *grid, int32_t *timed_out);
 FDTD_API int fdtd_halo_volumes(fdtd_grid *grid, float *fields, int32_t which, float **vol0, float **vol1);
 FDTD_API int fdtd_halo_attach(fdtd_grid *grid, int32_t which, int32_t side, float *peer_vol0, float *peer_vol1, int32_t peer_nz);
 FDTD_API int fdtd_ipc_export(const void *dev_ptr, uint8_t handle[64], int64_t *offset);

@@ -74,7 +74,7 @@ EXPORTS = ("fdtd_grad_rho", "fdtd_set_profiling", "fdtd_get_profile", "fdtd_crea
            "fdtd_get_info", "fdtd_version", "fdtd_forward_host", "fdtd_backward_host", "fdtd_debug_partition",
            "fdtd_forward_td", "fdtd_backward_td", "fdtd_flux", "fdtd_flux_vjp", "fdtd_tfsf_plane",
            "fdtd_forward_range", "fdtd_backward_range", "fdtd_halo_export", "fdtd_halo_import",
-           "fdtd_halo_volumes", "fdtd_halo_attach", "fdtd_ipc_export", "fdtd_ipc_open", "fdtd_ipc_close", "fdtd_backward_mu", "fdtd_set_conductivity", "fdtd_probe_bandwidth", "fdtd_flux_static")
+           "fdtd_halo_volumes", "fdtd_halo_attach", "fdtd_halo_flags", "fdtd_halo_attach_flags", "fdtd_halo_sync_error", "fdtd_ipc_export", "fdtd_ipc_open", "fdtd_ipc_close", "fdtd_backward_mu", "fdtd_set_conductivity", "fdtd_probe_bandwidth", "fdtd_flux_static")
 
 
 def _load():
@@ -112,6 +112,12 @@ def _load():
     L.fdtd_halo_volumes.argtypes = [vp, vp, i32, C.POINTER(vp), C.POINTER(vp)]
     L.fdtd_halo_attach.restype = C.c_int
     L.fdtd_halo_attach.argtypes = [vp, i32, i32, vp, vp, i32]
+    L.fdtd_halo_flags.restype = C.c_int
+    L.fdtd_halo_flags.argtypes = [vp, i32, C.POINTER(vp)]
+    L.fdtd_halo_attach_flags.restype = C.c_int
+    L.fdtd_halo_attach_flags.argtypes = [vp, i32, i32, vp]
+    L.fdtd_halo_sync_error.restype = C.c_int
+    L.fdtd_halo_sync_error.argtypes = [vp, C.POINTER(i32)]
     L.fdtd_ipc_export.restype = C.c_int
     L.fdtd_ipc_export.argtypes = [vp, C.c_char_p, C.POINTER(C.c_int64)]
     L.fdtd_ipc_open.restype = C.c_int
@@ -291,6 +297,23 @@ def fdtd_halo_volumes(grid, fields, which):
 def fdtd_halo_attach(grid, which, side, peer_vol0, peer_vol1, peer_nz) -> None:
     """peer_vol0 / peer_vol1: device addresses (int) of the neighbour's fdtd_halo_volumes, or None / None to detach."""
     _check(_L.fdtd_halo_attach(grid, int(which), int(side), C.c_void_p(peer_vol0), C.c_void_p(peer_vol1), int(peer_nz)))
+
+
+def fdtd_halo_flags(grid, which) -> int:
+    """Device address (int) of this grid's two ordering flags of `which`."""
+    p = C.c_void_p()
+    _check(_L.fdtd_halo_flags(grid, int(which), C.byref(p)))
+    return int(p.value)
+
+
+def fdtd_halo_attach_flags(grid, which, side, peer_flags) -> None:
+    _check(_L.fdtd_halo_attach_flags(grid, int(which), int(side), C.c_void_p(peer_flags)))
+
+
+def fdtd_halo_sync_error(grid) -> int:
+    v = C.c_int32(0)
+    _check(_L.fdtd_halo_sync_error(grid, C.byref(v)))
+    return int(v.value)
 
 
 def fdtd_ipc_export(dev_ptr: int):

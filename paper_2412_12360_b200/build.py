@@ -14,7 +14,7 @@ from pathlib import Path
 HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 LIB = HERE / "libfdtd_b200.so"
-SOURCES = ["fdtd_api.cu", "kernels_generic.cu", "kernels_step.cu", "kernels_n2.cu", "probe.cu", "flux_static.cu"]
+SOURCES = ["fdtd_api.cu", "kernels_generic.cu", "kernels_step.cu", "kernels_n2.cu", "probe.cu", "flux_static.cu", "halo_sync.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--use-local-env"]
 

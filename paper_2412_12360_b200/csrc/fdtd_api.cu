@@ -1136,7 +1136,7 @@ extern "C" int fdtd_halo_attach(fdtd_grid *g, int32_t which, int32_t side, float
     if (!g) return fail(FDTD_EINVAL, "fdtd_halo_attach: NULL grid");
     if ((which != 0 && which != 1) || (side != 0 && side != 1)) return fail(FDTD_EINVAL, "fdtd_halo_attach: which and side must be 0 or 1");
     fdtd_grid::PeerLink &L = g->peer[which][side];
-    if (!peer_vol0 && !peer_vol1) { L = fdtd_grid::PeerLink{}; return FDTD_OK; }      // detach
+    if (!peer_vol0 && !peer_vol1) { L = fdtd_grid::PeerLink{}; return FDTD_OK; }      // detach (the flag too)
     if (!peer_vol0 || !peer_vol1) return fail(FDTD_EINVAL, "fdtd_halo_attach: both volumes of the neighbour are needed");
     if (g->path != FDTD_PATH_FUSED || (which == 1 && !g->fused_backward_ready))
         return fail(FDTD_ESTATE, "fdtd_halo_attach: peer stores run on the fused kernels only");
@@ -1150,6 +1150,48 @@ extern "C" int fdtd_halo_attach(fdtd_grid *g, int32_t which, int32_t side, float
     L.vol[0] = peer_vol0 + 3 * pnc + k * plane;
     L.vol[1] = peer_vol1 + 3 * pnc + k * plane;
     L.nc = pnc;
+    return FDTD_OK;
+}
+
+// device-side ordering of the slabs (halo_sync.cu)
+extern "C" int fdtd_halo_flags(fdtd_grid *g, int32_t which, int32_t **flags)
+{
+    if (!g || !flags) return fail(FDTD_EINVAL, "fdtd_halo_flags: NULL argument");
+    if (which != 0 && which != 1) return fail(FDTD_EINVAL, "fdtd_halo_flags: which must be 0 (fields) or 1 (cotangents)");
+    if (g->path != FDTD_PATH_FUSED) return fail(FDTD_ESTATE, "fdtd_halo_flags: peer stores run on the fused kernels only");
+    if (!g->d_hflags) {
+        int rc = g->alloc((void **)&g->d_hflags, 5 * sizeof(int));       // [which][side] + the error flag
+        if (rc) return rc;
+        CK(cudaMemset(g->d_hflags, 0xff, 4 * sizeof(int)));               // -1: no state reached yet
+        CK(cudaMemset(g->d_hflags + 4, 0, sizeof(int)));
+        g->d_herr = g->d_hflags + 4;
+    }
+    *flags = g->d_hflags + which * 2;
+    return FDTD_OK;
+}
+
+extern "C" int fdtd_halo_attach_flags(fdtd_grid *g, int32_t which, int32_t side, int32_t *peer_flags)
+{
+    if (!g) return fail(FDTD_EINVAL, "fdtd_halo_attach_flags: NULL grid");
+    if ((which != 0 && which != 1) || (side != 0 && side != 1)) return fail(FDTD_EINVAL, "fdtd_halo_attach_flags: which and side must be 0 or 1");
+    fdtd_grid::PeerLink &L = g->peer[which][side];
+    if (!peer_flags) { L.flag = nullptr; return FDTD_OK; }
+    if (!L.vol[0]) return fail(FDTD_ESTATE, "fdtd_halo_attach_flags: attach the neighbour's volumes first (fdtd_halo_attach)");
+    if (!g->d_hflags) return fail(FDTD_ESTATE, "fdtd_halo_attach_flags: call fdtd_halo_flags first (the neighbour needs this grid's flags too)");
+    // the neighbour below keeps the flag I write in its slot "above" (1); the neighbour above in its slot "below" (0)
+    L.flag = peer_flags + (side == 0 ? 1 : 0);
+    return FDTD_OK;
+}
+
+extern "C" int fdtd_halo_sync_error(fdtd_grid *g, int32_t *timed_out)
+{
+    if (!g || !timed_out) return fail(FDTD_EINVAL, "fdtd_halo_sync_error: NULL argument");
+    *timed_out = 0;
+    if (!g->d_herr) return FDTD_OK;
+    int v = 0;
+    CK(cudaMemcpy(&v, g->d_herr, sizeof(int), cudaMemcpyDeviceToHost));
+    if (v) CK(cudaMemset(g->d_herr, 0, sizeof(int)));
+    *timed_out = v;
     return FDTD_OK;
 }
 

@@ -82,8 +82,11 @@ struct fdtd_grid {
 
     // N3 peer stores (fdtd_halo_attach): [which: 0 primal, 1 cotangents][side: 0 below, 1 above].  vol[q] = component 3 of
     // the plane of the neighbour's volume q that this grid's step kernel writes; nc = the neighbour's component stride
-    struct PeerLink { float *vol[2] = { nullptr, nullptr }; long long nc = 0; };
+    struct PeerLink { float *vol[2] = { nullptr, nullptr }; long long nc = 0; int *flag = nullptr; };
     PeerLink peer[2][2];
+    // device-side ordering of the slabs (halo_sync.cu): my flags [which][side] (written by that neighbour), PeerLink.flag =
+    // the flag of mine in the neighbour's set; herr: raised by a wait that gave up
+    int *d_hflags = nullptr, *d_herr = nullptr;
 
     // per-kernel profiling (fdtd_set_profiling)
     enum ProfClass { PC_UPDATE_E, PC_UPDATE_H, PC_ADJ_H, PC_INV_H, PC_INV_E_GRAD, PC_ADJ_E,
@@ -122,6 +125,11 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
                    bool seeded_H, cudaStream_t st, float *dL_dinv_mu = nullptr);
 // the volume that holds state n of the fused path's ping-pong: which = 0 primal (fields / second buffer), 1 cotangents
 float *fused_volume(fdtd_grid *g, float *fields, int which, int n);
+
+namespace fdtd {
+void launch_halo_signal(int *f_lo, int *f_hi, const int *slot, int add, cudaStream_t st);
+void launch_halo_wait(const int *f_lo, const int *f_hi, const int *slot, int add, int skip, int dir, int *err, cudaStream_t st);
+}
 
 // RAII span: brackets the launches made in its lifetime with two events when profiling is on
 struct ProfScope {

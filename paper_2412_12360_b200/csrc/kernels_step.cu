@@ -1874,9 +1874,31 @@ void set_peers(const fdtd_grid *g, int which, StepParams &P)
     }
 }
 
+// N3, device-side ordering of the slabs (halo_sync.cu): active when every attached side has a flag
+struct HaloSync {                                   // (no padding: it is part of the graph key)
+    const int *mine[2] = { nullptr, nullptr };      // my flags, written by the neighbour below / above
+    int *theirs[2] = { nullptr, nullptr };          // my flag in the set of the neighbour below / above
+    int *err = nullptr;
+    long long active = 0;
+};
+HaloSync halo_sync_of(const fdtd_grid *g, int which, int peer_on)
+{
+    HaloSync H;
+    if (!peer_on || !g->d_hflags) return H;
+    for (int sd = 0; sd < 2; ++sd) {
+        if (!((peer_on >> sd) & 1)) continue;
+        if (!g->peer[which][sd].flag) return HaloSync{};      // a side without a flag: the host orders the steps
+        H.mine[sd] = g->d_hflags + which * 2 + sd;
+        H.theirs[sd] = g->peer[which][sd].flag;
+    }
+    H.active = 1; H.err = g->d_herr;
+    return H;
+}
+
 struct FwdCtx {
     fdtd_grid *g; StepParams P; bool recording; float *A; float *B; int n_steps;
     const std::vector<TimeDetDev> *TD; const float *ie; const float *im;
+    HaloSync hs;
 };
 // forward step n; with the recorder on, k_record_pipe runs beside it on a side stream: both only read buffer n&1
 // (pre-step H of step n -> rec[n], E' of step n-1 -> rec[n-1]); the step after next overwrites that buffer, so the
@@ -1888,6 +1910,8 @@ void enqueue_fwd(void *vctx, cudaStream_t cs)
     FusedState *F = g->fused;
     StepParams Q = c->P;
     Q.step = g->step_in(); Q.step_next = g->step_out(); Q.step_delta = 1;
+    // N3: the neighbours must have reached state n (their step n-1 stored my ghost planes) before anything reads buffer n&1
+    if (c->hs.active) launch_halo_wait(c->hs.mine[0], c->hs.mine[1], g->step_in(), 0, 0, 1, c->hs.err, cs);
     ProfScope p(g, fdtd_grid::PC_FUSED_FWD, cs);
     if (c->recording) {
         fork_side(g, cs, 1);
@@ -1895,6 +1919,7 @@ void enqueue_fwd(void *vctx, cudaStream_t cs)
     }
     F->tile->launch_fwd(Q, F->n_cta, F->smem, cs);
     if (c->recording) join_side(g, cs, 1);
+    if (c->hs.active) launch_halo_signal(c->hs.theirs[0], c->hs.theirs[1], g->step_in(), 1, cs);      // state n+1 reached
     // N2: time-domain detectors on the state step n just wrote (volume (n+1)&1)
     for (const TimeDetDev &q : *c->TD) launch_time_detect(g->G, c->A, c->B, 1, c->ie, c->im, q, g->red, g->step_in(), cs);
     // N4, replay of a segment in the checkpointed reverse sweep: D = dE'/d inv_eps of step n from the two volumes
@@ -1910,6 +1935,7 @@ struct BwdCtx {
     fdtd_grid *g; StepParams P; InvParams I; bool fused_inv; bool fused_det; bool pipelined; bool want_grad; float *bufB; float *fields; const float *ie; const float *im; float *grad; float *lamA; float *lamB;
     const std::vector<SourceDev> *S; const std::vector<DetectorDev> *D; int total_freq;
     const std::vector<TimeDetDev> *TD; float *grad_mu;
+    HaloSync hs; int n_total;
 };
 // Reverse step n.  One kernel after the other: B1 (detector cotangents into the volume about to be read), B2+B5
 // (fused adjoint step), face injection, then the primal inverse step B3+B4 with lamE' taken from the volume the
@@ -1928,6 +1954,8 @@ void enqueue_bwd(void *vctx, cudaStream_t cs)
     const Dims &G = g->G;
     StepParams Q = c->P;
     Q.step = g->step_in(); Q.step_next = g->step_out(); Q.step_delta = -1;
+    // N3: reverse step n reads the cotangents of state n+1; the seed (state n_total) is the caller's
+    if (c->hs.active) launch_halo_wait(c->hs.mine[0], c->hs.mine[1], g->step_in(), 1, c->n_total, -1, c->hs.err, cs);
     if (c->pipelined) {
         ProfScope p(g, fdtd_grid::PC_FUSED_BWD, cs);
         const int n_side = G.d > 0 ? 2 : 1;
@@ -1938,6 +1966,7 @@ void enqueue_bwd(void *vctx, cudaStream_t cs)
         if (G.d > 0) launch_inject_pipe(G, g->R, c->fields, c->bufB, g->rec, g->step_in(), g->side_stream[1]);
         F->tile->launch_adj(Q, F->n_adj, F->smem, cs);
         join_side(g, cs, n_side);
+        if (c->hs.active) launch_halo_signal(c->hs.theirs[0], c->hs.theirs[1], g->step_in(), 0, cs);      // state n reached
         ++g->enq_step; ++g->enq_inv;
         return;
     }
@@ -1960,6 +1989,7 @@ void enqueue_bwd(void *vctx, cudaStream_t cs)
       F->tile->launch_adj(Q, F->n_adj, F->smem, cs);
       ++g->enq_step;
       if (side_inject) join_side(g, cs, 1); }
+    if (c->hs.active) launch_halo_signal(c->hs.theirs[0], c->hs.theirs[1], g->step_in(), 0, cs);          // state n reached
     // N4, checkpointed reverse sweep: g += lamE' . D with lamE' in the volume the adjoint step just wrote (n&1), or, for a
     // lossy medium (the volume holds Ca lamE'), in the scratch volumes
     if (g->ck_gradhook) { ProfScope p(g, fdtd_grid::PC_INV_E_GRAD, cs);
@@ -2010,7 +2040,10 @@ int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float
     for (size_t q = 0; q < D.size(); ++q) P.det[q] = D[q];
     P.cs = g->d_cs;
     set_peers(g, 0, P);
-    if (P.peer_on && n_count > 1) return fdtd_fail(FDTD_EINVAL, "with attached neighbours (fdtd_halo_attach) a range call advances one step: the slabs synchronise after every step");
+    ctx.hs = halo_sync_of(g, 0, P.peer_on);
+    if (ctx.hs.active && n_total < 3) return fdtd_fail(FDTD_EINVAL, "device-side ordering of the slabs (fdtd_halo_attach_flags) needs runs of at least 3 steps");
+    if (P.peer_on && n_count > 1 && !ctx.hs.active)
+        return fdtd_fail(FDTD_EINVAL, "with attached neighbours (fdtd_halo_attach) and no flags (fdtd_halo_attach_flags) a range call advances one step: the caller orders the slabs after every step");
     P.sEl = P.sHl = P.dEl = P.dHl = 1 << 30; P.sEh = P.sHh = P.dEh = P.dHh = -1;
     for (const SourceDev &q : S) {
         if (q.comp < 3) { P.sEl = std::min(P.sEl, q.lo[2]); P.sEh = std::max(P.sEh, q.hi[2]); }
@@ -2028,7 +2061,8 @@ int fused_forward(fdtd_grid *g, float *fields, const float *inv_eps, const float
     int n_store = 0;
     if (g->ck_store) { n_store = 1; for (const SourceDev &q : S) if (q.comp < 3) ++n_store; }
     key.push_back((char)n_store);
-    rc = fdtd_run_steps_fwd(g, key, n_count, 1 + (recording ? 1 : 0) + (int)TD.size() + n_store, st, enqueue_fwd, &ctx);
+    key.append((const char *)&ctx.hs, sizeof(ctx.hs));
+    rc = fdtd_run_steps_fwd(g, key, n_count, 1 + (recording ? 1 : 0) + (int)TD.size() + n_store + (ctx.hs.active ? 2 : 0), st, enqueue_fwd, &ctx);
     if (rc) return rc;
     if (n_end != n_total || g->replaying) return FDTD_OK;      // (replaying: the checkpointed reverse sweep leaves the state in its volume)
     if (recording) {      // E' of the last step; the p-th step of the call read counter slot p&1, so the count sits in slot n_count&1
@@ -2113,7 +2147,11 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     }
     P.cs = g->d_cs;
     set_peers(g, 1, P);
-    if (P.peer_on && n_count > 1) return fdtd_fail(FDTD_EINVAL, "with attached neighbours (fdtd_halo_attach) a range call advances one step: the slabs synchronise after every step");
+    ctx.hs = halo_sync_of(g, 1, P.peer_on);
+    if (ctx.hs.active && n_total < 3) return fdtd_fail(FDTD_EINVAL, "device-side ordering of the slabs (fdtd_halo_attach_flags) needs runs of at least 3 steps");
+    ctx.n_total = n_total;
+    if (P.peer_on && n_count > 1 && !ctx.hs.active)
+        return fdtd_fail(FDTD_EINVAL, "with attached neighbours (fdtd_halo_attach) and no flags (fdtd_halo_attach_flags) a range call advances one step: the caller orders the slabs after every step");
     int n_adj = 0;
     for (const DetectorDev &dt : D) if (dt.phasor) ++n_adj;
     std::string key(fused_inv ? "fB" : "fb");
@@ -2127,7 +2165,9 @@ int fused_backward(fdtd_grid *g, float *fields, const float *inv_eps, const floa
     if (!D.empty()) key.append((const char *)D.data(), D.size() * sizeof(DetectorDev));
     if (!TD.empty()) key.append((const char *)TD.data(), TD.size() * sizeof(TimeDetDev));
     const int n_inj = g->G.d > 0 ? 1 : 0;
-    const int launches = (int)TD.size() + (g->ck_gradhook ? 1 : 0) + (!want_grad ? 1 + (fused_det ? 0 : n_adj)
+    key.append((const char *)&ctx.hs, sizeof(ctx.hs));
+    key.append((const char *)&ctx.n_total, sizeof(ctx.n_total));
+    const int launches = (ctx.hs.active ? 2 : 0) + (int)TD.size() + (g->ck_gradhook ? 1 : 0) + (!want_grad ? 1 + (fused_det ? 0 : n_adj)
                          : (fused_inv ? 2 + (fused_det ? 0 : n_adj) + n_inj : 3 + (fused_det ? 0 : n_adj) + (int)S.size() + n_inj));
     rc = fdtd_run_steps_bwd(g, key, n_count, launches, st, enqueue_bwd, &ctx);
     if (rc || !pipelined) return rc;

@@ -199,6 +199,13 @@ class SlabRunner:
     def attach(self, which: int, side: int, peer_vols, peer_nz: int):
         self.B.fdtd_halo_attach(self.grid.h, which, side, peer_vols[0], peer_vols[1], peer_nz)
 
+    def flags(self, which: int) -> int:
+        """Device address of my two ordering flags (include/fdtd.h "Device-side ordering")."""
+        return self.B.fdtd_halo_flags(self.grid.h, which)
+
+    def attach_flags(self, which: int, side: int, peer_flags):
+        self.B.fdtd_halo_attach_flags(self.grid.h, which, side, peer_flags)
+
     def detach(self, which: int):
         for side in (0, 1):
             self.B.fdtd_halo_attach(self.grid.h, which, side, None, None, 0)
@@ -227,24 +234,29 @@ class SlabRunner:
                                    self.lam0, self.grid.stream())
 
 
-def attach_neighbours_local(runners: List["SlabRunner"], which: int):
-    """Slabs of one process: every runner gets its neighbours' volumes (plain device pointers)."""
+def attach_neighbours_local(runners: List["SlabRunner"], which: int, flags: bool = False):
+    """Slabs of one process: every runner gets its neighbours' volumes (plain device pointers) and, with flags = True,
+    their ordering flags."""
     vols = [r.volumes(which) for r in runners]
+    fl = [r.flags(which) for r in runners] if flags else None
     for q, r in enumerate(runners):
-        if r.slab.ghost_lo:
-            r.attach(which, 0, vols[q - 1], runners[q - 1].slab.nz)
-        if r.slab.ghost_hi:
-            r.attach(which, 1, vols[q + 1], runners[q + 1].slab.nz)
+        for side, nb, has in ((0, q - 1, r.slab.ghost_lo), (1, q + 1, r.slab.ghost_hi)):
+            if has:
+                r.attach(which, side, vols[nb], runners[nb].slab.nz)
+                if flags:
+                    r.attach_flags(which, side, fl[nb])
 
 
 def run_slabs_lockstep(runners: List["SlabRunner"], n_total: int, direction: str = "forward", peer: bool = False):
     """Advances the slabs of one process in lock step, one exchange per step (the single-device form of the protocol
     of include/fdtd.h; across processes every rank runs the same loop with exchange_halos_dist in the middle).
     peer = True: no exchange at all -- the step kernels store their boundary planes into the neighbours' volumes, and the
-    one stream all slabs share orders step n of every slab before step n+1 of any."""
+    one stream all slabs share orders step n of every slab before step n+1 of any.  peer = "flags": the same with the
+    device-side ordering kernels in the stream as well (every wait finds its flag already set: on one device the slabs
+    cannot run side by side, see include/fdtd.h)."""
     which = 0 if direction == "forward" else 1
     if peer:
-        attach_neighbours_local(runners, which)
+        attach_neighbours_local(runners, which, flags=(peer == "flags"))
         try:
             for n in (range(n_total) if direction == "forward" else range(n_total - 1, -1, -1)):
                 for r in runners:
@@ -279,12 +291,14 @@ class PeerLinks:
     its two ping-pong volumes (fdtd_ipc_export), opens its neighbours' (fdtd_ipc_open: plain stores over NVLink when the
     neighbour is another GPU) and attaches them (fdtd_halo_attach).  Host logic only."""
 
-    def __init__(self, runner: "SlabRunner", which: int, group=None):
+    def __init__(self, runner: "SlabRunner", which: int, group=None, flags: bool = False):
         B, slab = runner.B, runner.slab
-        self.runner, self.which, self.opened = runner, which, []
+        self.runner, self.which, self.opened, self.flags = runner, which, [], flags
         if slab.world == 1:                                  # the whole grid on one rank: no neighbour, nothing to map
             return
         mine = [B.fdtd_ipc_export(v) for v in runner.volumes(which)]
+        if flags:
+            mine.append(B.fdtd_ipc_export(runner.flags(which)))
         table = [None] * slab.world
         dist.all_gather_object(table, (slab.nz, mine), group=group)
         for side, nb in ((0, slab.rank - 1), (1, slab.rank + 1)):
@@ -293,7 +307,9 @@ class PeerLinks:
             nz_nb, handles = table[nb]
             ptrs = [B.fdtd_ipc_open(h, off) for h, off in handles]
             self.opened += [(p, off) for p, (_, off) in zip(ptrs, handles)]
-            runner.attach(which, side, ptrs, nz_nb)
+            runner.attach(which, side, ptrs[:2], nz_nb)
+            if flags:
+                runner.attach_flags(which, side, ptrs[2])
 
     def close(self):
         self.runner.detach(self.which)
@@ -318,7 +334,7 @@ def neighbour_tokens(slab: ZSlab, token, scratch, group=None):
 
 
 def run_slab_distributed(runner: "SlabRunner", n_total: int, direction: str = "forward", group=None, peer: bool = False,
-                         host_sync: bool = False):
+                         host_sync: bool = False, chunk: int = 64):
     """The same loop for one rank of a torch.distributed job (one slab per GPU, NCCL point-to-point).
     peer = True (or a PeerLinks built for this direction, to be reused over several runs): the step kernels store the halo
     planes into the neighbours' volumes; per step only a token travels.  host_sync = True (tokens on CPU tensors, e.g. a gloo group): the stream is synchronised before the token
@@ -335,6 +351,16 @@ def run_slab_distributed(runner: "SlabRunner", n_total: int, direction: str = "f
             multi = runner.slab.world > 1
             if multi:
                 dist.barrier(group=group)              # every rank has attached before any kernel stores
+            if links.flags:
+                # device-side ordering: ranges of `chunk` steps per call, no token, nothing between the ranks but the
+                # kernels' own stores and flags (one GPU per rank: the slabs must run side by side)
+                for a in range(0, n_total, chunk):
+                    b = min(a + chunk, n_total)
+                    if direction == "forward":
+                        runner.forward_steps(a, b)
+                    else:
+                        runner.backward_steps(n_total - a, n_total - b)
+                steps = ()
             for n in steps:
                 if direction == "forward":
                     runner.forward_steps(n, n + 1)
@@ -344,6 +370,8 @@ def run_slab_distributed(runner: "SlabRunner", n_total: int, direction: str = "f
                     torch.cuda.current_stream().synchronize()
                 neighbour_tokens(runner.slab, token, scratch, group)
             torch.cuda.current_stream().synchronize()
+            if links.flags and runner.B.fdtd_halo_sync_error(runner.grid.h):
+                raise RuntimeError("a slab waited for a neighbour that never reached the state (fdtd_halo_sync_error)")
             if multi:
                 dist.barrier(group=group)              # nobody closes a mapping a neighbour's kernel may still write
         finally:

@@ -69,6 +69,8 @@ def _slabs(B, w, path, n, cuts, ref, peer=False):
         grad[r.slab.k_lo:r.slab.k_hi] = r.grad[own].cpu().numpy()
         lam0[:, r.slab.k_lo:r.slab.k_hi] = r.lam0[:, own].cpu().numpy()
     paths = {r.grid.info().path for r in runners}
+    if peer == "flags":                                   # no wait of the device-side ordering gave up
+        assert all(B.fdtd_halo_sync_error(r.grid.h) == 0 for r in runners)
     for r in runners:
         r.close()
     return dict(fields=fields, phasors=phasors, grad=grad, lam0=lam0, paths=paths)
@@ -126,6 +128,39 @@ def test_peer_stores_replace_the_halo_exchange_bitwise(B, cuts, n):
     err = float(np.max(np.abs(got["grad"].astype(np.float64) - ref["grad"])) / np.max(np.abs(ref["grad"])))
     print(f"peer stores, z slabs {cuts}, {n} steps: fields, phasors, lam0 bit-identical; gradient differs by {err:.1e} of its maximum")
     assert err <= 1e-6
+
+
+def test_device_side_ordering_of_the_slabs(B, monkeypatch):
+    """include/fdtd.h "Device-side ordering": the wait / signal kernels beside every step kernel (peer = "flags").  On one
+    device the slabs are issued step by step in slab order on one stream, so every wait finds its flag set by a signal
+    that precedes it in the stream; the run is bit-identical to the undivided grid, no wait times out, and a slab that
+    runs ahead of its neighbour gives up after the (here: 200 ms) limit and reports the state that never came."""
+    import torch
+    monkeypatch.setenv("FDTD_HALO_TIMEOUT_MS", "200")
+    path = B.FDTD_PATH_FUSED
+    n = 11
+    w = wl.c3_mini(n_steps=n, kappa_max=3.0, alpha_max=0.05)
+    ref = _single(B, w, path, n)
+    got = _slabs(B, w, path, n, [13, 30], ref, peer="flags")
+    assert np.array_equal(got["fields"], ref["fields"]) and np.array_equal(got["lam0"], ref["lam0"])
+    for P, Pr in zip(got["phasors"], ref["phasors"]):
+        assert np.array_equal(P, Pr)
+    # flags and the bounded wait, on two fresh slabs
+    slabs = sharding.z_slabs(w.nz, 2, w.pml_cells, [21])
+    r0, r1 = (sharding.SlabRunner(B, w, s, n, record=1, path=path) for s in slabs)
+    sharding.attach_neighbours_local([r0, r1], 0, flags=True)
+    for k in range(3):
+        r0.forward_steps(k, k + 1)
+        r1.forward_steps(k, k + 1)
+    torch.cuda.synchronize()
+    assert B.fdtd_halo_sync_error(r0.grid.h) == 0 and B.fdtd_halo_sync_error(r1.grid.h) == 0
+    r0.forward_steps(3, 4)                              # state 4 on slab 0 only ...
+    r0.forward_steps(4, 5)                              # ... its next step waits for slab 1's state 4, which never comes
+    torch.cuda.synchronize()
+    assert B.fdtd_halo_sync_error(r0.grid.h) == 5       # 1 + the state index waited for
+    assert B.fdtd_halo_sync_error(r0.grid.h) == 0       # read and cleared
+    for r in (r0, r1):
+        r.close()
 
 
 def test_c3_full_size_slabs_with_peer_stores_bitwise(B):
