@@ -456,6 +456,11 @@ def run_probe(args):
                             (14, 10, 2, 512), (28, 20, 2, 512)):
         nb = (N + ty - 1) // ty * runs
         one(f"tile {N}x{ty} runs={runs} unroll={u} ({nb} blocks x {th}, {nb / sms:.2f}/SM)", 1, ty, runs, u, threads=th)
+    # the hand-over from one time step to the next: ping-pong volumes, marching upwards every time (2) or alternating (3)
+    for ty, runs, u, th in ((7, 5, 2, 384), (7, 10, 2, 384)):
+        nb = (N + ty - 1) // ty * runs
+        one(f"tile {N}x{ty} runs={runs} unroll={u}, ping-pong volumes, every launch marches upwards ({nb} blocks)", 2, ty, runs, u, threads=th)
+        one(f"tile {N}x{ty} runs={runs} unroll={u}, ping-pong volumes, marching direction alternates ({nb} blocks)", 3, ty, runs, u, threads=th)
     print(json.dumps({"probe": "7 volumes read + 6 written, float4 per thread, no arithmetic (fdtd_probe_bandwidth)",
                       "grid": [N, N, N], "bytes_per_launch": 13 * 4 * N ** 3, "peak_hbm_gbs": peaks["hbm_gbs"],
                       "peak_source": peaks["source"], "rows": rows}))

@@ -480,7 +480,10 @@ FDTD_API int fdtd_debug_partition(int32_t nx, int32_t ny, int32_t nz, int32_t d,
 /* Bandwidth probe for the roofline discussion (bench.py --probe; not on the hot path): moves the step kernel's bytes -- 7 volumes
  * read, 6 written, float4 per thread -- without its arithmetic.  pattern 0: grid-stride streaming with `blocks` x `threads`, `runs` passes over the volumes per launch;
  * pattern 1: the step kernel's traversal, a block per (tile column of tile_y whole-x rows, run of nz / runs planes), `unroll`
- * (1, 2, 4) planes in flight per iteration.  in: DEVICE 7 * nx*ny*nz floats, out: DEVICE 6 * nx*ny*nz floats.  Synchronous: times
+ * (1, 2, 4) planes in flight per iteration; pattern 2: pattern 1 on ping-pong volumes, the way a time step hands its results to
+ * the next (launch r reads the six volumes launch r-1 wrote plus the seventh of `in`; plain copies); pattern 3: pattern 2 with
+ * the marching direction alternating from launch to launch.  in: DEVICE 7 * nx*ny*nz floats (patterns 2, 3 also WRITE its first
+ * six volumes, with the values they held), out: DEVICE 6 * nx*ny*nz floats.  Synchronous: times
  * `reps` launches with CUDA events after 3 warm-up launches; *gbs = 13 volumes * reps / time in GB/s. */
 FDTD_API int fdtd_probe_bandwidth(int32_t pattern, int32_t nx, int32_t ny, int32_t nz, int32_t tile_y, int32_t runs, int32_t unroll,
                          int32_t blocks, int32_t threads, int32_t reps, const float *in, float *out, double *gbs,

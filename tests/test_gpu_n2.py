@@ -464,7 +464,16 @@ def test_bandwidth_probe_touches_every_cell(B):
         gbs = B.fdtd_probe_bandwidth(pattern, nx, ny, nz, ty, runs, unroll, blocks, threads, 2, vin, vout, st)
         assert gbs > 0
         assert torch.allclose(vout, want, rtol=1e-6, atol=1e-7), (pattern, ty, runs, unroll)     # fused multiply-add vs two roundings; NaN = not written
-    for bad in (dict(nx=42), dict(threads=100), dict(pattern=2), dict(pattern=1, unroll=3), dict(pattern=1, runs=nz + 1), dict(pattern=0, blocks=0)):
+    # patterns 2 / 3: the same traversal on ping-pong volumes (the first six volumes of `in` and `out` swap roles with every
+    # launch, plain copies), upwards every time or with the direction alternating: every cell of both sets is written
+    keep = vin.clone()
+    for pattern, ty, runs, unroll, threads in ((2, 7, 5, 2, 96), (3, 7, 4, 1, 384), (3, 5, 19, 4, 64), (3, 30, 1, 2, 512)):
+        vout = torch.full((6, nz, ny, nx), float("nan"), device="cuda")
+        vin[:6] = keep[:6] + 0.0
+        gbs = B.fdtd_probe_bandwidth(pattern, nx, ny, nz, ty, runs, unroll, 0, threads, 2, vin, vout, st)
+        assert gbs > 0
+        assert torch.equal(vout, keep[:6]) and torch.equal(vin, keep), (pattern, ty, runs, unroll)
+    for bad in (dict(nx=42), dict(threads=100), dict(pattern=4), dict(pattern=1, unroll=3), dict(pattern=1, runs=nz + 1), dict(pattern=0, blocks=0)):
         a = dict(pattern=0, nx=nx, ny=ny, nz=nz, tile_y=7, runs=2, unroll=1, blocks=8, threads=128)
         a.update(bad)
         with pytest.raises(B.FdtdError) as e:
