@@ -649,6 +649,10 @@ def main():
             n1 = {"value": sharding.whole_job_rate(w.cells * T, reps2, ms2, world), "unit": UNIT, "ms_per_step": ms2 / reps2,
                   "max_abs_dL_drho": float(drho.double().abs().max()), "loss": loss_value()}
 
+        # the recorded forward pass of the same grid alone: splits `ms_per_step` into forward(record) and reverse sweep
+        reps_fr = max(1, min(args.steps, 3))
+        ms_fwd_rec = timed(lambda: forward_only(grid), reps_fr) / reps_fr
+
         ms_fwd = ms_adj = None
         reps_adj = max(1, min(args.steps, 3))
         if grid_f is not None:
@@ -745,6 +749,18 @@ def main():
                                 alg_bytes_per_launch=g_["alg_bytes_per_launch"], frac_of_8000=g_["achieved"] / 8000.0,
                                 method=f"{ing}: CUDA events around a pass of {T} back-to-back launches of this kernel "
                                        "in the replayed graph, time / launches")
+        # the reverse sweep as it runs in the job (grouped launches): ms_per_step minus the recorded forward pass; what it
+        # takes beyond the adjoint-sweep-only pass is the inverse step (+ face injection) inside the job, without the launch
+        # latency that "events around every launch" adds to it
+        rev_us = (ms_total / args.steps - ms_fwd_rec) / T * 1e3
+        rs = {"forward_with_recorder_us_per_time_step": ms_fwd_rec / T * 1e3, "reverse_sweep_us_per_time_step": rev_us}
+        if ms_adj and "fused_inverse_step" in kernels:
+            inv_us = rev_us - ms_adj / reps_adj / T * 1e3
+            ib = kernels["fused_inverse_step"]["alg_bytes_per_launch"]
+            rs["inverse_step_in_job"] = {"avg_launch_us": inv_us, "alg_bytes_per_launch": ib, "achieved": ib / inv_us / 1e3,
+                                         "frac": ib / inv_us / 1e3 / peak,
+                                         "how": "reverse sweep per time step minus the adjoint-sweep-only pass per time step"}
+        roofline["in_job"] = rs
         # whole-job fractions: algorithmic B/cell/step x rate against the measured peak and the 8000 GB/s bar
         bpc = whole_job_bytes_per_cell_step(w, grad_cells, rbox=rbox_main)
         wj = {f"fwd_bwd_record{main_record}": {"bytes_per_cell_step": bpc["fwd_bwd"], "achieved": bpc["fwd_bwd"] * value / world / 1e3}}
