@@ -390,6 +390,8 @@ FDTD_API int fdtd_halo_import(fdtd_grid *grid, float *fields, int32_t which, int
  *   (fields) / the grid (the rest); they stay valid until fdtd_destroy.  ESTATE on a grid that runs the generic kernels.
  * fdtd_halo_attach: side 0 = the neighbour below, 1 = above; peer_vol0 / peer_vol1 = that neighbour's
  *   fdtd_halo_volumes of the same `which`, peer_nz its local plane count (ghosts included).  Both NULL detaches.  The
+ *   pointers are kept as given: the neighbour's volumes (and an IPC mapping of them) must stay valid until this grid is
+ *   detached or destroyed, and nothing checks that they are what they claim to be.  The
  *   grid must have a cut on that side and run the fused kernels (ESTATE otherwise); the neighbour must attach this
  *   grid in turn (a ghost plane on an attached side is written by the neighbour only).  While a neighbour is attached
  *   without flags (below) a range call must advance exactly one step (EINVAL otherwise) and the caller orders the steps
